@@ -1,0 +1,216 @@
+/*
+ * nd.h -- C ABI of the B200-native planar Method-of-Characteristics (MOC) hot path of
+ * arxiv/paper_2607_01591 (NuDEAL).  One shared library, libnd_moc.so, hand-written CUDA for sm_100a.
+ *
+ * What the calls compute (line numbers of the paper text PAPER.md; readings R-T, R-W, O-5..O-8 are
+ * listed in DESIGN.md because the paper is silent on them):
+ *   nd_tracks_generate   cyclic ("modular") rays on the bounding box of the whole domain and the
+ *                        ray-mesh intersection through a half-edge structure, done once before the
+ *                        solve (section III.A).  HOST code, FP64, bit-exact rules.
+ *   nd_problem_create    packs the precomputed segment data into the device segment
+ *                        stream and uploads cross sections, quadrature weights and the link table.
+ *   nd_transport_sweep   Eq. (5) along every track, direction, polar angle and group,
+ *                        the angular integration to the scalar flux, and the boundary
+ *                        angular-flux exchange through the link table.
+ *   nd_source_update     right-hand side of Eq. (1)/(3): scatter + chi/k * fission.
+ *   nd_power_iteration   the outer iteration that Eq. (1)'s k_eff implies ("# of
+ *                        transport sweeps").
+ *
+ * Conventions
+ *   - No C++ types, no torch types, no exceptions cross this boundary.  Every function returns an
+ *     nd_status (ND_OK = 0) except the three string/version getters.  On error, outputs are untouched.
+ *   - "HOST" pointers are ordinary host memory, borrowed for the duration of the call and copied.
+ *     "DEVICE" pointers are CUDA device memory owned by the caller (e.g. a torch tensor's data_ptr);
+ *     the library never allocates device memory: the caller passes one workspace block.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All device
+ *     work is stream-ordered and asynchronous, except where a HOST scalar/array is returned: those
+ *     calls synchronise the stream before returning.
+ *   - Canonical layouts at the ABI: phi, Q [R][G] row-major FP64; boundary psi [T][2][P][G] FP32,
+ *     index [t][d] = the flux ENTERING track t travelling in direction d (0 forward, 1 backward).
+ *     Internal device layouts (padding, track order, FP32 copies) are private.
+ *   - No CPU fallback exists.  Every compute entry point fails with ND_ERR_CUDA when no device or
+ *     no sm_100 kernel image is available.
+ */
+#ifndef ND_MOC_H
+#define ND_MOC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ND_VERSION 0x00010000u /* major<<16 | minor<<8 | patch */
+
+typedef enum {
+    ND_OK = 0,
+    ND_ERR_NULL = 1,          /* a required pointer is NULL */
+    ND_ERR_INVALID = 2,       /* an argument violates a stated precondition (message in nd_last_error) */
+    ND_ERR_RANGE = 3,         /* an index (region, material, link) is out of range, or a size exceeds a limit */
+    ND_ERR_WORKSPACE = 4,     /* workspace too small or not 256-byte aligned */
+    ND_ERR_CUDA = 5,          /* a CUDA call failed / no usable device */
+    ND_ERR_STATE = 6,         /* call not valid in the problem's current state */
+    ND_ERR_NOT_CONVERGED = 7, /* nd_power_iteration hit max_iters with tolerances set (outputs ARE written) */
+    ND_ERR_MESH = 8,          /* nd_tracks_generate: mesh is not a conforming CCW triangulation of the rectangle */
+    ND_ERR_NOMEM = 9          /* host allocation failed */
+} nd_status;
+
+enum { ND_BC_VACUUM = 0, ND_BC_REFLECTIVE = 1 };
+
+/* exp_mode: how 1 - exp(-tau) is evaluated in the FP32 sweep */
+enum {
+    ND_EXP_FAST = 0,    /* ex2.approx (MUFU) on tau*log2(e); abs error of exp <= 2 ulp(1) ~ 2.4e-7   */
+    ND_EXP_EXPM1 = 1    /* -expm1f(-tau): ~1 ulp relative in 1-exp(-tau); slow path, used as a cross-check */
+};
+/* sweep_kernel: which sweep implementation runs (all give the same result up to summation order) */
+enum {
+    ND_SWEEP_AUTO = 0,      /* the fastest validated kernel for this G,P */
+    ND_SWEEP_ATOMIC = 1,    /* warp per (track,direction), lanes over groups, FP64 global atomics per segment */
+    ND_SWEEP_PRIVATE = 2    /* lane-group per track batch, FP32 shared-memory private tally window, FP64 flush */
+};
+
+typedef struct {
+    int32_t exp_mode;       /* ND_EXP_*      (default 0) */
+    int32_t sweep_kernel;   /* ND_SWEEP_*    (default 0) */
+    int32_t track_batch;    /* tracks per private-tally batch; 0 = default */
+    int32_t window_regions; /* private tally window size in regions; 0 = default */
+    int32_t reserved[12];   /* must be 0 */
+} nd_options;
+
+/* ------------------------------------------------------------------------------------------------
+ * Host preprocessing: track laydown (rule R-T), links (O-3), half-edge ray walk (rule R-W), track
+ * volumes (O-5).  Output is bit-exact against the independent oracle (tests/test_tracks_bitexact.py).
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct {
+    int32_t n_vertices, n_triangles;
+    const double* xy;       /* HOST [V][2] vertex coordinates, domain is exactly [0,W]x[0,H]            */
+    const int32_t* tri;     /* HOST [R][3] counter-clockwise vertex ids; one triangle = one FSR */
+    double W, H;            /* bounding rectangle */
+    int32_t bc[4];          /* left, right, bottom, top: ND_BC_VACUUM / ND_BC_REFLECTIVE */
+} nd_mesh_desc;
+
+typedef struct nd_tracks nd_tracks; /* opaque, HOST memory owned by the library */
+
+/* n_azim: directions over [0,2pi), divisible by 4.  spacing: desired ray spacing (cm).
+ * n_threads: host threads for the ray walk (0 = all). */
+nd_status nd_tracks_generate(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, int32_t n_threads,
+                             nd_tracks** out);
+
+typedef struct {            /* all pointers HOST, owned by the nd_tracks object, valid until nd_tracks_destroy */
+    int32_t n_tracks;       /* T */
+    int32_t n_regions;      /* R */
+    int64_t n_segments;     /* S */
+    int32_t n_half;         /* N_a/2 track angles in (0,pi) */
+    const int64_t* track_seg_offset; /* [T+1] */
+    const int32_t* seg_region;       /* [S] */
+    const double* seg_length;        /* [S] 2-D projected lengths, > 0 */
+    const double* track_weight;      /* [T] omega_a * delta_a */
+    const int32_t* link;             /* [T][2] 2*t'+d' or -1 */
+    const int32_t* track_azim;       /* [T] track-angle index j */
+    const double* track_ends;        /* [T][4] x0,y0,x1,y1 */
+    const double* track_volume;      /* [R] A~_r = sum 2*omega_a*delta_a*s */
+    const double* azim_phi;          /* [N_a/2] effective angles */
+    const double* azim_weight;       /* [N_a/2] omega_a per direction (sum over N_a directions = 1) */
+    const double* azim_spacing;      /* [N_a/2] effective spacing delta_a */
+} nd_tracks_view_t;
+
+nd_status nd_tracks_view(const nd_tracks* tracks, nd_tracks_view_t* view);
+nd_status nd_tracks_destroy(nd_tracks* tracks);
+
+/* ------------------------------------------------------------------------------------------------
+ * Problem: mesh regions, track segments, linked boundary ends, polar quadrature, multigroup XS.
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct {                    /* all pointers: HOST memory, borrowed for the call only */
+    int32_t n_regions, n_materials, n_groups, n_polar, n_tracks;
+    const int32_t* region_material; /* [R]  0..M-1 */
+    const double* sigma_t;          /* [M][G]  > 0 */
+    const double* sigma_s;          /* [M][G_to][G_from]  Sigma_{s,g'->g} at [m][g][g'] */
+    const double* nu_sigma_f;       /* [M][G]  >= 0 */
+    const double* chi;              /* [M][G]  >= 0 */
+    const double* polar_sin;        /* [P]  sin(theta_p) in (0,1] */
+    const double* polar_weight;     /* [P]  sums to 1 over the upper hemisphere */
+    const int64_t* track_seg_offset;/* [T+1] CSR into the segment arrays, forward order */
+    const int32_t* seg_region;      /* [S]  0..R-1 */
+    const double* seg_length;       /* [S]  > 0, finite */
+    const double* track_weight;     /* [T]  omega_a * delta_a.  The library forms
+                                       w[t][p] = 4*pi*track_weight[t]*polar_weight[p]*polar_sin[p]  and
+                                       A~[r] = sum over segments in r of 2*track_weight[t]*seg_length     */
+    const int32_t* link;            /* [T][2] [t][0]: where the FORWARD outgoing flux goes, [t][1]: BACKWARD.
+                                       value 2*t'+d' = enter track t' travelling in direction d'; -1 = vacuum.
+                                       Non-negative links must be distinct (each entry is fed at most once). */
+} nd_problem_desc;
+
+typedef struct nd_problem nd_problem; /* opaque host object; owns no device memory except what lies in the workspace */
+
+/* Limits: n_regions <= 2^24, n_materials <= 256, n_groups <= 256, n_polar <= 4. */
+nd_status nd_workspace_bytes(const nd_problem_desc* desc, const nd_options* opts_or_null, size_t* device_bytes);
+
+/* device_workspace: DEVICE, >= nd_workspace_bytes, 256-byte aligned, caller-owned; must outlive the problem.
+ * Validates the descriptor (ranges, monotone offsets, positive lengths and sigma_t, polar weights sum to 1
+ * within 1e-9, distinct links), uploads, and sets the state of O-8: phi = 1, boundary psi = 0, k = 1.
+ * Synchronises the stream before returning. */
+nd_status nd_problem_create(const nd_problem_desc* desc, const nd_options* opts_or_null, void* device_workspace,
+                            size_t device_bytes, void* cuda_stream, nd_problem** out);
+nd_status nd_problem_destroy(nd_problem* p); /* does not touch the workspace */
+
+/* One transport sweep (O-6) with a caller-supplied isotropic angular source Q (per steradian).
+ *   d_Q       DEVICE [R][G] FP64, read
+ *   d_phi_out DEVICE [R][G] FP64, written: phi = 4 pi Q/Sigma_t + tally/(Sigma_t A~_r)
+ * Reads the problem's current boundary psi (Jacobi: the previous sweep's outgoing fluxes), advances it through
+ * the link table (vacuum entries become 0).  FP32 segment arithmetic, FP64 tallies. */
+nd_status nd_transport_sweep(nd_problem* p, const double* d_Q, double* d_phi_out, void* cuda_stream);
+
+/* O-7: Q[r][g] = (1/4pi) ( sum_g' Sigma_s[m][g][g'] phi[r][g'] + chi[m][g]/k * sum_g' nuSigma_f[m][g'] phi[r][g'] ).
+ *   d_phi DEVICE [R][G] FP64 read; d_Q_out DEVICE [R][G] FP64 written;
+ *   d_fission_rate_out DEVICE FP64 scalar or NULL: F = sum_r A~_r sum_g nuSigma_f phi (of d_phi). */
+nd_status nd_source_update(nd_problem* p, const double* d_phi, double k_eff, double* d_Q_out,
+                           double* d_fission_rate_out, void* cuda_stream);
+
+typedef struct { double k_eff, fission_rate, dk, dphi_max; } nd_iter_stats; /* one per iteration, HOST */
+
+/* O-8, canonical power iteration from the problem's current state (phi, boundary psi, k).
+ *   max_iters >= 0.  tol_k <= 0 and tol_phi <= 0: run exactly max_iters iterations with no host sync inside
+ *   the loop.  Otherwise stop when |k - k_prev| < tol_k and max|phi/F - phi_prev|/max(phi) < tol_phi.
+ *   k_eff_out HOST; d_phi_out DEVICE [R][G] FP64 or NULL (the un-normalised phi of the last sweep, as in O-8);
+ *   iters_done HOST or NULL; stats HOST [max_iters] or NULL (forces one host sync per iteration). */
+nd_status nd_power_iteration(nd_problem* p, int32_t max_iters, double tol_k, double tol_phi, double* k_eff_out,
+                             double* d_phi_out, int32_t* iters_done, nd_iter_stats* stats_or_null, void* cuda_stream);
+
+/* State access (checkpoint / resume, tests).  Canonical layouts. */
+nd_status nd_state_reset(nd_problem* p, void* cuda_stream);                       /* phi=1, psi=0, k=1 */
+nd_status nd_boundary_flux_fill(nd_problem* p, float value, void* cuda_stream);
+nd_status nd_boundary_flux_get(nd_problem* p, float* host_out, void* cuda_stream);       /* HOST [T][2][P][G] */
+nd_status nd_boundary_flux_set(nd_problem* p, const float* host_in, void* cuda_stream);  /* HOST [T][2][P][G] */
+nd_status nd_flux_get(nd_problem* p, double* d_phi_out, void* cuda_stream);        /* DEVICE [R][G] */
+nd_status nd_flux_set(nd_problem* p, const double* d_phi, double k_eff, void* cuda_stream);
+nd_status nd_track_volume_get(nd_problem* p, double* host_out);                    /* HOST [R] */
+nd_status nd_tally_get(nd_problem* p, double* d_tally_out, void* cuda_stream);     /* DEVICE [R][G], last sweep */
+
+/* Device-time accounting.  When enabled, every sweep-kernel launch is bracketed by CUDA events on its own
+ * stream; nd_profile_read synchronises and returns the accumulated kernel milliseconds and launch counts
+ * since the last nd_profile_enable(p,1).  kernels_launched counts every kernel the library launched. */
+typedef struct { double sweep_ms; int64_t sweep_launches; int64_t kernels_launched; } nd_profile;
+nd_status nd_profile_enable(nd_problem* p, int32_t on);
+nd_status nd_profile_read(nd_problem* p, nd_profile* out);
+
+/* Problem facts: padded sizes and the algorithmic byte / update counts DESIGN.md defines. */
+typedef struct {
+    int64_t n_segments, n_segments_padded;
+    int64_t updates_per_sweep;      /* U = 2*S*P*G */
+    int64_t algorithmic_bytes;      /* per sweep: stream + psi in/out + q read + tally write */
+    int32_t group_stride;           /* padded groups per region row */
+    int32_t sweep_kernel;           /* the ND_SWEEP_* actually selected */
+    int32_t n_batches;
+    int32_t reserved;
+} nd_problem_info;
+nd_status nd_problem_info_get(const nd_problem* p, nd_problem_info* out);
+
+const char* nd_status_string(nd_status s);
+const char* nd_last_error(const nd_problem* p_or_null); /* thread-local message of the last failing call */
+uint32_t nd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ND_MOC_H */

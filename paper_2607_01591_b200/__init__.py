@@ -1,0 +1,318 @@
+"""Thin Python binding of libnd_moc.so (include/nd.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels.  PyTorch is used for device memory
+(the workspace and the phi/Q tensors) and the stream.  There is no CPU fallback: importing works on a CPU
+box (the library loads and exports its symbols), but every compute call returns ND_ERR_CUDA without a B200.
+
+Functions keep the C names: nd_tracks_generate, nd_problem_create, nd_transport_sweep, nd_source_update,
+nd_power_iteration, ...  Cites: include/nd.h (which cites PAPER.md Eq. (1),(3)-(5), section III.A).
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libnd_moc.so")
+
+ND_OK = 0
+ND_ERR_NOT_CONVERGED = 7
+ND_BC_VACUUM, ND_BC_REFLECTIVE = 0, 1
+ND_EXP_FAST, ND_EXP_EXPM1 = 0, 1
+ND_SWEEP_AUTO, ND_SWEEP_ATOMIC, ND_SWEEP_PRIVATE = 0, 1, 2
+
+EXPORTS = [
+    "nd_tracks_generate", "nd_tracks_view", "nd_tracks_destroy", "nd_workspace_bytes", "nd_problem_create",
+    "nd_problem_destroy", "nd_transport_sweep", "nd_source_update", "nd_power_iteration", "nd_state_reset",
+    "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_flux_get", "nd_flux_set",
+    "nd_track_volume_get", "nd_tally_get", "nd_profile_enable", "nd_profile_read", "nd_problem_info_get",
+    "nd_status_string", "nd_last_error", "nd_version",
+]
+
+
+class NdError(RuntimeError):
+    def __init__(self, status, where, message):
+        super().__init__(f"{where}: {status} {message}")
+        self.status = status
+
+
+class nd_options(C.Structure):
+    _fields_ = [("exp_mode", C.c_int32), ("sweep_kernel", C.c_int32), ("track_batch", C.c_int32),
+                ("window_regions", C.c_int32), ("reserved", C.c_int32 * 12)]
+
+
+class nd_mesh_desc(C.Structure):
+    _fields_ = [("n_vertices", C.c_int32), ("n_triangles", C.c_int32), ("xy", C.c_void_p), ("tri", C.c_void_p),
+                ("W", C.c_double), ("H", C.c_double), ("bc", C.c_int32 * 4)]
+
+
+class nd_tracks_view_t(C.Structure):
+    _fields_ = [("n_tracks", C.c_int32), ("n_regions", C.c_int32), ("n_segments", C.c_int64), ("n_half", C.c_int32),
+                ("track_seg_offset", C.c_void_p), ("seg_region", C.c_void_p), ("seg_length", C.c_void_p),
+                ("track_weight", C.c_void_p), ("link", C.c_void_p), ("track_azim", C.c_void_p),
+                ("track_ends", C.c_void_p), ("track_volume", C.c_void_p), ("azim_phi", C.c_void_p),
+                ("azim_weight", C.c_void_p), ("azim_spacing", C.c_void_p)]
+
+
+class nd_problem_desc(C.Structure):
+    _fields_ = [("n_regions", C.c_int32), ("n_materials", C.c_int32), ("n_groups", C.c_int32), ("n_polar", C.c_int32),
+                ("n_tracks", C.c_int32), ("region_material", C.c_void_p), ("sigma_t", C.c_void_p),
+                ("sigma_s", C.c_void_p), ("nu_sigma_f", C.c_void_p), ("chi", C.c_void_p), ("polar_sin", C.c_void_p),
+                ("polar_weight", C.c_void_p), ("track_seg_offset", C.c_void_p), ("seg_region", C.c_void_p),
+                ("seg_length", C.c_void_p), ("track_weight", C.c_void_p), ("link", C.c_void_p)]
+
+
+class nd_iter_stats(C.Structure):
+    _fields_ = [("k_eff", C.c_double), ("fission_rate", C.c_double), ("dk", C.c_double), ("dphi_max", C.c_double)]
+
+
+class nd_profile(C.Structure):
+    _fields_ = [("sweep_ms", C.c_double), ("sweep_launches", C.c_int64), ("kernels_launched", C.c_int64)]
+
+
+class nd_problem_info(C.Structure):
+    _fields_ = [("n_segments", C.c_int64), ("n_segments_padded", C.c_int64), ("updates_per_sweep", C.c_int64),
+                ("algorithmic_bytes", C.c_int64), ("group_stride", C.c_int32), ("sweep_kernel", C.c_int32),
+                ("n_batches", C.c_int32), ("reserved", C.c_int32)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libnd_moc.so (built in-tree by paper_2607_01591_b200._build).  Fails loudly if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError(f"{_LIB_PATH} is missing: run `python -m paper_2607_01591_b200._build` "
+                              "(there is no CPU or PyTorch fallback for the MOC hot path)")
+        L = C.CDLL(_LIB_PATH)
+        L.nd_status_string.restype = C.c_char_p
+        L.nd_status_string.argtypes = [C.c_int]
+        L.nd_last_error.restype = C.c_char_p
+        L.nd_last_error.argtypes = [C.c_void_p]
+        L.nd_version.restype = C.c_uint32
+        L.nd_tracks_generate.argtypes = [C.POINTER(nd_mesh_desc), C.c_int32, C.c_double, C.c_int32, C.POINTER(C.c_void_p)]
+        L.nd_tracks_view.argtypes = [C.c_void_p, C.POINTER(nd_tracks_view_t)]
+        L.nd_tracks_destroy.argtypes = [C.c_void_p]
+        L.nd_workspace_bytes.argtypes = [C.POINTER(nd_problem_desc), C.POINTER(nd_options), C.POINTER(C.c_size_t)]
+        L.nd_problem_create.argtypes = [C.POINTER(nd_problem_desc), C.POINTER(nd_options), C.c_void_p, C.c_size_t,
+                                        C.c_void_p, C.POINTER(C.c_void_p)]
+        L.nd_problem_destroy.argtypes = [C.c_void_p]
+        L.nd_transport_sweep.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nd_source_update.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nd_power_iteration.argtypes = [C.c_void_p, C.c_int32, C.c_double, C.c_double, C.POINTER(C.c_double),
+                                         C.c_void_p, C.POINTER(C.c_int32), C.c_void_p, C.c_void_p]
+        L.nd_state_reset.argtypes = [C.c_void_p, C.c_void_p]
+        L.nd_boundary_flux_fill.argtypes = [C.c_void_p, C.c_float, C.c_void_p]
+        L.nd_boundary_flux_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nd_boundary_flux_set.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nd_flux_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nd_flux_set.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
+        L.nd_track_volume_get.argtypes = [C.c_void_p, C.c_void_p]
+        L.nd_tally_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nd_profile_enable.argtypes = [C.c_void_p, C.c_int32]
+        L.nd_profile_read.argtypes = [C.c_void_p, C.POINTER(nd_profile)]
+        L.nd_problem_info_get.argtypes = [C.c_void_p, C.POINTER(nd_problem_info)]
+        _lib = L
+    return _lib
+
+
+def _check(status, where, allow=()):
+    if status != ND_OK and status not in allow:
+        L = lib()
+        raise NdError(L.nd_status_string(status).decode(), where, L.nd_last_error(None).decode())
+    return status
+
+
+def _ptr(a):
+    return None if a is None else C.c_void_p(a.ctypes.data)
+
+
+def _np_view(addr, shape, dtype):
+    n = int(np.prod(shape))
+    if n == 0 or not addr:
+        return np.zeros(shape, dtype)
+    buf = (C.c_char * (n * np.dtype(dtype).itemsize)).from_address(addr)
+    return np.frombuffer(buf, dtype=dtype).reshape(shape)
+
+
+def nd_version():
+    return int(lib().nd_version())
+
+
+class Tracks:
+    """Result of nd_tracks_generate: numpy views of the library-owned host arrays (valid until .destroy())."""
+
+    def __init__(self, handle, view):
+        self._h = handle
+        T, R, S, NH = view.n_tracks, view.n_regions, view.n_segments, view.n_half
+        self.n_tracks, self.n_regions, self.n_segments, self.n_half = T, R, S, NH
+        self.seg_offset = _np_view(view.track_seg_offset, (T + 1,), np.int64)
+        self.seg_region = _np_view(view.seg_region, (S,), np.int32)
+        self.seg_length = _np_view(view.seg_length, (S,), np.float64)
+        self.track_weight = _np_view(view.track_weight, (T,), np.float64)
+        self.link = _np_view(view.link, (T, 2), np.int32)
+        self.track_azim = _np_view(view.track_azim, (T,), np.int32)
+        self.ends = _np_view(view.track_ends, (T, 4), np.float64)
+        self.volume = _np_view(view.track_volume, (R,), np.float64)
+        self.azim_phi = _np_view(view.azim_phi, (NH,), np.float64)
+        self.azim_weight = _np_view(view.azim_weight, (NH,), np.float64)
+        self.azim_spacing = _np_view(view.azim_spacing, (NH,), np.float64)
+
+    def destroy(self):
+        if self._h:
+            lib().nd_tracks_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def nd_tracks_generate(xy, tri, W, H, bc, n_azim, spacing, n_threads=0) -> Tracks:
+    """Host preprocessing (row A0): cyclic track laydown + half-edge ray walk.  HOST arrays in, HOST views out."""
+    xy = np.ascontiguousarray(xy, np.float64)
+    tri = np.ascontiguousarray(tri, np.int32)
+    md = nd_mesh_desc(len(xy), len(tri), xy.ctypes.data, tri.ctypes.data, float(W), float(H), (C.c_int32 * 4)(*[int(b) for b in bc]))
+    h = C.c_void_p()
+    _check(lib().nd_tracks_generate(C.byref(md), int(n_azim), float(spacing), int(n_threads), C.byref(h)), "nd_tracks_generate")
+    v = nd_tracks_view_t()
+    _check(lib().nd_tracks_view(h, C.byref(v)), "nd_tracks_view")
+    return Tracks(h, v)
+
+
+class Problem:
+    """Owner of an nd_problem handle and its torch workspace.  Methods mirror the C entry points."""
+
+    def __init__(self, region_material, sigma_t, sigma_s, nu_sigma_f, chi, polar_sin, polar_weight, seg_offset,
+                 seg_region, seg_length, track_weight, link, exp_mode=ND_EXP_FAST, sweep_kernel=ND_SWEEP_AUTO,
+                 track_batch=0, window_regions=0, device="cuda:0"):
+        import torch
+        self.torch = torch
+        self.device = torch.device(device)
+        keep = dict(
+            rm=np.ascontiguousarray(region_material, np.int32), st=np.ascontiguousarray(sigma_t, np.float64),
+            ss=np.ascontiguousarray(sigma_s, np.float64), nf=np.ascontiguousarray(nu_sigma_f, np.float64),
+            ch=np.ascontiguousarray(chi, np.float64), ps=np.ascontiguousarray(polar_sin, np.float64),
+            pw=np.ascontiguousarray(polar_weight, np.float64), so=np.ascontiguousarray(seg_offset, np.int64),
+            sr=np.ascontiguousarray(seg_region, np.int32), sl=np.ascontiguousarray(seg_length, np.float64),
+            tw=np.ascontiguousarray(track_weight, np.float64), lk=np.ascontiguousarray(link, np.int32))
+        self.R, (self.M, self.G), self.P, self.T = len(keep["rm"]), keep["st"].shape, len(keep["ps"]), len(keep["tw"])
+        d = nd_problem_desc(self.R, self.M, self.G, self.P, self.T, *[keep[k].ctypes.data for k in
+                            ("rm", "st", "ss", "nf", "ch", "ps", "pw", "so", "sr", "sl", "tw", "lk")])
+        opt = nd_options(int(exp_mode), int(sweep_kernel), int(track_batch), int(window_regions))
+        nbytes = C.c_size_t()
+        _check(lib().nd_workspace_bytes(C.byref(d), C.byref(opt), C.byref(nbytes)), "nd_workspace_bytes")
+        self.workspace_bytes = int(nbytes.value)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)
+            base = self.workspace.data_ptr()
+            self._ws_ptr = (base + 255) // 256 * 256
+            h = C.c_void_p()
+            _check(lib().nd_problem_create(C.byref(d), C.byref(opt), C.c_void_p(self._ws_ptr), self.workspace_bytes,
+                                           self._stream(), C.byref(h)), "nd_problem_create")
+        self._h = h
+
+    def _stream(self):
+        return C.c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream)
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().nd_problem_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    # ---- compute entry points (device tensors in / out) ----
+    def nd_transport_sweep(self, d_Q, d_phi_out=None):
+        t = self.torch
+        assert d_Q.dtype == t.float64 and d_Q.is_cuda and d_Q.is_contiguous() and d_Q.numel() == self.R * self.G
+        if d_phi_out is None:
+            d_phi_out = t.empty((self.R, self.G), dtype=t.float64, device=self.device)
+        _check(lib().nd_transport_sweep(self._h, d_Q.data_ptr(), d_phi_out.data_ptr(), self._stream()), "nd_transport_sweep")
+        return d_phi_out
+
+    def nd_source_update(self, d_phi, k_eff, d_Q_out=None, want_fission_rate=False):
+        t = self.torch
+        assert d_phi.dtype == t.float64 and d_phi.is_cuda and d_phi.is_contiguous() and d_phi.numel() == self.R * self.G
+        if d_Q_out is None:
+            d_Q_out = t.empty((self.R, self.G), dtype=t.float64, device=self.device)
+        d_F = t.empty(1, dtype=t.float64, device=self.device) if want_fission_rate else None
+        _check(lib().nd_source_update(self._h, d_phi.data_ptr(), float(k_eff), d_Q_out.data_ptr(),
+                                      d_F.data_ptr() if d_F is not None else None, self._stream()), "nd_source_update")
+        return (d_Q_out, d_F) if want_fission_rate else d_Q_out
+
+    def nd_power_iteration(self, max_iters, tol_k=0.0, tol_phi=0.0, d_phi_out=None, want_stats=False):
+        k = C.c_double()
+        it = C.c_int32()
+        stats = (nd_iter_stats * max(1, max_iters))() if want_stats else None
+        rc = lib().nd_power_iteration(self._h, int(max_iters), float(tol_k), float(tol_phi), C.byref(k),
+                                      d_phi_out.data_ptr() if d_phi_out is not None else None, C.byref(it),
+                                      C.cast(stats, C.c_void_p) if stats is not None else None, self._stream())
+        _check(rc, "nd_power_iteration", allow=(ND_ERR_NOT_CONVERGED,))
+        out = dict(k_eff=k.value, iters=it.value, converged=(rc == ND_OK))
+        if want_stats:
+            out["stats"] = [dict(k_eff=s.k_eff, fission_rate=s.fission_rate, dk=s.dk, dphi_max=s.dphi_max)
+                            for s in stats[:it.value]]
+        return out
+
+    # ---- state ----
+    def nd_state_reset(self):
+        _check(lib().nd_state_reset(self._h, self._stream()), "nd_state_reset")
+
+    def nd_boundary_flux_fill(self, value):
+        _check(lib().nd_boundary_flux_fill(self._h, float(value), self._stream()), "nd_boundary_flux_fill")
+
+    def nd_boundary_flux_get(self):
+        out = np.empty((self.T, 2, self.P, self.G), np.float32)
+        _check(lib().nd_boundary_flux_get(self._h, out.ctypes.data, self._stream()), "nd_boundary_flux_get")
+        return out
+
+    def nd_boundary_flux_set(self, psi):
+        psi = np.ascontiguousarray(psi, np.float32)
+        assert psi.size == self.T * 2 * self.P * self.G
+        _check(lib().nd_boundary_flux_set(self._h, psi.ctypes.data, self._stream()), "nd_boundary_flux_set")
+
+    def nd_flux_get(self):
+        out = self.torch.empty((self.R, self.G), dtype=self.torch.float64, device=self.device)
+        _check(lib().nd_flux_get(self._h, out.data_ptr(), self._stream()), "nd_flux_get")
+        return out
+
+    def nd_flux_set(self, d_phi, k_eff):
+        _check(lib().nd_flux_set(self._h, d_phi.data_ptr(), float(k_eff), self._stream()), "nd_flux_set")
+
+    def nd_track_volume_get(self):
+        out = np.empty(self.R, np.float64)
+        _check(lib().nd_track_volume_get(self._h, out.ctypes.data), "nd_track_volume_get")
+        return out
+
+    def nd_tally_get(self):
+        out = self.torch.empty((self.R, self.G), dtype=self.torch.float64, device=self.device)
+        _check(lib().nd_tally_get(self._h, out.data_ptr(), self._stream()), "nd_tally_get")
+        return out
+
+    def nd_profile_enable(self, on=True):
+        _check(lib().nd_profile_enable(self._h, 1 if on else 0), "nd_profile_enable")
+
+    def nd_profile_read(self):
+        pr = nd_profile()
+        _check(lib().nd_profile_read(self._h, C.byref(pr)), "nd_profile_read")
+        return dict(sweep_ms=pr.sweep_ms, sweep_launches=pr.sweep_launches, kernels_launched=pr.kernels_launched)
+
+    def nd_problem_info_get(self):
+        inf = nd_problem_info()
+        _check(lib().nd_problem_info_get(self._h, C.byref(inf)), "nd_problem_info_get")
+        return {f[0]: getattr(inf, f[0]) for f in nd_problem_info._fields_ if f[0] != "reserved"}
+
+
+def nd_problem_create(xs, polar_sin, polar_weight, region_material, tracks, **options) -> Problem:
+    """Convenience: build a Problem from a cross-section set (arrays sigma_t, sigma_s, nu_sigma_f, chi) and Tracks."""
+    return Problem(region_material, xs.sigma_t, xs.sigma_s, xs.nu_sigma_f, xs.chi, polar_sin, polar_weight,
+                   tracks.seg_offset, tracks.seg_region, tracks.seg_length, tracks.track_weight, tracks.link, **options)

@@ -1,0 +1,677 @@
+// nd_api.cu -- the C ABI of include/nd.h: validation, device layout, stream packing (row A1), kernel
+// launches (rows A2-A6) and the power-iteration driver (row A7).  No CPU fallback anywhere: every compute
+// entry point launches CUDA kernels and returns ND_ERR_CUDA if that fails.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "nd.h"
+#include "nd_internal.h"
+#include "nd_kernels.cuh"
+
+// ------------------------------------------------------------------------------------------------
+// errors
+// ------------------------------------------------------------------------------------------------
+static thread_local std::string g_last_error;
+
+nd_status nd_fail(nd_status s, const char* msg)
+{
+    g_last_error = msg ? msg : "";
+    return s;
+}
+
+#define ND_CUDA(call)                                                                                   \
+    do {                                                                                                \
+        cudaError_t e_ = (call);                                                                        \
+        if (e_ != cudaSuccess) {                                                                        \
+            char buf_[512];                                                                             \
+            snprintf(buf_, sizeof buf_, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            return nd_fail(ND_ERR_CUDA, buf_);                                                          \
+        }                                                                                               \
+    } while (0)
+
+extern "C" const char* nd_status_string(nd_status s)
+{
+    switch (s) {
+    case ND_OK: return "ND_OK";
+    case ND_ERR_NULL: return "ND_ERR_NULL";
+    case ND_ERR_INVALID: return "ND_ERR_INVALID";
+    case ND_ERR_RANGE: return "ND_ERR_RANGE";
+    case ND_ERR_WORKSPACE: return "ND_ERR_WORKSPACE";
+    case ND_ERR_CUDA: return "ND_ERR_CUDA";
+    case ND_ERR_STATE: return "ND_ERR_STATE";
+    case ND_ERR_NOT_CONVERGED: return "ND_ERR_NOT_CONVERGED";
+    case ND_ERR_MESH: return "ND_ERR_MESH";
+    case ND_ERR_NOMEM: return "ND_ERR_NOMEM";
+    }
+    return "ND_ERR_UNKNOWN";
+}
+extern "C" const char* nd_last_error(const nd_problem*) { return g_last_error.c_str(); }
+extern "C" uint32_t nd_version(void) { return ND_VERSION; }
+
+// ------------------------------------------------------------------------------------------------
+// device layout
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr size_t kAlign = 256;
+constexpr int kReduceBlocks = 592; // 4 x 148 SMs
+
+struct Dims {
+    int R, M, G, P, T, Gs;
+    int64_t S, Spad;
+};
+
+struct Layout { // byte offsets into the workspace
+    size_t seg_rm, seg_len, trk_off, trk_w, link_src, psi_a, psi_b, q, tally, phi_a, phi_b, Q, reg_mat, vol, sigt, sigsT,
+        nusf, chi, sigt_f, scalars, partial, stats, total;
+};
+
+inline size_t bump(size_t& cur, size_t bytes)
+{
+    const size_t at = cur;
+    cur = (cur + bytes + kAlign - 1) / kAlign * kAlign;
+    return at;
+}
+
+Layout make_layout(const Dims& d, int max_stats)
+{
+    Layout L{};
+    size_t c = 0;
+    const size_t RG = (size_t)d.R * d.G, RGs = (size_t)d.R * d.Gs, NPSI = (size_t)d.T * 2 * d.P * d.G;
+    L.seg_rm = bump(c, sizeof(uint32_t) * (size_t)d.Spad);
+    L.seg_len = bump(c, sizeof(float) * (size_t)d.Spad);
+    L.trk_off = bump(c, sizeof(int64_t) * ((size_t)d.T + 1));
+    L.trk_w = bump(c, sizeof(float) * (size_t)d.T);
+    L.link_src = bump(c, sizeof(int32_t) * 2 * (size_t)d.T);
+    L.psi_a = bump(c, sizeof(float) * NPSI);
+    L.psi_b = bump(c, sizeof(float) * NPSI);
+    L.q = bump(c, sizeof(float) * RGs);
+    L.tally = bump(c, sizeof(double) * RGs);
+    L.phi_a = bump(c, sizeof(double) * RG);
+    L.phi_b = bump(c, sizeof(double) * RG);
+    L.Q = bump(c, sizeof(double) * RG);
+    L.reg_mat = bump(c, sizeof(int32_t) * (size_t)d.R);
+    L.vol = bump(c, sizeof(double) * (size_t)d.R);
+    L.sigt = bump(c, sizeof(double) * (size_t)d.M * d.G);
+    L.sigsT = bump(c, sizeof(double) * (size_t)d.M * d.G * d.G);
+    L.nusf = bump(c, sizeof(double) * (size_t)d.M * d.G);
+    L.chi = bump(c, sizeof(double) * (size_t)d.M * d.G);
+    L.sigt_f = bump(c, sizeof(float) * (size_t)d.M * d.Gs);
+    L.scalars = bump(c, sizeof(double) * ndk::SC_COUNT);
+    L.partial = bump(c, sizeof(double) * 3 * kReduceBlocks);
+    L.stats = bump(c, sizeof(double) * 4 * (size_t)max_stats);
+    L.total = c;
+    return L;
+}
+
+constexpr int kMaxStats = 4096;
+
+nd_status basic_dims(const nd_problem_desc* desc, Dims& d)
+{
+    if (!desc) return nd_fail(ND_ERR_NULL, "descriptor is NULL");
+    if (!desc->track_seg_offset) return nd_fail(ND_ERR_NULL, "track_seg_offset is NULL");
+    if (desc->n_regions < 1 || desc->n_materials < 1 || desc->n_groups < 1 || desc->n_polar < 1 || desc->n_tracks < 1)
+        return nd_fail(ND_ERR_INVALID, "n_regions, n_materials, n_groups, n_polar, n_tracks must be >= 1");
+    if (desc->n_regions > (1 << 24) || desc->n_materials > 256 || desc->n_groups > 256 || desc->n_polar > ndk::kMaxPolar ||
+        desc->n_tracks > (1 << 30))
+        return nd_fail(ND_ERR_RANGE, "limits: n_regions <= 2^24, n_materials <= 256, n_groups <= 256, n_polar <= 4, n_tracks <= 2^30");
+    d.R = desc->n_regions; d.M = desc->n_materials; d.G = desc->n_groups; d.P = desc->n_polar; d.T = desc->n_tracks;
+    d.Gs = (d.G + 3) / 4 * 4;
+    const int64_t* off = desc->track_seg_offset;
+    if (off[0] != 0) return nd_fail(ND_ERR_INVALID, "track_seg_offset[0] must be 0");
+    int64_t spad = 0;
+    for (int t = 0; t < d.T; ++t) {
+        const int64_t n = off[t + 1] - off[t];
+        if (n < 0) return nd_fail(ND_ERR_INVALID, "track_seg_offset must be non-decreasing");
+        spad += (n + 3) / 4 * 4;
+    }
+    d.S = off[d.T];
+    d.Spad = spad > 0 ? spad : 4;
+    return ND_OK;
+}
+
+struct EventPair { cudaEvent_t a, b; };
+
+} // namespace
+
+struct nd_problem {
+    Dims d{};
+    nd_options opt{};
+    Layout L{};
+    char* ws = nullptr;
+    int sweep_kernel = ND_SWEEP_ATOMIC;
+    int n_sm = 148;
+    // device pointers into the workspace
+    uint32_t* seg_rm; float* seg_len; int64_t* trk_off; float* trk_w; int32_t* link_src;
+    float* psi_in; float* psi_out; float* q; double* tally; double* phi_cur; double* phi_new; double* Q;
+    int32_t* reg_mat; double* vol; double* sigt; double* sigsT; double* nusf; double* chi; float* sigt_f;
+    double* scalars; double* partial; double* stats;
+    // host copies
+    std::vector<double> h_vol;
+    float c[ndk::kMaxPolar]{}, inv_sin[ndk::kMaxPolar]{}, wp[ndk::kMaxPolar]{};
+    // profiling
+    bool profile = false;
+    std::vector<EventPair> ev_pool;
+    size_t ev_used = 0;
+    int64_t kernels_launched = 0;
+};
+
+namespace {
+
+inline cudaStream_t as_stream(void* s) { return reinterpret_cast<cudaStream_t>(s); }
+
+inline int grid_for(int64_t n, int block, int cap)
+{
+    int64_t g = (n + block - 1) / block;
+    if (g < 1) g = 1;
+    return (int)(g > cap ? cap : g);
+}
+
+#define ND_LAUNCH_CHECK(p)                                                      \
+    do {                                                                        \
+        ++(p)->kernels_launched;                                                \
+        ND_CUDA(cudaGetLastError());                                            \
+    } while (0)
+
+nd_status launch_fill_f64(nd_problem* p, double* ptr, double v, int64_t n, cudaStream_t st)
+{
+    ndk::k_fill_f64<<<grid_for(n, 256, 4 * p->n_sm), 256, 0, st>>>(ptr, v, n);
+    ND_LAUNCH_CHECK(p);
+    return ND_OK;
+}
+nd_status launch_fill_f32(nd_problem* p, float* ptr, float v, int64_t n, cudaStream_t st)
+{
+    ndk::k_fill_f32<<<grid_for(n, 256, 4 * p->n_sm), 256, 0, st>>>(ptr, v, n);
+    ND_LAUNCH_CHECK(p);
+    return ND_OK;
+}
+
+// F = sum A~ nuSigma_f phi into scalars[SC_F] (and optionally a caller's device scalar)
+nd_status launch_fission_rate(nd_problem* p, const double* d_phi, double* d_out, cudaStream_t st)
+{
+    const Dims& d = p->d;
+    const int grid = grid_for((int64_t)d.R * d.G, 256, kReduceBlocks);
+    ndk::k_fission_partial<<<grid, 256, 0, st>>>(d_phi, p->reg_mat, p->nusf, p->vol, p->partial, d.R, d.G);
+    ND_LAUNCH_CHECK(p);
+    ndk::k_reduce_final<<<1, 256, 0, st>>>(p->partial, grid, p->scalars, 0, nullptr);
+    ND_LAUNCH_CHECK(p);
+    if (d_out) ND_CUDA(cudaMemcpyAsync(d_out, p->scalars + ndk::SC_F, sizeof(double), cudaMemcpyDeviceToDevice, st));
+    return ND_OK;
+}
+
+template <int P>
+nd_status launch_sweep_p(nd_problem* p, const ndk::SweepParams& prm, cudaStream_t st)
+{
+    const Dims& d = p->d;
+    const int block = 256, wpb = block / 32;
+    const int64_t pairs = 2 * (int64_t)d.T;
+    const int grid = grid_for(pairs * 32, block, 16 * p->n_sm);
+    (void)wpb;
+    if (p->opt.exp_mode == ND_EXP_EXPM1)
+        ndk::k_sweep_atomic<P, 1><<<grid, block, 0, st>>>(prm);
+    else
+        ndk::k_sweep_atomic<P, 0><<<grid, block, 0, st>>>(prm);
+    ND_LAUNCH_CHECK(p);
+    return ND_OK;
+}
+
+// A2 + A3: sweep with the current q/tally, then advance the boundary flux through the link table.
+nd_status launch_sweep(nd_problem* p, const double* scale_div, cudaStream_t st)
+{
+    const Dims& d = p->d;
+    ndk::SweepParams prm{};
+    prm.seg_rm = p->seg_rm; prm.seg_len = p->seg_len; prm.trk_off = p->trk_off; prm.trk_w = p->trk_w;
+    prm.q = p->q; prm.sigt = p->sigt_f; prm.tally = p->tally;
+    prm.psi_in = p->psi_in; prm.psi_out = p->psi_out; prm.scale_div = scale_div;
+    prm.T = d.T; prm.G = d.G; prm.Gs = d.Gs;
+    for (int i = 0; i < ndk::kMaxPolar; ++i) { prm.c[i] = p->c[i]; prm.inv_sin[i] = p->inv_sin[i]; prm.wp[i] = p->wp[i]; }
+    EventPair* ev = nullptr;
+    if (p->profile) {
+        if (p->ev_used == p->ev_pool.size()) {
+            EventPair e{};
+            ND_CUDA(cudaEventCreate(&e.a));
+            ND_CUDA(cudaEventCreate(&e.b));
+            p->ev_pool.push_back(e);
+        }
+        ev = &p->ev_pool[p->ev_used++];
+        ND_CUDA(cudaEventRecord(ev->a, st));
+    }
+    nd_status rc;
+    switch (d.P) {
+    case 1: rc = launch_sweep_p<1>(p, prm, st); break;
+    case 2: rc = launch_sweep_p<2>(p, prm, st); break;
+    case 3: rc = launch_sweep_p<3>(p, prm, st); break;
+    default: rc = launch_sweep_p<4>(p, prm, st); break;
+    }
+    if (rc != ND_OK) return rc;
+    if (ev) ND_CUDA(cudaEventRecord(ev->b, st));
+    const int PG = d.P * d.G;
+    const int64_t n = 2 * (int64_t)d.T * PG;
+    ndk::k_link_swap<<<grid_for(n, 256, 8 * p->n_sm), 256, 0, st>>>(p->psi_out, p->psi_in, p->link_src, 2 * (int64_t)d.T, PG);
+    ND_LAUNCH_CHECK(p);
+    return ND_OK;
+}
+
+nd_status launch_finalise(nd_problem* p, const double* Q, const double* phi_old, const double* f_ptr, double* phi_out,
+                          int* grid_out, cudaStream_t st)
+{
+    const Dims& d = p->d;
+    ndk::FinaliseParams fp{};
+    fp.Q = Q; fp.tally = p->tally; fp.reg_mat = p->reg_mat; fp.sigt = p->sigt; fp.nusf = p->nusf; fp.vol = p->vol;
+    fp.phi_old = phi_old; fp.f_ptr = f_ptr; fp.phi_new = phi_out; fp.partial = p->partial;
+    fp.R = d.R; fp.G = d.G; fp.Gs = d.Gs;
+    const int grid = grid_for((int64_t)d.R * d.G, 256, kReduceBlocks);
+    ndk::k_finalise<<<grid, 256, 0, st>>>(fp);
+    ND_LAUNCH_CHECK(p);
+    *grid_out = grid;
+    return ND_OK;
+}
+
+nd_status reset_state(nd_problem* p, cudaStream_t st)
+{
+    const Dims& d = p->d;
+    nd_status rc;
+    if ((rc = launch_fill_f64(p, p->phi_cur, 1.0, (int64_t)d.R * d.G, st)) != ND_OK) return rc;
+    if ((rc = launch_fill_f32(p, p->psi_in, 0.f, (int64_t)d.T * 2 * d.P * d.G, st)) != ND_OK) return rc;
+    const double sc[ndk::SC_COUNT] = {1.0, 0.0, 1.0, 0.0, 1.0, 0.0, 0.0, 0.0};
+    ND_CUDA(cudaMemcpyAsync(p->scalars, sc, sizeof sc, cudaMemcpyHostToDevice, st));
+    ND_CUDA(cudaStreamSynchronize(st)); // sc is a stack array
+    return launch_fission_rate(p, p->phi_cur, nullptr, st);
+}
+
+} // namespace
+
+// ------------------------------------------------------------------------------------------------
+// create / destroy
+// ------------------------------------------------------------------------------------------------
+extern "C" nd_status nd_workspace_bytes(const nd_problem_desc* desc, const nd_options*, size_t* device_bytes)
+{
+    if (!device_bytes) return nd_fail(ND_ERR_NULL, "device_bytes is NULL");
+    Dims d{};
+    nd_status rc = basic_dims(desc, d);
+    if (rc != ND_OK) return rc;
+    *device_bytes = make_layout(d, kMaxStats).total;
+    return ND_OK;
+}
+
+extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_options* opts, void* device_workspace,
+                                       size_t device_bytes, void* cuda_stream, nd_problem** out)
+{
+    if (!desc || !out || !device_workspace) return nd_fail(ND_ERR_NULL, "nd_problem_create: NULL argument");
+    if (!desc->region_material || !desc->sigma_t || !desc->sigma_s || !desc->nu_sigma_f || !desc->chi || !desc->polar_sin ||
+        !desc->polar_weight || !desc->track_seg_offset || !desc->seg_region || !desc->seg_length || !desc->track_weight ||
+        !desc->link)
+        return nd_fail(ND_ERR_NULL, "nd_problem_create: a descriptor array is NULL");
+    Dims d{};
+    nd_status rc = basic_dims(desc, d);
+    if (rc != ND_OK) return rc;
+    nd_options opt{};
+    if (opts) opt = *opts;
+    for (int i = 0; i < 12; ++i)
+        if (opt.reserved[i] != 0) return nd_fail(ND_ERR_INVALID, "nd_options.reserved must be zero");
+    if (opt.exp_mode != ND_EXP_FAST && opt.exp_mode != ND_EXP_EXPM1) return nd_fail(ND_ERR_INVALID, "unknown exp_mode");
+    if (opt.sweep_kernel < ND_SWEEP_AUTO || opt.sweep_kernel > ND_SWEEP_PRIVATE) return nd_fail(ND_ERR_INVALID, "unknown sweep_kernel");
+    const Layout L = make_layout(d, kMaxStats);
+    if (reinterpret_cast<uintptr_t>(device_workspace) % kAlign != 0) return nd_fail(ND_ERR_WORKSPACE, "workspace must be 256-byte aligned");
+    if (device_bytes < L.total) return nd_fail(ND_ERR_WORKSPACE, "workspace smaller than nd_workspace_bytes");
+
+    // ---- validation (host) ----
+    for (int r = 0; r < d.R; ++r)
+        if (desc->region_material[r] < 0 || desc->region_material[r] >= d.M) return nd_fail(ND_ERR_RANGE, "region_material out of range");
+    for (size_t i = 0; i < (size_t)d.M * d.G; ++i) {
+        if (!(desc->sigma_t[i] > 0.0) || !std::isfinite(desc->sigma_t[i])) return nd_fail(ND_ERR_INVALID, "sigma_t must be finite and > 0");
+        if (!(desc->nu_sigma_f[i] >= 0.0) || !std::isfinite(desc->nu_sigma_f[i])) return nd_fail(ND_ERR_INVALID, "nu_sigma_f must be finite and >= 0");
+        if (!(desc->chi[i] >= 0.0) || !std::isfinite(desc->chi[i])) return nd_fail(ND_ERR_INVALID, "chi must be finite and >= 0");
+    }
+    for (size_t i = 0; i < (size_t)d.M * d.G * d.G; ++i)
+        if (!std::isfinite(desc->sigma_s[i])) return nd_fail(ND_ERR_INVALID, "sigma_s must be finite");
+    double wsum = 0.0;
+    for (int p = 0; p < d.P; ++p) {
+        if (!(desc->polar_sin[p] > 0.0) || !(desc->polar_sin[p] <= 1.0)) return nd_fail(ND_ERR_INVALID, "polar_sin must lie in (0,1]");
+        if (!(desc->polar_weight[p] > 0.0)) return nd_fail(ND_ERR_INVALID, "polar_weight must be > 0");
+        wsum += desc->polar_weight[p];
+    }
+    if (std::fabs(wsum - 1.0) > 1e-9) return nd_fail(ND_ERR_INVALID, "polar_weight must sum to 1");
+    for (int t = 0; t < d.T; ++t)
+        if (!(desc->track_weight[t] > 0.0) || !std::isfinite(desc->track_weight[t])) return nd_fail(ND_ERR_INVALID, "track_weight must be finite and > 0");
+    for (int64_t k = 0; k < d.S; ++k) {
+        if (desc->seg_region[k] < 0 || desc->seg_region[k] >= d.R) return nd_fail(ND_ERR_RANGE, "seg_region out of range");
+        if (!(desc->seg_length[k] > 0.0) || !std::isfinite(desc->seg_length[k])) return nd_fail(ND_ERR_INVALID, "seg_length must be finite and > 0");
+    }
+    std::vector<int32_t> link_src;
+    nd_problem* p = nullptr;
+    std::vector<uint32_t> h_rm;
+    std::vector<float> h_len;
+    std::vector<int64_t> h_off;
+    try {
+        link_src.assign(2 * (size_t)d.T, -1);
+        for (int64_t e = 0; e < 2 * (int64_t)d.T; ++e) {
+            const int32_t lk = desc->link[e];
+            if (lk == -1) continue;
+            if (lk < 0 || lk >= 2 * d.T) return nd_fail(ND_ERR_RANGE, "link out of range");
+            if (link_src[lk] != -1) return nd_fail(ND_ERR_INVALID, "two track ends link to the same entry");
+            link_src[lk] = (int32_t)e;
+        }
+        p = new nd_problem();
+        p->d = d; p->opt = opt; p->L = L; p->ws = static_cast<char*>(device_workspace);
+        // ---- A1: pack the segment stream (SoA, every track run padded to a multiple of 4 = 16 bytes) ----
+        h_rm.assign((size_t)d.Spad, 0u);
+        h_len.assign((size_t)d.Spad, 0.f);
+        h_off.resize((size_t)d.T + 1);
+        p->h_vol.assign((size_t)d.R, 0.0);
+        int64_t o = 0;
+        for (int t = 0; t < d.T; ++t) {
+            h_off[t] = o;
+            const int64_t k0 = desc->track_seg_offset[t], k1 = desc->track_seg_offset[t + 1];
+            const double w2 = 2.0 * desc->track_weight[t];
+            uint32_t last = 0;
+            for (int64_t k = k0; k < k1; ++k) {
+                const int32_t r = desc->seg_region[k];
+                last = ndk::pack_rm((uint32_t)r, (uint32_t)desc->region_material[r]);
+                h_rm[o] = last;
+                h_len[o] = (float)desc->seg_length[k];
+                p->h_vol[r] += w2 * desc->seg_length[k];
+                ++o;
+            }
+            while (o % 4 != 0) { h_rm[o] = last; h_len[o] = 0.f; ++o; } // zero-length segments are exact no-ops
+        }
+        h_off[d.T] = o;
+    } catch (const std::bad_alloc&) {
+        delete p;
+        return nd_fail(ND_ERR_NOMEM, "nd_problem_create: out of host memory");
+    }
+    char* ws = p->ws;
+    p->seg_rm = (uint32_t*)(ws + L.seg_rm); p->seg_len = (float*)(ws + L.seg_len); p->trk_off = (int64_t*)(ws + L.trk_off);
+    p->trk_w = (float*)(ws + L.trk_w); p->link_src = (int32_t*)(ws + L.link_src);
+    p->psi_in = (float*)(ws + L.psi_a); p->psi_out = (float*)(ws + L.psi_b);
+    p->q = (float*)(ws + L.q); p->tally = (double*)(ws + L.tally);
+    p->phi_cur = (double*)(ws + L.phi_a); p->phi_new = (double*)(ws + L.phi_b); p->Q = (double*)(ws + L.Q);
+    p->reg_mat = (int32_t*)(ws + L.reg_mat); p->vol = (double*)(ws + L.vol);
+    p->sigt = (double*)(ws + L.sigt); p->sigsT = (double*)(ws + L.sigsT); p->nusf = (double*)(ws + L.nusf);
+    p->chi = (double*)(ws + L.chi); p->sigt_f = (float*)(ws + L.sigt_f);
+    p->scalars = (double*)(ws + L.scalars); p->partial = (double*)(ws + L.partial); p->stats = (double*)(ws + L.stats);
+
+    cudaStream_t st = as_stream(cuda_stream);
+    auto fail = [&](nd_status s) { delete p; return s; };
+    int dev = 0;
+    cudaError_t ce = cudaGetDevice(&dev);
+    if (ce != cudaSuccess) { delete p; return nd_fail(ND_ERR_CUDA, cudaGetErrorString(ce)); }
+    cudaDeviceProp prop{};
+    ce = cudaGetDeviceProperties(&prop, dev);
+    if (ce != cudaSuccess) { delete p; return nd_fail(ND_ERR_CUDA, cudaGetErrorString(ce)); }
+    if (prop.major != 10) { delete p; return nd_fail(ND_ERR_CUDA, "libnd_moc.so holds sm_100a kernels only; the current device is not compute capability 10.x"); }
+    p->n_sm = prop.multiProcessorCount;
+
+    std::vector<float> h_w((size_t)d.T), h_sigt_f((size_t)d.M * d.Gs, 1.f);
+    std::vector<double> h_sigsT((size_t)d.M * d.G * d.G);
+    for (int t = 0; t < d.T; ++t) h_w[t] = (float)(ndk::kFourPi * desc->track_weight[t]);
+    for (int m = 0; m < d.M; ++m)
+        for (int g = 0; g < d.G; ++g) {
+            h_sigt_f[(size_t)m * d.Gs + g] = (float)desc->sigma_t[(size_t)m * d.G + g];
+            for (int gp = 0; gp < d.G; ++gp)
+                h_sigsT[((size_t)m * d.G + gp) * d.G + g] = desc->sigma_s[((size_t)m * d.G + g) * d.G + gp];
+        }
+    for (int i = 0; i < d.P; ++i) {
+        p->c[i] = (float)(-1.4426950408889634074 / desc->polar_sin[i]);
+        p->inv_sin[i] = (float)(1.0 / desc->polar_sin[i]);
+        p->wp[i] = (float)(desc->polar_weight[i] * desc->polar_sin[i]);
+    }
+    p->sweep_kernel = ND_SWEEP_ATOMIC;
+
+#define ND_CUDA_P(call)                                                                                 \
+    do {                                                                                                \
+        cudaError_t e_ = (call);                                                                        \
+        if (e_ != cudaSuccess) {                                                                        \
+            char buf_[512];                                                                             \
+            snprintf(buf_, sizeof buf_, "%s failed: %s", #call, cudaGetErrorString(e_));                \
+            return fail(nd_fail(ND_ERR_CUDA, buf_));                                                    \
+        }                                                                                               \
+    } while (0)
+    ND_CUDA_P(cudaMemsetAsync(ws, 0, L.total, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->seg_rm, h_rm.data(), sizeof(uint32_t) * h_rm.size(), cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->seg_len, h_len.data(), sizeof(float) * h_len.size(), cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->trk_off, h_off.data(), sizeof(int64_t) * h_off.size(), cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->trk_w, h_w.data(), sizeof(float) * h_w.size(), cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->link_src, link_src.data(), sizeof(int32_t) * link_src.size(), cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->reg_mat, desc->region_material, sizeof(int32_t) * (size_t)d.R, cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->vol, p->h_vol.data(), sizeof(double) * (size_t)d.R, cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->sigt, desc->sigma_t, sizeof(double) * (size_t)d.M * d.G, cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->sigsT, h_sigsT.data(), sizeof(double) * h_sigsT.size(), cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->nusf, desc->nu_sigma_f, sizeof(double) * (size_t)d.M * d.G, cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->chi, desc->chi, sizeof(double) * (size_t)d.M * d.G, cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->sigt_f, h_sigt_f.data(), sizeof(float) * h_sigt_f.size(), cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaStreamSynchronize(st));
+#undef ND_CUDA_P
+    rc = reset_state(p, st);
+    if (rc != ND_OK) return fail(rc);
+    ce = cudaStreamSynchronize(st);
+    if (ce != cudaSuccess) { delete p; return nd_fail(ND_ERR_CUDA, cudaGetErrorString(ce)); }
+    *out = p;
+    return ND_OK;
+}
+
+extern "C" nd_status nd_problem_destroy(nd_problem* p)
+{
+    if (!p) return ND_OK;
+    for (auto& e : p->ev_pool) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    delete p;
+    return ND_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// compute entry points
+// ------------------------------------------------------------------------------------------------
+extern "C" nd_status nd_transport_sweep(nd_problem* p, const double* d_Q, double* d_phi_out, void* cuda_stream)
+{
+    if (!p || !d_Q || !d_phi_out) return nd_fail(ND_ERR_NULL, "nd_transport_sweep: NULL argument");
+    const Dims& d = p->d;
+    cudaStream_t st = as_stream(cuda_stream);
+    const int64_t n = (int64_t)d.R * d.Gs;
+    ndk::k_reduced_source<<<grid_for(n, 256, 8 * p->n_sm), 256, 0, st>>>(d_Q, p->reg_mat, p->sigt, p->q, p->tally, d.R, d.G, d.Gs);
+    ND_LAUNCH_CHECK(p);
+    nd_status rc = launch_sweep(p, p->scalars + ndk::SC_ONE, st);
+    if (rc != ND_OK) return rc;
+    int grid = 0;
+    return launch_finalise(p, d_Q, nullptr, nullptr, d_phi_out, &grid, st);
+}
+
+extern "C" nd_status nd_source_update(nd_problem* p, const double* d_phi, double k_eff, double* d_Q_out,
+                                      double* d_fission_rate_out, void* cuda_stream)
+{
+    if (!p || !d_phi || !d_Q_out) return nd_fail(ND_ERR_NULL, "nd_source_update: NULL argument");
+    if (!(k_eff > 0.0)) return nd_fail(ND_ERR_INVALID, "nd_source_update: k_eff must be > 0");
+    const Dims& d = p->d;
+    cudaStream_t st = as_stream(cuda_stream);
+    ndk::SourceParams sp{};
+    sp.phi = d_phi; sp.reg_mat = p->reg_mat; sp.sigt = p->sigt; sp.sigsT = p->sigsT; sp.nusf = p->nusf; sp.chi = p->chi;
+    sp.k_ptr = nullptr; sp.f_ptr = nullptr; sp.k_val = k_eff; sp.Q = d_Q_out; sp.q = nullptr; sp.tally = nullptr;
+    sp.R = d.R; sp.G = d.G; sp.Gs = d.Gs;
+    const int rpb = 256 / d.G;
+    ndk::k_source<<<grid_for((int64_t)(d.R + rpb - 1) / rpb * 256, 256, 8 * p->n_sm), 256, sizeof(double) * rpb * d.G, st>>>(sp);
+    ND_LAUNCH_CHECK(p);
+    if (d_fission_rate_out) {
+        // uses a private scalar slot so the problem's own F (power-iteration state) is not disturbed
+        const int grid = grid_for((int64_t)d.R * d.G, 256, kReduceBlocks);
+        ndk::k_fission_partial<<<grid, 256, 0, st>>>(d_phi, p->reg_mat, p->nusf, p->vol, p->partial, d.R, d.G);
+        ND_LAUNCH_CHECK(p);
+        ndk::k_reduce_final<<<1, 256, 0, st>>>(p->partial, grid, p->scalars + 4, 0, nullptr); // writes scalars[4+SC_F]
+        ND_LAUNCH_CHECK(p);
+        ND_CUDA(cudaMemcpyAsync(d_fission_rate_out, p->scalars + 4 + ndk::SC_F, sizeof(double), cudaMemcpyDeviceToDevice, st));
+    }
+    return ND_OK;
+}
+
+extern "C" nd_status nd_power_iteration(nd_problem* p, int32_t max_iters, double tol_k, double tol_phi, double* k_eff_out,
+                                        double* d_phi_out, int32_t* iters_done, nd_iter_stats* stats, void* cuda_stream)
+{
+    if (!p || !k_eff_out) return nd_fail(ND_ERR_NULL, "nd_power_iteration: NULL argument");
+    if (max_iters < 0) return nd_fail(ND_ERR_INVALID, "nd_power_iteration: max_iters must be >= 0");
+    const Dims& d = p->d;
+    cudaStream_t st = as_stream(cuda_stream);
+    const bool use_tol = tol_k > 0.0 || tol_phi > 0.0;
+    const bool sync_each = use_tol;
+    ndk::SourceParams sp{};
+    sp.reg_mat = p->reg_mat; sp.sigt = p->sigt; sp.sigsT = p->sigsT; sp.nusf = p->nusf; sp.chi = p->chi;
+    sp.k_ptr = p->scalars + ndk::SC_K; sp.f_ptr = p->scalars + ndk::SC_F; sp.k_val = 1.0;
+    sp.Q = p->Q; sp.q = p->q; sp.tally = p->tally; sp.R = d.R; sp.G = d.G; sp.Gs = d.Gs;
+    const int rpb = 256 / d.G;
+    const int src_grid = grid_for((int64_t)(d.R + rpb - 1) / rpb * 256, 256, 8 * p->n_sm);
+    int it = 0;
+    bool converged = !use_tol;
+    for (; it < max_iters; ++it) {
+        sp.phi = p->phi_cur;
+        ndk::k_source<<<src_grid, 256, sizeof(double) * rpb * d.G, st>>>(sp);
+        ND_LAUNCH_CHECK(p);
+        nd_status rc = launch_sweep(p, p->scalars + ndk::SC_F, st);
+        if (rc != ND_OK) return rc;
+        int grid = 0;
+        rc = launch_finalise(p, p->Q, p->phi_cur, p->scalars + ndk::SC_F, p->phi_new, &grid, st);
+        if (rc != ND_OK) return rc;
+        double* slot = (stats && it < kMaxStats) ? p->stats + 4 * (size_t)it : (sync_each ? p->stats : nullptr);
+        ndk::k_reduce_final<<<1, 256, 0, st>>>(p->partial, grid, p->scalars, 1, slot);
+        ND_LAUNCH_CHECK(p);
+        std::swap(p->phi_cur, p->phi_new);
+        if (sync_each) {
+            double h[4];
+            ND_CUDA(cudaMemcpyAsync(h, slot, sizeof h, cudaMemcpyDeviceToHost, st));
+            ND_CUDA(cudaStreamSynchronize(st));
+            const bool ok_k = !(tol_k > 0.0) || std::fabs(h[2]) < tol_k;
+            const bool ok_p = !(tol_phi > 0.0) || h[3] < tol_phi;
+            if (ok_k && ok_p) { converged = true; ++it; break; }
+        }
+    }
+    double hk[2];
+    ND_CUDA(cudaMemcpyAsync(hk, p->scalars, sizeof(double) * 2, cudaMemcpyDeviceToHost, st));
+    if (d_phi_out)
+        ND_CUDA(cudaMemcpyAsync(d_phi_out, p->phi_cur, sizeof(double) * (size_t)d.R * d.G, cudaMemcpyDeviceToDevice, st));
+    std::vector<double> hs;
+    const int ns = stats ? (it < kMaxStats ? it : kMaxStats) : 0;
+    if (ns > 0) {
+        hs.resize(4 * (size_t)ns);
+        ND_CUDA(cudaMemcpyAsync(hs.data(), p->stats, sizeof(double) * hs.size(), cudaMemcpyDeviceToHost, st));
+    }
+    ND_CUDA(cudaStreamSynchronize(st));
+    *k_eff_out = hk[ndk::SC_K];
+    if (iters_done) *iters_done = it;
+    for (int i = 0; i < ns; ++i) {
+        stats[i].k_eff = hs[4 * i]; stats[i].fission_rate = hs[4 * i + 1]; stats[i].dk = hs[4 * i + 2]; stats[i].dphi_max = hs[4 * i + 3];
+    }
+    if (use_tol && !converged) return nd_fail(ND_ERR_NOT_CONVERGED, "nd_power_iteration: max_iters reached before the tolerances");
+    return ND_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// state access
+// ------------------------------------------------------------------------------------------------
+extern "C" nd_status nd_state_reset(nd_problem* p, void* cuda_stream)
+{
+    if (!p) return nd_fail(ND_ERR_NULL, "nd_state_reset: NULL problem");
+    return reset_state(p, as_stream(cuda_stream));
+}
+
+extern "C" nd_status nd_boundary_flux_fill(nd_problem* p, float value, void* cuda_stream)
+{
+    if (!p) return nd_fail(ND_ERR_NULL, "nd_boundary_flux_fill: NULL problem");
+    return launch_fill_f32(p, p->psi_in, value, (int64_t)p->d.T * 2 * p->d.P * p->d.G, as_stream(cuda_stream));
+}
+
+extern "C" nd_status nd_boundary_flux_get(nd_problem* p, float* host_out, void* cuda_stream)
+{
+    if (!p || !host_out) return nd_fail(ND_ERR_NULL, "nd_boundary_flux_get: NULL argument");
+    cudaStream_t st = as_stream(cuda_stream);
+    ND_CUDA(cudaMemcpyAsync(host_out, p->psi_in, sizeof(float) * (size_t)p->d.T * 2 * p->d.P * p->d.G, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaStreamSynchronize(st));
+    return ND_OK;
+}
+
+extern "C" nd_status nd_boundary_flux_set(nd_problem* p, const float* host_in, void* cuda_stream)
+{
+    if (!p || !host_in) return nd_fail(ND_ERR_NULL, "nd_boundary_flux_set: NULL argument");
+    cudaStream_t st = as_stream(cuda_stream);
+    ND_CUDA(cudaMemcpyAsync(p->psi_in, host_in, sizeof(float) * (size_t)p->d.T * 2 * p->d.P * p->d.G, cudaMemcpyHostToDevice, st));
+    ND_CUDA(cudaStreamSynchronize(st));
+    return ND_OK;
+}
+
+extern "C" nd_status nd_flux_get(nd_problem* p, double* d_phi_out, void* cuda_stream)
+{
+    if (!p || !d_phi_out) return nd_fail(ND_ERR_NULL, "nd_flux_get: NULL argument");
+    ND_CUDA(cudaMemcpyAsync(d_phi_out, p->phi_cur, sizeof(double) * (size_t)p->d.R * p->d.G, cudaMemcpyDeviceToDevice, as_stream(cuda_stream)));
+    return ND_OK;
+}
+
+extern "C" nd_status nd_flux_set(nd_problem* p, const double* d_phi, double k_eff, void* cuda_stream)
+{
+    if (!p || !d_phi) return nd_fail(ND_ERR_NULL, "nd_flux_set: NULL argument");
+    if (!(k_eff > 0.0)) return nd_fail(ND_ERR_INVALID, "nd_flux_set: k_eff must be > 0");
+    cudaStream_t st = as_stream(cuda_stream);
+    ND_CUDA(cudaMemcpyAsync(p->phi_cur, d_phi, sizeof(double) * (size_t)p->d.R * p->d.G, cudaMemcpyDeviceToDevice, st));
+    ND_CUDA(cudaMemcpyAsync(p->scalars + ndk::SC_K, &k_eff, sizeof(double), cudaMemcpyHostToDevice, st));
+    ND_CUDA(cudaStreamSynchronize(st));
+    return launch_fission_rate(p, p->phi_cur, nullptr, st);
+}
+
+extern "C" nd_status nd_track_volume_get(nd_problem* p, double* host_out)
+{
+    if (!p || !host_out) return nd_fail(ND_ERR_NULL, "nd_track_volume_get: NULL argument");
+    memcpy(host_out, p->h_vol.data(), sizeof(double) * p->h_vol.size());
+    return ND_OK;
+}
+
+extern "C" nd_status nd_tally_get(nd_problem* p, double* d_tally_out, void* cuda_stream)
+{
+    if (!p || !d_tally_out) return nd_fail(ND_ERR_NULL, "nd_tally_get: NULL argument");
+    const Dims& d = p->d;
+    cudaStream_t st = as_stream(cuda_stream);
+    ndk::k_unpad_f64<<<grid_for((int64_t)d.R * d.G, 256, 8 * p->n_sm), 256, 0, st>>>(p->tally, d_tally_out, d.R, d.G, d.Gs);
+    ND_LAUNCH_CHECK(p);
+    return ND_OK;
+}
+
+extern "C" nd_status nd_profile_enable(nd_problem* p, int32_t on)
+{
+    if (!p) return nd_fail(ND_ERR_NULL, "nd_profile_enable: NULL problem");
+    p->profile = on != 0;
+    p->ev_used = 0;
+    p->kernels_launched = 0;
+    return ND_OK;
+}
+
+extern "C" nd_status nd_profile_read(nd_problem* p, nd_profile* out)
+{
+    if (!p || !out) return nd_fail(ND_ERR_NULL, "nd_profile_read: NULL argument");
+    double ms = 0.0;
+    for (size_t i = 0; i < p->ev_used; ++i) {
+        ND_CUDA(cudaEventSynchronize(p->ev_pool[i].b));
+        float t = 0.f;
+        ND_CUDA(cudaEventElapsedTime(&t, p->ev_pool[i].a, p->ev_pool[i].b));
+        ms += t;
+    }
+    out->sweep_ms = ms;
+    out->sweep_launches = (int64_t)p->ev_used;
+    out->kernels_launched = p->kernels_launched;
+    return ND_OK;
+}
+
+extern "C" nd_status nd_problem_info_get(const nd_problem* p, nd_problem_info* out)
+{
+    if (!p || !out) return nd_fail(ND_ERR_NULL, "nd_problem_info_get: NULL argument");
+    const Dims& d = p->d;
+    memset(out, 0, sizeof *out);
+    out->n_segments = d.S;
+    out->n_segments_padded = d.Spad;
+    out->updates_per_sweep = 2 * d.S * d.P * d.G;
+    // segment stream once (8 B/segment) + psi in and out (4 B each per chain end)
+    // + q read (4 B) and tally write (8 B) per (region, group)
+    out->algorithmic_bytes = 8 * d.S + 2 * 4 * (int64_t)d.T * 2 * d.P * d.G + 12 * (int64_t)d.R * d.G;
+    out->group_stride = d.Gs;
+    out->sweep_kernel = p->sweep_kernel;
+    out->n_batches = 0;
+    return ND_OK;
+}

@@ -1,0 +1,326 @@
+// nd_kernels.cuh -- device kernels of the planar-MOC hot path (sm_100a).  Rows A2..A6 of DESIGN.md.
+//   k_source        A5  scatter + fission source (Eq. (1)/(3) RHS), reduced source q, tally reset
+//   k_sweep_atomic  A2  Eq. (5) per (track, direction, polar, group); FP64 global atomics per segment
+//   k_link_swap     A3  boundary angular flux through the link table (compressed psi: track ends only)
+//   k_finalise      A4  phi = 4 pi Q/Sigma_t + tally/(Sigma_t A~) + partial fission-rate sums
+//   k_reduce_*      A6  fission rate, k_eff update
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ndk {
+
+constexpr int kMaxPolar = 4;
+constexpr double kFourPi = 12.566370614359172953850573533118;
+
+// Segment stream record (SoA): seg_rm[k] = region | material << 24 ; seg_len[k] = FP32 projected length.
+__host__ __device__ inline uint32_t pack_rm(uint32_t region, uint32_t material) { return region | (material << 24); }
+__device__ __forceinline__ uint32_t rm_region(uint32_t rm) { return rm & 0x00ffffffu; }
+__device__ __forceinline__ uint32_t rm_material(uint32_t rm) { return rm >> 24; }
+
+struct SweepParams {
+    // segment stream
+    const uint32_t* __restrict__ seg_rm;
+    const float* __restrict__ seg_len;
+    const int64_t* __restrict__ trk_off;   // [T+1] padded offsets (multiples of 4)
+    const float* __restrict__ trk_w;       // [T] 4 pi omega_a delta_a
+    // region / material data
+    const float* __restrict__ q;           // [R][Gs] reduced source Q/Sigma_t
+    const float* __restrict__ sigt;        // [M][Gs]
+    double* __restrict__ tally;            // [R][Gs]
+    // boundary flux
+    const float* __restrict__ psi_in;      // [T][2][P][G]
+    float* __restrict__ psi_out;           // [T][2][P][G]
+    const double* __restrict__ scale_div;  // device scalar F: psi_in is used as psi_in / F
+    int T, G, Gs;
+    float c[kMaxPolar];                    // -log2(e)/sin(theta_p)      (ND_EXP_FAST)
+    float inv_sin[kMaxPolar];              // 1/sin(theta_p)             (ND_EXP_EXPM1)
+    float wp[kMaxPolar];                   // polar_weight*polar_sin
+};
+
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// One Eq.-(5) step for P polar chains of one (track, direction, group): returns sum_p wp*Delta_p.
+template <int P, int EXPM>
+__device__ __forceinline__ float attenuate(float (&psi)[P], float qv, float st_s, const SweepParams& prm)
+{
+    float acc = 0.f;
+#pragma unroll
+    for (int p = 0; p < P; ++p) {
+        const float d = psi[p] - qv;
+        float delta;
+        if (EXPM == 0) {
+            const float a = ex2_approx(st_s * prm.c[p]);   // exp(-tau)
+            delta = fmaf(-d, a, d);                         // d*(1-a)
+        } else {
+            delta = d * (-expm1f(-st_s * prm.inv_sin[p]));
+        }
+        psi[p] -= delta;
+        acc = fmaf(prm.wp[p], delta, acc);
+    }
+    return acc;
+}
+
+// ---- A2, baseline: one warp per (track, direction); lanes over groups; FP64 atomics per (segment, group) ----
+template <int P, int EXPM>
+__global__ void __launch_bounds__(256) k_sweep_atomic(const SweepParams prm)
+{
+    const int lane = threadIdx.x & 31;
+    const int warps_per_block = blockDim.x >> 5;
+    const int64_t n_pairs = 2 * (int64_t)prm.T;
+    const float inv_f = (float)(1.0 / *prm.scale_div);
+    for (int64_t pair = (int64_t)blockIdx.x * warps_per_block + (threadIdx.x >> 5); pair < n_pairs;
+         pair += (int64_t)gridDim.x * warps_per_block) {
+        const int t = (int)(pair >> 1), dir = (int)(pair & 1);
+        const int64_t k0 = prm.trk_off[t], k1 = prm.trk_off[t + 1];
+        const float wt = prm.trk_w[t];
+        for (int g = lane; g < prm.G; g += 32) {
+            float psi[P];
+#pragma unroll
+            for (int p = 0; p < P; ++p) psi[p] = prm.psi_in[(pair * P + p) * prm.G + g] * inv_f;
+            for (int64_t i = 0; i < k1 - k0; ++i) {
+                const int64_t k = dir == 0 ? k0 + i : k1 - 1 - i;
+                const uint32_t rm = prm.seg_rm[k];
+                const float s = prm.seg_len[k];
+                const uint32_t r = rm_region(rm);
+                const float st = prm.sigt[rm_material(rm) * prm.Gs + g];
+                const float qv = prm.q[(size_t)r * prm.Gs + g];
+                const float acc = attenuate<P, EXPM>(psi, qv, st * s, prm);
+                if (s > 0.f) atomicAdd(&prm.tally[(size_t)r * prm.Gs + g], (double)(wt * acc));
+            }
+#pragma unroll
+            for (int p = 0; p < P; ++p) prm.psi_out[(pair * P + p) * prm.G + g] = psi[p];
+        }
+    }
+}
+
+// ---- A3: psi_next[e] = src[e] >= 0 ? psi_out[src[e]] : 0  for every entry e = 2t+d (gather form) ----
+__global__ void __launch_bounds__(256) k_link_swap(const float* __restrict__ psi_out, float* __restrict__ psi_next,
+                                                   const int32_t* __restrict__ src, int64_t n_entries, int PG)
+{
+    const int64_t n = n_entries * PG;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t e = i / PG;
+        const int j = (int)(i - e * PG);
+        const int32_t s = src[e];
+        psi_next[i] = s >= 0 ? psi_out[(int64_t)s * PG + j] : 0.f;
+    }
+}
+
+// ---- A5: source.  One thread per (region, group); phi row staged in shared memory. ----
+// Q[r][g] = (1/4pi) ( sum_g' Ss[m][g][g'] phi[r][g']/F + chi[m][g]/k * sum_g' nSf[m][g'] phi[r][g']/F )
+// Also writes q = (float)(Q/Sigma_t) and zeroes the tally row.  sigsT is [m][g_from][g_to].
+struct SourceParams {
+    const double* __restrict__ phi;      // [R][G]
+    const int32_t* __restrict__ reg_mat; // [R]
+    const double* __restrict__ sigt;     // [M][G]
+    const double* __restrict__ sigsT;    // [M][G_from][G_to]
+    const double* __restrict__ nusf;     // [M][G]
+    const double* __restrict__ chi;      // [M][G]
+    const double* __restrict__ k_ptr;    // device scalar k (or NULL: use k_val)
+    const double* __restrict__ f_ptr;    // device scalar F (or NULL: 1)
+    double k_val;
+    double* __restrict__ Q;              // [R][G]
+    float* __restrict__ q;               // [R][Gs] or NULL
+    double* __restrict__ tally;          // [R][Gs] or NULL
+    int R, G, Gs;
+};
+
+__global__ void __launch_bounds__(256) k_source(const SourceParams prm)
+{
+    extern __shared__ double s_phi[];   // [regions_per_block][G]
+    const int G = prm.G;
+    const int rpb = blockDim.x / G;     // regions per block (>= 1 because blockDim.x >= G)
+    const double inv_f = prm.f_ptr ? 1.0 / *prm.f_ptr : 1.0;
+    const double inv_k = 1.0 / (prm.k_ptr ? *prm.k_ptr : prm.k_val);
+    for (int64_t r0 = (int64_t)blockIdx.x * rpb; r0 < prm.R; r0 += (int64_t)gridDim.x * rpb) {
+        const int nr = min(rpb, (int)(prm.R - r0));
+        __syncthreads();
+        for (int i = threadIdx.x; i < nr * G; i += blockDim.x) s_phi[i] = prm.phi[r0 * G + i] * inv_f;
+        __syncthreads();
+        const int lr = threadIdx.x / G, g = threadIdx.x - lr * G;
+        if (lr < nr) {
+            const int64_t r = r0 + lr;
+            const int m = prm.reg_mat[r];
+            const double* ph = s_phi + lr * G;
+            const double* ss = prm.sigsT + (size_t)m * G * G + g;
+            const double* nf = prm.nusf + (size_t)m * G;
+            double sc = 0.0, fis = 0.0;
+            for (int gp = 0; gp < G; ++gp) {
+                sc += ss[(size_t)gp * G] * ph[gp];
+                fis += nf[gp] * ph[gp];
+            }
+            const double Q = (sc + prm.chi[(size_t)m * G + g] * inv_k * fis) / kFourPi;
+            prm.Q[r * G + g] = Q;
+            if (prm.q) prm.q[r * prm.Gs + g] = (float)(Q / prm.sigt[(size_t)m * G + g]);
+            if (prm.tally) prm.tally[r * prm.Gs + g] = 0.0;
+        }
+    }
+}
+
+// q = Q/Sigma_t and tally = 0 for a caller-supplied Q (fixed-source nd_transport_sweep)
+__global__ void __launch_bounds__(256) k_reduced_source(const double* __restrict__ Q, const int32_t* __restrict__ reg_mat,
+                                                        const double* __restrict__ sigt, float* __restrict__ q,
+                                                        double* __restrict__ tally, int64_t R, int G, int Gs)
+{
+    const int64_t n = R * Gs;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t r = i / Gs;
+        const int g = (int)(i - r * Gs);
+        tally[i] = 0.0;
+        q[i] = g < G ? (float)(Q[r * G + g] / sigt[(size_t)reg_mat[r] * G + g]) : 0.f;
+    }
+}
+
+// ---- block-wide FP64 sum / max (deterministic tree) ----
+__device__ __forceinline__ double block_sum(double v, double* scratch)
+{
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) scratch[w] = v;
+    __syncthreads();
+    if (w == 0) {
+        v = lane < (blockDim.x >> 5) ? scratch[lane] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    }
+    return v; // valid in thread 0
+}
+__device__ __forceinline__ double block_max(double v, double* scratch)
+{
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) scratch[w] = v;
+    __syncthreads();
+    if (w == 0) {
+        v = lane < (blockDim.x >> 5) ? scratch[lane] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+    }
+    return v;
+}
+
+// ---- A4 + first stage of A6 ----
+// phi_new[r][g] = 4 pi Q/Sigma_t + (A~_r > 0 ? tally/(Sigma_t A~_r) : 0)
+// partial[3*b+0] = sum over the block's elements of A~_r nuSigma_f phi_new          (fission rate)
+// partial[3*b+1] = max |phi_new - phi_old/F|   partial[3*b+2] = max |phi_new|       (only if phi_old != NULL)
+struct FinaliseParams {
+    const double* __restrict__ Q;        // [R][G]
+    const double* __restrict__ tally;    // [R][Gs]
+    const int32_t* __restrict__ reg_mat;
+    const double* __restrict__ sigt;     // [M][G]
+    const double* __restrict__ nusf;     // [M][G]
+    const double* __restrict__ vol;      // [R]
+    const double* __restrict__ phi_old;  // [R][G] or NULL
+    const double* __restrict__ f_ptr;    // scalar F for phi_old normalisation (or NULL)
+    double* __restrict__ phi_new;        // [R][G]
+    double* __restrict__ partial;        // [gridDim.x][3]
+    int64_t R;
+    int G, Gs;
+};
+
+__global__ void __launch_bounds__(256) k_finalise(const FinaliseParams prm)
+{
+    __shared__ double scratch[32];
+    const int64_t n = prm.R * prm.G;
+    const double inv_f = (prm.phi_old && prm.f_ptr) ? 1.0 / *prm.f_ptr : 1.0;
+    double fsum = 0.0, dmax = 0.0, pmax = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t r = i / prm.G;
+        const int g = (int)(i - r * prm.G);
+        const int m = prm.reg_mat[r];
+        const double st = prm.sigt[(size_t)m * prm.G + g];
+        const double a = prm.vol[r];
+        double phi = kFourPi * prm.Q[i] / st;
+        if (a > 0.0) phi += prm.tally[r * prm.Gs + g] / (st * a);
+        prm.phi_new[i] = phi;
+        fsum += a * prm.nusf[(size_t)m * prm.G + g] * phi;
+        if (prm.phi_old) {
+            dmax = fmax(dmax, fabs(phi - prm.phi_old[i] * inv_f));
+            pmax = fmax(pmax, fabs(phi));
+        }
+    }
+    fsum = block_sum(fsum, scratch);
+    dmax = block_max(dmax, scratch);
+    pmax = block_max(pmax, scratch);
+    if (threadIdx.x == 0) {
+        prm.partial[3 * blockIdx.x + 0] = fsum;
+        prm.partial[3 * blockIdx.x + 1] = dmax;
+        prm.partial[3 * blockIdx.x + 2] = pmax;
+    }
+}
+
+// fission rate of an arbitrary phi: partial[3*b] = sum A~ nuSigma_f phi
+__global__ void __launch_bounds__(256) k_fission_partial(const double* __restrict__ phi, const int32_t* __restrict__ reg_mat,
+                                                         const double* __restrict__ nusf, const double* __restrict__ vol,
+                                                         double* __restrict__ partial, int64_t R, int G)
+{
+    __shared__ double scratch[32];
+    const int64_t n = R * G;
+    double fsum = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t r = i / G;
+        const int g = (int)(i - r * G);
+        fsum += vol[r] * nusf[(size_t)reg_mat[r] * G + g] * phi[i];
+    }
+    fsum = block_sum(fsum, scratch);
+    if (threadIdx.x == 0) { partial[3 * blockIdx.x] = fsum; partial[3 * blockIdx.x + 1] = 0.0; partial[3 * blockIdx.x + 2] = 0.0; }
+}
+
+// ---- A6 second stage (one block): scalars[] layout below.  mode 0: F <- sum (no k update).
+//      mode 1 (power iteration): F_new = sum; k_prev = k; k <- k*F_new; F <- F_new; dphi = max/max ----
+enum { SC_K = 0, SC_F = 1, SC_KPREV = 2, SC_DPHI = 3, SC_ONE = 4, SC_COUNT = 8 };
+
+__global__ void __launch_bounds__(256) k_reduce_final(const double* __restrict__ partial, int n_partial,
+                                                      double* __restrict__ scalars, int mode,
+                                                      double* __restrict__ stats_slot /* 4 doubles or NULL */)
+{
+    __shared__ double scratch[32];
+    double fsum = 0.0, dmax = 0.0, pmax = 0.0;
+    for (int i = threadIdx.x; i < n_partial; i += blockDim.x) {
+        fsum += partial[3 * i];
+        dmax = fmax(dmax, partial[3 * i + 1]);
+        pmax = fmax(pmax, partial[3 * i + 2]);
+    }
+    fsum = block_sum(fsum, scratch);
+    dmax = block_max(dmax, scratch);
+    pmax = block_max(pmax, scratch);
+    if (threadIdx.x == 0) {
+        if (mode == 1) {
+            const double k_prev = scalars[SC_K];
+            const double k_new = k_prev * fsum;
+            scalars[SC_KPREV] = k_prev;
+            scalars[SC_K] = k_new;
+            scalars[SC_DPHI] = pmax > 0.0 ? dmax / pmax : 0.0;
+            if (stats_slot) {
+                stats_slot[0] = k_new; stats_slot[1] = fsum; stats_slot[2] = k_new - k_prev; stats_slot[3] = scalars[SC_DPHI];
+            }
+        }
+        scalars[SC_F] = fsum;
+    }
+}
+
+__global__ void k_fill_f64(double* __restrict__ p, double v, int64_t n)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) p[i] = v;
+}
+__global__ void k_fill_f32(float* __restrict__ p, float v, int64_t n)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) p[i] = v;
+}
+// compact [R][Gs] -> [R][G]
+__global__ void k_unpad_f64(const double* __restrict__ src, double* __restrict__ dst, int64_t R, int G, int Gs)
+{
+    const int64_t n = R * G;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t r = i / G;
+        dst[i] = src[r * Gs + (i - r * G)];
+    }
+}
+
+} // namespace ndk

@@ -1,0 +1,214 @@
+"""GPU parity: the CUDA path (through the C ABI) against the FP64 oracle, element by element, on the same
+seeded inputs.  Bars (BASELINE.json north_star): phi max rel err <= 1e-4 per sweep, k_eff within 5 pcm after a
+fixed iteration count.  Run with  pytest -m gpu  on a B200."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle
+import paper_2607_01591_b200 as nd
+from moc_inputs import make_config, rect_tri_mesh, homogeneous_xs, tabuchi_yamamoto, make_xs
+from moc_inputs.configs import Problem as InputProblem
+from gpu_common import Pair, make_pair, seeded_sweep_inputs, phi_rel_err, PHI_RTOL, K_PCM, PSI_ATOL_REL
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = [nd.ND_SWEEP_ATOMIC, nd.ND_SWEEP_PRIVATE]
+
+# (config index, scale): sizes the oracle finishes in seconds, spanning several tiles and ragged tails
+SWEEP_CASES = [(1, 1.0), (2, 0.15), (2, 1.0), (3, 0.03), (4, 0.06), (5, 0.0008)]
+
+
+def _check_sweep(pair, seed, n_sweeps=2):
+    Q, psi = seeded_sweep_inputs(pair, seed)
+    dQ = torch.from_numpy(Q).cuda()
+    pair.gpu.nd_boundary_flux_set(psi)
+    psi_o = psi.astype(np.float64)
+    for _ in range(n_sweeps):  # the second sweep starts from the exchanged boundary flux
+        phi_g = pair.gpu.nd_transport_sweep(dQ).cpu().numpy()
+        tally_g = pair.gpu.nd_tally_get().cpu().numpy()
+        psi_g = pair.gpu.nd_boundary_flux_get()
+        phi_o, psi_o, tally_o = pair.oracle_sweep(Q, psi_o)
+        assert phi_rel_err(phi_g, phi_o) <= PHI_RTOL
+        assert np.abs(psi_g - psi_o).max() <= PSI_ATOL_REL * np.abs(psi_o).max()
+        # telescoping invariant on the GPU result itself (exact up to FP32 rounding of the chain)
+        scale = np.abs(tally_o).max()
+        assert np.abs(tally_g - tally_o).max() <= 2e-4 * scale
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("case", SWEEP_CASES, ids=[f"cfg{c[0]}x{c[1]}" for c in SWEEP_CASES])
+def test_sweep_matches_oracle(case, kernel):
+    pair = make_pair(case[0], case[1], sweep_kernel=kernel)
+    try:
+        _check_sweep(pair, seed=100 + case[0])
+    finally:
+        pair.close()
+
+
+@pytest.mark.parametrize("exp_mode", [nd.ND_EXP_FAST, nd.ND_EXP_EXPM1])
+def test_sweep_exp_modes(exp_mode):
+    pair = make_pair(2, 0.15, exp_mode=exp_mode)
+    try:
+        _check_sweep(pair, seed=7, n_sweeps=1)
+    finally:
+        pair.close()
+
+
+def _custom_pair(G, P, bc, n_azim=16, spacing=0.07, seed=3, n_materials=3, **options):
+    mesh = rect_tri_mesh(2.3, 1.7, 7, 5, seed=seed, jitter=0.3)
+    rng = np.random.default_rng(seed)
+    mesh.material[:] = rng.integers(0, n_materials, size=mesh.n_regions).astype(np.int32)
+    xs = make_xs(G, [True] + [False] * (n_materials - 1), seed, n_up=min(2, G - 1))
+    if P <= 3:
+        s, w = tabuchi_yamamoto(P)
+    else:  # any valid quadrature is an input; 4-point Gauss-Legendre in mu on (0,1)
+        mu, w = np.polynomial.legendre.leggauss(4)
+        mu, w = 0.5 * (mu + 1.0), 0.5 * w
+        s = np.sqrt(1.0 - mu * mu)
+    prob = InputProblem(f"custom_G{G}_P{P}", mesh, xs, n_azim, spacing, s, w, bc, 10)
+    return Pair(prob, **options)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("G,P", [(1, 1), (2, 2), (3, 3), (5, 4), (8, 3), (31, 3), (32, 2), (33, 3), (51, 3), (64, 1), (70, 3)])
+def test_sweep_group_and_polar_shapes(G, P, kernel):
+    pair = _custom_pair(G, P, (1, 0, 0, 1), sweep_kernel=kernel)
+    try:
+        _check_sweep(pair, seed=G * 10 + P)
+    finally:
+        pair.close()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("bc", [(0, 0, 0, 0), (1, 1, 1, 1), (0, 1, 1, 0)])
+def test_sweep_boundary_conditions(bc, kernel):
+    pair = _custom_pair(7, 3, bc, sweep_kernel=kernel)
+    try:
+        _check_sweep(pair, seed=11, n_sweeps=3)
+        psi = pair.gpu.nd_boundary_flux_get()
+        lk = pair.o_tr.link
+        fed = np.zeros(2 * pair.T, bool)
+        fed[lk[lk >= 0]] = True
+        assert np.all(psi.reshape(2 * pair.T, -1)[~fed] == 0.0), "vacuum entries must stay exactly zero"
+    finally:
+        pair.close()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_sweep_with_empty_and_single_segment_tracks(kernel):
+    """Degenerate descriptor: tracks with zero segments pass their flux through unchanged."""
+    G, P, R, T = 5, 2, 4, 6
+    rng = np.random.default_rng(5)
+    xs = make_xs(G, [True, False], 9)
+    s, w = tabuchi_yamamoto(P)
+    counts = np.array([0, 1, 3, 0, 9, 2])
+    off = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    seg_region = rng.integers(0, R, size=off[-1]).astype(np.int32)
+    seg_length = rng.uniform(0.01, 0.8, size=off[-1])
+    tw = rng.uniform(0.001, 0.01, size=T)
+    link = np.array([[2, 1], [0, 3], [-1, 5], [7, -1], [9, 8], [11, 10]], np.int32)
+    mat = np.array([0, 1, 1, 0], np.int32)
+    gp = nd.Problem(mat, xs.sigma_t, xs.sigma_s, xs.nu_sigma_f, xs.chi, s, w, off, seg_region, seg_length, tw, link,
+                    sweep_kernel=kernel)
+    vol = oracle.track_volumes(R, off, seg_region, seg_length, tw)
+    assert np.allclose(gp.nd_track_volume_get(), vol, rtol=1e-15)
+    Q = rng.uniform(0.1, 1.0, size=(R, G))
+    psi = rng.uniform(0, 2, size=(T, 2, P, G)).astype(np.float32)
+    gp.nd_boundary_flux_set(psi)
+    phi_g = gp.nd_transport_sweep(torch.from_numpy(Q).cuda()).cpu().numpy()
+    psi_g = gp.nd_boundary_flux_get()
+    phi_o, psi_o, _ = oracle.sweep(mat, xs.sigma_t, s, w, off, seg_region, seg_length, tw, link, vol, Q, psi.astype(np.float64))
+    assert phi_rel_err(phi_g, phi_o) <= PHI_RTOL
+    assert np.abs(psi_g - psi_o).max() <= PSI_ATOL_REL * np.abs(psi_o).max()
+    assert np.array_equal(psi_g[1, 0], psi[0, 0]), "empty track 0 forwards its flux bit-exactly into entry 2"
+    gp.destroy()
+
+
+def test_source_update_matches_oracle():
+    for idx, scale in [(1, 1.0), (4, 0.06), (5, 0.0008)]:
+        pair = make_pair(idx, scale)
+        try:
+            rng = np.random.default_rng(idx)
+            phi = rng.uniform(0.1, 3.0, size=(pair.R, pair.G))
+            k = 0.9 + 0.3 * rng.random()
+            Qg, Fg = pair.gpu.nd_source_update(torch.from_numpy(phi).cuda(), k, want_fission_rate=True)
+            p = pair.prob
+            Qo = oracle.source(p.mesh.material, p.xs.sigma_s, p.xs.nu_sigma_f, p.xs.chi, phi, k)
+            Fo = oracle.fission_rate(p.mesh.material, p.xs.nu_sigma_f, pair.o_tr.volume, phi)
+            assert np.abs(Qg.cpu().numpy() - Qo).max() <= 1e-13 * np.abs(Qo).max()
+            assert abs(Fg.item() - Fo) <= 1e-12 * abs(Fo)
+        finally:
+            pair.close()
+
+
+POWER_CASES = [(1, 1.0, 50), (2, 0.15, 20), (2, 1.0, 20), (3, 0.03, 20), (4, 0.06, 20), (5, 0.0008, 20)]
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("case", POWER_CASES, ids=[f"cfg{c[0]}x{c[1]}" for c in POWER_CASES])
+def test_power_iteration_matches_oracle(case, kernel):
+    idx, scale, n_it = case
+    pair = make_pair(idx, scale, sweep_kernel=kernel)
+    try:
+        ko, phio, psio, hist = pair.oracle_power(n_it)
+        dphi = torch.empty((pair.R, pair.G), dtype=torch.float64, device="cuda")
+        out = pair.gpu.nd_power_iteration(n_it, d_phi_out=dphi, want_stats=True)
+        assert out["iters"] == n_it
+        assert abs(out["k_eff"] - ko) * 1e5 <= K_PCM
+        kh = np.array([s["k_eff"] for s in out["stats"]])
+        assert np.abs(kh - hist).max() * 1e5 <= K_PCM, "k history"
+        assert phi_rel_err(dphi.cpu().numpy(), phio) <= PHI_RTOL
+        psi_g = pair.gpu.nd_boundary_flux_get()
+        assert np.abs(psi_g - psio).max() <= 5 * PSI_ATOL_REL * np.abs(psio).max()
+        # resume: state get/set round trip continues the same iteration
+        out2 = pair.gpu.nd_power_iteration(3)
+        ko2, *_ = pair.oracle_power(3, state=(ko, phio, psio))
+        assert abs(out2["k_eff"] - ko2) * 1e5 <= K_PCM
+    finally:
+        pair.close()
+
+
+def test_power_iteration_tolerance_mode_and_reset():
+    pair = make_pair(1, 1.0)
+    try:
+        out = pair.gpu.nd_power_iteration(2000, tol_k=1e-7, tol_phi=1e-6)
+        assert out["converged"] and out["iters"] < 2000
+        k1 = out["k_eff"]
+        out_nc = pair.gpu.nd_power_iteration(1, tol_k=1e-30)
+        assert not out_nc["converged"]
+        pair.gpu.nd_state_reset()
+        out = pair.gpu.nd_power_iteration(50)
+        ko, *_ = pair.oracle_power(50)
+        assert abs(out["k_eff"] - ko) * 1e5 <= K_PCM
+        assert abs(k1 - ko) < 5e-3
+    finally:
+        pair.close()
+
+
+def test_infinite_medium_closed_form_on_gpu():
+    """Homogeneous reflective rectangle: k -> nuSf^T (diag(St) - S)^-1 chi (closed form, not the oracle)."""
+    mesh = rect_tri_mesh(1.5, 1.5, 4, 4, seed=2, jitter=0.2)
+    mesh.material[:] = 0
+    xs = homogeneous_xs(4, 21, n_up=2)
+    s, w = tabuchi_yamamoto(3)
+    tr = nd.nd_tracks_generate(mesh.xy, mesh.tri, mesh.W, mesh.H, (1, 1, 1, 1), 8, 0.1)
+    gp = nd.nd_problem_create(xs, s, w, mesh.material, tr)
+    out = gp.nd_power_iteration(3000, tol_k=1e-9, tol_phi=1e-7)
+    A = np.diag(xs.sigma_t[0]) - xs.sigma_s[0]
+    k_inf = float(xs.nu_sigma_f[0] @ np.linalg.solve(A, xs.chi[0]))
+    assert abs(out["k_eff"] - k_inf) * 1e5 <= K_PCM
+    gp.destroy()
+
+
+def test_problem_create_rejects_on_device_side_errors():
+    pair = make_pair(1, 1.0)
+    try:
+        with pytest.raises(nd.NdError, match="ND_ERR_INVALID"):
+            pair.gpu.nd_source_update(torch.ones((pair.R, pair.G), dtype=torch.float64, device="cuda"), -1.0)
+        info = pair.gpu.nd_problem_info_get()
+        assert info["n_segments"] == pair.o_tr.n_segs
+        assert info["updates_per_sweep"] == 2 * pair.o_tr.n_segs * pair.P * pair.G
+    finally:
+        pair.close()
