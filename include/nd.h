@@ -139,6 +139,11 @@ typedef struct {                    /* all pointers: HOST memory, borrowed for t
     const int32_t* link;            /* [T][2] [t][0]: where the FORWARD outgoing flux goes, [t][1]: BACKWARD.
                                        value 2*t'+d' = enter track t' travelling in direction d'; -1 = vacuum.
                                        Non-negative links must be distinct (each entry is fed at most once). */
+    /* Optional track geometry (both NULL or both set; nd_tracks_view provides them).  Used ONLY to order the
+       device segment stream (adjacent parallel tracks are batched so that they share flat-source regions);
+       results do not depend on it.  Without it ND_SWEEP_AUTO selects the atomic sweep kernel. */
+    const int32_t* track_azim;      /* [T] id of the track's angle; tracks with equal id are parallel */
+    const double* track_ends;       /* [T][4] x0,y0,x1,y1 (forward direction runs from 0 to 1) */
 } nd_problem_desc;
 
 typedef struct nd_problem nd_problem; /* opaque host object; owns no device memory except what lies in the workspace */

@@ -59,7 +59,8 @@ class nd_problem_desc(C.Structure):
                 ("n_tracks", C.c_int32), ("region_material", C.c_void_p), ("sigma_t", C.c_void_p),
                 ("sigma_s", C.c_void_p), ("nu_sigma_f", C.c_void_p), ("chi", C.c_void_p), ("polar_sin", C.c_void_p),
                 ("polar_weight", C.c_void_p), ("track_seg_offset", C.c_void_p), ("seg_region", C.c_void_p),
-                ("seg_length", C.c_void_p), ("track_weight", C.c_void_p), ("link", C.c_void_p)]
+                ("seg_length", C.c_void_p), ("track_weight", C.c_void_p), ("link", C.c_void_p),
+                ("track_azim", C.c_void_p), ("track_ends", C.c_void_p)]
 
 
 class nd_iter_stats(C.Structure):
@@ -188,8 +189,8 @@ class Problem:
     """Owner of an nd_problem handle and its torch workspace.  Methods mirror the C entry points."""
 
     def __init__(self, region_material, sigma_t, sigma_s, nu_sigma_f, chi, polar_sin, polar_weight, seg_offset,
-                 seg_region, seg_length, track_weight, link, exp_mode=ND_EXP_FAST, sweep_kernel=ND_SWEEP_AUTO,
-                 track_batch=0, window_regions=0, device="cuda:0"):
+                 seg_region, seg_length, track_weight, link, track_azim=None, track_ends=None, exp_mode=ND_EXP_FAST,
+                 sweep_kernel=ND_SWEEP_AUTO, track_batch=0, window_regions=0, device="cuda:0"):
         import torch
         self.torch = torch
         self.device = torch.device(device)
@@ -200,9 +201,14 @@ class Problem:
             pw=np.ascontiguousarray(polar_weight, np.float64), so=np.ascontiguousarray(seg_offset, np.int64),
             sr=np.ascontiguousarray(seg_region, np.int32), sl=np.ascontiguousarray(seg_length, np.float64),
             tw=np.ascontiguousarray(track_weight, np.float64), lk=np.ascontiguousarray(link, np.int32))
+        geo = [None, None]
+        if track_azim is not None and track_ends is not None:
+            keep["ta"] = np.ascontiguousarray(track_azim, np.int32)
+            keep["te"] = np.ascontiguousarray(track_ends, np.float64)
+            geo = [keep["ta"].ctypes.data, keep["te"].ctypes.data]
         self.R, (self.M, self.G), self.P, self.T = len(keep["rm"]), keep["st"].shape, len(keep["ps"]), len(keep["tw"])
         d = nd_problem_desc(self.R, self.M, self.G, self.P, self.T, *[keep[k].ctypes.data for k in
-                            ("rm", "st", "ss", "nf", "ch", "ps", "pw", "so", "sr", "sl", "tw", "lk")])
+                            ("rm", "st", "ss", "nf", "ch", "ps", "pw", "so", "sr", "sl", "tw", "lk")], *geo)
         opt = nd_options(int(exp_mode), int(sweep_kernel), int(track_batch), int(window_regions))
         nbytes = C.c_size_t()
         _check(lib().nd_workspace_bytes(C.byref(d), C.byref(opt), C.byref(nbytes)), "nd_workspace_bytes")
@@ -315,4 +321,5 @@ class Problem:
 def nd_problem_create(xs, polar_sin, polar_weight, region_material, tracks, **options) -> Problem:
     """Convenience: build a Problem from a cross-section set (arrays sigma_t, sigma_s, nu_sigma_f, chi) and Tracks."""
     return Problem(region_material, xs.sigma_t, xs.sigma_s, xs.nu_sigma_f, xs.chi, polar_sin, polar_weight,
-                   tracks.seg_offset, tracks.seg_region, tracks.seg_length, tracks.track_weight, tracks.link, **options)
+                   tracks.seg_offset, tracks.seg_region, tracks.seg_length, tracks.track_weight, tracks.link,
+                   track_azim=tracks.track_azim, track_ends=tracks.ends, **options)

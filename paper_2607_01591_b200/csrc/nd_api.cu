@@ -13,6 +13,8 @@
 #include "nd.h"
 #include "nd_internal.h"
 #include "nd_kernels.cuh"
+#include "nd_sweep_private.cuh"
+#include "nd_tiles.h"
 
 // ------------------------------------------------------------------------------------------------
 // errors
@@ -67,9 +69,50 @@ struct Dims {
     int64_t S, Spad;
 };
 
+// Configuration of the private-tally sweep (ND_SWEEP_PRIVATE) for a given G; feasible == false -> atomic kernel only.
+struct PrivConfig {
+    bool feasible = false;
+    NdTileParams tp{};
+    int GPL = 4, LPT = 0, slot_bytes = 0, sigt_bytes = 0, chunk_cap = 0, warps = 0, smem_bytes = 0;
+    int64_t max_tiles = 0, max_swaths = 0;
+    size_t max_blob = 0;
+};
+
+constexpr int kSmemMax = 227 * 1024;
+
+PrivConfig make_priv_config(const Dims& d, const nd_options& opt)
+{
+    PrivConfig c;
+    c.GPL = 4;
+    c.LPT = d.Gs / 4;
+    if (c.LPT > 32) return c;
+    const int tpw = 32 / c.LPT;
+    int B = opt.track_batch > 0 ? opt.track_batch : (tpw >= 8 ? 8 : 16);
+    int Lw = opt.window_regions > 0 ? opt.window_regions : 32;
+    if (B > 64) B = 64;
+    if (Lw > 255) Lw = 255;
+    if (Lw < B) Lw = B;
+    c.tp.B = B; c.tp.Lw = Lw; c.tp.Nmax = 16 * B; c.tp.TPW = tpw;
+    c.chunk_cap = nd_chunk_capacity_bytes(c.tp);
+    c.slot_bytes = 8 * Lw * d.Gs + 4 * ((B + 3) / 4 * 4) + 2 * c.chunk_cap;
+    const int sig = 4 * d.M * d.Gs;
+    if (sig > 48 * 1024) return c;
+    c.sigt_bytes = (sig + 15) / 16 * 16;
+    c.warps = (kSmemMax - c.sigt_bytes) / (tpw * c.slot_bytes);
+    if (c.warps > 16) c.warps = 16;
+    if (c.warps < 1) return c;
+    c.smem_bytes = c.sigt_bytes + c.warps * tpw * c.slot_bytes;
+    c.max_swaths = d.T;
+    c.max_tiles = d.S / (Lw < c.tp.Nmax ? Lw : c.tp.Nmax) + d.T + 2;
+    const size_t per_tile = 16 + (size_t)((2 * (B + 1) + 15) / 16 * 16) + 4 * (size_t)Lw + 64;
+    c.max_blob = 6 * (size_t)d.S + (size_t)c.max_tiles * per_tile + 256;
+    c.feasible = true;
+    return c;
+}
+
 struct Layout { // byte offsets into the workspace
     size_t seg_rm, seg_len, trk_off, trk_w, link_src, psi_a, psi_b, q, tally, phi_a, phi_b, Q, reg_mat, vol, sigt, sigsT,
-        nusf, chi, sigt_f, scalars, partial, stats, total;
+        nusf, chi, sigt_f, scalars, partial, stats, blob, tile_chunk, swath_tile0, swath_track, items, counter, total;
 };
 
 inline size_t bump(size_t& cur, size_t bytes)
@@ -79,11 +122,11 @@ inline size_t bump(size_t& cur, size_t bytes)
     return at;
 }
 
-Layout make_layout(const Dims& d, int max_stats)
+Layout make_layout(const Dims& d, int max_stats, const PrivConfig& pc)
 {
     Layout L{};
     size_t c = 0;
-    const size_t RG = (size_t)d.R * d.G, RGs = (size_t)d.R * d.Gs, NPSI = (size_t)d.T * 2 * d.P * d.G;
+    const size_t RG = (size_t)d.R * d.G, RGs = (size_t)d.R * d.Gs, NPSI = (size_t)d.T * 2 * d.P * d.Gs;
     L.seg_rm = bump(c, sizeof(uint32_t) * (size_t)d.Spad);
     L.seg_len = bump(c, sizeof(float) * (size_t)d.Spad);
     L.trk_off = bump(c, sizeof(int64_t) * ((size_t)d.T + 1));
@@ -106,6 +149,14 @@ Layout make_layout(const Dims& d, int max_stats)
     L.scalars = bump(c, sizeof(double) * ndk::SC_COUNT);
     L.partial = bump(c, sizeof(double) * 3 * kReduceBlocks);
     L.stats = bump(c, sizeof(double) * 4 * (size_t)max_stats);
+    if (pc.feasible) {
+        L.blob = bump(c, pc.max_blob);
+        L.tile_chunk = bump(c, sizeof(uint32_t) * (size_t)pc.max_tiles);
+        L.swath_tile0 = bump(c, sizeof(int64_t) * ((size_t)pc.max_swaths + 1));
+        L.swath_track = bump(c, sizeof(int32_t) * (size_t)pc.max_swaths * pc.tp.B);
+        L.items = bump(c, sizeof(int4) * (2 * (size_t)pc.max_swaths + 2));
+        L.counter = bump(c, 256);
+    }
     L.total = c;
     return L;
 }
@@ -152,6 +203,13 @@ struct nd_problem {
     float* psi_in; float* psi_out; float* q; double* tally; double* phi_cur; double* phi_new; double* Q;
     int32_t* reg_mat; double* vol; double* sigt; double* sigsT; double* nusf; double* chi; float* sigt_f;
     double* scalars; double* partial; double* stats;
+    // private-tally sweep
+    PrivConfig pc{};
+    uint8_t* blob = nullptr; uint32_t* tile_chunk = nullptr; int64_t* swath_tile0 = nullptr; int32_t* swath_track = nullptr;
+    int4* items = nullptr; int* counter = nullptr;
+    int n_items = 0;
+    int64_t n_tiles = 0;
+    double mean_regions_per_tile = 0.0, mean_segments_per_tile = 0.0;
     // host copies
     std::vector<double> h_vol;
     float c[ndk::kMaxPolar]{}, inv_sin[ndk::kMaxPolar]{}, wp[ndk::kMaxPolar]{};
@@ -206,6 +264,37 @@ nd_status launch_fission_rate(nd_problem* p, const double* d_phi, double* d_out,
 }
 
 template <int P>
+nd_status launch_private_p(nd_problem* p, const ndk::PrivParams& prm, cudaStream_t st)
+{
+    const PrivConfig& c = p->pc;
+    auto kern = p->opt.exp_mode == ND_EXP_EXPM1 ? ndk::k_sweep_private<P, 4, 1> : ndk::k_sweep_private<P, 4, 0>;
+    ND_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes));
+    kern<<<p->n_sm, 32 * c.warps, c.smem_bytes, st>>>(prm);
+    ND_LAUNCH_CHECK(p);
+    return ND_OK;
+}
+
+nd_status launch_private(nd_problem* p, const double* scale_div, cudaStream_t st)
+{
+    const Dims& d = p->d;
+    const PrivConfig& c = p->pc;
+    ndk::PrivParams prm{};
+    prm.blob = p->blob; prm.tile_chunk = p->tile_chunk; prm.swath_tile0 = p->swath_tile0; prm.swath_track = p->swath_track;
+    prm.items = p->items; prm.counter = p->counter; prm.q = p->q; prm.sigt = p->sigt_f; prm.tally = p->tally; prm.trk_w = p->trk_w;
+    prm.psi_in = p->psi_in; prm.psi_out = p->psi_out; prm.scale_div = scale_div;
+    prm.n_items = p->n_items; prm.G = d.G; prm.Gs = d.Gs; prm.M = d.M; prm.B = c.tp.B; prm.Lw = c.tp.Lw; prm.LPT = c.LPT; prm.TPW = c.tp.TPW;
+    prm.slot_bytes = c.slot_bytes; prm.sigt_bytes = c.sigt_bytes; prm.chunk_cap = c.chunk_cap;
+    for (int i = 0; i < ndk::kMaxPolar; ++i) { prm.c[i] = p->c[i]; prm.inv_sin[i] = p->inv_sin[i]; prm.wp[i] = p->wp[i]; }
+    ND_CUDA(cudaMemsetAsync(p->counter, 0, sizeof(int), st));
+    switch (d.P) {
+    case 1: return launch_private_p<1>(p, prm, st);
+    case 2: return launch_private_p<2>(p, prm, st);
+    case 3: return launch_private_p<3>(p, prm, st);
+    default: return launch_private_p<4>(p, prm, st);
+    }
+}
+
+template <int P>
 nd_status launch_sweep_p(nd_problem* p, const ndk::SweepParams& prm, cudaStream_t st)
 {
     const Dims& d = p->d;
@@ -243,15 +332,19 @@ nd_status launch_sweep(nd_problem* p, const double* scale_div, cudaStream_t st)
         ND_CUDA(cudaEventRecord(ev->a, st));
     }
     nd_status rc;
-    switch (d.P) {
-    case 1: rc = launch_sweep_p<1>(p, prm, st); break;
-    case 2: rc = launch_sweep_p<2>(p, prm, st); break;
-    case 3: rc = launch_sweep_p<3>(p, prm, st); break;
-    default: rc = launch_sweep_p<4>(p, prm, st); break;
+    if (p->sweep_kernel == ND_SWEEP_PRIVATE) {
+        rc = launch_private(p, scale_div, st);
+    } else {
+        switch (d.P) {
+        case 1: rc = launch_sweep_p<1>(p, prm, st); break;
+        case 2: rc = launch_sweep_p<2>(p, prm, st); break;
+        case 3: rc = launch_sweep_p<3>(p, prm, st); break;
+        default: rc = launch_sweep_p<4>(p, prm, st); break;
+        }
     }
     if (rc != ND_OK) return rc;
     if (ev) ND_CUDA(cudaEventRecord(ev->b, st));
-    const int PG = d.P * d.G;
+    const int PG = d.P * d.Gs;
     const int64_t n = 2 * (int64_t)d.T * PG;
     ndk::k_link_swap<<<grid_for(n, 256, 8 * p->n_sm), 256, 0, st>>>(p->psi_out, p->psi_in, p->link_src, 2 * (int64_t)d.T, PG);
     ND_LAUNCH_CHECK(p);
@@ -278,7 +371,7 @@ nd_status reset_state(nd_problem* p, cudaStream_t st)
     const Dims& d = p->d;
     nd_status rc;
     if ((rc = launch_fill_f64(p, p->phi_cur, 1.0, (int64_t)d.R * d.G, st)) != ND_OK) return rc;
-    if ((rc = launch_fill_f32(p, p->psi_in, 0.f, (int64_t)d.T * 2 * d.P * d.G, st)) != ND_OK) return rc;
+    if ((rc = launch_fill_f32(p, p->psi_in, 0.f, (int64_t)d.T * 2 * d.P * d.Gs, st)) != ND_OK) return rc;
     const double sc[ndk::SC_COUNT] = {1.0, 0.0, 1.0, 0.0, 1.0, 0.0, 0.0, 0.0};
     ND_CUDA(cudaMemcpyAsync(p->scalars, sc, sizeof sc, cudaMemcpyHostToDevice, st));
     ND_CUDA(cudaStreamSynchronize(st)); // sc is a stack array
@@ -290,13 +383,17 @@ nd_status reset_state(nd_problem* p, cudaStream_t st)
 // ------------------------------------------------------------------------------------------------
 // create / destroy
 // ------------------------------------------------------------------------------------------------
-extern "C" nd_status nd_workspace_bytes(const nd_problem_desc* desc, const nd_options*, size_t* device_bytes)
+extern "C" nd_status nd_workspace_bytes(const nd_problem_desc* desc, const nd_options* opts, size_t* device_bytes)
 {
     if (!device_bytes) return nd_fail(ND_ERR_NULL, "device_bytes is NULL");
     Dims d{};
     nd_status rc = basic_dims(desc, d);
     if (rc != ND_OK) return rc;
-    *device_bytes = make_layout(d, kMaxStats).total;
+    nd_options opt{};
+    if (opts) opt = *opts;
+    PrivConfig pc;
+    if (opt.sweep_kernel != ND_SWEEP_ATOMIC) pc = make_priv_config(d, opt);
+    *device_bytes = make_layout(d, kMaxStats, pc).total;
     return ND_OK;
 }
 
@@ -317,7 +414,11 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         if (opt.reserved[i] != 0) return nd_fail(ND_ERR_INVALID, "nd_options.reserved must be zero");
     if (opt.exp_mode != ND_EXP_FAST && opt.exp_mode != ND_EXP_EXPM1) return nd_fail(ND_ERR_INVALID, "unknown exp_mode");
     if (opt.sweep_kernel < ND_SWEEP_AUTO || opt.sweep_kernel > ND_SWEEP_PRIVATE) return nd_fail(ND_ERR_INVALID, "unknown sweep_kernel");
-    const Layout L = make_layout(d, kMaxStats);
+    if ((desc->track_azim == nullptr) != (desc->track_ends == nullptr))
+        return nd_fail(ND_ERR_INVALID, "track_azim and track_ends must both be set or both be NULL");
+    PrivConfig pc;
+    if (opt.sweep_kernel != ND_SWEEP_ATOMIC) pc = make_priv_config(d, opt);
+    const Layout L = make_layout(d, kMaxStats, pc);
     if (reinterpret_cast<uintptr_t>(device_workspace) % kAlign != 0) return nd_fail(ND_ERR_WORKSPACE, "workspace must be 256-byte aligned");
     if (device_bytes < L.total) return nd_fail(ND_ERR_WORKSPACE, "workspace smaller than nd_workspace_bytes");
 
@@ -386,6 +487,18 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         delete p;
         return nd_fail(ND_ERR_NOMEM, "nd_problem_create: out of host memory");
     }
+    // ---- A1 (fast path): swath/tile chunk stream for the private-tally sweep ----
+    NdTileSet tiles;
+    const bool want_private = pc.feasible && (opt.sweep_kernel == ND_SWEEP_PRIVATE || (opt.sweep_kernel == ND_SWEEP_AUTO && desc->track_ends));
+    if (want_private) {
+        rc = nd_build_tiles(desc, desc->track_azim, desc->track_ends, pc.tp, 0, &tiles);
+        if (rc != ND_OK) { delete p; return rc; }
+        if (tiles.blob.size() > pc.max_blob || tiles.n_tiles + 1 > pc.max_tiles || tiles.n_swaths > pc.max_swaths) {
+            delete p;
+            return nd_fail(ND_ERR_WORKSPACE, "internal: tile stream larger than its workspace bound");
+        }
+    }
+    p->pc = pc;
     char* ws = p->ws;
     p->seg_rm = (uint32_t*)(ws + L.seg_rm); p->seg_len = (float*)(ws + L.seg_len); p->trk_off = (int64_t*)(ws + L.trk_off);
     p->trk_w = (float*)(ws + L.trk_w); p->link_src = (int32_t*)(ws + L.link_src);
@@ -396,6 +509,10 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     p->sigt = (double*)(ws + L.sigt); p->sigsT = (double*)(ws + L.sigsT); p->nusf = (double*)(ws + L.nusf);
     p->chi = (double*)(ws + L.chi); p->sigt_f = (float*)(ws + L.sigt_f);
     p->scalars = (double*)(ws + L.scalars); p->partial = (double*)(ws + L.partial); p->stats = (double*)(ws + L.stats);
+    if (pc.feasible) {
+        p->blob = (uint8_t*)(ws + L.blob); p->tile_chunk = (uint32_t*)(ws + L.tile_chunk); p->swath_tile0 = (int64_t*)(ws + L.swath_tile0);
+        p->swath_track = (int32_t*)(ws + L.swath_track); p->items = (int4*)(ws + L.items); p->counter = (int*)(ws + L.counter);
+    }
 
     cudaStream_t st = as_stream(cuda_stream);
     auto fail = [&](nd_status s) { delete p; return s; };
@@ -422,7 +539,7 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         p->inv_sin[i] = (float)(1.0 / desc->polar_sin[i]);
         p->wp[i] = (float)(desc->polar_weight[i] * desc->polar_sin[i]);
     }
-    p->sweep_kernel = ND_SWEEP_ATOMIC;
+    p->sweep_kernel = want_private ? ND_SWEEP_PRIVATE : ND_SWEEP_ATOMIC;
 
 #define ND_CUDA_P(call)                                                                                 \
     do {                                                                                                \
@@ -433,7 +550,19 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
             return fail(nd_fail(ND_ERR_CUDA, buf_));                                                    \
         }                                                                                               \
     } while (0)
-    ND_CUDA_P(cudaMemsetAsync(ws, 0, L.total, st));
+    ND_CUDA_P(cudaMemsetAsync(ws, 0, pc.feasible ? L.blob : L.total, st));
+    if (want_private) {
+        static_assert(sizeof(NdTileItem) == sizeof(int4), "work item layout");
+        p->n_items = (int)tiles.items.size();
+        p->n_tiles = tiles.n_tiles;
+        p->mean_regions_per_tile = tiles.mean_regions_per_tile;
+        p->mean_segments_per_tile = tiles.mean_segments_per_tile;
+        ND_CUDA_P(cudaMemcpyAsync(p->blob, tiles.blob.data(), tiles.blob.size(), cudaMemcpyHostToDevice, st));
+        ND_CUDA_P(cudaMemcpyAsync(p->tile_chunk, tiles.tile_chunk.data(), sizeof(uint32_t) * tiles.tile_chunk.size(), cudaMemcpyHostToDevice, st));
+        ND_CUDA_P(cudaMemcpyAsync(p->swath_tile0, tiles.swath_tile0.data(), sizeof(int64_t) * tiles.swath_tile0.size(), cudaMemcpyHostToDevice, st));
+        ND_CUDA_P(cudaMemcpyAsync(p->swath_track, tiles.swath_track.data(), sizeof(int32_t) * tiles.swath_track.size(), cudaMemcpyHostToDevice, st));
+        ND_CUDA_P(cudaMemcpyAsync(p->items, tiles.items.data(), sizeof(NdTileItem) * tiles.items.size(), cudaMemcpyHostToDevice, st));
+    }
     ND_CUDA_P(cudaMemcpyAsync(p->seg_rm, h_rm.data(), sizeof(uint32_t) * h_rm.size(), cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->seg_len, h_len.data(), sizeof(float) * h_len.size(), cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->trk_off, h_off.data(), sizeof(int64_t) * h_off.size(), cudaMemcpyHostToDevice, st));
@@ -578,14 +707,16 @@ extern "C" nd_status nd_state_reset(nd_problem* p, void* cuda_stream)
 extern "C" nd_status nd_boundary_flux_fill(nd_problem* p, float value, void* cuda_stream)
 {
     if (!p) return nd_fail(ND_ERR_NULL, "nd_boundary_flux_fill: NULL problem");
-    return launch_fill_f32(p, p->psi_in, value, (int64_t)p->d.T * 2 * p->d.P * p->d.G, as_stream(cuda_stream));
+    return launch_fill_f32(p, p->psi_in, value, (int64_t)p->d.T * 2 * p->d.P * p->d.Gs, as_stream(cuda_stream));
 }
 
 extern "C" nd_status nd_boundary_flux_get(nd_problem* p, float* host_out, void* cuda_stream)
 {
     if (!p || !host_out) return nd_fail(ND_ERR_NULL, "nd_boundary_flux_get: NULL argument");
     cudaStream_t st = as_stream(cuda_stream);
-    ND_CUDA(cudaMemcpyAsync(host_out, p->psi_in, sizeof(float) * (size_t)p->d.T * 2 * p->d.P * p->d.G, cudaMemcpyDeviceToHost, st));
+    const Dims& d = p->d;
+    const size_t rows = (size_t)d.T * 2 * d.P;
+    ND_CUDA(cudaMemcpy2DAsync(host_out, sizeof(float) * d.G, p->psi_in, sizeof(float) * d.Gs, sizeof(float) * d.G, rows, cudaMemcpyDeviceToHost, st));
     ND_CUDA(cudaStreamSynchronize(st));
     return ND_OK;
 }
@@ -594,7 +725,10 @@ extern "C" nd_status nd_boundary_flux_set(nd_problem* p, const float* host_in, v
 {
     if (!p || !host_in) return nd_fail(ND_ERR_NULL, "nd_boundary_flux_set: NULL argument");
     cudaStream_t st = as_stream(cuda_stream);
-    ND_CUDA(cudaMemcpyAsync(p->psi_in, host_in, sizeof(float) * (size_t)p->d.T * 2 * p->d.P * p->d.G, cudaMemcpyHostToDevice, st));
+    const Dims& d = p->d;
+    const size_t rows = (size_t)d.T * 2 * d.P;
+    ND_CUDA(cudaMemsetAsync(p->psi_in, 0, sizeof(float) * rows * d.Gs, st));
+    ND_CUDA(cudaMemcpy2DAsync(p->psi_in, sizeof(float) * d.Gs, host_in, sizeof(float) * d.G, sizeof(float) * d.G, rows, cudaMemcpyHostToDevice, st));
     ND_CUDA(cudaStreamSynchronize(st));
     return ND_OK;
 }
@@ -672,6 +806,6 @@ extern "C" nd_status nd_problem_info_get(const nd_problem* p, nd_problem_info* o
     out->algorithmic_bytes = 8 * d.S + 2 * 4 * (int64_t)d.T * 2 * d.P * d.G + 12 * (int64_t)d.R * d.G;
     out->group_stride = d.Gs;
     out->sweep_kernel = p->sweep_kernel;
-    out->n_batches = 0;
+    out->n_batches = (int32_t)(p->n_tiles > INT32_MAX ? INT32_MAX : p->n_tiles);
     return ND_OK;
 }

@@ -29,8 +29,8 @@ struct SweepParams {
     const float* __restrict__ sigt;        // [M][Gs]
     double* __restrict__ tally;            // [R][Gs]
     // boundary flux
-    const float* __restrict__ psi_in;      // [T][2][P][G]
-    float* __restrict__ psi_out;           // [T][2][P][G]
+    const float* __restrict__ psi_in;      // [T][2][P][Gs]
+    float* __restrict__ psi_out;           // [T][2][P][Gs]
     const double* __restrict__ scale_div;  // device scalar F: psi_in is used as psi_in / F
     int T, G, Gs;
     float c[kMaxPolar];                    // -log2(e)/sin(theta_p)      (ND_EXP_FAST)
@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(256) k_sweep_atomic(const SweepParams prm)
         for (int g = lane; g < prm.G; g += 32) {
             float psi[P];
 #pragma unroll
-            for (int p = 0; p < P; ++p) psi[p] = prm.psi_in[(pair * P + p) * prm.G + g] * inv_f;
+            for (int p = 0; p < P; ++p) psi[p] = prm.psi_in[(pair * P + p) * prm.Gs + g] * inv_f;
             for (int64_t i = 0; i < k1 - k0; ++i) {
                 const int64_t k = dir == 0 ? k0 + i : k1 - 1 - i;
                 const uint32_t rm = prm.seg_rm[k];
@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(256) k_sweep_atomic(const SweepParams prm)
                 if (s > 0.f) atomicAdd(&prm.tally[(size_t)r * prm.Gs + g], (double)(wt * acc));
             }
 #pragma unroll
-            for (int p = 0; p < P; ++p) prm.psi_out[(pair * P + p) * prm.G + g] = psi[p];
+            for (int p = 0; p < P; ++p) prm.psi_out[(pair * P + p) * prm.Gs + g] = psi[p];
         }
     }
 }

@@ -97,7 +97,8 @@ def _desc_for(m, xs, tr, P=2):
                 so=tr.seg_offset.copy(), sr=tr.seg_region.copy(), sl=tr.seg_length.copy(), tw=tr.track_weight.copy(),
                 lk=tr.link.copy())
     d = nd.nd_problem_desc(len(keep["rm"]), xs.n_materials, xs.n_groups, P, tr.n_tracks,
-                           *[keep[k].ctypes.data for k in ("rm", "st", "ss", "nf", "ch", "ps", "pw", "so", "sr", "sl", "tw", "lk")])
+                           *[keep[k].ctypes.data for k in ("rm", "st", "ss", "nf", "ch", "ps", "pw", "so", "sr", "sl", "tw", "lk")],
+                           None, None)
     return d, keep
 
 
