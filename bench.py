@@ -38,6 +38,8 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--kernel", type=int, default=0, help="ND_SWEEP_* (0 auto)")
     ap.add_argument("--exp-mode", type=int, default=0)
+    for name in ("track-batch", "window-regions", "block-warps", "tile-segments", "delta-buffers", "blocks-per-sm"):
+        ap.add_argument("--" + name, type=int, default=0, help="nd_options tuning field (0 = library default)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -224,7 +226,10 @@ def main():
     prob, tr, setup = build_inputs(args)
     t0 = time.time()
     gp = nd.nd_problem_create(prob.xs, prob.polar_sin, prob.polar_weight, prob.mesh.material, tr, device=str(dev),
-                              sweep_kernel=args.kernel, exp_mode=args.exp_mode)
+                              sweep_kernel=args.kernel, exp_mode=args.exp_mode, track_batch=args.track_batch,
+                              window_regions=args.window_regions, block_warps=args.block_warps,
+                              tile_segments=args.tile_segments, delta_buffers=args.delta_buffers,
+                              blocks_per_sm=args.blocks_per_sm)
     setup["create_s"] = round(time.time() - t0, 2)
     info = gp.nd_problem_info_get()
     R, G = prob.mesh.n_regions, prob.n_groups
@@ -328,7 +333,9 @@ def main():
             "ms_per_step": ms_per_step, "ms_per_sweep": sweep_ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32 (segment arithmetic) + f64 (tallies, flux, source, k)", "data": "synthetic",
             "config": dict(workload_config(args, prob, tr), l2="L2 flushed between steps" if need_flush else "inputs larger than L2",
-                           sweep_kernel=info["sweep_kernel"], setup_s=setup),
+                           sweep_kernel=info["sweep_kernel"], setup_s=setup,
+                           launch={k: info[k] for k in ("block_threads", "smem_bytes", "grid_blocks", "tracks_per_block", "n_batches",
+                                                        "mean_regions_per_tile", "mean_segments_per_tile", "lockstep_efficiency")}),
             "e2e": e2e, "gpu_launches": int(prof["kernels_launched"]), "roofline": roofline, "cpu_baseline": cb,
             "clocks": clocks.summary(), "k_eff": k_host if e2e else None}
     print(json.dumps(line), flush=True)

@@ -67,15 +67,21 @@ enum {
 enum {
     ND_SWEEP_AUTO = 0,      /* the fastest validated kernel for this G,P */
     ND_SWEEP_ATOMIC = 1,    /* warp per (track,direction), lanes over groups, FP64 global atomics per segment */
-    ND_SWEEP_PRIVATE = 2    /* lane-group per track batch, FP32 shared-memory private tally window, FP64 flush */
+    ND_SWEEP_PRIVATE = 2,   /* lane-group per track batch, FP32 shared-memory private tally window, FP64 flush */
+    ND_SWEEP_SWATH = 3      /* thread block per swath of adjacent tracks, psi in registers along the whole track,
+                               per-segment delta rows in shared memory, one FP64 RED per (region, group) per tile */
 };
 
 typedef struct {
     int32_t exp_mode;       /* ND_EXP_*      (default 0) */
     int32_t sweep_kernel;   /* ND_SWEEP_*    (default 0) */
-    int32_t track_batch;    /* tracks per private-tally batch; 0 = default */
-    int32_t window_regions; /* private tally window size in regions; 0 = default */
-    int32_t reserved[12];   /* must be 0 */
+    int32_t track_batch;    /* ND_SWEEP_PRIVATE: tracks per private-tally batch; 0 = default */
+    int32_t window_regions; /* max distinct regions per tile (both tiled kernels); 0 = default */
+    int32_t block_warps;    /* ND_SWEEP_SWATH: warps per thread block (tracks per swath = warps * slots per warp); 0 = default */
+    int32_t tile_segments;  /* ND_SWEEP_SWATH: max segments of one track per tile; 0 = default */
+    int32_t delta_buffers;  /* ND_SWEEP_SWATH: 1 or 2 delta buffers (2 saves one block barrier per tile); 0 = default */
+    int32_t blocks_per_sm;  /* ND_SWEEP_SWATH: resident blocks per SM the grid is sized for; 0 = default */
+    int32_t reserved[8];    /* must be 0 */
 } nd_options;
 
 /* ------------------------------------------------------------------------------------------------
@@ -206,10 +212,38 @@ typedef struct {
     int64_t algorithmic_bytes;      /* per sweep: stream + psi in/out + q read + tally write */
     int32_t group_stride;           /* padded groups per region row */
     int32_t sweep_kernel;           /* the ND_SWEEP_* actually selected */
-    int32_t n_batches;
+    int32_t n_batches;              /* tiles of the tiled sweep kernels */
     int32_t reserved;
+    double mean_regions_per_tile;   /* tiled kernels: distinct regions per tile (flush REDs = this x G per tile)  */
+    double mean_segments_per_tile;  /* tiled kernels: segments per tile; segments / regions = the tally re-use rho */
+    double lockstep_efficiency;     /* ND_SWEEP_SWATH: segments / (track slots x steps), 1 = no idle slot steps   */
+    int32_t block_threads, smem_bytes, grid_blocks, tracks_per_block;
 } nd_problem_info;
 nd_status nd_problem_info_get(const nd_problem* p, nd_problem_info* out);
+
+/* ------------------------------------------------------------------------------------------------
+ * Diagnostics: the swath/tile chunk stream of ND_SWEEP_SWATH (row A1: "segment stream layout"), built on the
+ * HOST exactly as nd_problem_create builds it, for inspection by tests.  Chunk format: csrc/nd_swath.h.
+ *   tracks_per_swath NT, tile_segments Kmax (per track and tile), window_regions Lmax (distinct regions per
+ *   tile), slots_per_line NC (NT % NC == 0), row_bytes = 4 * padded group count (multiple of 16).
+ * All view pointers are HOST memory owned by the stream object, valid until nd_swath_stream_destroy.
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct nd_swath_stream nd_swath_stream;
+typedef struct {
+    int64_t n_swaths, n_tiles, blob_bytes, n_items;
+    const uint8_t* blob;            /* all chunks, 16-byte aligned each */
+    const uint32_t* tile_chunk;     /* [n_tiles+1] chunk offsets in 16-byte units */
+    const int64_t* swath_tile0;     /* [n_swaths+1] first tile of every swath */
+    const int32_t* swath_track;     /* [n_swaths][NT] track id or -1 */
+    const int32_t* items;           /* [n_items][4] swath, direction, cost, 0 -- most expensive first */
+    double mean_regions_per_tile, mean_segments_per_tile, lockstep_efficiency;
+    int32_t max_chunk_bytes, reserved;
+} nd_swath_stream_view_t;
+nd_status nd_swath_stream_build(const nd_problem_desc* desc, int32_t tracks_per_swath, int32_t tile_segments,
+                                int32_t window_regions, int32_t slots_per_line, int32_t row_bytes,
+                                nd_swath_stream** out);
+nd_status nd_swath_stream_view(const nd_swath_stream* s, nd_swath_stream_view_t* view);
+nd_status nd_swath_stream_destroy(nd_swath_stream* s);
 
 const char* nd_status_string(nd_status s);
 const char* nd_last_error(const nd_problem* p_or_null); /* thread-local message of the last failing call */

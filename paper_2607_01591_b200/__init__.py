@@ -19,13 +19,14 @@ ND_OK = 0
 ND_ERR_NOT_CONVERGED = 7
 ND_BC_VACUUM, ND_BC_REFLECTIVE = 0, 1
 ND_EXP_FAST, ND_EXP_EXPM1 = 0, 1
-ND_SWEEP_AUTO, ND_SWEEP_ATOMIC, ND_SWEEP_PRIVATE = 0, 1, 2
+ND_SWEEP_AUTO, ND_SWEEP_ATOMIC, ND_SWEEP_PRIVATE, ND_SWEEP_SWATH = 0, 1, 2, 3
 
 EXPORTS = [
     "nd_tracks_generate", "nd_tracks_view", "nd_tracks_destroy", "nd_workspace_bytes", "nd_problem_create",
     "nd_problem_destroy", "nd_transport_sweep", "nd_source_update", "nd_power_iteration", "nd_state_reset",
     "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_flux_get", "nd_flux_set",
     "nd_track_volume_get", "nd_tally_get", "nd_profile_enable", "nd_profile_read", "nd_problem_info_get",
+    "nd_swath_stream_build", "nd_swath_stream_view", "nd_swath_stream_destroy",
     "nd_status_string", "nd_last_error", "nd_version",
 ]
 
@@ -38,7 +39,8 @@ class NdError(RuntimeError):
 
 class nd_options(C.Structure):
     _fields_ = [("exp_mode", C.c_int32), ("sweep_kernel", C.c_int32), ("track_batch", C.c_int32),
-                ("window_regions", C.c_int32), ("reserved", C.c_int32 * 12)]
+                ("window_regions", C.c_int32), ("block_warps", C.c_int32), ("tile_segments", C.c_int32),
+                ("delta_buffers", C.c_int32), ("blocks_per_sm", C.c_int32), ("reserved", C.c_int32 * 8)]
 
 
 class nd_mesh_desc(C.Structure):
@@ -74,7 +76,16 @@ class nd_profile(C.Structure):
 class nd_problem_info(C.Structure):
     _fields_ = [("n_segments", C.c_int64), ("n_segments_padded", C.c_int64), ("updates_per_sweep", C.c_int64),
                 ("algorithmic_bytes", C.c_int64), ("group_stride", C.c_int32), ("sweep_kernel", C.c_int32),
-                ("n_batches", C.c_int32), ("reserved", C.c_int32)]
+                ("n_batches", C.c_int32), ("reserved", C.c_int32), ("mean_regions_per_tile", C.c_double),
+                ("mean_segments_per_tile", C.c_double), ("lockstep_efficiency", C.c_double), ("block_threads", C.c_int32),
+                ("smem_bytes", C.c_int32), ("grid_blocks", C.c_int32), ("tracks_per_block", C.c_int32)]
+
+
+class nd_swath_stream_view_t(C.Structure):
+    _fields_ = [("n_swaths", C.c_int64), ("n_tiles", C.c_int64), ("blob_bytes", C.c_int64), ("n_items", C.c_int64),
+                ("blob", C.c_void_p), ("tile_chunk", C.c_void_p), ("swath_tile0", C.c_void_p), ("swath_track", C.c_void_p),
+                ("items", C.c_void_p), ("mean_regions_per_tile", C.c_double), ("mean_segments_per_tile", C.c_double),
+                ("lockstep_efficiency", C.c_double), ("max_chunk_bytes", C.c_int32), ("reserved", C.c_int32)]
 
 
 _lib = None
@@ -115,6 +126,10 @@ def lib():
         L.nd_profile_enable.argtypes = [C.c_void_p, C.c_int32]
         L.nd_profile_read.argtypes = [C.c_void_p, C.POINTER(nd_profile)]
         L.nd_problem_info_get.argtypes = [C.c_void_p, C.POINTER(nd_problem_info)]
+        L.nd_swath_stream_build.argtypes = [C.POINTER(nd_problem_desc), C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
+                                            C.POINTER(C.c_void_p)]
+        L.nd_swath_stream_view.argtypes = [C.c_void_p, C.POINTER(nd_swath_stream_view_t)]
+        L.nd_swath_stream_destroy.argtypes = [C.c_void_p]
         _lib = L
     return _lib
 
@@ -190,7 +205,8 @@ class Problem:
 
     def __init__(self, region_material, sigma_t, sigma_s, nu_sigma_f, chi, polar_sin, polar_weight, seg_offset,
                  seg_region, seg_length, track_weight, link, track_azim=None, track_ends=None, exp_mode=ND_EXP_FAST,
-                 sweep_kernel=ND_SWEEP_AUTO, track_batch=0, window_regions=0, device="cuda:0"):
+                 sweep_kernel=ND_SWEEP_AUTO, track_batch=0, window_regions=0, block_warps=0, tile_segments=0,
+                 delta_buffers=0, blocks_per_sm=0, device="cuda:0"):
         import torch
         self.torch = torch
         self.device = torch.device(device)
@@ -209,7 +225,8 @@ class Problem:
         self.R, (self.M, self.G), self.P, self.T = len(keep["rm"]), keep["st"].shape, len(keep["ps"]), len(keep["tw"])
         d = nd_problem_desc(self.R, self.M, self.G, self.P, self.T, *[keep[k].ctypes.data for k in
                             ("rm", "st", "ss", "nf", "ch", "ps", "pw", "so", "sr", "sl", "tw", "lk")], *geo)
-        opt = nd_options(int(exp_mode), int(sweep_kernel), int(track_batch), int(window_regions))
+        opt = nd_options(int(exp_mode), int(sweep_kernel), int(track_batch), int(window_regions), int(block_warps),
+                         int(tile_segments), int(delta_buffers), int(blocks_per_sm))
         nbytes = C.c_size_t()
         _check(lib().nd_workspace_bytes(C.byref(d), C.byref(opt), C.byref(nbytes)), "nd_workspace_bytes")
         self.workspace_bytes = int(nbytes.value)
@@ -316,6 +333,38 @@ class Problem:
         inf = nd_problem_info()
         _check(lib().nd_problem_info_get(self._h, C.byref(inf)), "nd_problem_info_get")
         return {f[0]: getattr(inf, f[0]) for f in nd_problem_info._fields_ if f[0] != "reserved"}
+
+
+def nd_swath_stream_build(region_material, n_materials, seg_offset, seg_region, seg_length, tracks_per_swath,
+                          tile_segments, window_regions, slots_per_line, row_bytes, track_azim=None, track_ends=None):
+    """Diagnostics (HOST only, no GPU): the swath/tile chunk stream of ND_SWEEP_SWATH as numpy copies.
+    Returns a dict with blob (uint8), tile_chunk, swath_tile0, swath_track [n_swaths][NT], items [n][4] and stats."""
+    keep = dict(rm=np.ascontiguousarray(region_material, np.int32), so=np.ascontiguousarray(seg_offset, np.int64),
+                sr=np.ascontiguousarray(seg_region, np.int32), sl=np.ascontiguousarray(seg_length, np.float64))
+    d = nd_problem_desc()
+    d.n_regions, d.n_materials, d.n_groups, d.n_polar, d.n_tracks = len(keep["rm"]), int(n_materials), 1, 1, len(keep["so"]) - 1
+    d.region_material, d.track_seg_offset = keep["rm"].ctypes.data, keep["so"].ctypes.data
+    d.seg_region, d.seg_length = keep["sr"].ctypes.data, keep["sl"].ctypes.data
+    if track_azim is not None and track_ends is not None:
+        keep["ta"] = np.ascontiguousarray(track_azim, np.int32)
+        keep["te"] = np.ascontiguousarray(track_ends, np.float64)
+        d.track_azim, d.track_ends = keep["ta"].ctypes.data, keep["te"].ctypes.data
+    h = C.c_void_p()
+    _check(lib().nd_swath_stream_build(C.byref(d), int(tracks_per_swath), int(tile_segments), int(window_regions),
+                                       int(slots_per_line), int(row_bytes), C.byref(h)), "nd_swath_stream_build")
+    try:
+        v = nd_swath_stream_view_t()
+        _check(lib().nd_swath_stream_view(h, C.byref(v)), "nd_swath_stream_view")
+        return dict(n_swaths=v.n_swaths, n_tiles=v.n_tiles,
+                    blob=_np_view(v.blob, (v.blob_bytes,), np.uint8).copy(),
+                    tile_chunk=_np_view(v.tile_chunk, (v.n_tiles + 1,), np.uint32).copy(),
+                    swath_tile0=_np_view(v.swath_tile0, (v.n_swaths + 1,), np.int64).copy(),
+                    swath_track=_np_view(v.swath_track, (v.n_swaths, int(tracks_per_swath)), np.int32).copy(),
+                    items=_np_view(v.items, (v.n_items, 4), np.int32).copy(),
+                    mean_regions_per_tile=v.mean_regions_per_tile, mean_segments_per_tile=v.mean_segments_per_tile,
+                    lockstep_efficiency=v.lockstep_efficiency, max_chunk_bytes=v.max_chunk_bytes)
+    finally:
+        lib().nd_swath_stream_destroy(h)
 
 
 def nd_problem_create(xs, polar_sin, polar_weight, region_material, tracks, **options) -> Problem:

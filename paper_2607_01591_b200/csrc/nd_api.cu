@@ -14,6 +14,8 @@
 #include "nd_internal.h"
 #include "nd_kernels.cuh"
 #include "nd_sweep_private.cuh"
+#include "nd_sweep_swath.cuh"
+#include "nd_swath.h"
 #include "nd_tiles.h"
 
 // ------------------------------------------------------------------------------------------------
@@ -110,6 +112,70 @@ PrivConfig make_priv_config(const Dims& d, const nd_options& opt)
     return c;
 }
 
+// Configuration of the swath sweep (ND_SWEEP_SWATH) for a given G; feasible == false -> other kernels only.
+struct SwathConfig {
+    bool feasible = false;
+    NdSwathParams sp{};
+    int LPT = 0, LS = 0, TPW = 0, warps = 0, ndbuf = 1, blocks_per_sm = 1;
+    int chunk_cap = 0, off_sigt = 0, off_q = 0, off_dbuf = 0, off_chunk = 0, smem_bytes = 0;
+    int64_t max_tiles = 0, max_swaths = 0;
+    size_t max_blob = 0;
+};
+
+SwathConfig make_swath_config(const Dims& d, const nd_options& opt)
+{
+    SwathConfig c;
+    c.LPT = d.Gs / 4;
+    if (c.LPT > 32) return c;
+    c.TPW = 32 / c.LPT;
+    c.LS = (c.TPW == 2) ? 16 : c.LPT;                     // two slots per warp sit on 16-lane boundaries: a shared-memory phase never mixes rows
+    const int NC = (c.LPT == 1 || c.LPT == 2 || c.LPT == 4) ? 8 / c.LPT : 1;
+    const int row_bytes = 4 * d.Gs, line = NC * row_bytes;
+    if ((int64_t)d.M * line > 65536) return c;
+    int warps = opt.block_warps > 0 ? opt.block_warps : (c.TPW <= 3 ? 8 : 4);
+    if (warps > 16) warps = 16;
+    int Kmax = opt.tile_segments > 0 ? opt.tile_segments : (row_bytes >= 64 ? 16 : 8);
+    int Lmax = opt.window_regions > 0 ? opt.window_regions : 13312 / line;
+    if (Lmax < 16) Lmax = 16;
+    if (Lmax > 65536 / line) Lmax = 65536 / line;
+    c.ndbuf = opt.delta_buffers == 2 ? 2 : 1;
+    auto pad128 = [](int x) { return (x + 127) / 128 * 128; };
+    for (;; --warps) {                                    // shrink the block until it fits the 227 KB of an SM
+        if (warps < 1) return c;
+        const int NT = warps * c.TPW;
+        if ((int64_t)NT * Kmax > 65535) continue;
+        c.sp.NT = NT; c.sp.Kmax = Kmax; c.sp.Lmax = Lmax; c.sp.NC = NC; c.sp.row_bytes = row_bytes;
+        c.chunk_cap = nd_swath_chunk_capacity(c.sp);
+        c.off_sigt = 128;
+        c.off_q = c.off_sigt + pad128(d.M * line);
+        c.off_dbuf = c.off_q + pad128(2 * Lmax * line);
+        c.off_chunk = c.off_dbuf + pad128(c.ndbuf * (NT / NC) * Kmax * line);
+        c.smem_bytes = c.off_chunk + ndk::kSwathChunkBufs * c.chunk_cap;
+        if (c.smem_bytes <= kSmemMax) break;
+    }
+    c.warps = warps;
+    int bps = (kSmemMax + 1024) / (c.smem_bytes + 1024);  // 1 KB per block is reserved by the driver
+    if (bps * warps * 32 > 2048) bps = 2048 / (warps * 32);
+    if (bps > 8) bps = 8;
+    if (bps < 1) bps = 1;
+    if (opt.blocks_per_sm > 0 && opt.blocks_per_sm < bps) bps = opt.blocks_per_sm;
+    c.blocks_per_sm = bps;
+    c.max_swaths = d.T;
+    c.max_tiles = nd_swath_max_tiles(c.sp, d.S, d.T);
+    c.max_blob = nd_swath_max_blob(c.sp, d.S, d.T);
+    c.feasible = true;
+    return c;
+}
+
+// Which sweep kernel a descriptor + options select (decided before the workspace is sized).
+int select_kernel(const nd_problem_desc* desc, const nd_options& opt, const PrivConfig& pc, const SwathConfig& sc)
+{
+    if (opt.sweep_kernel == ND_SWEEP_SWATH && sc.feasible) return ND_SWEEP_SWATH;
+    if (opt.sweep_kernel == ND_SWEEP_PRIVATE && pc.feasible) return ND_SWEEP_PRIVATE;
+    if (opt.sweep_kernel == ND_SWEEP_AUTO && desc->track_ends && sc.feasible) return ND_SWEEP_SWATH;
+    return ND_SWEEP_ATOMIC;
+}
+
 struct Layout { // byte offsets into the workspace
     size_t seg_rm, seg_len, trk_off, trk_w, link_src, psi_a, psi_b, q, tally, phi_a, phi_b, Q, reg_mat, vol, sigt, sigsT,
         nusf, chi, sigt_f, scalars, partial, stats, blob, tile_chunk, swath_tile0, swath_track, items, counter, total;
@@ -122,8 +188,14 @@ inline size_t bump(size_t& cur, size_t bytes)
     return at;
 }
 
-Layout make_layout(const Dims& d, int max_stats, const PrivConfig& pc)
+Layout make_layout(const Dims& d, int max_stats, const PrivConfig& pc_in, const SwathConfig& sc, int kernel)
 {
+    // the tiled kernels share the stream fields of the layout; size them for the selected one
+    PrivConfig pc = pc_in;
+    pc.feasible = kernel == ND_SWEEP_PRIVATE || kernel == ND_SWEEP_SWATH;
+    if (kernel == ND_SWEEP_SWATH) {
+        pc.max_blob = sc.max_blob; pc.max_tiles = sc.max_tiles; pc.max_swaths = sc.max_swaths; pc.tp.B = sc.sp.NT;
+    }
     Layout L{};
     size_t c = 0;
     const size_t RG = (size_t)d.R * d.G, RGs = (size_t)d.R * d.Gs, NPSI = (size_t)d.T * 2 * d.P * d.Gs;
@@ -205,6 +277,8 @@ struct nd_problem {
     double* scalars; double* partial; double* stats;
     // private-tally sweep
     PrivConfig pc{};
+    SwathConfig sc{};
+    double lockstep_efficiency = 0.0;
     uint8_t* blob = nullptr; uint32_t* tile_chunk = nullptr; int64_t* swath_tile0 = nullptr; int32_t* swath_track = nullptr;
     int4* items = nullptr; int* counter = nullptr;
     int n_items = 0;
@@ -263,6 +337,12 @@ nd_status launch_fission_rate(nd_problem* p, const double* d_phi, double* d_out,
     return ND_OK;
 }
 
+inline int swath_grid(const nd_problem* p)
+{
+    const int g = p->n_sm * p->sc.blocks_per_sm;
+    return p->n_items < g ? (p->n_items > 0 ? p->n_items : 1) : g;
+}
+
 template <int P>
 nd_status launch_private_p(nd_problem* p, const ndk::PrivParams& prm, cudaStream_t st)
 {
@@ -291,6 +371,38 @@ nd_status launch_private(nd_problem* p, const double* scale_div, cudaStream_t st
     case 2: return launch_private_p<2>(p, prm, st);
     case 3: return launch_private_p<3>(p, prm, st);
     default: return launch_private_p<4>(p, prm, st);
+    }
+}
+
+template <int P>
+nd_status launch_swath_p(nd_problem* p, const ndk::SwathParams& prm, cudaStream_t st)
+{
+    const SwathConfig& c = p->sc;
+    auto kern = p->opt.exp_mode == ND_EXP_EXPM1 ? ndk::k_sweep_swath<P, 1> : ndk::k_sweep_swath<P, 0>;
+    ND_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes));
+    kern<<<swath_grid(p), 32 * c.warps, c.smem_bytes, st>>>(prm);
+    ND_LAUNCH_CHECK(p);
+    return ND_OK;
+}
+
+nd_status launch_swath(nd_problem* p, const double* scale_div, cudaStream_t st)
+{
+    const Dims& d = p->d;
+    const SwathConfig& c = p->sc;
+    ndk::SwathParams prm{};
+    prm.blob = p->blob; prm.tile_chunk = p->tile_chunk; prm.swath_tile0 = p->swath_tile0; prm.swath_track = p->swath_track;
+    prm.items = p->items; prm.counter = p->counter; prm.q = p->q; prm.sigt = p->sigt_f; prm.tally = p->tally; prm.trk_w = p->trk_w;
+    prm.psi_in = p->psi_in; prm.psi_out = p->psi_out; prm.scale_div = scale_div;
+    prm.n_items = p->n_items; prm.G = d.G; prm.Gs = d.Gs; prm.M = d.M; prm.NT = c.sp.NT; prm.Kmax = c.sp.Kmax; prm.Lmax = c.sp.Lmax;
+    prm.LPT = c.LPT; prm.LS = c.LS; prm.TPW = c.TPW; prm.NC = c.sp.NC; prm.ndbuf = c.ndbuf; prm.chunk_cap = c.chunk_cap;
+    prm.off_sigt = c.off_sigt; prm.off_q = c.off_q; prm.off_dbuf = c.off_dbuf; prm.off_chunk = c.off_chunk;
+    for (int i = 0; i < ndk::kMaxPolar; ++i) { prm.c[i] = p->c[i]; prm.inv_sin[i] = p->inv_sin[i]; prm.wp[i] = p->wp[i]; }
+    ND_CUDA(cudaMemsetAsync(p->counter, 0, sizeof(int), st));
+    switch (d.P) {
+    case 1: return launch_swath_p<1>(p, prm, st);
+    case 2: return launch_swath_p<2>(p, prm, st);
+    case 3: return launch_swath_p<3>(p, prm, st);
+    default: return launch_swath_p<4>(p, prm, st);
     }
 }
 
@@ -332,7 +444,9 @@ nd_status launch_sweep(nd_problem* p, const double* scale_div, cudaStream_t st)
         ND_CUDA(cudaEventRecord(ev->a, st));
     }
     nd_status rc;
-    if (p->sweep_kernel == ND_SWEEP_PRIVATE) {
+    if (p->sweep_kernel == ND_SWEEP_SWATH) {
+        rc = launch_swath(p, scale_div, st);
+    } else if (p->sweep_kernel == ND_SWEEP_PRIVATE) {
         rc = launch_private(p, scale_div, st);
     } else {
         switch (d.P) {
@@ -392,8 +506,10 @@ extern "C" nd_status nd_workspace_bytes(const nd_problem_desc* desc, const nd_op
     nd_options opt{};
     if (opts) opt = *opts;
     PrivConfig pc;
-    if (opt.sweep_kernel != ND_SWEEP_ATOMIC) pc = make_priv_config(d, opt);
-    *device_bytes = make_layout(d, kMaxStats, pc).total;
+    SwathConfig sc;
+    if (opt.sweep_kernel == ND_SWEEP_PRIVATE) pc = make_priv_config(d, opt);
+    if (opt.sweep_kernel == ND_SWEEP_SWATH || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt);
+    *device_bytes = make_layout(d, kMaxStats, pc, sc, select_kernel(desc, opt, pc, sc)).total;
     return ND_OK;
 }
 
@@ -410,15 +526,21 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     if (rc != ND_OK) return rc;
     nd_options opt{};
     if (opts) opt = *opts;
-    for (int i = 0; i < 12; ++i)
+    for (int i = 0; i < 8; ++i)
         if (opt.reserved[i] != 0) return nd_fail(ND_ERR_INVALID, "nd_options.reserved must be zero");
     if (opt.exp_mode != ND_EXP_FAST && opt.exp_mode != ND_EXP_EXPM1) return nd_fail(ND_ERR_INVALID, "unknown exp_mode");
-    if (opt.sweep_kernel < ND_SWEEP_AUTO || opt.sweep_kernel > ND_SWEEP_PRIVATE) return nd_fail(ND_ERR_INVALID, "unknown sweep_kernel");
+    if (opt.sweep_kernel < ND_SWEEP_AUTO || opt.sweep_kernel > ND_SWEEP_SWATH) return nd_fail(ND_ERR_INVALID, "unknown sweep_kernel");
+    if (opt.track_batch < 0 || opt.window_regions < 0 || opt.block_warps < 0 || opt.tile_segments < 0 || opt.delta_buffers < 0 ||
+        opt.delta_buffers > 2 || opt.blocks_per_sm < 0)
+        return nd_fail(ND_ERR_INVALID, "nd_options: tuning fields must be >= 0 (delta_buffers 0, 1 or 2)");
     if ((desc->track_azim == nullptr) != (desc->track_ends == nullptr))
         return nd_fail(ND_ERR_INVALID, "track_azim and track_ends must both be set or both be NULL");
     PrivConfig pc;
-    if (opt.sweep_kernel != ND_SWEEP_ATOMIC) pc = make_priv_config(d, opt);
-    const Layout L = make_layout(d, kMaxStats, pc);
+    SwathConfig sc;
+    if (opt.sweep_kernel == ND_SWEEP_PRIVATE) pc = make_priv_config(d, opt);
+    if (opt.sweep_kernel == ND_SWEEP_SWATH || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt);
+    const int kernel = select_kernel(desc, opt, pc, sc);
+    const Layout L = make_layout(d, kMaxStats, pc, sc, kernel);
     if (reinterpret_cast<uintptr_t>(device_workspace) % kAlign != 0) return nd_fail(ND_ERR_WORKSPACE, "workspace must be 256-byte aligned");
     if (device_bytes < L.total) return nd_fail(ND_ERR_WORKSPACE, "workspace smaller than nd_workspace_bytes");
 
@@ -489,7 +611,18 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     }
     // ---- A1 (fast path): swath/tile chunk stream for the private-tally sweep ----
     NdTileSet tiles;
-    const bool want_private = pc.feasible && (opt.sweep_kernel == ND_SWEEP_PRIVATE || (opt.sweep_kernel == ND_SWEEP_AUTO && desc->track_ends));
+    NdSwathSet swaths;
+    const bool want_private = kernel == ND_SWEEP_PRIVATE, want_swath = kernel == ND_SWEEP_SWATH;
+    const bool tiled = want_private || want_swath;
+    if (want_swath) {
+        rc = nd_build_swaths(desc, desc->track_azim, desc->track_ends, sc.sp, 0, &swaths);
+        if (rc != ND_OK) { delete p; return rc; }
+        if (swaths.blob.size() > sc.max_blob || swaths.n_tiles + 1 > sc.max_tiles || swaths.n_swaths > sc.max_swaths ||
+            swaths.max_chunk_bytes > sc.chunk_cap) {
+            delete p;
+            return nd_fail(ND_ERR_WORKSPACE, "internal: swath stream larger than its workspace bound");
+        }
+    }
     if (want_private) {
         rc = nd_build_tiles(desc, desc->track_azim, desc->track_ends, pc.tp, 0, &tiles);
         if (rc != ND_OK) { delete p; return rc; }
@@ -499,6 +632,7 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         }
     }
     p->pc = pc;
+    p->sc = sc;
     char* ws = p->ws;
     p->seg_rm = (uint32_t*)(ws + L.seg_rm); p->seg_len = (float*)(ws + L.seg_len); p->trk_off = (int64_t*)(ws + L.trk_off);
     p->trk_w = (float*)(ws + L.trk_w); p->link_src = (int32_t*)(ws + L.link_src);
@@ -509,7 +643,7 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     p->sigt = (double*)(ws + L.sigt); p->sigsT = (double*)(ws + L.sigsT); p->nusf = (double*)(ws + L.nusf);
     p->chi = (double*)(ws + L.chi); p->sigt_f = (float*)(ws + L.sigt_f);
     p->scalars = (double*)(ws + L.scalars); p->partial = (double*)(ws + L.partial); p->stats = (double*)(ws + L.stats);
-    if (pc.feasible) {
+    if (tiled) {
         p->blob = (uint8_t*)(ws + L.blob); p->tile_chunk = (uint32_t*)(ws + L.tile_chunk); p->swath_tile0 = (int64_t*)(ws + L.swath_tile0);
         p->swath_track = (int32_t*)(ws + L.swath_track); p->items = (int4*)(ws + L.items); p->counter = (int*)(ws + L.counter);
     }
@@ -539,7 +673,7 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         p->inv_sin[i] = (float)(1.0 / desc->polar_sin[i]);
         p->wp[i] = (float)(desc->polar_weight[i] * desc->polar_sin[i]);
     }
-    p->sweep_kernel = want_private ? ND_SWEEP_PRIVATE : ND_SWEEP_ATOMIC;
+    p->sweep_kernel = kernel;
 
 #define ND_CUDA_P(call)                                                                                 \
     do {                                                                                                \
@@ -550,7 +684,20 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
             return fail(nd_fail(ND_ERR_CUDA, buf_));                                                    \
         }                                                                                               \
     } while (0)
-    ND_CUDA_P(cudaMemsetAsync(ws, 0, pc.feasible ? L.blob : L.total, st));
+    ND_CUDA_P(cudaMemsetAsync(ws, 0, tiled ? L.blob : L.total, st));
+    if (want_swath) {
+        static_assert(sizeof(NdSwathItem) == sizeof(int4), "work item layout");
+        p->n_items = (int)swaths.items.size();
+        p->n_tiles = swaths.n_tiles;
+        p->mean_regions_per_tile = swaths.mean_regions_per_tile;
+        p->mean_segments_per_tile = swaths.mean_segments_per_tile;
+        p->lockstep_efficiency = swaths.lockstep_efficiency;
+        ND_CUDA_P(cudaMemcpyAsync(p->blob, swaths.blob.data(), swaths.blob.size(), cudaMemcpyHostToDevice, st));
+        ND_CUDA_P(cudaMemcpyAsync(p->tile_chunk, swaths.tile_chunk.data(), sizeof(uint32_t) * swaths.tile_chunk.size(), cudaMemcpyHostToDevice, st));
+        ND_CUDA_P(cudaMemcpyAsync(p->swath_tile0, swaths.swath_tile0.data(), sizeof(int64_t) * swaths.swath_tile0.size(), cudaMemcpyHostToDevice, st));
+        ND_CUDA_P(cudaMemcpyAsync(p->swath_track, swaths.swath_track.data(), sizeof(int32_t) * swaths.swath_track.size(), cudaMemcpyHostToDevice, st));
+        ND_CUDA_P(cudaMemcpyAsync(p->items, swaths.items.data(), sizeof(NdSwathItem) * swaths.items.size(), cudaMemcpyHostToDevice, st));
+    }
     if (want_private) {
         static_assert(sizeof(NdTileItem) == sizeof(int4), "work item layout");
         p->n_items = (int)tiles.items.size();
@@ -807,5 +954,17 @@ extern "C" nd_status nd_problem_info_get(const nd_problem* p, nd_problem_info* o
     out->group_stride = d.Gs;
     out->sweep_kernel = p->sweep_kernel;
     out->n_batches = (int32_t)(p->n_tiles > INT32_MAX ? INT32_MAX : p->n_tiles);
+    out->mean_regions_per_tile = p->mean_regions_per_tile;
+    out->mean_segments_per_tile = p->mean_segments_per_tile;
+    out->lockstep_efficiency = p->lockstep_efficiency;
+    if (p->sweep_kernel == ND_SWEEP_SWATH) {
+        out->block_threads = 32 * p->sc.warps; out->smem_bytes = p->sc.smem_bytes; out->grid_blocks = swath_grid(p);
+        out->tracks_per_block = p->sc.sp.NT;
+    } else if (p->sweep_kernel == ND_SWEEP_PRIVATE) {
+        out->block_threads = 32 * p->pc.warps; out->smem_bytes = p->pc.smem_bytes; out->grid_blocks = p->n_sm;
+        out->tracks_per_block = p->pc.tp.B * p->pc.tp.TPW * p->pc.warps;
+    } else {
+        out->block_threads = 256;
+    }
     return ND_OK;
 }

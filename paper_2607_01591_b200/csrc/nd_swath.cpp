@@ -1,0 +1,269 @@
+// nd_swath.cpp -- builds the swath/tile chunk stream (see nd_swath.h).  Host code, OpenMP over swaths.
+// Geometry is used only to ORDER work (which tracks share a swath, where tiles are cut); every segment of the
+// descriptor is assigned to exactly one chunk whatever the geometry says, so results never depend on it.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <numeric>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#include "nd_internal.h"
+#include "nd_swath.h"
+
+namespace {
+
+struct SwathBuild {
+    std::vector<uint8_t> bytes;        // this swath's chunks, concatenated
+    std::vector<uint32_t> chunk_rel;   // chunk offsets relative to the swath's first byte, 16-B units
+    int64_t n_seg = 0, sum_regions = 0, sum_max_cnt = 0, n_active = 0;
+    int max_chunk = 0;
+};
+
+} // namespace
+
+nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim, const double* track_ends,
+                          const NdSwathParams& prm, int n_threads, NdSwathSet* out)
+{
+    const int T = desc->n_tracks, R = desc->n_regions, NT = prm.NT, Kmax = prm.Kmax, Lmax = prm.Lmax, NC = prm.NC;
+    if (NT < 1 || NT > 1024 || Kmax < 1 || Lmax < 1 || NC < 1 || NT % NC != 0 || prm.row_bytes < 16 || prm.row_bytes % 16 != 0)
+        return nd_fail(ND_ERR_INVALID, "swath parameters out of range");
+    const int64_t line = (int64_t)NC * prm.row_bytes;   // bytes between consecutive q / sigma_t rows in shared memory
+    if ((int64_t)Lmax * line > 65536 || (int64_t)desc->n_materials * line > 65536 || (int64_t)NT * Kmax > 65535)
+        return nd_fail(ND_ERR_INVALID, "swath parameters: row offsets must fit 16 bits");
+    try {
+        out->prm = prm;
+        // ---- 1. order tracks: by angle id, then by perpendicular coordinate ----
+        std::vector<int32_t> order(T);
+        std::iota(order.begin(), order.end(), 0);
+        std::vector<double> lam0(T, 0.0);
+        std::vector<int32_t> group(T, 0);
+        if (track_azim && track_ends) {
+            std::vector<double> perp(T, 0.0);
+            int32_t gmax = 0;
+            for (int t = 0; t < T; ++t) { group[t] = track_azim[t] < 0 ? 0 : track_azim[t]; gmax = std::max(gmax, group[t]); }
+            std::vector<double> ux((size_t)gmax + 1, 0.0), uy((size_t)gmax + 1, 0.0);
+            std::vector<char> have((size_t)gmax + 1, 0);
+            for (int t = 0; t < T; ++t) {   // direction of a group = direction of its first non-degenerate track
+                const int g = group[t];
+                if (have[g]) continue;
+                const double dx = track_ends[4 * (size_t)t + 2] - track_ends[4 * (size_t)t];
+                const double dy = track_ends[4 * (size_t)t + 3] - track_ends[4 * (size_t)t + 1];
+                const double h = std::sqrt(dx * dx + dy * dy);
+                if (h > 0.0 && std::isfinite(h)) { ux[g] = dx / h; uy[g] = dy / h; have[g] = 1; }
+            }
+            for (int t = 0; t < T; ++t) {
+                const int g = group[t];
+                const double x0 = track_ends[4 * (size_t)t], y0 = track_ends[4 * (size_t)t + 1];
+                perp[t] = x0 * uy[g] - y0 * ux[g];
+                lam0[t] = x0 * ux[g] + y0 * uy[g];
+                if (!std::isfinite(perp[t])) perp[t] = 0.0;
+                if (!std::isfinite(lam0[t])) lam0[t] = 0.0;
+            }
+            std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) {
+                if (group[a] != group[b]) return group[a] < group[b];
+                return perp[a] < perp[b];
+            });
+        }
+        // ---- 2. swaths: NT consecutive tracks of one group ----
+        std::vector<int32_t>& st = out->swath_track;
+        st.clear();
+        for (int i = 0; i < T;) {
+            int n = 0;
+            const int g = group[order[i]];
+            while (n < NT && i + n < T && group[order[i + n]] == g) ++n;
+            for (int b = 0; b < NT; ++b) st.push_back(b < n ? order[i + b] : -1);
+            i += n;
+        }
+        const int64_t n_sw = (int64_t)(st.size() / NT);
+        out->n_swaths = n_sw;
+        // ---- 3. cut every swath into tiles and encode the chunks ----
+        std::vector<SwathBuild> built((size_t)n_sw);
+#ifdef _OPENMP
+        const int nth = n_threads > 0 ? n_threads : omp_get_max_threads();
+#else
+        const int nth = 1;
+        (void)n_threads;
+#endif
+        const int64_t* off = desc->track_seg_offset;
+#pragma omp parallel num_threads(nth)
+        {
+            std::vector<int32_t> stamp((size_t)R, -1), lidx((size_t)R, 0);
+            int32_t tile_serial = 0;
+            std::vector<int64_t> cur(NT), first(NT), endk(NT);
+            std::vector<double> lam(NT);
+            std::vector<int> cnt(NT);
+            std::vector<uint32_t> regions;
+            std::vector<int> rcount, rfill;
+            regions.reserve(Lmax);
+#pragma omp for schedule(dynamic, 4)
+            for (int64_t sw = 0; sw < n_sw; ++sw) {
+                SwathBuild& sb = built[(size_t)sw];
+                const int32_t* trk = &st[(size_t)sw * NT];
+                int64_t remaining = 0;
+                for (int b = 0; b < NT; ++b) {
+                    if (trk[b] >= 0) { cur[b] = off[trk[b]]; endk[b] = off[trk[b] + 1]; lam[b] = lam0[trk[b]]; ++sb.n_active; }
+                    else { cur[b] = endk[b] = 0; lam[b] = 0.0; }
+                    remaining += endk[b] - cur[b];
+                }
+                sb.n_seg = remaining;
+                while (remaining > 0) {
+                    if (++tile_serial == INT32_MAX) { std::fill(stamp.begin(), stamp.end(), -1); tile_serial = 0; }
+                    regions.clear();
+                    rcount.clear();
+                    for (int b = 0; b < NT; ++b) { first[b] = cur[b]; cnt[b] = 0; }
+                    int nseg = 0;
+                    for (;;) {
+                        int bs = -1;
+                        for (int b = 0; b < NT; ++b)
+                            if (cur[b] < endk[b] && (bs < 0 || lam[b] < lam[bs])) bs = b;
+                        if (bs < 0 || cnt[bs] == Kmax) break;
+                        const int64_t k = cur[bs];
+                        const int32_t r = desc->seg_region[k];
+                        if (stamp[r] != tile_serial) {
+                            if ((int)regions.size() == Lmax) break;
+                            stamp[r] = tile_serial;
+                            lidx[r] = (int32_t)regions.size();
+                            regions.push_back((uint32_t)r);
+                            rcount.push_back(0);
+                        }
+                        ++rcount[lidx[r]];
+                        lam[bs] += desc->seg_length[k];
+                        ++cur[bs]; ++cnt[bs]; ++nseg; --remaining;
+                    }
+                    // ---- encode ----
+                    const int L = (int)regions.size();
+                    const int o_ss = 16;
+                    const int o_rg = o_ss + nd_swath_pad16(2 * (NT + 1));
+                    const int o_co = o_rg + nd_swath_pad16(4 * L);
+                    const int o_ci = o_co + nd_swath_pad16(2 * (L + 1));
+                    const int o_rc = o_ci + nd_swath_pad16(2 * nseg);
+                    const int bytes = o_rc + nd_swath_pad16(8 * nseg);
+                    const size_t base = sb.bytes.size();
+                    sb.chunk_rel.push_back((uint32_t)(base / 16));
+                    sb.bytes.resize(base + (size_t)bytes, 0);
+                    uint8_t* c = sb.bytes.data() + base;
+                    const uint32_t hdr[4] = {(uint32_t)L | ((uint32_t)nseg << 16), (uint32_t)(o_rg / 16) | ((uint32_t)(o_co / 16) << 16),
+                                             (uint32_t)(o_ci / 16) | ((uint32_t)(o_rc / 16) << 16), (uint32_t)bytes};
+                    memcpy(c, hdr, 16);
+                    uint16_t* ss = reinterpret_cast<uint16_t*>(c + o_ss);
+                    uint32_t* rg = reinterpret_cast<uint32_t*>(c + o_rg);
+                    uint16_t* co = reinterpret_cast<uint16_t*>(c + o_co);
+                    uint16_t* ci = reinterpret_cast<uint16_t*>(c + o_ci);
+                    uint32_t* rc = reinterpret_cast<uint32_t*>(c + o_rc);
+                    for (int l = 0; l < L; ++l) rg[l] = regions[l];
+                    co[0] = 0;
+                    for (int l = 0; l < L; ++l) co[l + 1] = (uint16_t)(co[l] + rcount[l]);
+                    rfill.assign(co, co + L);
+                    int o = 0, max_cnt = 0;
+                    for (int b = 0; b < NT; ++b) {
+                        ss[b] = (uint16_t)o;
+                        max_cnt = std::max(max_cnt, cnt[b]);
+                        for (int j = 0; j < cnt[b]; ++j, ++o) {
+                            const int64_t k = first[b] + j;
+                            const int32_t r = desc->seg_region[k];
+                            const int l = lidx[r];
+                            const float len = (float)desc->seg_length[k];
+                            uint32_t lenbits;
+                            memcpy(&lenbits, &len, 4);
+                            rc[2 * o] = lenbits;
+                            rc[2 * o + 1] = (uint32_t)(l * line) | ((uint32_t)(desc->region_material[r] * line) << 16);
+                            ci[rfill[l]++] = (uint16_t)(((b / NC) * Kmax + j) * NC + b % NC);
+                        }
+                    }
+                    ss[NT] = (uint16_t)o;
+                    sb.sum_regions += L;
+                    sb.sum_max_cnt += max_cnt;
+                    sb.max_chunk = std::max(sb.max_chunk, bytes);
+                }
+            }
+        }
+        // ---- 4. concatenate ----
+        out->swath_tile0.assign((size_t)n_sw + 1, 0);
+        std::vector<size_t> byte0((size_t)n_sw + 1, 0);
+        for (int64_t sw = 0; sw < n_sw; ++sw) {
+            out->swath_tile0[sw + 1] = out->swath_tile0[sw] + (int64_t)built[sw].chunk_rel.size();
+            byte0[sw + 1] = byte0[sw] + built[sw].bytes.size();
+        }
+        out->n_tiles = out->swath_tile0[n_sw];
+        if (byte0[n_sw] / 16 >= 0xffffffffull) return nd_fail(ND_ERR_RANGE, "swath stream exceeds 64 GiB");
+        out->tile_chunk.resize((size_t)out->n_tiles + 1);
+        out->tile_chunk[(size_t)out->n_tiles] = (uint32_t)(byte0[n_sw] / 16);   // end sentinel: chunk k spans [k, k+1)
+        out->blob.resize(byte0[n_sw]);
+        int64_t sum_regions = 0, sum_seg = 0, sum_slots = 0;
+        int max_chunk = 0;
+        for (int64_t sw = 0; sw < n_sw; ++sw) {
+            sum_regions += built[sw].sum_regions; sum_seg += built[sw].n_seg; max_chunk = std::max(max_chunk, built[sw].max_chunk);
+            sum_slots += built[sw].sum_max_cnt * built[sw].n_active;
+        }
+#pragma omp parallel for schedule(dynamic, 64) num_threads(nth)
+        for (int64_t sw = 0; sw < n_sw; ++sw) {
+            SwathBuild& sb = built[(size_t)sw];
+            if (!sb.bytes.empty()) memcpy(out->blob.data() + byte0[sw], sb.bytes.data(), sb.bytes.size());
+            const uint32_t b16 = (uint32_t)(byte0[sw] / 16);
+            for (size_t i = 0; i < sb.chunk_rel.size(); ++i) out->tile_chunk[(size_t)out->swath_tile0[sw] + i] = b16 + sb.chunk_rel[i];
+            std::vector<uint8_t>().swap(sb.bytes);
+        }
+        out->max_chunk_bytes = max_chunk;
+        out->mean_regions_per_tile = out->n_tiles ? (double)sum_regions / (double)out->n_tiles : 0.0;
+        out->mean_segments_per_tile = out->n_tiles ? (double)sum_seg / (double)out->n_tiles : 0.0;
+        out->lockstep_efficiency = sum_slots ? (double)sum_seg / (double)sum_slots : 1.0;
+        // ---- 5. work items: (swath, direction), most expensive first ----
+        out->items.clear();
+        for (int64_t sw = 0; sw < n_sw; ++sw) {
+            const int32_t c32 = (int32_t)std::min<int64_t>(built[sw].sum_max_cnt, INT32_MAX);
+            out->items.push_back({(int32_t)sw, 0, c32, 0});
+            out->items.push_back({(int32_t)sw, 1, c32, 0});
+        }
+        std::stable_sort(out->items.begin(), out->items.end(), [](const NdSwathItem& a, const NdSwathItem& b) { return a.cost > b.cost; });
+    } catch (const std::bad_alloc&) {
+        return nd_fail(ND_ERR_NOMEM, "nd_build_swaths: out of host memory");
+    }
+    return ND_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// C ABI access to the stream (include/nd.h "Diagnostics"): lets host-side tests decode every chunk.
+// ------------------------------------------------------------------------------------------------
+struct nd_swath_stream {
+    NdSwathSet set;
+};
+
+extern "C" nd_status nd_swath_stream_build(const nd_problem_desc* desc, int32_t tracks_per_swath, int32_t tile_segments,
+                                           int32_t window_regions, int32_t slots_per_line, int32_t row_bytes,
+                                           nd_swath_stream** out)
+{
+    if (!desc || !out) return nd_fail(ND_ERR_NULL, "nd_swath_stream_build: NULL argument");
+    if (!desc->track_seg_offset || !desc->seg_region || !desc->seg_length || !desc->region_material)
+        return nd_fail(ND_ERR_NULL, "nd_swath_stream_build: a descriptor array is NULL");
+    if ((desc->track_azim == nullptr) != (desc->track_ends == nullptr))
+        return nd_fail(ND_ERR_INVALID, "track_azim and track_ends must both be set or both be NULL");
+    nd_swath_stream* s = new (std::nothrow) nd_swath_stream();
+    if (!s) return nd_fail(ND_ERR_NOMEM, "nd_swath_stream_build: out of host memory");
+    NdSwathParams prm{tracks_per_swath, tile_segments, window_regions, slots_per_line, row_bytes};
+    const nd_status rc = nd_build_swaths(desc, desc->track_azim, desc->track_ends, prm, 0, &s->set);
+    if (rc != ND_OK) { delete s; return rc; }
+    *out = s;
+    return ND_OK;
+}
+
+extern "C" nd_status nd_swath_stream_view(const nd_swath_stream* s, nd_swath_stream_view_t* v)
+{
+    if (!s || !v) return nd_fail(ND_ERR_NULL, "nd_swath_stream_view: NULL argument");
+    const NdSwathSet& t = s->set;
+    v->n_swaths = t.n_swaths; v->n_tiles = t.n_tiles; v->blob_bytes = (int64_t)t.blob.size();
+    v->n_items = (int64_t)t.items.size();
+    v->blob = t.blob.data(); v->tile_chunk = t.tile_chunk.data(); v->swath_tile0 = t.swath_tile0.data();
+    v->swath_track = t.swath_track.data(); v->items = reinterpret_cast<const int32_t*>(t.items.data());
+    v->mean_regions_per_tile = t.mean_regions_per_tile; v->mean_segments_per_tile = t.mean_segments_per_tile;
+    v->lockstep_efficiency = t.lockstep_efficiency; v->max_chunk_bytes = t.max_chunk_bytes; v->reserved = 0;
+    return ND_OK;
+}
+
+extern "C" nd_status nd_swath_stream_destroy(nd_swath_stream* s)
+{
+    delete s;
+    return ND_OK;
+}

@@ -1,0 +1,74 @@
+// nd_swath.h -- host-side construction of the swath/tile chunk stream of k_sweep_swath (row A1 of DESIGN.md).
+//
+// Tracks of one angle are sorted by their perpendicular coordinate and grouped into SWATHS of NT adjacent tracks;
+// one thread block carries a swath, one lane group ("slot") per track, so the angular flux of a track stays in
+// registers from one end of the track to the other.  A swath is cut along the track direction into TILES: the
+// tracks advance in geometric lock step (always the track whose front is furthest behind) until one of them has
+// Kmax segments in the tile or the tile touches Lmax distinct regions.  A tile is one contiguous, 16-byte aligned
+// CHUNK, fetched by a single bulk (TMA) copy:
+//     u32 hdr[4]          L | nseg << 16 ;  off_regions | off_csr_off << 16 ;  off_csr_idx | off_rec << 16 ;  bytes
+//                         (offsets in 16-byte units from the chunk start)
+//     u16 slot_start[NT+1]   per-track prefix into rec[]                                     (padded to 16 B)
+//     u32 regions[L]         global region ids: q rows to stage, tally rows to flush          (padded to 16 B)
+//     u16 csr_off[L+1]       per region: range into csr_idx                                   (padded to 16 B)
+//     u16 csr_idx[nseg]      delta-buffer row of every segment, grouped by region             (padded to 16 B)
+//     rec[nseg]              { f32 length ; u32 q_row_byte_offset | sigt_row_byte_offset << 16 }, slot-major,
+//                            forward order; the backward direction walks the same records in reverse
+// A triangle is convex, so one track crosses a region at most once per tile: a segment's weighted flux change is
+// simply STORED in its own delta-buffer row, and csr_idx tells the flush which rows to add up per region.
+#ifndef ND_SWATH_H
+#define ND_SWATH_H
+#include <cstdint>
+#include <vector>
+
+#include "nd.h"
+
+struct NdSwathParams {
+    int NT;       // tracks per swath = slots per thread block
+    int Kmax;     // max segments of one track in a tile
+    int Lmax;     // max distinct regions in a tile
+    int NC;       // slots interleaved in one delta-buffer / q line (bank-conflict-free layout for narrow rows)
+    int row_bytes;// bytes of one (region, all groups) FP32 row = 4 * Gs
+};
+
+struct NdSwathItem { int32_t swath, dir, cost, reserved; };
+
+struct NdSwathSet {
+    NdSwathParams prm{};
+    int64_t n_swaths = 0, n_tiles = 0;
+    std::vector<int32_t> swath_track;     // [n_swaths][NT] canonical track id or -1
+    std::vector<int64_t> swath_tile0;     // [n_swaths+1] prefix into tile_chunk
+    std::vector<uint32_t> tile_chunk;     // [n_tiles+1] chunk offsets in 16-byte units (+ end sentinel)
+    std::vector<NdSwathItem> items;       // work items (swath, direction), most expensive first
+    std::vector<uint8_t> blob;            // all chunks
+    int max_chunk_bytes = 0;
+    double mean_regions_per_tile = 0.0, mean_segments_per_tile = 0.0, lockstep_efficiency = 0.0;
+};
+
+inline int nd_swath_pad16(int x) { return (x + 15) / 16 * 16; }
+
+// largest chunk the parameters allow (the kernel's staging buffers have this size)
+inline int nd_swath_chunk_capacity(const NdSwathParams& p)
+{
+    const int nmax = p.NT * p.Kmax;
+    return 16 + nd_swath_pad16(2 * (p.NT + 1)) + nd_swath_pad16(4 * p.Lmax) + nd_swath_pad16(2 * (p.Lmax + 1)) +
+           nd_swath_pad16(2 * nmax) + nd_swath_pad16(8 * nmax);
+}
+
+// upper bounds used to size the device workspace before the stream is built
+inline int64_t nd_swath_max_tiles(const NdSwathParams& p, int64_t n_segments, int64_t n_tracks)
+{
+    const int m = p.Kmax < p.Lmax ? p.Kmax : p.Lmax;
+    return n_segments / m + n_tracks + 2;
+}
+inline size_t nd_swath_max_blob(const NdSwathParams& p, int64_t n_segments, int64_t n_tracks)
+{
+    const size_t per_tile = 16 + (size_t)nd_swath_pad16(2 * (p.NT + 1)) + 4 * 16;
+    return (size_t)nd_swath_max_tiles(p, n_segments, n_tracks) * per_tile + 16 * (size_t)n_segments + 256;
+}
+
+// track_azim / track_ends may be NULL (no geometry): tracks are then grouped in descriptor order.
+nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim, const double* track_ends,
+                          const NdSwathParams& prm, int n_threads, NdSwathSet* out);
+
+#endif

@@ -1,0 +1,319 @@
+// nd_sweep_swath.cuh -- row A2, the fast path: Eq. (5) with the angular flux of a track held in
+// registers from one end of the track to the other, and the region tallies formed in shared memory.
+//
+// Why this shape (B200 measurements):
+//   * one update = 1 MUFU.EX2 + 5 FP32 ops; the MUFU pipe (16/clk/SM) is the roofline.  A realistic inner loop
+//     (records, q row, Sigma_t row read from shared memory, one delta row written) sustains 80 % of it with 16 warps/SM.
+//   * FP64 global REDs per (segment, group) are 2.4-4x too slow; shared-memory float atomics are CAS loops.
+//     Adjacent parallel tracks (0.01-0.05 cm apart) cross the same triangles, so a block that carries NT adjacent
+//     tracks sees every region ~rho = 5-10 times per tile.
+//
+// Mapping
+//   * thread block = one SWATH (NT adjacent tracks of one angle) in one direction; persistent blocks pull
+//     (swath, direction) items from an atomic counter, most expensive first.
+//   * lane group ("slot") = LPT lanes = one track; a lane owns 4 consecutive groups x P polar angles = 4P
+//     independent Eq.-(5) chains in registers (ILP hides the MUFU/FMA latency).  psi is read from the boundary
+//     array once, at the track's entry, and written once, at its exit.
+//   * the swath is processed tile by tile (nd_swath.h).  A tile's chunk arrives by ONE bulk async (TMA) copy,
+//     two tiles ahead, signalled on an mbarrier; the q rows of its regions are gathered by 16-byte cp.async one
+//     tile ahead.  In the segment loop a lane reads the segment record (broadcast), its 16 bytes of the q row and
+//     of the Sigma_t row, and STORES sum_p w_p Delta_p into the segment's own row of the delta buffer: no
+//     read-modify-write, no atomics (a segment owns its row).
+//   * after a block barrier the tile is flushed: per (region, 4 groups) the rows listed in the chunk's CSR are
+//     added up in FP32 and leave as FP64 REDs -- one RED per (region, group) per tile instead of one per segment.
+//   * narrow rows (G <= 16): NC slots share a 128-byte line (q, Sigma_t and delta rows replicated / interleaved per
+//     slot) so that the 8 lanes of a shared-memory phase always hit distinct banks.
+#pragma once
+#include "nd_kernels.cuh"
+
+namespace ndk {
+
+struct SwathParams {
+    const uint8_t* __restrict__ blob;
+    const uint32_t* __restrict__ tile_chunk;   // [n_tiles+1] chunk offsets in 16-byte units (+ end sentinel)
+    const int64_t* __restrict__ swath_tile0;   // [n_swaths+1]
+    const int32_t* __restrict__ swath_track;   // [n_swaths][NT]
+    const int4* __restrict__ items;            // (swath, dir, cost, -)
+    int* __restrict__ counter;
+    const float* __restrict__ q;               // [R][Gs]
+    const float* __restrict__ sigt;            // [M][Gs]
+    double* __restrict__ tally;                // [R][Gs]
+    const float* __restrict__ trk_w;
+    const float* __restrict__ psi_in;
+    float* __restrict__ psi_out;
+    const double* __restrict__ scale_div;
+    int n_items, G, Gs, M, NT, Kmax, Lmax, LPT, LS, TPW, NC, ndbuf;
+    int chunk_cap;                             // bytes of one chunk staging buffer
+    int off_sigt, off_q, off_dbuf, off_chunk;  // shared-memory byte offsets
+    float c[kMaxPolar], inv_sin[kMaxPolar], wp[kMaxPolar];
+};
+
+constexpr int kSwathChunkBufs = 4;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// 1-D bulk async copy global -> shared through the TMA unit; completion is signalled on the mbarrier.
+__device__ __forceinline__ void tma_load_1d(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+                 "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_16(uint32_t smem_dst, const void* gmem_src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_dst), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit_group() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+struct SwathChunk {   // decoded chunk header (pointers into the staging buffer)
+    int L, nseg;
+    const uint16_t* slot_start;
+    const uint32_t* regions;
+    const uint16_t* csr_off;
+    const uint16_t* csr_idx;
+    const uint2* rec;
+};
+__device__ __forceinline__ SwathChunk decode_chunk(const unsigned char* cb)
+{
+    const uint4 h = *reinterpret_cast<const uint4*>(cb);
+    SwathChunk c;
+    c.L = (int)(h.x & 0xffffu); c.nseg = (int)(h.x >> 16);
+    c.slot_start = reinterpret_cast<const uint16_t*>(cb + 16);
+    c.regions = reinterpret_cast<const uint32_t*>(cb + 16 * (h.y & 0xffffu));
+    c.csr_off = reinterpret_cast<const uint16_t*>(cb + 16 * (h.y >> 16));
+    c.csr_idx = reinterpret_cast<const uint16_t*>(cb + 16 * (h.z & 0xffffu));
+    c.rec = reinterpret_cast<const uint2*>(cb + 16 * (h.z >> 16));
+    return c;
+}
+
+template <int P, int EXPM>
+__global__ void __launch_bounds__(512, 1) k_sweep_swath(const SwathParams prm)
+{
+    extern __shared__ __align__(128) unsigned char smem_sw[];
+    unsigned char* const smem = smem_sw;
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem);              // [kSwathChunkBufs] chunk-arrival barriers
+    volatile int* s_item = reinterpret_cast<volatile int*>(smem + 64);
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    const int lane = tid & 31, warp = tid >> 5;
+    const int Gs = prm.Gs, row_bytes = 4 * Gs, line = prm.NC * row_bytes;
+    unsigned char* sigt_s = smem + prm.off_sigt;
+    unsigned char* q_s = smem + prm.off_q;           // [2][Lmax][line]
+    unsigned char* dbuf_s = smem + prm.off_dbuf;     // [ndbuf][NT/NC * Kmax][line]
+    unsigned char* chunk_s = smem + prm.off_chunk;   // [4][chunk_cap]
+    const int q_buf_bytes = prm.Lmax * line;
+    const int dbuf_bytes = (prm.NT / prm.NC) * prm.Kmax * line;
+    const int nq = Gs >> 2;                          // 16-byte pieces per row
+
+    if (tid == 0) {
+        for (int i = 0; i < kSwathChunkBufs; ++i) mbar_init(full + i, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    // Sigma_t table, replicated NC times per line
+    for (int i = tid; i < prm.M * prm.NC * nq; i += nthr) {
+        const int m = i / (prm.NC * nq), rem = i - m * (prm.NC * nq), piece = rem % nq;
+        *reinterpret_cast<float4*>(sigt_s + (size_t)m * line + rem * 16) = *reinterpret_cast<const float4*>(prm.sigt + (size_t)m * Gs + piece * 4);
+    }
+    __syncthreads();
+
+    // ---- slot geometry ----
+    const int wslot = lane / prm.LS, ll = lane - wslot * prm.LS;
+    const bool lane_ok = wslot < prm.TPW && ll < prm.LPT;
+    const int slot = warp * prm.TPW + (wslot < prm.TPW ? wslot : 0);
+    const int sub = slot % prm.NC;                    // position of the slot inside a shared line
+    const int lane_off = sub * row_bytes + ll * 16;   // byte offset of this lane's 4 groups inside a line
+    const unsigned char* sigt_lane = sigt_s + lane_off;
+    const int d_slot_off = (slot / prm.NC) * prm.Kmax * line + lane_off;
+    const float inv_f = (float)(1.0 / *prm.scale_div);
+    const int g0 = ll * 4;
+    // flush mapping: thread -> (region l0 + i*l_step, 16-byte piece qd)
+    const int f_qd = tid % nq, f_l0 = tid / nq, f_lstep = nthr / nq;
+    const bool f_ok = f_l0 < f_lstep;
+
+    uint32_t seq = 0;   // tiles processed by this block so far: staging buffers and barrier parities follow it
+    for (;;) {
+        if (tid == 0) *s_item = atomicAdd(prm.counter, 1);
+        __syncthreads();
+        const int item = *s_item;
+        if (item >= prm.n_items) break;
+        const int4 it = prm.items[item];
+        const int sw = it.x, dir = it.y;
+        const int64_t tile0 = prm.swath_tile0[sw];
+        const int nt = (int)(prm.swath_tile0[sw + 1] - tile0);
+        // ---- this slot's track: psi enters the registers ----
+        const int t = lane_ok ? prm.swath_track[(size_t)sw * prm.NT + slot] : -1;
+        float psi[P][4], wpt[P];
+        size_t psi_at = 0;
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+            wpt[p] = 0.f;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) psi[p][j] = 0.f;
+        }
+        if (t >= 0) {
+            psi_at = ((size_t)(2 * t + dir) * P) * Gs + g0;
+            const float wt = prm.trk_w[t];
+#pragma unroll
+            for (int p = 0; p < P; ++p) {
+                const float4 v = *reinterpret_cast<const float4*>(prm.psi_in + psi_at + (size_t)p * Gs);
+                psi[p][0] = v.x * inv_f; psi[p][1] = v.y * inv_f; psi[p][2] = v.z * inv_f; psi[p][3] = v.w * inv_f;
+                wpt[p] = wt * prm.wp[p];
+            }
+        }
+        // ---- prologue: chunks of the first two tiles in flight, q rows of the first tile ----
+        auto tile_index = [&](int k) -> int64_t { return tile0 + (dir ? nt - 1 - k : k); };
+        auto issue_chunk = [&](int k) {   // one thread
+            const int64_t ti = tile_index(k);
+            const uint32_t o0 = prm.tile_chunk[ti], o1 = prm.tile_chunk[ti + 1];
+            const uint32_t bytes = (o1 - o0) * 16u;
+            const uint32_t b = (seq + k) % kSwathChunkBufs;
+            mbar_expect_tx(full + b, bytes);
+            tma_load_1d(chunk_s + (size_t)b * prm.chunk_cap, prm.blob + (size_t)o0 * 16, bytes, full + b);
+        };
+        auto wait_chunk = [&](int k) {
+            const uint32_t s = seq + k;
+            mbar_wait(full + (s % kSwathChunkBufs), (s / kSwathChunkBufs) & 1u);
+        };
+        auto issue_q_rows = [&](int k) {   // all threads: regions of tile k -> q buffer (seq+k)&1, NC copies per row
+            const uint32_t s = seq + k;
+            const unsigned char* cb = chunk_s + (size_t)(s % kSwathChunkBufs) * prm.chunk_cap;
+            const uint4 h = *reinterpret_cast<const uint4*>(cb);
+            const int L = (int)(h.x & 0xffffu);
+            const uint32_t* regions = reinterpret_cast<const uint32_t*>(cb + 16 * (h.y & 0xffffu));
+            const uint32_t qb = smem_u32(q_s + (size_t)(s & 1u) * q_buf_bytes);
+            const int per_row = prm.NC * nq;
+            for (int i = tid; i < L * per_row; i += nthr) {
+                const int l = i / per_row, rem = i - l * per_row, piece = rem % nq;
+                cp_async_16(qb + l * line + rem * 16, prm.q + (size_t)regions[l] * Gs + piece * 4);
+            }
+        };
+        if (nt > 0) {
+            if (tid == 0) {
+                issue_chunk(0);
+                if (nt > 1) issue_chunk(1);
+            }
+            wait_chunk(0);
+            issue_q_rows(0);
+            cp_async_commit_group();
+            cp_async_wait_all();
+        }
+        __syncthreads();
+
+        for (int k = 0; k < nt; ++k) {
+            const uint32_t s = seq + k;
+            const unsigned char* cb = chunk_s + (size_t)(s % kSwathChunkBufs) * prm.chunk_cap;
+            // ---- stage ahead: q rows of tile k+1 (its chunk landed a tile ago), chunk of tile k+2 ----
+            if (k + 1 < nt) {
+                wait_chunk(k + 1);
+                issue_q_rows(k + 1);
+            }
+            cp_async_commit_group();
+            if (tid == 0 && k + 2 < nt) issue_chunk(k + 2);
+            if (prm.ndbuf == 1) __syncthreads();   // single delta buffer: the previous tile's flush must be over
+            const SwathChunk ch = decode_chunk(cb);
+            unsigned char* dbuf = dbuf_s + (size_t)(prm.ndbuf == 1 ? 0u : (s & 1u)) * dbuf_bytes;
+            // ---- segment loop of this slot's track through the tile ----
+            {
+                int s0 = 0, cnt = 0;
+                if (t >= 0) { s0 = ch.slot_start[slot]; cnt = ch.slot_start[slot + 1] - s0; }
+                const int steps = __reduce_max_sync(0xffffffffu, cnt);
+                const unsigned char* q_lane = q_s + (size_t)(s & 1u) * q_buf_bytes + lane_off;
+                // segment j (forward index inside the tile) is visited at step i: j = dir ? cnt-1-i : i
+                const int jstep = dir ? -1 : 1;
+                int j_c = dir ? cnt - 1 : 0;                // segment of the current step
+                unsigned char* d_ptr = dbuf + d_slot_off + j_c * line;
+                const int d_step = jstep * line;
+                // software pipeline: record two steps ahead, rows one step ahead
+                uint2 r_n = make_uint2(0u, 0u), r_nn = make_uint2(0u, 0u);
+                if (cnt > 0) r_n = ch.rec[s0 + j_c];
+                if (cnt > 1) r_nn = ch.rec[s0 + j_c + jstep];
+                float4 q_n = *reinterpret_cast<const float4*>(q_lane + (r_n.y & 0xffffu));
+                float4 st_n = *reinterpret_cast<const float4*>(sigt_lane + (r_n.y >> 16));
+                float s_n = __uint_as_float(r_n.x);
+                const uint2* rec_pf = ch.rec + s0 + j_c + 2 * jstep;   // record of step i+2
+                for (int i = 0; i < steps; ++i) {
+                    const float sl = s_n;
+                    const float4 qv = q_n, stv = st_n;
+                    // next step's rows, the step after's record (zero-length no-op records past the end)
+                    const uint2 r_use = r_nn;
+                    r_nn = make_uint2(0u, 0u);
+                    if (i + 2 < cnt) r_nn = *rec_pf;
+                    rec_pf += jstep;
+                    q_n = *reinterpret_cast<const float4*>(q_lane + (r_use.y & 0xffffu));
+                    st_n = *reinterpret_cast<const float4*>(sigt_lane + (r_use.y >> 16));
+                    s_n = __uint_as_float(r_use.x);
+                    float sc[P];
+#pragma unroll
+                    for (int p = 0; p < P; ++p) sc[p] = sl * (EXPM == 0 ? prm.c[p] : -prm.inv_sin[p]);
+                    const float qa[4] = {qv.x, qv.y, qv.z, qv.w}, sa[4] = {stv.x, stv.y, stv.z, stv.w};
+                    float a4[4];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        float acc = 0.f;
+#pragma unroll
+                        for (int p = 0; p < P; ++p) {
+                            const float d = psi[p][j] - qa[j];
+                            float delta;
+                            if (EXPM == 0) delta = fmaf(-d, ex2_approx(sa[j] * sc[p]), d);
+                            else delta = d * (-expm1f(sa[j] * sc[p]));
+                            psi[p][j] -= delta;
+                            acc = fmaf(wpt[p], delta, acc);
+                        }
+                        a4[j] = acc;
+                    }
+                    if (i < cnt) *reinterpret_cast<float4*>(d_ptr) = make_float4(a4[0], a4[1], a4[2], a4[3]);
+                    d_ptr += d_step;
+                }
+            }
+            cp_async_wait_all();   // this thread's q-row copies for tile k+1
+            __syncthreads();
+            // ---- flush: one FP64 RED per (region, group) of the tile ----
+            if (f_ok) {
+                for (int l = f_l0; l < ch.L; l += f_lstep) {
+                    const int e0 = ch.csr_off[l], e1 = ch.csr_off[l + 1];
+                    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+                    for (int e = e0; e < e1; ++e) {
+                        const float4 x = *reinterpret_cast<const float4*>(dbuf + (size_t)ch.csr_idx[e] * row_bytes + f_qd * 16);
+                        v.x += x.x; v.y += x.y; v.z += x.z; v.w += x.w;
+                    }
+                    double* tp = prm.tally + (size_t)ch.regions[l] * Gs + f_qd * 4;
+                    const int gq = f_qd * 4;
+                    atomicAdd(tp, (double)v.x);
+                    if (gq + 1 < prm.G) atomicAdd(tp + 1, (double)v.y);
+                    if (gq + 2 < prm.G) atomicAdd(tp + 2, (double)v.z);
+                    if (gq + 3 < prm.G) atomicAdd(tp + 3, (double)v.w);
+                }
+            }
+        }
+        seq += (uint32_t)nt;
+        // ---- psi leaves the registers ----
+        if (t >= 0) {
+#pragma unroll
+            for (int p = 0; p < P; ++p)
+                *reinterpret_cast<float4*>(prm.psi_out + psi_at + (size_t)p * Gs) = make_float4(psi[p][0], psi[p][1], psi[p][2], psi[p][3]);
+        }
+        __syncthreads();   // s_item may be rewritten; the last flush is over before the next item's staging
+    }
+}
+
+} // namespace ndk

@@ -14,7 +14,8 @@ from gpu_common import Pair, make_pair, seeded_sweep_inputs, phi_rel_err, PHI_RT
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [nd.ND_SWEEP_ATOMIC, nd.ND_SWEEP_PRIVATE]
+KERNELS = [pytest.param(nd.ND_SWEEP_ATOMIC, id="atomic"), pytest.param(nd.ND_SWEEP_PRIVATE, id="private"),
+           pytest.param(nd.ND_SWEEP_SWATH, id="swath")]
 
 # (config index, scale): sizes the oracle finishes in seconds, spanning several tiles and ragged tails
 SWEEP_CASES = [(1, 1.0), (2, 0.15), (2, 1.0), (3, 0.03), (4, 0.06), (5, 0.0008)]

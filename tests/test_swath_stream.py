@@ -1,0 +1,112 @@
+"""Host logic of row A1 (no GPU): the swath/tile chunk stream of ND_SWEEP_SWATH, decoded chunk by chunk.
+
+Checks the format csrc/nd_swath.h documents and the properties the kernel relies on: every segment of the
+descriptor appears exactly once, in track order, with its FP32 length and its q / Sigma_t row offsets; the per-region
+CSR lists every delta-buffer row exactly once; the limits (Kmax, Lmax, chunk capacity) hold; work items cover every
+(swath, direction) once."""
+import numpy as np
+import pytest
+
+import paper_2607_01591_b200 as nd
+from moc_inputs import make_config
+
+
+def _decode_and_check(st, mat, seg_offset, seg_region, seg_length, NT, Kmax, Lmax, NC, row_bytes):
+    blob, tc = st["blob"], st["tile_chunk"].astype(np.int64) * 16
+    line = NC * row_bytes
+    T = len(seg_offset) - 1
+    cursor = seg_offset[:-1].copy()
+    tracks_seen = np.zeros(T, bool)
+    total = 0
+    for sw in range(st["n_swaths"]):
+        trk = st["swath_track"][sw]
+        for b in trk[trk >= 0]:
+            assert not tracks_seen[b]
+            tracks_seen[b] = True
+        for ti in range(st["swath_tile0"][sw], st["swath_tile0"][sw + 1]):
+            c = blob[tc[ti]:tc[ti + 1]]
+            hdr = c[:16].view(np.uint32)
+            L, nseg = int(hdr[0] & 0xffff), int(hdr[0] >> 16)
+            o_rg, o_co = 16 * int(hdr[1] & 0xffff), 16 * int(hdr[1] >> 16)
+            o_ci, o_rc = 16 * int(hdr[2] & 0xffff), 16 * int(hdr[2] >> 16)
+            assert hdr[3] == len(c) and len(c) % 16 == 0 and len(c) <= st["max_chunk_bytes"]
+            assert 1 <= L <= Lmax and 1 <= nseg <= NT * Kmax
+            ss = c[16:16 + 2 * (NT + 1)].view(np.uint16).astype(np.int64)
+            regions = c[o_rg:o_rg + 4 * L].view(np.uint32).astype(np.int64)
+            co = c[o_co:o_co + 2 * (L + 1)].view(np.uint16).astype(np.int64)
+            ci = c[o_ci:o_ci + 2 * nseg].view(np.uint16).astype(np.int64)
+            rec = c[o_rc:o_rc + 8 * nseg].view(np.uint32).reshape(nseg, 2)
+            assert ss[0] == 0 and ss[NT] == nseg and np.all(np.diff(ss) >= 0) and np.all(np.diff(ss) <= Kmax)
+            assert len(np.unique(regions)) == L
+            assert co[0] == 0 and co[L] == nseg and np.all(np.diff(co) >= 1)
+            row_region = {}
+            for l in range(L):
+                for row in ci[co[l]:co[l + 1]]:
+                    assert row not in row_region
+                    row_region[int(row)] = regions[l]
+            for b in range(NT):
+                n = ss[b + 1] - ss[b]
+                if trk[b] < 0:
+                    assert n == 0
+                    continue
+                k0 = cursor[trk[b]]
+                assert k0 + n <= seg_offset[trk[b] + 1]
+                for j in range(n):
+                    r = seg_region[k0 + j]
+                    lenbits, w = rec[ss[b] + j]
+                    assert np.uint32(lenbits).view(np.float32) == np.float32(seg_length[k0 + j])
+                    l = int(w & 0xffff) // line
+                    assert (w & 0xffff) % line == 0 and regions[l] == r
+                    assert int(w >> 16) == mat[r] * line
+                    row = ((b // NC) * Kmax + j) * NC + b % NC
+                    assert row_region[row] == r
+                cursor[trk[b]] += n
+            total += nseg
+    assert tracks_seen.all()
+    assert np.array_equal(cursor, seg_offset[1:]), "every segment exactly once, in order"
+    assert total == seg_offset[-1]
+    items = st["items"]
+    assert len(items) == 2 * st["n_swaths"]
+    assert sorted(map(tuple, items[:, :2])) == sorted((s, d) for s in range(st["n_swaths"]) for d in (0, 1))
+    assert np.all(np.diff(items[:, 2]) <= 0), "most expensive first"
+
+
+@pytest.mark.parametrize("NT,Kmax,Lmax,NC,row_bytes", [(16, 16, 64, 1, 208), (64, 8, 96, 4, 32), (24, 16, 92, 1, 144), (3, 2, 4, 1, 16)])
+def test_stream_of_a_traced_problem(NT, Kmax, Lmax, NC, row_bytes):
+    prob = make_config(2, scale=0.12)
+    m = prob.mesh
+    tr = nd.nd_tracks_generate(m.xy, m.tri, m.W, m.H, prob.bc, prob.n_azim, prob.spacing)
+    st = nd.nd_swath_stream_build(m.material, prob.xs.sigma_t.shape[0], tr.seg_offset, tr.seg_region, tr.seg_length,
+                                  NT, Kmax, Lmax, NC, row_bytes, tr.track_azim, tr.ends)
+    _decode_and_check(st, m.material, tr.seg_offset, tr.seg_region, tr.seg_length, NT, Kmax, Lmax, NC, row_bytes)
+    assert 0.3 < st["lockstep_efficiency"] <= 1.0
+    # swaths hold tracks of ONE angle, adjacent in the perpendicular coordinate
+    for trk in st["swath_track"]:
+        t = trk[trk >= 0]
+        assert len(set(tr.track_azim[t])) == 1
+    tr.destroy()
+
+
+def test_stream_without_geometry_and_with_degenerate_tracks():
+    rng = np.random.default_rng(4)
+    R, T = 5, 23
+    counts = rng.integers(0, 40, size=T)
+    counts[[0, 7, 22]] = 0
+    off = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    seg_region = rng.integers(0, R, size=off[-1]).astype(np.int32)      # a track may re-enter a region
+    seg_length = rng.uniform(1e-3, 1.0, size=off[-1])
+    mat = rng.integers(0, 3, size=R).astype(np.int32)
+    for NT, Kmax, Lmax, NC in [(8, 4, 3, 1), (8, 16, 5, 4), (1, 1, 1, 1)]:
+        st = nd.nd_swath_stream_build(mat, 3, off, seg_region, seg_length, NT, Kmax, Lmax, NC, 32)
+        _decode_and_check(st, mat, off, seg_region, seg_length, NT, Kmax, Lmax, NC, 32)
+
+
+def test_stream_rejects_bad_parameters():
+    off = np.array([0, 2], np.int64)
+    args = (np.zeros(1, np.int32), 1, off, np.zeros(2, np.int32), np.ones(2))
+    with pytest.raises(nd.NdError, match="ND_ERR_INVALID"):
+        nd.nd_swath_stream_build(*args, 6, 4, 4, 4, 32)        # NT % NC != 0
+    with pytest.raises(nd.NdError, match="ND_ERR_INVALID"):
+        nd.nd_swath_stream_build(*args, 8, 4, 4000, 1, 208)    # row offsets exceed 16 bits
+    with pytest.raises(nd.NdError, match="ND_ERR_INVALID"):
+        nd.nd_swath_stream_build(*args, 8, 4, 4, 1, 20)        # row_bytes not a multiple of 16
