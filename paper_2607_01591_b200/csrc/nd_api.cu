@@ -396,7 +396,14 @@ nd_status launch_swath(nd_problem* p, const double* scale_div, cudaStream_t st)
     prm.n_items = p->n_items; prm.G = d.G; prm.Gs = d.Gs; prm.M = d.M; prm.NT = c.sp.NT; prm.Kmax = c.sp.Kmax; prm.Lmax = c.sp.Lmax;
     prm.LPT = c.LPT; prm.LS = c.LS; prm.TPW = c.TPW; prm.NC = c.sp.NC; prm.ndbuf = c.ndbuf; prm.chunk_cap = c.chunk_cap;
     prm.off_sigt = c.off_sigt; prm.off_q = c.off_q; prm.off_dbuf = c.off_dbuf; prm.off_chunk = c.off_chunk;
-    for (int i = 0; i < ndk::kMaxPolar; ++i) { prm.c[i] = p->c[i]; prm.inv_sin[i] = p->inv_sin[i]; prm.wp[i] = p->wp[i]; }
+    for (int i = 0; i < ndk::kMaxPolar; ++i) {
+        prm.c[i] = p->c[i]; prm.inv_sin[i] = p->inv_sin[i]; prm.wp[i] = p->wp[i];
+        uint32_t bits;
+        memcpy(&bits, &p->c[i], 4);
+        prm.c2[i] = (unsigned long long)bits | ((unsigned long long)bits << 32);
+    }
+    prm.magic_per_row = ndk::fastdiv_magic((uint32_t)(c.sp.NC * (d.Gs / 4)));
+    prm.magic_nq = ndk::fastdiv_magic((uint32_t)(d.Gs / 4));
     ND_CUDA(cudaMemsetAsync(p->counter, 0, sizeof(int), st));
     switch (d.P) {
     case 1: return launch_swath_p<1>(p, prm, st);

@@ -96,7 +96,8 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
             std::vector<double> lam(NT);
             std::vector<int> cnt(NT);
             std::vector<uint32_t> regions;
-            std::vector<int> rcount, rfill;
+            std::vector<int> rcount, rfill, perm, sorted_count;
+            std::vector<uint32_t> sorted_regions;
             regions.reserve(Lmax);
 #pragma omp for schedule(dynamic, 4)
             for (int64_t sw = 0; sw < n_sw; ++sw) {
@@ -135,6 +136,14 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
                     }
                     // ---- encode ----
                     const int L = (int)regions.size();
+                    {   // regions in descending order of their segment count: flush threads of a warp get lists of similar length
+                        perm.resize(L);
+                        std::iota(perm.begin(), perm.end(), 0);
+                        std::stable_sort(perm.begin(), perm.end(), [&](int a, int b) { return rcount[a] > rcount[b]; });
+                        sorted_regions.resize(L); sorted_count.resize(L);
+                        for (int l = 0; l < L; ++l) { sorted_regions[l] = regions[perm[l]]; sorted_count[l] = rcount[perm[l]]; lidx[regions[perm[l]]] = l; }
+                        regions.swap(sorted_regions); rcount.swap(sorted_count);
+                    }
                     const int o_ss = 16;
                     const int o_rg = o_ss + nd_swath_pad16(2 * (NT + 1));
                     const int o_co = o_rg + nd_swath_pad16(4 * L);

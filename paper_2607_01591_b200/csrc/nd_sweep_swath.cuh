@@ -46,6 +46,8 @@ struct SwathParams {
     int chunk_cap;                             // bytes of one chunk staging buffer
     int off_sigt, off_q, off_dbuf, off_chunk;  // shared-memory byte offsets
     float c[kMaxPolar], inv_sin[kMaxPolar], wp[kMaxPolar];
+    unsigned long long c2[kMaxPolar];          // {c[p], c[p]} packed for the FP32x2 path
+    uint32_t magic_per_row, magic_nq;          // fastdiv constants of NC*Gs/4 and Gs/4
 };
 
 constexpr int kSwathChunkBufs = 4;
@@ -105,6 +107,113 @@ __device__ __forceinline__ SwathChunk decode_chunk(const unsigned char* cb)
     c.csr_idx = reinterpret_cast<const uint16_t*>(cb + 16 * (h.z & 0xffffu));
     c.rec = reinterpret_cast<const uint2*>(cb + 16 * (h.z >> 16));
     return c;
+}
+
+// ---- packed FP32x2 arithmetic (sm_100: FFMA2 / FADD2 / FMUL2 halve the issue slots of the FP32 work) ----
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void upk2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+
+// x / d for x < 2^16 and d >= 1, with m = fastdiv_magic(d); m == 0 encodes d == 1
+__host__ __device__ inline uint32_t fastdiv_magic(uint32_t d) { return d <= 1 ? 0u : (uint32_t)((0x100000000ull + d - 1) / d); }
+__device__ __forceinline__ uint32_t fastdiv(uint32_t x, uint32_t m) { return m ? __umulhi(x, m) : x; }
+
+// One track through one tile: cnt segments starting at record rec0 (stepping jstep = +-1), `steps` >= cnt loop trips
+// (slots of a warp run in lock step; trips past cnt are exact no-ops: zero length -> exp = 1 -> Delta = 0).
+// Software pipeline: the record of step i+2 and the q / Sigma_t rows of step i+1 are loaded during step i.
+template <int P, int EXPM>
+__device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&wpt)[P], const SwathParams& prm, const uint2* rec0,
+                                             int jstep, int cnt, int steps, const unsigned char* q_lane,
+                                             const unsigned char* sigt_lane, unsigned char* d_ptr, int d_step)
+{
+    uint2 r_n = make_uint2(0u, 0u), r_nn = make_uint2(0u, 0u);
+    if (cnt > 0) r_n = rec0[0];
+    if (cnt > 1) r_nn = rec0[jstep];
+    const uint2* rec_pf = rec0 + 2 * jstep;   // record of step i+2
+    if (EXPM == 0) {
+        f32x2 ps[P][2], w2[P];
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+            ps[p][0] = pk2(psi[p][0], psi[p][1]);
+            ps[p][1] = pk2(psi[p][2], psi[p][3]);
+            w2[p] = pk2(wpt[p], wpt[p]);
+        }
+        ulonglong2 q_n = *reinterpret_cast<const ulonglong2*>(q_lane + (r_n.y & 0xffffu));
+        ulonglong2 st_n = *reinterpret_cast<const ulonglong2*>(sigt_lane + (r_n.y >> 16));
+        float s_n = __uint_as_float(r_n.x);
+        for (int i = 0; i < steps; ++i) {
+            const f32x2 s2 = pk2(s_n, s_n);
+            const f32x2 qa[2] = {q_n.x, q_n.y};
+            const f32x2 ts[2] = {mul2(st_n.x, s2), mul2(st_n.y, s2)};
+            const uint2 r_use = r_nn;
+            r_nn = make_uint2(0u, 0u);
+            if (i + 2 < cnt) r_nn = *rec_pf;
+            rec_pf += jstep;
+            q_n = *reinterpret_cast<const ulonglong2*>(q_lane + (r_use.y & 0xffffu));
+            st_n = *reinterpret_cast<const ulonglong2*>(sigt_lane + (r_use.y >> 16));
+            s_n = __uint_as_float(r_use.x);
+            f32x2 acc[2];
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const f32x2 tau = mul2(ts[j], prm.c2[p]);
+                    float t0, t1;
+                    upk2(tau, t0, t1);
+                    const f32x2 a = pk2(ex2_approx(t0), ex2_approx(t1));
+                    const f32x2 d = sub2(ps[p][j], qa[j]);
+                    const f32x2 delta = sub2(d, mul2(d, a));      // d*(1-a); contracts to one FFMA2
+                    ps[p][j] = sub2(ps[p][j], delta);
+                    acc[j] = p == 0 ? mul2(w2[0], delta) : fma2(w2[p], delta, acc[j]);
+                }
+            }
+            if (i < cnt) {
+                ulonglong2 o;
+                o.x = acc[0]; o.y = acc[1];
+                *reinterpret_cast<ulonglong2*>(d_ptr) = o;
+            }
+            d_ptr += d_step;
+        }
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+            upk2(ps[p][0], psi[p][0], psi[p][1]);
+            upk2(ps[p][1], psi[p][2], psi[p][3]);
+        }
+    } else {
+        float4 q_n = *reinterpret_cast<const float4*>(q_lane + (r_n.y & 0xffffu));
+        float4 st_n = *reinterpret_cast<const float4*>(sigt_lane + (r_n.y >> 16));
+        float s_n = __uint_as_float(r_n.x);
+        for (int i = 0; i < steps; ++i) {
+            const float sl = s_n;
+            const float4 qv = q_n, stv = st_n;
+            const uint2 r_use = r_nn;
+            r_nn = make_uint2(0u, 0u);
+            if (i + 2 < cnt) r_nn = *rec_pf;
+            rec_pf += jstep;
+            q_n = *reinterpret_cast<const float4*>(q_lane + (r_use.y & 0xffffu));
+            st_n = *reinterpret_cast<const float4*>(sigt_lane + (r_use.y >> 16));
+            s_n = __uint_as_float(r_use.x);
+            const float qa[4] = {qv.x, qv.y, qv.z, qv.w}, sa[4] = {stv.x, stv.y, stv.z, stv.w};
+            float a4[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                float acc = 0.f;
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const float d = psi[p][j] - qa[j];
+                    const float delta = d * (-expm1f(-(sa[j] * sl) * prm.inv_sin[p]));
+                    psi[p][j] -= delta;
+                    acc = fmaf(wpt[p], delta, acc);
+                }
+                a4[j] = acc;
+            }
+            if (i < cnt) *reinterpret_cast<float4*>(d_ptr) = make_float4(a4[0], a4[1], a4[2], a4[3]);
+            d_ptr += d_step;
+        }
+    }
 }
 
 template <int P, int EXPM>
@@ -203,7 +312,8 @@ __global__ void __launch_bounds__(512, 1) k_sweep_swath(const SwathParams prm)
             const uint32_t qb = smem_u32(q_s + (size_t)(s & 1u) * q_buf_bytes);
             const int per_row = prm.NC * nq;
             for (int i = tid; i < L * per_row; i += nthr) {
-                const int l = i / per_row, rem = i - l * per_row, piece = rem % nq;
+                const int l = (int)fastdiv((uint32_t)i, prm.magic_per_row), rem = i - l * per_row;
+                const int piece = rem - (int)fastdiv((uint32_t)rem, prm.magic_nq) * nq;
                 cp_async_16(qb + l * line + rem * 16, prm.q + (size_t)regions[l] * Gs + piece * 4);
             }
         };
@@ -243,47 +353,7 @@ __global__ void __launch_bounds__(512, 1) k_sweep_swath(const SwathParams prm)
                 int j_c = dir ? cnt - 1 : 0;                // segment of the current step
                 unsigned char* d_ptr = dbuf + d_slot_off + j_c * line;
                 const int d_step = jstep * line;
-                // software pipeline: record two steps ahead, rows one step ahead
-                uint2 r_n = make_uint2(0u, 0u), r_nn = make_uint2(0u, 0u);
-                if (cnt > 0) r_n = ch.rec[s0 + j_c];
-                if (cnt > 1) r_nn = ch.rec[s0 + j_c + jstep];
-                float4 q_n = *reinterpret_cast<const float4*>(q_lane + (r_n.y & 0xffffu));
-                float4 st_n = *reinterpret_cast<const float4*>(sigt_lane + (r_n.y >> 16));
-                float s_n = __uint_as_float(r_n.x);
-                const uint2* rec_pf = ch.rec + s0 + j_c + 2 * jstep;   // record of step i+2
-                for (int i = 0; i < steps; ++i) {
-                    const float sl = s_n;
-                    const float4 qv = q_n, stv = st_n;
-                    // next step's rows, the step after's record (zero-length no-op records past the end)
-                    const uint2 r_use = r_nn;
-                    r_nn = make_uint2(0u, 0u);
-                    if (i + 2 < cnt) r_nn = *rec_pf;
-                    rec_pf += jstep;
-                    q_n = *reinterpret_cast<const float4*>(q_lane + (r_use.y & 0xffffu));
-                    st_n = *reinterpret_cast<const float4*>(sigt_lane + (r_use.y >> 16));
-                    s_n = __uint_as_float(r_use.x);
-                    float sc[P];
-#pragma unroll
-                    for (int p = 0; p < P; ++p) sc[p] = sl * (EXPM == 0 ? prm.c[p] : -prm.inv_sin[p]);
-                    const float qa[4] = {qv.x, qv.y, qv.z, qv.w}, sa[4] = {stv.x, stv.y, stv.z, stv.w};
-                    float a4[4];
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        float acc = 0.f;
-#pragma unroll
-                        for (int p = 0; p < P; ++p) {
-                            const float d = psi[p][j] - qa[j];
-                            float delta;
-                            if (EXPM == 0) delta = fmaf(-d, ex2_approx(sa[j] * sc[p]), d);
-                            else delta = d * (-expm1f(sa[j] * sc[p]));
-                            psi[p][j] -= delta;
-                            acc = fmaf(wpt[p], delta, acc);
-                        }
-                        a4[j] = acc;
-                    }
-                    if (i < cnt) *reinterpret_cast<float4*>(d_ptr) = make_float4(a4[0], a4[1], a4[2], a4[3]);
-                    d_ptr += d_step;
-                }
+                segment_loop<P, EXPM>(psi, wpt, prm, ch.rec + s0 + j_c, jstep, cnt, steps, q_lane, sigt_lane, d_ptr, d_step);
             }
             cp_async_wait_all();   // this thread's q-row copies for tile k+1
             __syncthreads();
