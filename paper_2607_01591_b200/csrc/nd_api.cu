@@ -116,7 +116,7 @@ PrivConfig make_priv_config(const Dims& d, const nd_options& opt)
 struct SwathConfig {
     bool feasible = false;
     NdSwathParams sp{};
-    int LPT = 0, LS = 0, TPW = 0, warps = 0, ndbuf = 1, blocks_per_sm = 1;
+    int LPT = 0, warps = 0, ndbuf = 1, blocks_per_sm = 1;
     int chunk_cap = 0, off_sigt = 0, off_q = 0, off_dbuf = 0, off_chunk = 0, smem_bytes = 0;
     int64_t max_tiles = 0, max_swaths = 0;
     size_t max_blob = 0;
@@ -127,12 +127,10 @@ SwathConfig make_swath_config(const Dims& d, const nd_options& opt)
     SwathConfig c;
     c.LPT = d.Gs / 4;
     if (c.LPT > 32) return c;
-    c.TPW = 32 / c.LPT;
-    c.LS = (c.TPW == 2) ? 16 : c.LPT;                     // two slots per warp sit on 16-lane boundaries: a shared-memory phase never mixes rows
     const int NC = (c.LPT == 1 || c.LPT == 2 || c.LPT == 4) ? 8 / c.LPT : 1;
     const int row_bytes = 4 * d.Gs, line = NC * row_bytes;
     if ((int64_t)d.M * line > 65536) return c;
-    int warps = opt.block_warps > 0 ? opt.block_warps : (c.TPW <= 3 ? 8 : 4);
+    int warps = opt.block_warps > 0 ? opt.block_warps : (c.LPT > 8 ? 8 : 4);
     if (warps > 16) warps = 16;
     int Kmax = opt.tile_segments > 0 ? opt.tile_segments : (row_bytes >= 64 ? 16 : 8);
     int Lmax = opt.window_regions > 0 ? opt.window_regions : 13312 / line;
@@ -142,8 +140,8 @@ SwathConfig make_swath_config(const Dims& d, const nd_options& opt)
     auto pad128 = [](int x) { return (x + 127) / 128 * 128; };
     for (;; --warps) {                                    // shrink the block until it fits the 227 KB of an SM
         if (warps < 1) return c;
-        const int NT = warps * c.TPW;
-        if ((int64_t)NT * Kmax > 65535) continue;
+        const int NT = warps * 32 / c.LPT / NC * NC;        // slots are packed over the lanes of the whole block
+        if (NT < 1 || (int64_t)NT * Kmax > 65535) continue;
         c.sp.NT = NT; c.sp.Kmax = Kmax; c.sp.Lmax = Lmax; c.sp.NC = NC; c.sp.row_bytes = row_bytes;
         c.chunk_cap = nd_swath_chunk_capacity(c.sp);
         c.off_sigt = 128;
@@ -394,7 +392,7 @@ nd_status launch_swath(nd_problem* p, const double* scale_div, cudaStream_t st)
     prm.items = p->items; prm.counter = p->counter; prm.q = p->q; prm.sigt = p->sigt_f; prm.tally = p->tally; prm.trk_w = p->trk_w;
     prm.psi_in = p->psi_in; prm.psi_out = p->psi_out; prm.scale_div = scale_div;
     prm.n_items = p->n_items; prm.G = d.G; prm.Gs = d.Gs; prm.M = d.M; prm.NT = c.sp.NT; prm.Kmax = c.sp.Kmax; prm.Lmax = c.sp.Lmax;
-    prm.LPT = c.LPT; prm.LS = c.LS; prm.TPW = c.TPW; prm.NC = c.sp.NC; prm.ndbuf = c.ndbuf; prm.chunk_cap = c.chunk_cap;
+    prm.LPT = c.LPT; prm.NC = c.sp.NC; prm.ndbuf = c.ndbuf; prm.chunk_cap = c.chunk_cap;
     prm.off_sigt = c.off_sigt; prm.off_q = c.off_q; prm.off_dbuf = c.off_dbuf; prm.off_chunk = c.off_chunk;
     for (int i = 0; i < ndk::kMaxPolar; ++i) {
         prm.c[i] = p->c[i]; prm.inv_sin[i] = p->inv_sin[i]; prm.wp[i] = p->wp[i];

@@ -11,7 +11,8 @@
 // Mapping
 //   * thread block = one SWATH (NT adjacent tracks of one angle) in one direction; persistent blocks pull
 //     (swath, direction) items from an atomic counter, most expensive first.
-//   * lane group ("slot") = LPT lanes = one track; a lane owns 4 consecutive groups x P polar angles = 4P
+//   * lane group ("slot") = LPT lanes = one track, slots packed over the lanes of the whole block (19 slots of 13 lanes in
+//     256 threads for G = 51: 96 % of the lanes carry chains); a lane owns 4 consecutive groups x P polar angles = 4P
 //     independent Eq.-(5) chains in registers (ILP hides the MUFU/FMA latency).  psi is read from the boundary
 //     array once, at the track's entry, and written once, at its exit.
 //   * the swath is processed tile by tile (nd_swath.h).  A tile's chunk arrives by ONE bulk async (TMA) copy,
@@ -42,7 +43,7 @@ struct SwathParams {
     const float* __restrict__ psi_in;
     float* __restrict__ psi_out;
     const double* __restrict__ scale_div;
-    int n_items, G, Gs, M, NT, Kmax, Lmax, LPT, LS, TPW, NC, ndbuf;
+    int n_items, G, Gs, M, NT, Kmax, Lmax, LPT, NC, ndbuf;
     int chunk_cap;                             // bytes of one chunk staging buffer
     int off_sigt, off_q, off_dbuf, off_chunk;  // shared-memory byte offsets
     float c[kMaxPolar], inv_sin[kMaxPolar], wp[kMaxPolar];
@@ -126,7 +127,7 @@ __device__ __forceinline__ uint32_t fastdiv(uint32_t x, uint32_t m) { return m ?
 // Software pipeline: the record of step i+2 and the q / Sigma_t rows of step i+1 are loaded during step i.
 template <int P, int EXPM>
 __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&wpt)[P], const SwathParams& prm, const uint2* rec0,
-                                             int jstep, int cnt, int steps, const unsigned char* q_lane,
+                                             int jstep, int cnt, int steps, bool store_ok, const unsigned char* q_lane,
                                              const unsigned char* sigt_lane, unsigned char* d_ptr, int d_step)
 {
     uint2 r_n = make_uint2(0u, 0u), r_nn = make_uint2(0u, 0u);
@@ -170,7 +171,7 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
                     acc[j] = p == 0 ? mul2(w2[0], delta) : fma2(w2[p], delta, acc[j]);
                 }
             }
-            if (i < cnt) {
+            if (i < cnt && store_ok) {
                 ulonglong2 o;
                 o.x = acc[0]; o.y = acc[1];
                 *reinterpret_cast<ulonglong2*>(d_ptr) = o;
@@ -210,7 +211,7 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
                 }
                 a4[j] = acc;
             }
-            if (i < cnt) *reinterpret_cast<float4*>(d_ptr) = make_float4(a4[0], a4[1], a4[2], a4[3]);
+            if (i < cnt && store_ok) *reinterpret_cast<float4*>(d_ptr) = make_float4(a4[0], a4[1], a4[2], a4[3]);
             d_ptr += d_step;
         }
     }
@@ -246,9 +247,13 @@ __global__ void __launch_bounds__(512, 1) k_sweep_swath(const SwathParams prm)
     __syncthreads();
 
     // ---- slot geometry ----
-    const int wslot = lane / prm.LS, ll = lane - wslot * prm.LS;
-    const bool lane_ok = wslot < prm.TPW && ll < prm.LPT;
-    const int slot = warp * prm.TPW + (wslot < prm.TPW ? wslot : 0);
+    // Slots are packed over the lanes of the whole BLOCK (slot = tid / LPT), so a slot may straddle two warps: lanes only
+    // share read-only records, and every lane runs its warp's maximum trip count with its own slot's segment count.
+    // Lanes beyond the last slot are SHADOWS of the last slot's last lane: same shared-memory addresses (a broadcast,
+    // no extra bank conflict), no stores.
+    int slot = tid / prm.LPT, ll = tid - slot * prm.LPT;
+    const bool lane_ok = slot < prm.NT;
+    if (!lane_ok) { slot = prm.NT - 1; ll = prm.LPT - 1; }
     const int sub = slot % prm.NC;                    // position of the slot inside a shared line
     const int lane_off = sub * row_bytes + ll * 16;   // byte offset of this lane's 4 groups inside a line
     const unsigned char* sigt_lane = sigt_s + lane_off;
@@ -270,7 +275,7 @@ __global__ void __launch_bounds__(512, 1) k_sweep_swath(const SwathParams prm)
         const int64_t tile0 = prm.swath_tile0[sw];
         const int nt = (int)(prm.swath_tile0[sw + 1] - tile0);
         // ---- this slot's track: psi enters the registers ----
-        const int t = lane_ok ? prm.swath_track[(size_t)sw * prm.NT + slot] : -1;
+        const int t = prm.swath_track[(size_t)sw * prm.NT + slot];
         float psi[P][4], wpt[P];
         size_t psi_at = 0;
 #pragma unroll
@@ -353,7 +358,7 @@ __global__ void __launch_bounds__(512, 1) k_sweep_swath(const SwathParams prm)
                 int j_c = dir ? cnt - 1 : 0;                // segment of the current step
                 unsigned char* d_ptr = dbuf + d_slot_off + j_c * line;
                 const int d_step = jstep * line;
-                segment_loop<P, EXPM>(psi, wpt, prm, ch.rec + s0 + j_c, jstep, cnt, steps, q_lane, sigt_lane, d_ptr, d_step);
+                segment_loop<P, EXPM>(psi, wpt, prm, ch.rec + s0 + j_c, jstep, cnt, steps, lane_ok, q_lane, sigt_lane, d_ptr, d_step);
             }
             cp_async_wait_all();   // this thread's q-row copies for tile k+1
             __syncthreads();
@@ -377,7 +382,7 @@ __global__ void __launch_bounds__(512, 1) k_sweep_swath(const SwathParams prm)
         }
         seq += (uint32_t)nt;
         // ---- psi leaves the registers ----
-        if (t >= 0) {
+        if (t >= 0 && lane_ok) {
 #pragma unroll
             for (int p = 0; p < P; ++p)
                 *reinterpret_cast<float4*>(prm.psi_out + psi_at + (size_t)p * Gs) = make_float4(psi[p][0], psi[p][1], psi[p][2], psi[p][3]);
