@@ -81,7 +81,9 @@ typedef struct {
     int32_t tile_segments;  /* ND_SWEEP_SWATH: max segments of one track per tile; 0 = default */
     int32_t delta_buffers;  /* ND_SWEEP_SWATH: 1 or 2 delta buffers (2 saves one block barrier per tile); 0 = default */
     int32_t blocks_per_sm;  /* ND_SWEEP_SWATH: resident blocks per SM the grid is sized for; 0 = default */
-    int32_t reserved[8];    /* must be 0 */
+    int32_t tile_lag;       /* ND_SWEEP_SWATH: drift of the track fronts (in mean segment lengths) under which a tile gives
+                               every track the same number of segments; 0 = default, -1 = always cut geometrically */
+    int32_t reserved[7];    /* must be 0 */
 } nd_options;
 
 /* ------------------------------------------------------------------------------------------------
@@ -225,7 +227,9 @@ nd_status nd_problem_info_get(const nd_problem* p, nd_problem_info* out);
  * Diagnostics: the swath/tile chunk stream of ND_SWEEP_SWATH (row A1: "segment stream layout"), built on the
  * HOST exactly as nd_problem_create builds it, for inspection by tests.  Chunk format: csrc/nd_swath.h.
  *   tracks_per_swath NT, tile_segments Kmax (per track and tile), window_regions Lmax (distinct regions per
- *   tile), slots_per_line NC (NT % NC == 0), row_bytes = 4 * padded group count (multiple of 16).
+ *   tile), slots_per_line NC (NT % NC == 0), row_bytes = 4 * padded group count (multiple of 16), lag_segments =
+ *   allowed drift of the track fronts, in mean segment lengths, under which tiles give every track equal counts
+ *   (< 0: always cut geometrically).
  * All view pointers are HOST memory owned by the stream object, valid until nd_swath_stream_destroy.
  * ---------------------------------------------------------------------------------------------- */
 typedef struct nd_swath_stream nd_swath_stream;
@@ -241,7 +245,7 @@ typedef struct {
 } nd_swath_stream_view_t;
 nd_status nd_swath_stream_build(const nd_problem_desc* desc, int32_t tracks_per_swath, int32_t tile_segments,
                                 int32_t window_regions, int32_t slots_per_line, int32_t row_bytes,
-                                nd_swath_stream** out);
+                                double lag_segments, nd_swath_stream** out);
 nd_status nd_swath_stream_view(const nd_swath_stream* s, nd_swath_stream_view_t* view);
 nd_status nd_swath_stream_destroy(nd_swath_stream* s);
 

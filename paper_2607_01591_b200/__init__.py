@@ -40,7 +40,7 @@ class NdError(RuntimeError):
 class nd_options(C.Structure):
     _fields_ = [("exp_mode", C.c_int32), ("sweep_kernel", C.c_int32), ("track_batch", C.c_int32),
                 ("window_regions", C.c_int32), ("block_warps", C.c_int32), ("tile_segments", C.c_int32),
-                ("delta_buffers", C.c_int32), ("blocks_per_sm", C.c_int32), ("reserved", C.c_int32 * 8)]
+                ("delta_buffers", C.c_int32), ("blocks_per_sm", C.c_int32), ("tile_lag", C.c_int32), ("reserved", C.c_int32 * 7)]
 
 
 class nd_mesh_desc(C.Structure):
@@ -127,7 +127,7 @@ def lib():
         L.nd_profile_read.argtypes = [C.c_void_p, C.POINTER(nd_profile)]
         L.nd_problem_info_get.argtypes = [C.c_void_p, C.POINTER(nd_problem_info)]
         L.nd_swath_stream_build.argtypes = [C.POINTER(nd_problem_desc), C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
-                                            C.POINTER(C.c_void_p)]
+                                            C.c_double, C.POINTER(C.c_void_p)]
         L.nd_swath_stream_view.argtypes = [C.c_void_p, C.POINTER(nd_swath_stream_view_t)]
         L.nd_swath_stream_destroy.argtypes = [C.c_void_p]
         _lib = L
@@ -206,7 +206,7 @@ class Problem:
     def __init__(self, region_material, sigma_t, sigma_s, nu_sigma_f, chi, polar_sin, polar_weight, seg_offset,
                  seg_region, seg_length, track_weight, link, track_azim=None, track_ends=None, exp_mode=ND_EXP_FAST,
                  sweep_kernel=ND_SWEEP_AUTO, track_batch=0, window_regions=0, block_warps=0, tile_segments=0,
-                 delta_buffers=0, blocks_per_sm=0, device="cuda:0"):
+                 delta_buffers=0, blocks_per_sm=0, tile_lag=0, device="cuda:0"):
         import torch
         self.torch = torch
         self.device = torch.device(device)
@@ -226,7 +226,7 @@ class Problem:
         d = nd_problem_desc(self.R, self.M, self.G, self.P, self.T, *[keep[k].ctypes.data for k in
                             ("rm", "st", "ss", "nf", "ch", "ps", "pw", "so", "sr", "sl", "tw", "lk")], *geo)
         opt = nd_options(int(exp_mode), int(sweep_kernel), int(track_batch), int(window_regions), int(block_warps),
-                         int(tile_segments), int(delta_buffers), int(blocks_per_sm))
+                         int(tile_segments), int(delta_buffers), int(blocks_per_sm), int(tile_lag))
         nbytes = C.c_size_t()
         _check(lib().nd_workspace_bytes(C.byref(d), C.byref(opt), C.byref(nbytes)), "nd_workspace_bytes")
         self.workspace_bytes = int(nbytes.value)
@@ -336,7 +336,8 @@ class Problem:
 
 
 def nd_swath_stream_build(region_material, n_materials, seg_offset, seg_region, seg_length, tracks_per_swath,
-                          tile_segments, window_regions, slots_per_line, row_bytes, track_azim=None, track_ends=None):
+                          tile_segments, window_regions, slots_per_line, row_bytes, track_azim=None, track_ends=None,
+                          lag_segments=-1.0):
     """Diagnostics (HOST only, no GPU): the swath/tile chunk stream of ND_SWEEP_SWATH as numpy copies.
     Returns a dict with blob (uint8), tile_chunk, swath_tile0, swath_track [n_swaths][NT], items [n][4] and stats."""
     keep = dict(rm=np.ascontiguousarray(region_material, np.int32), so=np.ascontiguousarray(seg_offset, np.int64),
@@ -351,7 +352,8 @@ def nd_swath_stream_build(region_material, n_materials, seg_offset, seg_region, 
         d.track_azim, d.track_ends = keep["ta"].ctypes.data, keep["te"].ctypes.data
     h = C.c_void_p()
     _check(lib().nd_swath_stream_build(C.byref(d), int(tracks_per_swath), int(tile_segments), int(window_regions),
-                                       int(slots_per_line), int(row_bytes), C.byref(h)), "nd_swath_stream_build")
+                                       int(slots_per_line), int(row_bytes), float(lag_segments), C.byref(h)),
+               "nd_swath_stream_build")
     try:
         v = nd_swath_stream_view_t()
         _check(lib().nd_swath_stream_view(h, C.byref(v)), "nd_swath_stream_view")

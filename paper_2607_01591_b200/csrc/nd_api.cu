@@ -143,6 +143,9 @@ SwathConfig make_swath_config(const Dims& d, const nd_options& opt)
         const int NT = warps * 32 / c.LPT / NC * NC;        // slots are packed over the lanes of the whole block
         if (NT < 1 || (int64_t)NT * Kmax > 65535) continue;
         c.sp.NT = NT; c.sp.Kmax = Kmax; c.sp.Lmax = Lmax; c.sp.NC = NC; c.sp.row_bytes = row_bytes;
+        // narrow rows (G <= 16): the flush is cheap, idle slot steps are not -> equal-count tiles while the fronts stay within
+        // 16 segments; wide rows: always geometric (the tally re-use rho pays more than level counts), measured in profiles/
+        c.sp.lag = opt.tile_lag < 0 ? -1.0 : (opt.tile_lag > 0 ? (double)opt.tile_lag : (row_bytes < 64 ? 16.0 : -1.0));
         c.chunk_cap = nd_swath_chunk_capacity(c.sp);
         c.off_sigt = 128;
         c.off_q = c.off_sigt + pad128(d.M * line);
@@ -531,12 +534,12 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     if (rc != ND_OK) return rc;
     nd_options opt{};
     if (opts) opt = *opts;
-    for (int i = 0; i < 8; ++i)
+    for (int i = 0; i < 7; ++i)
         if (opt.reserved[i] != 0) return nd_fail(ND_ERR_INVALID, "nd_options.reserved must be zero");
     if (opt.exp_mode != ND_EXP_FAST && opt.exp_mode != ND_EXP_EXPM1) return nd_fail(ND_ERR_INVALID, "unknown exp_mode");
     if (opt.sweep_kernel < ND_SWEEP_AUTO || opt.sweep_kernel > ND_SWEEP_SWATH) return nd_fail(ND_ERR_INVALID, "unknown sweep_kernel");
     if (opt.track_batch < 0 || opt.window_regions < 0 || opt.block_warps < 0 || opt.tile_segments < 0 || opt.delta_buffers < 0 ||
-        opt.delta_buffers > 2 || opt.blocks_per_sm < 0)
+        opt.delta_buffers > 2 || opt.blocks_per_sm < 0 || opt.tile_lag < -1)
         return nd_fail(ND_ERR_INVALID, "nd_options: tuning fields must be >= 0 (delta_buffers 0, 1 or 2)");
     if ((desc->track_azim == nullptr) != (desc->track_ends == nullptr))
         return nd_fail(ND_ERR_INVALID, "track_azim and track_ends must both be set or both be NULL");

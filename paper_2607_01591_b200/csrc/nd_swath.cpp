@@ -88,6 +88,14 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
         (void)n_threads;
 #endif
         const int64_t* off = desc->track_seg_offset;
+        double lag_len = -1.0;
+        if (prm.lag >= 0.0) {
+            double sum = 0.0;
+            const int64_t S = off[T];
+#pragma omp parallel for reduction(+ : sum) num_threads(nth)
+            for (int64_t k = 0; k < S; ++k) sum += desc->seg_length[k];
+            lag_len = S > 0 ? prm.lag * sum / (double)S : 0.0;
+        }
 #pragma omp parallel num_threads(nth)
         {
             std::vector<int32_t> stamp((size_t)R, -1), lidx((size_t)R, 0);
@@ -116,23 +124,44 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
                     rcount.clear();
                     for (int b = 0; b < NT; ++b) { first[b] = cur[b]; cnt[b] = 0; }
                     int nseg = 0;
-                    for (;;) {
-                        int bs = -1;
-                        for (int b = 0; b < NT; ++b)
-                            if (cur[b] < endk[b] && (bs < 0 || lam[b] < lam[bs])) bs = b;
-                        if (bs < 0 || cnt[bs] == Kmax) break;
-                        const int64_t k = cur[bs];
+                    auto take = [&](int b) -> bool {   // next segment of track b into the tile; false: region window full
+                        const int64_t k = cur[b];
                         const int32_t r = desc->seg_region[k];
                         if (stamp[r] != tile_serial) {
-                            if ((int)regions.size() == Lmax) break;
+                            if ((int)regions.size() == Lmax) return false;
                             stamp[r] = tile_serial;
                             lidx[r] = (int32_t)regions.size();
                             regions.push_back((uint32_t)r);
                             rcount.push_back(0);
                         }
                         ++rcount[lidx[r]];
-                        lam[bs] += desc->seg_length[k];
-                        ++cur[bs]; ++cnt[bs]; ++nseg; --remaining;
+                        lam[b] += desc->seg_length[k];
+                        ++cur[b]; ++cnt[b]; ++nseg; --remaining;
+                        return true;
+                    };
+                    bool level = false;
+                    if (lag_len >= 0.0) {
+                        double lo = 0.0, hi = 0.0;
+                        bool any = false;
+                        for (int b = 0; b < NT; ++b)
+                            if (cur[b] < endk[b]) {
+                                if (!any) { lo = hi = lam[b]; any = true; }
+                                else { lo = std::min(lo, lam[b]); hi = std::max(hi, lam[b]); }
+                            }
+                        level = hi - lo <= lag_len;
+                    }
+                    if (level) {   // equal counts: round j gives every unfinished track its j-th segment
+                        bool full = false;
+                        for (int j = 0; j < Kmax && !full && remaining > 0; ++j)
+                            for (int b = 0; b < NT; ++b)
+                                if (cur[b] < endk[b] && cnt[b] == j && !take(b)) { full = true; break; }
+                    } else {       // geometric: the track furthest behind advances
+                        for (;;) {
+                            int bs = -1;
+                            for (int b = 0; b < NT; ++b)
+                                if (cur[b] < endk[b] && (bs < 0 || lam[b] < lam[bs])) bs = b;
+                            if (bs < 0 || cnt[bs] == Kmax || !take(bs)) break;
+                        }
                     }
                     // ---- encode ----
                     const int L = (int)regions.size();
@@ -242,7 +271,7 @@ struct nd_swath_stream {
 
 extern "C" nd_status nd_swath_stream_build(const nd_problem_desc* desc, int32_t tracks_per_swath, int32_t tile_segments,
                                            int32_t window_regions, int32_t slots_per_line, int32_t row_bytes,
-                                           nd_swath_stream** out)
+                                           double lag_segments, nd_swath_stream** out)
 {
     if (!desc || !out) return nd_fail(ND_ERR_NULL, "nd_swath_stream_build: NULL argument");
     if (!desc->track_seg_offset || !desc->seg_region || !desc->seg_length || !desc->region_material)
@@ -251,7 +280,7 @@ extern "C" nd_status nd_swath_stream_build(const nd_problem_desc* desc, int32_t 
         return nd_fail(ND_ERR_INVALID, "track_azim and track_ends must both be set or both be NULL");
     nd_swath_stream* s = new (std::nothrow) nd_swath_stream();
     if (!s) return nd_fail(ND_ERR_NOMEM, "nd_swath_stream_build: out of host memory");
-    NdSwathParams prm{tracks_per_swath, tile_segments, window_regions, slots_per_line, row_bytes};
+    NdSwathParams prm{tracks_per_swath, tile_segments, window_regions, slots_per_line, row_bytes, lag_segments};
     const nd_status rc = nd_build_swaths(desc, desc->track_azim, desc->track_ends, prm, 0, &s->set);
     if (rc != ND_OK) { delete s; return rc; }
     *out = s;

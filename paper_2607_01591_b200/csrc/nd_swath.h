@@ -3,8 +3,9 @@
 // Tracks of one angle are sorted by their perpendicular coordinate and grouped into SWATHS of NT adjacent tracks;
 // one thread block carries a swath, one lane group ("slot") per track, so the angular flux of a track stays in
 // registers from one end of the track to the other.  A swath is cut along the track direction into TILES: the
-// tracks advance in geometric lock step (always the track whose front is furthest behind) until one of them has
-// Kmax segments in the tile or the tile touches Lmax distinct regions.  A tile is one contiguous, 16-byte aligned
+// tracks advance either by equal counts (every track Kmax segments) or, when their fronts have drifted apart, in
+// geometric lock step (always the track whose front is furthest behind) until one of them has Kmax segments in the
+// tile; in both modes a tile touches at most Lmax distinct regions.  A tile is one contiguous, 16-byte aligned
 // CHUNK, fetched by a single bulk (TMA) copy:
 //     u32 hdr[4]          L | nseg << 16 ;  off_regions | off_csr_off << 16 ;  off_csr_idx | off_rec << 16 ;  bytes
 //                         (offsets in 16-byte units from the chunk start)
@@ -29,6 +30,9 @@ struct NdSwathParams {
     int Lmax;     // max distinct regions in a tile
     int NC;       // slots interleaved in one delta-buffer / q line (bank-conflict-free layout for narrow rows)
     int row_bytes;// bytes of one (region, all groups) FP32 row = 4 * Gs
+    double lag;   // >= 0: while the fronts of the swath's tracks lie within `lag` mean segment lengths of each other a
+                  // tile gives EVERY track Kmax segments (no idle slot steps); beyond it the tile is cut geometrically
+                  // (the track furthest behind advances first) until the fronts are level again.  < 0: always geometric.
 };
 
 struct NdSwathItem { int32_t swath, dir, cost, reserved; };

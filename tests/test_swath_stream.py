@@ -71,13 +71,14 @@ def _decode_and_check(st, mat, seg_offset, seg_region, seg_length, NT, Kmax, Lma
     assert np.all(np.diff(items[:, 2]) <= 0), "most expensive first"
 
 
-@pytest.mark.parametrize("NT,Kmax,Lmax,NC,row_bytes", [(16, 16, 64, 1, 208), (64, 8, 96, 4, 32), (24, 16, 92, 1, 144), (3, 2, 4, 1, 16)])
-def test_stream_of_a_traced_problem(NT, Kmax, Lmax, NC, row_bytes):
+@pytest.mark.parametrize("lag", [-1.0, 0.0, 4.0, 1e9])
+@pytest.mark.parametrize("NT,Kmax,Lmax,NC,row_bytes", [(19, 16, 64, 1, 208), (64, 8, 96, 4, 32), (28, 16, 92, 1, 144), (3, 2, 4, 1, 16)])
+def test_stream_of_a_traced_problem(NT, Kmax, Lmax, NC, row_bytes, lag):
     prob = make_config(2, scale=0.12)
     m = prob.mesh
     tr = nd.nd_tracks_generate(m.xy, m.tri, m.W, m.H, prob.bc, prob.n_azim, prob.spacing)
     st = nd.nd_swath_stream_build(m.material, prob.xs.sigma_t.shape[0], tr.seg_offset, tr.seg_region, tr.seg_length,
-                                  NT, Kmax, Lmax, NC, row_bytes, tr.track_azim, tr.ends)
+                                  NT, Kmax, Lmax, NC, row_bytes, tr.track_azim, tr.ends, lag_segments=lag)
     _decode_and_check(st, m.material, tr.seg_offset, tr.seg_region, tr.seg_length, NT, Kmax, Lmax, NC, row_bytes)
     assert 0.3 < st["lockstep_efficiency"] <= 1.0
     # swaths hold tracks of ONE angle, adjacent in the perpendicular coordinate
@@ -97,8 +98,9 @@ def test_stream_without_geometry_and_with_degenerate_tracks():
     seg_length = rng.uniform(1e-3, 1.0, size=off[-1])
     mat = rng.integers(0, 3, size=R).astype(np.int32)
     for NT, Kmax, Lmax, NC in [(8, 4, 3, 1), (8, 16, 5, 4), (1, 1, 1, 1)]:
-        st = nd.nd_swath_stream_build(mat, 3, off, seg_region, seg_length, NT, Kmax, Lmax, NC, 32)
-        _decode_and_check(st, mat, off, seg_region, seg_length, NT, Kmax, Lmax, NC, 32)
+        for lag in (-1.0, 2.0):
+            st = nd.nd_swath_stream_build(mat, 3, off, seg_region, seg_length, NT, Kmax, Lmax, NC, 32, lag_segments=lag)
+            _decode_and_check(st, mat, off, seg_region, seg_length, NT, Kmax, Lmax, NC, 32)
 
 
 def test_stream_rejects_bad_parameters():
