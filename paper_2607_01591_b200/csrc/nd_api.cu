@@ -117,6 +117,7 @@ struct SwathConfig {
     bool feasible = false;
     NdSwathParams sp{};
     int LPT = 0, warps = 0, ndbuf = 1, blocks_per_sm = 1;
+    bool tight = false;                                   // register-capped kernel variant (more than 512 resident threads per SM)
     int chunk_cap = 0, off_sigt = 0, off_q = 0, off_dbuf = 0, off_chunk = 0, smem_bytes = 0;
     int64_t max_tiles = 0, max_swaths = 0;
     size_t max_blob = 0;
@@ -132,16 +133,13 @@ SwathConfig make_swath_config(const Dims& d, const nd_options& opt)
     if ((int64_t)d.M * line > 65536) return c;
     int warps = opt.block_warps > 0 ? opt.block_warps : (c.LPT > 8 ? 8 : 4);
     if (warps > 16) warps = 16;
-    int Kmax = opt.tile_segments > 0 ? opt.tile_segments : (row_bytes >= 64 ? 16 : 8);
-    int Lmax = opt.window_regions > 0 ? opt.window_regions : 13312 / line;
-    if (Lmax < 16) Lmax = 16;
-    if (Lmax > 65536 / line) Lmax = 65536 / line;
     c.ndbuf = opt.delta_buffers == 2 ? 2 : 1;
     auto pad128 = [](int x) { return (x + 127) / 128 * 128; };
-    for (;; --warps) {                                    // shrink the block until it fits the 227 KB of an SM
-        if (warps < 1) return c;
-        const int NT = warps * 32 / c.LPT / NC * NC;        // slots are packed over the lanes of the whole block
-        if (NT < 1 || (int64_t)NT * Kmax > 65535) continue;
+    auto layout = [&](int w, int Kmax, int Lmax) -> bool {   // fills c for (w, Kmax, Lmax); false if the slot count is unusable
+        const int NT = w * 32 / c.LPT / NC * NC;               // slots are packed over the lanes of the whole block
+        if (NT < 1 || (int64_t)NT * Kmax > 65535) return false;
+        if (Lmax < 16) Lmax = 16;
+        if (Lmax > 65536 / line) Lmax = 65536 / line;
         c.sp.NT = NT; c.sp.Kmax = Kmax; c.sp.Lmax = Lmax; c.sp.NC = NC; c.sp.row_bytes = row_bytes;
         // narrow rows (G <= 16): the flush is cheap, idle slot steps are not -> equal-count tiles while the fronts stay within
         // 16 segments; wide rows: always geometric (the tally re-use rho pays more than level counts), measured in profiles/
@@ -152,15 +150,40 @@ SwathConfig make_swath_config(const Dims& d, const nd_options& opt)
         c.off_dbuf = c.off_q + pad128(2 * Lmax * line);
         c.off_chunk = c.off_dbuf + pad128(c.ndbuf * (NT / NC) * Kmax * line);
         c.smem_bytes = c.off_chunk + ndk::kSwathChunkBufs * c.chunk_cap;
-        if (c.smem_bytes <= kSmemMax) break;
+        return true;
+    };
+    // Defaults (measured, profiles/): occupancy beats tile length once a tile holds >= 8 segments per track.  Aim at
+    // 3 resident blocks per SM (4 for narrow rows), the longest tile that fits, and a region window sized for the
+    // tally re-use the configs show (rho ~ 6.5 wide rows, ~ 8 narrow rows).
+    const int target_blocks = row_bytes < 64 ? 4 : 3;
+    const double rho_est = row_bytes < 64 ? 8.0 : 6.5;
+    bool placed = false;
+    for (; warps >= 1 && !placed; --warps) {
+        const int NT = warps * 32 / c.LPT / NC * NC;
+        if (NT < 1) continue;
+        if (opt.tile_segments > 0 || opt.window_regions > 0) {   // explicit tile shape: take it if it fits at all
+            const int K = opt.tile_segments > 0 ? opt.tile_segments : 16;
+            const int Lw = opt.window_regions > 0 ? opt.window_regions : (int)(NT * K / rho_est + 3) / 4 * 4;
+            placed = layout(warps, K, Lw) && c.smem_bytes <= kSmemMax;
+        } else {
+            for (int blocks = target_blocks; blocks >= 1 && !placed; --blocks)
+                for (int K = 16; K >= 8 && !placed; K -= 2) {
+                    const int Lw = (int)(NT * K / rho_est + 3) / 4 * 4;
+                    placed = layout(warps, K, Lw < 24 ? 24 : Lw) && c.smem_bytes + 1024 <= (kSmemMax + 1024) / blocks;
+                }
+        }
+        if (placed) break;
     }
+    if (!placed) return c;
     c.warps = warps;
     int bps = (kSmemMax + 1024) / (c.smem_bytes + 1024);  // 1 KB per block is reserved by the driver
-    if (bps * warps * 32 > 2048) bps = 2048 / (warps * 32);
+    if (bps * warps * 32 > 768) bps = 768 / (warps * 32);  // 85 registers per thread at most
     if (bps > 8) bps = 8;
     if (bps < 1) bps = 1;
     if (opt.blocks_per_sm > 0 && opt.blocks_per_sm < bps) bps = opt.blocks_per_sm;
     c.blocks_per_sm = bps;
+    c.tight = bps * warps * 32 > 512 && warps <= 12;
+    if (bps * warps * 32 > 512 && !c.tight) c.blocks_per_sm = bps = 512 / (warps * 32) > 0 ? 512 / (warps * 32) : 1;
     c.max_swaths = d.T;
     c.max_tiles = nd_swath_max_tiles(c.sp, d.S, d.T);
     c.max_blob = nd_swath_max_blob(c.sp, d.S, d.T);
@@ -379,7 +402,9 @@ template <int P>
 nd_status launch_swath_p(nd_problem* p, const ndk::SwathParams& prm, cudaStream_t st)
 {
     const SwathConfig& c = p->sc;
-    auto kern = p->opt.exp_mode == ND_EXP_EXPM1 ? ndk::k_sweep_swath<P, 1> : ndk::k_sweep_swath<P, 0>;
+    const bool expm1 = p->opt.exp_mode == ND_EXP_EXPM1;
+    const bool tight = c.tight && !expm1;   // the expm1f cross-check path keeps the roomy register budget
+    auto kern = expm1 ? ndk::k_sweep_swath<P, 1, 0> : (tight ? ndk::k_sweep_swath<P, 0, 1> : ndk::k_sweep_swath<P, 0, 0>);
     ND_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes));
     kern<<<swath_grid(p), 32 * c.warps, c.smem_bytes, st>>>(prm);
     ND_LAUNCH_CHECK(p);

@@ -217,8 +217,9 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
     }
 }
 
-template <int P, int EXPM>
-__global__ void __launch_bounds__(512, 1) k_sweep_swath(const SwathParams prm)
+// TIGHT = 1 caps the registers at 85 (768 resident threads per SM: three 256-thread or two 384-thread blocks).
+template <int P, int EXPM, int TIGHT>
+__global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swath(const SwathParams prm)
 {
     extern __shared__ __align__(128) unsigned char smem_sw[];
     unsigned char* const smem = smem_sw;
