@@ -15,8 +15,8 @@
 //     u16 csr_idx[nseg]      delta-buffer row of every segment, grouped by region             (padded to 16 B)
 //     rec[nseg]              { f32 length ; u32 q_row_byte_offset | sigt_row_byte_offset << 16 }, slot-major,
 //                            forward order; the backward direction walks the same records in reverse
-// A triangle is convex, so one track crosses a region at most once per tile: a segment's weighted flux change is
-// simply STORED in its own delta-buffer row, and csr_idx tells the flush which rows to add up per region.
+// A segment's weighted flux change is simply STORED in its own delta-buffer row, and csr_idx tells the flush which rows
+// to add up per region (a track may re-enter a region; every visit has its own row).
 #ifndef ND_SWATH_H
 #define ND_SWATH_H
 #include <cstdint>
