@@ -202,7 +202,7 @@ int select_kernel(const nd_problem_desc* desc, const nd_options& opt, const Priv
 
 struct Layout { // byte offsets into the workspace
     size_t seg_rm, seg_len, trk_off, trk_w, link_src, psi_a, psi_b, q, tally, phi_a, phi_b, Q, reg_mat, vol, sigt, sigsT,
-        nusf, chi, sigt_f, scalars, partial, stats, blob, tile_chunk, swath_tile0, swath_track, items, counter, total;
+        nusf, chi, sigt_f, scalars, partial, stats, src_region, src_chunks, blob, tile_chunk, swath_tile0, swath_track, items, counter, total;
 };
 
 inline size_t bump(size_t& cur, size_t bytes)
@@ -245,6 +245,8 @@ Layout make_layout(const Dims& d, int max_stats, const PrivConfig& pc_in, const 
     L.scalars = bump(c, sizeof(double) * ndk::SC_COUNT);
     L.partial = bump(c, sizeof(double) * 3 * kReduceBlocks);
     L.stats = bump(c, sizeof(double) * 4 * (size_t)max_stats);
+    L.src_region = bump(c, sizeof(int32_t) * (size_t)d.R);
+    L.src_chunks = bump(c, sizeof(int4) * ((size_t)d.R / 4 + (size_t)d.M + 1));   // chunks hold >= 4 regions except one per material
     if (pc.feasible) {
         L.blob = bump(c, pc.max_blob);
         L.tile_chunk = bump(c, sizeof(uint32_t) * (size_t)pc.max_tiles);
@@ -299,6 +301,8 @@ struct nd_problem {
     float* psi_in; float* psi_out; float* q; double* tally; double* phi_cur; double* phi_new; double* Q;
     int32_t* reg_mat; double* vol; double* sigt; double* sigsT; double* nusf; double* chi; float* sigt_f;
     double* scalars; double* partial; double* stats;
+    int32_t* src_region = nullptr; int4* src_chunks = nullptr;
+    int n_src_chunks = 0, src_chunk_regions = 0;
     // private-tally sweep
     PrivConfig pc{};
     SwathConfig sc{};
@@ -451,6 +455,21 @@ nd_status launch_sweep_p(nd_problem* p, const ndk::SweepParams& prm, cudaStream_
         ndk::k_sweep_atomic<P, 1><<<grid, block, 0, st>>>(prm);
     else
         ndk::k_sweep_atomic<P, 0><<<grid, block, 0, st>>>(prm);
+    ND_LAUNCH_CHECK(p);
+    return ND_OK;
+}
+
+// A5: source update over material-grouped chunks
+nd_status launch_source(nd_problem* p, const ndk::SourceParams& sp, cudaStream_t st)
+{
+    const Dims& d = p->d;
+    ndk::SourceChunkParams cp{};
+    cp.base = sp; cp.src_region = p->src_region; cp.chunks = p->src_chunks; cp.n_chunks = p->n_src_chunks;
+    cp.chunk_regions = p->src_chunk_regions;
+    const int block = 256;
+    const size_t smem = sizeof(double) * ((size_t)p->src_chunk_regions * d.G + p->src_chunk_regions);
+    const int grid = p->n_src_chunks < 8 * p->n_sm ? (p->n_src_chunks > 0 ? p->n_src_chunks : 1) : 8 * p->n_sm;
+    ndk::k_source_chunks<<<grid, block, smem, st>>>(cp);
     ND_LAUNCH_CHECK(p);
     return ND_OK;
 }
@@ -676,6 +695,7 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     p->sigt = (double*)(ws + L.sigt); p->sigsT = (double*)(ws + L.sigsT); p->nusf = (double*)(ws + L.nusf);
     p->chi = (double*)(ws + L.chi); p->sigt_f = (float*)(ws + L.sigt_f);
     p->scalars = (double*)(ws + L.scalars); p->partial = (double*)(ws + L.partial); p->stats = (double*)(ws + L.stats);
+    p->src_region = (int32_t*)(ws + L.src_region); p->src_chunks = (int4*)(ws + L.src_chunks);
     if (tiled) {
         p->blob = (uint8_t*)(ws + L.blob); p->tile_chunk = (uint32_t*)(ws + L.tile_chunk); p->swath_tile0 = (int64_t*)(ws + L.swath_tile0);
         p->swath_track = (int32_t*)(ws + L.swath_track); p->items = (int4*)(ws + L.items); p->counter = (int*)(ws + L.counter);
@@ -705,6 +725,24 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         p->c[i] = (float)(-1.4426950408889634074 / desc->polar_sin[i]);
         p->inv_sin[i] = (float)(1.0 / desc->polar_sin[i]);
         p->wp[i] = (float)(desc->polar_weight[i] * desc->polar_sin[i]);
+    }
+    // A5: regions grouped by material into chunks of nsub*4 regions (k_source_chunks)
+    std::vector<int32_t> h_src_region((size_t)d.R);
+    std::vector<int4> h_src_chunks;
+    {
+        const int nsub = 256 / d.G > 0 ? 256 / d.G : 1;
+        p->src_chunk_regions = nsub * ndk::kSrcRegionsPerThread;
+        std::vector<int64_t> count((size_t)d.M + 1, 0);
+        for (int r = 0; r < d.R; ++r) ++count[desc->region_material[r] + 1];
+        for (int m = 0; m < d.M; ++m) count[m + 1] += count[m];
+        std::vector<int64_t> fill(count.begin(), count.end() - 1);
+        for (int r = 0; r < d.R; ++r) h_src_region[(size_t)fill[desc->region_material[r]]++] = r;
+        for (int m = 0; m < d.M; ++m)
+            for (int64_t i = count[m]; i < count[m + 1]; i += p->src_chunk_regions) {
+                const int n = (int)std::min<int64_t>(p->src_chunk_regions, count[m + 1] - i);
+                h_src_chunks.push_back(make_int4((int)i, n, m, 0));
+            }
+        p->n_src_chunks = (int)h_src_chunks.size();
     }
     p->sweep_kernel = kernel;
 
@@ -755,6 +793,8 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     ND_CUDA_P(cudaMemcpyAsync(p->nusf, desc->nu_sigma_f, sizeof(double) * (size_t)d.M * d.G, cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->chi, desc->chi, sizeof(double) * (size_t)d.M * d.G, cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->sigt_f, h_sigt_f.data(), sizeof(float) * h_sigt_f.size(), cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->src_region, h_src_region.data(), sizeof(int32_t) * h_src_region.size(), cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->src_chunks, h_src_chunks.data(), sizeof(int4) * h_src_chunks.size(), cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaStreamSynchronize(st));
 #undef ND_CUDA_P
     rc = reset_state(p, st);
@@ -801,9 +841,8 @@ extern "C" nd_status nd_source_update(nd_problem* p, const double* d_phi, double
     sp.phi = d_phi; sp.reg_mat = p->reg_mat; sp.sigt = p->sigt; sp.sigsT = p->sigsT; sp.nusf = p->nusf; sp.chi = p->chi;
     sp.k_ptr = nullptr; sp.f_ptr = nullptr; sp.k_val = k_eff; sp.Q = d_Q_out; sp.q = nullptr; sp.tally = nullptr;
     sp.R = d.R; sp.G = d.G; sp.Gs = d.Gs;
-    const int rpb = 256 / d.G;
-    ndk::k_source<<<grid_for((int64_t)(d.R + rpb - 1) / rpb * 256, 256, 8 * p->n_sm), 256, sizeof(double) * rpb * d.G, st>>>(sp);
-    ND_LAUNCH_CHECK(p);
+    nd_status rc_src = launch_source(p, sp, st);
+    if (rc_src != ND_OK) return rc_src;
     if (d_fission_rate_out) {
         // uses a private scalar slot so the problem's own F (power-iteration state) is not disturbed
         const int grid = grid_for((int64_t)d.R * d.G, 256, kReduceBlocks);
@@ -829,15 +868,13 @@ extern "C" nd_status nd_power_iteration(nd_problem* p, int32_t max_iters, double
     sp.reg_mat = p->reg_mat; sp.sigt = p->sigt; sp.sigsT = p->sigsT; sp.nusf = p->nusf; sp.chi = p->chi;
     sp.k_ptr = p->scalars + ndk::SC_K; sp.f_ptr = p->scalars + ndk::SC_F; sp.k_val = 1.0;
     sp.Q = p->Q; sp.q = p->q; sp.tally = p->tally; sp.R = d.R; sp.G = d.G; sp.Gs = d.Gs;
-    const int rpb = 256 / d.G;
-    const int src_grid = grid_for((int64_t)(d.R + rpb - 1) / rpb * 256, 256, 8 * p->n_sm);
     int it = 0;
     bool converged = !use_tol;
     for (; it < max_iters; ++it) {
         sp.phi = p->phi_cur;
-        ndk::k_source<<<src_grid, 256, sizeof(double) * rpb * d.G, st>>>(sp);
-        ND_LAUNCH_CHECK(p);
-        nd_status rc = launch_sweep(p, p->scalars + ndk::SC_F, st);
+        nd_status rc = launch_source(p, sp, st);
+        if (rc != ND_OK) return rc;
+        rc = launch_sweep(p, p->scalars + ndk::SC_F, st);
         if (rc != ND_OK) return rc;
         int grid = 0;
         rc = launch_finalise(p, p->Q, p->phi_cur, p->scalars + ndk::SC_F, p->phi_new, &grid, st);

@@ -226,7 +226,6 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);              // [kSwathChunkBufs] chunk-arrival barriers
     volatile int* s_item = reinterpret_cast<volatile int*>(smem + 64);
     const int tid = threadIdx.x, nthr = blockDim.x;
-    const int lane = tid & 31, warp = tid >> 5;
     const int Gs = prm.Gs, row_bytes = 4 * Gs, line = prm.NC * row_bytes;
     unsigned char* sigt_s = smem + prm.off_sigt;
     unsigned char* q_s = smem + prm.off_q;           // [2][Lmax][line]
