@@ -7,6 +7,7 @@
  *   nd_tracks_generate   cyclic ("modular") rays on the bounding box of the whole domain and the
  *                        ray-mesh intersection through a half-edge structure, done once before the
  *                        solve (section III.A).  HOST code, FP64, bit-exact rules.
+ *                        nd_tracks_generate_device runs the ray walk on the GPU, bit-identically.
  *   nd_problem_create    packs the precomputed segment data into the device segment
  *                        stream and uploads cross sections, quadrature weights and the link table.
  *   nd_transport_sweep   Eq. (5) along every track, direction, polar angle and group,
@@ -122,6 +123,29 @@ typedef struct {            /* all pointers HOST, owned by the nd_tracks object,
     const double* azim_weight;       /* [N_a/2] omega_a per direction (sum over N_a directions = 1) */
     const double* azim_spacing;      /* [N_a/2] effective spacing delta_a */
 } nd_tracks_view_t;
+
+/* The same preprocessing with the ray walk (rule R-W, one step per segment: almost all of the work) on the GPU:
+ * one thread per track, FP64 round-to-nearest intrinsics only, so the output is bit-identical to nd_tracks_generate's.
+ * Laydown, links and the half-edge twins are still built on the host.  The result is the same HOST object.
+ *   device_workspace  DEVICE, 256-byte aligned, caller-owned, free to reuse after the call.  It must hold at least
+ *                     *min_bytes; every further *bytes_per_segment bytes let one more segment be traced per batch (the
+ *                     fill pass runs in as many batches of tracks as the workspace requires).
+ * Synchronises the stream before returning.  ND_ERR_WORKSPACE if the workspace is too small for the longest track. */
+nd_status nd_tracks_device_workspace_bytes(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, size_t* min_bytes,
+                                           size_t* bytes_per_segment);
+typedef struct {                /* where the time of nd_tracks_generate_device went (HOST wall clock / CUDA events) */
+    double prepare_s;           /* host: laydown, links, half-edge twins, start triangles */
+    double count_kernel_ms;     /* device: walk pass 1 (segment counts) */
+    double fill_kernel_ms;      /* device: walk pass 2 (segments), summed over the batches */
+    double copy_s;              /* device -> host copies of the segment arrays */
+    double finish_s;            /* host: track volumes in canonical order */
+    double total_s;
+    int64_t n_segments;
+    int32_t batches, reserved;
+} nd_trace_timing;
+nd_status nd_tracks_generate_device(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, void* device_workspace,
+                                    size_t device_bytes, void* cuda_stream, nd_trace_timing* timing_or_null,
+                                    nd_tracks** out);
 
 nd_status nd_tracks_view(const nd_tracks* tracks, nd_tracks_view_t* view);
 nd_status nd_tracks_destroy(nd_tracks* tracks);

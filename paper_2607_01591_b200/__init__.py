@@ -22,7 +22,7 @@ ND_EXP_FAST, ND_EXP_EXPM1 = 0, 1
 ND_SWEEP_AUTO, ND_SWEEP_ATOMIC, ND_SWEEP_PRIVATE, ND_SWEEP_SWATH = 0, 1, 2, 3
 
 EXPORTS = [
-    "nd_tracks_generate", "nd_tracks_view", "nd_tracks_destroy", "nd_workspace_bytes", "nd_problem_create",
+    "nd_tracks_generate", "nd_tracks_device_workspace_bytes", "nd_tracks_generate_device", "nd_tracks_view", "nd_tracks_destroy", "nd_workspace_bytes", "nd_problem_create",
     "nd_problem_destroy", "nd_transport_sweep", "nd_source_update", "nd_power_iteration", "nd_state_reset",
     "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_flux_get", "nd_flux_set",
     "nd_track_volume_get", "nd_tally_get", "nd_profile_enable", "nd_profile_read", "nd_problem_info_get",
@@ -81,6 +81,12 @@ class nd_problem_info(C.Structure):
                 ("smem_bytes", C.c_int32), ("grid_blocks", C.c_int32), ("tracks_per_block", C.c_int32)]
 
 
+class nd_trace_timing(C.Structure):
+    _fields_ = [("prepare_s", C.c_double), ("count_kernel_ms", C.c_double), ("fill_kernel_ms", C.c_double),
+                ("copy_s", C.c_double), ("finish_s", C.c_double), ("total_s", C.c_double), ("n_segments", C.c_int64),
+                ("batches", C.c_int32), ("reserved", C.c_int32)]
+
+
 class nd_swath_stream_view_t(C.Structure):
     _fields_ = [("n_swaths", C.c_int64), ("n_tiles", C.c_int64), ("blob_bytes", C.c_int64), ("n_items", C.c_int64),
                 ("blob", C.c_void_p), ("tile_chunk", C.c_void_p), ("swath_tile0", C.c_void_p), ("swath_track", C.c_void_p),
@@ -105,6 +111,10 @@ def lib():
         L.nd_last_error.argtypes = [C.c_void_p]
         L.nd_version.restype = C.c_uint32
         L.nd_tracks_generate.argtypes = [C.POINTER(nd_mesh_desc), C.c_int32, C.c_double, C.c_int32, C.POINTER(C.c_void_p)]
+        L.nd_tracks_device_workspace_bytes.argtypes = [C.POINTER(nd_mesh_desc), C.c_int32, C.c_double, C.POINTER(C.c_size_t),
+                                                       C.POINTER(C.c_size_t)]
+        L.nd_tracks_generate_device.argtypes = [C.POINTER(nd_mesh_desc), C.c_int32, C.c_double, C.c_void_p, C.c_size_t,
+                                                C.c_void_p, C.POINTER(nd_trace_timing), C.POINTER(C.c_void_p)]
         L.nd_tracks_view.argtypes = [C.c_void_p, C.POINTER(nd_tracks_view_t)]
         L.nd_tracks_destroy.argtypes = [C.c_void_p]
         L.nd_workspace_bytes.argtypes = [C.POINTER(nd_problem_desc), C.POINTER(nd_options), C.POINTER(C.c_size_t)]
@@ -198,6 +208,34 @@ def nd_tracks_generate(xy, tri, W, H, bc, n_azim, spacing, n_threads=0) -> Track
     v = nd_tracks_view_t()
     _check(lib().nd_tracks_view(h, C.byref(v)), "nd_tracks_view")
     return Tracks(h, v)
+
+
+def nd_tracks_generate_device(xy, tri, W, H, bc, n_azim, spacing, segment_capacity=1 << 28, device="cuda:0") -> Tracks:
+    """Row A0 with the ray walk on the GPU; bit-identical to nd_tracks_generate.  The torch
+    workspace holds `segment_capacity` segments per fill batch (12 bytes each) and is released on return."""
+    import torch
+    xy = np.ascontiguousarray(xy, np.float64)
+    tri = np.ascontiguousarray(tri, np.int32)
+    md = nd_mesh_desc(len(xy), len(tri), xy.ctypes.data, tri.ctypes.data, float(W), float(H), (C.c_int32 * 4)(*[int(b) for b in bc]))
+    nmin, per = C.c_size_t(), C.c_size_t()
+    _check(lib().nd_tracks_device_workspace_bytes(C.byref(md), int(n_azim), float(spacing), C.byref(nmin), C.byref(per)),
+           "nd_tracks_device_workspace_bytes")
+    dev = torch.device(device)
+    nbytes = int(nmin.value) + int(per.value) * int(segment_capacity)
+    with torch.cuda.device(dev):
+        ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev)
+        ptr = (ws.data_ptr() + 255) // 256 * 256
+        h = C.c_void_p()
+        tm = nd_trace_timing()
+        _check(lib().nd_tracks_generate_device(C.byref(md), int(n_azim), float(spacing), C.c_void_p(ptr), nbytes,
+                                               C.c_void_p(torch.cuda.current_stream(dev).cuda_stream), C.byref(tm), C.byref(h)),
+               "nd_tracks_generate_device")
+    del ws
+    v = nd_tracks_view_t()
+    _check(lib().nd_tracks_view(h, C.byref(v)), "nd_tracks_view")
+    out = Tracks(h, v)
+    out.timing = {f[0]: getattr(tm, f[0]) for f in nd_trace_timing._fields_ if f[0] != "reserved"}
+    return out
 
 
 class Problem:

@@ -22,6 +22,7 @@
 
 #include "nd.h"
 #include "nd_internal.h"
+#include "nd_tracks_internal.h"
 
 namespace {
 
@@ -29,16 +30,7 @@ constexpr double kPi = 3.14159265358979323846;
 
 enum Side : int { kLeft = 0, kRight = 1, kBottom = 2, kTop = 3 };
 
-struct AngleSet {            // one track angle j in (0, pi)
-    int nx = 0, ny = 0;      // tracks leaving the bottom side / the vertical side
-    double dx = 0, dy = 0;   // slot widths
-    double ux = 0, uy = 0;   // unit forward direction (uy > 0)
-    double delta = 0;        // effective spacing
-    double phi = 0;          // effective angle of the first-quadrant partner
-    double omega = 0;        // azimuthal weight per direction
-    int first = 0;           // id of the angle's first track
-    bool mirrored = false;   // second quadrant (ux < 0)
-};
+using AngleSet = NdAngleSet;
 
 struct EndKey { int side, slot; };
 
@@ -224,23 +216,11 @@ int64_t walk(const HalfEdgeMesh& m, int start_side, double x0, double y0, double
 
 } // namespace
 
-struct nd_tracks {
-    int n_azim = 0, n_half = 0, n_tracks = 0, n_regions = 0;
-    int64_t n_segments = 0;
-    std::vector<AngleSet> angles;
-    std::vector<int64_t> seg_offset;
-    std::vector<int32_t> seg_region;
-    std::vector<double> seg_length;
-    std::vector<double> track_weight;
-    std::vector<int32_t> link;
-    std::vector<int32_t> track_azim;
-    std::vector<double> ends;
-    std::vector<double> volume;
-    std::vector<double> azim_phi, azim_weight, azim_spacing;
-};
+namespace {
 
-extern "C" nd_status nd_tracks_generate(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, int32_t n_threads,
-                                        nd_tracks** out)
+// Laydown (R-T), links (O-3) and the half-edge mesh; on success *out owns the tracks (no segments yet).
+nd_status prepare_impl(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, nd_tracks** out, HalfEdgeMesh& hm,
+                       std::vector<EndKey>& kstart)
 {
     if (!mesh || !out || !mesh->xy || !mesh->tri) return nd_fail(ND_ERR_NULL, "nd_tracks_generate: NULL argument");
     if (mesh->n_vertices < 3 || mesh->n_triangles < 1 || !(mesh->W > 0.0) || !(mesh->H > 0.0) || !(spacing > 0.0) ||
@@ -290,7 +270,8 @@ extern "C" nd_status nd_tracks_generate(const nd_mesh_desc* mesh, int32_t n_azim
         tr->n_tracks = T;
         tr->track_weight.resize(T); tr->track_azim.resize(T); tr->ends.resize(4 * static_cast<size_t>(T));
         tr->link.assign(2 * static_cast<size_t>(T), -1);
-        std::vector<EndKey> kstart(T), kend(T);
+        kstart.assign(T, EndKey{0, 0});
+        std::vector<EndKey> kend(T);
         for (int j = 0; j < nh; ++j) {
             const AngleSet& A = tr->angles[j];
             for (int i = 0; i < A.nx + A.ny; ++i) {
@@ -326,10 +307,78 @@ extern "C" nd_status nd_tracks_generate(const nd_mesh_desc* mesh, int32_t n_azim
                 }
             }
         }
-        // ---- R-W: walk every track through the half-edge mesh (count pass, then fill pass) ----
-        HalfEdgeMesh hm;
         nd_status rc = build_mesh(hm, mesh);
         if (rc != ND_OK) { delete tr; return nd_fail(rc, "nd_tracks_generate: mesh is not a conforming CCW triangulation of [0,W]x[0,H]"); }
+    } catch (const std::bad_alloc&) {
+        delete tr;
+        return nd_fail(ND_ERR_NOMEM, "nd_tracks_generate: out of host memory");
+    }
+    *out = tr;
+    return ND_OK;
+}
+
+} // namespace
+
+nd_status nd_tracks_prepare(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, nd_tracks** out, NdWalkInput* walk_in)
+{
+    if (!walk_in) return nd_fail(ND_ERR_NULL, "nd_tracks_prepare: NULL argument");
+    HalfEdgeMesh hm;
+    std::vector<EndKey> kstart;
+    nd_tracks* tr = nullptr;
+    nd_status rc = prepare_impl(mesh, n_azim, spacing, &tr, hm, kstart);
+    if (rc != ND_OK) return rc;
+    try {
+        walk_in->twin = hm.twin;
+        walk_in->start_tri.resize(static_cast<size_t>(tr->n_tracks));
+        for (int t = 0; t < tr->n_tracks; ++t) {
+            const double x0 = tr->ends[4 * static_cast<size_t>(t)], y0 = tr->ends[4 * static_cast<size_t>(t) + 1];
+            const int side = kstart[t].side;
+            walk_in->start_tri[t] = first_triangle(hm, side, (side == kBottom || side == kTop) ? x0 : y0);
+        }
+    } catch (const std::bad_alloc&) {
+        delete tr;
+        return nd_fail(ND_ERR_NOMEM, "nd_tracks_prepare: out of host memory");
+    }
+    *out = tr;
+    return ND_OK;
+}
+
+nd_status nd_tracks_finish(nd_tracks* tr)
+{
+    if (!tr) return nd_fail(ND_ERR_NULL, "nd_tracks_finish: NULL argument");
+    try {
+        const int T = tr->n_tracks, nh = tr->n_half;
+        // ---- O-5: track-estimated areas, summed in canonical (track, segment) order ----
+        tr->volume.assign(static_cast<size_t>(tr->n_regions), 0.0);
+        for (int t = 0; t < T; ++t) {
+            const double w2 = 2.0 * tr->track_weight[t];
+            for (int64_t k = tr->seg_offset[t]; k < tr->seg_offset[static_cast<size_t>(t) + 1]; ++k)
+                tr->volume[tr->seg_region[k]] += w2 * tr->seg_length[k];
+        }
+        tr->azim_phi.resize(nh); tr->azim_weight.resize(nh); tr->azim_spacing.resize(nh);
+        for (int j = 0; j < nh; ++j) {
+            tr->azim_phi[j] = tr->angles[j].mirrored ? kPi - tr->angles[j].phi : tr->angles[j].phi;
+            tr->azim_weight[j] = tr->angles[j].omega;
+            tr->azim_spacing[j] = tr->angles[j].delta;
+        }
+    } catch (const std::bad_alloc&) {
+        return nd_fail(ND_ERR_NOMEM, "nd_tracks_finish: out of host memory");
+    }
+    return ND_OK;
+}
+
+extern "C" nd_status nd_tracks_generate(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, int32_t n_threads,
+                                        nd_tracks** out)
+{
+    if (!out) return nd_fail(ND_ERR_NULL, "nd_tracks_generate: NULL argument");
+    HalfEdgeMesh hm;
+    std::vector<EndKey> kstart;
+    nd_tracks* tr = nullptr;
+    nd_status rc = prepare_impl(mesh, n_azim, spacing, &tr, hm, kstart);
+    if (rc != ND_OK) return rc;
+    try {
+        const int T = tr->n_tracks;
+        // ---- R-W: walk every track through the half-edge mesh (count pass, then fill pass) ----
 #ifdef _OPENMP
         const int nth = n_threads > 0 ? n_threads : omp_get_max_threads();
 #else
@@ -357,23 +406,12 @@ extern "C" nd_status nd_tracks_generate(const nd_mesh_desc* mesh, int32_t n_azim
             walk<true>(hm, kstart[t].side, tr->ends[4 * static_cast<size_t>(t)], tr->ends[4 * static_cast<size_t>(t) + 1],
                        A.ux, A.uy, tr->seg_region.data() + o, tr->seg_length.data() + o);
         }
-        // ---- O-5: track-estimated areas, summed in canonical (track, segment) order ----
-        tr->volume.assign(static_cast<size_t>(tr->n_regions), 0.0);
-        for (int t = 0; t < T; ++t) {
-            const double w2 = 2.0 * tr->track_weight[t];
-            for (int64_t k = tr->seg_offset[t]; k < tr->seg_offset[static_cast<size_t>(t) + 1]; ++k)
-                tr->volume[tr->seg_region[k]] += w2 * tr->seg_length[k];
-        }
-        tr->azim_phi.resize(nh); tr->azim_weight.resize(nh); tr->azim_spacing.resize(nh);
-        for (int j = 0; j < nh; ++j) {
-            tr->azim_phi[j] = tr->angles[j].mirrored ? kPi - tr->angles[j].phi : tr->angles[j].phi;
-            tr->azim_weight[j] = tr->angles[j].omega;
-            tr->azim_spacing[j] = tr->angles[j].delta;
-        }
     } catch (const std::bad_alloc&) {
         delete tr;
         return nd_fail(ND_ERR_NOMEM, "nd_tracks_generate: out of host memory");
     }
+    rc = nd_tracks_finish(tr);
+    if (rc != ND_OK) { delete tr; return rc; }
     *out = tr;
     return ND_OK;
 }

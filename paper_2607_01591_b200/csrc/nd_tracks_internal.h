@@ -1,0 +1,48 @@
+// nd_tracks_internal.h -- private: the nd_tracks object and the host steps shared by nd_tracks_generate (host ray
+// walk) and nd_tracks_generate_device (CUDA ray walk).  All FP64 geometry on the host lives in nd_tracks.cpp, which is
+// compiled with -ffp-contract=off (rule R-T / R-W: bit-exact expression trees).
+#ifndef ND_TRACKS_INTERNAL_H
+#define ND_TRACKS_INTERNAL_H
+#include <cstdint>
+#include <vector>
+
+#include "nd.h"
+
+struct NdAngleSet {          // one track angle j in (0, pi)
+    int nx = 0, ny = 0;      // tracks leaving the bottom side / the vertical side
+    double dx = 0, dy = 0;   // slot widths
+    double ux = 0, uy = 0;   // unit forward direction (uy > 0)
+    double delta = 0;        // effective spacing
+    double phi = 0;          // effective angle of the first-quadrant partner
+    double omega = 0;        // azimuthal weight per direction
+    int first = 0;           // id of the angle's first track
+    bool mirrored = false;   // second quadrant (ux < 0)
+};
+
+struct nd_tracks {
+    int n_azim = 0, n_half = 0, n_tracks = 0, n_regions = 0;
+    int64_t n_segments = 0;
+    std::vector<NdAngleSet> angles;
+    std::vector<int64_t> seg_offset;
+    std::vector<int32_t> seg_region;
+    std::vector<double> seg_length;
+    std::vector<double> track_weight;
+    std::vector<int32_t> link;
+    std::vector<int32_t> track_azim;
+    std::vector<double> ends;
+    std::vector<double> volume;
+    std::vector<double> azim_phi, azim_weight, azim_spacing;
+};
+
+// What a ray walker needs besides the mesh arrays: the half-edge twins and every track's first triangle.
+struct NdWalkInput {
+    std::vector<int32_t> twin;        // [3R] opposite half-edge or -1
+    std::vector<int32_t> start_tri;   // [T]  triangle that holds the track's start point (rule R-W)
+};
+
+// Laydown (R-T), links (O-3), half-edge mesh and start triangles.  *out owns the result (segments still empty).
+nd_status nd_tracks_prepare(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, nd_tracks** out, NdWalkInput* walk);
+// After seg_offset / seg_region / seg_length are filled: track volumes (O-5, canonical order) and the per-angle views.
+nd_status nd_tracks_finish(nd_tracks* tr);
+
+#endif
