@@ -142,8 +142,8 @@ SwathConfig make_swath_config(const Dims& d, const nd_options& opt)
         if (Lmax > 65536 / line) Lmax = 65536 / line;
         c.sp.NT = NT; c.sp.Kmax = Kmax; c.sp.Lmax = Lmax; c.sp.NC = NC; c.sp.row_bytes = row_bytes;
         // narrow rows (G <= 16): the flush is cheap, idle slot steps are not -> equal-count tiles while the fronts stay within
-        // 16 segments; wide rows: always geometric (the tally re-use rho pays more than level counts), measured in profiles/
-        c.sp.lag = opt.tile_lag < 0 ? -1.0 : (opt.tile_lag > 0 ? (double)opt.tile_lag : (row_bytes < 64 ? 16.0 : -1.0));
+        // 16 segments; wide rows: only within 4 segments (the tally re-use rho pays more than level counts), measured in profiles/
+        c.sp.lag = opt.tile_lag < 0 ? -1.0 : (opt.tile_lag > 0 ? (double)opt.tile_lag : (row_bytes < 64 ? 16.0 : 4.0));
         c.chunk_cap = nd_swath_chunk_capacity(c.sp);
         c.off_sigt = 128;
         c.off_q = c.off_sigt + pad128(d.M * line);
