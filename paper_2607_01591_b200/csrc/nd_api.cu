@@ -156,6 +156,12 @@ SwathConfig make_swath_config(const Dims& d, const nd_options& opt)
     // 3 resident blocks per SM (4 for narrow rows), the longest tile that fits, and a region window sized for the
     // tally re-use the configs show (rho ~ 6.5 wide rows, ~ 8 narrow rows).
     const int target_blocks = row_bytes < 64 ? 4 : 3;
+    if (opt.block_warps <= 0) {
+        // small problems: fewer tracks per block until there are about two work items (swath, direction) per resident
+        // block of a 148-SM part -- the sweep of a small problem is bound by its longest track, not by throughput
+        auto slots = [&](int w) { const int n = w * 32 / c.LPT / NC * NC; return n > 0 ? n : 1; };
+        while (warps > 1 && 2 * ((int64_t)d.T / slots(warps)) < 2 * 148 * target_blocks) warps /= 2;
+    }
     const double rho_est = row_bytes < 64 ? 8.0 : 6.5;
     bool placed = false;
     for (; warps >= 1 && !placed; --warps) {

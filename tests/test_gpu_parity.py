@@ -48,6 +48,25 @@ def test_sweep_matches_oracle(case, kernel):
         pair.close()
 
 
+SHAPES = [dict(block_warps=1), dict(block_warps=3, tile_segments=2, window_regions=5), dict(block_warps=8, tile_segments=16),
+          dict(block_warps=16, tile_segments=5, delta_buffers=2), dict(block_warps=8, tile_lag=-1), dict(block_warps=4, tile_lag=1000),
+          dict(block_warps=12, tile_segments=12, blocks_per_sm=1)]
+
+
+@pytest.mark.parametrize("case", [(2, 0.15), (4, 0.06), (5, 0.0008)], ids=["cfg2", "cfg4", "cfg5"])
+@pytest.mark.parametrize("shape", SHAPES, ids=[str(i) for i in range(len(SHAPES))])
+def test_swath_block_and_tile_shapes(case, shape):
+    """The swath kernel's tuning options (block size, tile length, region window, delta buffers, tile policy) never
+    change the result beyond summation order."""
+    pair = make_pair(case[0], case[1], sweep_kernel=nd.ND_SWEEP_SWATH, **shape)
+    try:
+        info = pair.gpu.nd_problem_info_get()
+        assert info["sweep_kernel"] == nd.ND_SWEEP_SWATH and 32 <= info["block_threads"] <= 32 * shape["block_warps"]
+        _check_sweep(pair, seed=300 + case[0])
+    finally:
+        pair.close()
+
+
 @pytest.mark.parametrize("exp_mode", [nd.ND_EXP_FAST, nd.ND_EXP_EXPM1])
 def test_sweep_exp_modes(exp_mode):
     pair = make_pair(2, 0.15, exp_mode=exp_mode)
