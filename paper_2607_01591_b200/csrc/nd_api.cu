@@ -229,8 +229,10 @@ Layout make_layout(const Dims& d, int max_stats, const PrivConfig& pc_in, const 
     Layout L{};
     size_t c = 0;
     const size_t RG = (size_t)d.R * d.G, RGs = (size_t)d.R * d.Gs, NPSI = (size_t)d.T * 2 * d.P * d.Gs;
-    L.seg_rm = bump(c, sizeof(uint32_t) * (size_t)d.Spad);
-    L.seg_len = bump(c, sizeof(float) * (size_t)d.Spad);
+    // the v0 SoA stream is read by the atomic kernel only; the tiled kernels carry their own chunk stream
+    const size_t soa = kernel == ND_SWEEP_ATOMIC ? (size_t)d.Spad : 4;
+    L.seg_rm = bump(c, sizeof(uint32_t) * soa);
+    L.seg_len = bump(c, sizeof(float) * soa);
     L.trk_off = bump(c, sizeof(int64_t) * ((size_t)d.T + 1));
     L.trk_w = bump(c, sizeof(float) * (size_t)d.T);
     L.link_src = bump(c, sizeof(int32_t) * 2 * (size_t)d.T);
@@ -642,8 +644,9 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         p = new nd_problem();
         p->d = d; p->opt = opt; p->L = L; p->ws = static_cast<char*>(device_workspace);
         // ---- A1: pack the segment stream (SoA, every track run padded to a multiple of 4 = 16 bytes) ----
-        h_rm.assign((size_t)d.Spad, 0u);
-        h_len.assign((size_t)d.Spad, 0.f);
+        const bool soa = kernel == ND_SWEEP_ATOMIC;
+        h_rm.assign(soa ? (size_t)d.Spad : 4, 0u);
+        h_len.assign(soa ? (size_t)d.Spad : 4, 0.f);
         h_off.resize((size_t)d.T + 1);
         p->h_vol.assign((size_t)d.R, 0.0);
         int64_t o = 0;
@@ -654,13 +657,15 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
             uint32_t last = 0;
             for (int64_t k = k0; k < k1; ++k) {
                 const int32_t r = desc->seg_region[k];
-                last = ndk::pack_rm((uint32_t)r, (uint32_t)desc->region_material[r]);
-                h_rm[o] = last;
-                h_len[o] = (float)desc->seg_length[k];
                 p->h_vol[r] += w2 * desc->seg_length[k];
+                if (soa) {
+                    last = ndk::pack_rm((uint32_t)r, (uint32_t)desc->region_material[r]);
+                    h_rm[o] = last;
+                    h_len[o] = (float)desc->seg_length[k];
+                }
                 ++o;
             }
-            while (o % 4 != 0) { h_rm[o] = last; h_len[o] = 0.f; ++o; } // zero-length segments are exact no-ops
+            while (o % 4 != 0) { if (soa) { h_rm[o] = last; h_len[o] = 0.f; } ++o; } // zero-length segments are exact no-ops
         }
         h_off[d.T] = o;
     } catch (const std::bad_alloc&) {

@@ -232,3 +232,59 @@ def test_problem_create_rejects_on_device_side_errors():
         assert info["updates_per_sweep"] == 2 * pair.o_tr.n_segs * pair.P * pair.G
     finally:
         pair.close()
+
+
+def test_pure_absorber_fixed_source_closed_form_on_gpu():
+    """Fixed-source mode against mathematics, not the oracle: pure absorber (Sigma_s = 0), uniform isotropic emission
+    density q0, reflective box -> phi = q0 / Sigma_a in every region and group once the boundary flux has converged."""
+    mesh = rect_tri_mesh(1.3, 0.9, 5, 4, seed=8, jitter=0.25)
+    mesh.material[:] = 0
+    G = 3
+    xs = homogeneous_xs(G, 5)
+    xs.sigma_s[:] = 0.0
+    xs.nu_sigma_f[:] = 0.0
+    s, w = tabuchi_yamamoto(3)
+    tr = nd.nd_tracks_generate(mesh.xy, mesh.tri, mesh.W, mesh.H, (1, 1, 1, 1), 16, 0.03)
+    gp = nd.nd_problem_create(xs, s, w, mesh.material, tr)
+    try:
+        q0 = np.array([1.0, 0.4, 2.5])
+        Q = torch.from_numpy(np.tile(q0 / (4.0 * np.pi), (mesh.n_regions, 1))).cuda()
+        gp.nd_boundary_flux_fill(0.0)
+        for _ in range(400):                       # the boundary flux advances one track per sweep
+            phi = gp.nd_transport_sweep(Q)
+        expect = q0 / xs.sigma_t[0]
+        assert np.abs(phi.cpu().numpy() / expect - 1.0).max() <= 2e-5
+    finally:
+        gp.destroy()
+        tr.destroy()
+
+
+def test_vacuum_rectangle_worked_example_on_gpu():
+    """The worked example of tests/golden/vacuum_rectangle.txt through the CUDA path: homogeneous 2 x 1.5 cm
+    rectangle, Sigma_t = Sigma_a = 1, unit emission density, vacuum on all sides, N_a = 64, 0.01 cm, TY-3, one sweep:
+    the track-volume weighted mean flux is 0.57485289 whatever the triangulation."""
+    import os
+    golden = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "vacuum_rectangle.txt")):
+        if line.strip() and not line.lstrip().startswith("#"):
+            k, v = line.split()[:2]
+            golden[k] = float(v)
+    target = golden["phi_bar"]
+    assert (golden["W"], golden["H"], golden["n_azim"], golden["spacing"], golden["n_polar"]) == (2.0, 1.5, 64, 0.01, 3)
+    mesh = rect_tri_mesh(2.0, 1.5, 6, 5, seed=4, jitter=0.3)
+    mesh.material[:] = 0
+    xs = homogeneous_xs(1, 1)
+    xs.sigma_t[:] = 1.0
+    xs.sigma_s[:] = 0.0
+    xs.nu_sigma_f[:] = 0.0
+    s, w = tabuchi_yamamoto(3)
+    tr = nd.nd_tracks_generate(mesh.xy, mesh.tri, mesh.W, mesh.H, (0, 0, 0, 0), 64, 0.01)
+    gp = nd.nd_problem_create(xs, s, w, mesh.material, tr)
+    try:
+        Q = torch.full((mesh.n_regions, 1), 1.0 / (4.0 * np.pi), dtype=torch.float64, device="cuda")
+        phi = gp.nd_transport_sweep(Q).cpu().numpy()[:, 0]
+        vol = gp.nd_track_volume_get()
+        assert abs(float((phi * vol).sum() / vol.sum()) - target) <= 2e-6
+    finally:
+        gp.destroy()
+        tr.destroy()
