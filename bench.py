@@ -275,19 +275,19 @@ def main():
     # ---- end to end through the C ABI with HOST buffers: H2D phi -> nd_flux_set -> one power iteration -> D2H phi ----
     e2e = None
     if not args.no_e2e:
-        h_in = torch.ones((R, G), dtype=torch.float64).pin_memory()
-        h_out = torch.empty((R, G), dtype=torch.float64).pin_memory()
+        h_bufs = [torch.ones((R, G), dtype=torch.float64).pin_memory(), torch.empty((R, G), dtype=torch.float64).pin_memory()]
         d_in = torch.empty((R, G), dtype=torch.float64, device=dev)
         d_out = torch.empty((R, G), dtype=torch.float64, device=dev)
         k_host = 1.0
 
         def e2e_step(k):
+            h_in, h_out = h_bufs
             d_in.copy_(h_in, non_blocking=True)
             gp.nd_flux_set(d_in, k)
             out = gp.nd_power_iteration(1, d_phi_out=d_out)
             h_out.copy_(d_out, non_blocking=True)
             torch.cuda.synchronize(dev)
-            h_in.copy_(h_out)                      # next step starts from this step's result (host-side state)
+            h_bufs.reverse()                       # next step starts from this step's result (the state lives on the host)
             return out["k_eff"]
 
         for _ in range(2):

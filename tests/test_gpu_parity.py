@@ -288,3 +288,34 @@ def test_vacuum_rectangle_worked_example_on_gpu():
     finally:
         gp.destroy()
         tr.destroy()
+
+
+@pytest.mark.parametrize("case", [(3, 0.3, {}), (4, 0.5, {}), (5, 0.02, {}), (5, 0.01, dict(block_warps=16, tile_segments=6, delta_buffers=2))],
+                         ids=["cfg3", "cfg4", "cfg5", "cfg5-2buf"])
+def test_swath_sweep_is_reproducible(case):
+    """Race check by repetition: the segment chains and the per-tile FP32 sums have a fixed order, so the boundary flux
+    must come back BIT-identical run after run and the tally may differ only by the order of the FP64 REDs.  A
+    shared-memory hazard (staging buffers, delta buffer, barriers) would show up here as run-to-run differences."""
+    idx, scale, opts = case
+    prob = make_config(idx, scale=scale)
+    m = prob.mesh
+    tr = nd.nd_tracks_generate(m.xy, m.tri, m.W, m.H, prob.bc, prob.n_azim, prob.spacing)
+    gp = nd.nd_problem_create(prob.xs, prob.polar_sin, prob.polar_weight, m.material, tr, sweep_kernel=nd.ND_SWEEP_SWATH, **opts)
+    try:
+        rng = np.random.default_rng(77)
+        Q = torch.from_numpy(rng.uniform(0.05, 1.0, size=(m.n_regions, prob.n_groups))).cuda()
+        psi0 = rng.uniform(0.0, 2.0, size=(tr.n_tracks, 2, prob.n_polar, prob.n_groups)).astype(np.float32)
+        ref_psi = ref_tally = None
+        for _ in range(6):
+            gp.nd_boundary_flux_set(psi0)
+            gp.nd_transport_sweep(Q)
+            psi = gp.nd_boundary_flux_get()
+            tally = gp.nd_tally_get().cpu().numpy()
+            if ref_psi is None:
+                ref_psi, ref_tally = psi, tally
+            else:
+                assert np.array_equal(psi, ref_psi), "boundary flux differs between identical runs"
+                assert np.abs(tally - ref_tally).max() <= 1e-12 * np.abs(ref_tally).max()
+    finally:
+        gp.destroy()
+        tr.destroy()
