@@ -228,7 +228,12 @@ nd_status nd_tally_get(nd_problem* p, double* d_tally_out, void* cuda_stream);  
  * stream; nd_profile_read synchronises and returns the accumulated kernel milliseconds and launch counts
  * since the last nd_profile_enable(p,1).  kernels_launched counts every kernel the library launched. */
 typedef struct { double sweep_ms; int64_t sweep_launches; int64_t kernels_launched; } nd_profile;
-nd_status nd_profile_enable(nd_problem* p, int32_t on);
+nd_status nd_profile_enable(nd_problem* p, int32_t on);   /* 0 off, 1 event timing, 2 event timing + the INSTRUMENTED swath kernel */
+/* After sweeps run with nd_profile_enable(p, 2): the share of the swath kernel's warp cycles spent in
+ * [0] staging issue (chunk TMA, q-row cp.async), [1] waiting at the barrier before the segment loop, [2] the segment loop,
+ * [3] waiting for the q rows and at the barrier behind the loop, [4] the tally flush, [5] between tiles (item fetch, psi in /
+ * out).  HOST [6], sums to 1.  The instrumented kernel is a separate build (clock64 marks); its timings are not bench values. */
+nd_status nd_sweep_phases_get(nd_problem* p, double* host_out);
 nd_status nd_profile_read(nd_problem* p, nd_profile* out);
 
 /* Problem facts: padded sizes and the algorithmic byte / update counts DESIGN.md defines. */

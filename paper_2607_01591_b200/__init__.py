@@ -25,7 +25,7 @@ EXPORTS = [
     "nd_tracks_generate", "nd_tracks_device_workspace_bytes", "nd_tracks_generate_device", "nd_tracks_view", "nd_tracks_destroy", "nd_workspace_bytes", "nd_problem_create",
     "nd_problem_destroy", "nd_transport_sweep", "nd_source_update", "nd_power_iteration", "nd_state_reset",
     "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_flux_get", "nd_flux_set",
-    "nd_track_volume_get", "nd_tally_get", "nd_profile_enable", "nd_profile_read", "nd_problem_info_get",
+    "nd_track_volume_get", "nd_tally_get", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
     "nd_swath_stream_build", "nd_swath_stream_view", "nd_swath_stream_destroy",
     "nd_status_string", "nd_last_error", "nd_version",
 ]
@@ -135,6 +135,7 @@ def lib():
         L.nd_tally_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.nd_profile_enable.argtypes = [C.c_void_p, C.c_int32]
         L.nd_profile_read.argtypes = [C.c_void_p, C.POINTER(nd_profile)]
+        L.nd_sweep_phases_get.argtypes = [C.c_void_p, C.c_void_p]
         L.nd_problem_info_get.argtypes = [C.c_void_p, C.POINTER(nd_problem_info)]
         L.nd_swath_stream_build.argtypes = [C.POINTER(nd_problem_desc), C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
                                             C.c_double, C.POINTER(C.c_void_p)]
@@ -360,7 +361,12 @@ class Problem:
         return out
 
     def nd_profile_enable(self, on=True):
-        _check(lib().nd_profile_enable(self._h, 1 if on else 0), "nd_profile_enable")
+        _check(lib().nd_profile_enable(self._h, int(on)), "nd_profile_enable")
+
+    def nd_sweep_phases_get(self):
+        out = np.zeros(6, np.float64)
+        _check(lib().nd_sweep_phases_get(self._h, out.ctypes.data), "nd_sweep_phases_get")
+        return dict(zip(("stage", "wait_before_loop", "segment_loop", "wait_after_loop", "flush", "between_tiles"), out.tolist()))
 
     def nd_profile_read(self):
         pr = nd_profile()

@@ -208,7 +208,7 @@ int select_kernel(const nd_problem_desc* desc, const nd_options& opt, const Priv
 
 struct Layout { // byte offsets into the workspace
     size_t seg_rm, seg_len, trk_off, trk_w, link_src, psi_a, psi_b, q, tally, phi_a, phi_b, Q, reg_mat, vol, sigt, sigsT,
-        nusf, chi, sigt_f, scalars, partial, stats, src_region, src_chunks, blob, tile_chunk, swath_tile0, swath_track, items, counter, total;
+        nusf, chi, sigt_f, scalars, partial, stats, src_region, src_chunks, phase, blob, tile_chunk, swath_tile0, swath_track, items, counter, total;
 };
 
 inline size_t bump(size_t& cur, size_t bytes)
@@ -253,6 +253,7 @@ Layout make_layout(const Dims& d, int max_stats, const PrivConfig& pc_in, const 
     L.scalars = bump(c, sizeof(double) * ndk::SC_COUNT);
     L.partial = bump(c, sizeof(double) * 3 * kReduceBlocks);
     L.stats = bump(c, sizeof(double) * 4 * (size_t)max_stats);
+    L.phase = bump(c, 256);
     L.src_region = bump(c, sizeof(int32_t) * (size_t)d.R);
     L.src_chunks = bump(c, sizeof(int4) * ((size_t)d.R / 4 + (size_t)d.M + 1));   // chunks hold >= 4 regions except one per material
     if (pc.feasible) {
@@ -324,7 +325,8 @@ struct nd_problem {
     std::vector<double> h_vol;
     float c[ndk::kMaxPolar]{}, inv_sin[ndk::kMaxPolar]{}, wp[ndk::kMaxPolar]{};
     // profiling
-    bool profile = false;
+    bool profile = false, phase_profile = false;
+    unsigned long long* phase = nullptr;   // [kSwathPhases] device counters of the instrumented swath kernel
     std::vector<EventPair> ev_pool;
     size_t ev_used = 0;
     int64_t kernels_launched = 0;
@@ -416,7 +418,10 @@ nd_status launch_swath_p(nd_problem* p, const ndk::SwathParams& prm, cudaStream_
     const SwathConfig& c = p->sc;
     const bool expm1 = p->opt.exp_mode == ND_EXP_EXPM1;
     const bool tight = c.tight && !expm1;   // the expm1f cross-check path keeps the roomy register budget
-    auto kern = expm1 ? ndk::k_sweep_swath<P, 1, 0> : (tight ? ndk::k_sweep_swath<P, 0, 1> : ndk::k_sweep_swath<P, 0, 0>);
+    const bool prof = p->phase_profile && !expm1;   // instrumented build: clock64 marks around the phases of a tile
+    auto kern = expm1 ? ndk::k_sweep_swath<P, 1, 0, 0>
+                      : (tight ? (prof ? ndk::k_sweep_swath<P, 0, 1, 1> : ndk::k_sweep_swath<P, 0, 1, 0>)
+                               : (prof ? ndk::k_sweep_swath<P, 0, 0, 1> : ndk::k_sweep_swath<P, 0, 0, 0>));
     ND_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes));
     kern<<<swath_grid(p), 32 * c.warps, c.smem_bytes, st>>>(prm);
     ND_LAUNCH_CHECK(p);
@@ -442,6 +447,7 @@ nd_status launch_swath(nd_problem* p, const double* scale_div, cudaStream_t st)
     }
     prm.magic_per_row = ndk::fastdiv_magic((uint32_t)(c.sp.NC * (d.Gs / 4)));
     prm.magic_nq = ndk::fastdiv_magic((uint32_t)(d.Gs / 4));
+    prm.phase = p->phase;
     ND_CUDA(cudaMemsetAsync(p->counter, 0, sizeof(int), st));
     switch (d.P) {
     case 1: return launch_swath_p<1>(p, prm, st);
@@ -706,6 +712,7 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     p->sigt = (double*)(ws + L.sigt); p->sigsT = (double*)(ws + L.sigsT); p->nusf = (double*)(ws + L.nusf);
     p->chi = (double*)(ws + L.chi); p->sigt_f = (float*)(ws + L.sigt_f);
     p->scalars = (double*)(ws + L.scalars); p->partial = (double*)(ws + L.partial); p->stats = (double*)(ws + L.stats);
+    p->phase = (unsigned long long*)(ws + L.phase);
     p->src_region = (int32_t*)(ws + L.src_region); p->src_chunks = (int4*)(ws + L.src_chunks);
     if (tiled) {
         p->blob = (uint8_t*)(ws + L.blob); p->tile_chunk = (uint32_t*)(ws + L.tile_chunk); p->swath_tile0 = (int64_t*)(ws + L.swath_tile0);
@@ -1000,8 +1007,10 @@ extern "C" nd_status nd_profile_enable(nd_problem* p, int32_t on)
 {
     if (!p) return nd_fail(ND_ERR_NULL, "nd_profile_enable: NULL problem");
     p->profile = on != 0;
+    p->phase_profile = on == 2 && p->sweep_kernel == ND_SWEEP_SWATH;
     p->ev_used = 0;
     p->kernels_launched = 0;
+    if (p->phase_profile) ND_CUDA(cudaMemset(p->phase, 0, sizeof(unsigned long long) * ndk::kSwathPhases));
     return ND_OK;
 }
 
@@ -1018,6 +1027,19 @@ extern "C" nd_status nd_profile_read(nd_problem* p, nd_profile* out)
     out->sweep_ms = ms;
     out->sweep_launches = (int64_t)p->ev_used;
     out->kernels_launched = p->kernels_launched;
+    return ND_OK;
+}
+
+extern "C" nd_status nd_sweep_phases_get(nd_problem* p, double* host_out)
+{
+    if (!p || !host_out) return nd_fail(ND_ERR_NULL, "nd_sweep_phases_get: NULL argument");
+    if (!p->phase_profile) return nd_fail(ND_ERR_STATE, "nd_sweep_phases_get: call nd_profile_enable(p, 2) on a swath-kernel problem first");
+    unsigned long long h[ndk::kSwathPhases];
+    ND_CUDA(cudaDeviceSynchronize());
+    ND_CUDA(cudaMemcpy(h, p->phase, sizeof h, cudaMemcpyDeviceToHost));
+    double tot = 0.0;
+    for (int i = 0; i < ndk::kSwathPhases; ++i) tot += (double)h[i];
+    for (int i = 0; i < ndk::kSwathPhases; ++i) host_out[i] = tot > 0.0 ? (double)h[i] / tot : 0.0;
     return ND_OK;
 }
 

@@ -49,7 +49,11 @@ struct SwathParams {
     float c[kMaxPolar], inv_sin[kMaxPolar], wp[kMaxPolar];
     unsigned long long c2[kMaxPolar];          // {c[p], c[p]} packed for the FP32x2 path
     uint32_t magic_per_row, magic_nq;          // fastdiv constants of NC*Gs/4 and Gs/4
+    unsigned long long* phase;                 // PROF builds: [kSwathPhases] warp-cycle sums (lane 0 of every warp)
 };
+
+// phases of the instrumented build (nd_profile_enable(p, 2)): where the warps' cycles go
+enum { PH_STAGE = 0, PH_WAIT_A, PH_COMPUTE, PH_WAIT_B, PH_FLUSH, PH_ITEM, kSwathPhases };
 
 constexpr int kSwathChunkBufs = 4;
 
@@ -218,9 +222,15 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
 }
 
 // TIGHT = 1 caps the registers at 85 (768 resident threads per SM: three 256-thread or two 384-thread blocks).
-template <int P, int EXPM, int TIGHT>
+template <int P, int EXPM, int TIGHT, int PROF>
 __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swath(const SwathParams prm)
 {
+    long long ph[kSwathPhases] = {0, 0, 0, 0, 0, 0};
+    long long t_mark = PROF ? clock64() : 0;
+    int prof_sink = 0;
+    auto mark = [&](int phase) {   // PROF: charge the cycles since the last mark to `phase`
+        if (PROF) { const long long now = clock64(); ph[phase] += now - t_mark; t_mark = now; }
+    };
     extern __shared__ __align__(128) unsigned char smem_sw[];
     unsigned char* const smem = smem_sw;
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);              // [kSwathChunkBufs] chunk-arrival barriers
@@ -335,6 +345,7 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
         __syncthreads();
 
         for (int k = 0; k < nt; ++k) {
+            mark(PH_ITEM);
             const uint32_t s = seq + k;
             const unsigned char* cb = chunk_s + (size_t)(s % kSwathChunkBufs) * prm.chunk_cap;
             // ---- stage ahead: q rows of tile k+1 (its chunk landed a tile ago), chunk of tile k+2 ----
@@ -344,7 +355,10 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
             }
             cp_async_commit_group();
             if (tid == 0 && k + 2 < nt) issue_chunk(k + 2);
+            mark(PH_STAGE);
             if (prm.ndbuf == 1) __syncthreads();   // single delta buffer: the previous tile's flush must be over
+            if (PROF) prof_sink += *s_item;        // BAR.SYNC defers its blocking to the next consumer: make one here
+            mark(PH_WAIT_A);
             const SwathChunk ch = decode_chunk(cb);
             unsigned char* dbuf = dbuf_s + (size_t)(prm.ndbuf == 1 ? 0u : (s & 1u)) * dbuf_bytes;
             // ---- segment loop of this slot's track through the tile ----
@@ -360,8 +374,11 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
                 const int d_step = jstep * line;
                 segment_loop<P, EXPM>(psi, wpt, prm, ch.rec + s0 + j_c, jstep, cnt, steps, lane_ok, q_lane, sigt_lane, d_ptr, d_step);
             }
+            mark(PH_COMPUTE);
             cp_async_wait_all();   // this thread's q-row copies for tile k+1
             __syncthreads();
+            if (PROF) prof_sink += *s_item;
+            mark(PH_WAIT_B);
             // ---- flush: one FP64 RED per (region, group) of the tile ----
             if (f_ok) {
                 for (int l = f_l0; l < ch.L; l += f_lstep) {
@@ -379,6 +396,7 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
                     if (gq + 3 < prm.G) atomicAdd(tp + 3, (double)v.w);
                 }
             }
+            mark(PH_FLUSH);
         }
         seq += (uint32_t)nt;
         // ---- psi leaves the registers ----
@@ -388,6 +406,12 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
                 *reinterpret_cast<float4*>(prm.psi_out + psi_at + (size_t)p * Gs) = make_float4(psi[p][0], psi[p][1], psi[p][2], psi[p][3]);
         }
         __syncthreads();   // s_item may be rewritten; the last flush is over before the next item's staging
+    }
+    if (PROF) {
+        mark(PH_ITEM);
+        if (prof_sink == 0x7fffffff) prm.phase[kSwathPhases] = 1ull;   // keeps the sink alive
+        if ((tid & 31) == 0)
+            for (int i = 0; i < kSwathPhases; ++i) atomicAdd(prm.phase + i, (unsigned long long)ph[i]);
     }
 }
 

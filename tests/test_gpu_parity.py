@@ -319,3 +319,20 @@ def test_swath_sweep_is_reproducible(case):
     finally:
         gp.destroy()
         tr.destroy()
+
+
+def test_phase_profile_of_the_instrumented_swath_kernel():
+    pair = make_pair(4, 0.06, sweep_kernel=nd.ND_SWEEP_SWATH)
+    try:
+        with pytest.raises(nd.NdError, match="ND_ERR_STATE"):
+            pair.gpu.nd_sweep_phases_get()
+        ko, *_ = pair.oracle_power(4)
+        pair.gpu.nd_profile_enable(2)
+        out = pair.gpu.nd_power_iteration(4)           # the instrumented build computes the same thing
+        assert abs(out["k_eff"] - ko) * 1e5 <= K_PCM
+        ph = pair.gpu.nd_sweep_phases_get()
+        assert abs(sum(ph.values()) - 1.0) < 1e-9 and all(v >= 0.0 for v in ph.values())
+        assert ph["segment_loop"] == max(ph.values())
+        pair.gpu.nd_profile_enable(0)
+    finally:
+        pair.close()
