@@ -69,8 +69,10 @@ enum {
     ND_SWEEP_AUTO = 0,      /* the fastest validated kernel for this G,P */
     ND_SWEEP_ATOMIC = 1,    /* warp per (track,direction), lanes over groups, FP64 global atomics per segment */
     ND_SWEEP_PRIVATE = 2,   /* lane-group per track batch, FP32 shared-memory private tally window, FP64 flush */
-    ND_SWEEP_SWATH = 3      /* thread block per swath of adjacent tracks, psi in registers along the whole track,
+    ND_SWEEP_SWATH = 3,     /* thread block per swath of adjacent tracks, psi in registers along the whole track,
                                per-segment delta rows in shared memory, one FP64 RED per (region, group) per tile */
+    ND_SWEEP_SWATH_WS = 4   /* the swath kernel warp-specialised: compute warps run only the segment loop, service warps
+                               stage the tiles and flush the tallies one tile behind, meeting at mbarriers */
 };
 
 typedef struct {
@@ -84,7 +86,9 @@ typedef struct {
     int32_t blocks_per_sm;  /* ND_SWEEP_SWATH: resident blocks per SM the grid is sized for; 0 = default */
     int32_t tile_lag;       /* ND_SWEEP_SWATH: drift of the track fronts (in mean segment lengths) under which a tile gives
                                every track the same number of segments; 0 = default, -1 = always cut geometrically */
-    int32_t reserved[7];    /* must be 0 */
+    int32_t service_warps;  /* ND_SWEEP_SWATH_WS: staging + flush warps per block (block_warps then counts the compute warps;
+                               compute + service <= 12); 0 = default */
+    int32_t reserved[6];    /* must be 0 */
 } nd_options;
 
 /* ------------------------------------------------------------------------------------------------

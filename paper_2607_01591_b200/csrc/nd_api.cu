@@ -3,6 +3,7 @@
 // entry point launches CUDA kernels and returns ND_ERR_CUDA if that fails.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -15,6 +16,7 @@
 #include "nd_kernels.cuh"
 #include "nd_sweep_private.cuh"
 #include "nd_sweep_swath.cuh"
+#include "nd_sweep_swath_ws.cuh"
 #include "nd_swath.h"
 #include "nd_tiles.h"
 
@@ -116,24 +118,30 @@ PrivConfig make_priv_config(const Dims& d, const nd_options& opt)
 struct SwathConfig {
     bool feasible = false;
     NdSwathParams sp{};
-    int LPT = 0, warps = 0, ndbuf = 1, blocks_per_sm = 1;
+    int LPT = 0, warps = 0, nsw = 0, ndbuf = 1, blocks_per_sm = 1;
     bool tight = false;                                   // register-capped kernel variant (more than 512 resident threads per SM)
     int chunk_cap = 0, off_sigt = 0, off_q = 0, off_dbuf = 0, off_chunk = 0, smem_bytes = 0;
     int64_t max_tiles = 0, max_swaths = 0;
     size_t max_blob = 0;
 };
 
-SwathConfig make_swath_config(const Dims& d, const nd_options& opt)
+inline bool is_swath(int kernel) { return kernel == ND_SWEEP_SWATH || kernel == ND_SWEEP_SWATH_WS; }
+constexpr int kServiceWarps = 5;   // ND_SWEEP_SWATH_WS: staging + flush warps per block (measured best with 7 compute warps at G = 51)
+
+// ws: the warp-specialised variant -- `warps` counts COMPUTE warps, two delta buffers, two blocks of <= 384 threads per SM
+SwathConfig make_swath_config(const Dims& d, const nd_options& opt, bool ws = false)
 {
     SwathConfig c;
+    c.nsw = ws ? (opt.service_warps > 0 ? (opt.service_warps > 8 ? 8 : opt.service_warps) : kServiceWarps) : 0;
     c.LPT = d.Gs / 4;
     if (c.LPT > 32) return c;
     const int NC = (c.LPT == 1 || c.LPT == 2 || c.LPT == 4) ? 8 / c.LPT : 1;
     const int row_bytes = 4 * d.Gs, line = NC * row_bytes;
     if ((int64_t)d.M * line > 65536) return c;
-    int warps = opt.block_warps > 0 ? opt.block_warps : (c.LPT > 8 ? 8 : 4);
+    int warps = opt.block_warps > 0 ? opt.block_warps : (ws ? 12 - c.nsw : (c.LPT > 8 ? 8 : 4));
     if (warps > 16) warps = 16;
-    c.ndbuf = opt.delta_buffers == 2 ? 2 : 1;
+    if (ws && warps > 12 - c.nsw) warps = 12 - c.nsw;
+    c.ndbuf = (ws || opt.delta_buffers == 2) ? 2 : 1;
     auto pad128 = [](int x) { return (x + 127) / 128 * 128; };
     auto layout = [&](int w, int Kmax, int Lmax) -> bool {   // fills c for (w, Kmax, Lmax); false if the slot count is unusable
         const int NT = w * 32 / c.LPT / NC * NC;               // slots are packed over the lanes of the whole block
@@ -155,7 +163,7 @@ SwathConfig make_swath_config(const Dims& d, const nd_options& opt)
     // Defaults (measured, profiles/): occupancy beats tile length once a tile holds >= 8 segments per track.  Aim at
     // 3 resident blocks per SM (4 for narrow rows), the longest tile that fits, and a region window sized for the
     // tally re-use the configs show (rho ~ 6.5 wide rows, ~ 8 narrow rows).
-    const int target_blocks = row_bytes < 64 ? 4 : 3;
+    const int target_blocks = ws ? 2 : (row_bytes < 64 ? 4 : 3);
     if (opt.block_warps <= 0) {
         // small problems: fewer tracks per block until there are about two work items (swath, direction) per resident
         // block of a 148-SM part -- the sweep of a small problem is bound by its longest track, not by throughput
@@ -183,7 +191,8 @@ SwathConfig make_swath_config(const Dims& d, const nd_options& opt)
     if (!placed) return c;
     c.warps = warps;
     int bps = (kSmemMax + 1024) / (c.smem_bytes + 1024);  // 1 KB per block is reserved by the driver
-    if (bps * warps * 32 > 768) bps = 768 / (warps * 32);  // 85 registers per thread at most
+    if (ws && bps > 2) bps = 2;
+    if (!ws && bps * warps * 32 > 768) bps = 768 / (warps * 32);  // 85 registers per thread at most
     if (bps > 8) bps = 8;
     if (bps < 1) bps = 1;
     if (opt.blocks_per_sm > 0 && opt.blocks_per_sm < bps) bps = opt.blocks_per_sm;
@@ -200,7 +209,7 @@ SwathConfig make_swath_config(const Dims& d, const nd_options& opt)
 // Which sweep kernel a descriptor + options select (decided before the workspace is sized).
 int select_kernel(const nd_problem_desc* desc, const nd_options& opt, const PrivConfig& pc, const SwathConfig& sc)
 {
-    if (opt.sweep_kernel == ND_SWEEP_SWATH && sc.feasible) return ND_SWEEP_SWATH;
+    if (is_swath(opt.sweep_kernel) && sc.feasible) return opt.sweep_kernel;
     if (opt.sweep_kernel == ND_SWEEP_PRIVATE && pc.feasible) return ND_SWEEP_PRIVATE;
     if (opt.sweep_kernel == ND_SWEEP_AUTO && desc->track_ends && sc.feasible) return ND_SWEEP_SWATH;
     return ND_SWEEP_ATOMIC;
@@ -222,8 +231,8 @@ Layout make_layout(const Dims& d, int max_stats, const PrivConfig& pc_in, const 
 {
     // the tiled kernels share the stream fields of the layout; size them for the selected one
     PrivConfig pc = pc_in;
-    pc.feasible = kernel == ND_SWEEP_PRIVATE || kernel == ND_SWEEP_SWATH;
-    if (kernel == ND_SWEEP_SWATH) {
+    pc.feasible = kernel == ND_SWEEP_PRIVATE || is_swath(kernel);
+    if (is_swath(kernel)) {
         pc.max_blob = sc.max_blob; pc.max_tiles = sc.max_tiles; pc.max_swaths = sc.max_swaths; pc.tp.B = sc.sp.NT;
     }
     Layout L{};
@@ -449,6 +458,23 @@ nd_status launch_swath(nd_problem* p, const double* scale_div, cudaStream_t st)
     prm.magic_nq = ndk::fastdiv_magic((uint32_t)(d.Gs / 4));
     prm.phase = p->phase;
     ND_CUDA(cudaMemsetAsync(p->counter, 0, sizeof(int), st));
+    if (p->sweep_kernel == ND_SWEEP_SWATH_WS) {
+        ndk::SwathWsParams wsp{};
+        wsp.base = prm; wsp.ncw = c.warps; wsp.nsw = c.nsw;
+        const int threads = 32 * (c.warps + c.nsw);
+        auto launch = [&](auto kern) -> nd_status {
+            ND_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes));
+            kern<<<swath_grid(p), threads, c.smem_bytes, st>>>(wsp);
+            ND_LAUNCH_CHECK(p);
+            return ND_OK;
+        };
+        switch (d.P) {
+        case 1: return launch(ndk::k_sweep_swath_ws<1>);
+        case 2: return launch(ndk::k_sweep_swath_ws<2>);
+        case 3: return launch(ndk::k_sweep_swath_ws<3>);
+        default: return launch(ndk::k_sweep_swath_ws<4>);
+        }
+    }
     switch (d.P) {
     case 1: return launch_swath_p<1>(p, prm, st);
     case 2: return launch_swath_p<2>(p, prm, st);
@@ -510,7 +536,7 @@ nd_status launch_sweep(nd_problem* p, const double* scale_div, cudaStream_t st)
         ND_CUDA(cudaEventRecord(ev->a, st));
     }
     nd_status rc;
-    if (p->sweep_kernel == ND_SWEEP_SWATH) {
+    if (is_swath(p->sweep_kernel)) {
         rc = launch_swath(p, scale_div, st);
     } else if (p->sweep_kernel == ND_SWEEP_PRIVATE) {
         rc = launch_private(p, scale_div, st);
@@ -574,7 +600,7 @@ extern "C" nd_status nd_workspace_bytes(const nd_problem_desc* desc, const nd_op
     PrivConfig pc;
     SwathConfig sc;
     if (opt.sweep_kernel == ND_SWEEP_PRIVATE) pc = make_priv_config(d, opt);
-    if (opt.sweep_kernel == ND_SWEEP_SWATH || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt);
+    if (is_swath(opt.sweep_kernel) || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt, opt.sweep_kernel == ND_SWEEP_SWATH_WS);
     *device_bytes = make_layout(d, kMaxStats, pc, sc, select_kernel(desc, opt, pc, sc)).total;
     return ND_OK;
 }
@@ -592,19 +618,19 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     if (rc != ND_OK) return rc;
     nd_options opt{};
     if (opts) opt = *opts;
-    for (int i = 0; i < 7; ++i)
+    for (int i = 0; i < 6; ++i)
         if (opt.reserved[i] != 0) return nd_fail(ND_ERR_INVALID, "nd_options.reserved must be zero");
     if (opt.exp_mode != ND_EXP_FAST && opt.exp_mode != ND_EXP_EXPM1) return nd_fail(ND_ERR_INVALID, "unknown exp_mode");
-    if (opt.sweep_kernel < ND_SWEEP_AUTO || opt.sweep_kernel > ND_SWEEP_SWATH) return nd_fail(ND_ERR_INVALID, "unknown sweep_kernel");
+    if (opt.sweep_kernel < ND_SWEEP_AUTO || opt.sweep_kernel > ND_SWEEP_SWATH_WS) return nd_fail(ND_ERR_INVALID, "unknown sweep_kernel");
     if (opt.track_batch < 0 || opt.window_regions < 0 || opt.block_warps < 0 || opt.tile_segments < 0 || opt.delta_buffers < 0 ||
-        opt.delta_buffers > 2 || opt.blocks_per_sm < 0 || opt.tile_lag < -1)
+        opt.delta_buffers > 2 || opt.blocks_per_sm < 0 || opt.tile_lag < -1 || opt.service_warps < 0)
         return nd_fail(ND_ERR_INVALID, "nd_options: tuning fields must be >= 0 (delta_buffers 0, 1 or 2)");
     if ((desc->track_azim == nullptr) != (desc->track_ends == nullptr))
         return nd_fail(ND_ERR_INVALID, "track_azim and track_ends must both be set or both be NULL");
     PrivConfig pc;
     SwathConfig sc;
     if (opt.sweep_kernel == ND_SWEEP_PRIVATE) pc = make_priv_config(d, opt);
-    if (opt.sweep_kernel == ND_SWEEP_SWATH || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt);
+    if (is_swath(opt.sweep_kernel) || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt, opt.sweep_kernel == ND_SWEEP_SWATH_WS);
     const int kernel = select_kernel(desc, opt, pc, sc);
     const Layout L = make_layout(d, kMaxStats, pc, sc, kernel);
     if (reinterpret_cast<uintptr_t>(device_workspace) % kAlign != 0) return nd_fail(ND_ERR_WORKSPACE, "workspace must be 256-byte aligned");
@@ -681,7 +707,7 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     // ---- A1 (fast path): swath/tile chunk stream for the private-tally sweep ----
     NdTileSet tiles;
     NdSwathSet swaths;
-    const bool want_private = kernel == ND_SWEEP_PRIVATE, want_swath = kernel == ND_SWEEP_SWATH;
+    const bool want_private = kernel == ND_SWEEP_PRIVATE, want_swath = is_swath(kernel);
     const bool tiled = want_private || want_swath;
     if (want_swath) {
         rc = nd_build_swaths(desc, desc->track_azim, desc->track_ends, sc.sp, 0, &swaths);
@@ -1060,8 +1086,8 @@ extern "C" nd_status nd_problem_info_get(const nd_problem* p, nd_problem_info* o
     out->mean_regions_per_tile = p->mean_regions_per_tile;
     out->mean_segments_per_tile = p->mean_segments_per_tile;
     out->lockstep_efficiency = p->lockstep_efficiency;
-    if (p->sweep_kernel == ND_SWEEP_SWATH) {
-        out->block_threads = 32 * p->sc.warps; out->smem_bytes = p->sc.smem_bytes; out->grid_blocks = swath_grid(p);
+    if (is_swath(p->sweep_kernel)) {
+        out->block_threads = 32 * (p->sc.warps + p->sc.nsw); out->smem_bytes = p->sc.smem_bytes; out->grid_blocks = swath_grid(p);
         out->tracks_per_block = p->sc.sp.NT;
     } else if (p->sweep_kernel == ND_SWEEP_PRIVATE) {
         out->block_threads = 32 * p->pc.warps; out->smem_bytes = p->pc.smem_bytes; out->grid_blocks = p->n_sm;

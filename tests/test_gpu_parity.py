@@ -15,7 +15,7 @@ from gpu_common import Pair, make_pair, seeded_sweep_inputs, phi_rel_err, PHI_RT
 pytestmark = pytest.mark.gpu
 
 KERNELS = [pytest.param(nd.ND_SWEEP_ATOMIC, id="atomic"), pytest.param(nd.ND_SWEEP_PRIVATE, id="private"),
-           pytest.param(nd.ND_SWEEP_SWATH, id="swath")]
+           pytest.param(nd.ND_SWEEP_SWATH, id="swath"), pytest.param(nd.ND_SWEEP_SWATH_WS, id="wsp")]
 
 # (config index, scale): sizes the oracle finishes in seconds, spanning several tiles and ragged tails
 SWEEP_CASES = [(1, 1.0), (2, 0.15), (2, 1.0), (3, 0.03), (4, 0.06), (5, 0.0008)]
@@ -63,6 +63,19 @@ def test_swath_block_and_tile_shapes(case, shape):
         info = pair.gpu.nd_problem_info_get()
         assert info["sweep_kernel"] == nd.ND_SWEEP_SWATH and 32 <= info["block_threads"] <= 32 * shape["block_warps"]
         _check_sweep(pair, seed=300 + case[0])
+    finally:
+        pair.close()
+
+
+@pytest.mark.parametrize("shape", [dict(block_warps=8, service_warps=4), dict(block_warps=2, service_warps=1, tile_segments=3),
+                                   dict(block_warps=6, service_warps=6, tile_segments=16, window_regions=24)], ids=["8+4", "2+1", "6+6"])
+@pytest.mark.parametrize("case", [(2, 0.15), (4, 0.06), (5, 0.0008)], ids=["cfg2", "cfg4", "cfg5"])
+def test_warp_specialised_block_shapes(case, shape):
+    pair = make_pair(case[0], case[1], sweep_kernel=nd.ND_SWEEP_SWATH_WS, **shape)
+    try:
+        info = pair.gpu.nd_problem_info_get()
+        assert info["sweep_kernel"] == nd.ND_SWEEP_SWATH_WS and info["block_threads"] <= 384
+        _check_sweep(pair, seed=500 + case[0], n_sweeps=3)
     finally:
         pair.close()
 
