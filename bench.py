@@ -316,10 +316,13 @@ def main():
     sweep_ms = prof["sweep_ms"] / max(1, prof["sweep_launches"])
     achieved = info["algorithmic_bytes"] / (sweep_ms * 1e-3) / 1e9
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "sweep_traffic.json")
-    if os.path.exists(tpath):
-        tj = json.load(open(tpath))
-        traffic = tj.get(f"config{args.config}", {}).get("dram_bytes_per_launch") if args.scale == 1.0 else None
+    # DRAM bytes of one sweep launch as ncu saw them (profiles/r01b_sweep_traffic.csv, from the --set full captures)
+    tpath = os.path.join(ROOT, "profiles", "r01b_sweep_traffic.csv")
+    if os.path.exists(tpath) and args.scale == 1.0 and info["sweep_kernel"] == 3:
+        for row in open(tpath).read().split("\n")[1:]:
+            f = row.split(",")
+            if len(f) == 5 and f[0] == str(args.config):
+                traffic = int(f[4])
     # The sweep is bound by the exp pipe, not by HBM: one update = one MUFU.EX2, and the SM issues
     # 16 of them per clock -> peak = 148 SMs x 16 x max SM clock.  The HBM view (algorithmic bytes / kernel time against
     # the measured copy bandwidth, and the DRAM traffic ncu saw) is reported beside it.
