@@ -223,6 +223,10 @@ nd_status nd_state_reset(nd_problem* p, void* cuda_stream);                     
 nd_status nd_boundary_flux_fill(nd_problem* p, float value, void* cuda_stream);
 nd_status nd_boundary_flux_get(nd_problem* p, float* host_out, void* cuda_stream);       /* HOST [T][2][P][G] */
 nd_status nd_boundary_flux_set(nd_problem* p, const float* host_in, void* cuda_stream);  /* HOST [T][2][P][G] */
+/* The flux LEAVING every track end in the last sweep, [t][d] = exit of track t swept in direction d, before the link
+ * table is applied (vacuum exits included): with the entering flux it closes the telescoping balance
+ * sum_r tally[r][g] = sum_{t,d,p} w_{t,p} (psi_in - psi_out)[g] at any problem size. */
+nd_status nd_outgoing_flux_get(nd_problem* p, float* host_out, void* cuda_stream);       /* HOST [T][2][P][G] */
 nd_status nd_flux_get(nd_problem* p, double* d_phi_out, void* cuda_stream);        /* DEVICE [R][G] */
 nd_status nd_flux_set(nd_problem* p, const double* d_phi, double k_eff, void* cuda_stream);
 nd_status nd_track_volume_get(nd_problem* p, double* host_out);                    /* HOST [R] */

@@ -24,7 +24,7 @@ ND_SWEEP_AUTO, ND_SWEEP_ATOMIC, ND_SWEEP_PRIVATE, ND_SWEEP_SWATH, ND_SWEEP_SWATH
 EXPORTS = [
     "nd_tracks_generate", "nd_tracks_device_workspace_bytes", "nd_tracks_generate_device", "nd_tracks_view", "nd_tracks_destroy", "nd_workspace_bytes", "nd_problem_create",
     "nd_problem_destroy", "nd_transport_sweep", "nd_source_update", "nd_power_iteration", "nd_state_reset",
-    "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_flux_get", "nd_flux_set",
+    "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_outgoing_flux_get", "nd_flux_get", "nd_flux_set",
     "nd_track_volume_get", "nd_tally_get", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
     "nd_swath_stream_build", "nd_swath_stream_view", "nd_swath_stream_destroy",
     "nd_status_string", "nd_last_error", "nd_version",
@@ -129,6 +129,7 @@ def lib():
         L.nd_boundary_flux_fill.argtypes = [C.c_void_p, C.c_float, C.c_void_p]
         L.nd_boundary_flux_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.nd_boundary_flux_set.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nd_outgoing_flux_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.nd_flux_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.nd_flux_set.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         L.nd_track_volume_get.argtypes = [C.c_void_p, C.c_void_p]
@@ -335,6 +336,11 @@ class Problem:
     def nd_boundary_flux_get(self):
         out = np.empty((self.T, 2, self.P, self.G), np.float32)
         _check(lib().nd_boundary_flux_get(self._h, out.ctypes.data, self._stream()), "nd_boundary_flux_get")
+        return out
+
+    def nd_outgoing_flux_get(self):
+        out = np.empty((self.T, 2, self.P, self.G), np.float32)
+        _check(lib().nd_outgoing_flux_get(self._h, out.ctypes.data, self._stream()), "nd_outgoing_flux_get")
         return out
 
     def nd_boundary_flux_set(self, psi):

@@ -982,6 +982,17 @@ extern "C" nd_status nd_boundary_flux_get(nd_problem* p, float* host_out, void* 
     return ND_OK;
 }
 
+extern "C" nd_status nd_outgoing_flux_get(nd_problem* p, float* host_out, void* cuda_stream)
+{
+    if (!p || !host_out) return nd_fail(ND_ERR_NULL, "nd_outgoing_flux_get: NULL argument");
+    cudaStream_t st = as_stream(cuda_stream);
+    const Dims& d = p->d;
+    const size_t rows = (size_t)d.T * 2 * d.P;
+    ND_CUDA(cudaMemcpy2DAsync(host_out, sizeof(float) * d.G, p->psi_out, sizeof(float) * d.Gs, sizeof(float) * d.G, rows, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaStreamSynchronize(st));
+    return ND_OK;
+}
+
 extern "C" nd_status nd_boundary_flux_set(nd_problem* p, const float* host_in, void* cuda_stream)
 {
     if (!p || !host_in) return nd_fail(ND_ERR_NULL, "nd_boundary_flux_set: NULL argument");

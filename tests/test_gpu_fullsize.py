@@ -70,6 +70,12 @@ def test_config5_full_size_sampled_outputs():
         psi_g = gp.nd_boundary_flux_get().reshape(2 * T, P, G)
         vol = gp.nd_track_volume_get()
         assert np.isfinite(phi_g).all() and (phi_g > 0).all()
+        # (0) telescoping balance over the WHOLE problem, per group: what the chains lost is what the regions tallied
+        psi_exit_all = gp.nd_outgoing_flux_get().astype(np.float64)
+        w_tp = 4.0 * np.pi * tr.track_weight[:, None] * (prob.polar_weight * prob.polar_sin)[None, :]      # [T][P]
+        lost = np.einsum("tp,tdpg->g", w_tp, psi.astype(np.float64) - psi_exit_all)
+        assert np.abs(tally_g.sum(axis=0) - lost).max() <= 2e-5 * np.abs(lost).max()
+        del psi_exit_all
         # (a) sampled tracks: the oracle's chain along each track alone; compare where the exit is linked
         tracks = np.unique(np.concatenate([rng.integers(0, T, size=96), [0, T - 1]])).astype(np.int64)
         off, sr, sl, tw = _subset(tr, tracks)

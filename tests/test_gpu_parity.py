@@ -34,6 +34,10 @@ def _check_sweep(pair, seed, n_sweeps=2):
         assert phi_rel_err(phi_g, phi_o) <= PHI_RTOL
         assert np.abs(psi_g - psi_o).max() <= PSI_ATOL_REL * np.abs(psi_o).max()
         # telescoping invariant on the GPU result itself (exact up to FP32 rounding of the chain)
+        if _ == 0:
+            w_tp = 4.0 * np.pi * pair.o_tr.track_weight[:, None] * (pair.prob.polar_weight * pair.prob.polar_sin)[None, :]
+            lost = np.einsum("tp,tdpg->g", w_tp, psi.astype(np.float64) - pair.gpu.nd_outgoing_flux_get().astype(np.float64))
+            assert np.abs(tally_g.sum(axis=0) - lost).max() <= 2e-5 * max(np.abs(lost).max(), 1e-30)
         scale = np.abs(tally_o).max()
         assert np.abs(tally_g - tally_o).max() <= 2e-4 * scale
 
