@@ -38,7 +38,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--kernel", type=int, default=0, help="ND_SWEEP_* (0 auto)")
     ap.add_argument("--exp-mode", type=int, default=0)
-    for name in ("track-batch", "window-regions", "block-warps", "tile-segments", "delta-buffers", "blocks-per-sm", "tile-lag", "service-warps"):
+    for name in ("track-batch", "window-regions", "block-warps", "tile-segments", "delta-buffers", "blocks-per-sm", "tile-lag", "service-warps", "q-copies"):
         ap.add_argument("--" + name, type=int, default=0, help="nd_options tuning field (0 = library default)")
     ap.add_argument("--cpu-seconds", type=float, default=None,
                     help="target CPU time of one oracle sample (default: 15 s for cpu_baseline; --impl reference: 150 s / steps, 2..30 s)")
@@ -230,7 +230,8 @@ def main():
                               sweep_kernel=args.kernel, exp_mode=args.exp_mode, track_batch=args.track_batch,
                               window_regions=args.window_regions, block_warps=args.block_warps,
                               tile_segments=args.tile_segments, delta_buffers=args.delta_buffers,
-                              blocks_per_sm=args.blocks_per_sm, tile_lag=args.tile_lag, service_warps=args.service_warps)
+                              blocks_per_sm=args.blocks_per_sm, tile_lag=args.tile_lag, service_warps=args.service_warps,
+                              q_copies=args.q_copies)
     setup["create_s"] = round(time.time() - t0, 2)
     info = gp.nd_problem_info_get()
     R, G = prob.mesh.n_regions, prob.n_groups

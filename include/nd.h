@@ -88,7 +88,13 @@ typedef struct {
                                every track the same number of segments; 0 = default, -1 = always cut geometrically */
     int32_t service_warps;  /* ND_SWEEP_SWATH_WS: staging + flush warps per block (block_warps then counts the compute warps;
                                compute + service <= 12); 0 = default */
-    int32_t reserved[6];    /* must be 0 */
+    int32_t q_copies;       /* ND_SWEEP_SWATH, rows of <= 16 groups: copies of a staged q row per shared-memory line.  The
+                               Sigma_t table and the delta rows are interleaved NC = 8 / (lanes per track) slots to a line so
+                               that the slots of a warp never meet in a bank; q_copies = NC does the same for the q rows
+                               (NC cp.async copies per region and tile), 1 stages one copy per region (adjacent tracks in the
+                               same region read it as a broadcast, tracks in different regions may conflict).  0 = default
+                               (1); values above NC or not dividing it are rounded down to a divisor of NC */
+    int32_t reserved[5];    /* must be 0 */
 } nd_options;
 
 /* ------------------------------------------------------------------------------------------------

@@ -30,7 +30,9 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
     const int T = desc->n_tracks, R = desc->n_regions, NT = prm.NT, Kmax = prm.Kmax, Lmax = prm.Lmax, NC = prm.NC;
     if (NT < 1 || NT > 1024 || Kmax < 1 || Lmax < 1 || NC < 1 || NT % NC != 0 || prm.row_bytes < 16 || prm.row_bytes % 16 != 0)
         return nd_fail(ND_ERR_INVALID, "swath parameters out of range");
-    const int64_t line = (int64_t)NC * prm.row_bytes;   // bytes between consecutive q / sigma_t rows in shared memory
+    const int64_t line = (int64_t)NC * prm.row_bytes;   // bytes between consecutive sigma_t / delta rows in shared memory
+    const int NCq = prm.NCq > 0 ? prm.NCq : NC;
+    const int64_t line_q = (int64_t)NCq * prm.row_bytes; // bytes between consecutive q rows
     if ((int64_t)Lmax * line > 65536 || (int64_t)desc->n_materials * line > 65536 || (int64_t)NT * Kmax > 65535)
         return nd_fail(ND_ERR_INVALID, "swath parameters: row offsets must fit 16 bits");
     try {
@@ -207,7 +209,7 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
                             uint32_t lenbits;
                             memcpy(&lenbits, &len, 4);
                             rc[2 * o] = lenbits;
-                            rc[2 * o + 1] = (uint32_t)(l * line) | ((uint32_t)(desc->region_material[r] * line) << 16);
+                            rc[2 * o + 1] = (uint32_t)(l * line_q) | ((uint32_t)(desc->region_material[r] * line) << 16);
                             ci[rfill[l]++] = (uint16_t)(((b / NC) * Kmax + j) * NC + b % NC);
                         }
                     }

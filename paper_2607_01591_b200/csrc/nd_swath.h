@@ -33,6 +33,8 @@ struct NdSwathParams {
     double lag;   // >= 0: while the fronts of the swath's tracks lie within `lag` mean segment lengths of each other a
                   // tile gives EVERY track Kmax segments (no idle slot steps); beyond it the tile is cut geometrically
                   // (the track furthest behind advances first) until the fronts are level again.  < 0: always geometric.
+    int NCq = 0;  // copies of a q row per shared line (0: = NC).  1 = one copy per region: adjacent slots in the same region
+                  // read it as a broadcast, slots in different regions may meet in a bank
 };
 
 struct NdSwathItem { int32_t swath, dir, cost, reserved; };

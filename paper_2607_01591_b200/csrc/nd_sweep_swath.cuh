@@ -43,7 +43,7 @@ struct SwathParams {
     const float* __restrict__ psi_in;
     float* __restrict__ psi_out;
     const double* __restrict__ scale_div;
-    int n_items, G, Gs, M, NT, Kmax, Lmax, LPT, NC, ndbuf;
+    int n_items, G, Gs, M, NT, Kmax, Lmax, LPT, NC, NCq, ndbuf;
     int chunk_cap;                             // bytes of one chunk staging buffer
     int off_sigt, off_q, off_dbuf, off_chunk;  // shared-memory byte offsets
     float c[kMaxPolar], inv_sin[kMaxPolar], wp[kMaxPolar];
@@ -236,12 +236,12 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);              // [kSwathChunkBufs] chunk-arrival barriers
     volatile int* s_item = reinterpret_cast<volatile int*>(smem + 64);
     const int tid = threadIdx.x, nthr = blockDim.x;
-    const int Gs = prm.Gs, row_bytes = 4 * Gs, line = prm.NC * row_bytes;
+    const int Gs = prm.Gs, row_bytes = 4 * Gs, line = prm.NC * row_bytes, line_q = prm.NCq * row_bytes;
     unsigned char* sigt_s = smem + prm.off_sigt;
-    unsigned char* q_s = smem + prm.off_q;           // [2][Lmax][line]
+    unsigned char* q_s = smem + prm.off_q;           // [2][Lmax][line_q]
     unsigned char* dbuf_s = smem + prm.off_dbuf;     // [ndbuf][NT/NC * Kmax][line]
     unsigned char* chunk_s = smem + prm.off_chunk;   // [4][chunk_cap]
-    const int q_buf_bytes = prm.Lmax * line;
+    const int q_buf_bytes = prm.Lmax * line_q;
     const int dbuf_bytes = (prm.NT / prm.NC) * prm.Kmax * line;
     const int nq = Gs >> 2;                          // 16-byte pieces per row
 
@@ -267,6 +267,7 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
     const int sub = slot % prm.NC;                    // position of the slot inside a shared line
     const int lane_off = sub * row_bytes + ll * 16;   // byte offset of this lane's 4 groups inside a line
     const unsigned char* sigt_lane = sigt_s + lane_off;
+    const int lane_off_q = (slot % prm.NCq) * row_bytes + ll * 16;
     const int d_slot_off = (slot / prm.NC) * prm.Kmax * line + lane_off;
     const float inv_f = (float)(1.0 / *prm.scale_div);
     const int g0 = ll * 4;
@@ -325,11 +326,11 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
             const int L = (int)(h.x & 0xffffu);
             const uint32_t* regions = reinterpret_cast<const uint32_t*>(cb + 16 * (h.y & 0xffffu));
             const uint32_t qb = smem_u32(q_s + (size_t)(s & 1u) * q_buf_bytes);
-            const int per_row = prm.NC * nq;
+            const int per_row = prm.NCq * nq;
             for (int i = tid; i < L * per_row; i += nthr) {
                 const int l = (int)fastdiv((uint32_t)i, prm.magic_per_row), rem = i - l * per_row;
                 const int piece = rem - (int)fastdiv((uint32_t)rem, prm.magic_nq) * nq;
-                cp_async_16(qb + l * line + rem * 16, prm.q + (size_t)regions[l] * Gs + piece * 4);
+                cp_async_16(qb + l * line_q + rem * 16, prm.q + (size_t)regions[l] * Gs + piece * 4);
             }
         };
         if (nt > 0) {
@@ -366,7 +367,7 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
                 int s0 = 0, cnt = 0;
                 if (t >= 0) { s0 = ch.slot_start[slot]; cnt = ch.slot_start[slot + 1] - s0; }
                 const int steps = __reduce_max_sync(0xffffffffu, cnt);
-                const unsigned char* q_lane = q_s + (size_t)(s & 1u) * q_buf_bytes + lane_off;
+                const unsigned char* q_lane = q_s + (size_t)(s & 1u) * q_buf_bytes + lane_off_q;
                 // segment j (forward index inside the tile) is visited at step i: j = dir ? cnt-1-i : i
                 const int jstep = dir ? -1 : 1;
                 int j_c = dir ? cnt - 1 : 0;                // segment of the current step

@@ -54,7 +54,8 @@ def test_sweep_matches_oracle(case, kernel):
 
 SHAPES = [dict(block_warps=1), dict(block_warps=3, tile_segments=2, window_regions=5), dict(block_warps=8, tile_segments=16),
           dict(block_warps=16, tile_segments=5, delta_buffers=2), dict(block_warps=8, tile_lag=-1), dict(block_warps=4, tile_lag=1000),
-          dict(block_warps=12, tile_segments=12, blocks_per_sm=1)]
+          dict(block_warps=12, tile_segments=12, blocks_per_sm=1), dict(block_warps=4, q_copies=4), dict(block_warps=2, q_copies=2),
+          dict(block_warps=4, q_copies=3, tile_segments=6)]
 
 
 @pytest.mark.parametrize("case", [(2, 0.15), (4, 0.06), (5, 0.0008)], ids=["cfg2", "cfg4", "cfg5"])
