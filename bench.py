@@ -102,17 +102,26 @@ class ClockSampler:
         return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def build_inputs(args):
-    """Seeded synthetic problem + the library's own host ray tracing (not timed)."""
-    import paper_2607_01591_b200 as nd
+def build_inputs(args, tracer="device"):
+    """Seeded synthetic problem + ray tracing (not timed).  tracer = "device": the library's GPU ray walk (row NEXT-1,
+    bit-identical to its host tracer and to the oracle's); "oracle": the oracle's own tracer (reference arm: nothing of
+    the library runs there)."""
     from moc_inputs import make_config
     t0 = time.time()
     prob = make_config(args.config, scale=args.scale)
     m = prob.mesh
     t1 = time.time()
-    tr = nd.nd_tracks_generate(m.xy, m.tri, m.W, m.H, prob.bc, prob.n_azim, prob.spacing)
+    if tracer == "oracle":
+        import oracle
+        tr = oracle.generate_tracks(m.xy, m.tri, m.W, m.H, prob.bc, prob.n_azim, prob.spacing)
+        tr.n_segments = tr.n_segs
+    else:
+        import paper_2607_01591_b200 as nd
+        local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+        tr = nd.nd_tracks_generate_device(m.xy, m.tri, m.W, m.H, prob.bc, prob.n_azim, prob.spacing,
+                                          segment_capacity=1 << 28, device=f"cuda:{local_rank}")
     t2 = time.time()
-    return prob, tr, {"mesh_s": round(t1 - t0, 2), "trace_s": round(t2 - t1, 2)}
+    return prob, tr, {"mesh_s": round(t1 - t0, 2), "trace_s": round(t2 - t1, 2), "tracer": tracer}
 
 
 def oracle_sample(prob, tr, cpu_seconds):
@@ -160,7 +169,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    prob, tr, setup = build_inputs(args)
+    prob, tr, setup = build_inputs(args, tracer="oracle")
     per_step = args.cpu_seconds if args.cpu_seconds else max(2.0, min(30.0, 150.0 / max(1, args.steps + args.warmup)))
     vals, times = [], []
     cb = None
