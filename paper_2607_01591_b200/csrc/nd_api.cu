@@ -129,7 +129,7 @@ inline bool is_swath(int kernel) { return kernel == ND_SWEEP_SWATH || kernel == 
 constexpr int kServiceWarps = 5;   // ND_SWEEP_SWATH_WS: staging + flush warps per block (measured best with 7 compute warps at G = 51)
 
 // ws: the warp-specialised variant -- `warps` counts COMPUTE warps, two delta buffers, two blocks of <= 384 threads per SM
-SwathConfig make_swath_config(const Dims& d, const nd_options& opt, bool ws = false)
+SwathConfig make_swath_config_q(const Dims& d, const nd_options& opt, bool ws, int q_copies)
 {
     SwathConfig c;
     c.nsw = ws ? (opt.service_warps > 0 ? (opt.service_warps > 8 ? 8 : opt.service_warps) : kServiceWarps) : 0;
@@ -137,10 +137,7 @@ SwathConfig make_swath_config(const Dims& d, const nd_options& opt, bool ws = fa
     if (c.LPT > 32) return c;
     const int NC = (c.LPT == 1 || c.LPT == 2 || c.LPT == 4) ? 8 / c.LPT : 1;
     const int row_bytes = 4 * d.Gs, line = NC * row_bytes;
-    // q rows: one copy per region unless asked otherwise (measured: config 3 0.628 -> 0.555 ms, config 2 0.079 -> 0.070 ms);
-    // the warp-specialised variant keeps the replicated rows
-    int NCq = ws ? NC : 1;
-    if (!ws && opt.q_copies > 0) NCq = opt.q_copies;
+    int NCq = q_copies > 0 ? q_copies : NC;
     if (NCq > NC) NCq = NC;
     while (NC % NCq != 0) --NCq;   // rounded down to a divisor of NC
     const int line_q = NCq * row_bytes;
@@ -210,6 +207,18 @@ SwathConfig make_swath_config(const Dims& d, const nd_options& opt, bool ws = fa
     c.max_tiles = nd_swath_max_tiles(c.sp, d.S, d.T);
     c.max_blob = nd_swath_max_blob(c.sp, d.S, d.T);
     c.feasible = true;
+    return c;
+}
+
+// q rows: one copy per region unless asked otherwise (measured: config 3 0.628 -> 0.555 ms, config 2 0.079 -> 0.070 ms).
+// The warp-specialised variant and the register-capped variant of k_sweep_swath are compiled for q rows laid out like
+// the Sigma_t table (NCq = NC, no extra registers): if the one-copy layout ends up on the capped variant the
+// configuration is redone with replicated rows.
+SwathConfig make_swath_config(const Dims& d, const nd_options& opt, bool ws = false)
+{
+    if (ws) return make_swath_config_q(d, opt, true, 0);
+    SwathConfig c = make_swath_config_q(d, opt, false, opt.q_copies > 0 ? opt.q_copies : 1);
+    if (c.feasible && c.tight && c.sp.NCq != c.sp.NC) c = make_swath_config_q(d, opt, false, 0);
     return c;
 }
 

@@ -236,7 +236,8 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);              // [kSwathChunkBufs] chunk-arrival barriers
     volatile int* s_item = reinterpret_cast<volatile int*>(smem + 64);
     const int tid = threadIdx.x, nthr = blockDim.x;
-    const int Gs = prm.Gs, row_bytes = 4 * Gs, line = prm.NC * row_bytes, line_q = prm.NCq * row_bytes;
+    const int Gs = prm.Gs, row_bytes = 4 * Gs, line = prm.NC * row_bytes;
+    const int line_q = TIGHT ? line : prm.NCq * row_bytes;   // the capped variant is only used with NCq == NC
     unsigned char* sigt_s = smem + prm.off_sigt;
     unsigned char* q_s = smem + prm.off_q;           // [2][Lmax][line_q]
     unsigned char* dbuf_s = smem + prm.off_dbuf;     // [ndbuf][NT/NC * Kmax][line]
@@ -267,7 +268,7 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
     const int sub = slot % prm.NC;                    // position of the slot inside a shared line
     const int lane_off = sub * row_bytes + ll * 16;   // byte offset of this lane's 4 groups inside a line
     const unsigned char* sigt_lane = sigt_s + lane_off;
-    const int lane_off_q = (slot % prm.NCq) * row_bytes + ll * 16;
+    const int lane_off_q = TIGHT ? lane_off : (slot % prm.NCq) * row_bytes + ll * 16;
     const int d_slot_off = (slot / prm.NC) * prm.Kmax * line + lane_off;
     const float inv_f = (float)(1.0 / *prm.scale_div);
     const int g0 = ll * 4;
@@ -326,7 +327,7 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
             const int L = (int)(h.x & 0xffffu);
             const uint32_t* regions = reinterpret_cast<const uint32_t*>(cb + 16 * (h.y & 0xffffu));
             const uint32_t qb = smem_u32(q_s + (size_t)(s & 1u) * q_buf_bytes);
-            const int per_row = prm.NCq * nq;
+            const int per_row = (TIGHT ? prm.NC : prm.NCq) * nq;
             for (int i = tid; i < L * per_row; i += nthr) {
                 const int l = (int)fastdiv((uint32_t)i, prm.magic_per_row), rem = i - l * per_row;
                 const int piece = rem - (int)fastdiv((uint32_t)rem, prm.magic_nq) * nq;
