@@ -93,7 +93,8 @@ typedef struct {
                                that the slots of a warp never meet in a bank; q_copies = NC does the same for the q rows
                                (NC cp.async copies per region and tile), 1 stages one copy per region (adjacent tracks in the
                                same region read it as a broadcast, tracks in different regions may conflict).  0 = default
-                               (1); values above NC or not dividing it are rounded down to a divisor of NC */
+                               (1); values above NC or not dividing it are rounded down to a divisor of NC.  Configurations that
+                               land on the register-capped kernel variant (more than 512 resident threads per SM) always use NC */
     int32_t reserved[5];    /* must be 0 */
 } nd_options;
 
