@@ -24,6 +24,8 @@
  * particle-balance invariants; infinite-medium k_inf closed form; pure-absorber flux; the vacuum
  * rectangle worked example against an escape-probability Monte Carlo and an independent per-track
  * closed form; brute-force triangle clipping for the ray walker; laydown integer invariants.
+ * O-9 (coarse-mesh net currents for CMFD, with oracle/cmfd.py; tests/test_oracle_cmfd.py): exact per-cell balance of
+ * the tallied currents, exact coarse balance at the collapsed flux, closed-form k_inf in one step, unchanged fixed point.
  * "parity unpinned": heterogeneous eigenvalues of configs 1-5 have no external truth.
  *
  * Build: gcc -O2 -std=c11 -ffp-contract=off -fopenmp -shared -fPIC  (no -ffast-math, no -march).
@@ -623,6 +625,100 @@ int orc_power_iteration(int R, int M, int G, int P, int T, const int *region_mat
     *k_io = k;
     free(Q); free(phi_new); free(psi_next);
     return rc;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O-9  Net currents of a sweep on a coarse mesh (CMFD, Algorithm 1 line 5 "Solve CMFD on the coarse
+ *      mesh"; the paper gives no formula -- DESIGN.md section 8d states the reading).
+ *      cell[r] maps every region to a coarse cell.  The walk is the one of O-6 (same psi_in, same Q, same
+ *      w_{t,p}); wherever a chain steps from a region of cell C into a region of another cell C' the
+ *      weighted angular flux crosses the interior surface {C, C'}:
+ *            J_surf[s][g] += sgn * w_{t,p} * psi ,   s = index of (min(C,C'), max(C,C')) in the sorted
+ *                                                    pair list,  sgn = +1 if C < C' else -1
+ *      and at the exit end of a chain (track t, direction d) in cell C, with psi_in' the flux that
+ *      enters the opposite direction at that same end:
+ *            J_end[C][g] += w_{t,p} * (psi_exit - psi_in')       into J_vac if that end is a vacuum end
+ *                                                                (link[t][d] < 0), else into J_ref.
+ *      A reflective end hands psi_exit to the chain link[t][d]; if that chain ENTERS in another cell C' (the two tracks
+ *      meet at a mesh vertex on the boundary and rule R-W puts them into different triangles) the hand-over is a
+ *      crossing of the surface {C, C'} like any other:  J_surf += sgn * w * psi_exit,  J_ref[C] -= w * psi_exit,
+ *      J_ref[C'] += w * psi_exit -- so J_ref holds only what vanishes when the boundary flux has converged.
+ *      Exact consequence (telescoping, checked in tests): for every cell and group
+ *            sum_{r in C} tally[r][g] + sum_{s=(C,.)} J_surf - sum_{s=(.,C)} J_surf + J_vac[C] + J_ref[C] = 0.
+ *      pair_lo/pair_hi: the n_pairs interior surfaces, sorted by (lo, hi), lo < hi.
+ * ---------------------------------------------------------------------------------------------- */
+static int64_t find_pair(int n, const int *lo, const int *hi, int a, int b)
+{
+    int64_t l = 0, h = n - 1;
+    while (l <= h) {
+        int64_t m = (l + h) / 2;
+        if (lo[m] < a || (lo[m] == a && hi[m] < b)) l = m + 1;
+        else if (lo[m] > a || hi[m] > b) h = m - 1;
+        else return m;
+    }
+    return -1;
+}
+
+int orc_sweep_currents(int R, int M, int G, int P, int T, const int *region_material, const double *sigma_t,
+                       const double *polar_sin, const double *polar_weight, const int64_t *seg_offset,
+                       const int *seg_region, const double *seg_length, const double *track_weight, const int *link,
+                       const double *Q, const double *psi_in, int n_cells, const int *cell, int n_pairs,
+                       const int *pair_lo, const int *pair_hi, double *J_surf, double *J_vac, double *J_ref)
+{
+    if (!region_material || !sigma_t || !polar_sin || !polar_weight || !seg_offset || !seg_region || !seg_length ||
+        !track_weight || !link || !Q || !psi_in || !cell || !J_surf || !J_vac || !J_ref || R < 1 || M < 1 || G < 1 ||
+        P < 1 || T < 1 || n_cells < 1 || n_pairs < 0 || (n_pairs > 0 && (!pair_lo || !pair_hi)))
+        return ORC_ERR_ARG;
+    size_t PG = (size_t)P * (size_t)G;
+    memset(J_surf, 0, sizeof(double) * (size_t)n_pairs * G);
+    memset(J_vac, 0, sizeof(double) * (size_t)n_cells * G);
+    memset(J_ref, 0, sizeof(double) * (size_t)n_cells * G);
+    for (int t = 0; t < T; ++t) {
+        int64_t k0 = seg_offset[t], k1 = seg_offset[t + 1];
+        if (k1 == k0) continue;
+        for (int d = 0; d < 2; ++d)
+            for (int p = 0; p < P; ++p) {
+                double w = 4.0 * ORC_PI * track_weight[t] * polar_weight[p] * polar_sin[p];
+                for (int g = 0; g < G; ++g) {
+                    double psi = psi_in[((size_t)t * 2 + d) * PG + (size_t)p * G + g];
+                    int c_prev = -1;
+                    for (int64_t q = 0; q < k1 - k0; ++q) {
+                        int64_t k = d == 0 ? k0 + q : k1 - 1 - q;
+                        int r = seg_region[k];
+                        int c = cell[r];
+                        if (c < 0 || c >= n_cells) return ORC_ERR_ARG;
+                        if (c_prev >= 0 && c != c_prev) {
+                            int a = c_prev < c ? c_prev : c, b = c_prev < c ? c : c_prev;
+                            int64_t s = find_pair(n_pairs, pair_lo, pair_hi, a, b);
+                            if (s < 0) return ORC_ERR_ARG;
+                            J_surf[(size_t)s * G + g] += (c_prev < c ? 1.0 : -1.0) * w * psi;
+                        }
+                        double st = sigma_t[(size_t)region_material[r] * G + g];
+                        double tau = st * seg_length[k] / polar_sin[p];
+                        psi -= (psi - Q[(size_t)r * G + g] / st) * (-expm1(-tau));
+                        c_prev = c;
+                    }
+                    double back = psi_in[((size_t)t * 2 + (1 - d)) * PG + (size_t)p * G + g];
+                    int lk = link[2 * t + d];
+                    double *J = lk < 0 ? J_vac : J_ref;
+                    J[(size_t)c_prev * G + g] += w * (psi - back);
+                    if (lk >= 0) {
+                        int t2 = lk / 2, d2 = lk % 2;
+                        if (t2 >= T || seg_offset[t2 + 1] == seg_offset[t2]) return ORC_ERR_ARG;
+                        int c2 = cell[seg_region[d2 == 0 ? seg_offset[t2] : seg_offset[t2 + 1] - 1]];
+                        if (c2 != c_prev) {
+                            int a = c_prev < c2 ? c_prev : c2, b = c_prev < c2 ? c2 : c_prev;
+                            int64_t s = find_pair(n_pairs, pair_lo, pair_hi, a, b);
+                            if (s < 0) return ORC_ERR_ARG;
+                            J_surf[(size_t)s * G + g] += (c_prev < c2 ? 1.0 : -1.0) * w * psi;
+                            J_ref[(size_t)c_prev * G + g] -= w * psi;
+                            J_ref[(size_t)c2 * G + g] += w * psi;
+                        }
+                    }
+                }
+            }
+    }
+    return ORC_OK;
 }
 
 int orc_num_threads(void)
