@@ -231,7 +231,7 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
         if (byte0[n_sw] / 16 >= 0xffffffffull) return nd_fail(ND_ERR_RANGE, "swath stream exceeds 64 GiB");
         out->tile_chunk.resize((size_t)out->n_tiles + 1);
         out->tile_chunk[(size_t)out->n_tiles] = (uint32_t)(byte0[n_sw] / 16);   // end sentinel: chunk k spans [k, k+1)
-        out->blob.resize(byte0[n_sw]);
+        out->blob.resize_uninitialised(byte0[n_sw]);   // first touched by the parallel copies below
         int64_t sum_regions = 0, sum_seg = 0, sum_slots = 0;
         int max_chunk = 0;
         for (int64_t sw = 0; sw < n_sw; ++sw) {

@@ -19,7 +19,9 @@
 // to add up per region (a track may re-enter a region; every visit has its own row).
 #ifndef ND_SWATH_H
 #define ND_SWATH_H
+#include <cstddef>
 #include <cstdint>
+#include <memory>
 #include <vector>
 
 #include "nd.h"
@@ -39,6 +41,17 @@ struct NdSwathParams {
 
 struct NdSwathItem { int32_t swath, dir, cost, reserved; };
 
+// Byte buffer that is NOT value-initialised: the 4-5 GB chunk stream of a 5e8-segment problem is written exactly once by
+// parallel copies; zero-filling it first (std::vector::resize) cost 2 s of single-threaded page faults.
+struct NdRawBytes {
+    std::unique_ptr<uint8_t[]> p;
+    size_t n = 0;
+    void resize_uninitialised(size_t bytes) { p.reset(bytes ? new uint8_t[bytes] : nullptr); n = bytes; }
+    uint8_t* data() { return p.get(); }
+    const uint8_t* data() const { return p.get(); }
+    size_t size() const { return n; }
+};
+
 struct NdSwathSet {
     NdSwathParams prm{};
     int64_t n_swaths = 0, n_tiles = 0;
@@ -46,7 +59,7 @@ struct NdSwathSet {
     std::vector<int64_t> swath_tile0;     // [n_swaths+1] prefix into tile_chunk
     std::vector<uint32_t> tile_chunk;     // [n_tiles+1] chunk offsets in 16-byte units (+ end sentinel)
     std::vector<NdSwathItem> items;       // work items (swath, direction), most expensive first
-    std::vector<uint8_t> blob;            // all chunks
+    NdRawBytes blob;                      // all chunks (every byte written by nd_build_swaths)
     int max_chunk_bytes = 0;
     double mean_regions_per_tile = 0.0, mean_segments_per_tile = 0.0, lockstep_efficiency = 0.0;
 };
