@@ -193,6 +193,8 @@ extern "C" nd_status nd_tracks_generate_device(const nd_mesh_desc* mesh, int32_t
         tr->n_segments = tr->seg_offset[T];
         tr->seg_region.resize((size_t)tr->n_segments);
         tr->seg_length.resize((size_t)tr->n_segments);
+        nd_touch_pages(tr->seg_region.data(), 4 * (size_t)tr->n_segments);
+        nd_touch_pages(tr->seg_length.data(), 8 * (size_t)tr->n_segments);
         ND_TRACE_CUDA(cudaMemcpyAsync(ws + L.seg_off, tr->seg_offset.data(), 8 * (T + 1), cudaMemcpyHostToDevice, st));
         // ---- pass 2: fill, in batches of tracks whose segments fit the output area ----
         for (size_t t0 = 0; t0 < T;) {

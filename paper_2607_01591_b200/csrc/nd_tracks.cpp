@@ -439,3 +439,11 @@ extern "C" nd_status nd_tracks_destroy(nd_tracks* tr)
     delete tr;
     return ND_OK;
 }
+
+void nd_touch_pages(void* p, size_t bytes)
+{
+    volatile unsigned char* b = static_cast<volatile unsigned char*>(p);
+    const int64_t n_pages = (int64_t)((bytes + 4095) / 4096);
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n_pages; ++i) b[(size_t)i * 4096] = 0;
+}

@@ -4,9 +4,28 @@
 #ifndef ND_TRACKS_INTERNAL_H
 #define ND_TRACKS_INTERNAL_H
 #include <cstdint>
+#include <memory>
 #include <vector>
 
 #include "nd.h"
+
+// Array that is NOT value-initialised: the segment arrays of a 5e8-segment problem (5.8 GB) are written exactly once, by
+// the parallel host walk or by device-to-host copies; std::vector::resize would zero-fill them first on one thread (~2 s).
+template <class T>
+struct NdRawArray {
+    std::unique_ptr<T[]> p;
+    size_t n = 0;
+    void resize(size_t count) { p.reset(count ? new T[count] : nullptr); n = count; }
+    T* data() { return p.get(); }
+    const T* data() const { return p.get(); }
+    size_t size() const { return n; }
+    T& operator[](size_t i) { return p[i]; }
+    const T& operator[](size_t i) const { return p[i]; }
+};
+
+// writes one byte per 4 KB page with all host threads: first touch of a freshly allocated array before a
+// device-to-host copy fills it (the copy would otherwise fault the pages in one by one)
+void nd_touch_pages(void* p, size_t bytes);
 
 struct NdAngleSet {          // one track angle j in (0, pi)
     int nx = 0, ny = 0;      // tracks leaving the bottom side / the vertical side
@@ -24,8 +43,8 @@ struct nd_tracks {
     int64_t n_segments = 0;
     std::vector<NdAngleSet> angles;
     std::vector<int64_t> seg_offset;
-    std::vector<int32_t> seg_region;
-    std::vector<double> seg_length;
+    NdRawArray<int32_t> seg_region;   // every element written by the walk
+    NdRawArray<double> seg_length;
     std::vector<double> track_weight;
     std::vector<int32_t> link;
     std::vector<int32_t> track_azim;
