@@ -95,7 +95,10 @@ typedef struct {
                                same region read it as a broadcast, tracks in different regions may conflict).  0 = default
                                (1); values above NC or not dividing it are rounded down to a divisor of NC.  Configurations that
                                land on the register-capped kernel variant (more than 512 resident threads per SM) always use NC */
-    int32_t reserved[5];    /* must be 0 */
+    int32_t graph_mode;     /* nd_power_iteration with a fixed iteration count (no tolerances, no per-iteration stats, profiling
+                               off) replays a CUDA graph of two iterations instead of launching their kernels one by one:
+                               0 = default (on for calls of >= 4 iterations), 1 = never */
+    int32_t reserved[4];    /* must be 0 */
 } nd_options;
 
 /* ------------------------------------------------------------------------------------------------

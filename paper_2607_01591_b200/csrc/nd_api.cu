@@ -355,6 +355,11 @@ struct nd_problem {
     std::vector<EventPair> ev_pool;
     size_t ev_used = 0;
     int64_t kernels_launched = 0;
+    // CUDA graph of two power iterations (phi_cur returns to the buffer it started in), see nd_power_iteration
+    cudaGraphExec_t iter_graph = nullptr;
+    cudaStream_t cap_stream = nullptr;        // capture only; replays run on the caller's stream
+    const double* iter_graph_phi = nullptr;   // phi_cur the graph was captured with
+    int64_t iter_graph_kernels = 0;           // kernels one replay launches
 };
 
 namespace {
@@ -634,12 +639,12 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     if (rc != ND_OK) return rc;
     nd_options opt{};
     if (opts) opt = *opts;
-    for (int i = 0; i < 5; ++i)
+    for (int i = 0; i < 4; ++i)
         if (opt.reserved[i] != 0) return nd_fail(ND_ERR_INVALID, "nd_options.reserved must be zero");
     if (opt.exp_mode != ND_EXP_FAST && opt.exp_mode != ND_EXP_EXPM1) return nd_fail(ND_ERR_INVALID, "unknown exp_mode");
     if (opt.sweep_kernel < ND_SWEEP_AUTO || opt.sweep_kernel > ND_SWEEP_SWATH_WS) return nd_fail(ND_ERR_INVALID, "unknown sweep_kernel");
     if (opt.track_batch < 0 || opt.window_regions < 0 || opt.block_warps < 0 || opt.tile_segments < 0 || opt.delta_buffers < 0 ||
-        opt.delta_buffers > 2 || opt.blocks_per_sm < 0 || opt.tile_lag < -1 || opt.service_warps < 0 || opt.q_copies < 0)
+        opt.delta_buffers > 2 || opt.blocks_per_sm < 0 || opt.tile_lag < -1 || opt.service_warps < 0 || opt.q_copies < 0 || opt.graph_mode < 0 || opt.graph_mode > 1)
         return nd_fail(ND_ERR_INVALID, "nd_options: tuning fields must be >= 0 (delta_buffers 0, 1 or 2)");
     if ((desc->track_azim == nullptr) != (desc->track_ends == nullptr))
         return nd_fail(ND_ERR_INVALID, "track_azim and track_ends must both be set or both be NULL");
@@ -869,6 +874,8 @@ extern "C" nd_status nd_problem_destroy(nd_problem* p)
 {
     if (!p) return ND_OK;
     for (auto& e : p->ev_pool) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    if (p->iter_graph) cudaGraphExecDestroy(p->iter_graph);
+    if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
     delete p;
     return ND_OK;
 }
@@ -930,7 +937,7 @@ extern "C" nd_status nd_power_iteration(nd_problem* p, int32_t max_iters, double
     sp.Q = p->Q; sp.q = p->q; sp.tally = p->tally; sp.R = d.R; sp.G = d.G; sp.Gs = d.Gs;
     int it = 0;
     bool converged = !use_tol;
-    for (; it < max_iters; ++it) {
+    auto one_iteration = [&](double* slot, cudaStream_t st) -> nd_status {
         sp.phi = p->phi_cur;
         nd_status rc = launch_source(p, sp, st);
         if (rc != ND_OK) return rc;
@@ -939,10 +946,51 @@ extern "C" nd_status nd_power_iteration(nd_problem* p, int32_t max_iters, double
         int grid = 0;
         rc = launch_finalise(p, p->Q, p->phi_cur, p->scalars + ndk::SC_F, p->phi_new, &grid, st);
         if (rc != ND_OK) return rc;
-        double* slot = (stats && it < kMaxStats) ? p->stats + 4 * (size_t)it : (sync_each ? p->stats : nullptr);
         ndk::k_reduce_final<<<1, 256, 0, st>>>(p->partial, grid, p->scalars, 1, slot);
         ND_LAUNCH_CHECK(p);
         std::swap(p->phi_cur, p->phi_new);
+        return ND_OK;
+    };
+    // Fixed-count calls replay a CUDA graph of TWO iterations (after two, phi_cur is back in the buffer it started in, so
+    // one graph serves every pair); an odd iteration and anything with tolerances, stats or profiling is launched plainly.
+    const bool graph_ok = !use_tol && !stats && !p->profile && !p->phase_profile && p->opt.graph_mode == 0 && max_iters >= 4;
+    if (graph_ok) {
+        if (p->iter_graph && p->iter_graph_phi != p->phi_cur) {   // an odd number of plain iterations since the capture
+            nd_status rc = one_iteration(nullptr, st);
+            if (rc != ND_OK) return rc;
+            ++it;
+        }
+        if (!p->iter_graph) {
+            const int64_t before = p->kernels_launched;
+            const double* phi0 = p->phi_cur;
+            cudaGraph_t graph = nullptr;
+            // captured on a stream of our own: the caller's may be the legacy default stream, which cannot capture
+            if (!p->cap_stream) ND_CUDA(cudaStreamCreateWithFlags(&p->cap_stream, cudaStreamNonBlocking));
+            ND_CUDA(cudaStreamBeginCapture(p->cap_stream, cudaStreamCaptureModeRelaxed));
+            nd_status rc = one_iteration(nullptr, p->cap_stream);
+            if (rc == ND_OK) rc = one_iteration(nullptr, p->cap_stream);
+            const cudaError_t ce = cudaStreamEndCapture(p->cap_stream, &graph);
+            if (rc != ND_OK || ce != cudaSuccess) {
+                if (graph) cudaGraphDestroy(graph);
+                if (p->phi_cur != phi0) std::swap(p->phi_cur, p->phi_new);
+                return rc != ND_OK ? rc : nd_fail(ND_ERR_CUDA, cudaGetErrorString(ce));
+            }
+            p->iter_graph_kernels = p->kernels_launched - before;
+            p->kernels_launched = before;                          // captured, not launched
+            const cudaError_t ci = cudaGraphInstantiate(&p->iter_graph, graph, 0);
+            cudaGraphDestroy(graph);
+            if (ci != cudaSuccess) { p->iter_graph = nullptr; return nd_fail(ND_ERR_CUDA, cudaGetErrorString(ci)); }
+            p->iter_graph_phi = p->phi_cur;                        // == phi0 after two swaps
+        }
+        for (; it + 2 <= max_iters; it += 2) {
+            ND_CUDA(cudaGraphLaunch(p->iter_graph, st));
+            p->kernels_launched += p->iter_graph_kernels;
+        }
+    }
+    for (; it < max_iters; ++it) {
+        double* slot = (stats && it < kMaxStats) ? p->stats + 4 * (size_t)it : (sync_each ? p->stats : nullptr);
+        nd_status rc = one_iteration(slot, st);
+        if (rc != ND_OK) return rc;
         if (sync_each) {
             double h[4];
             ND_CUDA(cudaMemcpyAsync(h, slot, sizeof h, cudaMemcpyDeviceToHost, st));

@@ -225,6 +225,49 @@ def test_power_iteration_tolerance_mode_and_reset():
         pair.close()
 
 
+@pytest.mark.parametrize("case", [(1, 1.0), (2, 0.15), (4, 0.06)], ids=["cfg1", "cfg2", "cfg4"])
+def test_power_iteration_graph_replay_matches_plain_launches(case):
+    """Fixed-count calls of >= 4 iterations replay a CUDA graph of two iterations (nd_options.graph_mode 0); the result,
+    the iteration count and the launch count are those of the plain launches (graph_mode 1), also when plain and
+    replayed calls are mixed so that an odd iteration comes first, and after a reset."""
+    import time
+    import torch
+    a = make_pair(case[0], case[1])
+    b = make_pair(case[0], case[1], graph_mode=1)
+    try:
+        for g in (a.gpu, b.gpu):
+            g.nd_profile_enable(0)
+        seq = [3, 9, 4, 1, 6]                     # 3 plain, odd start + pairs, pairs, plain, pairs
+        for n in seq:
+            oa, ob = a.gpu.nd_power_iteration(n), b.gpu.nd_power_iteration(n)
+            assert oa["iters"] == ob["iters"] == n
+            assert abs(oa["k_eff"] - ob["k_eff"]) < 1e-9 * abs(ob["k_eff"])
+        pa, pb = a.gpu.nd_flux_get().cpu().numpy(), b.gpu.nd_flux_get().cpu().numpy()
+        assert np.max(np.abs(pa - pb) / np.maximum(np.abs(pb), 1e-6 * np.abs(pb).max())) < 1e-6
+        assert a.gpu.nd_profile_read()["kernels_launched"] == b.gpu.nd_profile_read()["kernels_launched"] > 0
+        ko, *_ = a.oracle_power(sum(seq))
+        assert abs(oa["k_eff"] - ko) * 1e5 <= K_PCM
+        for g in (a.gpu, b.gpu):
+            g.nd_state_reset()
+        assert abs(a.gpu.nd_power_iteration(8)["k_eff"] - b.gpu.nd_power_iteration(8)["k_eff"]) < 1e-9
+        a.gpu.nd_profile_enable(1)                # profiling on: plain launches again, sweep events recorded
+        a.gpu.nd_power_iteration(6)
+        assert a.gpu.nd_profile_read()["sweep_launches"] == 6
+        a.gpu.nd_profile_enable(0)
+        t = []
+        for g in (a.gpu, b.gpu):
+            g.nd_power_iteration(40)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            g.nd_power_iteration(200)
+            torch.cuda.synchronize()
+            t.append((time.perf_counter() - t0) / 200 * 1e3)
+        print(f"cfg{case[0]}: {t[0]:.4f} ms / iteration replayed, {t[1]:.4f} ms plain")
+    finally:
+        a.close()
+        b.close()
+
+
 def test_infinite_medium_closed_form_on_gpu():
     """Homogeneous reflective rectangle: k -> nuSf^T (diag(St) - S)^-1 chi (closed form, not the oracle)."""
     mesh = rect_tri_mesh(1.5, 1.5, 4, 4, seed=2, jitter=0.2)
