@@ -110,7 +110,7 @@ def _custom_pair(G, P, bc, n_azim=16, spacing=0.07, seed=3, n_materials=3, **opt
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
-@pytest.mark.parametrize("G,P", [(1, 1), (2, 2), (3, 3), (5, 4), (8, 3), (31, 3), (32, 2), (33, 3), (51, 3), (64, 1), (70, 3)])
+@pytest.mark.parametrize("G,P", [(1, 1), (2, 2), (3, 3), (5, 4), (8, 3), (31, 3), (32, 2), (33, 3), (51, 3), (64, 1), (70, 3), (128, 2), (129, 1), (200, 3)])
 def test_sweep_group_and_polar_shapes(G, P, kernel):
     pair = _custom_pair(G, P, (1, 0, 0, 1), sweep_kernel=kernel)
     try:
