@@ -82,7 +82,8 @@ typedef struct {
     int32_t window_regions; /* max distinct regions per tile (both tiled kernels); 0 = default */
     int32_t block_warps;    /* ND_SWEEP_SWATH: warps per thread block (tracks per swath = warps * slots per warp); 0 = default */
     int32_t tile_segments;  /* ND_SWEEP_SWATH: max segments of one track per tile; 0 = default */
-    int32_t delta_buffers;  /* ND_SWEEP_SWATH: 1 or 2 delta buffers (2 saves one block barrier per tile); 0 = default */
+    int32_t delta_buffers;  /* ND_SWEEP_SWATH: 1 or 2 delta buffers; 0 = default (1).  Two buffers no longer save the barrier
+                               before the segment loop (it also guards the chunk ring); kept for experiments */
     int32_t blocks_per_sm;  /* ND_SWEEP_SWATH: resident blocks per SM the grid is sized for; 0 = default */
     int32_t tile_lag;       /* ND_SWEEP_SWATH: drift of the track fronts (in mean segment lengths) under which a tile gives
                                every track the same number of segments; 0 = default, -1 = always cut geometrically */

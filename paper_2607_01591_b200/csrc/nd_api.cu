@@ -161,7 +161,7 @@ SwathConfig make_swath_config_q(const Dims& d, const nd_options& opt, bool ws, i
         c.off_q = c.off_sigt + pad128(d.M * line);
         c.off_dbuf = c.off_q + pad128(2 * Lmax * line_q);
         c.off_chunk = c.off_dbuf + pad128(c.ndbuf * (NT / NC) * Kmax * line);
-        c.smem_bytes = c.off_chunk + ndk::kSwathChunkBufs * c.chunk_cap;
+        c.smem_bytes = c.off_chunk + (ws ? 4 : ndk::kSwathChunkBufs) * c.chunk_cap;   // the warp-specialised kernel keeps four
         return true;
     };
     // Defaults (measured, profiles/): occupancy beats tile length once a tile holds >= 8 segments per track.  Aim at
@@ -184,11 +184,13 @@ SwathConfig make_swath_config_q(const Dims& d, const nd_options& opt, bool ws, i
             const int Lw = opt.window_regions > 0 ? opt.window_regions : (int)(NT * K / rho_est + 3) / 4 * 4;
             placed = layout(warps, K, Lw) && c.smem_bytes <= kSmemMax;
         } else {
+            // longest tile that fits `blocks` per SM; the region window may shrink by up to 8 rows below the estimate
             for (int blocks = target_blocks; blocks >= 1 && !placed; --blocks)
-                for (int K = 16; K >= 8 && !placed; K -= 2) {
-                    const int Lw = (int)(NT * K / rho_est + 3) / 4 * 4;
-                    placed = layout(warps, K, Lw < 24 ? 24 : Lw) && c.smem_bytes + 1024 <= (kSmemMax + 1024) / blocks;
-                }
+                for (int K = 16; K >= 8 && !placed; --K)
+                    for (int cut = 0; cut <= 8 && !placed; cut += 2) {
+                        const int Lw = (int)(NT * K / rho_est + 3) / 4 * 4 - cut;
+                        placed = layout(warps, K, Lw < 24 ? 24 : Lw) && c.smem_bytes + 1024 <= (kSmemMax + 1024) / blocks;
+                    }
         }
         if (placed) break;
     }

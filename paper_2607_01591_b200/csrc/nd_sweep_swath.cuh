@@ -16,7 +16,7 @@
 //     independent Eq.-(5) chains in registers (ILP hides the MUFU/FMA latency).  psi is read from the boundary
 //     array once, at the track's entry, and written once, at its exit.
 //   * the swath is processed tile by tile (nd_swath.h).  A tile's chunk arrives by ONE bulk async (TMA) copy,
-//     two tiles ahead, signalled on an mbarrier; the q rows of its regions are gathered by 16-byte cp.async one
+//     two tiles ahead (ring of three chunk buffers), signalled on an mbarrier; the q rows of its regions are gathered by 16-byte cp.async one
 //     tile ahead.  In the segment loop a lane reads the segment record (broadcast), its 16 bytes of the q row and
 //     of the Sigma_t row, and STORES sum_p w_p Delta_p into the segment's own row of the delta buffer: no
 //     read-modify-write, no atomics (a segment owns its row).
@@ -55,7 +55,7 @@ struct SwathParams {
 // phases of the instrumented build (nd_profile_enable(p, 2)): where the warps' cycles go
 enum { PH_STAGE = 0, PH_WAIT_A, PH_COMPUTE, PH_WAIT_B, PH_FLUSH, PH_ITEM, kSwathPhases };
 
-constexpr int kSwathChunkBufs = 4;
+constexpr int kSwathChunkBufs = 3;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -356,9 +356,11 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
                 issue_q_rows(k + 1);
             }
             cp_async_commit_group();
-            if (tid == 0 && k + 2 < nt) issue_chunk(k + 2);
             mark(PH_STAGE);
-            if (prm.ndbuf == 1) __syncthreads();   // single delta buffer: the previous tile's flush must be over
+            // Three chunk buffers: the chunk of tile k+2 goes into the buffer of tile k-1, free once every thread is past
+            // that tile's flush, i.e. behind this barrier (which also frees the delta rows of a single delta buffer).
+            __syncthreads();
+            if (tid == 0 && k + 2 < nt) issue_chunk(k + 2);
             if (PROF) prof_sink += *s_item;        // BAR.SYNC defers its blocking to the next consumer: make one here
             mark(PH_WAIT_A);
             const SwathChunk ch = decode_chunk(cb);
