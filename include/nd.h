@@ -243,6 +243,29 @@ nd_status nd_flux_set(nd_problem* p, const double* d_phi, double k_eff, void* cu
 nd_status nd_track_volume_get(nd_problem* p, double* host_out);                    /* HOST [R] */
 nd_status nd_tally_get(nd_problem* p, double* d_tally_out, void* cuda_stream);     /* DEVICE [R][G], last sweep */
 
+/* NEXT-3 (CMFD, Algorithm 1 "Solve CMFD on the coarse mesh"), step C-3 of DESIGN.md 8d: the net
+ * currents of ONE sweep (Eq. (5)) through the surfaces of a coarse mesh, integrated over each surface with
+ * the sweep's own weights w_{t,p} = 4 pi omega_a delta_a w_p sin(theta_p).
+ *   d_Q              DEVICE [R][G] FP64, read: the isotropic angular source of the sweep (as nd_transport_sweep)
+ *   cell             HOST [R]: coarse cell of every region, 0 <= cell[r] < n_cells
+ *   pair_lo/pair_hi  HOST [n_pairs]: the interior surfaces as cell pairs lo < hi, in any order, each listed once; every
+ *                    pair of cells that consecutive segments of a track or a reflective hand-over join must be listed
+ *   J_surf           HOST [n_pairs][G] FP64, written: sum of +w psi at every crossing lo -> hi, -w psi at hi -> lo
+ *   J_vac, J_ref     HOST [n_cells][G] FP64, written: at the exit end of every chain (t, d), w (psi_exit - psi_in of the
+ *                    opposite direction), into J_vac[cell of the end] at a vacuum end, J_ref at a reflective one; a
+ *                    hand-over into another cell c2 also adds w psi_exit to the surface and moves it from J_ref[c] to
+ *                    J_ref[c2].  Per cell and group: sum of the sweep's tallies + sum +-J_surf + J_vac + J_ref = 0.
+ * Reads the problem's current boundary psi and leaves ALL state unchanged (the boundary flux is not advanced, the tally
+ * of the last sweep is kept): nd_transport_sweep with the same d_Q afterwards performs the sweep these currents belong
+ * to.  FP32 segment arithmetic, FP64 atomics.  This round: the simple one-warp-per-chain kernel over the SoA stream,
+ * so the problem must have been created with sweep_kernel = ND_SWEEP_ATOMIC (else ND_ERR_STATE); scratch is allocated
+ * and freed inside the call and the stream is synchronised before it returns.
+ * Errors: ND_ERR_NULL, ND_ERR_INVALID (sizes; a surface listed twice; a crossing between cells that are not a listed
+ * surface -- outputs are then unspecified), ND_ERR_RANGE (cell or pair out of range), ND_ERR_STATE, ND_ERR_CUDA. */
+nd_status nd_sweep_currents(nd_problem* p, const double* d_Q, int32_t n_cells, const int32_t* cell, int32_t n_pairs,
+                            const int32_t* pair_lo, const int32_t* pair_hi, double* J_surf, double* J_vac, double* J_ref,
+                            void* cuda_stream);
+
 /* Device-time accounting.  When enabled, every sweep-kernel launch is bracketed by CUDA events on its own
  * stream; nd_profile_read synchronises and returns the accumulated kernel milliseconds and launch counts
  * since the last nd_profile_enable(p,1).  kernels_launched counts every kernel the library launched. */

@@ -25,7 +25,7 @@ EXPORTS = [
     "nd_tracks_generate", "nd_tracks_device_workspace_bytes", "nd_tracks_generate_device", "nd_tracks_view", "nd_tracks_destroy", "nd_workspace_bytes", "nd_problem_create",
     "nd_problem_destroy", "nd_transport_sweep", "nd_source_update", "nd_power_iteration", "nd_state_reset",
     "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_outgoing_flux_get", "nd_flux_get", "nd_flux_set",
-    "nd_track_volume_get", "nd_tally_get", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
+    "nd_track_volume_get", "nd_tally_get", "nd_sweep_currents", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
     "nd_swath_stream_build", "nd_swath_stream_view", "nd_swath_stream_destroy",
     "nd_status_string", "nd_last_error", "nd_version",
 ]
@@ -134,6 +134,8 @@ def lib():
         L.nd_flux_set.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         L.nd_track_volume_get.argtypes = [C.c_void_p, C.c_void_p]
         L.nd_tally_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nd_sweep_currents.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p,
+                                        C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.nd_profile_enable.argtypes = [C.c_void_p, C.c_int32]
         L.nd_profile_read.argtypes = [C.c_void_p, C.POINTER(nd_profile)]
         L.nd_sweep_phases_get.argtypes = [C.c_void_p, C.c_void_p]
@@ -365,6 +367,19 @@ class Problem:
         out = self.torch.empty((self.R, self.G), dtype=self.torch.float64, device=self.device)
         _check(lib().nd_tally_get(self._h, out.data_ptr(), self._stream()), "nd_tally_get")
         return out
+
+    def nd_sweep_currents(self, d_Q, cell, n_cells, pair_lo, pair_hi):
+        """C-3 (nd.h): returns HOST arrays J_surf [n_pairs][G], J_vac [n_cells][G], J_ref [n_cells][G]."""
+        t = self.torch
+        assert d_Q.dtype == t.float64 and d_Q.is_cuda and d_Q.is_contiguous() and d_Q.numel() == self.R * self.G
+        cell = np.ascontiguousarray(cell, np.int32)
+        lo, hi = np.ascontiguousarray(pair_lo, np.int32), np.ascontiguousarray(pair_hi, np.int32)
+        assert cell.shape == (self.R,) and lo.shape == hi.shape and lo.ndim == 1
+        Js, Jv, Jr = np.empty((len(lo), self.G)), np.empty((int(n_cells), self.G)), np.empty((int(n_cells), self.G))
+        _check(lib().nd_sweep_currents(self._h, d_Q.data_ptr(), int(n_cells), cell.ctypes.data, len(lo), lo.ctypes.data,
+                                       hi.ctypes.data, Js.ctypes.data, Jv.ctypes.data, Jr.ctypes.data, self._stream()),
+               "nd_sweep_currents")
+        return Js, Jv, Jr
 
     def nd_profile_enable(self, on=True):
         _check(lib().nd_profile_enable(self._h, int(on)), "nd_profile_enable")

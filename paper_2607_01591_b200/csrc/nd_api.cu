@@ -1,6 +1,7 @@
 // nd_api.cu -- the C ABI of include/nd.h: validation, device layout, stream packing (row A1), kernel
 // launches (rows A2-A6) and the power-iteration driver (row A7).  No CPU fallback anywhere: every compute
 // entry point launches CUDA kernels and returns ND_ERR_CUDA if that fails.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -14,6 +15,7 @@
 #include "nd.h"
 #include "nd_internal.h"
 #include "nd_kernels.cuh"
+#include "nd_cmfd.cuh"
 #include "nd_sweep_private.cuh"
 #include "nd_sweep_swath.cuh"
 #include "nd_sweep_swath_ws.cuh"
@@ -1103,6 +1105,111 @@ extern "C" nd_status nd_tally_get(nd_problem* p, double* d_tally_out, void* cuda
     cudaStream_t st = as_stream(cuda_stream);
     ndk::k_unpad_f64<<<grid_for((int64_t)d.R * d.G, 256, 8 * p->n_sm), 256, 0, st>>>(p->tally, d_tally_out, d.R, d.G, d.Gs);
     ND_LAUNCH_CHECK(p);
+    return ND_OK;
+}
+
+namespace {
+
+template <int P>
+void launch_currents_p(const nd_problem* p, const ndk::CurrentParams& cp, int grid, cudaStream_t st)
+{
+    if (p->opt.exp_mode == ND_EXP_EXPM1)
+        ndk::k_sweep_currents<P, 1><<<grid, 256, 0, st>>>(cp);
+    else
+        ndk::k_sweep_currents<P, 0><<<grid, 256, 0, st>>>(cp);
+}
+
+} // namespace
+
+// NEXT-3, C-3: see nd.h.  Not on the hot path yet: it allocates its scratch with cudaMalloc, runs the
+// simple one-warp-per-chain sweep and synchronises the stream before it returns.
+extern "C" nd_status nd_sweep_currents(nd_problem* p, const double* d_Q, int32_t n_cells, const int32_t* cell,
+                                       int32_t n_pairs, const int32_t* pair_lo, const int32_t* pair_hi, double* J_surf,
+                                       double* J_vac, double* J_ref, void* cuda_stream)
+{
+    if (!p || !d_Q || !cell || !J_vac || !J_ref || (n_pairs > 0 && (!pair_lo || !pair_hi || !J_surf)))
+        return nd_fail(ND_ERR_NULL, "nd_sweep_currents: NULL argument");
+    if (n_cells < 1 || n_pairs < 0) return nd_fail(ND_ERR_INVALID, "nd_sweep_currents: n_cells must be >= 1 and n_pairs >= 0");
+    if (p->sweep_kernel != ND_SWEEP_ATOMIC)
+        return nd_fail(ND_ERR_STATE, "nd_sweep_currents: needs a problem created with sweep_kernel = ND_SWEEP_ATOMIC "
+                                     "(the current tally reads the SoA segment stream)");
+    const Dims& d = p->d;
+    cudaStream_t st = as_stream(cuda_stream);
+    for (int64_t r = 0; r < d.R; ++r)
+        if (cell[r] < 0 || cell[r] >= n_cells) return nd_fail(ND_ERR_RANGE, "nd_sweep_currents: cell[r] out of [0, n_cells)");
+    std::vector<std::pair<int64_t, int32_t>> keyed;
+    std::vector<int64_t> h_key;
+    std::vector<int32_t> h_idx;
+    try {
+        keyed.reserve((size_t)n_pairs);
+        for (int32_t s = 0; s < n_pairs; ++s) {
+            if (pair_lo[s] < 0 || pair_hi[s] >= n_cells || pair_lo[s] >= pair_hi[s])
+                return nd_fail(ND_ERR_RANGE, "nd_sweep_currents: a surface needs 0 <= lo < hi < n_cells");
+            keyed.emplace_back((int64_t)pair_lo[s] * n_cells + pair_hi[s], s);
+        }
+        std::sort(keyed.begin(), keyed.end());
+        h_key.resize((size_t)n_pairs + 1);
+        h_idx.resize((size_t)n_pairs + 1);
+        for (int32_t s = 0; s < n_pairs; ++s) {
+            if (s > 0 && keyed[s].first == keyed[s - 1].first) return nd_fail(ND_ERR_INVALID, "nd_sweep_currents: a surface is listed twice");
+            h_key[s] = keyed[s].first;
+            h_idx[s] = keyed[s].second;
+        }
+    } catch (const std::bad_alloc&) {
+        return nd_fail(ND_ERR_NOMEM, "nd_sweep_currents: out of host memory");
+    }
+    // scratch: [J_surf | J_vac | J_ref] FP64, pair keys, q, cell, link_fwd, entry_cell, pair index, flag
+    const size_t nJs = (size_t)n_pairs * d.G, nJc = (size_t)n_cells * d.G, nE = 2 * (size_t)d.T;
+    auto up = [](size_t b) { return (b + 255) / 256 * 256; };
+    const size_t oJ = 0, oKey = oJ + up(sizeof(double) * (nJs + 2 * nJc)), oQ = oKey + up(sizeof(int64_t) * ((size_t)n_pairs + 1)),
+                 oCell = oQ + up(sizeof(float) * (size_t)d.R * d.Gs), oFwd = oCell + up(sizeof(int32_t) * (size_t)d.R),
+                 oEnt = oFwd + up(sizeof(int32_t) * nE), oIdx = oEnt + up(sizeof(int32_t) * nE),
+                 oFlag = oIdx + up(sizeof(int32_t) * ((size_t)n_pairs + 1)), total = oFlag + 256;
+    char* buf = nullptr;
+    ND_CUDA(cudaMalloc(&buf, total));
+    struct Free { char* b; ~Free() { cudaFree(b); } } guard{buf};
+    double* dJ = (double*)(buf + oJ);
+    int* d_flag = (int*)(buf + oFlag);
+    ndk::CurrentParams cp{};
+    ndk::SweepParams& prm = cp.sw;
+    prm.seg_rm = p->seg_rm; prm.seg_len = p->seg_len; prm.trk_off = p->trk_off; prm.trk_w = p->trk_w;
+    prm.q = (float*)(buf + oQ); prm.sigt = p->sigt_f; prm.tally = nullptr;
+    prm.psi_in = p->psi_in; prm.psi_out = nullptr; prm.scale_div = p->scalars + ndk::SC_ONE;
+    prm.T = d.T; prm.G = d.G; prm.Gs = d.Gs;
+    for (int i = 0; i < ndk::kMaxPolar; ++i) { prm.c[i] = p->c[i]; prm.inv_sin[i] = p->inv_sin[i]; prm.wp[i] = p->wp[i]; }
+    cp.cell = (int32_t*)(buf + oCell); cp.link_fwd = (int32_t*)(buf + oFwd); cp.entry_cell = (int32_t*)(buf + oEnt);
+    cp.pair_key = (int64_t*)(buf + oKey); cp.pair_idx = (int32_t*)(buf + oIdx);
+    cp.J_surf = dJ; cp.J_vac = dJ + nJs; cp.J_ref = dJ + nJs + nJc; cp.missing = d_flag;
+    cp.n_pairs = n_pairs; cp.n_cells = n_cells;
+    ND_CUDA(cudaMemsetAsync(dJ, 0, sizeof(double) * (nJs + 2 * nJc), st));
+    ND_CUDA(cudaMemsetAsync(d_flag, 0, sizeof(int), st));
+    ND_CUDA(cudaMemsetAsync(buf + oFwd, 0xff, sizeof(int32_t) * nE, st));
+    ND_CUDA(cudaMemcpyAsync(buf + oCell, cell, sizeof(int32_t) * (size_t)d.R, cudaMemcpyHostToDevice, st));
+    if (n_pairs > 0) {
+        ND_CUDA(cudaMemcpyAsync(buf + oKey, h_key.data(), sizeof(int64_t) * (size_t)n_pairs, cudaMemcpyHostToDevice, st));
+        ND_CUDA(cudaMemcpyAsync(buf + oIdx, h_idx.data(), sizeof(int32_t) * (size_t)n_pairs, cudaMemcpyHostToDevice, st));
+    }
+    ndk::k_reduced_q<<<grid_for((int64_t)d.R * d.Gs, 256, 8 * p->n_sm), 256, 0, st>>>(d_Q, p->reg_mat, p->sigt, (float*)(buf + oQ), d.R, d.G, d.Gs);
+    ND_LAUNCH_CHECK(p);
+    ndk::k_link_forward<<<grid_for((int64_t)nE, 256, 8 * p->n_sm), 256, 0, st>>>(p->link_src, (int32_t*)(buf + oFwd), (int64_t)nE);
+    ND_LAUNCH_CHECK(p);
+    ndk::k_entry_cell<<<grid_for((int64_t)nE, 256, 8 * p->n_sm), 256, 0, st>>>(p->seg_rm, p->trk_off, cp.cell, (int32_t*)(buf + oEnt), (int64_t)nE);
+    ND_LAUNCH_CHECK(p);
+    const int grid = grid_for((int64_t)nE * 32, 256, 16 * p->n_sm);
+    switch (d.P) {
+    case 1: launch_currents_p<1>(p, cp, grid, st); break;
+    case 2: launch_currents_p<2>(p, cp, grid, st); break;
+    case 3: launch_currents_p<3>(p, cp, grid, st); break;
+    default: launch_currents_p<4>(p, cp, grid, st); break;
+    }
+    ND_LAUNCH_CHECK(p);
+    int flag = 0;
+    if (nJs) ND_CUDA(cudaMemcpyAsync(J_surf, cp.J_surf, sizeof(double) * nJs, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaMemcpyAsync(J_vac, cp.J_vac, sizeof(double) * nJc, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaMemcpyAsync(J_ref, cp.J_ref, sizeof(double) * nJc, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaMemcpyAsync(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaStreamSynchronize(st));
+    if (flag) return nd_fail(ND_ERR_INVALID, "nd_sweep_currents: a track crosses between two coarse cells that are not a listed surface");
     return ND_OK;
 }
 

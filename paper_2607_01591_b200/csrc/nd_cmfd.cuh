@@ -1,0 +1,143 @@
+// nd_cmfd.cuh -- NEXT-3 (CMFD, Algorithm 1), step C-3 of DESIGN.md 8d: the net currents of one sweep
+// through the surfaces of a coarse mesh.  First CUDA step of that row: the simple (atomic) sweep with crossings tallied.
+//   k_reduced_q       q = (float)(Q / Sigma_t), the reduced source the sweep kernels read
+//   k_link_forward    inverts the gather-form link table: fwd[src[e]] = e  (exit of chain src[e] feeds entry e)
+//   k_entry_cell      coarse cell of the first region of every chain (t, d)
+//   k_sweep_currents  Eq. (5) per (track, direction, polar, group) as in k_sweep_atomic; instead of the
+//                     region tally it adds +-w psi at every change of coarse cell (C-3) and the end terms of C-3
+#pragma once
+#include "nd_kernels.cuh"
+
+namespace ndk {
+
+__global__ void __launch_bounds__(256) k_reduced_q(const double* __restrict__ Q, const int32_t* __restrict__ reg_mat,
+                                                   const double* __restrict__ sigt, float* __restrict__ q, int64_t R,
+                                                   int G, int Gs)
+{
+    const int64_t n = R * Gs;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t r = i / Gs;
+        const int g = (int)(i - r * Gs);
+        q[i] = g < G ? (float)(Q[r * G + g] / sigt[(size_t)reg_mat[r] * G + g]) : 0.f;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_link_forward(const int32_t* __restrict__ src, int32_t* __restrict__ fwd,
+                                                      int64_t n_entries)
+{
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_entries; e += (int64_t)gridDim.x * blockDim.x)
+        if (src[e] >= 0) fwd[src[e]] = (int32_t)e;
+}
+
+__global__ void __launch_bounds__(256) k_entry_cell(const uint32_t* __restrict__ seg_rm, const int64_t* __restrict__ trk_off,
+                                                    const int32_t* __restrict__ cell, int32_t* __restrict__ entry_cell,
+                                                    int64_t n_entries)
+{
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_entries; e += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t t = e >> 1;
+        const int64_t k0 = trk_off[t], k1 = trk_off[t + 1];
+        // the padding records at the end of a run repeat its last region, so k1 - 1 is the entry of direction 1
+        entry_cell[e] = k1 == k0 ? -1 : cell[rm_region(seg_rm[(e & 1) ? k1 - 1 : k0])];
+    }
+}
+
+struct CurrentParams {
+    SweepParams sw;                        // stream, q, Sigma_t, psi_in, polar tables (tally and psi_out are not touched)
+    const int32_t* __restrict__ cell;      // [R] coarse cell of a region
+    const int32_t* __restrict__ link_fwd;  // [2T] entry that the exit of chain e feeds, -1 = vacuum
+    const int32_t* __restrict__ entry_cell;// [2T]
+    const int64_t* __restrict__ pair_key;  // [n_pairs] sorted lo * n_cells + hi
+    const int32_t* __restrict__ pair_idx;  // [n_pairs] the caller's index of the sorted key
+    double* __restrict__ J_surf;           // [n_pairs][G], positive from lo to hi
+    double* __restrict__ J_vac;            // [n_cells][G]
+    double* __restrict__ J_ref;            // [n_cells][G]
+    int* __restrict__ missing;             // set when a crossing joins a pair that is not listed
+    int n_pairs, n_cells;
+};
+
+__device__ __forceinline__ int find_surface(const CurrentParams& cp, int a, int b)
+{
+    const int64_t key = (int64_t)(a < b ? a : b) * cp.n_cells + (a < b ? b : a);
+    int l = 0, h = cp.n_pairs - 1;
+    while (l <= h) {
+        const int m = (l + h) >> 1;
+        const int64_t v = cp.pair_key[m];
+        if (v < key) l = m + 1;
+        else if (v > key) h = m - 1;
+        else return cp.pair_idx[m];
+    }
+    return -1;
+}
+
+// One warp per (track, direction), lanes over groups (the layout of k_sweep_atomic).  The cell of a segment and the
+// surface search are warp-uniform.
+template <int P, int EXPM>
+__global__ void __launch_bounds__(256) k_sweep_currents(const CurrentParams cp)
+{
+    const SweepParams& prm = cp.sw;
+    const int lane = threadIdx.x & 31;
+    const int warps_per_block = blockDim.x >> 5;
+    const int64_t n_chains = 2 * (int64_t)prm.T;
+    const float inv_f = (float)(1.0 / *prm.scale_div);
+    for (int64_t chain = (int64_t)blockIdx.x * warps_per_block + (threadIdx.x >> 5); chain < n_chains;
+         chain += (int64_t)gridDim.x * warps_per_block) {
+        const int t = (int)(chain >> 1), dir = (int)(chain & 1);
+        const int64_t k0 = prm.trk_off[t], k1 = prm.trk_off[t + 1];
+        if (k1 == k0) continue;
+        const float wt = prm.trk_w[t];
+        const int32_t lk = cp.link_fwd[chain];
+        const int32_t c2 = lk >= 0 ? cp.entry_cell[lk] : -1;
+        for (int g = lane; g < prm.G; g += 32) {
+            float psi[P];
+#pragma unroll
+            for (int p = 0; p < P; ++p) psi[p] = prm.psi_in[(chain * P + p) * prm.Gs + g] * inv_f;
+            int c_prev = -1;
+            for (int64_t i = 0; i < k1 - k0; ++i) {
+                const int64_t k = dir == 0 ? k0 + i : k1 - 1 - i;
+                const uint32_t rm = prm.seg_rm[k];
+                const float s = prm.seg_len[k];
+                const uint32_t r = rm_region(rm);
+                const int c = cp.cell[r];
+                if (c_prev >= 0 && c != c_prev) {
+                    const int sidx = find_surface(cp, c_prev, c);
+                    if (sidx < 0) {
+                        *cp.missing = 1;
+                    } else {
+                        float cur = 0.f;
+#pragma unroll
+                        for (int p = 0; p < P; ++p) cur = fmaf(prm.wp[p], psi[p], cur);
+                        const double j = (double)wt * (double)cur;
+                        atomicAdd(&cp.J_surf[(size_t)sidx * prm.G + g], c_prev < c ? j : -j);
+                    }
+                }
+                const float st = prm.sigt[rm_material(rm) * prm.Gs + g];
+                const float qv = prm.q[(size_t)r * prm.Gs + g];
+                attenuate<P, EXPM>(psi, qv, st * s, prm);
+                c_prev = c;
+            }
+            // chain end (C-3): what leaves minus what the opposite direction brings in at this end
+            float out = 0.f, net = 0.f;
+#pragma unroll
+            for (int p = 0; p < P; ++p) {
+                const float back = prm.psi_in[((chain ^ 1) * P + p) * prm.Gs + g] * inv_f;
+                out = fmaf(prm.wp[p], psi[p], out);
+                net = fmaf(prm.wp[p], psi[p] - back, net);
+            }
+            double* J = lk < 0 ? cp.J_vac : cp.J_ref;
+            atomicAdd(&J[(size_t)c_prev * prm.G + g], (double)wt * (double)net);
+            if (lk >= 0 && c2 != c_prev) {   // reflective hand-over into another coarse cell: a surface crossing
+                const int sidx = c2 >= 0 ? find_surface(cp, c_prev, c2) : -1;
+                if (sidx < 0) {
+                    *cp.missing = 1;
+                } else {
+                    const double j = (double)wt * (double)out;
+                    atomicAdd(&cp.J_surf[(size_t)sidx * prm.G + g], c_prev < c2 ? j : -j);
+                    atomicAdd(&cp.J_ref[(size_t)c_prev * prm.G + g], -j);
+                    atomicAdd(&cp.J_ref[(size_t)c2 * prm.G + g], j);
+                }
+            }
+        }
+    }
+}
+
+} // namespace ndk
