@@ -266,6 +266,33 @@ nd_status nd_sweep_currents(nd_problem* p, const double* d_Q, int32_t n_cells, c
                             const int32_t* pair_lo, const int32_t* pair_hi, double* J_surf, double* J_vac, double* J_ref,
                             void* cuda_stream);
 
+/* NEXT-3, step C-4 of DESIGN.md 8d: flux-volume weighted constants of the coarse cells ("Solve CMFD on the coarse mesh",
+ * PAPER.md:131-140), with the track-estimated areas A~_r the sweep itself uses.
+ *   d_phi_or_null  DEVICE [R][G] FP64, read; NULL = the problem's current flux (the result of the last power iteration)
+ *   cell           HOST [R], 0 <= cell[r] < n_cells
+ *   V              HOST [n_cells]           sum of A~_r
+ *   Phi            HOST [n_cells][G]        sum A~ phi / V
+ *   sigma_t, nu_sigma_f  HOST [n_cells][G]  sum A~ Sigma phi / sum A~ phi
+ *   sigma_s        HOST [n_cells][g][g']    from g' into g, weighted with phi_g'
+ *   chi            HOST [n_cells][G]        weighted with the fission emission sum_g' nuSigma_f phi_g' (0 where there is none)
+ * All G groups are kept.  A cell without regions gives NaN (0/0), as the plain definition does.  FP64 throughout; FP64
+ * atomics, so sums differ from a sequential sum in the last bits only.  Scratch is allocated and freed inside the call,
+ * the stream is synchronised before it returns; no state is changed.  Errors: ND_ERR_NULL, ND_ERR_INVALID, ND_ERR_RANGE,
+ * ND_ERR_CUDA. */
+nd_status nd_cmfd_collapse(nd_problem* p, const double* d_phi_or_null, int32_t n_cells, const int32_t* cell, double* V,
+                           double* Phi, double* sigma_t, double* sigma_s, double* nu_sigma_f, double* chi,
+                           void* cuda_stream);
+
+/* NEXT-3, step C-9 of DESIGN.md 8d ("update the fine-mesh flux", Algorithm 1): prolongation of a coarse
+ * solution onto the power-iteration state.
+ *   ratio  HOST [n_cells][G] FP64: Phi_new / Phi_old of every coarse cell
+ *   k_eff  the coarse eigenvalue; becomes the state's k
+ * phi[r][g] *= ratio[cell[r]][g]; the stored boundary flux of chain (t, d) *= ratio[cell of the region it enters][g]
+ * (FP32 storage, multiplied in FP64); the state's fission rate is recomputed from the new flux.  Works with every sweep
+ * kernel.  Synchronises the stream.  Errors: ND_ERR_NULL, ND_ERR_INVALID (k_eff <= 0, n_cells < 1), ND_ERR_RANGE. */
+nd_status nd_cmfd_prolong(nd_problem* p, int32_t n_cells, const int32_t* cell, const double* ratio, double k_eff,
+                          void* cuda_stream);
+
 /* Device-time accounting.  When enabled, every sweep-kernel launch is bracketed by CUDA events on its own
  * stream; nd_profile_read synchronises and returns the accumulated kernel milliseconds and launch counts
  * since the last nd_profile_enable(p,1).  kernels_launched counts every kernel the library launched. */

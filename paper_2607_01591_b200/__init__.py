@@ -25,7 +25,7 @@ EXPORTS = [
     "nd_tracks_generate", "nd_tracks_device_workspace_bytes", "nd_tracks_generate_device", "nd_tracks_view", "nd_tracks_destroy", "nd_workspace_bytes", "nd_problem_create",
     "nd_problem_destroy", "nd_transport_sweep", "nd_source_update", "nd_power_iteration", "nd_state_reset",
     "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_outgoing_flux_get", "nd_flux_get", "nd_flux_set",
-    "nd_track_volume_get", "nd_tally_get", "nd_sweep_currents", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
+    "nd_track_volume_get", "nd_tally_get", "nd_sweep_currents", "nd_cmfd_collapse", "nd_cmfd_prolong", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
     "nd_swath_stream_build", "nd_swath_stream_view", "nd_swath_stream_destroy",
     "nd_status_string", "nd_last_error", "nd_version",
 ]
@@ -136,6 +136,8 @@ def lib():
         L.nd_tally_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.nd_sweep_currents.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p,
                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nd_cmfd_collapse.argtypes = [C.c_void_p, C.c_void_p, C.c_int32] + [C.c_void_p] * 8
+        L.nd_cmfd_prolong.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         L.nd_profile_enable.argtypes = [C.c_void_p, C.c_int32]
         L.nd_profile_read.argtypes = [C.c_void_p, C.POINTER(nd_profile)]
         L.nd_sweep_phases_get.argtypes = [C.c_void_p, C.c_void_p]
@@ -380,6 +382,29 @@ class Problem:
                                        hi.ctypes.data, Js.ctypes.data, Jv.ctypes.data, Jr.ctypes.data, self._stream()),
                "nd_sweep_currents")
         return Js, Jv, Jr
+
+    def nd_cmfd_collapse(self, cell, n_cells, d_phi=None):
+        """C-4 (nd.h): returns HOST arrays as a dict V, Phi, sigt, sigs [C][g][g'], nusf, chi."""
+        cell = np.ascontiguousarray(cell, np.int32)
+        assert cell.shape == (self.R,)
+        if d_phi is not None:
+            t = self.torch
+            assert d_phi.dtype == t.float64 and d_phi.is_cuda and d_phi.is_contiguous() and d_phi.numel() == self.R * self.G
+        n, G = int(n_cells), self.G
+        out = dict(V=np.empty(n), Phi=np.empty((n, G)), sigt=np.empty((n, G)), sigs=np.empty((n, G, G)),
+                   nusf=np.empty((n, G)), chi=np.empty((n, G)))
+        _check(lib().nd_cmfd_collapse(self._h, d_phi.data_ptr() if d_phi is not None else None, n, cell.ctypes.data,
+                                      out["V"].ctypes.data, out["Phi"].ctypes.data, out["sigt"].ctypes.data,
+                                      out["sigs"].ctypes.data, out["nusf"].ctypes.data, out["chi"].ctypes.data,
+                                      self._stream()), "nd_cmfd_collapse")
+        return out
+
+    def nd_cmfd_prolong(self, cell, n_cells, ratio, k_eff):
+        cell = np.ascontiguousarray(cell, np.int32)
+        ratio = np.ascontiguousarray(ratio, np.float64)
+        assert cell.shape == (self.R,) and ratio.shape == (int(n_cells), self.G)
+        _check(lib().nd_cmfd_prolong(self._h, int(n_cells), cell.ctypes.data, ratio.ctypes.data, float(k_eff),
+                                     self._stream()), "nd_cmfd_prolong")
 
     def nd_profile_enable(self, on=True):
         _check(lib().nd_profile_enable(self._h, int(on)), "nd_profile_enable")

@@ -352,6 +352,7 @@ struct nd_problem {
     double mean_regions_per_tile = 0.0, mean_segments_per_tile = 0.0;
     // host copies
     std::vector<double> h_vol;
+    std::vector<int32_t> h_entry_region;   // [2T] first region of chain (t, d), -1 for an empty track (C-9)
     float c[ndk::kMaxPolar]{}, inv_sin[ndk::kMaxPolar]{}, wp[ndk::kMaxPolar]{};
     // profiling
     bool profile = false, phase_profile = false;
@@ -706,10 +707,15 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         h_len.assign(soa ? (size_t)d.Spad : 4, 0.f);
         h_off.resize((size_t)d.T + 1);
         p->h_vol.assign((size_t)d.R, 0.0);
+        p->h_entry_region.assign(2 * (size_t)d.T, -1);
         int64_t o = 0;
         for (int t = 0; t < d.T; ++t) {
             h_off[t] = o;
             const int64_t k0 = desc->track_seg_offset[t], k1 = desc->track_seg_offset[t + 1];
+            if (k1 > k0) {
+                p->h_entry_region[2 * (size_t)t] = desc->seg_region[k0];
+                p->h_entry_region[2 * (size_t)t + 1] = desc->seg_region[k1 - 1];
+            }
             const double w2 = 2.0 * desc->track_weight[t];
             uint32_t last = 0;
             for (int64_t k = k0; k < k1; ++k) {
@@ -1210,6 +1216,94 @@ extern "C" nd_status nd_sweep_currents(nd_problem* p, const double* d_Q, int32_t
     ND_CUDA(cudaMemcpyAsync(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
     ND_CUDA(cudaStreamSynchronize(st));
     if (flag) return nd_fail(ND_ERR_INVALID, "nd_sweep_currents: a track crosses between two coarse cells that are not a listed surface");
+    return ND_OK;
+}
+
+namespace {
+
+struct DeviceScratch {   // call-local device memory of the CMFD entry points (not on the hot path)
+    char* b = nullptr;
+    ~DeviceScratch() { if (b) cudaFree(b); }
+};
+
+nd_status check_cells(const nd_problem* p, int32_t n_cells, const int32_t* cell, const char* who)
+{
+    if (n_cells < 1) return nd_fail(ND_ERR_INVALID, (std::string(who) + ": n_cells must be >= 1").c_str());
+    for (int64_t r = 0; r < p->d.R; ++r)
+        if (cell[r] < 0 || cell[r] >= n_cells) return nd_fail(ND_ERR_RANGE, (std::string(who) + ": cell[r] out of [0, n_cells)").c_str());
+    return ND_OK;
+}
+
+} // namespace
+
+// NEXT-3, C-4: see nd.h.
+extern "C" nd_status nd_cmfd_collapse(nd_problem* p, const double* d_phi_or_null, int32_t n_cells, const int32_t* cell,
+                                      double* V, double* Phi, double* sigma_t, double* sigma_s, double* nu_sigma_f,
+                                      double* chi, void* cuda_stream)
+{
+    if (!p || !cell || !V || !Phi || !sigma_t || !sigma_s || !nu_sigma_f || !chi)
+        return nd_fail(ND_ERR_NULL, "nd_cmfd_collapse: NULL argument");
+    nd_status rc = check_cells(p, n_cells, cell, "nd_cmfd_collapse");
+    if (rc != ND_OK) return rc;
+    const Dims& d = p->d;
+    cudaStream_t st = as_stream(cuda_stream);
+    const double* phi = d_phi_or_null ? d_phi_or_null : p->phi_cur;
+    const size_t CG = (size_t)n_cells * d.G, nPsi = (size_t)n_cells * d.M * d.G, nOut = 4 * CG + CG * d.G;
+    auto up = [](size_t b) { return (b + 255) / 256 * 256; };
+    const size_t oPsi = 0, oV = oPsi + up(sizeof(double) * nPsi), oOut = oV + up(sizeof(double) * (size_t)n_cells),
+                 oCell = oOut + up(sizeof(double) * nOut), total = oCell + up(sizeof(int32_t) * (size_t)d.R);
+    DeviceScratch ds;
+    ND_CUDA(cudaMalloc(&ds.b, total));
+    double* dPsi = (double*)(ds.b + oPsi);
+    double* dV = (double*)(ds.b + oV);
+    double* dOut = (double*)(ds.b + oOut);
+    int32_t* dCell = (int32_t*)(ds.b + oCell);
+    ND_CUDA(cudaMemsetAsync(ds.b, 0, oOut, st));
+    ND_CUDA(cudaMemcpyAsync(dCell, cell, sizeof(int32_t) * (size_t)d.R, cudaMemcpyHostToDevice, st));
+    ndk::k_cmfd_accumulate<<<grid_for((int64_t)d.R * d.G, 256, 8 * p->n_sm), 256, 0, st>>>(phi, p->vol, p->reg_mat, dCell, dPsi, dV, d.R, d.G, d.M);
+    ND_LAUNCH_CHECK(p);
+    ndk::k_cmfd_constants<<<grid_for((int64_t)CG, 128, 8 * p->n_sm), 128, 0, st>>>(dPsi, dV, p->sigt, p->sigsT, p->nusf, p->chi, dOut, n_cells, d.G, d.M);
+    ND_LAUNCH_CHECK(p);
+    ND_CUDA(cudaMemcpyAsync(V, dV, sizeof(double) * (size_t)n_cells, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaMemcpyAsync(Phi, dOut, sizeof(double) * CG, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaMemcpyAsync(sigma_t, dOut + CG, sizeof(double) * CG, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaMemcpyAsync(nu_sigma_f, dOut + 2 * CG, sizeof(double) * CG, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaMemcpyAsync(chi, dOut + 3 * CG, sizeof(double) * CG, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaMemcpyAsync(sigma_s, dOut + 4 * CG, sizeof(double) * CG * d.G, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaStreamSynchronize(st));
+    return ND_OK;
+}
+
+// NEXT-3, C-9: see nd.h.
+extern "C" nd_status nd_cmfd_prolong(nd_problem* p, int32_t n_cells, const int32_t* cell, const double* ratio, double k_eff,
+                                     void* cuda_stream)
+{
+    if (!p || !cell || !ratio) return nd_fail(ND_ERR_NULL, "nd_cmfd_prolong: NULL argument");
+    if (!(k_eff > 0.0)) return nd_fail(ND_ERR_INVALID, "nd_cmfd_prolong: k_eff must be > 0");
+    nd_status rc = check_cells(p, n_cells, cell, "nd_cmfd_prolong");
+    if (rc != ND_OK) return rc;
+    const Dims& d = p->d;
+    cudaStream_t st = as_stream(cuda_stream);
+    const size_t CG = (size_t)n_cells * d.G, nE = 2 * (size_t)d.T;
+    auto up = [](size_t b) { return (b + 255) / 256 * 256; };
+    const size_t oRatio = 0, oCell = oRatio + up(sizeof(double) * CG), oEnt = oCell + up(sizeof(int32_t) * (size_t)d.R),
+                 total = oEnt + up(sizeof(int32_t) * nE);
+    DeviceScratch ds;
+    ND_CUDA(cudaMalloc(&ds.b, total));
+    double* dRatio = (double*)(ds.b + oRatio);
+    int32_t* dCell = (int32_t*)(ds.b + oCell);
+    int32_t* dEnt = (int32_t*)(ds.b + oEnt);
+    ND_CUDA(cudaMemcpyAsync(dRatio, ratio, sizeof(double) * CG, cudaMemcpyHostToDevice, st));
+    ND_CUDA(cudaMemcpyAsync(dCell, cell, sizeof(int32_t) * (size_t)d.R, cudaMemcpyHostToDevice, st));
+    ND_CUDA(cudaMemcpyAsync(dEnt, p->h_entry_region.data(), sizeof(int32_t) * nE, cudaMemcpyHostToDevice, st));
+    ND_CUDA(cudaMemcpyAsync(p->scalars + ndk::SC_K, &k_eff, sizeof(double), cudaMemcpyHostToDevice, st));
+    ndk::k_cmfd_prolong_phi<<<grid_for((int64_t)d.R * d.G, 256, 8 * p->n_sm), 256, 0, st>>>(p->phi_cur, dCell, dRatio, d.R, d.G);
+    ND_LAUNCH_CHECK(p);
+    ndk::k_cmfd_prolong_psi<<<grid_for((int64_t)nE * d.P * d.Gs, 256, 8 * p->n_sm), 256, 0, st>>>(p->psi_in, dEnt, dCell, dRatio, (int64_t)nE, d.P, d.G, d.Gs);
+    ND_LAUNCH_CHECK(p);
+    rc = launch_fission_rate(p, p->phi_cur, nullptr, st);   // the state's F belongs to its flux
+    if (rc != ND_OK) return rc;
+    ND_CUDA(cudaStreamSynchronize(st));
     return ND_OK;
 }
 

@@ -5,6 +5,9 @@
 //   k_entry_cell      coarse cell of the first region of every chain (t, d)
 //   k_sweep_currents  Eq. (5) per (track, direction, polar, group) as in k_sweep_atomic; instead of the
 //                     region tally it adds +-w psi at every change of coarse cell (C-3) and the end terms of C-3
+//   k_cmfd_accumulate C-4: Psi[c][m][g] = sum over the regions r of cell c with material m of A~_r phi[r][g], V[c]
+//   k_cmfd_constants  C-4: the flux-volume weighted coarse constants from Psi (every sum over regions is a sum over m)
+//   k_cmfd_prolong_*  C-9: phi[r][g] *= ratio[cell[r]][g]; boundary psi of chain (t, d) *= ratio[cell it enters][g]
 #pragma once
 #include "nd_kernels.cuh"
 
@@ -137,6 +140,85 @@ __global__ void __launch_bounds__(256) k_sweep_currents(const CurrentParams cp)
                 }
             }
         }
+    }
+}
+
+// ---- C-4, pass 1: thread per (r, g) ----
+__global__ void __launch_bounds__(256) k_cmfd_accumulate(const double* __restrict__ phi, const double* __restrict__ vol,
+                                                         const int32_t* __restrict__ reg_mat, const int32_t* __restrict__ cell,
+                                                         double* __restrict__ Psi, double* __restrict__ V, int64_t R, int G, int M)
+{
+    const int64_t n = R * G;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t r = i / G;
+        const int g = (int)(i - r * G);
+        const int c = cell[r];
+        const double a = vol[r];
+        atomicAdd(&Psi[((size_t)c * M + reg_mat[r]) * G + g], a * phi[i]);
+        if (g == 0) atomicAdd(&V[c], a);
+    }
+}
+
+// ---- C-4, pass 2: thread per (c, g).  out = [Phi | sigt | nusf | chi] each [C][G], then sigs [C][g][g'] ----
+__global__ void __launch_bounds__(128) k_cmfd_constants(const double* __restrict__ Psi, const double* __restrict__ V,
+                                                        const double* __restrict__ sigt, const double* __restrict__ sigsT,
+                                                        const double* __restrict__ nusf, const double* __restrict__ chi,
+                                                        double* __restrict__ out, int C, int G, int M)
+{
+    const int64_t n = (int64_t)C * G;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int c = (int)(i / G), g = (int)(i - (int64_t)c * G);
+        const double* psi_c = Psi + (size_t)c * M * G;
+        double phiV = 0.0, stPhi = 0.0, nfPhi = 0.0, chF = 0.0, F = 0.0;
+        for (int m = 0; m < M; ++m) {
+            const double x = psi_c[(size_t)m * G + g];
+            phiV += x;
+            stPhi += sigt[(size_t)m * G + g] * x;
+            nfPhi += nusf[(size_t)m * G + g] * x;
+            double f = 0.0;                                   // fission emission of material m in cell c
+            for (int gp = 0; gp < G; ++gp) f += nusf[(size_t)m * G + gp] * psi_c[(size_t)m * G + gp];
+            chF += chi[(size_t)m * G + g] * f;
+            F += f;
+        }
+        out[i] = phiV / V[c];
+        out[n + i] = stPhi / phiV;
+        out[2 * n + i] = nfPhi / phiV;
+        out[3 * n + i] = F > 0.0 ? chF / F : 0.0;
+        double* sigs = out + 4 * n + (size_t)i * G;           // row g of cell c: from g' into g
+        for (int gp = 0; gp < G; ++gp) {
+            double ss = 0.0, pv = 0.0;
+            for (int m = 0; m < M; ++m) {
+                const double x = psi_c[(size_t)m * G + gp];
+                ss += sigsT[((size_t)m * G + gp) * G + g] * x;
+                pv += x;
+            }
+            sigs[gp] = ss / pv;
+        }
+    }
+}
+
+// ---- C-9 ----
+__global__ void __launch_bounds__(256) k_cmfd_prolong_phi(double* __restrict__ phi, const int32_t* __restrict__ cell,
+                                                          const double* __restrict__ ratio, int64_t R, int G)
+{
+    const int64_t n = R * G;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t r = i / G;
+        phi[i] *= ratio[(size_t)cell[r] * G + (i - r * G)];
+    }
+}
+
+// psi [2T][P][Gs] FP32; entry_region[e] = first region of chain e (-1: empty track)
+__global__ void __launch_bounds__(256) k_cmfd_prolong_psi(float* __restrict__ psi, const int32_t* __restrict__ entry_region,
+                                                          const int32_t* __restrict__ cell, const double* __restrict__ ratio,
+                                                          int64_t n_entries, int P, int G, int Gs)
+{
+    const int64_t PG = (int64_t)P * Gs, n = n_entries * PG;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t e = i / PG;
+        const int g = (int)((i - e * PG) % Gs);
+        const int32_t r = entry_region[e];
+        if (r >= 0 && g < G) psi[i] = (float)((double)psi[i] * ratio[(size_t)cell[r] * G + g]);
     }
 }
 
