@@ -225,3 +225,53 @@ def test_cmfd_iteration_composed_from_the_gpu_steps(case):
         assert phi_rel_err(phi_g / phi_g.sum(), phi_o / phi_o.sum()) <= PHI_RTOL
     finally:
         pair.close()
+
+
+@pytest.mark.parametrize("idx,nx,ny,with_oracle", [(3, 12, 12, True), (4, 16, 16, False)], ids=["cfg3", "cfg4"])
+def test_currents_at_full_size(idx, nx, ny, with_oracle):
+    """BASELINE.json's full configs 3 and 4: config 3 against the oracle surface by surface; both by the C-3 balance with
+    the tallies of the GPU's own sweep, which holds at any size.  Prints the whole-call times (wall clock; the calls
+    allocate, copy the cell map in and the currents out, and synchronise)."""
+    import time
+    pair = make_pair(idx, 1.0, sweep_kernel=nd.ND_SWEEP_ATOMIC)
+    try:
+        Q, psi = seeded_sweep_inputs(pair, seed=700 + idx)
+        n_cells = nx * ny
+        cell = cartesian_cells(pair.prob.mesh, nx, ny)
+        lo, hi = cmfd.coarse_surfaces(pair.o_tr.seg_offset, pair.o_tr.seg_region, cell, pair.o_tr.link)
+        dQ = torch.from_numpy(Q).cuda()
+        pair.gpu.nd_boundary_flux_set(psi)
+        pair.gpu.nd_sweep_currents(dQ, cell, n_cells, lo, hi)            # warm-up
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        Js, Jv, Jr = pair.gpu.nd_sweep_currents(dQ, cell, n_cells, lo, hi)
+        t_cur = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        co = pair.gpu.nd_cmfd_collapse(cell, n_cells, dQ)
+        t_col = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        pair.gpu.nd_transport_sweep(dQ)
+        torch.cuda.synchronize()
+        t_swp = time.perf_counter() - t0
+        tally = pair.gpu.nd_tally_get().cpu().numpy()
+        print(f"cfg{idx} full: R {pair.R} G {pair.G} segments {pair.o_tr.seg_offset[-1]} cells {n_cells} surfaces {len(lo)}: "
+              f"nd_sweep_currents {t_cur * 1e3:.2f} ms, nd_cmfd_collapse {t_col * 1e3:.2f} ms, "
+              f"nd_transport_sweep (atomic kernel) {t_swp * 1e3:.2f} ms")
+        assert np.isfinite(co["Phi"]).all() and abs(co["V"].sum() - pair.o_tr.volume.sum()) <= 1e-12 * co["V"].sum()
+        net = np.zeros((n_cells, pair.G))
+        np.add.at(net, cell, tally)
+        np.add.at(net, lo, Js)
+        np.add.at(net, hi, -Js)
+        net += Jv + Jr
+        gross = np.zeros((n_cells, pair.G))
+        np.add.at(gross, cell, np.abs(tally))
+        print(f"cfg{idx} full balance: {np.abs(net).max() / gross.max():.3e}")
+        assert np.abs(net).max() <= BALANCE_RTOL * gross.max()
+        if with_oracle:
+            Js_o, Jv_o, Jr_o = _oracle_currents(pair, Q, psi, cell, n_cells, lo, hi)
+            for name, g, o in (("J_surf", Js, Js_o), ("J_vac", Jv, Jv_o), ("J_ref", Jr, Jr_o)):
+                ref = np.abs(o).max()
+                print(f"cfg{idx} full {name}: ratio {np.abs(g - o).max() / max(ref, 1e-300):.3e}")
+                assert np.abs(g - o).max() <= J_RTOL * ref, name
+    finally:
+        pair.close()
