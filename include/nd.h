@@ -293,6 +293,25 @@ nd_status nd_cmfd_collapse(nd_problem* p, const double* d_phi_or_null, int32_t n
 nd_status nd_cmfd_prolong(nd_problem* p, int32_t n_cells, const int32_t* cell, const double* ratio, double k_eff,
                           void* cuda_stream);
 
+/* NEXT-3, steps C-5..C-8 of DESIGN.md 8d ("Solve CMFD on the coarse mesh", Algorithm 1): the coarse
+ * balance  sum_s outflow + alpha Phi + Sigma_t V Phi - V sum_g' Sigma_s Phi_g' = (1/k) chi V sum_g' nuSigma_f Phi_g'
+ * with D = 1/(3 Sigma_t), Dhat_s = 2 D_lo D_hi / (D_lo + D_hi) x coupling_s, Dtil_s = -(J_s + Dhat (Phi_hi - Phi_lo)) /
+ * (Phi_hi + Phi_lo), alpha = J_vac / Phi (reflective ends: J = 0), and its dominant eigenpair by power iteration with an
+ * exact inner solve (dense inverse of the loss operator, in-place Gauss-Jordan on the device), started from Phi and k0.
+ * All pointers HOST (the coarse arrays are small); all arithmetic runs in CUDA kernels, FP64.
+ *   V [C]; Phi, sigma_t, nu_sigma_f, chi, J_vac [C][G]; sigma_s [C][g][g'] (from g' into g): as nd_cmfd_collapse and
+ *   nd_sweep_currents return them (currents on the scale of Phi)
+ *   pair_lo/pair_hi/coupling [S], J_surf [S][G]: the surfaces, A_s / d_s per surface (0: no diffusive coupling)
+ *   tol: |dk| < tol |k| and max |dPhi| < 1e-11 max |Phi| end the iteration (at most max_outer iterations)
+ *   k_out, Phi_new [C][G] (normalised to the fission production of Phi), iters_done (may be NULL)
+ * Errors: ND_ERR_NULL, ND_ERR_INVALID, ND_ERR_RANGE (a pair out of range; more than 8192 unknowns),
+ * ND_ERR_NOT_CONVERGED (outputs are written), ND_ERR_CUDA.  Synchronises the stream. */
+nd_status nd_cmfd_coarse_solve(int32_t n_cells, int32_t n_groups, const double* V, const double* Phi, const double* sigma_t,
+                               const double* sigma_s, const double* nu_sigma_f, const double* chi, int32_t n_pairs,
+                               const int32_t* pair_lo, const int32_t* pair_hi, const double* coupling, const double* J_surf,
+                               const double* J_vac, double k0, double tol, int32_t max_outer, double* k_out,
+                               double* Phi_new, int32_t* iters_done, void* cuda_stream);
+
 /* Device-time accounting.  When enabled, every sweep-kernel launch is bracketed by CUDA events on its own
  * stream; nd_profile_read synchronises and returns the accumulated kernel milliseconds and launch counts
  * since the last nd_profile_enable(p,1).  kernels_launched counts every kernel the library launched. */

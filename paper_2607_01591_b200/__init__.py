@@ -25,7 +25,7 @@ EXPORTS = [
     "nd_tracks_generate", "nd_tracks_device_workspace_bytes", "nd_tracks_generate_device", "nd_tracks_view", "nd_tracks_destroy", "nd_workspace_bytes", "nd_problem_create",
     "nd_problem_destroy", "nd_transport_sweep", "nd_source_update", "nd_power_iteration", "nd_state_reset",
     "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_outgoing_flux_get", "nd_flux_get", "nd_flux_set",
-    "nd_track_volume_get", "nd_tally_get", "nd_sweep_currents", "nd_cmfd_collapse", "nd_cmfd_prolong", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
+    "nd_track_volume_get", "nd_tally_get", "nd_sweep_currents", "nd_cmfd_collapse", "nd_cmfd_prolong", "nd_cmfd_coarse_solve", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
     "nd_swath_stream_build", "nd_swath_stream_view", "nd_swath_stream_destroy",
     "nd_status_string", "nd_last_error", "nd_version",
 ]
@@ -138,6 +138,9 @@ def lib():
                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.nd_cmfd_collapse.argtypes = [C.c_void_p, C.c_void_p, C.c_int32] + [C.c_void_p] * 8
         L.nd_cmfd_prolong.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
+        L.nd_cmfd_coarse_solve.argtypes = ([C.c_int32, C.c_int32] + [C.c_void_p] * 6 + [C.c_int32] + [C.c_void_p] * 5 +
+                                           [C.c_double, C.c_double, C.c_int32, C.POINTER(C.c_double), C.c_void_p,
+                                            C.POINTER(C.c_int32), C.c_void_p])
         L.nd_profile_enable.argtypes = [C.c_void_p, C.c_int32]
         L.nd_profile_read.argtypes = [C.c_void_p, C.POINTER(nd_profile)]
         L.nd_sweep_phases_get.argtypes = [C.c_void_p, C.c_void_p]
@@ -242,6 +245,24 @@ def nd_tracks_generate_device(xy, tri, W, H, bc, n_azim, spacing, segment_capaci
     out = Tracks(h, v)
     out.timing = {f[0]: getattr(tm, f[0]) for f in nd_trace_timing._fields_ if f[0] != "reserved"}
     return out
+
+
+def nd_cmfd_coarse_solve(co, pair_lo, pair_hi, coupling, J_surf, J_vac, k0, tol=1e-13, max_outer=100000, stream=None):
+    """C-5..C-8 (nd.h): co = the dict nd_cmfd_collapse returns.  Returns (k, Phi_new [C][G], iterations)."""
+    def f8(a):
+        return np.ascontiguousarray(a, np.float64)
+    V, Phi, st, ss, nf, ch = (f8(co[k]) for k in ("V", "Phi", "sigt", "sigs", "nusf", "chi"))
+    n, G = Phi.shape
+    lo, hi = np.ascontiguousarray(pair_lo, np.int32), np.ascontiguousarray(pair_hi, np.int32)
+    cpl, Js, Jv = f8(coupling), f8(J_surf), f8(J_vac)
+    assert ss.shape == (n, G, G) and Jv.shape == (n, G) and Js.shape == (len(lo), G) and cpl.shape == (len(lo),)
+    k, it, out = C.c_double(), C.c_int32(), np.empty((n, G))
+    rc = lib().nd_cmfd_coarse_solve(n, G, V.ctypes.data, Phi.ctypes.data, st.ctypes.data, ss.ctypes.data, nf.ctypes.data,
+                                    ch.ctypes.data, len(lo), lo.ctypes.data, hi.ctypes.data, cpl.ctypes.data, Js.ctypes.data,
+                                    Jv.ctypes.data, float(k0), float(tol), int(max_outer), C.byref(k), out.ctypes.data,
+                                    C.byref(it), stream)
+    _check(rc, "nd_cmfd_coarse_solve")
+    return k.value, out, it.value
 
 
 class Problem:

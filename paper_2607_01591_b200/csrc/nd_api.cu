@@ -1307,6 +1307,99 @@ extern "C" nd_status nd_cmfd_prolong(nd_problem* p, int32_t n_cells, const int32
     return ND_OK;
 }
 
+// NEXT-3, C-5..C-8: see nd.h.
+extern "C" nd_status nd_cmfd_coarse_solve(int32_t n_cells, int32_t n_groups, const double* V, const double* Phi,
+                                          const double* sigma_t, const double* sigma_s, const double* nu_sigma_f,
+                                          const double* chi, int32_t n_pairs, const int32_t* pair_lo, const int32_t* pair_hi,
+                                          const double* coupling, const double* J_surf, const double* J_vac, double k0,
+                                          double tol, int32_t max_outer, double* k_out, double* Phi_new, int32_t* iters_done,
+                                          void* cuda_stream)
+{
+    if (!V || !Phi || !sigma_t || !sigma_s || !nu_sigma_f || !chi || !J_vac || !k_out || !Phi_new ||
+        (n_pairs > 0 && (!pair_lo || !pair_hi || !coupling || !J_surf)))
+        return nd_fail(ND_ERR_NULL, "nd_cmfd_coarse_solve: NULL argument");
+    if (n_cells < 1 || n_groups < 1 || n_pairs < 0 || !(k0 > 0.0) || !(tol > 0.0) || max_outer < 1)
+        return nd_fail(ND_ERR_INVALID, "nd_cmfd_coarse_solve: sizes must be positive, k0 > 0, tol > 0, max_outer >= 1");
+    const int64_t n = (int64_t)n_cells * n_groups;
+    if (n > 8192) return nd_fail(ND_ERR_RANGE, "nd_cmfd_coarse_solve: more than 8192 coarse unknowns (dense inverse)");
+    for (int32_t s = 0; s < n_pairs; ++s)
+        if (pair_lo[s] < 0 || pair_hi[s] >= n_cells || pair_lo[s] >= pair_hi[s])
+            return nd_fail(ND_ERR_RANGE, "nd_cmfd_coarse_solve: a surface needs 0 <= lo < hi < n_cells");
+    cudaStream_t st = as_stream(cuda_stream);
+    int n_sm = 148;
+    {
+        int dev = 0;
+        ND_CUDA(cudaGetDevice(&dev));
+        ND_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    }
+    const int C = n_cells, G = n_groups, S = n_pairs;
+    const size_t CG = (size_t)n, SG = (size_t)S * G;
+    // scratch (doubles): A[n][n] | V | Phi | sigt | sigs | nusf | chi | J_vac | coupling | J_surf | x | y | f | col | row | state[2]
+    size_t o = 0;
+    auto take = [&o](size_t count) { const size_t at = o; o += (count + 31) / 32 * 32; return at; };
+    const size_t oA = take(CG * CG), oV = take(C), oPhi = take(CG), oSt = take(CG), oSs = take(CG * G), oNf = take(CG),
+                 oChi = take(CG), oJv = take(CG), oCo = take(S), oJs = take(SG), oX = take(CG), oY = take(CG), oF = take(CG),
+                 oCol = take(CG), oRow = take(CG), oState = take(2), nD = o;
+    const size_t bytes = sizeof(double) * nD + sizeof(int32_t) * (2 * (size_t)S + 64);
+    DeviceScratch ds;
+    ND_CUDA(cudaMalloc(&ds.b, bytes));
+    double* D = (double*)ds.b;
+    int32_t* I = (int32_t*)(ds.b + sizeof(double) * nD);   // lo [S] | hi [S] | done | iters
+    int32_t* d_lo = I; int32_t* d_hi = I + S; int* d_done = I + 2 * S; int* d_iters = d_done + 1;
+    ND_CUDA(cudaMemsetAsync(D + oA, 0, sizeof(double) * CG * CG, st));
+    ND_CUDA(cudaMemsetAsync(d_done, 0, 2 * sizeof(int), st));
+    auto h2d = [&](size_t at, const double* src, size_t count) {
+        return count ? cudaMemcpyAsync(D + at, src, sizeof(double) * count, cudaMemcpyHostToDevice, st) : cudaSuccess;
+    };
+    ND_CUDA(h2d(oV, V, C)); ND_CUDA(h2d(oPhi, Phi, CG)); ND_CUDA(h2d(oSt, sigma_t, CG)); ND_CUDA(h2d(oSs, sigma_s, CG * G));
+    ND_CUDA(h2d(oNf, nu_sigma_f, CG)); ND_CUDA(h2d(oChi, chi, CG)); ND_CUDA(h2d(oJv, J_vac, CG));
+    ND_CUDA(h2d(oCo, coupling, S)); ND_CUDA(h2d(oJs, J_surf, SG)); ND_CUDA(h2d(oX, Phi, CG));
+    const double state0[2] = {k0, 0.0};
+    ND_CUDA(h2d(oState, state0, 2));
+    if (S > 0) {
+        ND_CUDA(cudaMemcpyAsync(d_lo, pair_lo, sizeof(int32_t) * S, cudaMemcpyHostToDevice, st));
+        ND_CUDA(cudaMemcpyAsync(d_hi, pair_hi, sizeof(int32_t) * S, cudaMemcpyHostToDevice, st));
+    }
+    ndk::CoarseParams cp{};
+    cp.V = D + oV; cp.Phi = D + oPhi; cp.sigt = D + oSt; cp.sigs = D + oSs; cp.nusf = D + oNf; cp.chi = D + oChi;
+    cp.J_vac = D + oJv; cp.lo = d_lo; cp.hi = d_hi; cp.coupling = D + oCo; cp.J_surf = D + oJs; cp.A = D + oA;
+    cp.C = C; cp.G = G; cp.S = S;
+    const int cap = 8 * n_sm;
+    ndk::k_coarse_cell_blocks<<<grid_for((int64_t)CG * G, 256, cap), 256, 0, st>>>(cp);
+    if (S > 0) ndk::k_coarse_surfaces<<<grid_for((int64_t)SG, 256, cap), 256, 0, st>>>(cp);
+    for (int64_t piv = 0; piv < n; ++piv) {          // A <- A^-1 in place
+        ndk::k_gj_prepare<<<grid_for(n, 256, cap), 256, 0, st>>>(D + oA, D + oCol, D + oRow, n, piv);
+        ndk::k_gj_update<<<grid_for(n * n, 256, cap), 256, 0, st>>>(D + oA, D + oCol, D + oRow, n, piv);
+    }
+    ND_CUDA(cudaGetLastError());
+    // P0 = sum(B Phi), then outer iterations in batches; the kernels turn into no-ops once the flag is set
+    ndk::k_coarse_fission<<<grid_for(n, 256, cap), 256, 0, st>>>(D + oX, cp.V, cp.nusf, cp.chi, D + oF, C, G, nullptr);
+    ndk::k_coarse_update<<<1, 1024, 0, st>>>(D + oX, D + oY, D + oF, cp.V, cp.nusf, cp.chi, D + oState, d_done, d_iters, C, G, tol, 1);
+    int done = 0, iters = 0;
+    const int batch = 32;
+    while (!done && iters < max_outer) {
+        const int todo = max_outer - iters < batch ? max_outer - iters : batch;
+        for (int b = 0; b < todo; ++b) {
+            ndk::k_coarse_fission<<<grid_for(n, 256, cap), 256, 0, st>>>(D + oX, cp.V, cp.nusf, cp.chi, D + oF, C, G, d_done);
+            ndk::k_coarse_matvec<<<grid_for(n * 32, 256, cap), 256, 0, st>>>(D + oA, D + oF, D + oY, n, d_done);
+            ndk::k_coarse_update<<<1, 1024, 0, st>>>(D + oX, D + oY, D + oF, cp.V, cp.nusf, cp.chi, D + oState, d_done, d_iters, C, G, tol, 0);
+        }
+        ND_CUDA(cudaGetLastError());
+        int h[2];
+        ND_CUDA(cudaMemcpyAsync(h, d_done, sizeof h, cudaMemcpyDeviceToHost, st));
+        ND_CUDA(cudaStreamSynchronize(st));
+        done = h[0]; iters = h[1];
+    }
+    double hstate[2];
+    ND_CUDA(cudaMemcpyAsync(hstate, D + oState, sizeof hstate, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaMemcpyAsync(Phi_new, D + oX, sizeof(double) * CG, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaStreamSynchronize(st));
+    *k_out = hstate[0];
+    if (iters_done) *iters_done = iters;
+    if (!done) return nd_fail(ND_ERR_NOT_CONVERGED, "nd_cmfd_coarse_solve: max_outer reached (outputs are written)");
+    return ND_OK;
+}
+
 extern "C" nd_status nd_profile_enable(nd_problem* p, int32_t on)
 {
     if (!p) return nd_fail(ND_ERR_NULL, "nd_profile_enable: NULL problem");

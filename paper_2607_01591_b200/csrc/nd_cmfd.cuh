@@ -8,6 +8,9 @@
 //   k_cmfd_accumulate C-4: Psi[c][m][g] = sum over the regions r of cell c with material m of A~_r phi[r][g], V[c]
 //   k_cmfd_constants  C-4: the flux-volume weighted coarse constants from Psi (every sum over regions is a sum over m)
 //   k_cmfd_prolong_*  C-9: phi[r][g] *= ratio[cell[r]][g]; boundary psi of chain (t, d) *= ratio[cell it enters][g]
+//   k_coarse_*        C-5..C-8: dense coarse operator A (removal - scatter + alpha + Dhat -+ Dtil couplings), its inverse by
+//                     in-place Gauss-Jordan (no pivoting: A is a diagonally dominant M-matrix-like operator), and the
+//                     power iteration A Phi = (1/k) B Phi with B = chi (nuSigma_f V)^T applied cell by cell
 #pragma once
 #include "nd_kernels.cuh"
 
@@ -219,6 +222,154 @@ __global__ void __launch_bounds__(256) k_cmfd_prolong_psi(float* __restrict__ ps
         const int g = (int)((i - e * PG) % Gs);
         const int32_t r = entry_region[e];
         if (r >= 0 && g < G) psi[i] = (float)((double)psi[i] * ratio[(size_t)cell[r] * G + g]);
+    }
+}
+
+// ---- C-5..C-7: the dense coarse operator, unknowns ordered [cell][group], n = C G ----
+struct CoarseParams {
+    const double* __restrict__ V;      // [C]
+    const double* __restrict__ Phi;    // [C][G]
+    const double* __restrict__ sigt;   // [C][G]
+    const double* __restrict__ sigs;   // [C][g][g']
+    const double* __restrict__ nusf;   // [C][G]
+    const double* __restrict__ chi;    // [C][G]
+    const double* __restrict__ J_vac;  // [C][G]
+    const int32_t* __restrict__ lo;    // [S]
+    const int32_t* __restrict__ hi;    // [S]
+    const double* __restrict__ coupling; // [S] A_s / d_s
+    const double* __restrict__ J_surf; // [S][G]
+    double* __restrict__ A;            // [n][n], zeroed by the caller
+    int C, G, S;
+};
+
+__global__ void __launch_bounds__(256) k_coarse_cell_blocks(const CoarseParams cp)
+{
+    const int G = cp.G;
+    const int64_t n = (int64_t)cp.C * G, total = n * G;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t row = i / G;                 // c G + g
+        const int gp = (int)(i - row * G);
+        const int c = (int)(row / G), g = (int)(row - (int64_t)c * G);
+        double v = -cp.sigs[i] * cp.V[c];
+        if (gp == g) v += cp.sigt[row] * cp.V[c] + cp.J_vac[row] / cp.Phi[row];   // removal + vacuum ends (alpha, C-6)
+        cp.A[row * n + (int64_t)c * G + gp] = v;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_coarse_surfaces(const CoarseParams cp)
+{
+    const int G = cp.G;
+    const int64_t n = (int64_t)cp.C * G, total = (int64_t)cp.S * G;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        const int s = (int)(i / G), g = (int)(i - (int64_t)s * G);
+        const int64_t a = (int64_t)cp.lo[s] * G + g, b = (int64_t)cp.hi[s] * G + g;
+        const double Da = 1.0 / (3.0 * cp.sigt[a]), Db = 1.0 / (3.0 * cp.sigt[b]);                 // C-5
+        const double Dhat = 2.0 * Da * Db / (Da + Db) * cp.coupling[s];
+        const double Dtil = -(cp.J_surf[i] + Dhat * (cp.Phi[b] - cp.Phi[a])) / (cp.Phi[b] + cp.Phi[a]);   // C-6
+        const double out_lo = Dhat - Dtil, in_hi = Dhat + Dtil;                                     // J = out_lo Phi_lo - in_hi Phi_hi
+        atomicAdd(&cp.A[a * n + a], out_lo);
+        atomicAdd(&cp.A[a * n + b], -in_hi);
+        atomicAdd(&cp.A[b * n + b], in_hi);
+        atomicAdd(&cp.A[b * n + a], -out_lo);
+    }
+}
+
+// ---- in-place Gauss-Jordan inverse, pivot p: (1) save column p and the scaled pivot row, (2) rank-1 update ----
+__global__ void __launch_bounds__(256) k_gj_prepare(const double* __restrict__ A, double* __restrict__ col,
+                                                    double* __restrict__ row, int64_t n, int64_t p)
+{
+    const double inv = 1.0 / A[p * n + p];
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        col[i] = A[i * n + p];
+        row[i] = i == p ? inv : A[p * n + i] * inv;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_gj_update(double* __restrict__ A, const double* __restrict__ col,
+                                                   const double* __restrict__ row, int64_t n, int64_t p)
+{
+    const int64_t total = n * n;
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = k / n, j = k - i * n;
+        A[k] = i == p ? row[j] : (j == p ? 0.0 : A[k]) - col[i] * row[j];
+    }
+}
+
+// ---- C-8: f = B x, with B[(c,g),(c,g')] = chi[c][g] nuSigma_f[c][g'] V[c] ----
+__global__ void __launch_bounds__(256) k_coarse_fission(const double* __restrict__ x, const double* __restrict__ V,
+                                                        const double* __restrict__ nusf, const double* __restrict__ chi,
+                                                        double* __restrict__ f, int C, int G, const int* __restrict__ done)
+{
+    if (done && *done) return;
+    const int64_t n = (int64_t)C * G;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int c = (int)(i / G);
+        double e = 0.0;
+        for (int gp = 0; gp < G; ++gp) e += nusf[(size_t)c * G + gp] * x[(size_t)c * G + gp];
+        f[i] = chi[i] * V[c] * e;
+    }
+}
+
+// y = Ainv f, one warp per row
+__global__ void __launch_bounds__(256) k_coarse_matvec(const double* __restrict__ Ainv, const double* __restrict__ f,
+                                                       double* __restrict__ y, int64_t n, const int* __restrict__ done)
+{
+    if (*done) return;
+    const int lane = threadIdx.x & 31;
+    for (int64_t r = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; r < n; r += ((int64_t)gridDim.x * blockDim.x) >> 5) {
+        double acc = 0.0;
+        for (int64_t j = lane; j < n; j += 32) acc += Ainv[r * n + j] * f[j];
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+        if (lane == 0) y[r] = acc;
+    }
+}
+
+// One block.  With y' = Ainv f (= k times the oracle's y): k_new = sum(B y') / sum(f); x_new = y' P0 / sum(B y');
+// converged when |k_new - k| < tol |k_new| and max |x_new - x| < 1e-11 max |x_new| (the oracle's test).
+// state: [0] k, [1] P0 (sum B x0; set by the first call when init != 0).
+__global__ void __launch_bounds__(1024) k_coarse_update(double* __restrict__ x, const double* __restrict__ y,
+                                                        const double* __restrict__ f, const double* __restrict__ V, const double* __restrict__ nusf,
+                                                        const double* __restrict__ chi, double* __restrict__ state,
+                                                        int* __restrict__ done, int* __restrict__ iters, int C, int G,
+                                                        double tol, int init)
+{
+    __shared__ double scratch[32];
+    __shared__ double bc[2];                        // block_sum / block_max leave their result in thread 0 only
+    if (*done) return;
+    const int64_t n = (int64_t)C * G;
+    double sf = 0.0;
+    for (int64_t i = threadIdx.x; i < n; i += blockDim.x) sf += f[i];
+    sf = block_sum(sf, scratch);
+    if (init) {                                     // P0 = sum(B x0) = sum(f) of the first product
+        if (threadIdx.x == 0) state[1] = sf;
+        return;
+    }
+    double sby = 0.0;
+    for (int64_t i = threadIdx.x; i < n; i += blockDim.x) {
+        const int c = (int)(i / G);
+        double e = 0.0;
+        for (int gp = 0; gp < G; ++gp) e += nusf[(size_t)c * G + gp] * y[(size_t)c * G + gp];
+        sby += chi[i] * V[c] * e;
+    }
+    sby = block_sum(sby, scratch);
+    if (threadIdx.x == 0) { bc[0] = sf; bc[1] = sby; }
+    __syncthreads();
+    sf = bc[0]; sby = bc[1];
+    const double k_old = state[0], k_new = sby / sf, scale = state[1] / sby;
+    double dmax = 0.0, ymax = 0.0;
+    for (int64_t i = threadIdx.x; i < n; i += blockDim.x) {
+        const double v = y[i] * scale;
+        dmax = fmax(dmax, fabs(v - x[i]));
+        ymax = fmax(ymax, fabs(v));
+        x[i] = v;
+    }
+    dmax = block_max(dmax, scratch);
+    ymax = block_max(ymax, scratch);
+    __syncthreads();                                // every thread has read state[0] before it is replaced
+    if (threadIdx.x == 0) {
+        state[0] = k_new;
+        ++*iters;
+        if (fabs(k_new - k_old) < tol * fabs(k_new) && dmax < 1e-11 * ymax) *done = 1;
     }
 }
 

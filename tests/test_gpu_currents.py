@@ -6,6 +6,7 @@ import pytest
 
 torch = pytest.importorskip("torch")
 
+import oracle
 import paper_2607_01591_b200 as nd
 from oracle import cmfd
 from moc_inputs.coarse import cartesian_cells
@@ -273,5 +274,80 @@ def test_currents_at_full_size(idx, nx, ny, with_oracle):
                 ref = np.abs(o).max()
                 print(f"cfg{idx} full {name}: ratio {np.abs(g - o).max() / max(ref, 1e-300):.3e}")
                 assert np.abs(g - o).max() <= J_RTOL * ref, name
+    finally:
+        pair.close()
+
+
+def _coarse_inputs(pair, nx, ny, seed):
+    """A coarse problem as the accelerated iteration meets it: currents and collapse of one oracle sweep."""
+    p, t = pair.prob, pair.o_tr
+    rng = np.random.default_rng(seed)
+    phi = rng.uniform(0.5, 1.5, (pair.R, pair.G))
+    psi = rng.uniform(0.0, 0.2, (pair.T, 2, pair.P, pair.G))
+    cell = cartesian_cells(p.mesh, nx, ny)
+    lo, hi = cmfd.coarse_surfaces(t.seg_offset, t.seg_region, cell, t.link)
+    Q = oracle.source(p.mesh.material, p.xs.sigma_s, p.xs.nu_sigma_f, p.xs.chi, phi, 1.0)
+    phi_new, _, _ = pair.oracle_sweep(Q, psi)
+    Js, Jv, _ = _oracle_currents(pair, Q, psi, cell, nx * ny, lo, hi)
+    co = _oracle_collapse(pair, phi_new, cell, nx * ny)
+    return co, lo, hi, cartesian_coupling(p.mesh, nx, ny)(lo, hi), Js, Jv
+
+
+@pytest.mark.parametrize("case", [(1, 1.0, 3, 2), (2, 0.15, 8, 8), (3, 0.03, 5, 4)], ids=["cfg1", "cfg2", "cfg3"])
+def test_coarse_solve_matches_oracle(case):
+    """C-5..C-8: the same dominant eigenpair as the oracle's power iteration with numpy's dense inverse (both stop at
+    |dk| < 1e-13 |k|, max |dPhi| < 1e-11 max |Phi|)."""
+    idx, scale, nx, ny = case
+    pair = make_pair(idx, scale)
+    try:
+        co, lo, hi, coupling, Js, Jv = _coarse_inputs(pair, nx, ny, seed=900 + idx)
+        A, B, _, _, _ = cmfd.coarse_operators(co, lo, hi, coupling, Js, Jv)
+        k_o, Phi_o = cmfd.coarse_eigen(A, B, co["Phi"], 1.0)
+        k_g, Phi_g, iters = nd.nd_cmfd_coarse_solve(co, lo, hi, coupling, Js, Jv, 1.0)
+        print(f"cfg{idx} coarse solve: n {Phi_o.size} k gpu {k_g!r} oracle {k_o!r} iterations {iters} "
+              f"max rel dPhi {np.abs(Phi_g / Phi_o - 1).max():.2e}")
+        assert abs(k_g - k_o) <= 1e-10 * abs(k_o)
+        np.testing.assert_allclose(Phi_g, Phi_o, rtol=1e-8)
+        # the pair solves the balance: A Phi = (1/k) B Phi, with the oracle's operators
+        res = A @ Phi_g.reshape(-1) - (B @ Phi_g.reshape(-1)) / k_g
+        assert np.abs(res).max() <= 1e-9 * np.abs(A @ Phi_g.reshape(-1)).max()
+        with pytest.raises(nd.NdError, match="max_outer"):
+            nd.nd_cmfd_coarse_solve(co, lo, hi, coupling, Js, Jv, 1.0, max_outer=2)
+    finally:
+        pair.close()
+
+
+@pytest.mark.parametrize("case", [(1, 1.0, 3, 2), (2, 0.15, 8, 8)], ids=["cfg1", "cfg2"])
+def test_cmfd_iteration_all_steps_on_the_gpu(case):
+    """As the composed test above, with C-5..C-8 on the GPU too: nothing of the oracle runs in the loop."""
+    idx, scale, nx, ny = case
+    n_iters, n_cells = 6, nx * ny
+    pair = make_pair(idx, scale, sweep_kernel=nd.ND_SWEEP_ATOMIC)
+    try:
+        p, t = pair.prob, pair.o_tr
+        cell = cartesian_cells(p.mesh, nx, ny)
+        coupling_of = cartesian_coupling(p.mesh, nx, ny)
+        _, phi_o, _, hist_o = cmfd.power_iteration_cmfd(p.mesh.material, p.xs.sigma_t, p.xs.sigma_s, p.xs.nu_sigma_f,
+                                                        p.xs.chi, p.polar_sin, p.polar_weight, t.seg_offset, t.seg_region,
+                                                        t.seg_length, t.track_weight, t.link, t.volume, cell, n_cells,
+                                                        coupling_of, n_iters)
+        lo, hi = cmfd.coarse_surfaces(t.seg_offset, t.seg_region, cell, t.link)   # geometry of the overlay, not arithmetic
+        coupling = coupling_of(lo, hi)
+        g = pair.gpu
+        g.nd_state_reset()
+        k, hist_g = 1.0, []
+        for _ in range(n_iters):
+            Qp, F = g.nd_source_update(g.nd_flux_get(), k, want_fission_rate=True)
+            F = float(F.item())
+            Js, Jv, _ = g.nd_sweep_currents(Qp, cell, n_cells, lo, hi)
+            k_sweep = g.nd_power_iteration(1)["k_eff"]
+            co = g.nd_cmfd_collapse(cell, n_cells)
+            k, Phi_new, _ = nd.nd_cmfd_coarse_solve(co, lo, hi, coupling, Js / F, Jv / F, k_sweep)
+            g.nd_cmfd_prolong(cell, n_cells, Phi_new / co["Phi"], k)
+            hist_g.append(k)
+        print(f"cfg{idx} all-GPU k history {hist_g}")
+        assert np.abs(np.array(hist_g) - hist_o).max() <= 0.1e-5
+        phi_g = g.nd_flux_get().cpu().numpy()
+        assert phi_rel_err(phi_g / phi_g.sum(), phi_o / phi_o.sum()) <= PHI_RTOL
     finally:
         pair.close()
