@@ -312,6 +312,21 @@ nd_status nd_cmfd_coarse_solve(int32_t n_cells, int32_t n_groups, const double* 
                                const double* J_vac, double k0, double tol, int32_t max_outer, double* k_out,
                                double* Phi_new, int32_t* iters_done, void* cuda_stream);
 
+/* NEXT-3: one CMFD-accelerated power iteration, Algorithm 1 ("Perform MOC on the fine mesh", "Solve
+ * CMFD on the coarse mesh", update of the fine-mesh flux), steps C-1..C-9 of DESIGN.md 8d after the sweep of O-8:
+ * source -> nd_sweep_currents -> nd_power_iteration(1) -> nd_cmfd_collapse -> nd_cmfd_coarse_solve (tol 1e-13) ->
+ * nd_cmfd_prolong, on the problem's own state.  A host composition of those entry points this round: the coarse arrays
+ * pass through host memory between the steps and every step synchronises.
+ *   cell HOST [R]; pair_lo/pair_hi/coupling HOST [n_pairs] as in nd_sweep_currents / nd_cmfd_coarse_solve
+ *   k_sweep_out (may be NULL): k after the sweep, before the coarse solve; k_eff_out: the coarse eigenvalue = the state's k
+ *   coarse_iters (may be NULL): outer iterations of the coarse solve
+ * Needs sweep_kernel = ND_SWEEP_ATOMIC (nd_sweep_currents).  Errors: those of the steps; ND_ERR_STATE if the state has
+ * k <= 0 or a zero fission rate.  The undamped scheme diverges for coarse cells of several mean free paths;
+ * a coarse eigenvalue <= 0 is reported as ND_ERR_INVALID by the prolongation and the state is then one plain iteration on. */
+nd_status nd_cmfd_iteration(nd_problem* p, int32_t n_cells, const int32_t* cell, int32_t n_pairs, const int32_t* pair_lo,
+                            const int32_t* pair_hi, const double* coupling, double* k_sweep_out, double* k_eff_out,
+                            int32_t* coarse_iters, void* cuda_stream);
+
 /* Device-time accounting.  When enabled, every sweep-kernel launch is bracketed by CUDA events on its own
  * stream; nd_profile_read synchronises and returns the accumulated kernel milliseconds and launch counts
  * since the last nd_profile_enable(p,1).  kernels_launched counts every kernel the library launched. */

@@ -25,7 +25,7 @@ EXPORTS = [
     "nd_tracks_generate", "nd_tracks_device_workspace_bytes", "nd_tracks_generate_device", "nd_tracks_view", "nd_tracks_destroy", "nd_workspace_bytes", "nd_problem_create",
     "nd_problem_destroy", "nd_transport_sweep", "nd_source_update", "nd_power_iteration", "nd_state_reset",
     "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_outgoing_flux_get", "nd_flux_get", "nd_flux_set",
-    "nd_track_volume_get", "nd_tally_get", "nd_sweep_currents", "nd_cmfd_collapse", "nd_cmfd_prolong", "nd_cmfd_coarse_solve", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
+    "nd_track_volume_get", "nd_tally_get", "nd_sweep_currents", "nd_cmfd_collapse", "nd_cmfd_prolong", "nd_cmfd_coarse_solve", "nd_cmfd_iteration", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
     "nd_swath_stream_build", "nd_swath_stream_view", "nd_swath_stream_destroy",
     "nd_status_string", "nd_last_error", "nd_version",
 ]
@@ -141,6 +141,8 @@ def lib():
         L.nd_cmfd_coarse_solve.argtypes = ([C.c_int32, C.c_int32] + [C.c_void_p] * 6 + [C.c_int32] + [C.c_void_p] * 5 +
                                            [C.c_double, C.c_double, C.c_int32, C.POINTER(C.c_double), C.c_void_p,
                                             C.POINTER(C.c_int32), C.c_void_p])
+        L.nd_cmfd_iteration.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
+                                        C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int32), C.c_void_p]
         L.nd_profile_enable.argtypes = [C.c_void_p, C.c_int32]
         L.nd_profile_read.argtypes = [C.c_void_p, C.POINTER(nd_profile)]
         L.nd_sweep_phases_get.argtypes = [C.c_void_p, C.c_void_p]
@@ -419,6 +421,18 @@ class Problem:
                                       out["sigs"].ctypes.data, out["nusf"].ctypes.data, out["chi"].ctypes.data,
                                       self._stream()), "nd_cmfd_collapse")
         return out
+
+    def nd_cmfd_iteration(self, cell, n_cells, pair_lo, pair_hi, coupling):
+        """Algorithm 1 as one call (nd.h).  Returns dict k_eff, k_sweep, coarse_iters."""
+        cell = np.ascontiguousarray(cell, np.int32)
+        lo, hi = np.ascontiguousarray(pair_lo, np.int32), np.ascontiguousarray(pair_hi, np.int32)
+        cpl = np.ascontiguousarray(coupling, np.float64)
+        assert cell.shape == (self.R,) and lo.shape == hi.shape == cpl.shape and lo.ndim == 1
+        ks, k, it = C.c_double(), C.c_double(), C.c_int32()
+        _check(lib().nd_cmfd_iteration(self._h, int(n_cells), cell.ctypes.data, len(lo), lo.ctypes.data, hi.ctypes.data,
+                                       cpl.ctypes.data, C.byref(ks), C.byref(k), C.byref(it), self._stream()),
+               "nd_cmfd_iteration")
+        return dict(k_eff=k.value, k_sweep=ks.value, coarse_iters=it.value)
 
     def nd_cmfd_prolong(self, cell, n_cells, ratio, k_eff):
         cell = np.ascontiguousarray(cell, np.int32)

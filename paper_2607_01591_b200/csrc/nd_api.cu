@@ -1400,6 +1400,58 @@ extern "C" nd_status nd_cmfd_coarse_solve(int32_t n_cells, int32_t n_groups, con
     return ND_OK;
 }
 
+// NEXT-3, Algorithm 1 as one call: see nd.h.  A host composition of the entry points above.
+extern "C" nd_status nd_cmfd_iteration(nd_problem* p, int32_t n_cells, const int32_t* cell, int32_t n_pairs,
+                                       const int32_t* pair_lo, const int32_t* pair_hi, const double* coupling,
+                                       double* k_sweep_out, double* k_eff_out, int32_t* coarse_iters, void* cuda_stream)
+{
+    if (!p || !cell || !k_eff_out || (n_pairs > 0 && (!pair_lo || !pair_hi || !coupling)))
+        return nd_fail(ND_ERR_NULL, "nd_cmfd_iteration: NULL argument");
+    if (n_cells < 1 || n_pairs < 0) return nd_fail(ND_ERR_INVALID, "nd_cmfd_iteration: n_cells must be >= 1 and n_pairs >= 0");
+    const Dims& d = p->d;
+    cudaStream_t st = as_stream(cuda_stream);
+    const size_t CG = (size_t)n_cells * d.G, SG = (size_t)n_pairs * d.G;
+    std::vector<double> Js, Jv, Jr, V, Phi, sgt, sgs, nsf, chi, Phi_new;
+    try {
+        Js.resize(SG + 1); Jv.resize(CG); Jr.resize(CG); V.resize((size_t)n_cells); Phi.resize(CG); sgt.resize(CG);
+        sgs.resize(CG * d.G); nsf.resize(CG); chi.resize(CG); Phi_new.resize(CG);
+    } catch (const std::bad_alloc&) {
+        return nd_fail(ND_ERR_NOMEM, "nd_cmfd_iteration: out of host memory");
+    }
+    // state scalars: k and the fission rate F of the current flux (the sweep uses phi / F and psi / F)
+    double ks[2];
+    ND_CUDA(cudaMemcpyAsync(ks, p->scalars, sizeof ks, cudaMemcpyDeviceToHost, st));
+    ND_CUDA(cudaStreamSynchronize(st));
+    const double k = ks[ndk::SC_K], F = ks[ndk::SC_F];
+    if (!(k > 0.0) || !(F > 0.0)) return nd_fail(ND_ERR_STATE, "nd_cmfd_iteration: the state has k <= 0 or no fission rate");
+    DeviceScratch ds;
+    ND_CUDA(cudaMalloc(&ds.b, sizeof(double) * (size_t)d.R * d.G));
+    double* dQ = (double*)ds.b;
+    // C-3 with the un-normalised source: the currents are linear in (Q, psi), so they come out F times too large
+    nd_status rc = nd_source_update(p, p->phi_cur, k, dQ, nullptr, cuda_stream);
+    if (rc != ND_OK) return rc;
+    rc = nd_sweep_currents(p, dQ, n_cells, cell, n_pairs, pair_lo, pair_hi, Js.data(), Jv.data(), Jr.data(), cuda_stream);
+    if (rc != ND_OK) return rc;
+    for (double& v : Js) v /= F;
+    for (double& v : Jv) v /= F;
+    double k_sweep = 0.0;
+    rc = nd_power_iteration(p, 1, 0.0, 0.0, &k_sweep, nullptr, nullptr, nullptr, cuda_stream);   // source, sweep, flux, k
+    if (rc != ND_OK) return rc;
+    if (k_sweep_out) *k_sweep_out = k_sweep;
+    rc = nd_cmfd_collapse(p, nullptr, n_cells, cell, V.data(), Phi.data(), sgt.data(), sgs.data(), nsf.data(), chi.data(), cuda_stream);
+    if (rc != ND_OK) return rc;
+    double k_new = 0.0;
+    rc = nd_cmfd_coarse_solve(n_cells, d.G, V.data(), Phi.data(), sgt.data(), sgs.data(), nsf.data(), chi.data(), n_pairs,
+                              pair_lo, pair_hi, coupling, Js.data(), Jv.data(), k_sweep, 1e-13, 100000, &k_new, Phi_new.data(),
+                              coarse_iters, cuda_stream);
+    if (rc != ND_OK) return rc;
+    for (size_t i = 0; i < CG; ++i) Phi_new[i] /= Phi[i];                                        // C-9 ratio
+    rc = nd_cmfd_prolong(p, n_cells, cell, Phi_new.data(), k_new, cuda_stream);
+    if (rc != ND_OK) return rc;
+    *k_eff_out = k_new;
+    return ND_OK;
+}
+
 extern "C" nd_status nd_profile_enable(nd_problem* p, int32_t on)
 {
     if (!p) return nd_fail(ND_ERR_NULL, "nd_profile_enable: NULL problem");

@@ -351,3 +351,39 @@ def test_cmfd_iteration_all_steps_on_the_gpu(case):
         assert phi_rel_err(phi_g / phi_g.sum(), phi_o / phi_o.sum()) <= PHI_RTOL
     finally:
         pair.close()
+
+
+@pytest.mark.parametrize("case", [(1, 1.0, 3, 2), (2, 0.15, 8, 8), (3, 0.03, 6, 6)], ids=["cfg1", "cfg2", "cfg3"])
+def test_cmfd_iteration_entry_point(case):
+    """nd_cmfd_iteration (Algorithm 1 as one call) against oracle.cmfd.power_iteration_cmfd, and against the plain
+    iteration: same fixed point, fewer sweeps."""
+    idx, scale, nx, ny = case
+    n_iters, n_cells = 8, nx * ny
+    pair = make_pair(idx, scale, sweep_kernel=nd.ND_SWEEP_ATOMIC)
+    try:
+        p, t = pair.prob, pair.o_tr
+        cell = cartesian_cells(p.mesh, nx, ny)
+        coupling_of = cartesian_coupling(p.mesh, nx, ny)
+        _, phi_o, _, hist_o = cmfd.power_iteration_cmfd(p.mesh.material, p.xs.sigma_t, p.xs.sigma_s, p.xs.nu_sigma_f,
+                                                        p.xs.chi, p.polar_sin, p.polar_weight, t.seg_offset, t.seg_region,
+                                                        t.seg_length, t.track_weight, t.link, t.volume, cell, n_cells,
+                                                        coupling_of, n_iters)
+        assert np.isfinite(hist_o).all() and (hist_o > 0).all()
+        lo, hi = cmfd.coarse_surfaces(t.seg_offset, t.seg_region, cell, t.link)
+        coupling = coupling_of(lo, hi)
+        pair.gpu.nd_state_reset()
+        hist_g = [pair.gpu.nd_cmfd_iteration(cell, n_cells, lo, hi, coupling) for _ in range(n_iters)]
+        k_g = np.array([h["k_eff"] for h in hist_g])
+        print(f"cfg{idx} nd_cmfd_iteration: k {k_g.tolist()} coarse iterations {[h['coarse_iters'] for h in hist_g]}")
+        assert np.abs(k_g - hist_o).max() <= 0.1e-5
+        phi_g = pair.gpu.nd_flux_get().cpu().numpy()
+        assert phi_rel_err(phi_g / phi_g.sum(), phi_o / phi_o.sum()) <= PHI_RTOL
+        assert pair.gpu.nd_power_iteration(0)["k_eff"] == k_g[-1]
+    finally:
+        pair.close()
+    swath = make_pair(1, 1.0, sweep_kernel=nd.ND_SWEEP_SWATH)
+    try:
+        with pytest.raises(nd.NdError, match="ND_SWEEP_ATOMIC"):
+            swath.gpu.nd_cmfd_iteration(np.zeros(swath.R, np.int32), 1, [], [], [])
+    finally:
+        swath.close()
