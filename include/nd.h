@@ -99,7 +99,10 @@ typedef struct {
     int32_t graph_mode;     /* nd_power_iteration with a fixed iteration count (no tolerances, no per-iteration stats, profiling
                                off) replays a CUDA graph of two iterations instead of launching their kernels one by one:
                                0 = default (on for calls of >= 4 iterations), 1 = never */
-    int32_t reserved[4];    /* must be 0 */
+    int32_t cmfd_stream;    /* 1: keep the plain SoA segment stream on the device beside the tiled kernel's chunk stream (8 bytes
+                               per segment more workspace) so that nd_sweep_currents / nd_cmfd_iteration work with the fast
+                               sweep kernels; 0 = default (only ND_SWEEP_ATOMIC problems carry it) */
+    int32_t reserved[3];    /* must be 0 */
 } nd_options;
 
 /* ------------------------------------------------------------------------------------------------
@@ -258,7 +261,8 @@ nd_status nd_tally_get(nd_problem* p, double* d_tally_out, void* cuda_stream);  
  * Reads the problem's current boundary psi and leaves ALL state unchanged (the boundary flux is not advanced, the tally
  * of the last sweep is kept): nd_transport_sweep with the same d_Q afterwards performs the sweep these currents belong
  * to.  FP32 segment arithmetic, FP64 atomics.  This round: the simple one-warp-per-chain kernel over the SoA stream,
- * so the problem must have been created with sweep_kernel = ND_SWEEP_ATOMIC (else ND_ERR_STATE); scratch is allocated
+ * so the problem must have been created with sweep_kernel = ND_SWEEP_ATOMIC or nd_options.cmfd_stream = 1 (else
+ * ND_ERR_STATE); scratch is allocated
  * and freed inside the call and the stream is synchronised before it returns.
  * Errors: ND_ERR_NULL, ND_ERR_INVALID (sizes; a surface listed twice; a crossing between cells that are not a listed
  * surface -- outputs are then unspecified), ND_ERR_RANGE (cell or pair out of range), ND_ERR_STATE, ND_ERR_CUDA. */
@@ -320,7 +324,8 @@ nd_status nd_cmfd_coarse_solve(int32_t n_cells, int32_t n_groups, const double* 
  *   cell HOST [R]; pair_lo/pair_hi/coupling HOST [n_pairs] as in nd_sweep_currents / nd_cmfd_coarse_solve
  *   k_sweep_out (may be NULL): k after the sweep, before the coarse solve; k_eff_out: the coarse eigenvalue = the state's k
  *   coarse_iters (may be NULL): outer iterations of the coarse solve
- * Needs sweep_kernel = ND_SWEEP_ATOMIC (nd_sweep_currents).  Errors: those of the steps; ND_ERR_STATE if the state has
+ * Needs sweep_kernel = ND_SWEEP_ATOMIC or nd_options.cmfd_stream = 1 (nd_sweep_currents; the sweep of the iteration itself
+ * runs with the problem's sweep kernel).  Errors: those of the steps; ND_ERR_STATE if the state has
  * k <= 0 or a zero fission rate.  The undamped scheme diverges for coarse cells of several mean free paths;
  * a coarse eigenvalue <= 0 is reported as ND_ERR_INVALID by the prolongation and the state is then one plain iteration on. */
 nd_status nd_cmfd_iteration(nd_problem* p, int32_t n_cells, const int32_t* cell, int32_t n_pairs, const int32_t* pair_lo,

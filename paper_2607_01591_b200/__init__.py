@@ -40,7 +40,7 @@ class NdError(RuntimeError):
 class nd_options(C.Structure):
     _fields_ = [("exp_mode", C.c_int32), ("sweep_kernel", C.c_int32), ("track_batch", C.c_int32),
                 ("window_regions", C.c_int32), ("block_warps", C.c_int32), ("tile_segments", C.c_int32),
-                ("delta_buffers", C.c_int32), ("blocks_per_sm", C.c_int32), ("tile_lag", C.c_int32), ("service_warps", C.c_int32), ("q_copies", C.c_int32), ("graph_mode", C.c_int32), ("reserved", C.c_int32 * 4)]
+                ("delta_buffers", C.c_int32), ("blocks_per_sm", C.c_int32), ("tile_lag", C.c_int32), ("service_warps", C.c_int32), ("q_copies", C.c_int32), ("graph_mode", C.c_int32), ("cmfd_stream", C.c_int32), ("reserved", C.c_int32 * 3)]
 
 
 class nd_mesh_desc(C.Structure):
@@ -273,7 +273,7 @@ class Problem:
     def __init__(self, region_material, sigma_t, sigma_s, nu_sigma_f, chi, polar_sin, polar_weight, seg_offset,
                  seg_region, seg_length, track_weight, link, track_azim=None, track_ends=None, exp_mode=ND_EXP_FAST,
                  sweep_kernel=ND_SWEEP_AUTO, track_batch=0, window_regions=0, block_warps=0, tile_segments=0,
-                 delta_buffers=0, blocks_per_sm=0, tile_lag=0, service_warps=0, q_copies=0, graph_mode=0, device="cuda:0"):
+                 delta_buffers=0, blocks_per_sm=0, tile_lag=0, service_warps=0, q_copies=0, graph_mode=0, cmfd_stream=0, device="cuda:0"):
         import torch
         self.torch = torch
         self.device = torch.device(device)
@@ -293,7 +293,7 @@ class Problem:
         d = nd_problem_desc(self.R, self.M, self.G, self.P, self.T, *[keep[k].ctypes.data for k in
                             ("rm", "st", "ss", "nf", "ch", "ps", "pw", "so", "sr", "sl", "tw", "lk")], *geo)
         opt = nd_options(int(exp_mode), int(sweep_kernel), int(track_batch), int(window_regions), int(block_warps),
-                         int(tile_segments), int(delta_buffers), int(blocks_per_sm), int(tile_lag), int(service_warps), int(q_copies), int(graph_mode))
+                         int(tile_segments), int(delta_buffers), int(blocks_per_sm), int(tile_lag), int(service_warps), int(q_copies), int(graph_mode), int(cmfd_stream))
         nbytes = C.c_size_t()
         _check(lib().nd_workspace_bytes(C.byref(d), C.byref(opt), C.byref(nbytes)), "nd_workspace_bytes")
         self.workspace_bytes = int(nbytes.value)

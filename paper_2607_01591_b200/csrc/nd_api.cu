@@ -247,7 +247,7 @@ inline size_t bump(size_t& cur, size_t bytes)
     return at;
 }
 
-Layout make_layout(const Dims& d, int max_stats, const PrivConfig& pc_in, const SwathConfig& sc, int kernel)
+Layout make_layout(const Dims& d, int max_stats, const PrivConfig& pc_in, const SwathConfig& sc, int kernel, bool keep_soa)
 {
     // the tiled kernels share the stream fields of the layout; size them for the selected one
     PrivConfig pc = pc_in;
@@ -258,8 +258,9 @@ Layout make_layout(const Dims& d, int max_stats, const PrivConfig& pc_in, const 
     Layout L{};
     size_t c = 0;
     const size_t RG = (size_t)d.R * d.G, RGs = (size_t)d.R * d.Gs, NPSI = (size_t)d.T * 2 * d.P * d.Gs;
-    // the v0 SoA stream is read by the atomic kernel only; the tiled kernels carry their own chunk stream
-    const size_t soa = kernel == ND_SWEEP_ATOMIC ? (size_t)d.Spad : 4;
+    // the v0 SoA stream is read by the atomic kernel (and the CMFD current tally: nd_options.cmfd_stream); the tiled kernels
+    // carry their own chunk stream
+    const size_t soa = kernel == ND_SWEEP_ATOMIC || keep_soa ? (size_t)d.Spad : 4;
     L.seg_rm = bump(c, sizeof(uint32_t) * soa);
     L.seg_len = bump(c, sizeof(float) * soa);
     L.trk_off = bump(c, sizeof(int64_t) * ((size_t)d.T + 1));
@@ -333,6 +334,7 @@ struct nd_problem {
     Layout L{};
     char* ws = nullptr;
     int sweep_kernel = ND_SWEEP_ATOMIC;
+    bool has_soa = false;                  // the plain SoA segment stream is on the device (atomic kernel, CMFD currents)
     int n_sm = 148;
     // device pointers into the workspace
     uint32_t* seg_rm; float* seg_len; int64_t* trk_off; float* trk_w; int32_t* link_src;
@@ -627,7 +629,7 @@ extern "C" nd_status nd_workspace_bytes(const nd_problem_desc* desc, const nd_op
     SwathConfig sc;
     if (opt.sweep_kernel == ND_SWEEP_PRIVATE) pc = make_priv_config(d, opt);
     if (is_swath(opt.sweep_kernel) || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt, opt.sweep_kernel == ND_SWEEP_SWATH_WS);
-    *device_bytes = make_layout(d, kMaxStats, pc, sc, select_kernel(desc, opt, pc, sc)).total;
+    *device_bytes = make_layout(d, kMaxStats, pc, sc, select_kernel(desc, opt, pc, sc), opt.cmfd_stream != 0).total;
     return ND_OK;
 }
 
@@ -644,8 +646,9 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     if (rc != ND_OK) return rc;
     nd_options opt{};
     if (opts) opt = *opts;
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < 3; ++i)
         if (opt.reserved[i] != 0) return nd_fail(ND_ERR_INVALID, "nd_options.reserved must be zero");
+    if (opt.cmfd_stream < 0 || opt.cmfd_stream > 1) return nd_fail(ND_ERR_INVALID, "nd_options.cmfd_stream must be 0 or 1");
     if (opt.exp_mode != ND_EXP_FAST && opt.exp_mode != ND_EXP_EXPM1) return nd_fail(ND_ERR_INVALID, "unknown exp_mode");
     if (opt.sweep_kernel < ND_SWEEP_AUTO || opt.sweep_kernel > ND_SWEEP_SWATH_WS) return nd_fail(ND_ERR_INVALID, "unknown sweep_kernel");
     if (opt.track_batch < 0 || opt.window_regions < 0 || opt.block_warps < 0 || opt.tile_segments < 0 || opt.delta_buffers < 0 ||
@@ -658,7 +661,7 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     if (opt.sweep_kernel == ND_SWEEP_PRIVATE) pc = make_priv_config(d, opt);
     if (is_swath(opt.sweep_kernel) || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt, opt.sweep_kernel == ND_SWEEP_SWATH_WS);
     const int kernel = select_kernel(desc, opt, pc, sc);
-    const Layout L = make_layout(d, kMaxStats, pc, sc, kernel);
+    const Layout L = make_layout(d, kMaxStats, pc, sc, kernel, opt.cmfd_stream != 0);
     if (reinterpret_cast<uintptr_t>(device_workspace) % kAlign != 0) return nd_fail(ND_ERR_WORKSPACE, "workspace must be 256-byte aligned");
     if (device_bytes < L.total) return nd_fail(ND_ERR_WORKSPACE, "workspace smaller than nd_workspace_bytes");
 
@@ -702,7 +705,8 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         p = new nd_problem();
         p->d = d; p->opt = opt; p->L = L; p->ws = static_cast<char*>(device_workspace);
         // ---- A1: pack the segment stream (SoA, every track run padded to a multiple of 4 = 16 bytes) ----
-        const bool soa = kernel == ND_SWEEP_ATOMIC;
+        const bool soa = kernel == ND_SWEEP_ATOMIC || opt.cmfd_stream != 0;
+        p->has_soa = soa;
         h_rm.assign(soa ? (size_t)d.Spad : 4, 0u);
         h_len.assign(soa ? (size_t)d.Spad : 4, 0.f);
         h_off.resize((size_t)d.T + 1);
@@ -1136,9 +1140,9 @@ extern "C" nd_status nd_sweep_currents(nd_problem* p, const double* d_Q, int32_t
     if (!p || !d_Q || !cell || !J_vac || !J_ref || (n_pairs > 0 && (!pair_lo || !pair_hi || !J_surf)))
         return nd_fail(ND_ERR_NULL, "nd_sweep_currents: NULL argument");
     if (n_cells < 1 || n_pairs < 0) return nd_fail(ND_ERR_INVALID, "nd_sweep_currents: n_cells must be >= 1 and n_pairs >= 0");
-    if (p->sweep_kernel != ND_SWEEP_ATOMIC)
-        return nd_fail(ND_ERR_STATE, "nd_sweep_currents: needs a problem created with sweep_kernel = ND_SWEEP_ATOMIC "
-                                     "(the current tally reads the SoA segment stream)");
+    if (!p->has_soa)
+        return nd_fail(ND_ERR_STATE, "nd_sweep_currents: needs a problem created with sweep_kernel = ND_SWEEP_ATOMIC or "
+                                     "nd_options.cmfd_stream = 1 (the current tally reads the SoA segment stream)");
     const Dims& d = p->d;
     cudaStream_t st = as_stream(cuda_stream);
     for (int64_t r = 0; r < d.R; ++r)

@@ -387,3 +387,49 @@ def test_cmfd_iteration_entry_point(case):
             swath.gpu.nd_cmfd_iteration(np.zeros(swath.R, np.int32), 1, [], [], [])
     finally:
         swath.close()
+
+
+def test_cmfd_with_the_swath_sweep_kernel():
+    """nd_options.cmfd_stream = 1 keeps the SoA stream beside the chunk stream: the currents are those of the
+    atomic-kernel problem up to the order of the FP64 atomics (1e-12), and nd_cmfd_iteration runs its sweep with the swath
+    kernel and still follows the oracle."""
+    idx, scale, nx, ny, n_iters = 2, 0.15, 8, 8, 8
+    n_cells = nx * ny
+    a = make_pair(idx, scale, sweep_kernel=nd.ND_SWEEP_ATOMIC)
+    b = make_pair(idx, scale, sweep_kernel=nd.ND_SWEEP_SWATH, cmfd_stream=1)
+    try:
+        assert b.gpu.nd_problem_info_get()["sweep_kernel"] == nd.ND_SWEEP_SWATH
+        assert b.gpu.workspace_bytes > make_pair_bytes(idx, scale)
+        p, t = a.prob, a.o_tr
+        cell = cartesian_cells(p.mesh, nx, ny)
+        lo, hi = cmfd.coarse_surfaces(t.seg_offset, t.seg_region, cell, t.link)
+        Q, psi = seeded_sweep_inputs(a, seed=77)
+        dQ = torch.from_numpy(Q).cuda()
+        a.gpu.nd_boundary_flux_set(psi)
+        b.gpu.nd_boundary_flux_set(psi)
+        for x, y in zip(a.gpu.nd_sweep_currents(dQ, cell, n_cells, lo, hi), b.gpu.nd_sweep_currents(dQ, cell, n_cells, lo, hi)):
+            assert np.abs(x - y).max() <= 1e-12 * max(np.abs(x).max(), 1e-300)
+        coupling_of = cartesian_coupling(p.mesh, nx, ny)
+        _, phi_o, _, hist_o = cmfd.power_iteration_cmfd(p.mesh.material, p.xs.sigma_t, p.xs.sigma_s, p.xs.nu_sigma_f,
+                                                        p.xs.chi, p.polar_sin, p.polar_weight, t.seg_offset, t.seg_region,
+                                                        t.seg_length, t.track_weight, t.link, t.volume, cell, n_cells,
+                                                        coupling_of, n_iters)
+        b.gpu.nd_state_reset()
+        coupling = coupling_of(lo, hi)
+        k_g = np.array([b.gpu.nd_cmfd_iteration(cell, n_cells, lo, hi, coupling)["k_eff"] for _ in range(n_iters)])
+        print(f"swath + cmfd_stream: max |dk| {np.abs(k_g - hist_o).max():.2e}")
+        assert np.abs(k_g - hist_o).max() <= 0.1e-5
+        phi_g = b.gpu.nd_flux_get().cpu().numpy()
+        assert phi_rel_err(phi_g / phi_g.sum(), phi_o / phi_o.sum()) <= PHI_RTOL
+    finally:
+        a.close()
+        b.close()
+
+
+def make_pair_bytes(idx, scale):
+    """Workspace of the same problem with the swath kernel and no SoA stream."""
+    c = make_pair(idx, scale, sweep_kernel=nd.ND_SWEEP_SWATH)
+    try:
+        return c.gpu.workspace_bytes
+    finally:
+        c.close()
