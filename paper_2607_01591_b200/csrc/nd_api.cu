@@ -1191,6 +1191,8 @@ extern "C" nd_status nd_sweep_currents(nd_problem* p, const double* d_Q, int32_t
     cp.pair_key = (int64_t*)(buf + oKey); cp.pair_idx = (int32_t*)(buf + oIdx);
     cp.J_surf = dJ; cp.J_vac = dJ + nJs; cp.J_ref = dJ + nJs + nJc; cp.missing = d_flag;
     cp.n_pairs = n_pairs; cp.n_cells = n_cells;
+    cp.lanes_per_chain = 32;
+    while (cp.lanes_per_chain / 2 >= d.G) cp.lanes_per_chain /= 2;
     ND_CUDA(cudaMemsetAsync(dJ, 0, sizeof(double) * (nJs + 2 * nJc), st));
     ND_CUDA(cudaMemsetAsync(d_flag, 0, sizeof(int), st));
     ND_CUDA(cudaMemsetAsync(buf + oFwd, 0xff, sizeof(int32_t) * nE, st));
@@ -1205,7 +1207,7 @@ extern "C" nd_status nd_sweep_currents(nd_problem* p, const double* d_Q, int32_t
     ND_LAUNCH_CHECK(p);
     ndk::k_entry_cell<<<grid_for((int64_t)nE, 256, 8 * p->n_sm), 256, 0, st>>>(p->seg_rm, p->trk_off, cp.cell, (int32_t*)(buf + oEnt), (int64_t)nE);
     ND_LAUNCH_CHECK(p);
-    const int grid = grid_for((int64_t)nE * 32, 256, 16 * p->n_sm);
+    const int grid = grid_for((int64_t)nE * cp.lanes_per_chain, 256, 16 * p->n_sm);
     switch (d.P) {
     case 1: launch_currents_p<1>(p, cp, grid, st); break;
     case 2: launch_currents_p<2>(p, cp, grid, st); break;

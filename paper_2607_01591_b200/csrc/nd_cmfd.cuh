@@ -59,6 +59,7 @@ struct CurrentParams {
     double* __restrict__ J_ref;            // [n_cells][G]
     int* __restrict__ missing;             // set when a crossing joins a pair that is not listed
     int n_pairs, n_cells;
+    int lanes_per_chain;                   // power of two, min(32, >= G)
 };
 
 __device__ __forceinline__ int find_surface(const CurrentParams& cp, int a, int b)
@@ -75,25 +76,27 @@ __device__ __forceinline__ int find_surface(const CurrentParams& cp, int a, int 
     return -1;
 }
 
-// One warp per (track, direction), lanes over groups (the layout of k_sweep_atomic).  The cell of a segment and the
-// surface search are warp-uniform.
+// One chain (track, direction) per group of lanes_per_chain lanes, lanes over groups (the layout of k_sweep_atomic, with
+// 32 / lanes_per_chain chains to a warp when G <= 16).  The cell of a segment and the surface search are uniform within
+// a chain's lanes; the kernel uses no warp-wide primitive, so chains of different lengths may share a warp.
 template <int P, int EXPM>
 __global__ void __launch_bounds__(256) k_sweep_currents(const CurrentParams cp)
 {
     const SweepParams& prm = cp.sw;
-    const int lane = threadIdx.x & 31;
-    const int warps_per_block = blockDim.x >> 5;
+    const int lpc = cp.lanes_per_chain;              // 32 / lpc chains share a warp when G <= 16
+    const int lane = threadIdx.x % lpc;
+    const int chains_per_block = blockDim.x / lpc;
     const int64_t n_chains = 2 * (int64_t)prm.T;
     const float inv_f = (float)(1.0 / *prm.scale_div);
-    for (int64_t chain = (int64_t)blockIdx.x * warps_per_block + (threadIdx.x >> 5); chain < n_chains;
-         chain += (int64_t)gridDim.x * warps_per_block) {
+    for (int64_t chain = (int64_t)blockIdx.x * chains_per_block + threadIdx.x / lpc; chain < n_chains;
+         chain += (int64_t)gridDim.x * chains_per_block) {
         const int t = (int)(chain >> 1), dir = (int)(chain & 1);
         const int64_t k0 = prm.trk_off[t], k1 = prm.trk_off[t + 1];
         if (k1 == k0) continue;
         const float wt = prm.trk_w[t];
         const int32_t lk = cp.link_fwd[chain];
         const int32_t c2 = lk >= 0 ? cp.entry_cell[lk] : -1;
-        for (int g = lane; g < prm.G; g += 32) {
+        for (int g = lane; g < prm.G; g += lpc) {
             float psi[P];
 #pragma unroll
             for (int p = 0; p < P; ++p) psi[p] = prm.psi_in[(chain * P + p) * prm.Gs + g] * inv_f;
