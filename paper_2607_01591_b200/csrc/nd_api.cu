@@ -1123,10 +1123,14 @@ namespace {
 template <int P>
 void launch_currents_p(const nd_problem* p, const ndk::CurrentParams& cp, int grid, cudaStream_t st)
 {
-    if (p->opt.exp_mode == ND_EXP_EXPM1)
-        ndk::k_sweep_currents<P, 1><<<grid, 256, 0, st>>>(cp);
-    else
-        ndk::k_sweep_currents<P, 0><<<grid, 256, 0, st>>>(cp);
+    const bool two = p->d.G > 32;   // a lane carries two groups through one walk
+    if (p->opt.exp_mode == ND_EXP_EXPM1) {
+        if (two) ndk::k_sweep_currents<P, 1, 2><<<grid, 256, 0, st>>>(cp);
+        else ndk::k_sweep_currents<P, 1, 1><<<grid, 256, 0, st>>>(cp);
+    } else {
+        if (two) ndk::k_sweep_currents<P, 0, 2><<<grid, 256, 0, st>>>(cp);
+        else ndk::k_sweep_currents<P, 0, 1><<<grid, 256, 0, st>>>(cp);
+    }
 }
 
 } // namespace

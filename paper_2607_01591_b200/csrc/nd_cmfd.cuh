@@ -79,7 +79,8 @@ __device__ __forceinline__ int find_surface(const CurrentParams& cp, int a, int 
 // One chain (track, direction) per group of lanes_per_chain lanes, lanes over groups (the layout of k_sweep_atomic, with
 // 32 / lanes_per_chain chains to a warp when G <= 16).  The cell of a segment and the surface search are uniform within
 // a chain's lanes; the kernel uses no warp-wide primitive, so chains of different lengths may share a warp.
-template <int P, int EXPM>
+// NG = groups a lane carries through one walk (2 when G > 32: the walk of a chain is then done once for 64 groups).
+template <int P, int EXPM, int NG>
 __global__ void __launch_bounds__(256) k_sweep_currents(const CurrentParams cp)
 {
     const SweepParams& prm = cp.sw;
@@ -96,10 +97,17 @@ __global__ void __launch_bounds__(256) k_sweep_currents(const CurrentParams cp)
         const float wt = prm.trk_w[t];
         const int32_t lk = cp.link_fwd[chain];
         const int32_t c2 = lk >= 0 ? cp.entry_cell[lk] : -1;
-        for (int g = lane; g < prm.G; g += lpc) {
-            float psi[P];
+        for (int g0 = lane; g0 < prm.G; g0 += lpc * NG) {
+            float psi[NG][P];
+            int g[NG];
+            bool act[NG];
 #pragma unroll
-            for (int p = 0; p < P; ++p) psi[p] = prm.psi_in[(chain * P + p) * prm.Gs + g] * inv_f;
+            for (int j = 0; j < NG; ++j) {
+                act[j] = g0 + j * lpc < prm.G;
+                g[j] = act[j] ? g0 + j * lpc : g0;   // an idle slot repeats group g0 and adds nothing
+#pragma unroll
+                for (int p = 0; p < P; ++p) psi[j][p] = prm.psi_in[(chain * P + p) * prm.Gs + g[j]] * inv_f;
+            }
             int c_prev = -1;
             for (int64_t i = 0; i < k1 - k0; ++i) {
                 const int64_t k = dir == 0 ? k0 + i : k1 - 1 - i;
@@ -112,37 +120,44 @@ __global__ void __launch_bounds__(256) k_sweep_currents(const CurrentParams cp)
                     if (sidx < 0) {
                         *cp.missing = 1;
                     } else {
-                        float cur = 0.f;
 #pragma unroll
-                        for (int p = 0; p < P; ++p) cur = fmaf(prm.wp[p], psi[p], cur);
-                        const double j = (double)wt * (double)cur;
-                        atomicAdd(&cp.J_surf[(size_t)sidx * prm.G + g], c_prev < c ? j : -j);
+                        for (int j = 0; j < NG; ++j) {
+                            float cur = 0.f;
+#pragma unroll
+                            for (int p = 0; p < P; ++p) cur = fmaf(prm.wp[p], psi[j][p], cur);
+                            const double jj = (double)wt * (double)cur;
+                            if (act[j]) atomicAdd(&cp.J_surf[(size_t)sidx * prm.G + g[j]], c_prev < c ? jj : -jj);
+                        }
                     }
                 }
-                const float st = prm.sigt[rm_material(rm) * prm.Gs + g];
-                const float qv = prm.q[(size_t)r * prm.Gs + g];
-                attenuate<P, EXPM>(psi, qv, st * s, prm);
+#pragma unroll
+                for (int j = 0; j < NG; ++j) {
+                    const float st = prm.sigt[rm_material(rm) * prm.Gs + g[j]];
+                    const float qv = prm.q[(size_t)r * prm.Gs + g[j]];
+                    attenuate<P, EXPM>(psi[j], qv, st * s, prm);
+                }
                 c_prev = c;
             }
             // chain end (C-3): what leaves minus what the opposite direction brings in at this end
-            float out = 0.f, net = 0.f;
+            const int sidx2 = lk >= 0 && c2 != c_prev ? (c2 >= 0 ? find_surface(cp, c_prev, c2) : -1) : -2;
+            if (sidx2 == -1) *cp.missing = 1;
 #pragma unroll
-            for (int p = 0; p < P; ++p) {
-                const float back = prm.psi_in[((chain ^ 1) * P + p) * prm.Gs + g] * inv_f;
-                out = fmaf(prm.wp[p], psi[p], out);
-                net = fmaf(prm.wp[p], psi[p] - back, net);
-            }
-            double* J = lk < 0 ? cp.J_vac : cp.J_ref;
-            atomicAdd(&J[(size_t)c_prev * prm.G + g], (double)wt * (double)net);
-            if (lk >= 0 && c2 != c_prev) {   // reflective hand-over into another coarse cell: a surface crossing
-                const int sidx = c2 >= 0 ? find_surface(cp, c_prev, c2) : -1;
-                if (sidx < 0) {
-                    *cp.missing = 1;
-                } else {
-                    const double j = (double)wt * (double)out;
-                    atomicAdd(&cp.J_surf[(size_t)sidx * prm.G + g], c_prev < c2 ? j : -j);
-                    atomicAdd(&cp.J_ref[(size_t)c_prev * prm.G + g], -j);
-                    atomicAdd(&cp.J_ref[(size_t)c2 * prm.G + g], j);
+            for (int j = 0; j < NG; ++j) {
+                if (!act[j]) continue;
+                float out = 0.f, net = 0.f;
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    const float back = prm.psi_in[((chain ^ 1) * P + p) * prm.Gs + g[j]] * inv_f;
+                    out = fmaf(prm.wp[p], psi[j][p], out);
+                    net = fmaf(prm.wp[p], psi[j][p] - back, net);
+                }
+                double* J = lk < 0 ? cp.J_vac : cp.J_ref;
+                atomicAdd(&J[(size_t)c_prev * prm.G + g[j]], (double)wt * (double)net);
+                if (sidx2 >= 0) {   // reflective hand-over into another coarse cell: a surface crossing
+                    const double jj = (double)wt * (double)out;
+                    atomicAdd(&cp.J_surf[(size_t)sidx2 * prm.G + g[j]], c_prev < c2 ? jj : -jj);
+                    atomicAdd(&cp.J_ref[(size_t)c_prev * prm.G + g[j]], -jj);
+                    atomicAdd(&cp.J_ref[(size_t)c2 * prm.G + g[j]], jj);
                 }
             }
         }
