@@ -38,7 +38,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--kernel", type=int, default=0, help="ND_SWEEP_* (0 auto)")
     ap.add_argument("--exp-mode", type=int, default=0)
-    for name in ("track-batch", "window-regions", "block-warps", "tile-segments", "delta-buffers", "blocks-per-sm", "tile-lag", "service-warps", "q-copies"):
+    for name in ("window-regions", "block-warps", "tile-segments", "delta-buffers", "blocks-per-sm", "tile-lag", "q-copies", "item-order"):
         ap.add_argument("--" + name, type=int, default=0, help="nd_options tuning field (0 = library default)")
     ap.add_argument("--cpu-seconds", type=float, default=None,
                     help="target CPU time of one oracle sample (default: 15 s for cpu_baseline; --impl reference: 150 s / steps, 2..30 s)")
@@ -236,10 +236,10 @@ def main():
     prob, tr, setup = build_inputs(args)
     t0 = time.time()
     gp = nd.nd_problem_create(prob.xs, prob.polar_sin, prob.polar_weight, prob.mesh.material, tr, device=str(dev),
-                              sweep_kernel=args.kernel, exp_mode=args.exp_mode, track_batch=args.track_batch,
+                              sweep_kernel=args.kernel, exp_mode=args.exp_mode,
                               window_regions=args.window_regions, block_warps=args.block_warps,
                               tile_segments=args.tile_segments, delta_buffers=args.delta_buffers,
-                              blocks_per_sm=args.blocks_per_sm, tile_lag=args.tile_lag, service_warps=args.service_warps,
+                              blocks_per_sm=args.blocks_per_sm, tile_lag=args.tile_lag, item_order=args.item_order,
                               q_copies=args.q_copies)
     setup["create_s"] = round(time.time() - t0, 2)
     info = gp.nd_problem_info_get()

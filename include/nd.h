@@ -42,7 +42,7 @@
 extern "C" {
 #endif
 
-#define ND_VERSION 0x00010000u /* major<<16 | minor<<8 | patch */
+#define ND_VERSION 0x00020000u /* major<<16 | minor<<8 | patch */
 
 typedef enum {
     ND_OK = 0,
@@ -68,18 +68,15 @@ enum {
 enum {
     ND_SWEEP_AUTO = 0,      /* the fastest validated kernel for this G,P */
     ND_SWEEP_ATOMIC = 1,    /* warp per (track,direction), lanes over groups, FP64 global atomics per segment */
-    ND_SWEEP_PRIVATE = 2,   /* lane-group per track batch, FP32 shared-memory private tally window, FP64 flush */
-    ND_SWEEP_SWATH = 3,     /* thread block per swath of adjacent tracks, psi in registers along the whole track,
-                               per-segment delta rows in shared memory, one FP64 RED per (region, group) per tile */
-    ND_SWEEP_SWATH_WS = 4   /* the swath kernel warp-specialised: compute warps run only the segment loop, service warps
-                               stage the tiles and flush the tallies one tile behind, meeting at mbarriers */
+    ND_SWEEP_SWATH = 3      /* thread block per swath of adjacent tracks, psi in registers along the whole track,
+                               per-segment delta rows in shared memory, one FP64 RED per (region, group) per tile.
+                               (Values 2 and 4 named two slower round-1 kernels that were removed.) */
 };
 
 typedef struct {
     int32_t exp_mode;       /* ND_EXP_*      (default 0) */
     int32_t sweep_kernel;   /* ND_SWEEP_*    (default 0) */
-    int32_t track_batch;    /* ND_SWEEP_PRIVATE: tracks per private-tally batch; 0 = default */
-    int32_t window_regions; /* max distinct regions per tile (both tiled kernels); 0 = default */
+    int32_t window_regions; /* ND_SWEEP_SWATH: max distinct regions per tile; 0 = default */
     int32_t block_warps;    /* ND_SWEEP_SWATH: warps per thread block (tracks per swath = warps * slots per warp); 0 = default */
     int32_t tile_segments;  /* ND_SWEEP_SWATH: max segments of one track per tile; 0 = default */
     int32_t delta_buffers;  /* ND_SWEEP_SWATH: 1 or 2 delta buffers; 0 = default (1).  Two buffers no longer save the barrier
@@ -87,8 +84,6 @@ typedef struct {
     int32_t blocks_per_sm;  /* ND_SWEEP_SWATH: resident blocks per SM the grid is sized for; 0 = default */
     int32_t tile_lag;       /* ND_SWEEP_SWATH: drift of the track fronts (in mean segment lengths) under which a tile gives
                                every track the same number of segments; 0 = default, -1 = always cut geometrically */
-    int32_t service_warps;  /* ND_SWEEP_SWATH_WS: staging + flush warps per block (block_warps then counts the compute warps;
-                               compute + service <= 12); 0 = default */
     int32_t q_copies;       /* ND_SWEEP_SWATH, rows of <= 16 groups: copies of a staged q row per shared-memory line.  The
                                Sigma_t table and the delta rows are interleaved NC = 8 / (lanes per track) slots to a line so
                                that the slots of a warp never meet in a bank; q_copies = NC does the same for the q rows
@@ -102,12 +97,15 @@ typedef struct {
     int32_t cmfd_stream;    /* 1: keep the plain SoA segment stream on the device beside the tiled kernel's chunk stream (8 bytes
                                per segment more workspace) so that nd_sweep_currents / nd_cmfd_iteration work with the fast
                                sweep kernels; 0 = default (only ND_SWEEP_ATOMIC problems carry it) */
-    int32_t reserved[3];    /* must be 0 */
+    int32_t item_order;     /* ND_SWEEP_SWATH: order in which thread blocks take the (swath, direction) work items.  0 = default:
+                               most expensive first (best load balance; measured fastest at every config); 1 = angle by angle,
+                               adjacent swaths consecutively (blocks that run together touch neighbouring regions) */
+    int32_t reserved[4];    /* must be 0 */
 } nd_options;
 
 /* ------------------------------------------------------------------------------------------------
  * Host preprocessing: track laydown (rule R-T), links (O-3), half-edge ray walk (rule R-W), track
- * volumes (O-5).  Output is bit-exact against the independent oracle (tests/test_tracks_bitexact.py).
+ * volumes (O-5).  Output is bit-exact against the independent oracle (tests/test_abi_and_tracks.py).
  * ---------------------------------------------------------------------------------------------- */
 typedef struct {
     int32_t n_vertices, n_triangles;
@@ -222,13 +220,19 @@ nd_status nd_transport_sweep(nd_problem* p, const double* d_Q, double* d_phi_out
 nd_status nd_source_update(nd_problem* p, const double* d_phi, double k_eff, double* d_Q_out,
                            double* d_fission_rate_out, void* cuda_stream);
 
-typedef struct { double k_eff, fission_rate, dk, dphi_max; } nd_iter_stats; /* one per iteration, HOST */
+/* One record per iteration, HOST.  leakage = sum over the chains that end on a VACUUM side of w_{t,p} psi_exit, all groups
+ * (with the state normalised to a fission rate of 1, as O-8 sweeps it).  balance_residual = (in - out - sum of the tallies)
+ * / (in + out), in / out = sum of w_{t,p} psi over all track ends entering / leaving: the telescoping identity of Eq. (5)
+ * over the whole sweep, zero up to the FP32 rounding of the chains (~1e-7); a tally credited to no region or
+ * twice shows up here. */
+typedef struct { double k_eff, fission_rate, dk, dphi_max, leakage, balance_residual; } nd_iter_stats;
 
 /* O-8, canonical power iteration from the problem's current state (phi, boundary psi, k).
  *   max_iters >= 0.  tol_k <= 0 and tol_phi <= 0: run exactly max_iters iterations with no host sync inside
  *   the loop.  Otherwise stop when |k - k_prev| < tol_k and max|phi/F - phi_prev|/max(phi) < tol_phi.
  *   k_eff_out HOST; d_phi_out DEVICE [R][G] FP64 or NULL (the un-normalised phi of the last sweep, as in O-8);
- *   iters_done HOST or NULL; stats HOST [max_iters] or NULL (forces one host sync per iteration). */
+ *   iters_done HOST or NULL; stats HOST [max_iters] or NULL: every iteration is recorded (one extra pass over the
+ *   boundary flux per iteration for leakage / balance_residual; the host is synchronised once per 4096 iterations). */
 nd_status nd_power_iteration(nd_problem* p, int32_t max_iters, double tol_k, double tol_phi, double* k_eff_out,
                              double* d_phi_out, int32_t* iters_done, nd_iter_stats* stats_or_null, void* cuda_stream);
 
@@ -373,21 +377,24 @@ typedef struct nd_swath_stream nd_swath_stream;
 typedef struct {
     int64_t n_swaths, n_tiles, blob_bytes, n_items;
     const uint8_t* blob;            /* all chunks, 16-byte aligned each */
-    const uint32_t* tile_chunk;     /* [n_tiles+1] chunk offsets in 16-byte units */
+    const uint32_t* tile_ref;       /* [n_tiles+1][2] chunk offset, size of the chunk's head part; both in 16-byte units */
     const int64_t* swath_tile0;     /* [n_swaths+1] first tile of every swath */
     const int32_t* swath_track;     /* [n_swaths][NT] track id or -1 */
-    const int32_t* items;           /* [n_items][4] swath, direction, cost, 0 -- most expensive first */
+    const int32_t* items;           /* [n_items][4] swath, direction, cost, 0 -- in the order nd_options.item_order selects */
     double mean_regions_per_tile, mean_segments_per_tile, lockstep_efficiency;
-    int32_t max_chunk_bytes, reserved;
+    int32_t max_head_bytes, max_rec_bytes;
 } nd_swath_stream_view_t;
 nd_status nd_swath_stream_build(const nd_problem_desc* desc, int32_t tracks_per_swath, int32_t tile_segments,
                                 int32_t window_regions, int32_t slots_per_line, int32_t row_bytes,
-                                double lag_segments, nd_swath_stream** out);
+                                double lag_segments, int32_t item_order, nd_swath_stream** out);
 nd_status nd_swath_stream_view(const nd_swath_stream* s, nd_swath_stream_view_t* view);
 nd_status nd_swath_stream_destroy(nd_swath_stream* s);
 
 const char* nd_status_string(nd_status s);
-const char* nd_last_error(const nd_problem* p_or_null); /* thread-local message of the last failing call */
+/* Message of the last call that failed ON THE CALLING THREAD (thread-local storage, valid until that thread's next failing
+ * call).  The argument is accepted for symmetry and ignored: errors of calls that have no problem (nd_tracks_generate,
+ * nd_problem_create) are reported the same way. */
+const char* nd_last_error(const nd_problem* p_or_null);
 uint32_t nd_version(void);
 
 #ifdef __cplusplus

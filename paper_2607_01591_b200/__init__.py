@@ -19,7 +19,7 @@ ND_OK = 0
 ND_ERR_NOT_CONVERGED = 7
 ND_BC_VACUUM, ND_BC_REFLECTIVE = 0, 1
 ND_EXP_FAST, ND_EXP_EXPM1 = 0, 1
-ND_SWEEP_AUTO, ND_SWEEP_ATOMIC, ND_SWEEP_PRIVATE, ND_SWEEP_SWATH, ND_SWEEP_SWATH_WS = 0, 1, 2, 3, 4
+ND_SWEEP_AUTO, ND_SWEEP_ATOMIC, ND_SWEEP_SWATH = 0, 1, 3
 
 EXPORTS = [
     "nd_tracks_generate", "nd_tracks_device_workspace_bytes", "nd_tracks_generate_device", "nd_tracks_view", "nd_tracks_destroy", "nd_workspace_bytes", "nd_problem_create",
@@ -38,9 +38,9 @@ class NdError(RuntimeError):
 
 
 class nd_options(C.Structure):
-    _fields_ = [("exp_mode", C.c_int32), ("sweep_kernel", C.c_int32), ("track_batch", C.c_int32),
+    _fields_ = [("exp_mode", C.c_int32), ("sweep_kernel", C.c_int32),
                 ("window_regions", C.c_int32), ("block_warps", C.c_int32), ("tile_segments", C.c_int32),
-                ("delta_buffers", C.c_int32), ("blocks_per_sm", C.c_int32), ("tile_lag", C.c_int32), ("service_warps", C.c_int32), ("q_copies", C.c_int32), ("graph_mode", C.c_int32), ("cmfd_stream", C.c_int32), ("reserved", C.c_int32 * 3)]
+                ("delta_buffers", C.c_int32), ("blocks_per_sm", C.c_int32), ("tile_lag", C.c_int32), ("q_copies", C.c_int32), ("graph_mode", C.c_int32), ("cmfd_stream", C.c_int32), ("item_order", C.c_int32), ("reserved", C.c_int32 * 4)]
 
 
 class nd_mesh_desc(C.Structure):
@@ -66,7 +66,8 @@ class nd_problem_desc(C.Structure):
 
 
 class nd_iter_stats(C.Structure):
-    _fields_ = [("k_eff", C.c_double), ("fission_rate", C.c_double), ("dk", C.c_double), ("dphi_max", C.c_double)]
+    _fields_ = [("k_eff", C.c_double), ("fission_rate", C.c_double), ("dk", C.c_double), ("dphi_max", C.c_double),
+                ("leakage", C.c_double), ("balance_residual", C.c_double)]
 
 
 class nd_profile(C.Structure):
@@ -89,9 +90,9 @@ class nd_trace_timing(C.Structure):
 
 class nd_swath_stream_view_t(C.Structure):
     _fields_ = [("n_swaths", C.c_int64), ("n_tiles", C.c_int64), ("blob_bytes", C.c_int64), ("n_items", C.c_int64),
-                ("blob", C.c_void_p), ("tile_chunk", C.c_void_p), ("swath_tile0", C.c_void_p), ("swath_track", C.c_void_p),
+                ("blob", C.c_void_p), ("tile_ref", C.c_void_p), ("swath_tile0", C.c_void_p), ("swath_track", C.c_void_p),
                 ("items", C.c_void_p), ("mean_regions_per_tile", C.c_double), ("mean_segments_per_tile", C.c_double),
-                ("lockstep_efficiency", C.c_double), ("max_chunk_bytes", C.c_int32), ("reserved", C.c_int32)]
+                ("lockstep_efficiency", C.c_double), ("max_head_bytes", C.c_int32), ("max_rec_bytes", C.c_int32)]
 
 
 _lib = None
@@ -148,7 +149,7 @@ def lib():
         L.nd_sweep_phases_get.argtypes = [C.c_void_p, C.c_void_p]
         L.nd_problem_info_get.argtypes = [C.c_void_p, C.POINTER(nd_problem_info)]
         L.nd_swath_stream_build.argtypes = [C.POINTER(nd_problem_desc), C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
-                                            C.c_double, C.POINTER(C.c_void_p)]
+                                            C.c_double, C.c_int32, C.POINTER(C.c_void_p)]
         L.nd_swath_stream_view.argtypes = [C.c_void_p, C.POINTER(nd_swath_stream_view_t)]
         L.nd_swath_stream_destroy.argtypes = [C.c_void_p]
         _lib = L
@@ -272,8 +273,8 @@ class Problem:
 
     def __init__(self, region_material, sigma_t, sigma_s, nu_sigma_f, chi, polar_sin, polar_weight, seg_offset,
                  seg_region, seg_length, track_weight, link, track_azim=None, track_ends=None, exp_mode=ND_EXP_FAST,
-                 sweep_kernel=ND_SWEEP_AUTO, track_batch=0, window_regions=0, block_warps=0, tile_segments=0,
-                 delta_buffers=0, blocks_per_sm=0, tile_lag=0, service_warps=0, q_copies=0, graph_mode=0, cmfd_stream=0, device="cuda:0"):
+                 sweep_kernel=ND_SWEEP_AUTO, window_regions=0, block_warps=0, tile_segments=0,
+                 delta_buffers=0, blocks_per_sm=0, tile_lag=0, q_copies=0, graph_mode=0, cmfd_stream=0, item_order=0, device="cuda:0"):
         import torch
         self.torch = torch
         self.device = torch.device(device)
@@ -292,8 +293,8 @@ class Problem:
         self.R, (self.M, self.G), self.P, self.T = len(keep["rm"]), keep["st"].shape, len(keep["ps"]), len(keep["tw"])
         d = nd_problem_desc(self.R, self.M, self.G, self.P, self.T, *[keep[k].ctypes.data for k in
                             ("rm", "st", "ss", "nf", "ch", "ps", "pw", "so", "sr", "sl", "tw", "lk")], *geo)
-        opt = nd_options(int(exp_mode), int(sweep_kernel), int(track_batch), int(window_regions), int(block_warps),
-                         int(tile_segments), int(delta_buffers), int(blocks_per_sm), int(tile_lag), int(service_warps), int(q_copies), int(graph_mode), int(cmfd_stream))
+        opt = nd_options(int(exp_mode), int(sweep_kernel), int(window_regions), int(block_warps),
+                         int(tile_segments), int(delta_buffers), int(blocks_per_sm), int(tile_lag), int(q_copies), int(graph_mode), int(cmfd_stream), int(item_order))
         nbytes = C.c_size_t()
         _check(lib().nd_workspace_bytes(C.byref(d), C.byref(opt), C.byref(nbytes)), "nd_workspace_bytes")
         self.workspace_bytes = int(nbytes.value)
@@ -349,8 +350,8 @@ class Problem:
         _check(rc, "nd_power_iteration", allow=(ND_ERR_NOT_CONVERGED,))
         out = dict(k_eff=k.value, iters=it.value, converged=(rc == ND_OK))
         if want_stats:
-            out["stats"] = [dict(k_eff=s.k_eff, fission_rate=s.fission_rate, dk=s.dk, dphi_max=s.dphi_max)
-                            for s in stats[:it.value]]
+            out["stats"] = [dict(k_eff=s.k_eff, fission_rate=s.fission_rate, dk=s.dk, dphi_max=s.dphi_max, leakage=s.leakage,
+                                 balance_residual=s.balance_residual) for s in stats[:it.value]]
         return out
 
     # ---- state ----
@@ -462,9 +463,9 @@ class Problem:
 
 def nd_swath_stream_build(region_material, n_materials, seg_offset, seg_region, seg_length, tracks_per_swath,
                           tile_segments, window_regions, slots_per_line, row_bytes, track_azim=None, track_ends=None,
-                          lag_segments=-1.0):
+                          lag_segments=-1.0, item_order=0):
     """Diagnostics (HOST only, no GPU): the swath/tile chunk stream of ND_SWEEP_SWATH as numpy copies.
-    Returns a dict with blob (uint8), tile_chunk, swath_tile0, swath_track [n_swaths][NT], items [n][4] and stats."""
+    Returns a dict with blob (uint8), tile_ref [n_tiles+1][2], swath_tile0, swath_track [n_swaths][NT], items [n][4] and stats."""
     keep = dict(rm=np.ascontiguousarray(region_material, np.int32), so=np.ascontiguousarray(seg_offset, np.int64),
                 sr=np.ascontiguousarray(seg_region, np.int32), sl=np.ascontiguousarray(seg_length, np.float64))
     d = nd_problem_desc()
@@ -477,19 +478,19 @@ def nd_swath_stream_build(region_material, n_materials, seg_offset, seg_region, 
         d.track_azim, d.track_ends = keep["ta"].ctypes.data, keep["te"].ctypes.data
     h = C.c_void_p()
     _check(lib().nd_swath_stream_build(C.byref(d), int(tracks_per_swath), int(tile_segments), int(window_regions),
-                                       int(slots_per_line), int(row_bytes), float(lag_segments), C.byref(h)),
+                                       int(slots_per_line), int(row_bytes), float(lag_segments), int(item_order), C.byref(h)),
                "nd_swath_stream_build")
     try:
         v = nd_swath_stream_view_t()
         _check(lib().nd_swath_stream_view(h, C.byref(v)), "nd_swath_stream_view")
         return dict(n_swaths=v.n_swaths, n_tiles=v.n_tiles,
                     blob=_np_view(v.blob, (v.blob_bytes,), np.uint8).copy(),
-                    tile_chunk=_np_view(v.tile_chunk, (v.n_tiles + 1,), np.uint32).copy(),
+                    tile_ref=_np_view(v.tile_ref, (v.n_tiles + 1, 2), np.uint32).copy(),
                     swath_tile0=_np_view(v.swath_tile0, (v.n_swaths + 1,), np.int64).copy(),
                     swath_track=_np_view(v.swath_track, (v.n_swaths, int(tracks_per_swath)), np.int32).copy(),
                     items=_np_view(v.items, (v.n_items, 4), np.int32).copy(),
                     mean_regions_per_tile=v.mean_regions_per_tile, mean_segments_per_tile=v.mean_segments_per_tile,
-                    lockstep_efficiency=v.lockstep_efficiency, max_chunk_bytes=v.max_chunk_bytes)
+                    lockstep_efficiency=v.lockstep_efficiency, max_head_bytes=v.max_head_bytes, max_rec_bytes=v.max_rec_bytes)
     finally:
         lib().nd_swath_stream_destroy(h)
 

@@ -21,7 +21,7 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
 GXX_FLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fopenmp", "-fPIC", "-Wall"]
 
 CU_SOURCES = ["nd_api.cu", "nd_trace_device.cu"]
-CXX_SOURCES = ["nd_tracks.cpp", "nd_tiles.cpp", "nd_swath.cpp"]
+CXX_SOURCES = ["nd_tracks.cpp", "nd_swath.cpp"]
 
 
 def _nvcc():

@@ -16,11 +16,8 @@
 #include "nd_internal.h"
 #include "nd_kernels.cuh"
 #include "nd_cmfd.cuh"
-#include "nd_sweep_private.cuh"
 #include "nd_sweep_swath.cuh"
-#include "nd_sweep_swath_ws.cuh"
 #include "nd_swath.h"
-#include "nd_tiles.h"
 
 // ------------------------------------------------------------------------------------------------
 // errors
@@ -75,66 +72,24 @@ struct Dims {
     int64_t S, Spad;
 };
 
-// Configuration of the private-tally sweep (ND_SWEEP_PRIVATE) for a given G; feasible == false -> atomic kernel only.
-struct PrivConfig {
-    bool feasible = false;
-    NdTileParams tp{};
-    int GPL = 4, LPT = 0, slot_bytes = 0, sigt_bytes = 0, chunk_cap = 0, warps = 0, smem_bytes = 0;
-    int64_t max_tiles = 0, max_swaths = 0;
-    size_t max_blob = 0;
-};
-
 constexpr int kSmemMax = 227 * 1024;
-
-PrivConfig make_priv_config(const Dims& d, const nd_options& opt)
-{
-    PrivConfig c;
-    c.GPL = 4;
-    c.LPT = d.Gs / 4;
-    if (c.LPT > 32) return c;
-    const int tpw = 32 / c.LPT;
-    int B = opt.track_batch > 0 ? opt.track_batch : (tpw >= 8 ? 8 : 16);
-    int Lw = opt.window_regions > 0 ? opt.window_regions : 32;
-    if (B > 64) B = 64;
-    if (Lw > 255) Lw = 255;
-    if (Lw < B) Lw = B;
-    c.tp.B = B; c.tp.Lw = Lw; c.tp.Nmax = 16 * B; c.tp.TPW = tpw;
-    c.chunk_cap = nd_chunk_capacity_bytes(c.tp);
-    c.slot_bytes = 8 * Lw * d.Gs + 4 * ((B + 3) / 4 * 4) + 2 * c.chunk_cap;
-    const int sig = 4 * d.M * d.Gs;
-    if (sig > 48 * 1024) return c;
-    c.sigt_bytes = (sig + 15) / 16 * 16;
-    c.warps = (kSmemMax - c.sigt_bytes) / (tpw * c.slot_bytes);
-    if (c.warps > 16) c.warps = 16;
-    if (c.warps < 1) return c;
-    c.smem_bytes = c.sigt_bytes + c.warps * tpw * c.slot_bytes;
-    c.max_swaths = d.T;
-    c.max_tiles = d.S / (Lw < c.tp.Nmax ? Lw : c.tp.Nmax) + d.T + 2;
-    const size_t per_tile = 16 + (size_t)((2 * (B + 1) + 15) / 16 * 16) + 4 * (size_t)Lw + 64;
-    c.max_blob = 6 * (size_t)d.S + (size_t)c.max_tiles * per_tile + 256;
-    c.feasible = true;
-    return c;
-}
 
 // Configuration of the swath sweep (ND_SWEEP_SWATH) for a given G; feasible == false -> other kernels only.
 struct SwathConfig {
     bool feasible = false;
     NdSwathParams sp{};
-    int LPT = 0, warps = 0, nsw = 0, ndbuf = 1, blocks_per_sm = 1;
+    int LPT = 0, warps = 0, ndbuf = 1, blocks_per_sm = 1;
     bool tight = false;                                   // register-capped kernel variant (more than 512 resident threads per SM)
-    int chunk_cap = 0, off_sigt = 0, off_q = 0, off_dbuf = 0, off_chunk = 0, smem_bytes = 0;
+    int head_cap = 0, rec_cap = 0, off_sigt = 0, off_q = 0, off_dbuf = 0, off_head = 0, off_rec = 0, smem_bytes = 0;
     int64_t max_tiles = 0, max_swaths = 0;
     size_t max_blob = 0;
 };
 
-inline bool is_swath(int kernel) { return kernel == ND_SWEEP_SWATH || kernel == ND_SWEEP_SWATH_WS; }
-constexpr int kServiceWarps = 5;   // ND_SWEEP_SWATH_WS: staging + flush warps per block (measured best with 7 compute warps at G = 51)
+inline bool is_swath(int kernel) { return kernel == ND_SWEEP_SWATH; }
 
-// ws: the warp-specialised variant -- `warps` counts COMPUTE warps, two delta buffers, two blocks of <= 384 threads per SM
-SwathConfig make_swath_config_q(const Dims& d, const nd_options& opt, bool ws, int q_copies)
+SwathConfig make_swath_config_q(const Dims& d, const nd_options& opt, int q_copies)
 {
     SwathConfig c;
-    c.nsw = ws ? (opt.service_warps > 0 ? (opt.service_warps > 8 ? 8 : opt.service_warps) : kServiceWarps) : 0;
     c.LPT = d.Gs / 4;
     if (c.LPT > 32) return c;
     const int NC = (c.LPT == 1 || c.LPT == 2 || c.LPT == 4) ? 8 / c.LPT : 1;
@@ -143,33 +98,35 @@ SwathConfig make_swath_config_q(const Dims& d, const nd_options& opt, bool ws, i
     if (NCq > NC) NCq = NC;
     while (NC % NCq != 0) --NCq;   // rounded down to a divisor of NC
     const int line_q = NCq * row_bytes;
-    if ((int64_t)d.M * line > 65536) return c;
-    int warps = opt.block_warps > 0 ? opt.block_warps : (ws ? 12 - c.nsw : (c.LPT > 8 ? 8 : 4));
+    if ((int64_t)d.M * line > 64 * 1024) return c;   // the Sigma_t table must leave room for everything else
+    int warps = opt.block_warps > 0 ? opt.block_warps : (c.LPT > 8 ? 8 : 4);
     if (warps > 16) warps = 16;
-    if (ws && warps > 12 - c.nsw) warps = 12 - c.nsw;
-    c.ndbuf = (ws || opt.delta_buffers == 2) ? 2 : 1;
+    c.ndbuf = opt.delta_buffers == 2 ? 2 : 1;
     auto pad128 = [](int x) { return (x + 127) / 128 * 128; };
     auto layout = [&](int w, int Kmax, int Lmax) -> bool {   // fills c for (w, Kmax, Lmax); false if the slot count is unusable
         const int NT = w * 32 / c.LPT / NC * NC;               // slots are packed over the lanes of the whole block
         if (NT < 1 || (int64_t)NT * Kmax > 65535) return false;
         if (Lmax < 16) Lmax = 16;
-        if (Lmax > 65536 / line_q) Lmax = 65536 / line_q;
+        if (Lmax > 4096) Lmax = 4096;
         c.sp.NT = NT; c.sp.Kmax = Kmax; c.sp.Lmax = Lmax; c.sp.NC = NC; c.sp.NCq = NCq; c.sp.row_bytes = row_bytes;
         // narrow rows (G <= 16): the flush is cheap, idle slot steps are not -> equal-count tiles while the fronts stay within
         // 16 segments; wide rows: only within 4 segments (the tally re-use rho pays more than level counts), measured in profiles/
         c.sp.lag = opt.tile_lag < 0 ? -1.0 : (opt.tile_lag > 0 ? (double)opt.tile_lag : (row_bytes < 64 ? 16.0 : 4.0));
-        c.chunk_cap = nd_swath_chunk_capacity(c.sp);
+        c.sp.item_order = opt.item_order;
+        c.head_cap = nd_swath_head_capacity(c.sp);
+        c.rec_cap = nd_swath_rec_capacity(c.sp);
         c.off_sigt = 128;
         c.off_q = c.off_sigt + pad128(d.M * line);
         c.off_dbuf = c.off_q + pad128(2 * Lmax * line_q);
-        c.off_chunk = c.off_dbuf + pad128(c.ndbuf * (NT / NC) * Kmax * line);
-        c.smem_bytes = c.off_chunk + (ws ? 4 : ndk::kSwathChunkBufs) * c.chunk_cap;   // the warp-specialised kernel keeps four
+        c.off_head = c.off_dbuf + pad128(c.ndbuf * (NT * Kmax + 1) * row_bytes);   // + the spare row of the null record
+        c.off_rec = c.off_head + pad128(ndk::kSwathHeadBufs * c.head_cap);
+        c.smem_bytes = c.off_rec + ndk::kSwathRecBufs * c.rec_cap;
         return true;
     };
     // Defaults (measured, profiles/): occupancy beats tile length once a tile holds >= 8 segments per track.  Aim at
     // 3 resident blocks per SM (4 for narrow rows), the longest tile that fits, and a region window sized for the
     // tally re-use the configs show (rho ~ 6.5 wide rows, ~ 8 narrow rows).
-    const int target_blocks = ws ? 2 : (row_bytes < 64 ? 4 : 3);
+    const int target_blocks = row_bytes < 64 ? 4 : 3;
     if (opt.block_warps <= 0) {
         // small problems: fewer tracks per block until there are about two work items (swath, direction) per resident
         // block of a 148-SM part -- the sweep of a small problem is bound by its longest track, not by throughput
@@ -199,8 +156,7 @@ SwathConfig make_swath_config_q(const Dims& d, const nd_options& opt, bool ws, i
     if (!placed) return c;
     c.warps = warps;
     int bps = (kSmemMax + 1024) / (c.smem_bytes + 1024);  // 1 KB per block is reserved by the driver
-    if (ws && bps > 2) bps = 2;
-    if (!ws && bps * warps * 32 > 768) bps = 768 / (warps * 32);  // 85 registers per thread at most
+    if (bps * warps * 32 > 768) bps = 768 / (warps * 32);  // 85 registers per thread at most
     if (bps > 8) bps = 8;
     if (bps < 1) bps = 1;
     if (opt.blocks_per_sm > 0 && opt.blocks_per_sm < bps) bps = opt.blocks_per_sm;
@@ -215,29 +171,26 @@ SwathConfig make_swath_config_q(const Dims& d, const nd_options& opt, bool ws, i
 }
 
 // q rows: one copy per region unless asked otherwise (measured: config 3 0.628 -> 0.555 ms, config 2 0.079 -> 0.070 ms).
-// The warp-specialised variant and the register-capped variant of k_sweep_swath are compiled for q rows laid out like
-// the Sigma_t table (NCq = NC, no extra registers): if the one-copy layout ends up on the capped variant the
-// configuration is redone with replicated rows.
-SwathConfig make_swath_config(const Dims& d, const nd_options& opt, bool ws = false)
+// The register-capped variant of k_sweep_swath is compiled for q rows laid out like the Sigma_t table (NCq = NC, no
+// extra registers): if the one-copy layout ends up on the capped variant the configuration is redone with replicated rows.
+SwathConfig make_swath_config(const Dims& d, const nd_options& opt)
 {
-    if (ws) return make_swath_config_q(d, opt, true, 0);
-    SwathConfig c = make_swath_config_q(d, opt, false, opt.q_copies > 0 ? opt.q_copies : 1);
-    if (c.feasible && c.tight && c.sp.NCq != c.sp.NC) c = make_swath_config_q(d, opt, false, 0);
+    SwathConfig c = make_swath_config_q(d, opt, opt.q_copies > 0 ? opt.q_copies : 1);
+    if (c.feasible && c.tight && c.sp.NCq != c.sp.NC) c = make_swath_config_q(d, opt, 0);
     return c;
 }
 
 // Which sweep kernel a descriptor + options select (decided before the workspace is sized).
-int select_kernel(const nd_problem_desc* desc, const nd_options& opt, const PrivConfig& pc, const SwathConfig& sc)
+int select_kernel(const nd_problem_desc* desc, const nd_options& opt, const SwathConfig& sc)
 {
     if (is_swath(opt.sweep_kernel) && sc.feasible) return opt.sweep_kernel;
-    if (opt.sweep_kernel == ND_SWEEP_PRIVATE && pc.feasible) return ND_SWEEP_PRIVATE;
     if (opt.sweep_kernel == ND_SWEEP_AUTO && desc->track_ends && sc.feasible) return ND_SWEEP_SWATH;
     return ND_SWEEP_ATOMIC;
 }
 
 struct Layout { // byte offsets into the workspace
     size_t seg_rm, seg_len, trk_off, trk_w, link_src, psi_a, psi_b, q, tally, phi_a, phi_b, Q, reg_mat, vol, sigt, sigsT,
-        nusf, chi, sigt_f, scalars, partial, stats, src_region, src_chunks, phase, blob, tile_chunk, swath_tile0, swath_track, items, counter, total;
+        nusf, chi, sigt_f, scalars, partial, partial_b, exit_vac, stats, src_region, src_chunks, phase, blob, tile_chunk, swath_tile0, swath_track, items, counter, total;
 };
 
 inline size_t bump(size_t& cur, size_t bytes)
@@ -247,14 +200,8 @@ inline size_t bump(size_t& cur, size_t bytes)
     return at;
 }
 
-Layout make_layout(const Dims& d, int max_stats, const PrivConfig& pc_in, const SwathConfig& sc, int kernel, bool keep_soa)
+Layout make_layout(const Dims& d, int max_stats, const SwathConfig& sc, int kernel, bool keep_soa)
 {
-    // the tiled kernels share the stream fields of the layout; size them for the selected one
-    PrivConfig pc = pc_in;
-    pc.feasible = kernel == ND_SWEEP_PRIVATE || is_swath(kernel);
-    if (is_swath(kernel)) {
-        pc.max_blob = sc.max_blob; pc.max_tiles = sc.max_tiles; pc.max_swaths = sc.max_swaths; pc.tp.B = sc.sp.NT;
-    }
     Layout L{};
     size_t c = 0;
     const size_t RG = (size_t)d.R * d.G, RGs = (size_t)d.R * d.Gs, NPSI = (size_t)d.T * 2 * d.P * d.Gs;
@@ -281,17 +228,19 @@ Layout make_layout(const Dims& d, int max_stats, const PrivConfig& pc_in, const 
     L.chi = bump(c, sizeof(double) * (size_t)d.M * d.G);
     L.sigt_f = bump(c, sizeof(float) * (size_t)d.M * d.Gs);
     L.scalars = bump(c, sizeof(double) * ndk::SC_COUNT);
-    L.partial = bump(c, sizeof(double) * 3 * kReduceBlocks);
-    L.stats = bump(c, sizeof(double) * 4 * (size_t)max_stats);
+    L.partial = bump(c, sizeof(double) * ndk::kPartialStride * kReduceBlocks);
+    L.partial_b = bump(c, sizeof(double) * ndk::kPartialStride * kReduceBlocks);
+    L.exit_vac = bump(c, 2 * (size_t)d.T);
+    L.stats = bump(c, sizeof(double) * ndk::kStatsStride * (size_t)max_stats);
     L.phase = bump(c, 256);
     L.src_region = bump(c, sizeof(int32_t) * (size_t)d.R);
     L.src_chunks = bump(c, sizeof(int4) * ((size_t)d.R / 4 + (size_t)d.M + 1));   // chunks hold >= 4 regions except one per material
-    if (pc.feasible) {
-        L.blob = bump(c, pc.max_blob);
-        L.tile_chunk = bump(c, sizeof(uint32_t) * (size_t)pc.max_tiles);
-        L.swath_tile0 = bump(c, sizeof(int64_t) * ((size_t)pc.max_swaths + 1));
-        L.swath_track = bump(c, sizeof(int32_t) * (size_t)pc.max_swaths * pc.tp.B);
-        L.items = bump(c, sizeof(int4) * (2 * (size_t)pc.max_swaths + 2));
+    if (is_swath(kernel)) {
+        L.blob = bump(c, sc.max_blob);
+        L.tile_chunk = bump(c, sizeof(uint2) * (size_t)sc.max_tiles);
+        L.swath_tile0 = bump(c, sizeof(int64_t) * ((size_t)sc.max_swaths + 1));
+        L.swath_track = bump(c, sizeof(int32_t) * (size_t)sc.max_swaths * sc.sp.NT);
+        L.items = bump(c, sizeof(int4) * (2 * (size_t)sc.max_swaths + 2));
         L.counter = bump(c, 256);
     }
     L.total = c;
@@ -340,14 +289,13 @@ struct nd_problem {
     uint32_t* seg_rm; float* seg_len; int64_t* trk_off; float* trk_w; int32_t* link_src;
     float* psi_in; float* psi_out; float* q; double* tally; double* phi_cur; double* phi_new; double* Q;
     int32_t* reg_mat; double* vol; double* sigt; double* sigsT; double* nusf; double* chi; float* sigt_f;
-    double* scalars; double* partial; double* stats;
+    double* scalars; double* partial; double* partial_b; uint8_t* exit_vac; double* stats;
     int32_t* src_region = nullptr; int4* src_chunks = nullptr;
     int n_src_chunks = 0, src_chunk_regions = 0;
-    // private-tally sweep
-    PrivConfig pc{};
+    // swath sweep
     SwathConfig sc{};
     double lockstep_efficiency = 0.0;
-    uint8_t* blob = nullptr; uint32_t* tile_chunk = nullptr; int64_t* swath_tile0 = nullptr; int32_t* swath_track = nullptr;
+    uint8_t* blob = nullptr; uint2* tile_ref = nullptr; int64_t* swath_tile0 = nullptr; int32_t* swath_track = nullptr;
     int4* items = nullptr; int* counter = nullptr;
     int n_items = 0;
     int64_t n_tiles = 0;
@@ -406,7 +354,7 @@ nd_status launch_fission_rate(nd_problem* p, const double* d_phi, double* d_out,
     const int grid = grid_for((int64_t)d.R * d.G, 256, kReduceBlocks);
     ndk::k_fission_partial<<<grid, 256, 0, st>>>(d_phi, p->reg_mat, p->nusf, p->vol, p->partial, d.R, d.G);
     ND_LAUNCH_CHECK(p);
-    ndk::k_reduce_final<<<1, 256, 0, st>>>(p->partial, grid, p->scalars, 0, nullptr);
+    ndk::k_reduce_final<<<1, 256, 0, st>>>(p->partial, grid, p->scalars, 0, nullptr, nullptr, 0);
     ND_LAUNCH_CHECK(p);
     if (d_out) ND_CUDA(cudaMemcpyAsync(d_out, p->scalars + ndk::SC_F, sizeof(double), cudaMemcpyDeviceToDevice, st));
     return ND_OK;
@@ -416,37 +364,6 @@ inline int swath_grid(const nd_problem* p)
 {
     const int g = p->n_sm * p->sc.blocks_per_sm;
     return p->n_items < g ? (p->n_items > 0 ? p->n_items : 1) : g;
-}
-
-template <int P>
-nd_status launch_private_p(nd_problem* p, const ndk::PrivParams& prm, cudaStream_t st)
-{
-    const PrivConfig& c = p->pc;
-    auto kern = p->opt.exp_mode == ND_EXP_EXPM1 ? ndk::k_sweep_private<P, 4, 1> : ndk::k_sweep_private<P, 4, 0>;
-    ND_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes));
-    kern<<<p->n_sm, 32 * c.warps, c.smem_bytes, st>>>(prm);
-    ND_LAUNCH_CHECK(p);
-    return ND_OK;
-}
-
-nd_status launch_private(nd_problem* p, const double* scale_div, cudaStream_t st)
-{
-    const Dims& d = p->d;
-    const PrivConfig& c = p->pc;
-    ndk::PrivParams prm{};
-    prm.blob = p->blob; prm.tile_chunk = p->tile_chunk; prm.swath_tile0 = p->swath_tile0; prm.swath_track = p->swath_track;
-    prm.items = p->items; prm.counter = p->counter; prm.q = p->q; prm.sigt = p->sigt_f; prm.tally = p->tally; prm.trk_w = p->trk_w;
-    prm.psi_in = p->psi_in; prm.psi_out = p->psi_out; prm.scale_div = scale_div;
-    prm.n_items = p->n_items; prm.G = d.G; prm.Gs = d.Gs; prm.M = d.M; prm.B = c.tp.B; prm.Lw = c.tp.Lw; prm.LPT = c.LPT; prm.TPW = c.tp.TPW;
-    prm.slot_bytes = c.slot_bytes; prm.sigt_bytes = c.sigt_bytes; prm.chunk_cap = c.chunk_cap;
-    for (int i = 0; i < ndk::kMaxPolar; ++i) { prm.c[i] = p->c[i]; prm.inv_sin[i] = p->inv_sin[i]; prm.wp[i] = p->wp[i]; }
-    ND_CUDA(cudaMemsetAsync(p->counter, 0, sizeof(int), st));
-    switch (d.P) {
-    case 1: return launch_private_p<1>(p, prm, st);
-    case 2: return launch_private_p<2>(p, prm, st);
-    case 3: return launch_private_p<3>(p, prm, st);
-    default: return launch_private_p<4>(p, prm, st);
-    }
 }
 
 template <int P>
@@ -470,39 +387,23 @@ nd_status launch_swath(nd_problem* p, const double* scale_div, cudaStream_t st)
     const Dims& d = p->d;
     const SwathConfig& c = p->sc;
     ndk::SwathParams prm{};
-    prm.blob = p->blob; prm.tile_chunk = p->tile_chunk; prm.swath_tile0 = p->swath_tile0; prm.swath_track = p->swath_track;
+    prm.blob = p->blob; prm.tile_ref = p->tile_ref; prm.swath_tile0 = p->swath_tile0; prm.swath_track = p->swath_track;
     prm.items = p->items; prm.counter = p->counter; prm.q = p->q; prm.sigt = p->sigt_f; prm.tally = p->tally; prm.trk_w = p->trk_w;
     prm.psi_in = p->psi_in; prm.psi_out = p->psi_out; prm.scale_div = scale_div;
     prm.n_items = p->n_items; prm.G = d.G; prm.Gs = d.Gs; prm.M = d.M; prm.NT = c.sp.NT; prm.Kmax = c.sp.Kmax; prm.Lmax = c.sp.Lmax;
-    prm.LPT = c.LPT; prm.NC = c.sp.NC; prm.NCq = c.sp.NCq > 0 ? c.sp.NCq : c.sp.NC; prm.ndbuf = c.ndbuf; prm.chunk_cap = c.chunk_cap;
-    prm.off_sigt = c.off_sigt; prm.off_q = c.off_q; prm.off_dbuf = c.off_dbuf; prm.off_chunk = c.off_chunk;
+    prm.LPT = c.LPT; prm.NC = c.sp.NC; prm.NCq = c.sp.NCq > 0 ? c.sp.NCq : c.sp.NC; prm.ndbuf = c.ndbuf; prm.head_cap = c.head_cap; prm.rec_cap = c.rec_cap;
+    prm.off_sigt = c.off_sigt; prm.off_q = c.off_q; prm.off_dbuf = c.off_dbuf; prm.off_head = c.off_head; prm.off_rec = c.off_rec;
     for (int i = 0; i < ndk::kMaxPolar; ++i) {
         prm.c[i] = p->c[i]; prm.inv_sin[i] = p->inv_sin[i]; prm.wp[i] = p->wp[i];
+        const float ratio = p->c[0] != 0.f ? p->c[i] / p->c[0] : 0.f;   // the kernel's Sigma_t table carries c[0]
         uint32_t bits;
-        memcpy(&bits, &p->c[i], 4);
+        memcpy(&bits, &ratio, 4);
         prm.c2[i] = (unsigned long long)bits | ((unsigned long long)bits << 32);
     }
     prm.magic_per_row = ndk::fastdiv_magic((uint32_t)((c.sp.NCq > 0 ? c.sp.NCq : c.sp.NC) * (d.Gs / 4)));
     prm.magic_nq = ndk::fastdiv_magic((uint32_t)(d.Gs / 4));
     prm.phase = p->phase;
     ND_CUDA(cudaMemsetAsync(p->counter, 0, sizeof(int), st));
-    if (p->sweep_kernel == ND_SWEEP_SWATH_WS) {
-        ndk::SwathWsParams wsp{};
-        wsp.base = prm; wsp.ncw = c.warps; wsp.nsw = c.nsw;
-        const int threads = 32 * (c.warps + c.nsw);
-        auto launch = [&](auto kern) -> nd_status {
-            ND_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes));
-            kern<<<swath_grid(p), threads, c.smem_bytes, st>>>(wsp);
-            ND_LAUNCH_CHECK(p);
-            return ND_OK;
-        };
-        switch (d.P) {
-        case 1: return launch(ndk::k_sweep_swath_ws<1>);
-        case 2: return launch(ndk::k_sweep_swath_ws<2>);
-        case 3: return launch(ndk::k_sweep_swath_ws<3>);
-        default: return launch(ndk::k_sweep_swath_ws<4>);
-        }
-    }
     switch (d.P) {
     case 1: return launch_swath_p<1>(p, prm, st);
     case 2: return launch_swath_p<2>(p, prm, st);
@@ -542,8 +443,9 @@ nd_status launch_source(nd_problem* p, const ndk::SourceParams& sp, cudaStream_t
     return ND_OK;
 }
 
-// A2 + A3: sweep with the current q/tally, then advance the boundary flux through the link table.
-nd_status launch_sweep(nd_problem* p, const double* scale_div, cudaStream_t st)
+// A2 + A3: sweep with the current q/tally, then advance the boundary flux through the link table.  balance: also sum what
+// entered and left through the track ends (k_boundary_balance, between the sweep and the swap) into p->partial_b.
+nd_status launch_sweep(nd_problem* p, const double* scale_div, cudaStream_t st, bool balance = false)
 {
     const Dims& d = p->d;
     ndk::SweepParams prm{};
@@ -566,8 +468,6 @@ nd_status launch_sweep(nd_problem* p, const double* scale_div, cudaStream_t st)
     nd_status rc;
     if (is_swath(p->sweep_kernel)) {
         rc = launch_swath(p, scale_div, st);
-    } else if (p->sweep_kernel == ND_SWEEP_PRIVATE) {
-        rc = launch_private(p, scale_div, st);
     } else {
         switch (d.P) {
         case 1: rc = launch_sweep_p<1>(p, prm, st); break;
@@ -580,6 +480,12 @@ nd_status launch_sweep(nd_problem* p, const double* scale_div, cudaStream_t st)
     if (ev) ND_CUDA(cudaEventRecord(ev->b, st));
     const int PG = d.P * d.Gs;
     const int64_t n = 2 * (int64_t)d.T * PG;
+    if (balance) {
+        ndk::k_boundary_balance<<<grid_for(n, 256, kReduceBlocks), 256, 0, st>>>(p->psi_in, p->psi_out, p->trk_w, p->exit_vac, scale_div,
+                                                                             p->partial_b, 2 * (int64_t)d.T, d.P, d.G, d.Gs, p->wp[0],
+                                                                             p->wp[1], p->wp[2], p->wp[3]);
+        ND_LAUNCH_CHECK(p);
+    }
     ndk::k_link_swap<<<grid_for(n, 256, 8 * p->n_sm), 256, 0, st>>>(p->psi_out, p->psi_in, p->link_src, 2 * (int64_t)d.T, PG);
     ND_LAUNCH_CHECK(p);
     return ND_OK;
@@ -625,11 +531,9 @@ extern "C" nd_status nd_workspace_bytes(const nd_problem_desc* desc, const nd_op
     if (rc != ND_OK) return rc;
     nd_options opt{};
     if (opts) opt = *opts;
-    PrivConfig pc;
     SwathConfig sc;
-    if (opt.sweep_kernel == ND_SWEEP_PRIVATE) pc = make_priv_config(d, opt);
-    if (is_swath(opt.sweep_kernel) || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt, opt.sweep_kernel == ND_SWEEP_SWATH_WS);
-    *device_bytes = make_layout(d, kMaxStats, pc, sc, select_kernel(desc, opt, pc, sc), opt.cmfd_stream != 0).total;
+    if (is_swath(opt.sweep_kernel) || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt);
+    *device_bytes = make_layout(d, kMaxStats, sc, select_kernel(desc, opt, sc), opt.cmfd_stream != 0).total;
     return ND_OK;
 }
 
@@ -646,22 +550,22 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     if (rc != ND_OK) return rc;
     nd_options opt{};
     if (opts) opt = *opts;
-    for (int i = 0; i < 3; ++i)
+    if (opt.item_order < 0 || opt.item_order > 1) return nd_fail(ND_ERR_INVALID, "nd_options.item_order must be 0 or 1");
+    for (int i = 0; i < 4; ++i)
         if (opt.reserved[i] != 0) return nd_fail(ND_ERR_INVALID, "nd_options.reserved must be zero");
     if (opt.cmfd_stream < 0 || opt.cmfd_stream > 1) return nd_fail(ND_ERR_INVALID, "nd_options.cmfd_stream must be 0 or 1");
     if (opt.exp_mode != ND_EXP_FAST && opt.exp_mode != ND_EXP_EXPM1) return nd_fail(ND_ERR_INVALID, "unknown exp_mode");
-    if (opt.sweep_kernel < ND_SWEEP_AUTO || opt.sweep_kernel > ND_SWEEP_SWATH_WS) return nd_fail(ND_ERR_INVALID, "unknown sweep_kernel");
-    if (opt.track_batch < 0 || opt.window_regions < 0 || opt.block_warps < 0 || opt.tile_segments < 0 || opt.delta_buffers < 0 ||
-        opt.delta_buffers > 2 || opt.blocks_per_sm < 0 || opt.tile_lag < -1 || opt.service_warps < 0 || opt.q_copies < 0 || opt.graph_mode < 0 || opt.graph_mode > 1)
+    if (opt.sweep_kernel != ND_SWEEP_AUTO && opt.sweep_kernel != ND_SWEEP_ATOMIC && opt.sweep_kernel != ND_SWEEP_SWATH)
+        return nd_fail(ND_ERR_INVALID, "unknown sweep_kernel");
+    if (opt.window_regions < 0 || opt.block_warps < 0 || opt.tile_segments < 0 || opt.delta_buffers < 0 ||
+        opt.delta_buffers > 2 || opt.blocks_per_sm < 0 || opt.tile_lag < -1 || opt.q_copies < 0 || opt.graph_mode < 0 || opt.graph_mode > 1)
         return nd_fail(ND_ERR_INVALID, "nd_options: tuning fields must be >= 0 (delta_buffers 0, 1 or 2)");
     if ((desc->track_azim == nullptr) != (desc->track_ends == nullptr))
         return nd_fail(ND_ERR_INVALID, "track_azim and track_ends must both be set or both be NULL");
-    PrivConfig pc;
     SwathConfig sc;
-    if (opt.sweep_kernel == ND_SWEEP_PRIVATE) pc = make_priv_config(d, opt);
-    if (is_swath(opt.sweep_kernel) || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt, opt.sweep_kernel == ND_SWEEP_SWATH_WS);
-    const int kernel = select_kernel(desc, opt, pc, sc);
-    const Layout L = make_layout(d, kMaxStats, pc, sc, kernel, opt.cmfd_stream != 0);
+    if (is_swath(opt.sweep_kernel) || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt);
+    const int kernel = select_kernel(desc, opt, sc);
+    const Layout L = make_layout(d, kMaxStats, sc, kernel, opt.cmfd_stream != 0);
     if (reinterpret_cast<uintptr_t>(device_workspace) % kAlign != 0) return nd_fail(ND_ERR_WORKSPACE, "workspace must be 256-byte aligned");
     if (device_bytes < L.total) return nd_fail(ND_ERR_WORKSPACE, "workspace smaller than nd_workspace_bytes");
 
@@ -689,15 +593,17 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         if (!(desc->seg_length[k] > 0.0) || !std::isfinite(desc->seg_length[k])) return nd_fail(ND_ERR_INVALID, "seg_length must be finite and > 0");
     }
     std::vector<int32_t> link_src;
+    std::vector<uint8_t> h_exit_vac;
     nd_problem* p = nullptr;
     std::vector<uint32_t> h_rm;
     std::vector<float> h_len;
     std::vector<int64_t> h_off;
     try {
         link_src.assign(2 * (size_t)d.T, -1);
+        h_exit_vac.assign(2 * (size_t)d.T, 0);
         for (int64_t e = 0; e < 2 * (int64_t)d.T; ++e) {
             const int32_t lk = desc->link[e];
-            if (lk == -1) continue;
+            if (lk == -1) { h_exit_vac[(size_t)e] = 1; continue; }
             if (lk < 0 || lk >= 2 * d.T) return nd_fail(ND_ERR_RANGE, "link out of range");
             if (link_src[lk] != -1) return nd_fail(ND_ERR_INVALID, "two track ends link to the same entry");
             link_src[lk] = (int32_t)e;
@@ -739,29 +645,19 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         delete p;
         return nd_fail(ND_ERR_NOMEM, "nd_problem_create: out of host memory");
     }
-    // ---- A1 (fast path): swath/tile chunk stream for the private-tally sweep ----
-    NdTileSet tiles;
+    // ---- A1 (fast path): swath/tile chunk stream of k_sweep_swath ----
     NdSwathSet swaths;
-    const bool want_private = kernel == ND_SWEEP_PRIVATE, want_swath = is_swath(kernel);
-    const bool tiled = want_private || want_swath;
+    const bool want_swath = is_swath(kernel);
+    const bool tiled = want_swath;
     if (want_swath) {
         rc = nd_build_swaths(desc, desc->track_azim, desc->track_ends, sc.sp, 0, &swaths);
         if (rc != ND_OK) { delete p; return rc; }
         if (swaths.blob.size() > sc.max_blob || swaths.n_tiles + 1 > sc.max_tiles || swaths.n_swaths > sc.max_swaths ||
-            swaths.max_chunk_bytes > sc.chunk_cap) {
+            swaths.max_head_bytes > sc.head_cap || swaths.max_rec_bytes > sc.rec_cap) {
             delete p;
             return nd_fail(ND_ERR_WORKSPACE, "internal: swath stream larger than its workspace bound");
         }
     }
-    if (want_private) {
-        rc = nd_build_tiles(desc, desc->track_azim, desc->track_ends, pc.tp, 0, &tiles);
-        if (rc != ND_OK) { delete p; return rc; }
-        if (tiles.blob.size() > pc.max_blob || tiles.n_tiles + 1 > pc.max_tiles || tiles.n_swaths > pc.max_swaths) {
-            delete p;
-            return nd_fail(ND_ERR_WORKSPACE, "internal: tile stream larger than its workspace bound");
-        }
-    }
-    p->pc = pc;
     p->sc = sc;
     char* ws = p->ws;
     p->seg_rm = (uint32_t*)(ws + L.seg_rm); p->seg_len = (float*)(ws + L.seg_len); p->trk_off = (int64_t*)(ws + L.trk_off);
@@ -773,10 +669,11 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     p->sigt = (double*)(ws + L.sigt); p->sigsT = (double*)(ws + L.sigsT); p->nusf = (double*)(ws + L.nusf);
     p->chi = (double*)(ws + L.chi); p->sigt_f = (float*)(ws + L.sigt_f);
     p->scalars = (double*)(ws + L.scalars); p->partial = (double*)(ws + L.partial); p->stats = (double*)(ws + L.stats);
+    p->partial_b = (double*)(ws + L.partial_b); p->exit_vac = (uint8_t*)(ws + L.exit_vac);
     p->phase = (unsigned long long*)(ws + L.phase);
     p->src_region = (int32_t*)(ws + L.src_region); p->src_chunks = (int4*)(ws + L.src_chunks);
     if (tiled) {
-        p->blob = (uint8_t*)(ws + L.blob); p->tile_chunk = (uint32_t*)(ws + L.tile_chunk); p->swath_tile0 = (int64_t*)(ws + L.swath_tile0);
+        p->blob = (uint8_t*)(ws + L.blob); p->tile_ref = (uint2*)(ws + L.tile_chunk); p->swath_tile0 = (int64_t*)(ws + L.swath_tile0);
         p->swath_track = (int32_t*)(ws + L.swath_track); p->items = (int4*)(ws + L.items); p->counter = (int*)(ws + L.counter);
     }
 
@@ -843,28 +740,18 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         p->mean_segments_per_tile = swaths.mean_segments_per_tile;
         p->lockstep_efficiency = swaths.lockstep_efficiency;
         ND_CUDA_P(cudaMemcpyAsync(p->blob, swaths.blob.data(), swaths.blob.size(), cudaMemcpyHostToDevice, st));
-        ND_CUDA_P(cudaMemcpyAsync(p->tile_chunk, swaths.tile_chunk.data(), sizeof(uint32_t) * swaths.tile_chunk.size(), cudaMemcpyHostToDevice, st));
+        static_assert(sizeof(NdSwathTileRef) == sizeof(uint2), "tile reference layout");
+        ND_CUDA_P(cudaMemcpyAsync(p->tile_ref, swaths.tile_ref.data(), sizeof(NdSwathTileRef) * swaths.tile_ref.size(), cudaMemcpyHostToDevice, st));
         ND_CUDA_P(cudaMemcpyAsync(p->swath_tile0, swaths.swath_tile0.data(), sizeof(int64_t) * swaths.swath_tile0.size(), cudaMemcpyHostToDevice, st));
         ND_CUDA_P(cudaMemcpyAsync(p->swath_track, swaths.swath_track.data(), sizeof(int32_t) * swaths.swath_track.size(), cudaMemcpyHostToDevice, st));
         ND_CUDA_P(cudaMemcpyAsync(p->items, swaths.items.data(), sizeof(NdSwathItem) * swaths.items.size(), cudaMemcpyHostToDevice, st));
-    }
-    if (want_private) {
-        static_assert(sizeof(NdTileItem) == sizeof(int4), "work item layout");
-        p->n_items = (int)tiles.items.size();
-        p->n_tiles = tiles.n_tiles;
-        p->mean_regions_per_tile = tiles.mean_regions_per_tile;
-        p->mean_segments_per_tile = tiles.mean_segments_per_tile;
-        ND_CUDA_P(cudaMemcpyAsync(p->blob, tiles.blob.data(), tiles.blob.size(), cudaMemcpyHostToDevice, st));
-        ND_CUDA_P(cudaMemcpyAsync(p->tile_chunk, tiles.tile_chunk.data(), sizeof(uint32_t) * tiles.tile_chunk.size(), cudaMemcpyHostToDevice, st));
-        ND_CUDA_P(cudaMemcpyAsync(p->swath_tile0, tiles.swath_tile0.data(), sizeof(int64_t) * tiles.swath_tile0.size(), cudaMemcpyHostToDevice, st));
-        ND_CUDA_P(cudaMemcpyAsync(p->swath_track, tiles.swath_track.data(), sizeof(int32_t) * tiles.swath_track.size(), cudaMemcpyHostToDevice, st));
-        ND_CUDA_P(cudaMemcpyAsync(p->items, tiles.items.data(), sizeof(NdTileItem) * tiles.items.size(), cudaMemcpyHostToDevice, st));
     }
     ND_CUDA_P(cudaMemcpyAsync(p->seg_rm, h_rm.data(), sizeof(uint32_t) * h_rm.size(), cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->seg_len, h_len.data(), sizeof(float) * h_len.size(), cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->trk_off, h_off.data(), sizeof(int64_t) * h_off.size(), cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->trk_w, h_w.data(), sizeof(float) * h_w.size(), cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->link_src, link_src.data(), sizeof(int32_t) * link_src.size(), cudaMemcpyHostToDevice, st));
+    ND_CUDA_P(cudaMemcpyAsync(p->exit_vac, h_exit_vac.data(), h_exit_vac.size(), cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->reg_mat, desc->region_material, sizeof(int32_t) * (size_t)d.R, cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->vol, p->h_vol.data(), sizeof(double) * (size_t)d.R, cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->sigt, desc->sigma_t, sizeof(double) * (size_t)d.M * d.G, cudaMemcpyHostToDevice, st));
@@ -929,7 +816,7 @@ extern "C" nd_status nd_source_update(nd_problem* p, const double* d_phi, double
         const int grid = grid_for((int64_t)d.R * d.G, 256, kReduceBlocks);
         ndk::k_fission_partial<<<grid, 256, 0, st>>>(d_phi, p->reg_mat, p->nusf, p->vol, p->partial, d.R, d.G);
         ND_LAUNCH_CHECK(p);
-        ndk::k_reduce_final<<<1, 256, 0, st>>>(p->partial, grid, p->scalars + 4, 0, nullptr); // writes scalars[4+SC_F]
+        ndk::k_reduce_final<<<1, 256, 0, st>>>(p->partial, grid, p->scalars + 4, 0, nullptr, nullptr, 0); // writes scalars[4+SC_F]
         ND_LAUNCH_CHECK(p);
         ND_CUDA(cudaMemcpyAsync(d_fission_rate_out, p->scalars + 4 + ndk::SC_F, sizeof(double), cudaMemcpyDeviceToDevice, st));
     }
@@ -955,12 +842,14 @@ extern "C" nd_status nd_power_iteration(nd_problem* p, int32_t max_iters, double
         sp.phi = p->phi_cur;
         nd_status rc = launch_source(p, sp, st);
         if (rc != ND_OK) return rc;
-        rc = launch_sweep(p, p->scalars + ndk::SC_F, st);
+        const bool balance = slot != nullptr && stats != nullptr;   // leakage and the balance residual are only formed for stats
+        rc = launch_sweep(p, p->scalars + ndk::SC_F, st, balance);
         if (rc != ND_OK) return rc;
         int grid = 0;
         rc = launch_finalise(p, p->Q, p->phi_cur, p->scalars + ndk::SC_F, p->phi_new, &grid, st);
         if (rc != ND_OK) return rc;
-        ndk::k_reduce_final<<<1, 256, 0, st>>>(p->partial, grid, p->scalars, 1, slot);
+        const int grid_b = grid_for(2 * (int64_t)d.T * d.P * d.Gs, 256, kReduceBlocks);
+        ndk::k_reduce_final<<<1, 256, 0, st>>>(p->partial, grid, p->scalars, 1, slot, balance ? p->partial_b : nullptr, grid_b);
         ND_LAUNCH_CHECK(p);
         std::swap(p->phi_cur, p->phi_new);
         return ND_OK;
@@ -1001,35 +890,55 @@ extern "C" nd_status nd_power_iteration(nd_problem* p, int32_t max_iters, double
             p->kernels_launched += p->iter_graph_kernels;
         }
     }
+    // Per-iteration records live in a device ring of kMaxStats slots; a full ring (and the last, partial one) is copied to
+    // the caller's array, so any iteration count is recorded.  Without stats the convergence test reads slot 0.
+    constexpr int SS = ndk::kStatsStride;
+    std::vector<double> hs;
+    int flushed = 0;   // records already delivered to `stats`
+    auto deliver = [&](int upto) -> nd_status {   // stream is synchronised on return
+        const int n = upto - flushed;
+        if (n <= 0) return ND_OK;
+        hs.resize((size_t)SS * n);
+        ND_CUDA(cudaMemcpyAsync(hs.data(), p->stats, sizeof(double) * hs.size(), cudaMemcpyDeviceToHost, st));
+        ND_CUDA(cudaStreamSynchronize(st));
+        for (int i = 0; i < n; ++i) {
+            nd_iter_stats& o = stats[flushed + i];
+            o.k_eff = hs[SS * i]; o.fission_rate = hs[SS * i + 1]; o.dk = hs[SS * i + 2]; o.dphi_max = hs[SS * i + 3];
+            o.leakage = hs[SS * i + 4]; o.balance_residual = hs[SS * i + 5];
+        }
+        flushed = upto;
+        return ND_OK;
+    };
     for (; it < max_iters; ++it) {
-        double* slot = (stats && it < kMaxStats) ? p->stats + 4 * (size_t)it : (sync_each ? p->stats : nullptr);
+        double* slot = stats ? p->stats + (size_t)SS * ((it - flushed) % kMaxStats) : (sync_each ? p->stats : nullptr);
         nd_status rc = one_iteration(slot, st);
         if (rc != ND_OK) return rc;
+        bool stop = false;
         if (sync_each) {
             double h[4];
             ND_CUDA(cudaMemcpyAsync(h, slot, sizeof h, cudaMemcpyDeviceToHost, st));
             ND_CUDA(cudaStreamSynchronize(st));
             const bool ok_k = !(tol_k > 0.0) || std::fabs(h[2]) < tol_k;
             const bool ok_p = !(tol_phi > 0.0) || h[3] < tol_phi;
-            if (ok_k && ok_p) { converged = true; ++it; break; }
+            stop = ok_k && ok_p;
         }
+        if (stats && (it + 1 - flushed == kMaxStats || stop)) {
+            rc = deliver(it + 1);
+            if (rc != ND_OK) return rc;
+        }
+        if (stop) { converged = true; ++it; break; }
+    }
+    if (stats) {
+        const nd_status rc = deliver(it);
+        if (rc != ND_OK) return rc;
     }
     double hk[2];
     ND_CUDA(cudaMemcpyAsync(hk, p->scalars, sizeof(double) * 2, cudaMemcpyDeviceToHost, st));
     if (d_phi_out)
         ND_CUDA(cudaMemcpyAsync(d_phi_out, p->phi_cur, sizeof(double) * (size_t)d.R * d.G, cudaMemcpyDeviceToDevice, st));
-    std::vector<double> hs;
-    const int ns = stats ? (it < kMaxStats ? it : kMaxStats) : 0;
-    if (ns > 0) {
-        hs.resize(4 * (size_t)ns);
-        ND_CUDA(cudaMemcpyAsync(hs.data(), p->stats, sizeof(double) * hs.size(), cudaMemcpyDeviceToHost, st));
-    }
     ND_CUDA(cudaStreamSynchronize(st));
     *k_eff_out = hk[ndk::SC_K];
     if (iters_done) *iters_done = it;
-    for (int i = 0; i < ns; ++i) {
-        stats[i].k_eff = hs[4 * i]; stats[i].fission_rate = hs[4 * i + 1]; stats[i].dk = hs[4 * i + 2]; stats[i].dphi_max = hs[4 * i + 3];
-    }
     if (use_tol && !converged) return nd_fail(ND_ERR_NOT_CONVERGED, "nd_power_iteration: max_iters reached before the tolerances");
     return ND_OK;
 }
@@ -1520,11 +1429,8 @@ extern "C" nd_status nd_problem_info_get(const nd_problem* p, nd_problem_info* o
     out->mean_segments_per_tile = p->mean_segments_per_tile;
     out->lockstep_efficiency = p->lockstep_efficiency;
     if (is_swath(p->sweep_kernel)) {
-        out->block_threads = 32 * (p->sc.warps + p->sc.nsw); out->smem_bytes = p->sc.smem_bytes; out->grid_blocks = swath_grid(p);
+        out->block_threads = 32 * p->sc.warps; out->smem_bytes = p->sc.smem_bytes; out->grid_blocks = swath_grid(p);
         out->tracks_per_block = p->sc.sp.NT;
-    } else if (p->sweep_kernel == ND_SWEEP_PRIVATE) {
-        out->block_threads = 32 * p->pc.warps; out->smem_bytes = p->pc.smem_bytes; out->grid_blocks = p->n_sm;
-        out->tracks_per_block = p->pc.tp.B * p->pc.tp.TPW * p->pc.warps;
     } else {
         out->block_threads = 256;
     }

@@ -11,6 +11,7 @@
 namespace ndk {
 
 constexpr int kMaxPolar = 4;
+constexpr int kPartialStride = 4;   // doubles per block in the partial-sum arrays of the reductions
 constexpr double kFourPi = 12.566370614359172953850573533118;
 
 // Segment stream record (SoA): seg_rm[k] = region | material << 24 ; seg_len[k] = FP32 projected length.
@@ -248,8 +249,9 @@ __device__ __forceinline__ double block_max(double v, double* scratch)
 
 // ---- A4 + first stage of A6 ----
 // phi_new[r][g] = 4 pi Q/Sigma_t + (A~_r > 0 ? tally/(Sigma_t A~_r) : 0)
-// partial[3*b+0] = sum over the block's elements of A~_r nuSigma_f phi_new          (fission rate)
-// partial[3*b+1] = max |phi_new - phi_old/F|   partial[3*b+2] = max |phi_new|       (only if phi_old != NULL)
+// partial[4*b+0] = sum over the block's elements of A~_r nuSigma_f phi_new          (fission rate)
+// partial[4*b+1] = max |phi_new - phi_old/F|   partial[4*b+2] = max |phi_new|       (only if phi_old != NULL)
+// partial[4*b+3] = sum of the tally (what the chains of the sweep lost, by the telescoping identity)
 struct FinaliseParams {
     const double* __restrict__ Q;        // [R][G]
     const double* __restrict__ tally;    // [R][Gs]
@@ -260,7 +262,7 @@ struct FinaliseParams {
     const double* __restrict__ phi_old;  // [R][G] or NULL
     const double* __restrict__ f_ptr;    // scalar F for phi_old normalisation (or NULL)
     double* __restrict__ phi_new;        // [R][G]
-    double* __restrict__ partial;        // [gridDim.x][3]
+    double* __restrict__ partial;        // [gridDim.x][kPartialStride]
     int64_t R;
     int G, Gs;
 };
@@ -270,15 +272,17 @@ __global__ void __launch_bounds__(256) k_finalise(const FinaliseParams prm)
     __shared__ double scratch[32];
     const int64_t n = prm.R * prm.G;
     const double inv_f = (prm.phi_old && prm.f_ptr) ? 1.0 / *prm.f_ptr : 1.0;
-    double fsum = 0.0, dmax = 0.0, pmax = 0.0;
+    double fsum = 0.0, dmax = 0.0, pmax = 0.0, tsum = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         const int64_t r = i / prm.G;
         const int g = (int)(i - r * prm.G);
         const int m = prm.reg_mat[r];
         const double st = prm.sigt[(size_t)m * prm.G + g];
         const double a = prm.vol[r];
+        const double tl = prm.tally[r * prm.Gs + g];
+        tsum += tl;
         double phi = kFourPi * prm.Q[i] / st;
-        if (a > 0.0) phi += prm.tally[r * prm.Gs + g] / (st * a);
+        if (a > 0.0) phi += tl / (st * a);
         prm.phi_new[i] = phi;
         fsum += a * prm.nusf[(size_t)m * prm.G + g] * phi;
         if (prm.phi_old) {
@@ -289,14 +293,53 @@ __global__ void __launch_bounds__(256) k_finalise(const FinaliseParams prm)
     fsum = block_sum(fsum, scratch);
     dmax = block_max(dmax, scratch);
     pmax = block_max(pmax, scratch);
+    tsum = block_sum(tsum, scratch);
     if (threadIdx.x == 0) {
-        prm.partial[3 * blockIdx.x + 0] = fsum;
-        prm.partial[3 * blockIdx.x + 1] = dmax;
-        prm.partial[3 * blockIdx.x + 2] = pmax;
+        prm.partial[kPartialStride * blockIdx.x + 0] = fsum;
+        prm.partial[kPartialStride * blockIdx.x + 1] = dmax;
+        prm.partial[kPartialStride * blockIdx.x + 2] = pmax;
+        prm.partial[kPartialStride * blockIdx.x + 3] = tsum;
     }
 }
 
-// fission rate of an arbitrary phi: partial[3*b] = sum A~ nuSigma_f phi
+// ---- A6, boundary side of the balance: over every chain e = 2t+d of ONE sweep (run between the sweep and the link swap)
+//   partial[4*b+0] = sum w_{t,p} psi_in / F      what entered through the track ends (0 at vacuum ends)
+//   partial[4*b+1] = sum w_{t,p} psi_out         what left through them
+//   partial[4*b+2] = the part of [1] that left through VACUUM ends: the leakage
+__global__ void __launch_bounds__(256) k_boundary_balance(const float* __restrict__ psi_in, const float* __restrict__ psi_out,
+                                                          const float* __restrict__ trk_w, const uint8_t* __restrict__ exit_vacuum,
+                                                          const double* __restrict__ scale_div, double* __restrict__ partial,
+                                                          int64_t n_entries, int P, int G, int Gs, float wp0, float wp1, float wp2,
+                                                          float wp3)
+{
+    __shared__ double scratch[32];
+    const float wp[kMaxPolar] = {wp0, wp1, wp2, wp3};
+    const int PG = P * Gs;
+    const int64_t n = n_entries * PG;
+    const double inv_f = 1.0 / *scale_div;
+    double s_in = 0.0, s_out = 0.0, s_leak = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t e = i / PG;
+        const int j = (int)(i - e * PG), p = j / Gs, g = j - p * Gs;
+        if (g >= G) continue;
+        const double w = (double)trk_w[e >> 1] * (double)wp[p];
+        const double o = w * (double)psi_out[i];
+        s_in += w * (double)psi_in[i] * inv_f;
+        s_out += o;
+        if (exit_vacuum[e]) s_leak += o;
+    }
+    s_in = block_sum(s_in, scratch);
+    s_out = block_sum(s_out, scratch);
+    s_leak = block_sum(s_leak, scratch);
+    if (threadIdx.x == 0) {
+        partial[kPartialStride * blockIdx.x + 0] = s_in;
+        partial[kPartialStride * blockIdx.x + 1] = s_out;
+        partial[kPartialStride * blockIdx.x + 2] = s_leak;
+        partial[kPartialStride * blockIdx.x + 3] = 0.0;
+    }
+}
+
+// fission rate of an arbitrary phi: partial[4*b] = sum A~ nuSigma_f phi
 __global__ void __launch_bounds__(256) k_fission_partial(const double* __restrict__ phi, const int32_t* __restrict__ reg_mat,
                                                          const double* __restrict__ nusf, const double* __restrict__ vol,
                                                          double* __restrict__ partial, int64_t R, int G)
@@ -310,27 +353,45 @@ __global__ void __launch_bounds__(256) k_fission_partial(const double* __restric
         fsum += vol[r] * nusf[(size_t)reg_mat[r] * G + g] * phi[i];
     }
     fsum = block_sum(fsum, scratch);
-    if (threadIdx.x == 0) { partial[3 * blockIdx.x] = fsum; partial[3 * blockIdx.x + 1] = 0.0; partial[3 * blockIdx.x + 2] = 0.0; }
+    if (threadIdx.x == 0) {
+        partial[kPartialStride * blockIdx.x] = fsum;
+        partial[kPartialStride * blockIdx.x + 1] = partial[kPartialStride * blockIdx.x + 2] = partial[kPartialStride * blockIdx.x + 3] = 0.0;
+    }
 }
 
 // ---- A6 second stage (one block): scalars[] layout below.  mode 0: F <- sum (no k update).
 //      mode 1 (power iteration): F_new = sum; k_prev = k; k <- k*F_new; F <- F_new; dphi = max/max ----
 enum { SC_K = 0, SC_F = 1, SC_KPREV = 2, SC_DPHI = 3, SC_ONE = 4, SC_COUNT = 8 };
 
+constexpr int kStatsStride = 6;   // doubles per iteration record: k, F, dk, dphi, leakage, balance residual
+
 __global__ void __launch_bounds__(256) k_reduce_final(const double* __restrict__ partial, int n_partial,
                                                       double* __restrict__ scalars, int mode,
-                                                      double* __restrict__ stats_slot /* 4 doubles or NULL */)
+                                                      double* __restrict__ stats_slot /* kStatsStride doubles or NULL */,
+                                                      const double* __restrict__ partial_b /* k_boundary_balance's, or NULL */,
+                                                      int n_partial_b)
 {
     __shared__ double scratch[32];
-    double fsum = 0.0, dmax = 0.0, pmax = 0.0;
+    double fsum = 0.0, dmax = 0.0, pmax = 0.0, tsum = 0.0, s_in = 0.0, s_out = 0.0, s_leak = 0.0;
     for (int i = threadIdx.x; i < n_partial; i += blockDim.x) {
-        fsum += partial[3 * i];
-        dmax = fmax(dmax, partial[3 * i + 1]);
-        pmax = fmax(pmax, partial[3 * i + 2]);
+        fsum += partial[kPartialStride * i];
+        dmax = fmax(dmax, partial[kPartialStride * i + 1]);
+        pmax = fmax(pmax, partial[kPartialStride * i + 2]);
+        tsum += partial[kPartialStride * i + 3];
     }
+    if (partial_b)
+        for (int i = threadIdx.x; i < n_partial_b; i += blockDim.x) {
+            s_in += partial_b[kPartialStride * i];
+            s_out += partial_b[kPartialStride * i + 1];
+            s_leak += partial_b[kPartialStride * i + 2];
+        }
     fsum = block_sum(fsum, scratch);
     dmax = block_max(dmax, scratch);
     pmax = block_max(pmax, scratch);
+    tsum = block_sum(tsum, scratch);
+    s_in = block_sum(s_in, scratch);
+    s_out = block_sum(s_out, scratch);
+    s_leak = block_sum(s_leak, scratch);
     if (threadIdx.x == 0) {
         if (mode == 1) {
             const double k_prev = scalars[SC_K];
@@ -340,6 +401,10 @@ __global__ void __launch_bounds__(256) k_reduce_final(const double* __restrict__
             scalars[SC_DPHI] = pmax > 0.0 ? dmax / pmax : 0.0;
             if (stats_slot) {
                 stats_slot[0] = k_new; stats_slot[1] = fsum; stats_slot[2] = k_new - k_prev; stats_slot[3] = scalars[SC_DPHI];
+                // telescoping identity of the sweep: sum of the tallies = what entered - what left through the track ends
+                const double den = fabs(s_in) + fabs(s_out);
+                stats_slot[4] = partial_b ? s_leak : 0.0;
+                stats_slot[5] = partial_b && den > 0.0 ? (s_in - s_out - tsum) / den : 0.0;
             }
         }
         scalars[SC_F] = fsum;

@@ -18,8 +18,11 @@ namespace {
 struct SwathBuild {
     std::vector<uint8_t> bytes;        // this swath's chunks, concatenated
     std::vector<uint32_t> chunk_rel;   // chunk offsets relative to the swath's first byte, 16-B units
+    std::vector<uint32_t> head16;      // head size of every chunk, 16-B units
     int64_t n_seg = 0, sum_regions = 0, sum_max_cnt = 0, n_active = 0;
-    int max_chunk = 0;
+    int max_head = 0, max_rec = 0;
+    int32_t group = 0;                 // angle id of the swath's tracks
+    double perp = 0.0;                 // perpendicular coordinate of its first track
 };
 
 } // namespace
@@ -30,20 +33,21 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
     const int T = desc->n_tracks, R = desc->n_regions, NT = prm.NT, Kmax = prm.Kmax, Lmax = prm.Lmax, NC = prm.NC;
     if (NT < 1 || NT > 1024 || Kmax < 1 || Lmax < 1 || NC < 1 || NT % NC != 0 || prm.row_bytes < 16 || prm.row_bytes % 16 != 0)
         return nd_fail(ND_ERR_INVALID, "swath parameters out of range");
-    const int64_t line = (int64_t)NC * prm.row_bytes;   // bytes between consecutive sigma_t / delta rows in shared memory
+    const int64_t line = (int64_t)NC * prm.row_bytes;   // bytes between consecutive sigma_t rows in shared memory
     const int NCq = prm.NCq > 0 ? prm.NCq : NC;
     const int64_t line_q = (int64_t)NCq * prm.row_bytes; // bytes between consecutive q rows
-    if ((int64_t)Lmax * line > 65536 || (int64_t)desc->n_materials * line > 65536 || (int64_t)NT * Kmax > 65535)
-        return nd_fail(ND_ERR_INVALID, "swath parameters: row offsets must fit 16 bits");
+    const int64_t row_bytes = prm.row_bytes;             // bytes between consecutive delta rows
+    if (Lmax > 65535 || (int64_t)NT * Kmax > 65535 || nd_swath_head_capacity(prm) / 16 > 65535 ||
+        (int64_t)Lmax * line_q > (1ll << 30) || (int64_t)desc->n_materials * line > (1ll << 30))
+        return nd_fail(ND_ERR_INVALID, "swath parameters: tile sizes must fit 16 bits");
     try {
         out->prm = prm;
         // ---- 1. order tracks: by angle id, then by perpendicular coordinate ----
         std::vector<int32_t> order(T);
         std::iota(order.begin(), order.end(), 0);
-        std::vector<double> lam0(T, 0.0);
+        std::vector<double> lam0(T, 0.0), perp(T, 0.0);
         std::vector<int32_t> group(T, 0);
         if (track_azim && track_ends) {
-            std::vector<double> perp(T, 0.0);
             int32_t gmax = 0;
             for (int t = 0; t < T; ++t) { group[t] = track_azim[t] < 0 ? 0 : track_azim[t]; gmax = std::max(gmax, group[t]); }
             std::vector<double> ux((size_t)gmax + 1, 0.0), uy((size_t)gmax + 1, 0.0);
@@ -113,6 +117,7 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
             for (int64_t sw = 0; sw < n_sw; ++sw) {
                 SwathBuild& sb = built[(size_t)sw];
                 const int32_t* trk = &st[(size_t)sw * NT];
+                if (trk[0] >= 0) { sb.group = group[trk[0]]; sb.perp = perp[trk[0]]; }
                 int64_t remaining = 0;
                 for (int b = 0; b < NT; ++b) {
                     if (trk[b] >= 0) { cur[b] = off[trk[b]]; endk[b] = off[trk[b] + 1]; lam[b] = lam0[trk[b]]; ++sb.n_active; }
@@ -178,20 +183,19 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
                     const int o_ss = 16;
                     const int o_rg = o_ss + nd_swath_pad16(2 * (NT + 1));
                     const int o_co = o_rg + nd_swath_pad16(4 * L);
-                    const int o_ci = o_co + nd_swath_pad16(2 * (L + 1));
-                    const int o_rc = o_ci + nd_swath_pad16(2 * nseg);
-                    const int bytes = o_rc + nd_swath_pad16(8 * nseg);
+                    const int o_rc = o_co + nd_swath_pad16(2 * (L + 1));   // = head bytes
+                    const int bytes = o_rc + 16 * nseg;
                     const size_t base = sb.bytes.size();
                     sb.chunk_rel.push_back((uint32_t)(base / 16));
+                    sb.head16.push_back((uint32_t)(o_rc / 16));
                     sb.bytes.resize(base + (size_t)bytes, 0);
                     uint8_t* c = sb.bytes.data() + base;
                     const uint32_t hdr[4] = {(uint32_t)L | ((uint32_t)nseg << 16), (uint32_t)(o_rg / 16) | ((uint32_t)(o_co / 16) << 16),
-                                             (uint32_t)(o_ci / 16) | ((uint32_t)(o_rc / 16) << 16), (uint32_t)bytes};
+                                             (uint32_t)o_rc, (uint32_t)bytes};
                     memcpy(c, hdr, 16);
                     uint16_t* ss = reinterpret_cast<uint16_t*>(c + o_ss);
                     uint32_t* rg = reinterpret_cast<uint32_t*>(c + o_rg);
                     uint16_t* co = reinterpret_cast<uint16_t*>(c + o_co);
-                    uint16_t* ci = reinterpret_cast<uint16_t*>(c + o_ci);
                     uint32_t* rc = reinterpret_cast<uint32_t*>(c + o_rc);
                     for (int l = 0; l < L; ++l) rg[l] = regions[l];
                     co[0] = 0;
@@ -208,15 +212,17 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
                             const float len = (float)desc->seg_length[k];
                             uint32_t lenbits;
                             memcpy(&lenbits, &len, 4);
-                            rc[2 * o] = lenbits;
-                            rc[2 * o + 1] = (uint32_t)(l * line_q) | ((uint32_t)(desc->region_material[r] * line) << 16);
-                            ci[rfill[l]++] = (uint16_t)(((b / NC) * Kmax + j) * NC + b % NC);
+                            rc[4 * o] = lenbits;
+                            rc[4 * o + 1] = (uint32_t)(l * line_q);
+                            rc[4 * o + 2] = (uint32_t)(desc->region_material[r] * line);
+                            rc[4 * o + 3] = (uint32_t)(rfill[l]++ * row_bytes);   // region-major delta row: by slot, then along the track
                         }
                     }
                     ss[NT] = (uint16_t)o;
                     sb.sum_regions += L;
                     sb.sum_max_cnt += max_cnt;
-                    sb.max_chunk = std::max(sb.max_chunk, bytes);
+                    sb.max_head = std::max(sb.max_head, o_rc);
+                    sb.max_rec = std::max(sb.max_rec, 16 * nseg);
                 }
             }
         }
@@ -229,13 +235,14 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
         }
         out->n_tiles = out->swath_tile0[n_sw];
         if (byte0[n_sw] / 16 >= 0xffffffffull) return nd_fail(ND_ERR_RANGE, "swath stream exceeds 64 GiB");
-        out->tile_chunk.resize((size_t)out->n_tiles + 1);
-        out->tile_chunk[(size_t)out->n_tiles] = (uint32_t)(byte0[n_sw] / 16);   // end sentinel: chunk k spans [k, k+1)
+        out->tile_ref.resize((size_t)out->n_tiles + 1);
+        out->tile_ref[(size_t)out->n_tiles] = {(uint32_t)(byte0[n_sw] / 16), 0u};   // end sentinel: chunk k spans [k, k+1)
         out->blob.resize_uninitialised(byte0[n_sw]);   // first touched by the parallel copies below
         int64_t sum_regions = 0, sum_seg = 0, sum_slots = 0;
-        int max_chunk = 0;
+        int max_head = 0, max_rec = 0;
         for (int64_t sw = 0; sw < n_sw; ++sw) {
-            sum_regions += built[sw].sum_regions; sum_seg += built[sw].n_seg; max_chunk = std::max(max_chunk, built[sw].max_chunk);
+            sum_regions += built[sw].sum_regions; sum_seg += built[sw].n_seg;
+            max_head = std::max(max_head, built[sw].max_head); max_rec = std::max(max_rec, built[sw].max_rec);
             sum_slots += built[sw].sum_max_cnt * built[sw].n_active;
         }
 #pragma omp parallel for schedule(dynamic, 64) num_threads(nth)
@@ -243,21 +250,38 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
             SwathBuild& sb = built[(size_t)sw];
             if (!sb.bytes.empty()) memcpy(out->blob.data() + byte0[sw], sb.bytes.data(), sb.bytes.size());
             const uint32_t b16 = (uint32_t)(byte0[sw] / 16);
-            for (size_t i = 0; i < sb.chunk_rel.size(); ++i) out->tile_chunk[(size_t)out->swath_tile0[sw] + i] = b16 + sb.chunk_rel[i];
+            for (size_t i = 0; i < sb.chunk_rel.size(); ++i)
+                out->tile_ref[(size_t)out->swath_tile0[sw] + i] = {b16 + sb.chunk_rel[i], sb.head16[i]};
             std::vector<uint8_t>().swap(sb.bytes);
         }
-        out->max_chunk_bytes = max_chunk;
+        out->max_head_bytes = max_head;
+        out->max_rec_bytes = max_rec;
         out->mean_regions_per_tile = out->n_tiles ? (double)sum_regions / (double)out->n_tiles : 0.0;
         out->mean_segments_per_tile = out->n_tiles ? (double)sum_seg / (double)out->n_tiles : 0.0;
         out->lockstep_efficiency = sum_slots ? (double)sum_seg / (double)sum_slots : 1.0;
-        // ---- 5. work items: (swath, direction), most expensive first ----
+        // ---- 5. work items (swath, direction) ----
         out->items.clear();
-        for (int64_t sw = 0; sw < n_sw; ++sw) {
-            const int32_t c32 = (int32_t)std::min<int64_t>(built[sw].sum_max_cnt, INT32_MAX);
-            out->items.push_back({(int32_t)sw, 0, c32, 0});
-            out->items.push_back({(int32_t)sw, 1, c32, 0});
+        if (prm.item_order == 0) {   // most expensive first
+            for (int64_t sw = 0; sw < n_sw; ++sw) {
+                const int32_t c32 = (int32_t)std::min<int64_t>(built[sw].sum_max_cnt, INT32_MAX);
+                out->items.push_back({(int32_t)sw, 0, c32, 0});
+                out->items.push_back({(int32_t)sw, 1, c32, 0});
+            }
+            std::stable_sort(out->items.begin(), out->items.end(), [](const NdSwathItem& a, const NdSwathItem& b) { return a.cost > b.cost; });
+        } else {
+            // Angle by angle; inside an angle all forward items in the order of the perpendicular coordinate, then all
+            // backward items: thread blocks that run at the same time carry neighbouring swaths at the same stage of their
+            // tracks, so the q and tally rows of the triangles two swaths share are still in L2 for the second one.  Swaths
+            // are already stored in (angle, perpendicular) order; the last items of the last angle are short corner swaths.
+            for (int64_t a = 0; a < n_sw;) {
+                int64_t b = a;
+                while (b < n_sw && built[b].group == built[a].group) ++b;
+                for (int dir = 0; dir < 2; ++dir)
+                    for (int64_t sw = a; sw < b; ++sw)
+                        out->items.push_back({(int32_t)sw, dir, (int32_t)std::min<int64_t>(built[sw].sum_max_cnt, INT32_MAX), 0});
+                a = b;
+            }
         }
-        std::stable_sort(out->items.begin(), out->items.end(), [](const NdSwathItem& a, const NdSwathItem& b) { return a.cost > b.cost; });
     } catch (const std::bad_alloc&) {
         return nd_fail(ND_ERR_NOMEM, "nd_build_swaths: out of host memory");
     }
@@ -273,7 +297,7 @@ struct nd_swath_stream {
 
 extern "C" nd_status nd_swath_stream_build(const nd_problem_desc* desc, int32_t tracks_per_swath, int32_t tile_segments,
                                            int32_t window_regions, int32_t slots_per_line, int32_t row_bytes,
-                                           double lag_segments, nd_swath_stream** out)
+                                           double lag_segments, int32_t item_order, nd_swath_stream** out)
 {
     if (!desc || !out) return nd_fail(ND_ERR_NULL, "nd_swath_stream_build: NULL argument");
     if (!desc->track_seg_offset || !desc->seg_region || !desc->seg_length || !desc->region_material)
@@ -283,6 +307,7 @@ extern "C" nd_status nd_swath_stream_build(const nd_problem_desc* desc, int32_t 
     nd_swath_stream* s = new (std::nothrow) nd_swath_stream();
     if (!s) return nd_fail(ND_ERR_NOMEM, "nd_swath_stream_build: out of host memory");
     NdSwathParams prm{tracks_per_swath, tile_segments, window_regions, slots_per_line, row_bytes, lag_segments};
+    prm.item_order = item_order;
     const nd_status rc = nd_build_swaths(desc, desc->track_azim, desc->track_ends, prm, 0, &s->set);
     if (rc != ND_OK) { delete s; return rc; }
     *out = s;
@@ -295,10 +320,11 @@ extern "C" nd_status nd_swath_stream_view(const nd_swath_stream* s, nd_swath_str
     const NdSwathSet& t = s->set;
     v->n_swaths = t.n_swaths; v->n_tiles = t.n_tiles; v->blob_bytes = (int64_t)t.blob.size();
     v->n_items = (int64_t)t.items.size();
-    v->blob = t.blob.data(); v->tile_chunk = t.tile_chunk.data(); v->swath_tile0 = t.swath_tile0.data();
+    static_assert(sizeof(NdSwathTileRef) == 8, "tile reference layout");
+    v->blob = t.blob.data(); v->tile_ref = reinterpret_cast<const uint32_t*>(t.tile_ref.data()); v->swath_tile0 = t.swath_tile0.data();
     v->swath_track = t.swath_track.data(); v->items = reinterpret_cast<const int32_t*>(t.items.data());
     v->mean_regions_per_tile = t.mean_regions_per_tile; v->mean_segments_per_tile = t.mean_segments_per_tile;
-    v->lockstep_efficiency = t.lockstep_efficiency; v->max_chunk_bytes = t.max_chunk_bytes; v->reserved = 0;
+    v->lockstep_efficiency = t.lockstep_efficiency; v->max_head_bytes = t.max_head_bytes; v->max_rec_bytes = t.max_rec_bytes;
     return ND_OK;
 }
 

@@ -6,17 +6,19 @@
 // tracks advance either by equal counts (every track Kmax segments) or, when their fronts have drifted apart, in
 // geometric lock step (always the track whose front is furthest behind) until one of them has Kmax segments in the
 // tile; in both modes a tile touches at most Lmax distinct regions.  A tile is one contiguous, 16-byte aligned
-// CHUNK, fetched by a single bulk (TMA) copy:
-//     u32 hdr[4]          L | nseg << 16 ;  off_regions | off_csr_off << 16 ;  off_csr_idx | off_rec << 16 ;  bytes
-//                         (offsets in 16-byte units from the chunk start)
-//     u16 slot_start[NT+1]   per-track prefix into rec[]                                     (padded to 16 B)
-//     u32 regions[L]         global region ids: q rows to stage, tally rows to flush          (padded to 16 B)
-//     u16 csr_off[L+1]       per region: range into csr_idx                                   (padded to 16 B)
-//     u16 csr_idx[nseg]      delta-buffer row of every segment, grouped by region             (padded to 16 B)
-//     rec[nseg]              { f32 length ; u32 q_row_byte_offset | sigt_row_byte_offset << 16 }, slot-major,
-//                            forward order; the backward direction walks the same records in reverse
-// A segment's weighted flux change is simply STORED in its own delta-buffer row, and csr_idx tells the flush which rows
-// to add up per region (a track may re-enter a region; every visit has its own row).
+// CHUNK made of a HEAD and a RECORD part, each fetched by one bulk (TMA) copy into its own shared-memory ring:
+//   head  u32 hdr[4]          L | nseg << 16 ;  off_regions | off_csr << 16 (16-byte units from the chunk start) ;
+//                             head bytes ;  chunk bytes
+//         u16 slot_start[NT+1] per-track prefix into rec[]                                     (padded to 16 B)
+//         u32 regions[L]       global region ids: q rows to stage, tally rows to flush          (padded to 16 B)
+//         u16 csr[L+1]         per region: its range of delta-buffer rows                        (padded to 16 B)
+//   rec   rec[nseg]            16 bytes each: { f32 length ; u32 q-row byte offset ; u32 Sigma_t-row byte offset ;
+//                              u32 delta-row byte offset }, slot-major, forward order; the backward direction walks
+//                              the same records in reverse
+// Delta rows are REGION-MAJOR: the rows of region l are csr[l] .. csr[l+1]-1, ordered by slot then by position along
+// the track, so the flush adds up a contiguous run of rows per region (no index list) and adjacent tracks crossing
+// the same region store into adjacent rows.  A segment's weighted flux change is simply STORED in its own row (a
+// track may re-enter a region; every visit has its own row).
 #ifndef ND_SWATH_H
 #define ND_SWATH_H
 #include <cstddef>
@@ -30,19 +32,22 @@ struct NdSwathParams {
     int NT;       // tracks per swath = slots per thread block
     int Kmax;     // max segments of one track in a tile
     int Lmax;     // max distinct regions in a tile
-    int NC;       // slots interleaved in one delta-buffer / q line (bank-conflict-free layout for narrow rows)
+    int NC;       // slots whose Sigma_t rows share one shared-memory line (bank-conflict-free layout for narrow rows)
     int row_bytes;// bytes of one (region, all groups) FP32 row = 4 * Gs
     double lag;   // >= 0: while the fronts of the swath's tracks lie within `lag` mean segment lengths of each other a
                   // tile gives EVERY track Kmax segments (no idle slot steps); beyond it the tile is cut geometrically
                   // (the track furthest behind advances first) until the fronts are level again.  < 0: always geometric.
     int NCq = 0;  // copies of a q row per shared line (0: = NC).  1 = one copy per region: adjacent slots in the same region
                   // read it as a broadcast, slots in different regions may meet in a bank
+    int item_order = 0;   // 0: work items most expensive first (load balance); 1: angle by angle, adjacent swaths
+                          // consecutively, forward then backward (blocks that run together touch neighbouring regions)
 };
 
 struct NdSwathItem { int32_t swath, dir, cost, reserved; };
+struct NdSwathTileRef { uint32_t off16, head16; };   // chunk offset and head size, both in 16-byte units
 
-// Byte buffer that is NOT value-initialised: the 4-5 GB chunk stream of a 5e8-segment problem is written exactly once by
-// parallel copies; zero-filling it first (std::vector::resize) cost 2 s of single-threaded page faults.
+// Byte buffer that is NOT value-initialised: the chunk stream of a 5e8-segment problem (8-9 GB) is written exactly once by
+// parallel copies; zero-filling it first (std::vector::resize) cost seconds of single-threaded page faults.
 struct NdRawBytes {
     std::unique_ptr<uint8_t[]> p;
     size_t n = 0;
@@ -56,23 +61,22 @@ struct NdSwathSet {
     NdSwathParams prm{};
     int64_t n_swaths = 0, n_tiles = 0;
     std::vector<int32_t> swath_track;     // [n_swaths][NT] canonical track id or -1
-    std::vector<int64_t> swath_tile0;     // [n_swaths+1] prefix into tile_chunk
-    std::vector<uint32_t> tile_chunk;     // [n_tiles+1] chunk offsets in 16-byte units (+ end sentinel)
-    std::vector<NdSwathItem> items;       // work items (swath, direction), most expensive first
+    std::vector<int64_t> swath_tile0;     // [n_swaths+1] prefix into tile_ref
+    std::vector<NdSwathTileRef> tile_ref; // [n_tiles+1] (+ end sentinel: chunk k spans [off16[k], off16[k+1]))
+    std::vector<NdSwathItem> items;       // work items (swath, direction)
     NdRawBytes blob;                      // all chunks (every byte written by nd_build_swaths)
-    int max_chunk_bytes = 0;
+    int max_head_bytes = 0, max_rec_bytes = 0;
     double mean_regions_per_tile = 0.0, mean_segments_per_tile = 0.0, lockstep_efficiency = 0.0;
 };
 
 inline int nd_swath_pad16(int x) { return (x + 15) / 16 * 16; }
 
-// largest chunk the parameters allow (the kernel's staging buffers have this size)
-inline int nd_swath_chunk_capacity(const NdSwathParams& p)
+// largest head / record part the parameters allow (the kernel's staging rings have these sizes)
+inline int nd_swath_head_capacity(const NdSwathParams& p)
 {
-    const int nmax = p.NT * p.Kmax;
-    return 16 + nd_swath_pad16(2 * (p.NT + 1)) + nd_swath_pad16(4 * p.Lmax) + nd_swath_pad16(2 * (p.Lmax + 1)) +
-           nd_swath_pad16(2 * nmax) + nd_swath_pad16(8 * nmax);
+    return 16 + nd_swath_pad16(2 * (p.NT + 1)) + nd_swath_pad16(4 * p.Lmax) + nd_swath_pad16(2 * (p.Lmax + 1));
 }
+inline int nd_swath_rec_capacity(const NdSwathParams& p) { return 16 * p.NT * p.Kmax; }
 
 // upper bounds used to size the device workspace before the stream is built
 inline int64_t nd_swath_max_tiles(const NdSwathParams& p, int64_t n_segments, int64_t n_tracks)
@@ -82,8 +86,9 @@ inline int64_t nd_swath_max_tiles(const NdSwathParams& p, int64_t n_segments, in
 }
 inline size_t nd_swath_max_blob(const NdSwathParams& p, int64_t n_segments, int64_t n_tracks)
 {
-    const size_t per_tile = 16 + (size_t)nd_swath_pad16(2 * (p.NT + 1)) + 4 * 16;
-    return (size_t)nd_swath_max_tiles(p, n_segments, n_tracks) * per_tile + 16 * (size_t)n_segments + 256;
+    // head: 16 + slot prefix + (4 + 2) bytes per region (<= one region per segment) + three paddings
+    const size_t per_tile = 16 + (size_t)nd_swath_pad16(2 * (p.NT + 1)) + 3 * 16;
+    return (size_t)nd_swath_max_tiles(p, n_segments, n_tracks) * per_tile + 22 * (size_t)n_segments + 256;
 }
 
 // track_azim / track_ends may be NULL (no geometry): tracks are then grouped in descriptor order.

@@ -31,7 +31,7 @@ namespace ndk {
 
 struct SwathParams {
     const uint8_t* __restrict__ blob;
-    const uint32_t* __restrict__ tile_chunk;   // [n_tiles+1] chunk offsets in 16-byte units (+ end sentinel)
+    const uint2* __restrict__ tile_ref;        // [n_tiles+1] (chunk offset, head size) in 16-byte units (+ end sentinel)
     const int64_t* __restrict__ swath_tile0;   // [n_swaths+1]
     const int32_t* __restrict__ swath_track;   // [n_swaths][NT]
     const int4* __restrict__ items;            // (swath, dir, cost, -)
@@ -44,10 +44,11 @@ struct SwathParams {
     float* __restrict__ psi_out;
     const double* __restrict__ scale_div;
     int n_items, G, Gs, M, NT, Kmax, Lmax, LPT, NC, NCq, ndbuf;
-    int chunk_cap;                             // bytes of one chunk staging buffer
-    int off_sigt, off_q, off_dbuf, off_chunk;  // shared-memory byte offsets
+    int head_cap, rec_cap;                     // bytes of one head / record staging buffer
+    int off_sigt, off_q, off_dbuf, off_head, off_rec;  // shared-memory byte offsets
     float c[kMaxPolar], inv_sin[kMaxPolar], wp[kMaxPolar];
-    unsigned long long c2[kMaxPolar];          // {c[p], c[p]} packed for the FP32x2 path
+    unsigned long long c2[kMaxPolar];          // {c[p]/c[0], c[p]/c[0]} packed for the FP32x2 path (the Sigma_t table in shared
+                                               // memory is pre-multiplied by c[0] = -log2(e)/sin(theta_0) there)
     uint32_t magic_per_row, magic_nq;          // fastdiv constants of NC*Gs/4 and Gs/4
     unsigned long long* phase;                 // PROF builds: [kSwathPhases] warp-cycle sums (lane 0 of every warp)
 };
@@ -55,7 +56,8 @@ struct SwathParams {
 // phases of the instrumented build (nd_profile_enable(p, 2)): where the warps' cycles go
 enum { PH_STAGE = 0, PH_WAIT_A, PH_COMPUTE, PH_WAIT_B, PH_FLUSH, PH_ITEM, kSwathPhases };
 
-constexpr int kSwathChunkBufs = 3;
+constexpr int kSwathHeadBufs = 3;   // heads of tiles k, k+1 (its q rows are staged during tile k) and k+2 (in flight)
+constexpr int kSwathRecBufs = 2;    // records of tiles k and k+1 (in flight)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -93,24 +95,20 @@ __device__ __forceinline__ void cp_async_16(uint32_t smem_dst, const void* gmem_
 __device__ __forceinline__ void cp_async_commit_group() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-struct SwathChunk {   // decoded chunk header (pointers into the staging buffer)
+struct SwathHead {   // decoded chunk head (pointers into the head staging buffer)
     int L, nseg;
     const uint16_t* slot_start;
     const uint32_t* regions;
-    const uint16_t* csr_off;
-    const uint16_t* csr_idx;
-    const uint2* rec;
+    const uint16_t* csr;
 };
-__device__ __forceinline__ SwathChunk decode_chunk(const unsigned char* cb)
+__device__ __forceinline__ SwathHead decode_head(const unsigned char* hb)
 {
-    const uint4 h = *reinterpret_cast<const uint4*>(cb);
-    SwathChunk c;
+    const uint4 h = *reinterpret_cast<const uint4*>(hb);
+    SwathHead c;
     c.L = (int)(h.x & 0xffffu); c.nseg = (int)(h.x >> 16);
-    c.slot_start = reinterpret_cast<const uint16_t*>(cb + 16);
-    c.regions = reinterpret_cast<const uint32_t*>(cb + 16 * (h.y & 0xffffu));
-    c.csr_off = reinterpret_cast<const uint16_t*>(cb + 16 * (h.y >> 16));
-    c.csr_idx = reinterpret_cast<const uint16_t*>(cb + 16 * (h.z & 0xffffu));
-    c.rec = reinterpret_cast<const uint2*>(cb + 16 * (h.z >> 16));
+    c.slot_start = reinterpret_cast<const uint16_t*>(hb + 16);
+    c.regions = reinterpret_cast<const uint32_t*>(hb + 16 * (h.y & 0xffffu));
+    c.csr = reinterpret_cast<const uint16_t*>(hb + 16 * (h.y >> 16));
     return c;
 }
 
@@ -126,18 +124,48 @@ __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f
 __host__ __device__ inline uint32_t fastdiv_magic(uint32_t d) { return d <= 1 ? 0u : (uint32_t)((0x100000000ull + d - 1) / d); }
 __device__ __forceinline__ uint32_t fastdiv(uint32_t x, uint32_t m) { return m ? __umulhi(x, m) : x; }
 
-// One track through one tile: cnt segments starting at record rec0 (stepping jstep = +-1), `steps` >= cnt loop trips
-// (slots of a warp run in lock step; trips past cnt are exact no-ops: zero length -> exp = 1 -> Delta = 0).
-// Software pipeline: the record of step i+2 and the q / Sigma_t rows of step i+1 are loaded during step i.
-template <int P, int EXPM>
-__device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&wpt)[P], const SwathParams& prm, const uint2* rec0,
-                                             int jstep, int cnt, int steps, bool store_ok, const unsigned char* q_lane,
-                                             const unsigned char* sigt_lane, unsigned char* d_ptr, int d_step)
+// shared-memory accesses by 32-bit shared-space address (no generic-address conversion in the loop)
+__device__ __forceinline__ uint4 lds_u4(uint32_t a)
 {
-    uint2 r_n = make_uint2(0u, 0u), r_nn = make_uint2(0u, 0u);
-    if (cnt > 0) r_n = rec0[0];
-    if (cnt > 1) r_nn = rec0[jstep];
-    const uint2* rec_pf = rec0 + 2 * jstep;   // record of step i+2
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ ulonglong2 lds_2x64(uint32_t a)
+{
+    ulonglong2 v;
+    asm volatile("ld.shared.v2.u64 {%0,%1}, [%2];" : "=l"(v.x), "=l"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ float4 lds_f4(uint32_t a)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts_2x64(uint32_t a, unsigned long long x, unsigned long long y)
+{
+    asm volatile("st.shared.v2.u64 [%0], {%1,%2};" ::"r"(a), "l"(x), "l"(y) : "memory");
+}
+__device__ __forceinline__ void sts_f4(uint32_t a, float x, float y, float z, float w)
+{
+    asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(a), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
+}
+
+// One track through one tile: cnt segments starting at the record at shared address rec0 (stepping rstep = +-16 bytes),
+// `steps` >= cnt loop trips (slots of a warp run in lock step).  Trips past cnt read the block's NULL RECORD at `null_rec`:
+// zero length (exp = 1, Delta = 0: an exact no-op for psi), row offsets 0, and a delta row that no region owns, so the
+// loop body carries no predicate.  A record holds the byte offsets of its q row, its Sigma_t row and its delta row: one
+// add per access.  Software pipeline: the record of step i+2 and the q / Sigma_t rows of step i+1 are loaded during step i.
+template <int P, int EXPM>
+__device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&wpt)[P], const SwathParams& prm, uint32_t rec0,
+                                             int rstep, int cnt, int steps, uint32_t null_rec, uint32_t q_lane,
+                                             uint32_t sigt_lane, uint32_t d_lane)
+{
+    const uint4 r_n = lds_u4(cnt > 0 ? rec0 : null_rec);
+    uint4 r_nn = lds_u4(cnt > 1 ? rec0 + rstep : null_rec);
+    uint32_t rec_pf = rec0 + 2 * rstep;       // record of step i+2
+    uint32_t d_n = r_n.w;
     if (EXPM == 0) {
         f32x2 ps[P][2], w2[P];
 #pragma unroll
@@ -146,26 +174,27 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
             ps[p][1] = pk2(psi[p][2], psi[p][3]);
             w2[p] = pk2(wpt[p], wpt[p]);
         }
-        ulonglong2 q_n = *reinterpret_cast<const ulonglong2*>(q_lane + (r_n.y & 0xffffu));
-        ulonglong2 st_n = *reinterpret_cast<const ulonglong2*>(sigt_lane + (r_n.y >> 16));
+        ulonglong2 q_n = lds_2x64(q_lane + r_n.y);
+        ulonglong2 st_n = lds_2x64(sigt_lane + r_n.z);
         float s_n = __uint_as_float(r_n.x);
         for (int i = 0; i < steps; ++i) {
             const f32x2 s2 = pk2(s_n, s_n);
             const f32x2 qa[2] = {q_n.x, q_n.y};
-            const f32x2 ts[2] = {mul2(st_n.x, s2), mul2(st_n.y, s2)};
-            const uint2 r_use = r_nn;
-            r_nn = make_uint2(0u, 0u);
-            if (i + 2 < cnt) r_nn = *rec_pf;
-            rec_pf += jstep;
-            q_n = *reinterpret_cast<const ulonglong2*>(q_lane + (r_use.y & 0xffffu));
-            st_n = *reinterpret_cast<const ulonglong2*>(sigt_lane + (r_use.y >> 16));
+            const f32x2 ts[2] = {mul2(st_n.x, s2), mul2(st_n.y, s2)};   // Sigma_t * c_0 * s = log2 of the first polar angle's attenuation
+            const uint32_t d_cur = d_n;
+            const uint4 r_use = r_nn;
+            r_nn = lds_u4(i + 2 < cnt ? rec_pf : null_rec);
+            rec_pf += rstep;
+            q_n = lds_2x64(q_lane + r_use.y);
+            st_n = lds_2x64(sigt_lane + r_use.z);
             s_n = __uint_as_float(r_use.x);
+            d_n = r_use.w;
             f32x2 acc[2];
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
 #pragma unroll
                 for (int p = 0; p < P; ++p) {
-                    const f32x2 tau = mul2(ts[j], prm.c2[p]);
+                    const f32x2 tau = p == 0 ? ts[j] : mul2(ts[j], prm.c2[p]);
                     float t0, t1;
                     upk2(tau, t0, t1);
                     const f32x2 a = pk2(ex2_approx(t0), ex2_approx(t1));
@@ -175,12 +204,7 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
                     acc[j] = p == 0 ? mul2(w2[0], delta) : fma2(w2[p], delta, acc[j]);
                 }
             }
-            if (i < cnt && store_ok) {
-                ulonglong2 o;
-                o.x = acc[0]; o.y = acc[1];
-                *reinterpret_cast<ulonglong2*>(d_ptr) = o;
-            }
-            d_ptr += d_step;
+            sts_2x64(d_lane + d_cur, acc[0], acc[1]);
         }
 #pragma unroll
         for (int p = 0; p < P; ++p) {
@@ -188,19 +212,20 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
             upk2(ps[p][1], psi[p][2], psi[p][3]);
         }
     } else {
-        float4 q_n = *reinterpret_cast<const float4*>(q_lane + (r_n.y & 0xffffu));
-        float4 st_n = *reinterpret_cast<const float4*>(sigt_lane + (r_n.y >> 16));
+        float4 q_n = lds_f4(q_lane + r_n.y);
+        float4 st_n = lds_f4(sigt_lane + r_n.z);
         float s_n = __uint_as_float(r_n.x);
         for (int i = 0; i < steps; ++i) {
             const float sl = s_n;
             const float4 qv = q_n, stv = st_n;
-            const uint2 r_use = r_nn;
-            r_nn = make_uint2(0u, 0u);
-            if (i + 2 < cnt) r_nn = *rec_pf;
-            rec_pf += jstep;
-            q_n = *reinterpret_cast<const float4*>(q_lane + (r_use.y & 0xffffu));
-            st_n = *reinterpret_cast<const float4*>(sigt_lane + (r_use.y >> 16));
+            const uint32_t d_cur = d_n;
+            const uint4 r_use = r_nn;
+            r_nn = lds_u4(i + 2 < cnt ? rec_pf : null_rec);
+            rec_pf += rstep;
+            q_n = lds_f4(q_lane + r_use.y);
+            st_n = lds_f4(sigt_lane + r_use.z);
             s_n = __uint_as_float(r_use.x);
+            d_n = r_use.w;
             const float qa[4] = {qv.x, qv.y, qv.z, qv.w}, sa[4] = {stv.x, stv.y, stv.z, stv.w};
             float a4[4];
 #pragma unroll
@@ -215,8 +240,7 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
                 }
                 a4[j] = acc;
             }
-            if (i < cnt && store_ok) *reinterpret_cast<float4*>(d_ptr) = make_float4(a4[0], a4[1], a4[2], a4[3]);
-            d_ptr += d_step;
+            sts_f4(d_lane + d_cur, a4[0], a4[1], a4[2], a4[3]);
         }
     }
 }
@@ -233,27 +257,36 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
     };
     extern __shared__ __align__(128) unsigned char smem_sw[];
     unsigned char* const smem = smem_sw;
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem);              // [kSwathChunkBufs] chunk-arrival barriers
+    uint64_t* hfull = reinterpret_cast<uint64_t*>(smem);             // [kSwathHeadBufs] head-arrival barriers
+    uint64_t* rfull = hfull + kSwathHeadBufs;                        // [kSwathRecBufs] record-arrival barriers
     volatile int* s_item = reinterpret_cast<volatile int*>(smem + 64);
+    uint32_t* s_null = reinterpret_cast<uint32_t*>(smem + 80);       // the null record: { 0.0f, 0, 0, offset of the spare delta row }
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int Gs = prm.Gs, row_bytes = 4 * Gs, line = prm.NC * row_bytes;
     const int line_q = TIGHT ? line : prm.NCq * row_bytes;   // the capped variant is only used with NCq == NC
     unsigned char* sigt_s = smem + prm.off_sigt;
     unsigned char* q_s = smem + prm.off_q;           // [2][Lmax][line_q]
-    unsigned char* dbuf_s = smem + prm.off_dbuf;     // [ndbuf][NT/NC * Kmax][line]
-    unsigned char* chunk_s = smem + prm.off_chunk;   // [4][chunk_cap]
+    unsigned char* dbuf_s = smem + prm.off_dbuf;     // [ndbuf][NT * Kmax][row_bytes], rows region-major per tile
+    unsigned char* head_s = smem + prm.off_head;     // [kSwathHeadBufs][head_cap]
+    unsigned char* rec_s = smem + prm.off_rec;       // [kSwathRecBufs][rec_cap]
     const int q_buf_bytes = prm.Lmax * line_q;
-    const int dbuf_bytes = (prm.NT / prm.NC) * prm.Kmax * line;
+    const int dbuf_bytes = (prm.NT * prm.Kmax + 1) * row_bytes;   // one spare row behind the tile's rows: the null record's
     const int nq = Gs >> 2;                          // 16-byte pieces per row
 
     if (tid == 0) {
-        for (int i = 0; i < kSwathChunkBufs; ++i) mbar_init(full + i, 1);
+        for (int i = 0; i < kSwathHeadBufs + kSwathRecBufs; ++i) mbar_init(hfull + i, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        s_null[0] = 0u; s_null[1] = 0u; s_null[2] = 0u; s_null[3] = (uint32_t)(prm.NT * prm.Kmax * row_bytes);
     }
-    // Sigma_t table, replicated NC times per line
-    for (int i = tid; i < prm.M * prm.NC * nq; i += nthr) {
-        const int m = i / (prm.NC * nq), rem = i - m * (prm.NC * nq), piece = rem % nq;
-        *reinterpret_cast<float4*>(sigt_s + (size_t)m * line + rem * 16) = *reinterpret_cast<const float4*>(prm.sigt + (size_t)m * Gs + piece * 4);
+    // Sigma_t table, replicated NC times per line; the fast-exp path keeps it pre-multiplied by -log2(e)/sin(theta_0)
+    {
+        const float pre = EXPM == 0 ? prm.c[0] : 1.f;
+        for (int i = tid; i < prm.M * prm.NC * nq; i += nthr) {
+            const int m = i / (prm.NC * nq), rem = i - m * (prm.NC * nq), piece = rem % nq;
+            float4 v = *reinterpret_cast<const float4*>(prm.sigt + (size_t)m * Gs + piece * 4);
+            v.x *= pre; v.y *= pre; v.z *= pre; v.w *= pre;
+            *reinterpret_cast<float4*>(sigt_s + (size_t)m * line + rem * 16) = v;
+        }
     }
     __syncthreads();
 
@@ -265,11 +298,10 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
     int slot = tid / prm.LPT, ll = tid - slot * prm.LPT;
     const bool lane_ok = slot < prm.NT;
     if (!lane_ok) { slot = prm.NT - 1; ll = prm.LPT - 1; }
-    const int sub = slot % prm.NC;                    // position of the slot inside a shared line
-    const int lane_off = sub * row_bytes + ll * 16;   // byte offset of this lane's 4 groups inside a line
-    const unsigned char* sigt_lane = sigt_s + lane_off;
-    const int lane_off_q = TIGHT ? lane_off : (slot % prm.NCq) * row_bytes + ll * 16;
-    const int d_slot_off = (slot / prm.NC) * prm.Kmax * line + lane_off;
+    const int sub = slot % prm.NC;                    // position of the slot inside a Sigma_t line
+    const uint32_t sigt_lane = smem_u32(sigt_s) + sub * row_bytes + ll * 16;
+    const uint32_t null_rec = smem_u32(s_null);
+    const int lane_off_q = TIGHT ? sub * row_bytes + ll * 16 : (slot % prm.NCq) * row_bytes + ll * 16;
     const float inv_f = (float)(1.0 / *prm.scale_div);
     const int g0 = ll * 4;
     // flush mapping: thread -> (region l0 + i*l_step, 16-byte piece qd)
@@ -306,26 +338,36 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
                 wpt[p] = wt * prm.wp[p];
             }
         }
-        // ---- prologue: chunks of the first two tiles in flight, q rows of the first tile ----
+        // ---- prologue: head and records of the first tile and the head of the second in flight, q rows of the first tile ----
         auto tile_index = [&](int k) -> int64_t { return tile0 + (dir ? nt - 1 - k : k); };
-        auto issue_chunk = [&](int k) {   // one thread
+        auto issue_head = [&](int k) {   // one thread
+            const uint2 ref = prm.tile_ref[tile_index(k)];
+            const uint32_t b = (seq + k) % kSwathHeadBufs;
+            mbar_expect_tx(hfull + b, ref.y * 16u);
+            tma_load_1d(head_s + (size_t)b * prm.head_cap, prm.blob + (size_t)ref.x * 16, ref.y * 16u, hfull + b);
+        };
+        auto issue_rec = [&](int k) {    // one thread
             const int64_t ti = tile_index(k);
-            const uint32_t o0 = prm.tile_chunk[ti], o1 = prm.tile_chunk[ti + 1];
-            const uint32_t bytes = (o1 - o0) * 16u;
-            const uint32_t b = (seq + k) % kSwathChunkBufs;
-            mbar_expect_tx(full + b, bytes);
-            tma_load_1d(chunk_s + (size_t)b * prm.chunk_cap, prm.blob + (size_t)o0 * 16, bytes, full + b);
+            const uint2 ref = prm.tile_ref[ti];
+            const uint32_t bytes = (prm.tile_ref[ti + 1].x - ref.x - ref.y) * 16u;
+            const uint32_t b = (seq + k) % kSwathRecBufs;
+            mbar_expect_tx(rfull + b, bytes);
+            tma_load_1d(rec_s + (size_t)b * prm.rec_cap, prm.blob + ((size_t)ref.x + ref.y) * 16, bytes, rfull + b);
         };
-        auto wait_chunk = [&](int k) {
+        auto wait_head = [&](int k) {
             const uint32_t s = seq + k;
-            mbar_wait(full + (s % kSwathChunkBufs), (s / kSwathChunkBufs) & 1u);
+            mbar_wait(hfull + (s % kSwathHeadBufs), (s / kSwathHeadBufs) & 1u);
         };
-        auto issue_q_rows = [&](int k) {   // all threads: regions of tile k -> q buffer (seq+k)&1, NC copies per row
+        auto wait_rec = [&](int k) {
             const uint32_t s = seq + k;
-            const unsigned char* cb = chunk_s + (size_t)(s % kSwathChunkBufs) * prm.chunk_cap;
-            const uint4 h = *reinterpret_cast<const uint4*>(cb);
+            mbar_wait(rfull + (s % kSwathRecBufs), (s / kSwathRecBufs) & 1u);
+        };
+        auto issue_q_rows = [&](int k) {   // all threads: regions of tile k -> q buffer (seq+k)&1, NCq copies per row
+            const uint32_t s = seq + k;
+            const unsigned char* hb = head_s + (size_t)(s % kSwathHeadBufs) * prm.head_cap;
+            const uint4 h = *reinterpret_cast<const uint4*>(hb);
             const int L = (int)(h.x & 0xffffu);
-            const uint32_t* regions = reinterpret_cast<const uint32_t*>(cb + 16 * (h.y & 0xffffu));
+            const uint32_t* regions = reinterpret_cast<const uint32_t*>(hb + 16 * (h.y & 0xffffu));
             const uint32_t qb = smem_u32(q_s + (size_t)(s & 1u) * q_buf_bytes);
             const int per_row = (TIGHT ? prm.NC : prm.NCq) * nq;
             for (int i = tid; i < L * per_row; i += nthr) {
@@ -336,10 +378,11 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
         };
         if (nt > 0) {
             if (tid == 0) {
-                issue_chunk(0);
-                if (nt > 1) issue_chunk(1);
+                issue_head(0);
+                issue_rec(0);
+                if (nt > 1) issue_head(1);
             }
-            wait_chunk(0);
+            wait_head(0);
             issue_q_rows(0);
             cp_async_commit_group();
             cp_async_wait_all();
@@ -349,47 +392,53 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
         for (int k = 0; k < nt; ++k) {
             mark(PH_ITEM);
             const uint32_t s = seq + k;
-            const unsigned char* cb = chunk_s + (size_t)(s % kSwathChunkBufs) * prm.chunk_cap;
-            // ---- stage ahead: q rows of tile k+1 (its chunk landed a tile ago), chunk of tile k+2 ----
+            const unsigned char* hb = head_s + (size_t)(s % kSwathHeadBufs) * prm.head_cap;
+            // ---- stage ahead: q rows of tile k+1 (its head landed a tile ago) ----
             if (k + 1 < nt) {
-                wait_chunk(k + 1);
+                wait_head(k + 1);
                 issue_q_rows(k + 1);
             }
             cp_async_commit_group();
             mark(PH_STAGE);
-            // Three chunk buffers: the chunk of tile k+2 goes into the buffer of tile k-1, free once every thread is past
-            // that tile's flush, i.e. behind this barrier (which also frees the delta rows of a single delta buffer).
+            // Behind this barrier every thread is past the flush of tile k-1: its head buffer takes the head of tile k+2, its
+            // record buffer (free since the loop of tile k-1) the records of tile k+1, and its delta rows may be overwritten.
             __syncthreads();
-            if (tid == 0 && k + 2 < nt) issue_chunk(k + 2);
+            if (tid == 0) {
+                if (k + 2 < nt) issue_head(k + 2);
+                if (k + 1 < nt) issue_rec(k + 1);
+            }
+            wait_rec(k);
             if (PROF) prof_sink += *s_item;        // BAR.SYNC defers its blocking to the next consumer: make one here
             mark(PH_WAIT_A);
-            const SwathChunk ch = decode_chunk(cb);
+            const SwathHead ch = decode_head(hb);
             unsigned char* dbuf = dbuf_s + (size_t)(prm.ndbuf == 1 ? 0u : (s & 1u)) * dbuf_bytes;
             // ---- segment loop of this slot's track through the tile ----
             {
                 int s0 = 0, cnt = 0;
                 if (t >= 0) { s0 = ch.slot_start[slot]; cnt = ch.slot_start[slot + 1] - s0; }
                 const int steps = __reduce_max_sync(0xffffffffu, cnt);
-                const unsigned char* q_lane = q_s + (size_t)(s & 1u) * q_buf_bytes + lane_off_q;
-                // segment j (forward index inside the tile) is visited at step i: j = dir ? cnt-1-i : i
-                const int jstep = dir ? -1 : 1;
-                int j_c = dir ? cnt - 1 : 0;                // segment of the current step
-                unsigned char* d_ptr = dbuf + d_slot_off + j_c * line;
-                const int d_step = jstep * line;
-                segment_loop<P, EXPM>(psi, wpt, prm, ch.rec + s0 + j_c, jstep, cnt, steps, lane_ok, q_lane, sigt_lane, d_ptr, d_step);
+                const uint32_t q_lane = smem_u32(q_s) + (s & 1u) * q_buf_bytes + lane_off_q;
+                const uint32_t rec = smem_u32(rec_s) + (s % kSwathRecBufs) * prm.rec_cap;
+                // segment j (forward index inside the tile) is visited at step i: j = dir ? cnt-1-i : i.  Shadow lanes carry
+                // their slot's chains too and store the same values to the same rows.
+                const int j_c = dir ? cnt - 1 : 0;          // segment of the first step
+                segment_loop<P, EXPM>(psi, wpt, prm, rec + 16 * (s0 + j_c), dir ? -16 : 16, cnt, steps, null_rec, q_lane, sigt_lane,
+                                      smem_u32(dbuf) + ll * 16);
             }
             mark(PH_COMPUTE);
             cp_async_wait_all();   // this thread's q-row copies for tile k+1
             __syncthreads();
             if (PROF) prof_sink += *s_item;
             mark(PH_WAIT_B);
-            // ---- flush: one FP64 RED per (region, group) of the tile ----
+            // ---- flush: the rows of a region are contiguous; one FP64 RED per (region, group) of the tile ----
             if (f_ok) {
                 for (int l = f_l0; l < ch.L; l += f_lstep) {
-                    const int e0 = ch.csr_off[l], e1 = ch.csr_off[l + 1];
+                    const int e0 = ch.csr[l], e1 = ch.csr[l + 1];
+                    const unsigned char* row = dbuf + (size_t)e0 * row_bytes + f_qd * 16;
                     float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-                    for (int e = e0; e < e1; ++e) {
-                        const float4 x = *reinterpret_cast<const float4*>(dbuf + (size_t)ch.csr_idx[e] * row_bytes + f_qd * 16);
+#pragma unroll 4
+                    for (int e = e0; e < e1; ++e, row += row_bytes) {
+                        const float4 x = *reinterpret_cast<const float4*>(row);
                         v.x += x.x; v.y += x.y; v.z += x.z; v.w += x.w;
                     }
                     double* tp = prm.tally + (size_t)ch.regions[l] * Gs + f_qd * 4;

@@ -24,7 +24,7 @@ def test_library_exports_every_declared_symbol():
     for name in sorted(declared):
         assert hasattr(L, name), f"{name} is declared in include/nd.h but not exported"
     assert declared == set(nd.EXPORTS), declared ^ set(nd.EXPORTS)
-    assert nd.nd_version() >> 16 == 1
+    assert nd.nd_version() >> 16 == 2
 
 
 def test_no_product_file_touches_the_oracle():

@@ -109,3 +109,64 @@ def test_config5_full_size_sampled_outputs():
     finally:
         gp.destroy()
         tr.destroy()
+
+
+def test_config5_full_size_whole_sweep_against_the_oracle():
+    """ONE oracle sweep (O-6) at config 5's full size, compared element by element with the CUDA path in the launch
+    configuration bench.py times: every phi[r][g] (1e-4), every tally (2e-4 of the largest), every boundary psi (2e-5).
+    About 1.5e11 FP64 updates on the host cores (minutes) and ~10 GB of host arrays."""
+    prob = make_config(5, scale=1.0)
+    m = prob.mesh
+    tr = nd.nd_tracks_generate_device(m.xy, m.tri, m.W, m.H, prob.bc, prob.n_azim, prob.spacing, segment_capacity=1 << 28)
+    gp = nd.nd_problem_create(prob.xs, prob.polar_sin, prob.polar_weight, m.material, tr)
+    try:
+        R, G, P, T = m.n_regions, prob.n_groups, prob.n_polar, tr.n_tracks
+        info = gp.nd_problem_info_get()
+        assert info["sweep_kernel"] == nd.ND_SWEEP_SWATH and info["n_segments"] == tr.n_segments
+        rng = np.random.default_rng(515)
+        Q = rng.uniform(0.05, 1.0, size=(R, G))
+        psi = rng.uniform(0.0, 2.0, size=(T, 2, P, G)).astype(np.float32)
+        gp.nd_boundary_flux_set(psi)
+        phi_g = gp.nd_transport_sweep(torch.from_numpy(Q).cuda()).cpu().numpy()
+        tally_g = gp.nd_tally_get().cpu().numpy()
+        psi_g = gp.nd_boundary_flux_get()
+        vol = gp.nd_track_volume_get()
+        # the oracle on the library's (bit-exact, tests/test_gpu_trace.py) segment arrays; its own volumes from them
+        vol_o = oracle.track_volumes(R, tr.seg_offset, tr.seg_region, tr.seg_length, tr.track_weight)
+        assert np.abs(vol - vol_o).max() <= 1e-12 * vol_o.max()
+        psi64 = psi.astype(np.float64)
+        del psi
+        phi_o, psi_o, tally_o = oracle.sweep(m.material, prob.xs.sigma_t, prob.polar_sin, prob.polar_weight, tr.seg_offset,
+                                             tr.seg_region, tr.seg_length, tr.track_weight, tr.link, vol_o, Q, psi64)
+        del psi64
+        err_phi = phi_rel_err(phi_g, phi_o)
+        err_tally = float(np.abs(tally_g - tally_o).max() / np.abs(tally_o).max())
+        err_psi = float(np.abs(psi_g - psi_o).max() / np.abs(psi_o).max())
+        print(f"config 5 full sweep: phi rel err {err_phi:.3e}, tally {err_tally:.3e}, psi {err_psi:.3e}")
+        assert err_phi <= PHI_RTOL
+        assert err_tally <= 2e-4
+        assert err_psi <= PSI_ATOL_REL
+    finally:
+        gp.destroy()
+        tr.destroy()
+
+
+def test_config5_tenth_scale_twin_power_iteration():
+    """k_eff, k history and phi after 20 power iterations on config 5's 0.1-scale twin (~1e5 FSRs, 51 groups, the
+    production tile / swath shapes): SURVEY 8(d) 'k_eff parity ... on a stated 10x-down-scaled twin'."""
+    pair = make_pair(5, 0.1)
+    try:
+        assert pair.R > 90_000 and pair.gpu.nd_problem_info_get()["sweep_kernel"] == nd.ND_SWEEP_SWATH
+        n_it = 20
+        ko, phio, psio, hist = pair.oracle_power(n_it)
+        dphi = torch.empty((pair.R, pair.G), dtype=torch.float64, device="cuda")
+        out = pair.gpu.nd_power_iteration(n_it, d_phi_out=dphi, want_stats=True)
+        kg = np.array([s["k_eff"] for s in out["stats"]])
+        print(f"config 5 x0.1 twin: k_gpu {out['k_eff']:.8f} k_oracle {ko:.8f}, max history diff {np.abs(kg - hist).max() * 1e5:.3f} pcm")
+        assert np.abs(kg - hist).max() * 1e5 <= K_PCM
+        assert abs(out["k_eff"] - ko) * 1e5 <= K_PCM
+        assert phi_rel_err(dphi.cpu().numpy(), phio) <= PHI_RTOL
+        psi_g = pair.gpu.nd_boundary_flux_get()
+        assert np.abs(psi_g - psio).max() <= 5 * PSI_ATOL_REL * np.abs(psio).max()   # the bar of test_power_iteration_matches_oracle
+    finally:
+        pair.close()

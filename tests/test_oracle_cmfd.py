@@ -155,3 +155,54 @@ def test_cmfd_keeps_the_fixed_point_and_needs_fewer_sweeps(bc, coarse):
     fp = phip / oracle.fission_rate(m.material, xs.nu_sigma_f, tr.volume, phip)
     assert np.max(np.abs(fa - fp) / fp) < 2e-6
     assert len(ha) * 3 <= len(hp), (len(ha), len(hp))
+
+
+def test_boundary_flux_prolongation_uses_the_cell_the_chain_enters():
+    """The psi half of C-9: after one accelerated iteration the stored boundary flux of chain (t, d) -- the flux that will
+    ENTER track t travelling in direction d -- is the plain iteration's value times the flux ratio of the coarse cell that
+    GEOMETRICALLY contains the chain's entry point (the start point of the track for d = 0, its end point for d = 1).
+    The cell is located here from the track end coordinates, not from the segment list, on a mesh whose grid lines
+    coincide with the overlay (no jitter), and the ratio is read off the oracle's own phi (accelerated / plain).  A chain
+    scaled with the cell at its other end, or with the cell its feeding chain came from, fails."""
+    bc = (1, 0, 1, 1)                                   # reflective left, bottom, top; vacuum right
+    W, H, nx, ny = 4.0, 3.0, 8, 6
+    m = rect_tri_mesh(W, H, nx, ny, seed=41, jitter=0.0, n_materials=3)
+    xs = make_xs(3, [True, False, True], 41, sigt_range=(0.3, 1.2), c_range=(0.5, 0.9), n_up=1)
+    tr = _tracks(m, bc, 16, 0.05)
+    ps, pw = tabuchi_yamamoto(3)
+    ncx, ncy = 4, 3                                     # overlay lines on mesh grid lines: every triangle lies in one cell
+    cell = cartesian_cells(m, ncx, ncy)
+    args = (m.material, xs.sigma_t, xs.sigma_s, xs.nu_sigma_f, xs.chi, ps, pw, tr.seg_offset, tr.seg_region, tr.seg_length,
+            tr.track_weight, tr.link, tr.volume, cell, ncx * ncy, cartesian_coupling(m, ncx, ncy))
+    # a state three plain iterations from the flat start: the flux is far from converged, so the ratios differ by cell
+    k0, phi0, psi0, _ = cmfd.power_iteration_cmfd(*args, 3, accelerate=False)
+    _, phi_p, psi_p, _ = cmfd.power_iteration_cmfd(*args, 1, state=(k0, phi0, psi0), accelerate=False)
+    _, phi_a, psi_a, _ = cmfd.power_iteration_cmfd(*args, 1, state=(k0, phi0, psi0), accelerate=True)
+    ratio_r = phi_a / phi_p                              # the phi half of C-9: constant inside a coarse cell
+    ratio_c = np.zeros((ncx * ncy, xs.n_groups))
+    for c in range(ncx * ncy):
+        rr = ratio_r[cell == c]
+        assert len(rr) > 0 and np.abs(rr - rr[0]).max() < 1e-12
+        ratio_c[c] = rr[0]
+    assert (ratio_c.max(0) - ratio_c.min(0)).min() > 1e-3, "the cells' ratios must differ for the pin to bite"
+    # entry point of chain (t, d), nudged into the domain along the direction of travel
+    e = tr.ends
+    u = e[:, 2:] - e[:, :2]
+    u /= np.linalg.norm(u, axis=1)[:, None]
+    eps = 1e-7
+    pts = np.stack([e[:, :2] + eps * u, e[:, 2:] - eps * u], 1)             # [T][2][xy]
+    cx = np.clip((pts[..., 0] / W * ncx).astype(int), 0, ncx - 1)
+    cy = np.clip((pts[..., 1] / H * ncy).astype(int), 0, ncy - 1)
+    cell_geo = cy * ncx + cx                                                   # [T][2]
+    # a track end that sits ON an overlay line (a mesh vertex on the boundary) has no unique geometric cell: left out
+    fx, fy = pts[..., 0] / W * ncx, pts[..., 1] / H * ncy
+    clear = (np.abs(fx - np.round(fx)) > 1e-5) & (np.abs(fy - np.round(fy)) > 1e-5) | \
+            ((np.abs(fx - np.round(fx)) > 1e-5) & ((np.round(fy) == 0) | (np.round(fy) == ncy))) | \
+            ((np.abs(fy - np.round(fy)) > 1e-5) & ((np.round(fx) == 0) | (np.round(fx) == ncx)))
+    assert clear.mean() > 0.98
+    expect = psi_p * ratio_c[cell_geo][:, :, None, :]
+    scale = np.abs(psi_p).max()
+    assert scale > 0 and np.abs(psi_a - expect)[clear].max() < 1e-12 * scale
+    # the pin bites: scaling with the cell at the chain's OTHER end is off by orders of magnitude more than the bar
+    wrong = psi_p * ratio_c[cell_geo[:, ::-1]][:, :, None, :]
+    assert np.abs(psi_a - wrong)[clear].max() > 1e-6 * scale
