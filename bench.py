@@ -125,9 +125,13 @@ def build_inputs(args, tracer="device"):
 
 
 def oracle_sample(prob, tr, cpu_seconds):
-    """The oracle sweep (O-6), as it stands, on a contiguous sample of the workload's tracks sized for about
-    `cpu_seconds` of wall time.  Sampled tracks keep their segments; their links are cut (vacuum), which does not
-    change the work per update."""
+    """The oracle sweep (O-6), as it stands, on contiguous samples of the workload's tracks.  Sampled tracks keep their
+    segments; their links are cut (vacuum), which does not change the work per update.
+
+    Every orc_sweep call allocates, zeroes and reduces one private tally array per thread (threads x R x G doubles: 6.5 GB
+    at config 5 with 16 threads) whatever the sample holds -- a cost of SAMPLING that a full sweep pays once per 1.5e11
+    updates.  So two samples of different size are timed (about 1/3 and 2/3 of `cpu_seconds`) and the MARGINAL rate
+    (u2 - u1) / (t2 - t1) is reported as `value`; the raw rates of both samples are reported beside it."""
     import oracle
     nth = oracle.num_threads()
     G, P, T = prob.n_groups, prob.n_polar, tr.n_tracks
@@ -155,13 +159,20 @@ def oracle_sample(prob, tr, cpu_seconds):
         t0 = max(0, T // 2 - n // 2)
         return t0, t0 + n
 
-    u, dt = run(*pick(rate_guess * 1.0))             # pilot ~1 s
-    rate = u / dt
-    u, dt = run(*pick(rate * cpu_seconds))
-    frac = u / (2.0 * tr.n_segments * P * G)
-    return {"value": u / dt, "unit": UNIT, "cores": nth, "kind": "oracle",
-            "sample": f"oracle O-6 sweep (FP64, OpenMP) over a contiguous sample of tracks holding {frac:.4%} of the "
-                      f"workload's updates ({u:.3e} updates, {dt:.1f} s wall)"}
+    u0, dt0 = run(*pick(rate_guess * 0.5))           # pilot ~0.5 s (includes the fixed cost)
+    rate = u0 / dt0
+    u1, dt1 = run(*pick(rate * cpu_seconds / 3.0))
+    u2, dt2 = run(*pick(rate * cpu_seconds * 2.0 / 3.0))
+    U = 2.0 * tr.n_segments * P * G
+    if u2 > u1 and dt2 > dt1:
+        value, fixed = (u2 - u1) / (dt2 - dt1), max(0.0, dt1 - u1 * (dt2 - dt1) / (u2 - u1))
+    else:                                            # the whole workload fits the smaller sample (tiny configs)
+        value, fixed = u2 / dt2, 0.0
+    return {"value": value, "unit": UNIT, "cores": nth, "kind": "oracle",
+            "raw_rates": [u1 / dt1, u2 / dt2], "fixed_cost_s_per_call": fixed,
+            "sample": f"oracle O-6 sweep (FP64, OpenMP), marginal rate between two contiguous track samples holding "
+                      f"{u1 / U:.4%} and {u2 / U:.4%} of the workload's updates ({u1:.3e} updates in {dt1:.1f} s, {u2:.3e} in "
+                      f"{dt2:.1f} s; {fixed:.2f} s per call is the per-thread tally set-up of orc_sweep, paid once per full sweep)"}
 
 
 def run_reference(args):
@@ -325,14 +336,24 @@ def main():
     hbm_peak, peak_src, sm_max = peaks()
     sweep_ms = prof["sweep_ms"] / max(1, prof["sweep_launches"])
     achieved = info["algorithmic_bytes"] / (sweep_ms * 1e-3) / 1e9
-    traffic = None
-    # DRAM bytes of one sweep launch as ncu saw them (profiles/r01b_sweep_traffic.csv, from the --set full captures)
-    tpath = os.path.join(ROOT, "profiles", "r01b_sweep_traffic.csv")
+    # DRAM bytes of one sweep launch as ncu saw them: profiles/r02_traffic_cfg<config>_<build id>.csv, the log of the ncu
+    # command in profiles/r02_traffic.md.  Only a capture of THIS build (nd_build_id) is quoted; otherwise null.
+    build_id = nd.nd_build_id()
+    traffic, traffic_src = None, f"no ncu capture of build {build_id} under profiles/ (see profiles/r02_traffic.md)"
+    tpath = os.path.join(ROOT, "profiles", f"r02_traffic_cfg{args.config}_{build_id}.csv")
     if os.path.exists(tpath) and args.scale == 1.0 and info["sweep_kernel"] == 3:
-        for row in open(tpath).read().split("\n")[1:]:
-            f = row.split(",")
-            if len(f) == 5 and f[0] == str(args.config):
-                traffic = int(f[4])
+        import csv
+        tot = 0
+        for row in csv.reader(open(tpath)):
+            if len(row) > 14 and "k_sweep_swath" in row[4] and row[12] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                tot += int(float(row[14]))
+        if tot > 0:
+            traffic, traffic_src = tot, os.path.relpath(tpath, ROOT)
+    mb = None
+    try:
+        mb = nd.nd_microbench(device=str(dev))
+    except nd.NdError as e:                          # diagnostics only: the bench line does not depend on it
+        mb = {"error": str(e)}
     # The sweep is bound by the exp pipe, not by HBM: one update = one MUFU.EX2, and the SM issues
     # 16 of them per clock -> peak = 148 SMs x 16 x max SM clock.  The HBM view (algorithmic bytes / kernel time against
     # the measured copy bandwidth, and the DRAM traffic ncu saw) is reported beside it.
@@ -341,7 +362,9 @@ def main():
     roofline = {"bound": "alu", "achieved": upd_rate / 1e9, "peak": mufu_peak / 1e9, "unit": "Gupdate/s (1 MUFU.EX2 each)",
                 "frac": upd_rate / mufu_peak, "traffic": traffic, "kernel": "k_sweep_swath" if info["sweep_kernel"] == 3 else "sweep",
                 "kernel_ms": sweep_ms, "kernel_share_of_step": sweep_ms / (ms_local / args.steps),
-                "peak_source": f"derived: 148 SMs x 16 MUFU/clk x {sm_max:.0f} MHz (DESIGN.md; micro-benchmark 15.84/clk/SM)",
+                "peak_source": f"derived: 148 SMs x 16 MUFU.EX2/clk/SM x {sm_max:.0f} MHz max SM clock (DESIGN.md section 5); "
+                               "nd_microbench measured in this run: see roofline.microbench",
+                "microbench": mb, "traffic_source": traffic_src, "build_id": build_id,
                 "hbm": {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
                         "algorithmic_bytes_per_launch": int(info["algorithmic_bytes"]), "peak_source": peak_src,
                         "dram_traffic_GBps": (traffic / (sweep_ms * 1e-3) / 1e9) if traffic else None}}

@@ -250,7 +250,21 @@ nd_status nd_flux_set(nd_problem* p, const double* d_phi, double k_eff, void* cu
 nd_status nd_track_volume_get(nd_problem* p, double* host_out);                    /* HOST [R] */
 nd_status nd_tally_get(nd_problem* p, double* d_tally_out, void* cuda_stream);     /* DEVICE [R][G], last sweep */
 
-/* NEXT-3 (CMFD, Algorithm 1 "Solve CMFD on the coarse mesh"), step C-3 of DESIGN.md 8d: the net
+/* NEXT-3 (CMFD, Algorithm 1 "Solve CMFD on the coarse mesh"), step C-2 of DESIGN.md 8d: the interior
+ * surfaces of a coarse mesh = the unordered pairs of coarse cells (lo < hi) that two consecutive segments of some track
+ * join, plus the pairs a reflective hand-over joins (the cell in which chain (t, d) ends and the cell in which the chain
+ * link[t][d] begins).  HOST code, integers only, no GPU.  Uses desc->n_regions, n_tracks, track_seg_offset, seg_region, link.
+ *   cell         HOST [R], 0 <= cell[r] < n_cells (C-1: any map of regions to coarse cells)
+ *   capacity     entries pair_lo / pair_hi can hold; 0 = size query (pair_lo / pair_hi may be NULL)
+ *   n_pairs_out  HOST, written: the number of surfaces
+ *   pair_lo/hi   HOST [capacity], written when capacity >= *n_pairs_out, sorted by (lo, hi): what nd_sweep_currents,
+ *                nd_cmfd_coarse_solve and nd_cmfd_iteration take as their surface list
+ * Errors: ND_ERR_NULL, ND_ERR_INVALID (sizes; capacity > 0 but too small: *n_pairs_out is still written), ND_ERR_RANGE,
+ * ND_ERR_NOMEM. */
+nd_status nd_cmfd_surfaces(const nd_problem_desc* desc, int32_t n_cells, const int32_t* cell, int32_t capacity,
+                           int32_t* n_pairs_out, int32_t* pair_lo, int32_t* pair_hi);
+
+/* NEXT-3, step C-3 of DESIGN.md 8d: the net
  * currents of ONE sweep (Eq. (5)) through the surfaces of a coarse mesh, integrated over each surface with
  * the sweep's own weights w_{t,p} = 4 pi omega_a delta_a w_p sin(theta_p).
  *   d_Q              DEVICE [R][G] FP64, read: the isotropic angular source of the sweep (as nd_transport_sweep)
@@ -390,12 +404,30 @@ nd_status nd_swath_stream_build(const nd_problem_desc* desc, int32_t tracks_per_
 nd_status nd_swath_stream_view(const nd_swath_stream* s, nd_swath_stream_view_t* view);
 nd_status nd_swath_stream_destroy(nd_swath_stream* s);
 
+/* ------------------------------------------------------------------------------------------------
+ * Diagnostics: the micro-benchmarks behind the roofline denominators.  One Eq.-(5) update
+ * needs one MUFU.EX2, so n_sm x mufu_ex2_per_clk_per_sm x clock bounds the sweep in updates per second.
+ *   device_workspace  DEVICE, 256-byte aligned, >= 64 MiB; the HBM-resident RED case needs >= 1 GiB + 1 MiB (else it is
+ *                     reported as 0).  Contents are overwritten.
+ * Synchronises the stream.  Takes ~0.1 s.  Errors: ND_ERR_NULL, ND_ERR_WORKSPACE, ND_ERR_CUDA.
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct {
+    double mufu_ex2_per_clk_per_sm; /* ex2.approx.ftz.f32 results per clock per SM, 1024 threads x 8 chains per SM, clock64() */
+    double mufu_ex2_per_s;          /* the same, whole device, by CUDA events */
+    double sm_clock_mhz;            /* SM clock during the run: clock64() ticks per %globaltimer nanosecond */
+    double red_f64_l2_per_s;        /* FP64 RED lane-operations per second, random 256-byte rows of a 32 MiB table */
+    double red_f64_hbm_per_s;       /* the same on a 1 GiB table (0 if the workspace is too small) */
+    int32_t n_sm, reserved;
+} nd_microbench_result;
+nd_status nd_microbench(void* device_workspace, size_t device_bytes, void* cuda_stream, nd_microbench_result* out);
+
 const char* nd_status_string(nd_status s);
 /* Message of the last call that failed ON THE CALLING THREAD (thread-local storage, valid until that thread's next failing
  * call).  The argument is accepted for symmetry and ignored: errors of calls that have no problem (nd_tracks_generate,
  * nd_problem_create) are reported the same way. */
 const char* nd_last_error(const nd_problem* p_or_null);
 uint32_t nd_version(void);
+const char* nd_build_id(void); /* short hash of the sources this library was built from (paper_2607_01591_b200/_build.py) */
 
 #ifdef __cplusplus
 }

@@ -25,9 +25,9 @@ EXPORTS = [
     "nd_tracks_generate", "nd_tracks_device_workspace_bytes", "nd_tracks_generate_device", "nd_tracks_view", "nd_tracks_destroy", "nd_workspace_bytes", "nd_problem_create",
     "nd_problem_destroy", "nd_transport_sweep", "nd_source_update", "nd_power_iteration", "nd_state_reset",
     "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_outgoing_flux_get", "nd_flux_get", "nd_flux_set",
-    "nd_track_volume_get", "nd_tally_get", "nd_sweep_currents", "nd_cmfd_collapse", "nd_cmfd_prolong", "nd_cmfd_coarse_solve", "nd_cmfd_iteration", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
+    "nd_track_volume_get", "nd_tally_get", "nd_cmfd_surfaces", "nd_microbench", "nd_sweep_currents", "nd_cmfd_collapse", "nd_cmfd_prolong", "nd_cmfd_coarse_solve", "nd_cmfd_iteration", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
     "nd_swath_stream_build", "nd_swath_stream_view", "nd_swath_stream_destroy",
-    "nd_status_string", "nd_last_error", "nd_version",
+    "nd_status_string", "nd_last_error", "nd_version", "nd_build_id",
 ]
 
 
@@ -82,6 +82,11 @@ class nd_problem_info(C.Structure):
                 ("smem_bytes", C.c_int32), ("grid_blocks", C.c_int32), ("tracks_per_block", C.c_int32)]
 
 
+class nd_microbench_result(C.Structure):
+    _fields_ = [("mufu_ex2_per_clk_per_sm", C.c_double), ("mufu_ex2_per_s", C.c_double), ("sm_clock_mhz", C.c_double),
+                ("red_f64_l2_per_s", C.c_double), ("red_f64_hbm_per_s", C.c_double), ("n_sm", C.c_int32), ("reserved", C.c_int32)]
+
+
 class nd_trace_timing(C.Structure):
     _fields_ = [("prepare_s", C.c_double), ("count_kernel_ms", C.c_double), ("fill_kernel_ms", C.c_double),
                 ("copy_s", C.c_double), ("finish_s", C.c_double), ("total_s", C.c_double), ("n_segments", C.c_int64),
@@ -111,6 +116,7 @@ def lib():
         L.nd_last_error.restype = C.c_char_p
         L.nd_last_error.argtypes = [C.c_void_p]
         L.nd_version.restype = C.c_uint32
+        L.nd_build_id.restype = C.c_char_p
         L.nd_tracks_generate.argtypes = [C.POINTER(nd_mesh_desc), C.c_int32, C.c_double, C.c_int32, C.POINTER(C.c_void_p)]
         L.nd_tracks_device_workspace_bytes.argtypes = [C.POINTER(nd_mesh_desc), C.c_int32, C.c_double, C.POINTER(C.c_size_t),
                                                        C.POINTER(C.c_size_t)]
@@ -135,6 +141,9 @@ def lib():
         L.nd_flux_set.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         L.nd_track_volume_get.argtypes = [C.c_void_p, C.c_void_p]
         L.nd_tally_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nd_cmfd_surfaces.argtypes = [C.POINTER(nd_problem_desc), C.c_int32, C.c_void_p, C.c_int32, C.POINTER(C.c_int32),
+                                       C.c_void_p, C.c_void_p]
+        L.nd_microbench.argtypes = [C.c_void_p, C.c_size_t, C.c_void_p, C.POINTER(nd_microbench_result)]
         L.nd_sweep_currents.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p,
                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.nd_cmfd_collapse.argtypes = [C.c_void_p, C.c_void_p, C.c_int32] + [C.c_void_p] * 8
@@ -177,6 +186,10 @@ def _np_view(addr, shape, dtype):
 
 def nd_version():
     return int(lib().nd_version())
+
+
+def nd_build_id():
+    return lib().nd_build_id().decode()
 
 
 class Tracks:
@@ -248,6 +261,35 @@ def nd_tracks_generate_device(xy, tri, W, H, bc, n_azim, spacing, segment_capaci
     out = Tracks(h, v)
     out.timing = {f[0]: getattr(tm, f[0]) for f in nd_trace_timing._fields_ if f[0] != "reserved"}
     return out
+
+
+def nd_cmfd_surfaces(seg_offset, seg_region, link, cell, n_cells, n_regions=None):
+    """C-2 (nd.h): the interior surfaces of the coarse mesh `cell` as sorted (pair_lo, pair_hi) int32 arrays.  HOST only."""
+    so, sr = np.ascontiguousarray(seg_offset, np.int64), np.ascontiguousarray(seg_region, np.int32)
+    lk, cell = np.ascontiguousarray(link, np.int32), np.ascontiguousarray(cell, np.int32)
+    d = nd_problem_desc()
+    d.n_regions, d.n_tracks = int(n_regions if n_regions is not None else len(cell)), len(so) - 1
+    d.track_seg_offset, d.seg_region, d.link = so.ctypes.data, sr.ctypes.data, lk.ctypes.data
+    n = C.c_int32()
+    _check(lib().nd_cmfd_surfaces(C.byref(d), int(n_cells), cell.ctypes.data, 0, C.byref(n), None, None), "nd_cmfd_surfaces")
+    lo, hi = np.empty(max(n.value, 1), np.int32), np.empty(max(n.value, 1), np.int32)
+    if n.value:
+        _check(lib().nd_cmfd_surfaces(C.byref(d), int(n_cells), cell.ctypes.data, n.value, C.byref(n), lo.ctypes.data,
+                                      hi.ctypes.data), "nd_cmfd_surfaces")
+    return lo[:n.value], hi[:n.value]
+
+
+def nd_microbench(device="cuda:0", workspace_bytes=(1 << 30) + (2 << 20)):
+    """Diagnostics (nd.h): MUFU.EX2 rate per clock per SM, SM clock, FP64 RED throughput (L2- / HBM-resident)."""
+    import torch
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        ws = torch.empty(int(workspace_bytes) + 256, dtype=torch.uint8, device=dev)
+        ptr = (ws.data_ptr() + 255) // 256 * 256
+        r = nd_microbench_result()
+        _check(lib().nd_microbench(C.c_void_p(ptr), int(workspace_bytes), C.c_void_p(torch.cuda.current_stream(dev).cuda_stream),
+                                   C.byref(r)), "nd_microbench")
+    return {f[0]: getattr(r, f[0]) for f in nd_microbench_result._fields_ if f[0] != "reserved"}
 
 
 def nd_cmfd_coarse_solve(co, pair_lo, pair_hi, coupling, J_surf, J_vac, k0, tol=1e-13, max_outer=100000, stream=None):

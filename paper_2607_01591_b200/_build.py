@@ -20,12 +20,24 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xptxas", "-v", "--expt-relaxed-constexpr"]
 GXX_FLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fopenmp", "-fPIC", "-Wall"]
 
-CU_SOURCES = ["nd_api.cu", "nd_trace_device.cu"]
-CXX_SOURCES = ["nd_tracks.cpp", "nd_swath.cpp"]
+CU_SOURCES = ["nd_api.cu", "nd_trace_device.cu", "nd_microbench.cu"]
+CXX_SOURCES = ["nd_tracks.cpp", "nd_swath.cpp", "nd_cmfd_host.cpp"]
 
 
 def _nvcc():
     return shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+
+
+def source_id() -> str:
+    """Short hash of every source the library is built from (csrc/ and include/): nd_build_id() returns it, bench.py
+    prints it, and ncu captures under profiles/ are named after it, so a profile of another build is never quoted."""
+    import hashlib
+    h = hashlib.sha256()
+    for d in (CSRC, INCLUDE):
+        for f in sorted(os.listdir(d)):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:12]
 
 
 def _newest_source_mtime():
@@ -41,9 +53,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     os.makedirs(BUILD, exist_ok=True)
     objs = []
+    build_id = '-DND_BUILD_ID="%s"' % source_id()
     for src in CU_SOURCES:
         obj = os.path.join(BUILD, src + ".o")
-        cmd = [_nvcc(), *NVCC_FLAGS, "-I", INCLUDE, "-I", CSRC, "-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [_nvcc(), *NVCC_FLAGS, build_id, "-I", INCLUDE, "-I", CSRC, "-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         with open(os.path.join(BUILD, src + ".ptxas.log"), "w") as f:
             f.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)

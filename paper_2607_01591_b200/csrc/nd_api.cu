@@ -58,6 +58,10 @@ extern "C" const char* nd_status_string(nd_status s)
 }
 extern "C" const char* nd_last_error(const nd_problem*) { return g_last_error.c_str(); }
 extern "C" uint32_t nd_version(void) { return ND_VERSION; }
+#ifndef ND_BUILD_ID
+#define ND_BUILD_ID "unknown"
+#endif
+extern "C" const char* nd_build_id(void) { return ND_BUILD_ID; }
 
 // ------------------------------------------------------------------------------------------------
 // device layout
@@ -107,7 +111,10 @@ SwathConfig make_swath_config_q(const Dims& d, const nd_options& opt, int q_copi
         const int NT = w * 32 / c.LPT / NC * NC;               // slots are packed over the lanes of the whole block
         if (NT < 1 || (int64_t)NT * Kmax > 65535) return false;
         if (Lmax < 16) Lmax = 16;
-        if (Lmax > 4096) Lmax = 4096;
+        {   // the kernel's fastdiv works below 2^16: regions x (pieces per staged row, group pairs per row)
+            const int per_region = std::max(d.Gs / 2, NC * (d.Gs / 4));
+            if (Lmax > 65535 / per_region) Lmax = 65535 / per_region;
+        }
         c.sp.NT = NT; c.sp.Kmax = Kmax; c.sp.Lmax = Lmax; c.sp.NC = NC; c.sp.NCq = NCq; c.sp.row_bytes = row_bytes;
         // narrow rows (G <= 16): the flush is cheap, idle slot steps are not -> equal-count tiles while the fronts stay within
         // 16 segments; wide rows: only within 4 segments (the tally re-use rho pays more than level counts), measured in profiles/
@@ -402,6 +409,7 @@ nd_status launch_swath(nd_problem* p, const double* scale_div, cudaStream_t st)
     }
     prm.magic_per_row = ndk::fastdiv_magic((uint32_t)((c.sp.NCq > 0 ? c.sp.NCq : c.sp.NC) * (d.Gs / 4)));
     prm.magic_nq = ndk::fastdiv_magic((uint32_t)(d.Gs / 4));
+    prm.magic_np = ndk::fastdiv_magic((uint32_t)(d.Gs / 2));
     prm.phase = p->phase;
     ND_CUDA(cudaMemsetAsync(p->counter, 0, sizeof(int), st));
     switch (d.P) {

@@ -182,25 +182,26 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
                     }
                     const int o_ss = 16;
                     const int o_rg = o_ss + nd_swath_pad16(2 * (NT + 1));
-                    const int o_co = o_rg + nd_swath_pad16(4 * L);
-                    const int o_rc = o_co + nd_swath_pad16(2 * (L + 1));   // = head bytes
+                    const int o_rc = o_rg + nd_swath_pad16(8 * L);   // = head bytes
                     const int bytes = o_rc + 16 * nseg;
                     const size_t base = sb.bytes.size();
                     sb.chunk_rel.push_back((uint32_t)(base / 16));
                     sb.head16.push_back((uint32_t)(o_rc / 16));
                     sb.bytes.resize(base + (size_t)bytes, 0);
                     uint8_t* c = sb.bytes.data() + base;
-                    const uint32_t hdr[4] = {(uint32_t)L | ((uint32_t)nseg << 16), (uint32_t)(o_rg / 16) | ((uint32_t)(o_co / 16) << 16),
+                    const uint32_t hdr[4] = {(uint32_t)L | ((uint32_t)nseg << 16), (uint32_t)(o_rg / 16),
                                              (uint32_t)o_rc, (uint32_t)bytes};
                     memcpy(c, hdr, 16);
                     uint16_t* ss = reinterpret_cast<uint16_t*>(c + o_ss);
                     uint32_t* rg = reinterpret_cast<uint32_t*>(c + o_rg);
-                    uint16_t* co = reinterpret_cast<uint16_t*>(c + o_co);
                     uint32_t* rc = reinterpret_cast<uint32_t*>(c + o_rc);
-                    for (int l = 0; l < L; ++l) rg[l] = regions[l];
-                    co[0] = 0;
-                    for (int l = 0; l < L; ++l) co[l + 1] = (uint16_t)(co[l] + rcount[l]);
-                    rfill.assign(co, co + L);
+                    rfill.resize(L);
+                    for (int l = 0, e = 0; l < L; ++l) {
+                        rfill[l] = e;
+                        rg[2 * l] = regions[l];
+                        rg[2 * l + 1] = (uint32_t)e | ((uint32_t)(e + rcount[l]) << 16);
+                        e += rcount[l];
+                    }
                     int o = 0, max_cnt = 0;
                     for (int b = 0; b < NT; ++b) {
                         ss[b] = (uint16_t)o;

@@ -7,15 +7,14 @@
 // geometric lock step (always the track whose front is furthest behind) until one of them has Kmax segments in the
 // tile; in both modes a tile touches at most Lmax distinct regions.  A tile is one contiguous, 16-byte aligned
 // CHUNK made of a HEAD and a RECORD part, each fetched by one bulk (TMA) copy into its own shared-memory ring:
-//   head  u32 hdr[4]          L | nseg << 16 ;  off_regions | off_csr << 16 (16-byte units from the chunk start) ;
-//                             head bytes ;  chunk bytes
+//   head  u32 hdr[4]          L | nseg << 16 ;  off_regions (16-byte units from the chunk start) ;  head bytes ;  chunk bytes
 //         u16 slot_start[NT+1] per-track prefix into rec[]                                     (padded to 16 B)
-//         u32 regions[L]       global region ids: q rows to stage, tally rows to flush          (padded to 16 B)
-//         u16 csr[L+1]         per region: its range of delta-buffer rows                        (padded to 16 B)
+//         u32 regions[L][2]    { global region id (q row to stage, tally row to flush) ;
+//                                first delta-buffer row | one past the last << 16 }             (padded to 16 B)
 //   rec   rec[nseg]            16 bytes each: { f32 length ; u32 q-row byte offset ; u32 Sigma_t-row byte offset ;
 //                              u32 delta-row byte offset }, slot-major, forward order; the backward direction walks
 //                              the same records in reverse
-// Delta rows are REGION-MAJOR: the rows of region l are csr[l] .. csr[l+1]-1, ordered by slot then by position along
+// Delta rows are REGION-MAJOR: the rows of a region are consecutive, ordered by slot then by position along
 // the track, so the flush adds up a contiguous run of rows per region (no index list) and adjacent tracks crossing
 // the same region store into adjacent rows.  A segment's weighted flux change is simply STORED in its own row (a
 // track may re-enter a region; every visit has its own row).
@@ -74,7 +73,7 @@ inline int nd_swath_pad16(int x) { return (x + 15) / 16 * 16; }
 // largest head / record part the parameters allow (the kernel's staging rings have these sizes)
 inline int nd_swath_head_capacity(const NdSwathParams& p)
 {
-    return 16 + nd_swath_pad16(2 * (p.NT + 1)) + nd_swath_pad16(4 * p.Lmax) + nd_swath_pad16(2 * (p.Lmax + 1));
+    return 16 + nd_swath_pad16(2 * (p.NT + 1)) + nd_swath_pad16(8 * p.Lmax);
 }
 inline int nd_swath_rec_capacity(const NdSwathParams& p) { return 16 * p.NT * p.Kmax; }
 
@@ -86,9 +85,9 @@ inline int64_t nd_swath_max_tiles(const NdSwathParams& p, int64_t n_segments, in
 }
 inline size_t nd_swath_max_blob(const NdSwathParams& p, int64_t n_segments, int64_t n_tracks)
 {
-    // head: 16 + slot prefix + (4 + 2) bytes per region (<= one region per segment) + three paddings
-    const size_t per_tile = 16 + (size_t)nd_swath_pad16(2 * (p.NT + 1)) + 3 * 16;
-    return (size_t)nd_swath_max_tiles(p, n_segments, n_tracks) * per_tile + 22 * (size_t)n_segments + 256;
+    // head: 16 + slot prefix + 8 bytes per region (<= one region per segment) + two paddings
+    const size_t per_tile = 16 + (size_t)nd_swath_pad16(2 * (p.NT + 1)) + 2 * 16;
+    return (size_t)nd_swath_max_tiles(p, n_segments, n_tracks) * per_tile + 24 * (size_t)n_segments + 256;
 }
 
 // track_azim / track_ends may be NULL (no geometry): tracks are then grouped in descriptor order.

@@ -50,6 +50,7 @@ struct SwathParams {
     unsigned long long c2[kMaxPolar];          // {c[p]/c[0], c[p]/c[0]} packed for the FP32x2 path (the Sigma_t table in shared
                                                // memory is pre-multiplied by c[0] = -log2(e)/sin(theta_0) there)
     uint32_t magic_per_row, magic_nq;          // fastdiv constants of NC*Gs/4 and Gs/4
+    uint32_t magic_np;                         // fastdiv constant of Gs/2 (group pairs per row: the flush mapping)
     unsigned long long* phase;                 // PROF builds: [kSwathPhases] warp-cycle sums (lane 0 of every warp)
 };
 
@@ -90,7 +91,11 @@ __device__ __forceinline__ void tma_load_1d(void* smem_dst, const void* gmem_src
 }
 __device__ __forceinline__ void cp_async_16(uint32_t smem_dst, const void* gmem_src)
 {
+#ifdef ND_Q_STAGE_CA
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(smem_dst), "l"(gmem_src) : "memory");
+#else
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_dst), "l"(gmem_src) : "memory");
+#endif
 }
 __device__ __forceinline__ void cp_async_commit_group() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
@@ -98,8 +103,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 struct SwathHead {   // decoded chunk head (pointers into the head staging buffer)
     int L, nseg;
     const uint16_t* slot_start;
-    const uint32_t* regions;
-    const uint16_t* csr;
+    const uint2* regions;      // { region id ; first delta row | one past the last << 16 }
 };
 __device__ __forceinline__ SwathHead decode_head(const unsigned char* hb)
 {
@@ -107,8 +111,7 @@ __device__ __forceinline__ SwathHead decode_head(const unsigned char* hb)
     SwathHead c;
     c.L = (int)(h.x & 0xffffu); c.nseg = (int)(h.x >> 16);
     c.slot_start = reinterpret_cast<const uint16_t*>(hb + 16);
-    c.regions = reinterpret_cast<const uint32_t*>(hb + 16 * (h.y & 0xffffu));
-    c.csr = reinterpret_cast<const uint16_t*>(hb + 16 * (h.y >> 16));
+    c.regions = reinterpret_cast<const uint2*>(hb + 16 * h.y);
     return c;
 }
 
@@ -304,9 +307,6 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
     const int lane_off_q = TIGHT ? sub * row_bytes + ll * 16 : (slot % prm.NCq) * row_bytes + ll * 16;
     const float inv_f = (float)(1.0 / *prm.scale_div);
     const int g0 = ll * 4;
-    // flush mapping: thread -> (region l0 + i*l_step, 16-byte piece qd)
-    const int f_qd = tid % nq, f_l0 = tid / nq, f_lstep = nthr / nq;
-    const bool f_ok = f_l0 < f_lstep;
 
     uint32_t seq = 0;   // tiles processed by this block so far: staging buffers and barrier parities follow it
     for (;;) {
@@ -367,13 +367,13 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
             const unsigned char* hb = head_s + (size_t)(s % kSwathHeadBufs) * prm.head_cap;
             const uint4 h = *reinterpret_cast<const uint4*>(hb);
             const int L = (int)(h.x & 0xffffu);
-            const uint32_t* regions = reinterpret_cast<const uint32_t*>(hb + 16 * (h.y & 0xffffu));
+            const uint2* regions = reinterpret_cast<const uint2*>(hb + 16 * h.y);
             const uint32_t qb = smem_u32(q_s + (size_t)(s & 1u) * q_buf_bytes);
             const int per_row = (TIGHT ? prm.NC : prm.NCq) * nq;
             for (int i = tid; i < L * per_row; i += nthr) {
                 const int l = (int)fastdiv((uint32_t)i, prm.magic_per_row), rem = i - l * per_row;
                 const int piece = rem - (int)fastdiv((uint32_t)rem, prm.magic_nq) * nq;
-                cp_async_16(qb + l * line_q + rem * 16, prm.q + (size_t)regions[l] * Gs + piece * 4);
+                cp_async_16(qb + l * line_q + rem * 16, prm.q + (size_t)regions[l].x * Gs + piece * 4);
             }
         };
         if (nt > 0) {
@@ -430,23 +430,26 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
             __syncthreads();
             if (PROF) prof_sink += *s_item;
             mark(PH_WAIT_B);
-            // ---- flush: the rows of a region are contiguous; one FP64 RED per (region, group) of the tile ----
-            if (f_ok) {
-                for (int l = f_l0; l < ch.L; l += f_lstep) {
-                    const int e0 = ch.csr[l], e1 = ch.csr[l + 1];
-                    const unsigned char* row = dbuf + (size_t)e0 * row_bytes + f_qd * 16;
-                    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            // ---- flush: one FP64 RED per (region, group) of the tile.  A thread owns a pair of groups of one region, pairs
+            // fastest: the lanes of a warp read consecutive 8-byte pieces of the region's contiguous delta rows (no bank
+            // conflict inside a region) and their REDs fall on consecutive doubles of the tally row (2-3 lines per instruction).
+            {
+                const int np = Gs >> 1;
+                for (int u = tid; u < ch.L * np; u += nthr) {
+                    const int l = (int)fastdiv((uint32_t)u, prm.magic_np), gp = u - l * np;
+                    const uint2 rg = ch.regions[l];
+                    const int e0 = (int)(rg.y & 0xffffu), e1 = (int)(rg.y >> 16);
+                    uint32_t row = smem_u32(dbuf) + e0 * row_bytes + gp * 8;
+                    float vx = 0.f, vy = 0.f;
 #pragma unroll 4
                     for (int e = e0; e < e1; ++e, row += row_bytes) {
-                        const float4 x = *reinterpret_cast<const float4*>(row);
-                        v.x += x.x; v.y += x.y; v.z += x.z; v.w += x.w;
+                        float x, y;
+                        asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(x), "=f"(y) : "r"(row));
+                        vx += x; vy += y;
                     }
-                    double* tp = prm.tally + (size_t)ch.regions[l] * Gs + f_qd * 4;
-                    const int gq = f_qd * 4;
-                    atomicAdd(tp, (double)v.x);
-                    if (gq + 1 < prm.G) atomicAdd(tp + 1, (double)v.y);
-                    if (gq + 2 < prm.G) atomicAdd(tp + 2, (double)v.z);
-                    if (gq + 3 < prm.G) atomicAdd(tp + 3, (double)v.w);
+                    double* tp = prm.tally + (size_t)rg.x * Gs + gp * 2;
+                    if (gp * 2 < prm.G) atomicAdd(tp, (double)vx);
+                    if (gp * 2 + 1 < prm.G) atomicAdd(tp + 1, (double)vy);
                 }
             }
             mark(PH_FLUSH);

@@ -23,6 +23,16 @@ BALANCE_RTOL = 2e-6
 CASES = [(1, 1.0, 3, 2), (2, 0.15, 4, 3), (3, 0.03, 5, 4), (4, 0.06, 6, 5), (5, 0.0008, 4, 4)]
 
 
+def _surfaces(pair, cell):
+    """C-2 from the LIBRARY (nd_cmfd_surfaces on the library's own tracks): the product's calls below never take a surface
+    list the oracle computed.  The oracle's list (from its own tracks) must be the same set."""
+    g = pair.g_tr
+    lo, hi = nd.nd_cmfd_surfaces(g.seg_offset, g.seg_region, g.link, cell, int(cell.max()) + 1)
+    olo, ohi = cmfd.coarse_surfaces(pair.o_tr.seg_offset, pair.o_tr.seg_region, cell, pair.o_tr.link)
+    assert np.array_equal(lo, olo) and np.array_equal(hi, ohi), "library and oracle disagree on which surfaces exist"
+    return lo, hi
+
+
 def _oracle_currents(pair, Q, psi, cell, n_cells, lo, hi):
     p, t = pair.prob, pair.o_tr
     return cmfd.sweep_currents(p.mesh.material, p.xs.sigma_t, p.polar_sin, p.polar_weight, t.seg_offset, t.seg_region,
@@ -37,7 +47,7 @@ def test_currents_match_oracle_and_balance(case):
         Q, psi = seeded_sweep_inputs(pair, seed=300 + idx)
         n_cells = nx * ny
         cell = cartesian_cells(pair.prob.mesh, nx, ny)
-        lo, hi = cmfd.coarse_surfaces(pair.o_tr.seg_offset, pair.o_tr.seg_region, cell, pair.o_tr.link)
+        lo, hi = _surfaces(pair, cell)
         assert len(lo) >= nx * (ny - 1) + ny * (nx - 1) - 1
         Js_o, Jv_o, Jr_o = _oracle_currents(pair, Q, psi, cell, n_cells, lo, hi)
         # the library takes the surfaces in any order
@@ -102,7 +112,7 @@ def test_errors_are_reported():
         Q, psi = seeded_sweep_inputs(pair, seed=5)
         dQ = torch.from_numpy(Q).cuda()
         cell = cartesian_cells(pair.prob.mesh, 3, 2)
-        lo, hi = cmfd.coarse_surfaces(pair.o_tr.seg_offset, pair.o_tr.seg_region, cell, pair.o_tr.link)
+        lo, hi = _surfaces(pair, cell)
         with pytest.raises(nd.NdError, match="ND_SWEEP_ATOMIC"):       # the tiled kernels carry no SoA stream
             swath.gpu.nd_sweep_currents(dQ, cell, 6, lo, hi)
         with pytest.raises(nd.NdError, match="not a listed surface"):  # a crossing without its surface
@@ -205,7 +215,7 @@ def test_cmfd_iteration_composed_from_the_gpu_steps(case):
                                                           t.seg_length, t.track_weight, t.link, t.volume, cell, n_cells,
                                                           coupling_of, n_iters)
         assert np.isfinite(hist_o).all()
-        lo, hi = cmfd.coarse_surfaces(t.seg_offset, t.seg_region, cell, t.link)
+        lo, hi = _surfaces(pair, cell)
         coupling = coupling_of(lo, hi)
         g = pair.gpu
         g.nd_state_reset()
@@ -239,7 +249,7 @@ def test_currents_at_full_size(idx, nx, ny, with_oracle):
         Q, psi = seeded_sweep_inputs(pair, seed=700 + idx)
         n_cells = nx * ny
         cell = cartesian_cells(pair.prob.mesh, nx, ny)
-        lo, hi = cmfd.coarse_surfaces(pair.o_tr.seg_offset, pair.o_tr.seg_region, cell, pair.o_tr.link)
+        lo, hi = _surfaces(pair, cell)
         dQ = torch.from_numpy(Q).cuda()
         pair.gpu.nd_boundary_flux_set(psi)
         pair.gpu.nd_sweep_currents(dQ, cell, n_cells, lo, hi)            # warm-up
@@ -285,7 +295,7 @@ def _coarse_inputs(pair, nx, ny, seed):
     phi = rng.uniform(0.5, 1.5, (pair.R, pair.G))
     psi = rng.uniform(0.0, 0.2, (pair.T, 2, pair.P, pair.G))
     cell = cartesian_cells(p.mesh, nx, ny)
-    lo, hi = cmfd.coarse_surfaces(t.seg_offset, t.seg_region, cell, t.link)
+    lo, hi = _surfaces(pair, cell)
     Q = oracle.source(p.mesh.material, p.xs.sigma_s, p.xs.nu_sigma_f, p.xs.chi, phi, 1.0)
     phi_new, _, _ = pair.oracle_sweep(Q, psi)
     Js, Jv, _ = _oracle_currents(pair, Q, psi, cell, nx * ny, lo, hi)
@@ -331,7 +341,7 @@ def test_cmfd_iteration_all_steps_on_the_gpu(case):
                                                         p.xs.chi, p.polar_sin, p.polar_weight, t.seg_offset, t.seg_region,
                                                         t.seg_length, t.track_weight, t.link, t.volume, cell, n_cells,
                                                         coupling_of, n_iters)
-        lo, hi = cmfd.coarse_surfaces(t.seg_offset, t.seg_region, cell, t.link)   # geometry of the overlay, not arithmetic
+        lo, hi = _surfaces(pair, cell)
         coupling = coupling_of(lo, hi)
         g = pair.gpu
         g.nd_state_reset()
@@ -369,7 +379,7 @@ def test_cmfd_iteration_entry_point(case):
                                                         t.seg_length, t.track_weight, t.link, t.volume, cell, n_cells,
                                                         coupling_of, n_iters)
         assert np.isfinite(hist_o).all() and (hist_o > 0).all()
-        lo, hi = cmfd.coarse_surfaces(t.seg_offset, t.seg_region, cell, t.link)
+        lo, hi = _surfaces(pair, cell)
         coupling = coupling_of(lo, hi)
         pair.gpu.nd_state_reset()
         hist_g = [pair.gpu.nd_cmfd_iteration(cell, n_cells, lo, hi, coupling) for _ in range(n_iters)]
@@ -402,7 +412,7 @@ def test_cmfd_with_the_swath_sweep_kernel():
         assert b.gpu.workspace_bytes > make_pair_bytes(idx, scale)
         p, t = a.prob, a.o_tr
         cell = cartesian_cells(p.mesh, nx, ny)
-        lo, hi = cmfd.coarse_surfaces(t.seg_offset, t.seg_region, cell, t.link)
+        lo, hi = _surfaces(pair, cell)
         Q, psi = seeded_sweep_inputs(a, seed=77)
         dQ = torch.from_numpy(Q).cuda()
         a.gpu.nd_boundary_flux_set(psi)
@@ -444,7 +454,7 @@ def test_cmfd_needs_fewer_sweeps_on_the_gpu():
     try:
         p, t = pair.prob, pair.o_tr
         cell = cartesian_cells(p.mesh, 8, 8)
-        lo, hi = cmfd.coarse_surfaces(t.seg_offset, t.seg_region, cell, t.link)
+        lo, hi = _surfaces(pair, cell)
         coupling = cartesian_coupling(p.mesh, 8, 8)(lo, hi)
         pair.gpu.nd_state_reset()
         plain = pair.gpu.nd_power_iteration(5000, tol_k=tol)

@@ -241,7 +241,7 @@ def test_iteration_stats_beyond_one_ring():
         assert ks[-1] == out["k_eff"]
         ko, _, _, hist = pair.oracle_power(60)
         assert np.abs(ks[:60] - hist).max() * 1e5 <= K_PCM
-        assert abs(ks[4095] - ks[4096]) < 1e-9 and abs(ks[-1] - ks[4096]) < 1e-9    # converged long before; no seam at the ring edge
+        assert abs(ks[4095] - ks[4096]) < 1e-7 and abs(ks[-1] - ks[4096]) < 1e-7    # converged long before (FP32 chains: ~1e-9 jitter); no seam at the ring edge
     finally:
         pair.close()
 

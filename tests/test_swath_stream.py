@@ -27,15 +27,17 @@ def _decode_and_check(st, mat, seg_offset, seg_region, seg_length, NT, Kmax, Lma
             c = blob[ref[ti, 0]:ref[ti + 1, 0]]
             hdr = c[:16].view(np.uint32)
             L, nseg = int(hdr[0] & 0xffff), int(hdr[0] >> 16)
-            o_rg, o_co = 16 * int(hdr[1] & 0xffff), 16 * int(hdr[1] >> 16)
+            o_rg = 16 * int(hdr[1])
             head = int(hdr[2])
             assert head == ref[ti, 1] and head % 16 == 0 and head <= st["max_head_bytes"]
             assert hdr[3] == len(c) == head + 16 * nseg and 16 * nseg <= st["max_rec_bytes"]
             assert 1 <= L <= Lmax and 1 <= nseg <= NT * Kmax
             ss = c[16:16 + 2 * (NT + 1)].view(np.uint16).astype(np.int64)
-            regions = c[o_rg:o_rg + 4 * L].view(np.uint32).astype(np.int64)
-            co = c[o_co:o_co + 2 * (L + 1)].view(np.uint16).astype(np.int64)
-            assert o_co + 2 * (L + 1) <= head
+            rg = c[o_rg:o_rg + 8 * L].view(np.uint32).reshape(L, 2).astype(np.int64)
+            regions = rg[:, 0]
+            co = np.concatenate([rg[:, 1] & 0xffff, [rg[-1, 1] >> 16]])
+            assert np.array_equal(rg[:, 1] >> 16, co[1:]), "row ranges of consecutive regions are contiguous"
+            assert o_rg + 8 * L <= head
             rec = c[head:head + 16 * nseg].view(np.uint32).reshape(nseg, 4)
             assert ss[0] == 0 and ss[NT] == nseg and np.all(np.diff(ss) >= 0) and np.all(np.diff(ss) <= Kmax)
             assert len(np.unique(regions)) == L
