@@ -94,9 +94,9 @@ typedef struct {
     int32_t graph_mode;     /* nd_power_iteration with a fixed iteration count (no tolerances, no per-iteration stats, profiling
                                off) replays a CUDA graph of two iterations instead of launching their kernels one by one:
                                0 = default (on for calls of >= 4 iterations), 1 = never */
-    int32_t cmfd_stream;    /* 1: keep the plain SoA segment stream on the device beside the tiled kernel's chunk stream (8 bytes
-                               per segment more workspace) so that nd_sweep_currents / nd_cmfd_iteration work with the fast
-                               sweep kernels; 0 = default (only ND_SWEEP_ATOMIC problems carry it) */
+    int32_t cmfd_stream;    /* 1: lay the swath kernel's shared memory out for the CMFD current tally (a W row per track and a
+                               ring of crossing lists: ~8 KB per block more, so tiles may come out a segment shorter) and keep
+                               on the host what nd_cmfd_create needs to place the crossings; 0 = default */
     int32_t item_order;     /* ND_SWEEP_SWATH: order in which thread blocks take the (swath, direction) work items.  0 = default:
                                most expensive first (best load balance; measured fastest at every config); 1 = angle by angle,
                                adjacent swaths consecutively (blocks that run together touch neighbouring regions) */
@@ -138,6 +138,7 @@ typedef struct {            /* all pointers HOST, owned by the nd_tracks object,
     const double* azim_phi;          /* [N_a/2] effective angles */
     const double* azim_weight;       /* [N_a/2] omega_a per direction (sum over N_a directions = 1) */
     const double* azim_spacing;      /* [N_a/2] effective spacing delta_a */
+    const int32_t* track_global;     /* [T] id of the track in the unsharded laydown (identity unless made by nd_tracks_shard) */
 } nd_tracks_view_t;
 
 /* The same preprocessing with the ray walk (rule R-W, one step per segment: almost all of the work) on the GPU:
@@ -162,6 +163,16 @@ typedef struct {                /* where the time of nd_tracks_generate_device w
 nd_status nd_tracks_generate_device(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, void* device_workspace,
                                     size_t device_bytes, void* cuda_stream, nd_trace_timing* timing_or_null,
                                     nd_tracks** out);
+
+/* NEXT-2 (the paper names multi-GPU as future work): shard `shard` of `n_shards` of an ANGLE-PAIR
+ * partition of a cyclic laydown.  A reflective link joins a track of angle j only to one of its complement N_a/2-1-j (O-3),
+ * so a shard that owns whole pairs {j, N_a/2-1-j} exchanges no boundary flux; the shards share the additive tally alone
+ * (nd_tally_reducer_set).  Pairs are dealt to the shards by segment count, longest first (deterministic).
+ * The result is a new HOST object with the shard's tracks in canonical order, ids renumbered, links remapped,
+ * track_global = their ids in `full`, and track_volume = the areas A~_r of the WHOLE laydown (pass it to nd_problem_create
+ * as nd_problem_desc.region_volume: every shard divides its flux by the full track-estimated area).
+ * Errors: ND_ERR_NULL, ND_ERR_INVALID (shard out of range, n_shards > N_a/4), ND_ERR_STATE (`full` is itself a shard). */
+nd_status nd_tracks_shard(const nd_tracks* full, int32_t n_shards, int32_t shard, nd_tracks** out);
 
 nd_status nd_tracks_view(const nd_tracks* tracks, nd_tracks_view_t* view);
 nd_status nd_tracks_destroy(nd_tracks* tracks);
@@ -192,9 +203,14 @@ typedef struct {                    /* all pointers: HOST memory, borrowed for t
        results do not depend on it.  Without it ND_SWEEP_AUTO selects the atomic sweep kernel. */
     const int32_t* track_azim;      /* [T] id of the track's angle; tracks with equal id are parallel */
     const double* track_ends;       /* [T][4] x0,y0,x1,y1 (forward direction runs from 0 to 1) */
+    /* Optional (NULL = the library forms A~ from this descriptor's own segments): the track-estimated areas A~_r to divide
+       by, HOST [R], finite and >= 0.  A shard of an angle-pair partition (nd_tracks_shard) holds a part of the tracks but
+       must use the areas of all of them. */
+    const double* region_volume;
 } nd_problem_desc;
 
 typedef struct nd_problem nd_problem; /* opaque host object; owns no device memory except what lies in the workspace */
+typedef struct nd_cmfd nd_cmfd;       /* a CMFD plan bound to one problem (NEXT-3, below) */
 
 /* Limits: n_regions <= 2^24, n_materials <= 256, n_groups <= 256, n_polar <= 4. */
 nd_status nd_workspace_bytes(const nd_problem_desc* desc, const nd_options* opts_or_null, size_t* device_bytes);
@@ -213,6 +229,18 @@ nd_status nd_problem_destroy(nd_problem* p); /* does not touch the workspace */
  * Reads the problem's current boundary psi (Jacobi: the previous sweep's outgoing fluxes), advances it through
  * the link table (vacuum entries become 0).  FP32 segment arithmetic, FP64 tallies. */
 nd_status nd_transport_sweep(nd_problem* p, const double* d_Q, double* d_phi_out, void* cuda_stream);
+
+/* NEXT-2: a problem built from one shard of an angle-pair partition (nd_tracks_shard, with
+ * nd_problem_desc.region_volume = the areas of the whole laydown) tallies only its own tracks.  The reducer is called by
+ * nd_transport_sweep and by every iteration of nd_power_iteration right after the sweep, before the tally is turned into a
+ * flux (O-6 finalise): it must replace d_tally (DEVICE [n_doubles] FP64, the padded [R][Gs] tally) by the SUM over all
+ * shards, in stream order on `cuda_stream` (e.g. one NCCL all-reduce).  Everything else -- source, flux, k -- is then
+ * computed redundantly and identically by every shard; boundary flux never leaves a shard.  Return 0 on success.
+ * fn = NULL removes the reducer.  With a reducer set nd_power_iteration launches its kernels one by one (no CUDA graph),
+ * and nd_iter_stats.leakage / balance_residual are reported as 0 (they compare a problem's own boundary flux with its own
+ * tally). */
+typedef int32_t (*nd_tally_reduce_fn)(void* user, double* d_tally, int64_t n_doubles, void* cuda_stream);
+nd_status nd_tally_reducer_set(nd_problem* p, nd_tally_reduce_fn fn, void* user);
 
 /* O-7: Q[r][g] = (1/4pi) ( sum_g' Sigma_s[m][g][g'] phi[r][g'] + chi[m][g]/k * sum_g' nuSigma_f[m][g'] phi[r][g'] ).
  *   d_phi DEVICE [R][G] FP64 read; d_Q_out DEVICE [R][G] FP64 written;
@@ -257,98 +285,97 @@ nd_status nd_tally_get(nd_problem* p, double* d_tally_out, void* cuda_stream);  
  *   cell         HOST [R], 0 <= cell[r] < n_cells (C-1: any map of regions to coarse cells)
  *   capacity     entries pair_lo / pair_hi can hold; 0 = size query (pair_lo / pair_hi may be NULL)
  *   n_pairs_out  HOST, written: the number of surfaces
- *   pair_lo/hi   HOST [capacity], written when capacity >= *n_pairs_out, sorted by (lo, hi): what nd_sweep_currents,
- *                nd_cmfd_coarse_solve and nd_cmfd_iteration take as their surface list
+ *   pair_lo/hi   HOST [capacity], written when capacity >= *n_pairs_out, sorted by (lo, hi): what nd_cmfd_create takes
+ *                as its surface list
  * Errors: ND_ERR_NULL, ND_ERR_INVALID (sizes; capacity > 0 but too small: *n_pairs_out is still written), ND_ERR_RANGE,
  * ND_ERR_NOMEM. */
 nd_status nd_cmfd_surfaces(const nd_problem_desc* desc, int32_t n_cells, const int32_t* cell, int32_t capacity,
                            int32_t* n_pairs_out, int32_t* pair_lo, int32_t* pair_hi);
 
-/* NEXT-3, step C-3 of DESIGN.md 8d: the net
- * currents of ONE sweep (Eq. (5)) through the surfaces of a coarse mesh, integrated over each surface with
- * the sweep's own weights w_{t,p} = 4 pi omega_a delta_a w_p sin(theta_p).
- *   d_Q              DEVICE [R][G] FP64, read: the isotropic angular source of the sweep (as nd_transport_sweep)
- *   cell             HOST [R]: coarse cell of every region, 0 <= cell[r] < n_cells
- *   pair_lo/pair_hi  HOST [n_pairs]: the interior surfaces as cell pairs lo < hi, in any order, each listed once; every
- *                    pair of cells that consecutive segments of a track or a reflective hand-over join must be listed
- *   J_surf           HOST [n_pairs][G] FP64, written: sum of +w psi at every crossing lo -> hi, -w psi at hi -> lo
- *   J_vac, J_ref     HOST [n_cells][G] FP64, written: at the exit end of every chain (t, d), w (psi_exit - psi_in of the
- *                    opposite direction), into J_vac[cell of the end] at a vacuum end, J_ref at a reflective one; a
- *                    hand-over into another cell c2 also adds w psi_exit to the surface and moves it from J_ref[c] to
- *                    J_ref[c2].  Per cell and group: sum of the sweep's tallies + sum +-J_surf + J_vac + J_ref = 0.
- * Reads the problem's current boundary psi and leaves ALL state unchanged (the boundary flux is not advanced, the tally
- * of the last sweep is kept): nd_transport_sweep with the same d_Q afterwards performs the sweep these currents belong
- * to.  FP32 segment arithmetic, FP64 atomics.  This round: the simple one-warp-per-chain kernel over the SoA stream,
- * so the problem must have been created with sweep_kernel = ND_SWEEP_ATOMIC or nd_options.cmfd_stream = 1 (else
- * ND_ERR_STATE); scratch is allocated
- * and freed inside the call and the stream is synchronised before it returns.
- * Errors: ND_ERR_NULL, ND_ERR_INVALID (sizes; a surface listed twice; a crossing between cells that are not a listed
- * surface -- outputs are then unspecified), ND_ERR_RANGE (cell or pair out of range), ND_ERR_STATE, ND_ERR_CUDA. */
-nd_status nd_sweep_currents(nd_problem* p, const double* d_Q, int32_t n_cells, const int32_t* cell, int32_t n_pairs,
-                            const int32_t* pair_lo, const int32_t* pair_hi, double* J_surf, double* J_vac, double* J_ref,
-                            void* cuda_stream);
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-3: CMFD acceleration, Algorithm 1 of the paper ("Perform MOC on the fine mesh", "Solve CMFD on the
+ * coarse mesh", update of the fine-mesh flux; purpose PAPER.md:129).  The paper prints no formula; the reading C-1..C-9 is in
+ * DESIGN.md 8d.  A PLAN binds a coarse mesh to one problem.  Everything it needs lives in one caller-owned device workspace;
+ * the net currents of C-3 are tallied by the sweep kernel itself (the tracks are walked once), and an accelerated iteration
+ * only launches kernels: no allocation, no host arithmetic, no stream synchronisation between its steps.
+ * The problem must use the swath sweep kernel, exp_mode = ND_EXP_FAST, and have been created with nd_options.cmfd_stream = 1
+ * (its shared-memory layout then holds the per-track W rows and the crossing lists); else ND_ERR_STATE.
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct {
+    double tol;             /* coarse eigen-solve: |dk| < tol |k| and max |dPhi| < 100 tol max |Phi|; 0 = default 1e-12 */
+    int32_t max_outer;      /* fission-source iterations of the coarse solve at most; 0 = default 20000 */
+    int32_t inner_sweeps;   /* block-Jacobi sweeps per fission-source iteration; 0 = default 4 */
+    double relax;           /* C-9 with ratio = 1 + relax (Phi_new / Phi_old - 1), 0 < relax <= 1; 0 = default 1 (undamped).
+                               Coarse cells of several mean free paths make the undamped scheme diverge: use
+                               cells of at most ~2 mean free paths, or relax ~0.5-0.7 */
+    double rel_tol;         /* > 0: the coarse solve also stops once max |dPhi| has fallen to rel_tol x its value in the solve's first
+                               iteration.  An inexact coarse solve does not move the fixed point of the accelerated iteration
+                               (at the converged fine-mesh flux the collapsed flux IS the coarse eigenvector and the solve
+                               stops at once); it trades coarse iterations for a few more sweeps.  0 = default: off */
+    int32_t reserved[2];    /* must be 0 */
+} nd_cmfd_options;
+typedef struct {            /* one per accelerated iteration, HOST */
+    double k_sweep;         /* k after the transport sweep (the plain O-8 update) */
+    double k_eff;           /* the state's k after the coarse solve and prolongation */
+    int32_t coarse_iters;   /* fission-source iterations of the coarse solve */
+    int32_t coarse_ok;      /* 1: converged to a positive eigenpair and prolonged; 0: the solve failed and this iteration is a
+                               plain one (ratio 1, k = k_sweep) */
+} nd_cmfd_stats;
 
-/* NEXT-3, step C-4 of DESIGN.md 8d: flux-volume weighted constants of the coarse cells ("Solve CMFD on the coarse mesh",
- * PAPER.md:131-140), with the track-estimated areas A~_r the sweep itself uses.
- *   d_phi_or_null  DEVICE [R][G] FP64, read; NULL = the problem's current flux (the result of the last power iteration)
- *   cell           HOST [R], 0 <= cell[r] < n_cells
- *   V              HOST [n_cells]           sum of A~_r
- *   Phi            HOST [n_cells][G]        sum A~ phi / V
- *   sigma_t, nu_sigma_f  HOST [n_cells][G]  sum A~ Sigma phi / sum A~ phi
- *   sigma_s        HOST [n_cells][g][g']    from g' into g, weighted with phi_g'
- *   chi            HOST [n_cells][G]        weighted with the fission emission sum_g' nuSigma_f phi_g' (0 where there is none)
- * All G groups are kept.  A cell without regions gives NaN (0/0), as the plain definition does.  FP64 throughout; FP64
- * atomics, so sums differ from a sequential sum in the last bits only.  Scratch is allocated and freed inside the call,
- * the stream is synchronised before it returns; no state is changed.  Errors: ND_ERR_NULL, ND_ERR_INVALID, ND_ERR_RANGE,
- * ND_ERR_CUDA. */
-nd_status nd_cmfd_collapse(nd_problem* p, const double* d_phi_or_null, int32_t n_cells, const int32_t* cell, double* V,
-                           double* Phi, double* sigma_t, double* sigma_s, double* nu_sigma_f, double* chi,
-                           void* cuda_stream);
+/*   desc            the descriptor the problem was created from (HOST, borrowed): track_seg_offset, seg_region and link are read
+ *   cell            HOST [R], 0 <= cell[r] < n_cells (C-1)
+ *   pair_lo/hi      HOST [n_pairs], lo < hi, each surface once: nd_cmfd_surfaces gives the list (C-2).  Every pair of cells that
+ *                   consecutive segments of a track or a reflective hand-over join must be listed (else ND_ERR_INVALID)
+ *   coupling        HOST [n_pairs], A_s / d_s of every surface (C-5), >= 0; 0 = no diffusive coupling (Dtil alone carries it)
+ *   device_workspace DEVICE, >= nd_cmfd_workspace_bytes, 256-byte aligned, caller-owned, must outlive the plan
+ * nd_cmfd_create synchronises the stream before returning. */
+nd_status nd_cmfd_workspace_bytes(const nd_problem* p, const nd_problem_desc* desc, int32_t n_cells, const int32_t* cell,
+                                  int32_t n_pairs, size_t* device_bytes);
+nd_status nd_cmfd_create(nd_problem* p, const nd_problem_desc* desc, int32_t n_cells, const int32_t* cell, int32_t n_pairs,
+                         const int32_t* pair_lo, const int32_t* pair_hi, const double* coupling,
+                         const nd_cmfd_options* opts_or_null, void* device_workspace, size_t device_bytes, void* cuda_stream,
+                         nd_cmfd** out);
+nd_status nd_cmfd_destroy(nd_cmfd* c);
 
-/* NEXT-3, step C-9 of DESIGN.md 8d ("update the fine-mesh flux", Algorithm 1): prolongation of a coarse
- * solution onto the power-iteration state.
- *   ratio  HOST [n_cells][G] FP64: Phi_new / Phi_old of every coarse cell
- *   k_eff  the coarse eigenvalue; becomes the state's k
- * phi[r][g] *= ratio[cell[r]][g]; the stored boundary flux of chain (t, d) *= ratio[cell of the region it enters][g]
- * (FP32 storage, multiplied in FP64); the state's fission rate is recomputed from the new flux.  Works with every sweep
- * kernel.  Synchronises the stream.  Errors: ND_ERR_NULL, ND_ERR_INVALID (k_eff <= 0, n_cells < 1), ND_ERR_RANGE. */
-nd_status nd_cmfd_prolong(nd_problem* p, int32_t n_cells, const int32_t* cell, const double* ratio, double k_eff,
-                          void* cuda_stream);
+/* Algorithm 1, n_iters accelerated power iterations on the problem's own state: O-8's source, sweep (with C-3 in the sweep
+ * kernel), flux and k; then C-4 collapse, C-5..C-8 coarse eigen-solve started from the collapsed flux and the sweep's k, C-9
+ * prolongation of phi, of the stored boundary flux and of k.  Stream-ordered; the host is synchronised once, at the end.
+ *   k_eff_out HOST; stats HOST [n_iters] or NULL.
+ * Errors: ND_ERR_NULL, ND_ERR_INVALID, ND_ERR_CUDA, ND_ERR_STATE (a hand-over between unlisted cells). */
+nd_status nd_cmfd_iteration(nd_cmfd* c, int32_t n_iters, double* k_eff_out, nd_cmfd_stats* stats_or_null, void* cuda_stream);
 
-/* NEXT-3, steps C-5..C-8 of DESIGN.md 8d ("Solve CMFD on the coarse mesh", Algorithm 1): the coarse
- * balance  sum_s outflow + alpha Phi + Sigma_t V Phi - V sum_g' Sigma_s Phi_g' = (1/k) chi V sum_g' nuSigma_f Phi_g'
- * with D = 1/(3 Sigma_t), Dhat_s = 2 D_lo D_hi / (D_lo + D_hi) x coupling_s, Dtil_s = -(J_s + Dhat (Phi_hi - Phi_lo)) /
- * (Phi_hi + Phi_lo), alpha = J_vac / Phi (reflective ends: J = 0), and its dominant eigenpair by power iteration with an
- * exact inner solve (dense inverse of the loss operator, in-place Gauss-Jordan on the device), started from Phi and k0.
- * All pointers HOST (the coarse arrays are small); all arithmetic runs in CUDA kernels, FP64.
- *   V [C]; Phi, sigma_t, nu_sigma_f, chi, J_vac [C][G]; sigma_s [C][g][g'] (from g' into g): as nd_cmfd_collapse and
- *   nd_sweep_currents return them (currents on the scale of Phi)
- *   pair_lo/pair_hi/coupling [S], J_surf [S][G]: the surfaces, A_s / d_s per surface (0: no diffusive coupling)
- *   tol: |dk| < tol |k| and max |dPhi| < 1e-11 max |Phi| end the iteration (at most max_outer iterations)
- *   k_out, Phi_new [C][G] (normalised to the fission production of Phi), iters_done (may be NULL)
- * Errors: ND_ERR_NULL, ND_ERR_INVALID, ND_ERR_RANGE (a pair out of range; more than 8192 unknowns),
- * ND_ERR_NOT_CONVERGED (outputs are written), ND_ERR_CUDA.  Synchronises the stream. */
-nd_status nd_cmfd_coarse_solve(int32_t n_cells, int32_t n_groups, const double* V, const double* Phi, const double* sigma_t,
-                               const double* sigma_s, const double* nu_sigma_f, const double* chi, int32_t n_pairs,
-                               const int32_t* pair_lo, const int32_t* pair_hi, const double* coupling, const double* J_surf,
-                               const double* J_vac, double k0, double tol, int32_t max_outer, double* k_out,
-                               double* Phi_new, int32_t* iters_done, void* cuda_stream);
-
-/* NEXT-3: one CMFD-accelerated power iteration, Algorithm 1 ("Perform MOC on the fine mesh", "Solve
- * CMFD on the coarse mesh", update of the fine-mesh flux), steps C-1..C-9 of DESIGN.md 8d after the sweep of O-8:
- * source -> nd_sweep_currents -> nd_power_iteration(1) -> nd_cmfd_collapse -> nd_cmfd_coarse_solve (tol 1e-13) ->
- * nd_cmfd_prolong, on the problem's own state.  A host composition of those entry points this round: the coarse arrays
- * pass through host memory between the steps and every step synchronises.
- *   cell HOST [R]; pair_lo/pair_hi/coupling HOST [n_pairs] as in nd_sweep_currents / nd_cmfd_coarse_solve
- *   k_sweep_out (may be NULL): k after the sweep, before the coarse solve; k_eff_out: the coarse eigenvalue = the state's k
- *   coarse_iters (may be NULL): outer iterations of the coarse solve
- * Needs sweep_kernel = ND_SWEEP_ATOMIC or nd_options.cmfd_stream = 1 (nd_sweep_currents; the sweep of the iteration itself
- * runs with the problem's sweep kernel).  Errors: those of the steps; ND_ERR_STATE if the state has
- * k <= 0 or a zero fission rate.  The undamped scheme diverges for coarse cells of several mean free paths;
- * a coarse eigenvalue <= 0 is reported as ND_ERR_INVALID by the prolongation and the state is then one plain iteration on. */
-nd_status nd_cmfd_iteration(nd_problem* p, int32_t n_cells, const int32_t* cell, int32_t n_pairs, const int32_t* pair_lo,
-                            const int32_t* pair_hi, const double* coupling, double* k_sweep_out, double* k_eff_out,
-                            int32_t* coarse_iters, void* cuda_stream);
+/* The steps one by one (tests, diagnostics).  Device results stay in the plan; the *_get calls copy to HOST and synchronise.
+ *   nd_cmfd_sweep        C-3: nd_transport_sweep(d_Q -> d_phi_out) whose sweep kernel also tallies the net currents, integrated
+ *                        over each surface with the sweep's own weights w_{t,p} = 4 pi omega_a delta_a w_p sin(theta_p):
+ *                        J_surf [n_pairs][G] = sum of +w psi at every crossing lo -> hi, -w psi at hi -> lo;
+ *                        J_vac / J_ref [n_cells][G]: at the exit end of every chain (t, d), w (psi_exit - psi_in of the
+ *                        opposite direction), into J_vac[cell of the end] at a vacuum end, J_ref at a reflective one; a
+ *                        hand-over into another cell c2 also adds w psi_exit to the surface and moves it from J_ref[c] to
+ *                        J_ref[c2].  Per cell and group: sum of the sweep's tallies + sum +-J_surf + J_vac + J_ref = 0.
+ *   nd_cmfd_collapse     C-4 of d_phi (DEVICE [R][G]; NULL = the problem's current flux): V, Phi = sum A~ phi / V,
+ *                        sigma_t, nu_sigma_f = sum A~ Sigma phi / sum A~ phi, sigma_s [c][g][g'] weighted with phi_g',
+ *                        chi weighted with the fission emission (0 where there is none).  A cell without regions gives NaN.
+ *   nd_cmfd_coarse_set   loads coarse constants and currents from HOST arrays instead (to test the solve alone)
+ *   nd_cmfd_solve        C-5..C-8 from the plan's constants and currents: D = 1/(3 Sigma_t), Dhat_s = 2 D_lo D_hi / (D_lo +
+ *                        D_hi) coupling_s, Dtil_s = -(J_s + Dhat (Phi_hi - Phi_lo)) / (Phi_hi + Phi_lo), alpha = J_vac / Phi,
+ *                        balance sum_s outflow + alpha Phi + Sigma_t V Phi - V sum_g' Sigma_s Phi_g' = (1/k) chi V sum_g'
+ *                        nuSigma_f Phi_g'; dominant eigenpair by fission-source iteration with block-Jacobi inner sweeps (G x G
+ *                        cell blocks inverted with partial pivoting), in ONE cooperative kernel.  Phi_new [n_cells][G] HOST or
+ *                        NULL, normalised to the fission production of Phi.  ND_ERR_NOT_CONVERGED / ND_ERR_INVALID (eigenpair
+ *                        not positive): outputs are written.
+ *   nd_cmfd_prolong      C-9 with the last solve's Phi_new / Phi (ratio 1 if that solve failed): phi, the stored boundary flux
+ *                        of every chain (ratio of the cell it enters), k; the state's fission rate is recomputed. */
+nd_status nd_cmfd_sweep(nd_cmfd* c, const double* d_Q, double* d_phi_out, void* cuda_stream);
+nd_status nd_cmfd_currents_get(nd_cmfd* c, double* J_surf, double* J_vac, double* J_ref, void* cuda_stream);
+nd_status nd_cmfd_collapse(nd_cmfd* c, const double* d_phi_or_null, void* cuda_stream);
+nd_status nd_cmfd_coarse_get(nd_cmfd* c, double* V, double* Phi, double* sigma_t, double* sigma_s, double* nu_sigma_f, double* chi,
+                             void* cuda_stream);
+nd_status nd_cmfd_coarse_set(nd_cmfd* c, const double* V, const double* Phi, const double* sigma_t, const double* sigma_s,
+                             const double* nu_sigma_f, const double* chi, const double* J_surf, const double* J_vac,
+                             void* cuda_stream);
+nd_status nd_cmfd_solve(nd_cmfd* c, double k0, double* k_out, double* Phi_new_or_null, int32_t* iters_done_or_null,
+                        void* cuda_stream);
+nd_status nd_cmfd_prolong(nd_cmfd* c, void* cuda_stream);
 
 /* Device-time accounting.  When enabled, every sweep-kernel launch is bracketed by CUDA events on its own
  * stream; nd_profile_read synchronises and returns the accumulated kernel milliseconds and launch counts

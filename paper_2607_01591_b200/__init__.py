@@ -22,10 +22,12 @@ ND_EXP_FAST, ND_EXP_EXPM1 = 0, 1
 ND_SWEEP_AUTO, ND_SWEEP_ATOMIC, ND_SWEEP_SWATH = 0, 1, 3
 
 EXPORTS = [
-    "nd_tracks_generate", "nd_tracks_device_workspace_bytes", "nd_tracks_generate_device", "nd_tracks_view", "nd_tracks_destroy", "nd_workspace_bytes", "nd_problem_create",
+    "nd_tracks_generate", "nd_tracks_device_workspace_bytes", "nd_tracks_generate_device", "nd_tracks_view", "nd_tracks_shard", "nd_tracks_destroy", "nd_tally_reducer_set", "nd_workspace_bytes", "nd_problem_create",
     "nd_problem_destroy", "nd_transport_sweep", "nd_source_update", "nd_power_iteration", "nd_state_reset",
     "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_outgoing_flux_get", "nd_flux_get", "nd_flux_set",
-    "nd_track_volume_get", "nd_tally_get", "nd_cmfd_surfaces", "nd_microbench", "nd_sweep_currents", "nd_cmfd_collapse", "nd_cmfd_prolong", "nd_cmfd_coarse_solve", "nd_cmfd_iteration", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
+    "nd_track_volume_get", "nd_tally_get", "nd_cmfd_surfaces", "nd_microbench", "nd_cmfd_workspace_bytes", "nd_cmfd_create",
+    "nd_cmfd_destroy", "nd_cmfd_iteration", "nd_cmfd_sweep", "nd_cmfd_currents_get", "nd_cmfd_collapse", "nd_cmfd_coarse_get",
+    "nd_cmfd_coarse_set", "nd_cmfd_solve", "nd_cmfd_prolong", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
     "nd_swath_stream_build", "nd_swath_stream_view", "nd_swath_stream_destroy",
     "nd_status_string", "nd_last_error", "nd_version", "nd_build_id",
 ]
@@ -53,7 +55,7 @@ class nd_tracks_view_t(C.Structure):
                 ("track_seg_offset", C.c_void_p), ("seg_region", C.c_void_p), ("seg_length", C.c_void_p),
                 ("track_weight", C.c_void_p), ("link", C.c_void_p), ("track_azim", C.c_void_p),
                 ("track_ends", C.c_void_p), ("track_volume", C.c_void_p), ("azim_phi", C.c_void_p),
-                ("azim_weight", C.c_void_p), ("azim_spacing", C.c_void_p)]
+                ("azim_weight", C.c_void_p), ("azim_spacing", C.c_void_p), ("track_global", C.c_void_p)]
 
 
 class nd_problem_desc(C.Structure):
@@ -62,7 +64,10 @@ class nd_problem_desc(C.Structure):
                 ("sigma_s", C.c_void_p), ("nu_sigma_f", C.c_void_p), ("chi", C.c_void_p), ("polar_sin", C.c_void_p),
                 ("polar_weight", C.c_void_p), ("track_seg_offset", C.c_void_p), ("seg_region", C.c_void_p),
                 ("seg_length", C.c_void_p), ("track_weight", C.c_void_p), ("link", C.c_void_p),
-                ("track_azim", C.c_void_p), ("track_ends", C.c_void_p)]
+                ("track_azim", C.c_void_p), ("track_ends", C.c_void_p), ("region_volume", C.c_void_p)]
+
+
+ND_TALLY_REDUCE_FN = C.CFUNCTYPE(C.c_int32, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
 
 
 class nd_iter_stats(C.Structure):
@@ -80,6 +85,15 @@ class nd_problem_info(C.Structure):
                 ("n_batches", C.c_int32), ("reserved", C.c_int32), ("mean_regions_per_tile", C.c_double),
                 ("mean_segments_per_tile", C.c_double), ("lockstep_efficiency", C.c_double), ("block_threads", C.c_int32),
                 ("smem_bytes", C.c_int32), ("grid_blocks", C.c_int32), ("tracks_per_block", C.c_int32)]
+
+
+class nd_cmfd_options(C.Structure):
+    _fields_ = [("tol", C.c_double), ("max_outer", C.c_int32), ("inner_sweeps", C.c_int32), ("relax", C.c_double),
+                ("rel_tol", C.c_double), ("reserved", C.c_int32 * 2)]
+
+
+class nd_cmfd_stats(C.Structure):
+    _fields_ = [("k_sweep", C.c_double), ("k_eff", C.c_double), ("coarse_iters", C.c_int32), ("coarse_ok", C.c_int32)]
 
 
 class nd_microbench_result(C.Structure):
@@ -124,6 +138,8 @@ def lib():
                                                 C.c_void_p, C.POINTER(nd_trace_timing), C.POINTER(C.c_void_p)]
         L.nd_tracks_view.argtypes = [C.c_void_p, C.POINTER(nd_tracks_view_t)]
         L.nd_tracks_destroy.argtypes = [C.c_void_p]
+        L.nd_tracks_shard.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_void_p)]
+        L.nd_tally_reducer_set.argtypes = [C.c_void_p, ND_TALLY_REDUCE_FN, C.c_void_p]
         L.nd_workspace_bytes.argtypes = [C.POINTER(nd_problem_desc), C.POINTER(nd_options), C.POINTER(C.c_size_t)]
         L.nd_problem_create.argtypes = [C.POINTER(nd_problem_desc), C.POINTER(nd_options), C.c_void_p, C.c_size_t,
                                         C.c_void_p, C.POINTER(C.c_void_p)]
@@ -144,15 +160,20 @@ def lib():
         L.nd_cmfd_surfaces.argtypes = [C.POINTER(nd_problem_desc), C.c_int32, C.c_void_p, C.c_int32, C.POINTER(C.c_int32),
                                        C.c_void_p, C.c_void_p]
         L.nd_microbench.argtypes = [C.c_void_p, C.c_size_t, C.c_void_p, C.POINTER(nd_microbench_result)]
-        L.nd_sweep_currents.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p,
-                                        C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
-        L.nd_cmfd_collapse.argtypes = [C.c_void_p, C.c_void_p, C.c_int32] + [C.c_void_p] * 8
-        L.nd_cmfd_prolong.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
-        L.nd_cmfd_coarse_solve.argtypes = ([C.c_int32, C.c_int32] + [C.c_void_p] * 6 + [C.c_int32] + [C.c_void_p] * 5 +
-                                           [C.c_double, C.c_double, C.c_int32, C.POINTER(C.c_double), C.c_void_p,
-                                            C.POINTER(C.c_int32), C.c_void_p])
-        L.nd_cmfd_iteration.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
-                                        C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int32), C.c_void_p]
+        L.nd_cmfd_workspace_bytes.argtypes = [C.c_void_p, C.POINTER(nd_problem_desc), C.c_int32, C.c_void_p, C.c_int32,
+                                              C.POINTER(C.c_size_t)]
+        L.nd_cmfd_create.argtypes = [C.c_void_p, C.POINTER(nd_problem_desc), C.c_int32, C.c_void_p, C.c_int32, C.c_void_p,
+                                     C.c_void_p, C.c_void_p, C.POINTER(nd_cmfd_options), C.c_void_p, C.c_size_t, C.c_void_p,
+                                     C.POINTER(C.c_void_p)]
+        L.nd_cmfd_destroy.argtypes = [C.c_void_p]
+        L.nd_cmfd_iteration.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double), C.c_void_p, C.c_void_p]
+        L.nd_cmfd_sweep.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nd_cmfd_currents_get.argtypes = [C.c_void_p] * 5
+        L.nd_cmfd_collapse.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nd_cmfd_coarse_get.argtypes = [C.c_void_p] * 8
+        L.nd_cmfd_coarse_set.argtypes = [C.c_void_p] * 10
+        L.nd_cmfd_solve.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double), C.c_void_p, C.POINTER(C.c_int32), C.c_void_p]
+        L.nd_cmfd_prolong.argtypes = [C.c_void_p, C.c_void_p]
         L.nd_profile_enable.argtypes = [C.c_void_p, C.c_int32]
         L.nd_profile_read.argtypes = [C.c_void_p, C.POINTER(nd_profile)]
         L.nd_sweep_phases_get.argtypes = [C.c_void_p, C.c_void_p]
@@ -210,6 +231,19 @@ class Tracks:
         self.azim_phi = _np_view(view.azim_phi, (NH,), np.float64)
         self.azim_weight = _np_view(view.azim_weight, (NH,), np.float64)
         self.azim_spacing = _np_view(view.azim_spacing, (NH,), np.float64)
+        self.track_global = _np_view(view.track_global, (T,), np.int32)
+        self.is_shard = False
+
+    def shard(self, n_shards, shard):
+        """NEXT-2 (nd_tracks_shard): the tracks of one shard of the angle-pair partition, as a new Tracks object whose
+        `volume` holds the areas of the WHOLE laydown and `track_global` the ids in this object."""
+        h = C.c_void_p()
+        _check(lib().nd_tracks_shard(self._h, int(n_shards), int(shard), C.byref(h)), "nd_tracks_shard")
+        v = nd_tracks_view_t()
+        _check(lib().nd_tracks_view(h, C.byref(v)), "nd_tracks_view")
+        out = Tracks(h, v)
+        out.is_shard = True
+        return out
 
     def destroy(self):
         if self._h:
@@ -292,29 +326,12 @@ def nd_microbench(device="cuda:0", workspace_bytes=(1 << 30) + (2 << 20)):
     return {f[0]: getattr(r, f[0]) for f in nd_microbench_result._fields_ if f[0] != "reserved"}
 
 
-def nd_cmfd_coarse_solve(co, pair_lo, pair_hi, coupling, J_surf, J_vac, k0, tol=1e-13, max_outer=100000, stream=None):
-    """C-5..C-8 (nd.h): co = the dict nd_cmfd_collapse returns.  Returns (k, Phi_new [C][G], iterations)."""
-    def f8(a):
-        return np.ascontiguousarray(a, np.float64)
-    V, Phi, st, ss, nf, ch = (f8(co[k]) for k in ("V", "Phi", "sigt", "sigs", "nusf", "chi"))
-    n, G = Phi.shape
-    lo, hi = np.ascontiguousarray(pair_lo, np.int32), np.ascontiguousarray(pair_hi, np.int32)
-    cpl, Js, Jv = f8(coupling), f8(J_surf), f8(J_vac)
-    assert ss.shape == (n, G, G) and Jv.shape == (n, G) and Js.shape == (len(lo), G) and cpl.shape == (len(lo),)
-    k, it, out = C.c_double(), C.c_int32(), np.empty((n, G))
-    rc = lib().nd_cmfd_coarse_solve(n, G, V.ctypes.data, Phi.ctypes.data, st.ctypes.data, ss.ctypes.data, nf.ctypes.data,
-                                    ch.ctypes.data, len(lo), lo.ctypes.data, hi.ctypes.data, cpl.ctypes.data, Js.ctypes.data,
-                                    Jv.ctypes.data, float(k0), float(tol), int(max_outer), C.byref(k), out.ctypes.data,
-                                    C.byref(it), stream)
-    _check(rc, "nd_cmfd_coarse_solve")
-    return k.value, out, it.value
-
-
 class Problem:
     """Owner of an nd_problem handle and its torch workspace.  Methods mirror the C entry points."""
 
     def __init__(self, region_material, sigma_t, sigma_s, nu_sigma_f, chi, polar_sin, polar_weight, seg_offset,
-                 seg_region, seg_length, track_weight, link, track_azim=None, track_ends=None, exp_mode=ND_EXP_FAST,
+                 seg_region, seg_length, track_weight, link, track_azim=None, track_ends=None, region_volume=None,
+                 exp_mode=ND_EXP_FAST,
                  sweep_kernel=ND_SWEEP_AUTO, window_regions=0, block_warps=0, tile_segments=0,
                  delta_buffers=0, blocks_per_sm=0, tile_lag=0, q_copies=0, graph_mode=0, cmfd_stream=0, item_order=0, device="cuda:0"):
         import torch
@@ -332,6 +349,9 @@ class Problem:
             keep["ta"] = np.ascontiguousarray(track_azim, np.int32)
             keep["te"] = np.ascontiguousarray(track_ends, np.float64)
             geo = [keep["ta"].ctypes.data, keep["te"].ctypes.data]
+        if region_volume is not None:
+            keep["rv"] = np.ascontiguousarray(region_volume, np.float64)
+            geo = geo + [keep["rv"].ctypes.data]
         self.R, (self.M, self.G), self.P, self.T = len(keep["rm"]), keep["st"].shape, len(keep["ps"]), len(keep["tw"])
         d = nd_problem_desc(self.R, self.M, self.G, self.P, self.T, *[keep[k].ctypes.data for k in
                             ("rm", "st", "ss", "nf", "ch", "ps", "pw", "so", "sr", "sl", "tw", "lk")], *geo)
@@ -351,6 +371,28 @@ class Problem:
 
     def _stream(self):
         return C.c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream)
+
+    def nd_tally_reducer_set(self, fn):
+        """NEXT-2 (nd.h): fn(tally) is called after every sweep with a torch FP64 tensor that ALIASES the problem's padded
+        tally [R * Gs] and must replace it, in place and in stream order on the current stream, by the sum over the shards
+        (e.g. torch.distributed.all_reduce).  fn = None removes the reducer."""
+        if fn is None:
+            self._reduce_cb = None
+            _check(lib().nd_tally_reducer_set(self._h, C.cast(None, ND_TALLY_REDUCE_FN), None), "nd_tally_reducer_set")
+            return
+        t, base = self.torch, self.workspace.data_ptr()
+
+        def cb(_user, ptr, n, _stream):
+            try:
+                off = int(ptr) - base
+                fn(self.workspace[off:off + 8 * int(n)].view(t.float64))
+                return 0
+            except Exception:      # no exception may cross the C boundary
+                import traceback
+                traceback.print_exc()
+                return 1
+        self._reduce_cb = ND_TALLY_REDUCE_FN(cb)      # kept alive as long as the library may call it
+        _check(lib().nd_tally_reducer_set(self._h, self._reduce_cb, None), "nd_tally_reducer_set")
 
     def destroy(self):
         if getattr(self, "_h", None):
@@ -436,53 +478,11 @@ class Problem:
         _check(lib().nd_tally_get(self._h, out.data_ptr(), self._stream()), "nd_tally_get")
         return out
 
-    def nd_sweep_currents(self, d_Q, cell, n_cells, pair_lo, pair_hi):
-        """C-3 (nd.h): returns HOST arrays J_surf [n_pairs][G], J_vac [n_cells][G], J_ref [n_cells][G]."""
-        t = self.torch
-        assert d_Q.dtype == t.float64 and d_Q.is_cuda and d_Q.is_contiguous() and d_Q.numel() == self.R * self.G
-        cell = np.ascontiguousarray(cell, np.int32)
-        lo, hi = np.ascontiguousarray(pair_lo, np.int32), np.ascontiguousarray(pair_hi, np.int32)
-        assert cell.shape == (self.R,) and lo.shape == hi.shape and lo.ndim == 1
-        Js, Jv, Jr = np.empty((len(lo), self.G)), np.empty((int(n_cells), self.G)), np.empty((int(n_cells), self.G))
-        _check(lib().nd_sweep_currents(self._h, d_Q.data_ptr(), int(n_cells), cell.ctypes.data, len(lo), lo.ctypes.data,
-                                       hi.ctypes.data, Js.ctypes.data, Jv.ctypes.data, Jr.ctypes.data, self._stream()),
-               "nd_sweep_currents")
-        return Js, Jv, Jr
-
-    def nd_cmfd_collapse(self, cell, n_cells, d_phi=None):
-        """C-4 (nd.h): returns HOST arrays as a dict V, Phi, sigt, sigs [C][g][g'], nusf, chi."""
-        cell = np.ascontiguousarray(cell, np.int32)
-        assert cell.shape == (self.R,)
-        if d_phi is not None:
-            t = self.torch
-            assert d_phi.dtype == t.float64 and d_phi.is_cuda and d_phi.is_contiguous() and d_phi.numel() == self.R * self.G
-        n, G = int(n_cells), self.G
-        out = dict(V=np.empty(n), Phi=np.empty((n, G)), sigt=np.empty((n, G)), sigs=np.empty((n, G, G)),
-                   nusf=np.empty((n, G)), chi=np.empty((n, G)))
-        _check(lib().nd_cmfd_collapse(self._h, d_phi.data_ptr() if d_phi is not None else None, n, cell.ctypes.data,
-                                      out["V"].ctypes.data, out["Phi"].ctypes.data, out["sigt"].ctypes.data,
-                                      out["sigs"].ctypes.data, out["nusf"].ctypes.data, out["chi"].ctypes.data,
-                                      self._stream()), "nd_cmfd_collapse")
-        return out
-
-    def nd_cmfd_iteration(self, cell, n_cells, pair_lo, pair_hi, coupling):
-        """Algorithm 1 as one call (nd.h).  Returns dict k_eff, k_sweep, coarse_iters."""
-        cell = np.ascontiguousarray(cell, np.int32)
-        lo, hi = np.ascontiguousarray(pair_lo, np.int32), np.ascontiguousarray(pair_hi, np.int32)
-        cpl = np.ascontiguousarray(coupling, np.float64)
-        assert cell.shape == (self.R,) and lo.shape == hi.shape == cpl.shape and lo.ndim == 1
-        ks, k, it = C.c_double(), C.c_double(), C.c_int32()
-        _check(lib().nd_cmfd_iteration(self._h, int(n_cells), cell.ctypes.data, len(lo), lo.ctypes.data, hi.ctypes.data,
-                                       cpl.ctypes.data, C.byref(ks), C.byref(k), C.byref(it), self._stream()),
-               "nd_cmfd_iteration")
-        return dict(k_eff=k.value, k_sweep=ks.value, coarse_iters=it.value)
-
-    def nd_cmfd_prolong(self, cell, n_cells, ratio, k_eff):
-        cell = np.ascontiguousarray(cell, np.int32)
-        ratio = np.ascontiguousarray(ratio, np.float64)
-        assert cell.shape == (self.R,) and ratio.shape == (int(n_cells), self.G)
-        _check(lib().nd_cmfd_prolong(self._h, int(n_cells), cell.ctypes.data, ratio.ctypes.data, float(k_eff),
-                                     self._stream()), "nd_cmfd_prolong")
+    def nd_cmfd_create(self, seg_offset, seg_region, link, cell, n_cells, pair_lo, pair_hi, coupling, tol=0.0, max_outer=0,
+                       inner_sweeps=0, relax=0.0, rel_tol=0.0):
+        """NEXT-3 (nd.h): a CMFD plan on this problem.  seg_offset / seg_region / link: the arrays the problem was created from."""
+        return Cmfd(self, seg_offset, seg_region, link, cell, n_cells, pair_lo, pair_hi, coupling, tol, max_outer, inner_sweeps, relax,
+                    rel_tol)
 
     def nd_profile_enable(self, on=True):
         _check(lib().nd_profile_enable(self._h, int(on)), "nd_profile_enable")
@@ -501,6 +501,101 @@ class Problem:
         inf = nd_problem_info()
         _check(lib().nd_problem_info_get(self._h, C.byref(inf)), "nd_problem_info_get")
         return {f[0]: getattr(inf, f[0]) for f in nd_problem_info._fields_ if f[0] != "reserved"}
+
+
+class Cmfd:
+    """Owner of an nd_cmfd plan and its torch workspace (include/nd.h "NEXT-3").  Methods mirror the C entry points."""
+
+    def __init__(self, prob, seg_offset, seg_region, link, cell, n_cells, pair_lo, pair_hi, coupling, tol, max_outer,
+                 inner_sweeps, relax, rel_tol=0.0):
+        t = prob.torch
+        self.prob, self.n_cells, self.G = prob, int(n_cells), prob.G
+        keep = dict(so=np.ascontiguousarray(seg_offset, np.int64), sr=np.ascontiguousarray(seg_region, np.int32),
+                    lk=np.ascontiguousarray(link, np.int32), cell=np.ascontiguousarray(cell, np.int32),
+                    lo=np.ascontiguousarray(pair_lo, np.int32), hi=np.ascontiguousarray(pair_hi, np.int32),
+                    cp=np.ascontiguousarray(coupling, np.float64))
+        assert keep["cell"].shape == (prob.R,) and keep["lo"].shape == keep["hi"].shape == keep["cp"].shape
+        self.n_pairs = len(keep["lo"])
+        d = nd_problem_desc()
+        d.n_regions, d.n_tracks = prob.R, prob.T
+        d.track_seg_offset, d.seg_region, d.link = keep["so"].ctypes.data, keep["sr"].ctypes.data, keep["lk"].ctypes.data
+        nbytes = C.c_size_t()
+        _check(lib().nd_cmfd_workspace_bytes(prob._h, C.byref(d), self.n_cells, keep["cell"].ctypes.data, self.n_pairs,
+                                             C.byref(nbytes)), "nd_cmfd_workspace_bytes")
+        opt = nd_cmfd_options(float(tol), int(max_outer), int(inner_sweeps), float(relax), float(rel_tol))
+        with t.cuda.device(prob.device):
+            self.workspace = t.empty(int(nbytes.value) + 256, dtype=t.uint8, device=prob.device)
+            ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+            h = C.c_void_p()
+            _check(lib().nd_cmfd_create(prob._h, C.byref(d), self.n_cells, keep["cell"].ctypes.data, self.n_pairs,
+                                        keep["lo"].ctypes.data, keep["hi"].ctypes.data, keep["cp"].ctypes.data, C.byref(opt),
+                                        C.c_void_p(ptr), int(nbytes.value), prob._stream(), C.byref(h)), "nd_cmfd_create")
+        self._h = h
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().nd_cmfd_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def nd_cmfd_iteration(self, n_iters, want_stats=False):
+        k = C.c_double()
+        stats = (nd_cmfd_stats * max(1, n_iters))() if want_stats else None
+        _check(lib().nd_cmfd_iteration(self._h, int(n_iters), C.byref(k), C.cast(stats, C.c_void_p) if stats is not None else None,
+                                       self.prob._stream()), "nd_cmfd_iteration")
+        out = dict(k_eff=k.value)
+        if want_stats:
+            out["stats"] = [dict(k_sweep=s.k_sweep, k_eff=s.k_eff, coarse_iters=s.coarse_iters, coarse_ok=s.coarse_ok)
+                            for s in stats[:n_iters]]
+        return out
+
+    def nd_cmfd_sweep(self, d_Q, d_phi_out=None):
+        t = self.prob.torch
+        assert d_Q.dtype == t.float64 and d_Q.is_cuda and d_Q.is_contiguous() and d_Q.numel() == self.prob.R * self.G
+        if d_phi_out is None:
+            d_phi_out = t.empty((self.prob.R, self.G), dtype=t.float64, device=self.prob.device)
+        _check(lib().nd_cmfd_sweep(self._h, d_Q.data_ptr(), d_phi_out.data_ptr(), self.prob._stream()), "nd_cmfd_sweep")
+        return d_phi_out
+
+    def nd_cmfd_currents_get(self):
+        Js, Jv, Jr = np.empty((self.n_pairs, self.G)), np.empty((self.n_cells, self.G)), np.empty((self.n_cells, self.G))
+        _check(lib().nd_cmfd_currents_get(self._h, Js.ctypes.data, Jv.ctypes.data, Jr.ctypes.data, self.prob._stream()),
+               "nd_cmfd_currents_get")
+        return Js, Jv, Jr
+
+    def nd_cmfd_collapse(self, d_phi=None):
+        _check(lib().nd_cmfd_collapse(self._h, d_phi.data_ptr() if d_phi is not None else None, self.prob._stream()), "nd_cmfd_collapse")
+
+    def nd_cmfd_coarse_get(self):
+        n, G = self.n_cells, self.G
+        out = dict(V=np.empty(n), Phi=np.empty((n, G)), sigt=np.empty((n, G)), sigs=np.empty((n, G, G)), nusf=np.empty((n, G)),
+                   chi=np.empty((n, G)))
+        _check(lib().nd_cmfd_coarse_get(self._h, out["V"].ctypes.data, out["Phi"].ctypes.data, out["sigt"].ctypes.data,
+                                        out["sigs"].ctypes.data, out["nusf"].ctypes.data, out["chi"].ctypes.data,
+                                        self.prob._stream()), "nd_cmfd_coarse_get")
+        return out
+
+    def nd_cmfd_coarse_set(self, co, J_surf, J_vac):
+        f8 = lambda a: np.ascontiguousarray(a, np.float64)
+        V, Phi, st, ss, nf, ch, Js, Jv = (f8(a) for a in (co["V"], co["Phi"], co["sigt"], co["sigs"], co["nusf"], co["chi"], J_surf, J_vac))
+        n, G = self.n_cells, self.G
+        assert Phi.shape == (n, G) and ss.shape == (n, G, G) and Js.shape == (self.n_pairs, G) and Jv.shape == (n, G)
+        _check(lib().nd_cmfd_coarse_set(self._h, V.ctypes.data, Phi.ctypes.data, st.ctypes.data, ss.ctypes.data, nf.ctypes.data,
+                                        ch.ctypes.data, Js.ctypes.data, Jv.ctypes.data, self.prob._stream()), "nd_cmfd_coarse_set")
+
+    def nd_cmfd_solve(self, k0, allow=()):
+        k, it, out = C.c_double(), C.c_int32(), np.empty((self.n_cells, self.G))
+        rc = lib().nd_cmfd_solve(self._h, float(k0), C.byref(k), out.ctypes.data, C.byref(it), self.prob._stream())
+        _check(rc, "nd_cmfd_solve", allow=allow)
+        return k.value, out, it.value, rc
+
+    def nd_cmfd_prolong(self):
+        _check(lib().nd_cmfd_prolong(self._h, self.prob._stream()), "nd_cmfd_prolong")
 
 
 def nd_swath_stream_build(region_material, n_materials, seg_offset, seg_region, seg_length, tracks_per_swath,
@@ -541,4 +636,5 @@ def nd_problem_create(xs, polar_sin, polar_weight, region_material, tracks, **op
     """Convenience: build a Problem from a cross-section set (arrays sigma_t, sigma_s, nu_sigma_f, chi) and Tracks."""
     return Problem(region_material, xs.sigma_t, xs.sigma_s, xs.nu_sigma_f, xs.chi, polar_sin, polar_weight,
                    tracks.seg_offset, tracks.seg_region, tracks.seg_length, tracks.track_weight, tracks.link,
-                   track_azim=tracks.track_azim, track_ends=tracks.ends, **options)
+                   track_azim=tracks.track_azim, track_ends=tracks.ends,
+                   region_volume=tracks.volume if getattr(tracks, "is_shard", False) else None, **options)

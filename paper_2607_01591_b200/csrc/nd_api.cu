@@ -85,6 +85,7 @@ struct SwathConfig {
     int LPT = 0, warps = 0, ndbuf = 1, blocks_per_sm = 1;
     bool tight = false;                                   // register-capped kernel variant (more than 512 resident threads per SM)
     int head_cap = 0, rec_cap = 0, off_sigt = 0, off_q = 0, off_dbuf = 0, off_head = 0, off_rec = 0, smem_bytes = 0;
+    int x_cap = 0, off_x = 0, off_w = 0;                  // nd_options.cmfd_stream: crossing-list ring and the slots' W rows
     int64_t max_tiles = 0, max_swaths = 0;
     size_t max_blob = 0;
 };
@@ -111,7 +112,7 @@ SwathConfig make_swath_config_q(const Dims& d, const nd_options& opt, int q_copi
         const int NT = w * 32 / c.LPT / NC * NC;               // slots are packed over the lanes of the whole block
         if (NT < 1 || (int64_t)NT * Kmax > 65535) return false;
         if (Lmax < 16) Lmax = 16;
-        {   // the kernel's fastdiv works below 2^16: regions x (pieces per staged row, group pairs per row)
+        {   // the kernel's fastdiv works below 2^16: regions x pieces per staged row
             const int per_region = std::max(d.Gs / 2, NC * (d.Gs / 4));
             if (Lmax > 65535 / per_region) Lmax = 65535 / per_region;
         }
@@ -128,6 +129,13 @@ SwathConfig make_swath_config_q(const Dims& d, const nd_options& opt, int q_copi
         c.off_head = c.off_dbuf + pad128(c.ndbuf * (NT * Kmax + 1) * row_bytes);   // + the spare row of the null record
         c.off_rec = c.off_head + pad128(ndk::kSwathHeadBufs * c.head_cap);
         c.smem_bytes = c.off_rec + ndk::kSwathRecBufs * c.rec_cap;
+        if (opt.cmfd_stream) {   // CMFD current tally in the sweep kernel: W per slot + a ring of crossing lists
+            c.sp.keep_slot_start = true;
+            c.x_cap = (8 * (1 + NT * Kmax) + 15) / 16 * 16;
+            c.off_w = pad128(c.smem_bytes);
+            c.off_x = c.off_w + pad128(NT * row_bytes);
+            c.smem_bytes = c.off_x + ndk::kSwathXBufs * c.x_cap;
+        }
         return true;
     };
     // Defaults (measured, profiles/): occupancy beats tile length once a tile holds >= 8 segments per track.  Aim at
@@ -214,7 +222,8 @@ Layout make_layout(const Dims& d, int max_stats, const SwathConfig& sc, int kern
     const size_t RG = (size_t)d.R * d.G, RGs = (size_t)d.R * d.Gs, NPSI = (size_t)d.T * 2 * d.P * d.Gs;
     // the v0 SoA stream is read by the atomic kernel (and the CMFD current tally: nd_options.cmfd_stream); the tiled kernels
     // carry their own chunk stream
-    const size_t soa = kernel == ND_SWEEP_ATOMIC || keep_soa ? (size_t)d.Spad : 4;
+    (void)keep_soa;
+    const size_t soa = kernel == ND_SWEEP_ATOMIC ? (size_t)d.Spad : 4;
     L.seg_rm = bump(c, sizeof(uint32_t) * soa);
     L.seg_len = bump(c, sizeof(float) * soa);
     L.trk_off = bump(c, sizeof(int64_t) * ((size_t)d.T + 1));
@@ -310,6 +319,11 @@ struct nd_problem {
     // host copies
     std::vector<double> h_vol;
     std::vector<int32_t> h_entry_region;   // [2T] first region of chain (t, d), -1 for an empty track (C-9)
+    // nd_options.cmfd_stream: what nd_cmfd_create needs to place the coarse-surface crossings into the tiles
+    std::vector<int32_t> h_swath_track;    // [n_swaths][NT]
+    std::vector<int64_t> h_swath_tile0;    // [n_swaths+1]
+    std::vector<uint16_t> h_slot_start;    // [n_tiles][NT+1]
+    nd_cmfd* cmfd_sweep = nullptr;         // set while a sweep has to tally the currents of this plan (C-3)
     float c[ndk::kMaxPolar]{}, inv_sin[ndk::kMaxPolar]{}, wp[ndk::kMaxPolar]{};
     // profiling
     bool profile = false, phase_profile = false;
@@ -317,6 +331,9 @@ struct nd_problem {
     std::vector<EventPair> ev_pool;
     size_t ev_used = 0;
     int64_t kernels_launched = 0;
+    // NEXT-2: called on the tally of every sweep before it is turned into a flux (all-reduce over the shards)
+    nd_tally_reduce_fn reduce_fn = nullptr;
+    void* reduce_user = nullptr;
     // CUDA graph of two power iterations (phi_cur returns to the buffer it started in), see nd_power_iteration
     cudaGraphExec_t iter_graph = nullptr;
     cudaStream_t cap_stream = nullptr;        // capture only; replays run on the caller's stream
@@ -325,6 +342,9 @@ struct nd_problem {
 };
 
 namespace {
+
+void cmfd_fill_sweep_params(const nd_cmfd* c, ndk::SwathParams* prm);   // nd_cmfd_api.cuh
+nd_status cmfd_end_currents(nd_cmfd* c, const double* scale_div, cudaStream_t st);
 
 inline cudaStream_t as_stream(void* s) { return reinterpret_cast<cudaStream_t>(s); }
 
@@ -380,7 +400,9 @@ nd_status launch_swath_p(nd_problem* p, const ndk::SwathParams& prm, cudaStream_
     const bool expm1 = p->opt.exp_mode == ND_EXP_EXPM1;
     const bool tight = c.tight && !expm1;   // the expm1f cross-check path keeps the roomy register budget
     const bool prof = p->phase_profile && !expm1;   // instrumented build: clock64 marks around the phases of a tile
+    const bool cur = prm.xblob != nullptr;          // CMFD: the sweep also tallies the coarse-surface currents (fast-exp path only)
     auto kern = expm1 ? ndk::k_sweep_swath<P, 1, 0, 0>
+                : cur ? (tight ? ndk::k_sweep_swath<P, 0, 1, 0, 1> : ndk::k_sweep_swath<P, 0, 0, 0, 1>)
                       : (tight ? (prof ? ndk::k_sweep_swath<P, 0, 1, 1> : ndk::k_sweep_swath<P, 0, 1, 0>)
                                : (prof ? ndk::k_sweep_swath<P, 0, 0, 1> : ndk::k_sweep_swath<P, 0, 0, 0>));
     ND_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes));
@@ -411,6 +433,8 @@ nd_status launch_swath(nd_problem* p, const double* scale_div, cudaStream_t st)
     prm.magic_nq = ndk::fastdiv_magic((uint32_t)(d.Gs / 4));
     prm.magic_np = ndk::fastdiv_magic((uint32_t)(d.Gs / 2));
     prm.phase = p->phase;
+    prm.x_cap = c.x_cap; prm.off_x = c.off_x; prm.off_w = c.off_w;
+    if (p->cmfd_sweep) cmfd_fill_sweep_params(p->cmfd_sweep, &prm);
     ND_CUDA(cudaMemsetAsync(p->counter, 0, sizeof(int), st));
     switch (d.P) {
     case 1: return launch_swath_p<1>(p, prm, st);
@@ -494,8 +518,16 @@ nd_status launch_sweep(nd_problem* p, const double* scale_div, cudaStream_t st, 
                                                                              p->wp[1], p->wp[2], p->wp[3]);
         ND_LAUNCH_CHECK(p);
     }
+    if (p->cmfd_sweep) {   // C-3: the chain-end terms need what entered and what left, before the swap overwrites the former
+        const nd_status rcc = cmfd_end_currents(p->cmfd_sweep, scale_div, st);
+        if (rcc != ND_OK) return rcc;
+    }
     ndk::k_link_swap<<<grid_for(n, 256, 8 * p->n_sm), 256, 0, st>>>(p->psi_out, p->psi_in, p->link_src, 2 * (int64_t)d.T, PG);
     ND_LAUNCH_CHECK(p);
+    if (p->reduce_fn) {   // NEXT-2: the shards' tallies are summed before any of them forms its flux
+        if (p->reduce_fn(p->reduce_user, p->tally, (int64_t)d.R * d.Gs, st) != 0)
+            return nd_fail(ND_ERR_STATE, "the tally reducer (nd_tally_reducer_set) reported a failure");
+    }
     return ND_OK;
 }
 
@@ -619,7 +651,7 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         p = new nd_problem();
         p->d = d; p->opt = opt; p->L = L; p->ws = static_cast<char*>(device_workspace);
         // ---- A1: pack the segment stream (SoA, every track run padded to a multiple of 4 = 16 bytes) ----
-        const bool soa = kernel == ND_SWEEP_ATOMIC || opt.cmfd_stream != 0;
+        const bool soa = kernel == ND_SWEEP_ATOMIC;
         p->has_soa = soa;
         h_rm.assign(soa ? (size_t)d.Spad : 4, 0u);
         h_len.assign(soa ? (size_t)d.Spad : 4, 0.f);
@@ -649,6 +681,15 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
             while (o % 4 != 0) { if (soa) { h_rm[o] = last; h_len[o] = 0.f; } ++o; } // zero-length segments are exact no-ops
         }
         h_off[d.T] = o;
+        if (desc->region_volume) {   // a shard of an angle-pair partition: the areas of the whole laydown (nd_tracks_shard)
+            for (int r = 0; r < d.R; ++r) {
+                if (!(desc->region_volume[r] >= 0.0) || !std::isfinite(desc->region_volume[r])) {
+                    delete p;
+                    return nd_fail(ND_ERR_INVALID, "region_volume must be finite and >= 0");
+                }
+                p->h_vol[(size_t)r] = desc->region_volume[r];
+            }
+        }
     } catch (const std::bad_alloc&) {
         delete p;
         return nd_fail(ND_ERR_NOMEM, "nd_problem_create: out of host memory");
@@ -747,6 +788,11 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         p->mean_regions_per_tile = swaths.mean_regions_per_tile;
         p->mean_segments_per_tile = swaths.mean_segments_per_tile;
         p->lockstep_efficiency = swaths.lockstep_efficiency;
+        if (opt.cmfd_stream) {
+            p->h_swath_track = swaths.swath_track;
+            p->h_swath_tile0 = swaths.swath_tile0;
+            p->h_slot_start.swap(swaths.slot_start);
+        }
         ND_CUDA_P(cudaMemcpyAsync(p->blob, swaths.blob.data(), swaths.blob.size(), cudaMemcpyHostToDevice, st));
         static_assert(sizeof(NdSwathTileRef) == sizeof(uint2), "tile reference layout");
         ND_CUDA_P(cudaMemcpyAsync(p->tile_ref, swaths.tile_ref.data(), sizeof(NdSwathTileRef) * swaths.tile_ref.size(), cudaMemcpyHostToDevice, st));
@@ -850,7 +896,8 @@ extern "C" nd_status nd_power_iteration(nd_problem* p, int32_t max_iters, double
         sp.phi = p->phi_cur;
         nd_status rc = launch_source(p, sp, st);
         if (rc != ND_OK) return rc;
-        const bool balance = slot != nullptr && stats != nullptr;   // leakage and the balance residual are only formed for stats
+        // leakage and the balance residual are only formed for stats, and only when the tally is this problem's own
+        const bool balance = slot != nullptr && stats != nullptr && !p->reduce_fn;
         rc = launch_sweep(p, p->scalars + ndk::SC_F, st, balance);
         if (rc != ND_OK) return rc;
         int grid = 0;
@@ -864,7 +911,8 @@ extern "C" nd_status nd_power_iteration(nd_problem* p, int32_t max_iters, double
     };
     // Fixed-count calls replay a CUDA graph of TWO iterations (after two, phi_cur is back in the buffer it started in, so
     // one graph serves every pair); an odd iteration and anything with tolerances, stats or profiling is launched plainly.
-    const bool graph_ok = !use_tol && !stats && !p->profile && !p->phase_profile && p->opt.graph_mode == 0 && max_iters >= 4;
+    const bool graph_ok = !use_tol && !stats && !p->profile && !p->phase_profile && p->opt.graph_mode == 0 && max_iters >= 4 &&
+                          !p->reduce_fn;   // a host callback cannot be replayed from a graph
     if (graph_ok) {
         if (p->iter_graph && p->iter_graph_phi != p->phi_cur) {   // an odd number of plain iterations since the capture
             nd_status rc = one_iteration(nullptr, st);
@@ -954,6 +1002,14 @@ extern "C" nd_status nd_power_iteration(nd_problem* p, int32_t max_iters, double
 // ------------------------------------------------------------------------------------------------
 // state access
 // ------------------------------------------------------------------------------------------------
+extern "C" nd_status nd_tally_reducer_set(nd_problem* p, nd_tally_reduce_fn fn, void* user)
+{
+    if (!p) return nd_fail(ND_ERR_NULL, "nd_tally_reducer_set: NULL problem");
+    p->reduce_fn = fn;
+    p->reduce_user = user;
+    return ND_OK;
+}
+
 extern "C" nd_status nd_state_reset(nd_problem* p, void* cuda_stream)
 {
     if (!p) return nd_fail(ND_ERR_NULL, "nd_state_reset: NULL problem");
@@ -1035,349 +1091,7 @@ extern "C" nd_status nd_tally_get(nd_problem* p, double* d_tally_out, void* cuda
     return ND_OK;
 }
 
-namespace {
-
-template <int P>
-void launch_currents_p(const nd_problem* p, const ndk::CurrentParams& cp, int grid, cudaStream_t st)
-{
-    const bool two = p->d.G > 32;   // a lane carries two groups through one walk
-    if (p->opt.exp_mode == ND_EXP_EXPM1) {
-        if (two) ndk::k_sweep_currents<P, 1, 2><<<grid, 256, 0, st>>>(cp);
-        else ndk::k_sweep_currents<P, 1, 1><<<grid, 256, 0, st>>>(cp);
-    } else {
-        if (two) ndk::k_sweep_currents<P, 0, 2><<<grid, 256, 0, st>>>(cp);
-        else ndk::k_sweep_currents<P, 0, 1><<<grid, 256, 0, st>>>(cp);
-    }
-}
-
-} // namespace
-
-// NEXT-3, C-3: see nd.h.  Not on the hot path yet: it allocates its scratch with cudaMalloc, runs the
-// simple one-warp-per-chain sweep and synchronises the stream before it returns.
-extern "C" nd_status nd_sweep_currents(nd_problem* p, const double* d_Q, int32_t n_cells, const int32_t* cell,
-                                       int32_t n_pairs, const int32_t* pair_lo, const int32_t* pair_hi, double* J_surf,
-                                       double* J_vac, double* J_ref, void* cuda_stream)
-{
-    if (!p || !d_Q || !cell || !J_vac || !J_ref || (n_pairs > 0 && (!pair_lo || !pair_hi || !J_surf)))
-        return nd_fail(ND_ERR_NULL, "nd_sweep_currents: NULL argument");
-    if (n_cells < 1 || n_pairs < 0) return nd_fail(ND_ERR_INVALID, "nd_sweep_currents: n_cells must be >= 1 and n_pairs >= 0");
-    if (!p->has_soa)
-        return nd_fail(ND_ERR_STATE, "nd_sweep_currents: needs a problem created with sweep_kernel = ND_SWEEP_ATOMIC or "
-                                     "nd_options.cmfd_stream = 1 (the current tally reads the SoA segment stream)");
-    const Dims& d = p->d;
-    cudaStream_t st = as_stream(cuda_stream);
-    for (int64_t r = 0; r < d.R; ++r)
-        if (cell[r] < 0 || cell[r] >= n_cells) return nd_fail(ND_ERR_RANGE, "nd_sweep_currents: cell[r] out of [0, n_cells)");
-    std::vector<std::pair<int64_t, int32_t>> keyed;
-    std::vector<int64_t> h_key;
-    std::vector<int32_t> h_idx;
-    try {
-        keyed.reserve((size_t)n_pairs);
-        for (int32_t s = 0; s < n_pairs; ++s) {
-            if (pair_lo[s] < 0 || pair_hi[s] >= n_cells || pair_lo[s] >= pair_hi[s])
-                return nd_fail(ND_ERR_RANGE, "nd_sweep_currents: a surface needs 0 <= lo < hi < n_cells");
-            keyed.emplace_back((int64_t)pair_lo[s] * n_cells + pair_hi[s], s);
-        }
-        std::sort(keyed.begin(), keyed.end());
-        h_key.resize((size_t)n_pairs + 1);
-        h_idx.resize((size_t)n_pairs + 1);
-        for (int32_t s = 0; s < n_pairs; ++s) {
-            if (s > 0 && keyed[s].first == keyed[s - 1].first) return nd_fail(ND_ERR_INVALID, "nd_sweep_currents: a surface is listed twice");
-            h_key[s] = keyed[s].first;
-            h_idx[s] = keyed[s].second;
-        }
-    } catch (const std::bad_alloc&) {
-        return nd_fail(ND_ERR_NOMEM, "nd_sweep_currents: out of host memory");
-    }
-    // scratch: [J_surf | J_vac | J_ref] FP64, pair keys, q, cell, link_fwd, entry_cell, pair index, flag
-    const size_t nJs = (size_t)n_pairs * d.G, nJc = (size_t)n_cells * d.G, nE = 2 * (size_t)d.T;
-    auto up = [](size_t b) { return (b + 255) / 256 * 256; };
-    const size_t oJ = 0, oKey = oJ + up(sizeof(double) * (nJs + 2 * nJc)), oQ = oKey + up(sizeof(int64_t) * ((size_t)n_pairs + 1)),
-                 oCell = oQ + up(sizeof(float) * (size_t)d.R * d.Gs), oFwd = oCell + up(sizeof(int32_t) * (size_t)d.R),
-                 oEnt = oFwd + up(sizeof(int32_t) * nE), oIdx = oEnt + up(sizeof(int32_t) * nE),
-                 oFlag = oIdx + up(sizeof(int32_t) * ((size_t)n_pairs + 1)), total = oFlag + 256;
-    char* buf = nullptr;
-    ND_CUDA(cudaMalloc(&buf, total));
-    struct Free { char* b; ~Free() { cudaFree(b); } } guard{buf};
-    double* dJ = (double*)(buf + oJ);
-    int* d_flag = (int*)(buf + oFlag);
-    ndk::CurrentParams cp{};
-    ndk::SweepParams& prm = cp.sw;
-    prm.seg_rm = p->seg_rm; prm.seg_len = p->seg_len; prm.trk_off = p->trk_off; prm.trk_w = p->trk_w;
-    prm.q = (float*)(buf + oQ); prm.sigt = p->sigt_f; prm.tally = nullptr;
-    prm.psi_in = p->psi_in; prm.psi_out = nullptr; prm.scale_div = p->scalars + ndk::SC_ONE;
-    prm.T = d.T; prm.G = d.G; prm.Gs = d.Gs;
-    for (int i = 0; i < ndk::kMaxPolar; ++i) { prm.c[i] = p->c[i]; prm.inv_sin[i] = p->inv_sin[i]; prm.wp[i] = p->wp[i]; }
-    cp.cell = (int32_t*)(buf + oCell); cp.link_fwd = (int32_t*)(buf + oFwd); cp.entry_cell = (int32_t*)(buf + oEnt);
-    cp.pair_key = (int64_t*)(buf + oKey); cp.pair_idx = (int32_t*)(buf + oIdx);
-    cp.J_surf = dJ; cp.J_vac = dJ + nJs; cp.J_ref = dJ + nJs + nJc; cp.missing = d_flag;
-    cp.n_pairs = n_pairs; cp.n_cells = n_cells;
-    cp.lanes_per_chain = 32;
-    while (cp.lanes_per_chain / 2 >= d.G) cp.lanes_per_chain /= 2;
-    ND_CUDA(cudaMemsetAsync(dJ, 0, sizeof(double) * (nJs + 2 * nJc), st));
-    ND_CUDA(cudaMemsetAsync(d_flag, 0, sizeof(int), st));
-    ND_CUDA(cudaMemsetAsync(buf + oFwd, 0xff, sizeof(int32_t) * nE, st));
-    ND_CUDA(cudaMemcpyAsync(buf + oCell, cell, sizeof(int32_t) * (size_t)d.R, cudaMemcpyHostToDevice, st));
-    if (n_pairs > 0) {
-        ND_CUDA(cudaMemcpyAsync(buf + oKey, h_key.data(), sizeof(int64_t) * (size_t)n_pairs, cudaMemcpyHostToDevice, st));
-        ND_CUDA(cudaMemcpyAsync(buf + oIdx, h_idx.data(), sizeof(int32_t) * (size_t)n_pairs, cudaMemcpyHostToDevice, st));
-    }
-    ndk::k_reduced_q<<<grid_for((int64_t)d.R * d.Gs, 256, 8 * p->n_sm), 256, 0, st>>>(d_Q, p->reg_mat, p->sigt, (float*)(buf + oQ), d.R, d.G, d.Gs);
-    ND_LAUNCH_CHECK(p);
-    ndk::k_link_forward<<<grid_for((int64_t)nE, 256, 8 * p->n_sm), 256, 0, st>>>(p->link_src, (int32_t*)(buf + oFwd), (int64_t)nE);
-    ND_LAUNCH_CHECK(p);
-    ndk::k_entry_cell<<<grid_for((int64_t)nE, 256, 8 * p->n_sm), 256, 0, st>>>(p->seg_rm, p->trk_off, cp.cell, (int32_t*)(buf + oEnt), (int64_t)nE);
-    ND_LAUNCH_CHECK(p);
-    const int grid = grid_for((int64_t)nE * cp.lanes_per_chain, 256, 16 * p->n_sm);
-    switch (d.P) {
-    case 1: launch_currents_p<1>(p, cp, grid, st); break;
-    case 2: launch_currents_p<2>(p, cp, grid, st); break;
-    case 3: launch_currents_p<3>(p, cp, grid, st); break;
-    default: launch_currents_p<4>(p, cp, grid, st); break;
-    }
-    ND_LAUNCH_CHECK(p);
-    int flag = 0;
-    if (nJs) ND_CUDA(cudaMemcpyAsync(J_surf, cp.J_surf, sizeof(double) * nJs, cudaMemcpyDeviceToHost, st));
-    ND_CUDA(cudaMemcpyAsync(J_vac, cp.J_vac, sizeof(double) * nJc, cudaMemcpyDeviceToHost, st));
-    ND_CUDA(cudaMemcpyAsync(J_ref, cp.J_ref, sizeof(double) * nJc, cudaMemcpyDeviceToHost, st));
-    ND_CUDA(cudaMemcpyAsync(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
-    ND_CUDA(cudaStreamSynchronize(st));
-    if (flag) return nd_fail(ND_ERR_INVALID, "nd_sweep_currents: a track crosses between two coarse cells that are not a listed surface");
-    return ND_OK;
-}
-
-namespace {
-
-struct DeviceScratch {   // call-local device memory of the CMFD entry points (not on the hot path)
-    char* b = nullptr;
-    ~DeviceScratch() { if (b) cudaFree(b); }
-};
-
-nd_status check_cells(const nd_problem* p, int32_t n_cells, const int32_t* cell, const char* who)
-{
-    if (n_cells < 1) return nd_fail(ND_ERR_INVALID, (std::string(who) + ": n_cells must be >= 1").c_str());
-    for (int64_t r = 0; r < p->d.R; ++r)
-        if (cell[r] < 0 || cell[r] >= n_cells) return nd_fail(ND_ERR_RANGE, (std::string(who) + ": cell[r] out of [0, n_cells)").c_str());
-    return ND_OK;
-}
-
-} // namespace
-
-// NEXT-3, C-4: see nd.h.
-extern "C" nd_status nd_cmfd_collapse(nd_problem* p, const double* d_phi_or_null, int32_t n_cells, const int32_t* cell,
-                                      double* V, double* Phi, double* sigma_t, double* sigma_s, double* nu_sigma_f,
-                                      double* chi, void* cuda_stream)
-{
-    if (!p || !cell || !V || !Phi || !sigma_t || !sigma_s || !nu_sigma_f || !chi)
-        return nd_fail(ND_ERR_NULL, "nd_cmfd_collapse: NULL argument");
-    nd_status rc = check_cells(p, n_cells, cell, "nd_cmfd_collapse");
-    if (rc != ND_OK) return rc;
-    const Dims& d = p->d;
-    cudaStream_t st = as_stream(cuda_stream);
-    const double* phi = d_phi_or_null ? d_phi_or_null : p->phi_cur;
-    const size_t CG = (size_t)n_cells * d.G, nPsi = (size_t)n_cells * d.M * d.G, nOut = 4 * CG + CG * d.G;
-    auto up = [](size_t b) { return (b + 255) / 256 * 256; };
-    const size_t oPsi = 0, oV = oPsi + up(sizeof(double) * nPsi), oOut = oV + up(sizeof(double) * (size_t)n_cells),
-                 oCell = oOut + up(sizeof(double) * nOut), total = oCell + up(sizeof(int32_t) * (size_t)d.R);
-    DeviceScratch ds;
-    ND_CUDA(cudaMalloc(&ds.b, total));
-    double* dPsi = (double*)(ds.b + oPsi);
-    double* dV = (double*)(ds.b + oV);
-    double* dOut = (double*)(ds.b + oOut);
-    int32_t* dCell = (int32_t*)(ds.b + oCell);
-    ND_CUDA(cudaMemsetAsync(ds.b, 0, oOut, st));
-    ND_CUDA(cudaMemcpyAsync(dCell, cell, sizeof(int32_t) * (size_t)d.R, cudaMemcpyHostToDevice, st));
-    ndk::k_cmfd_accumulate<<<grid_for((int64_t)d.R * d.G, 256, 8 * p->n_sm), 256, 0, st>>>(phi, p->vol, p->reg_mat, dCell, dPsi, dV, d.R, d.G, d.M);
-    ND_LAUNCH_CHECK(p);
-    ndk::k_cmfd_constants<<<grid_for((int64_t)CG, 128, 8 * p->n_sm), 128, 0, st>>>(dPsi, dV, p->sigt, p->sigsT, p->nusf, p->chi, dOut, n_cells, d.G, d.M);
-    ND_LAUNCH_CHECK(p);
-    ND_CUDA(cudaMemcpyAsync(V, dV, sizeof(double) * (size_t)n_cells, cudaMemcpyDeviceToHost, st));
-    ND_CUDA(cudaMemcpyAsync(Phi, dOut, sizeof(double) * CG, cudaMemcpyDeviceToHost, st));
-    ND_CUDA(cudaMemcpyAsync(sigma_t, dOut + CG, sizeof(double) * CG, cudaMemcpyDeviceToHost, st));
-    ND_CUDA(cudaMemcpyAsync(nu_sigma_f, dOut + 2 * CG, sizeof(double) * CG, cudaMemcpyDeviceToHost, st));
-    ND_CUDA(cudaMemcpyAsync(chi, dOut + 3 * CG, sizeof(double) * CG, cudaMemcpyDeviceToHost, st));
-    ND_CUDA(cudaMemcpyAsync(sigma_s, dOut + 4 * CG, sizeof(double) * CG * d.G, cudaMemcpyDeviceToHost, st));
-    ND_CUDA(cudaStreamSynchronize(st));
-    return ND_OK;
-}
-
-// NEXT-3, C-9: see nd.h.
-extern "C" nd_status nd_cmfd_prolong(nd_problem* p, int32_t n_cells, const int32_t* cell, const double* ratio, double k_eff,
-                                     void* cuda_stream)
-{
-    if (!p || !cell || !ratio) return nd_fail(ND_ERR_NULL, "nd_cmfd_prolong: NULL argument");
-    if (!(k_eff > 0.0)) return nd_fail(ND_ERR_INVALID, "nd_cmfd_prolong: k_eff must be > 0");
-    nd_status rc = check_cells(p, n_cells, cell, "nd_cmfd_prolong");
-    if (rc != ND_OK) return rc;
-    const Dims& d = p->d;
-    cudaStream_t st = as_stream(cuda_stream);
-    const size_t CG = (size_t)n_cells * d.G, nE = 2 * (size_t)d.T;
-    auto up = [](size_t b) { return (b + 255) / 256 * 256; };
-    const size_t oRatio = 0, oCell = oRatio + up(sizeof(double) * CG), oEnt = oCell + up(sizeof(int32_t) * (size_t)d.R),
-                 total = oEnt + up(sizeof(int32_t) * nE);
-    DeviceScratch ds;
-    ND_CUDA(cudaMalloc(&ds.b, total));
-    double* dRatio = (double*)(ds.b + oRatio);
-    int32_t* dCell = (int32_t*)(ds.b + oCell);
-    int32_t* dEnt = (int32_t*)(ds.b + oEnt);
-    ND_CUDA(cudaMemcpyAsync(dRatio, ratio, sizeof(double) * CG, cudaMemcpyHostToDevice, st));
-    ND_CUDA(cudaMemcpyAsync(dCell, cell, sizeof(int32_t) * (size_t)d.R, cudaMemcpyHostToDevice, st));
-    ND_CUDA(cudaMemcpyAsync(dEnt, p->h_entry_region.data(), sizeof(int32_t) * nE, cudaMemcpyHostToDevice, st));
-    ND_CUDA(cudaMemcpyAsync(p->scalars + ndk::SC_K, &k_eff, sizeof(double), cudaMemcpyHostToDevice, st));
-    ndk::k_cmfd_prolong_phi<<<grid_for((int64_t)d.R * d.G, 256, 8 * p->n_sm), 256, 0, st>>>(p->phi_cur, dCell, dRatio, d.R, d.G);
-    ND_LAUNCH_CHECK(p);
-    ndk::k_cmfd_prolong_psi<<<grid_for((int64_t)nE * d.P * d.Gs, 256, 8 * p->n_sm), 256, 0, st>>>(p->psi_in, dEnt, dCell, dRatio, (int64_t)nE, d.P, d.G, d.Gs);
-    ND_LAUNCH_CHECK(p);
-    rc = launch_fission_rate(p, p->phi_cur, nullptr, st);   // the state's F belongs to its flux
-    if (rc != ND_OK) return rc;
-    ND_CUDA(cudaStreamSynchronize(st));
-    return ND_OK;
-}
-
-// NEXT-3, C-5..C-8: see nd.h.
-extern "C" nd_status nd_cmfd_coarse_solve(int32_t n_cells, int32_t n_groups, const double* V, const double* Phi,
-                                          const double* sigma_t, const double* sigma_s, const double* nu_sigma_f,
-                                          const double* chi, int32_t n_pairs, const int32_t* pair_lo, const int32_t* pair_hi,
-                                          const double* coupling, const double* J_surf, const double* J_vac, double k0,
-                                          double tol, int32_t max_outer, double* k_out, double* Phi_new, int32_t* iters_done,
-                                          void* cuda_stream)
-{
-    if (!V || !Phi || !sigma_t || !sigma_s || !nu_sigma_f || !chi || !J_vac || !k_out || !Phi_new ||
-        (n_pairs > 0 && (!pair_lo || !pair_hi || !coupling || !J_surf)))
-        return nd_fail(ND_ERR_NULL, "nd_cmfd_coarse_solve: NULL argument");
-    if (n_cells < 1 || n_groups < 1 || n_pairs < 0 || !(k0 > 0.0) || !(tol > 0.0) || max_outer < 1)
-        return nd_fail(ND_ERR_INVALID, "nd_cmfd_coarse_solve: sizes must be positive, k0 > 0, tol > 0, max_outer >= 1");
-    const int64_t n = (int64_t)n_cells * n_groups;
-    if (n > 8192) return nd_fail(ND_ERR_RANGE, "nd_cmfd_coarse_solve: more than 8192 coarse unknowns (dense inverse)");
-    for (int32_t s = 0; s < n_pairs; ++s)
-        if (pair_lo[s] < 0 || pair_hi[s] >= n_cells || pair_lo[s] >= pair_hi[s])
-            return nd_fail(ND_ERR_RANGE, "nd_cmfd_coarse_solve: a surface needs 0 <= lo < hi < n_cells");
-    cudaStream_t st = as_stream(cuda_stream);
-    int n_sm = 148;
-    {
-        int dev = 0;
-        ND_CUDA(cudaGetDevice(&dev));
-        ND_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    }
-    const int C = n_cells, G = n_groups, S = n_pairs;
-    const size_t CG = (size_t)n, SG = (size_t)S * G;
-    // scratch (doubles): A[n][n] | V | Phi | sigt | sigs | nusf | chi | J_vac | coupling | J_surf | x | y | f | col | row | state[2]
-    size_t o = 0;
-    auto take = [&o](size_t count) { const size_t at = o; o += (count + 31) / 32 * 32; return at; };
-    const size_t oA = take(CG * CG), oV = take(C), oPhi = take(CG), oSt = take(CG), oSs = take(CG * G), oNf = take(CG),
-                 oChi = take(CG), oJv = take(CG), oCo = take(S), oJs = take(SG), oX = take(CG), oY = take(CG), oF = take(CG),
-                 oCol = take(CG), oRow = take(CG), oState = take(2), nD = o;
-    const size_t bytes = sizeof(double) * nD + sizeof(int32_t) * (2 * (size_t)S + 64);
-    DeviceScratch ds;
-    ND_CUDA(cudaMalloc(&ds.b, bytes));
-    double* D = (double*)ds.b;
-    int32_t* I = (int32_t*)(ds.b + sizeof(double) * nD);   // lo [S] | hi [S] | done | iters
-    int32_t* d_lo = I; int32_t* d_hi = I + S; int* d_done = I + 2 * S; int* d_iters = d_done + 1;
-    ND_CUDA(cudaMemsetAsync(D + oA, 0, sizeof(double) * CG * CG, st));
-    ND_CUDA(cudaMemsetAsync(d_done, 0, 2 * sizeof(int), st));
-    auto h2d = [&](size_t at, const double* src, size_t count) {
-        return count ? cudaMemcpyAsync(D + at, src, sizeof(double) * count, cudaMemcpyHostToDevice, st) : cudaSuccess;
-    };
-    ND_CUDA(h2d(oV, V, C)); ND_CUDA(h2d(oPhi, Phi, CG)); ND_CUDA(h2d(oSt, sigma_t, CG)); ND_CUDA(h2d(oSs, sigma_s, CG * G));
-    ND_CUDA(h2d(oNf, nu_sigma_f, CG)); ND_CUDA(h2d(oChi, chi, CG)); ND_CUDA(h2d(oJv, J_vac, CG));
-    ND_CUDA(h2d(oCo, coupling, S)); ND_CUDA(h2d(oJs, J_surf, SG)); ND_CUDA(h2d(oX, Phi, CG));
-    const double state0[2] = {k0, 0.0};
-    ND_CUDA(h2d(oState, state0, 2));
-    if (S > 0) {
-        ND_CUDA(cudaMemcpyAsync(d_lo, pair_lo, sizeof(int32_t) * S, cudaMemcpyHostToDevice, st));
-        ND_CUDA(cudaMemcpyAsync(d_hi, pair_hi, sizeof(int32_t) * S, cudaMemcpyHostToDevice, st));
-    }
-    ndk::CoarseParams cp{};
-    cp.V = D + oV; cp.Phi = D + oPhi; cp.sigt = D + oSt; cp.sigs = D + oSs; cp.nusf = D + oNf; cp.chi = D + oChi;
-    cp.J_vac = D + oJv; cp.lo = d_lo; cp.hi = d_hi; cp.coupling = D + oCo; cp.J_surf = D + oJs; cp.A = D + oA;
-    cp.C = C; cp.G = G; cp.S = S;
-    const int cap = 8 * n_sm;
-    ndk::k_coarse_cell_blocks<<<grid_for((int64_t)CG * G, 256, cap), 256, 0, st>>>(cp);
-    if (S > 0) ndk::k_coarse_surfaces<<<grid_for((int64_t)SG, 256, cap), 256, 0, st>>>(cp);
-    for (int64_t piv = 0; piv < n; ++piv) {          // A <- A^-1 in place
-        ndk::k_gj_prepare<<<grid_for(n, 256, cap), 256, 0, st>>>(D + oA, D + oCol, D + oRow, n, piv);
-        ndk::k_gj_update<<<grid_for(n * n, 256, cap), 256, 0, st>>>(D + oA, D + oCol, D + oRow, n, piv);
-    }
-    ND_CUDA(cudaGetLastError());
-    // P0 = sum(B Phi), then outer iterations in batches; the kernels turn into no-ops once the flag is set
-    ndk::k_coarse_fission<<<grid_for(n, 256, cap), 256, 0, st>>>(D + oX, cp.V, cp.nusf, cp.chi, D + oF, C, G, nullptr);
-    ndk::k_coarse_update<<<1, 1024, 0, st>>>(D + oX, D + oY, D + oF, cp.V, cp.nusf, cp.chi, D + oState, d_done, d_iters, C, G, tol, 1);
-    int done = 0, iters = 0;
-    const int batch = 32;
-    while (!done && iters < max_outer) {
-        const int todo = max_outer - iters < batch ? max_outer - iters : batch;
-        for (int b = 0; b < todo; ++b) {
-            ndk::k_coarse_fission<<<grid_for(n, 256, cap), 256, 0, st>>>(D + oX, cp.V, cp.nusf, cp.chi, D + oF, C, G, d_done);
-            ndk::k_coarse_matvec<<<grid_for(n * 32, 256, cap), 256, 0, st>>>(D + oA, D + oF, D + oY, n, d_done);
-            ndk::k_coarse_update<<<1, 1024, 0, st>>>(D + oX, D + oY, D + oF, cp.V, cp.nusf, cp.chi, D + oState, d_done, d_iters, C, G, tol, 0);
-        }
-        ND_CUDA(cudaGetLastError());
-        int h[2];
-        ND_CUDA(cudaMemcpyAsync(h, d_done, sizeof h, cudaMemcpyDeviceToHost, st));
-        ND_CUDA(cudaStreamSynchronize(st));
-        done = h[0]; iters = h[1];
-    }
-    double hstate[2];
-    ND_CUDA(cudaMemcpyAsync(hstate, D + oState, sizeof hstate, cudaMemcpyDeviceToHost, st));
-    ND_CUDA(cudaMemcpyAsync(Phi_new, D + oX, sizeof(double) * CG, cudaMemcpyDeviceToHost, st));
-    ND_CUDA(cudaStreamSynchronize(st));
-    *k_out = hstate[0];
-    if (iters_done) *iters_done = iters;
-    if (!done) return nd_fail(ND_ERR_NOT_CONVERGED, "nd_cmfd_coarse_solve: max_outer reached (outputs are written)");
-    return ND_OK;
-}
-
-// NEXT-3, Algorithm 1 as one call: see nd.h.  A host composition of the entry points above.
-extern "C" nd_status nd_cmfd_iteration(nd_problem* p, int32_t n_cells, const int32_t* cell, int32_t n_pairs,
-                                       const int32_t* pair_lo, const int32_t* pair_hi, const double* coupling,
-                                       double* k_sweep_out, double* k_eff_out, int32_t* coarse_iters, void* cuda_stream)
-{
-    if (!p || !cell || !k_eff_out || (n_pairs > 0 && (!pair_lo || !pair_hi || !coupling)))
-        return nd_fail(ND_ERR_NULL, "nd_cmfd_iteration: NULL argument");
-    if (n_cells < 1 || n_pairs < 0) return nd_fail(ND_ERR_INVALID, "nd_cmfd_iteration: n_cells must be >= 1 and n_pairs >= 0");
-    const Dims& d = p->d;
-    cudaStream_t st = as_stream(cuda_stream);
-    const size_t CG = (size_t)n_cells * d.G, SG = (size_t)n_pairs * d.G;
-    std::vector<double> Js, Jv, Jr, V, Phi, sgt, sgs, nsf, chi, Phi_new;
-    try {
-        Js.resize(SG + 1); Jv.resize(CG); Jr.resize(CG); V.resize((size_t)n_cells); Phi.resize(CG); sgt.resize(CG);
-        sgs.resize(CG * d.G); nsf.resize(CG); chi.resize(CG); Phi_new.resize(CG);
-    } catch (const std::bad_alloc&) {
-        return nd_fail(ND_ERR_NOMEM, "nd_cmfd_iteration: out of host memory");
-    }
-    // state scalars: k and the fission rate F of the current flux (the sweep uses phi / F and psi / F)
-    double ks[2];
-    ND_CUDA(cudaMemcpyAsync(ks, p->scalars, sizeof ks, cudaMemcpyDeviceToHost, st));
-    ND_CUDA(cudaStreamSynchronize(st));
-    const double k = ks[ndk::SC_K], F = ks[ndk::SC_F];
-    if (!(k > 0.0) || !(F > 0.0)) return nd_fail(ND_ERR_STATE, "nd_cmfd_iteration: the state has k <= 0 or no fission rate");
-    DeviceScratch ds;
-    ND_CUDA(cudaMalloc(&ds.b, sizeof(double) * (size_t)d.R * d.G));
-    double* dQ = (double*)ds.b;
-    // C-3 with the un-normalised source: the currents are linear in (Q, psi), so they come out F times too large
-    nd_status rc = nd_source_update(p, p->phi_cur, k, dQ, nullptr, cuda_stream);
-    if (rc != ND_OK) return rc;
-    rc = nd_sweep_currents(p, dQ, n_cells, cell, n_pairs, pair_lo, pair_hi, Js.data(), Jv.data(), Jr.data(), cuda_stream);
-    if (rc != ND_OK) return rc;
-    for (double& v : Js) v /= F;
-    for (double& v : Jv) v /= F;
-    double k_sweep = 0.0;
-    rc = nd_power_iteration(p, 1, 0.0, 0.0, &k_sweep, nullptr, nullptr, nullptr, cuda_stream);   // source, sweep, flux, k
-    if (rc != ND_OK) return rc;
-    if (k_sweep_out) *k_sweep_out = k_sweep;
-    rc = nd_cmfd_collapse(p, nullptr, n_cells, cell, V.data(), Phi.data(), sgt.data(), sgs.data(), nsf.data(), chi.data(), cuda_stream);
-    if (rc != ND_OK) return rc;
-    double k_new = 0.0;
-    rc = nd_cmfd_coarse_solve(n_cells, d.G, V.data(), Phi.data(), sgt.data(), sgs.data(), nsf.data(), chi.data(), n_pairs,
-                              pair_lo, pair_hi, coupling, Js.data(), Jv.data(), k_sweep, 1e-13, 100000, &k_new, Phi_new.data(),
-                              coarse_iters, cuda_stream);
-    if (rc != ND_OK) return rc;
-    for (size_t i = 0; i < CG; ++i) Phi_new[i] /= Phi[i];                                        // C-9 ratio
-    rc = nd_cmfd_prolong(p, n_cells, cell, Phi_new.data(), k_new, cuda_stream);
-    if (rc != ND_OK) return rc;
-    *k_eff_out = k_new;
-    return ND_OK;
-}
+#include "nd_cmfd_api.cuh"   // NEXT-3: the CMFD plan (nd_cmfd_*), on the problem's internals above
 
 extern "C" nd_status nd_profile_enable(nd_problem* p, int32_t on)
 {

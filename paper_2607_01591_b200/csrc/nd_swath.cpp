@@ -19,6 +19,7 @@ struct SwathBuild {
     std::vector<uint8_t> bytes;        // this swath's chunks, concatenated
     std::vector<uint32_t> chunk_rel;   // chunk offsets relative to the swath's first byte, 16-B units
     std::vector<uint32_t> head16;      // head size of every chunk, 16-B units
+    std::vector<uint16_t> slot_start;  // [tiles][NT+1] when requested
     int64_t n_seg = 0, sum_regions = 0, sum_max_cnt = 0, n_active = 0;
     int max_head = 0, max_rec = 0;
     int32_t group = 0;                 // angle id of the swath's tracks
@@ -172,7 +173,7 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
                     }
                     // ---- encode ----
                     const int L = (int)regions.size();
-                    {   // regions in descending order of their segment count: flush threads of a warp get lists of similar length
+                    {   // regions in descending order of their segment count: the flush units of one pass have lists of similar length
                         perm.resize(L);
                         std::iota(perm.begin(), perm.end(), 0);
                         std::stable_sort(perm.begin(), perm.end(), [&](int a, int b) { return rcount[a] > rcount[b]; });
@@ -220,6 +221,7 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
                         }
                     }
                     ss[NT] = (uint16_t)o;
+                    if (prm.keep_slot_start) sb.slot_start.insert(sb.slot_start.end(), ss, ss + NT + 1);
                     sb.sum_regions += L;
                     sb.sum_max_cnt += max_cnt;
                     sb.max_head = std::max(sb.max_head, o_rc);
@@ -254,6 +256,16 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
             for (size_t i = 0; i < sb.chunk_rel.size(); ++i)
                 out->tile_ref[(size_t)out->swath_tile0[sw] + i] = {b16 + sb.chunk_rel[i], sb.head16[i]};
             std::vector<uint8_t>().swap(sb.bytes);
+        }
+        if (prm.keep_slot_start) {
+            out->slot_start.resize((size_t)out->n_tiles * (NT + 1));
+#pragma omp parallel for schedule(dynamic, 64) num_threads(nth)
+            for (int64_t sw = 0; sw < n_sw; ++sw) {
+                SwathBuild& sb = built[(size_t)sw];
+                if (!sb.slot_start.empty())
+                    memcpy(out->slot_start.data() + (size_t)out->swath_tile0[sw] * (NT + 1), sb.slot_start.data(), sizeof(uint16_t) * sb.slot_start.size());
+                std::vector<uint16_t>().swap(sb.slot_start);
+            }
         }
         out->max_head_bytes = max_head;
         out->max_rec_bytes = max_rec;

@@ -10,7 +10,8 @@
 //   head  u32 hdr[4]          L | nseg << 16 ;  off_regions (16-byte units from the chunk start) ;  head bytes ;  chunk bytes
 //         u16 slot_start[NT+1] per-track prefix into rec[]                                     (padded to 16 B)
 //         u32 regions[L][2]    { global region id (q row to stage, tally row to flush) ;
-//                                first delta-buffer row | one past the last << 16 }             (padded to 16 B)
+//                                first delta-buffer row | one past the last << 16 }             (padded to 16 B),
+//                              in descending order of their row counts
 //   rec   rec[nseg]            16 bytes each: { f32 length ; u32 q-row byte offset ; u32 Sigma_t-row byte offset ;
 //                              u32 delta-row byte offset }, slot-major, forward order; the backward direction walks
 //                              the same records in reverse
@@ -38,6 +39,7 @@ struct NdSwathParams {
                   // (the track furthest behind advances first) until the fronts are level again.  < 0: always geometric.
     int NCq = 0;  // copies of a q row per shared line (0: = NC).  1 = one copy per region: adjacent slots in the same region
                   // read it as a broadcast, slots in different regions may meet in a bank
+    bool keep_slot_start = false;   // also return every tile's slot_start array on the host (the CMFD crossing lists need it)
     int item_order = 0;   // 0: work items most expensive first (load balance); 1: angle by angle, adjacent swaths
                           // consecutively, forward then backward (blocks that run together touch neighbouring regions)
 };
@@ -63,6 +65,7 @@ struct NdSwathSet {
     std::vector<int64_t> swath_tile0;     // [n_swaths+1] prefix into tile_ref
     std::vector<NdSwathTileRef> tile_ref; // [n_tiles+1] (+ end sentinel: chunk k spans [off16[k], off16[k+1]))
     std::vector<NdSwathItem> items;       // work items (swath, direction)
+    std::vector<uint16_t> slot_start;     // [n_tiles][NT+1] (only with prm.keep_slot_start)
     NdRawBytes blob;                      // all chunks (every byte written by nd_build_swaths)
     int max_head_bytes = 0, max_rec_bytes = 0;
     double mean_regions_per_tile = 0.0, mean_segments_per_tile = 0.0, lockstep_efficiency = 0.0;

@@ -52,6 +52,16 @@ struct SwathParams {
     uint32_t magic_per_row, magic_nq;          // fastdiv constants of NC*Gs/4 and Gs/4
     uint32_t magic_np;                         // fastdiv constant of Gs/2 (group pairs per row: the flush mapping)
     unsigned long long* phase;                 // PROF builds: [kSwathPhases] warp-cycle sums (lane 0 of every warp)
+    // CUR builds (CMFD, C-3 of DESIGN.md 8d): the coarse-surface crossings of every tile and the current tally
+    const uint8_t* __restrict__ xblob;         // per tile: u32 {count, 0} then count entries {surface << 1 | forward sign bit,
+                                               // slot | position << 16}, padded to 16 bytes
+    const uint32_t* __restrict__ xoff;         // [n_tiles+1] offsets into xblob, 16-byte units
+    double* __restrict__ J_surf;               // [J_replicas][J_stride]: [n_pairs][G] net currents, positive from the lower to the
+                                               // higher cell id.  A block adds into replica blockIdx.x % J_replicas: a coarse mesh has
+                                               // few surfaces, and FP64 atomics of all blocks on the same few lines serialise in L2
+    long long J_stride;
+    int J_replicas;
+    int x_cap, off_x, off_w;                   // bytes of one crossing buffer; shared-memory offsets of the ring and of W
 };
 
 // phases of the instrumented build (nd_profile_enable(p, 2)): where the warps' cycles go
@@ -59,6 +69,7 @@ enum { PH_STAGE = 0, PH_WAIT_A, PH_COMPUTE, PH_WAIT_B, PH_FLUSH, PH_ITEM, kSwath
 
 constexpr int kSwathHeadBufs = 3;   // heads of tiles k, k+1 (its q rows are staged during tile k) and k+2 (in flight)
 constexpr int kSwathRecBufs = 2;    // records of tiles k and k+1 (in flight)
+constexpr int kSwathXBufs = 2;      // CUR builds: crossing lists of tiles k and k+1 (in flight)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -249,7 +260,10 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
 }
 
 // TIGHT = 1 caps the registers at 85 (768 resident threads per SM: three 256-thread or two 384-thread blocks).
-template <int P, int EXPM, int TIGHT, int PROF>
+// CUR = 1 also tallies the net currents through the surfaces of a coarse mesh (CMFD, C-3 of DESIGN.md 8d) WITHOUT touching the
+// segment loop: with W = sum_p w_p psi_p, a delta row is W before its segment minus W behind it, so W at a crossing is W at
+// the tile's entry (stored per slot before the loop) minus the delta rows of the slot's segments passed so far.
+template <int P, int EXPM, int TIGHT, int PROF, int CUR = 0>
 __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swath(const SwathParams prm)
 {
     long long ph[kSwathPhases] = {0, 0, 0, 0, 0, 0};
@@ -262,6 +276,7 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
     unsigned char* const smem = smem_sw;
     uint64_t* hfull = reinterpret_cast<uint64_t*>(smem);             // [kSwathHeadBufs] head-arrival barriers
     uint64_t* rfull = hfull + kSwathHeadBufs;                        // [kSwathRecBufs] record-arrival barriers
+    uint64_t* xfull = reinterpret_cast<uint64_t*>(smem + 96);        // [kSwathXBufs] crossing-list barriers (CUR)
     volatile int* s_item = reinterpret_cast<volatile int*>(smem + 64);
     uint32_t* s_null = reinterpret_cast<uint32_t*>(smem + 80);       // the null record: { 0.0f, 0, 0, offset of the spare delta row }
     const int tid = threadIdx.x, nthr = blockDim.x;
@@ -280,6 +295,10 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
         for (int i = 0; i < kSwathHeadBufs + kSwathRecBufs; ++i) mbar_init(hfull + i, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         s_null[0] = 0u; s_null[1] = 0u; s_null[2] = 0u; s_null[3] = (uint32_t)(prm.NT * prm.Kmax * row_bytes);
+        if (CUR) {
+            for (int i = 0; i < kSwathXBufs; ++i) mbar_init(xfull + i, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
     }
     // Sigma_t table, replicated NC times per line; the fast-exp path keeps it pre-multiplied by -log2(e)/sin(theta_0)
     {
@@ -307,6 +326,7 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
     const int lane_off_q = TIGHT ? sub * row_bytes + ll * 16 : (slot % prm.NCq) * row_bytes + ll * 16;
     const float inv_f = (float)(1.0 / *prm.scale_div);
     const int g0 = ll * 4;
+    const int f_np = Gs >> 1;                         // pairs of groups per row: the unit of the flush
 
     uint32_t seq = 0;   // tiles processed by this block so far: staging buffers and barrier parities follow it
     for (;;) {
@@ -362,6 +382,13 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
             const uint32_t s = seq + k;
             mbar_wait(rfull + (s % kSwathRecBufs), (s / kSwathRecBufs) & 1u);
         };
+        auto issue_x = [&](int k) {      // one thread (CUR): the crossing list of tile k
+            const int64_t ti = tile_index(k);
+            const uint32_t o0 = prm.xoff[ti], bytes = (prm.xoff[ti + 1] - o0) * 16u;
+            const uint32_t b = (seq + k) % kSwathXBufs;
+            mbar_expect_tx(xfull + b, bytes);
+            tma_load_1d(smem + prm.off_x + (size_t)b * prm.x_cap, prm.xblob + (size_t)o0 * 16, bytes, xfull + b);
+        };
         auto issue_q_rows = [&](int k) {   // all threads: regions of tile k -> q buffer (seq+k)&1, NCq copies per row
             const uint32_t s = seq + k;
             const unsigned char* hb = head_s + (size_t)(s % kSwathHeadBufs) * prm.head_cap;
@@ -381,6 +408,7 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
                 issue_head(0);
                 issue_rec(0);
                 if (nt > 1) issue_head(1);
+                if (CUR) issue_x(0);
             }
             wait_head(0);
             issue_q_rows(0);
@@ -406,12 +434,24 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
             if (tid == 0) {
                 if (k + 2 < nt) issue_head(k + 2);
                 if (k + 1 < nt) issue_rec(k + 1);
+                if (CUR && k + 1 < nt) issue_x(k + 1);
             }
             wait_rec(k);
             if (PROF) prof_sink += *s_item;        // BAR.SYNC defers its blocking to the next consumer: make one here
             mark(PH_WAIT_A);
             const SwathHead ch = decode_head(hb);
             unsigned char* dbuf = dbuf_s + (size_t)(prm.ndbuf == 1 ? 0u : (s & 1u)) * dbuf_bytes;
+            if (CUR) {   // W = sum_p w_p psi_p of this slot at the tile's entry (the previous tile's flush is over: barrier above)
+                float wv[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    float a = 0.f;
+#pragma unroll
+                    for (int p = 0; p < P; ++p) a = fmaf(wpt[p], psi[p][j], a);
+                    wv[j] = a;
+                }
+                sts_f4(smem_u32(smem + prm.off_w) + slot * row_bytes + ll * 16, wv[0], wv[1], wv[2], wv[3]);
+            }
             // ---- segment loop of this slot's track through the tile ----
             {
                 int s0 = 0, cnt = 0;
@@ -431,25 +471,52 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
             if (PROF) prof_sink += *s_item;
             mark(PH_WAIT_B);
             // ---- flush: one FP64 RED per (region, group) of the tile.  A thread owns a pair of groups of one region, pairs
-            // fastest: the lanes of a warp read consecutive 8-byte pieces of the region's contiguous delta rows (no bank
-            // conflict inside a region) and their REDs fall on consecutive doubles of the tally row (2-3 lines per instruction).
-            {
-                const int np = Gs >> 1;
-                for (int u = tid; u < ch.L * np; u += nthr) {
-                    const int l = (int)fastdiv((uint32_t)u, prm.magic_np), gp = u - l * np;
-                    const uint2 rg = ch.regions[l];
-                    const int e0 = (int)(rg.y & 0xffffu), e1 = (int)(rg.y >> 16);
-                    uint32_t row = smem_u32(dbuf) + e0 * row_bytes + gp * 8;
-                    float vx = 0.f, vy = 0.f;
+            // fastest: the lanes of a warp read consecutive 8-byte pieces of the region's contiguous delta rows and their REDs
+            // fall on consecutive doubles of the tally row (2-3 lines per instruction).  (A warp-per-region mapping with the
+            // regions dealt to the warps by row count was conflict-free and balanced, and 1.9 % slower at config 5.)
+            for (int u = tid; u < ch.L * f_np; u += nthr) {
+                const int l = (int)fastdiv((uint32_t)u, prm.magic_np), gp = u - l * f_np;
+                const uint2 rg = ch.regions[l];
+                const int e0 = (int)(rg.y & 0xffffu), e1 = (int)(rg.y >> 16);
+                uint32_t row = smem_u32(dbuf) + e0 * row_bytes + gp * 8;
+                float vx = 0.f, vy = 0.f;
 #pragma unroll 4
-                    for (int e = e0; e < e1; ++e, row += row_bytes) {
+                for (int e = e0; e < e1; ++e, row += row_bytes) {
+                    float x, y;
+                    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(x), "=f"(y) : "r"(row));
+                    vx += x; vy += y;
+                }
+                double* tp = prm.tally + (size_t)rg.x * Gs + gp * 2;
+                if (gp * 2 < prm.G) atomicAdd(tp, (double)vx);
+                if (gp * 2 + 1 < prm.G) atomicAdd(tp + 1, (double)vy);
+            }
+            if (CUR) {
+                // ---- currents: thread -> (crossing, pair of groups).  W at the crossing = W at the slot's entry minus the delta
+                // rows of the segments the chain has passed: positions 0..pos forward, pos+1..cnt-1 backward. ----
+                mbar_wait(xfull + (s % kSwathXBufs), (s / kSwathXBufs) & 1u);
+                const uint2* xl = reinterpret_cast<const uint2*>(smem + prm.off_x + (size_t)(s % kSwathXBufs) * prm.x_cap);
+                const int nx = (int)xl[0].x;
+                const uint32_t rec_b = smem_u32(rec_s) + (s % kSwathRecBufs) * prm.rec_cap + 12;   // delta offset of record 0
+                const uint32_t w_b = smem_u32(smem + prm.off_w);
+                for (int u = tid; u < nx * f_np; u += nthr) {
+                    const int c = (int)fastdiv((uint32_t)u, prm.magic_np), gp = u - c * f_np;
+                    const uint2 xe = xl[1 + c];
+                    const int xs = (int)(xe.y & 0xffffu), pos = (int)(xe.y >> 16);
+                    const int s0 = ch.slot_start[xs], cnt = ch.slot_start[xs + 1] - s0;
+                    const int j0 = dir ? pos + 1 : 0, j1 = dir ? cnt : pos + 1;
+                    float wx, wy;
+                    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(wx), "=f"(wy) : "r"(w_b + xs * row_bytes + gp * 8));
+                    for (int j = j0; j < j1; ++j) {
+                        uint32_t off;
+                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(off) : "r"(rec_b + 16 * (s0 + j)));
                         float x, y;
-                        asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(x), "=f"(y) : "r"(row));
-                        vx += x; vy += y;
+                        asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(x), "=f"(y) : "r"(smem_u32(dbuf) + off + gp * 8));
+                        wx -= x; wy -= y;
                     }
-                    double* tp = prm.tally + (size_t)rg.x * Gs + gp * 2;
-                    if (gp * 2 < prm.G) atomicAdd(tp, (double)vx);
-                    if (gp * 2 + 1 < prm.G) atomicAdd(tp + 1, (double)vy);
+                    const bool neg = ((xe.x & 1u) != 0u) != (dir != 0);      // forward sign bit, reversed for the backward chain
+                    double* jp = prm.J_surf + (size_t)(blockIdx.x % prm.J_replicas) * prm.J_stride + (size_t)(xe.x >> 1) * prm.G + gp * 2;
+                    if (gp * 2 < prm.G) atomicAdd(jp, (double)(neg ? -wx : wx));
+                    if (gp * 2 + 1 < prm.G) atomicAdd(jp + 1, (double)(neg ? -wy : wy));
                 }
             }
             mark(PH_FLUSH);

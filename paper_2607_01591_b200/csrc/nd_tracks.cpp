@@ -355,6 +355,8 @@ nd_status nd_tracks_finish(nd_tracks* tr)
             for (int64_t k = tr->seg_offset[t]; k < tr->seg_offset[static_cast<size_t>(t) + 1]; ++k)
                 tr->volume[tr->seg_region[k]] += w2 * tr->seg_length[k];
         }
+        tr->global_id.resize(static_cast<size_t>(T));
+        for (int t = 0; t < T; ++t) tr->global_id[t] = t;
         tr->azim_phi.resize(nh); tr->azim_weight.resize(nh); tr->azim_spacing.resize(nh);
         for (int j = 0; j < nh; ++j) {
             tr->azim_phi[j] = tr->angles[j].mirrored ? kPi - tr->angles[j].phi : tr->angles[j].phi;
@@ -431,6 +433,86 @@ extern "C" nd_status nd_tracks_view(const nd_tracks* tr, nd_tracks_view_t* v)
     v->azim_phi = tr->azim_phi.data();
     v->azim_weight = tr->azim_weight.data();
     v->azim_spacing = tr->azim_spacing.data();
+    v->track_global = tr->global_id.data();
+    return ND_OK;
+}
+
+// NEXT-2: the tracks of one shard of an angle-pair partition.  A reflective link joins a track of angle j
+// to one of its complement N_a/2-1-j (O-3), so a shard that owns whole pairs {j, N_a/2-1-j} never exchanges boundary flux.
+extern "C" nd_status nd_tracks_shard(const nd_tracks* full, int32_t n_shards, int32_t shard, nd_tracks** out)
+{
+    if (!full || !out) return nd_fail(ND_ERR_NULL, "nd_tracks_shard: NULL argument");
+    const int nh = full->n_half, np = nh / 2, T = full->n_tracks;
+    if (n_shards < 1 || shard < 0 || shard >= n_shards) return nd_fail(ND_ERR_INVALID, "nd_tracks_shard: need 0 <= shard < n_shards");
+    if (nh < 2 || nh % 2 != 0 || (int)full->angles.size() != nh) return nd_fail(ND_ERR_STATE, "nd_tracks_shard: not a cyclic laydown");
+    if (n_shards > np) return nd_fail(ND_ERR_INVALID, "nd_tracks_shard: more shards than angle pairs (N_a / 4)");
+    if ((int)full->global_id.size() != T) return nd_fail(ND_ERR_STATE, "nd_tracks_shard: incomplete tracks object");
+    for (int t = 0; t < T; ++t)
+        if (full->global_id[t] != t) return nd_fail(ND_ERR_STATE, "nd_tracks_shard: the input is already a shard");
+    nd_tracks* tr = nullptr;
+    try {
+        // ---- segments per angle pair, pairs dealt to the shards longest first (deterministic) ----
+        std::vector<int64_t> seg_of_angle(static_cast<size_t>(nh), 0);
+        for (int t = 0; t < T; ++t) seg_of_angle[full->track_azim[t]] += full->seg_offset[static_cast<size_t>(t) + 1] - full->seg_offset[t];
+        std::vector<int> order(static_cast<size_t>(np));
+        std::vector<int64_t> w(static_cast<size_t>(np));
+        for (int j = 0; j < np; ++j) { order[j] = j; w[j] = seg_of_angle[j] + seg_of_angle[nh - 1 - j]; }
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return w[a] > w[b]; });
+        std::vector<int64_t> load(static_cast<size_t>(n_shards), 0);
+        std::vector<int> owner(static_cast<size_t>(nh), -1);
+        for (int i = 0; i < np; ++i) {
+            int best = 0;
+            for (int s = 1; s < n_shards; ++s)
+                if (load[s] < load[best]) best = s;
+            load[best] += w[order[i]];
+            owner[order[i]] = owner[nh - 1 - order[i]] = best;
+        }
+        // ---- copy the shard's tracks in canonical order ----
+        tr = new nd_tracks();
+        tr->n_azim = full->n_azim; tr->n_half = nh; tr->n_regions = full->n_regions;
+        tr->angles = full->angles;
+        tr->azim_phi = full->azim_phi; tr->azim_weight = full->azim_weight; tr->azim_spacing = full->azim_spacing;
+        tr->volume = full->volume;                       // the areas A~_r of the WHOLE laydown: every shard divides by them
+        std::vector<int32_t> local(static_cast<size_t>(T), -1);
+        int n = 0;
+        int64_t S = 0;
+        for (int t = 0; t < T; ++t)
+            if (owner[full->track_azim[t]] == shard) {
+                local[t] = n++;
+                S += full->seg_offset[static_cast<size_t>(t) + 1] - full->seg_offset[t];
+            }
+        tr->n_tracks = n; tr->n_segments = S;
+        tr->seg_offset.assign(static_cast<size_t>(n) + 1, 0);
+        tr->seg_region.resize(static_cast<size_t>(S));
+        tr->seg_length.resize(static_cast<size_t>(S));
+        tr->track_weight.resize(static_cast<size_t>(n)); tr->track_azim.resize(static_cast<size_t>(n));
+        tr->link.resize(2 * static_cast<size_t>(n)); tr->ends.resize(4 * static_cast<size_t>(n));
+        tr->global_id.resize(static_cast<size_t>(n));
+        int64_t o = 0;
+        for (int t = 0; t < T; ++t) {
+            const int lt = local[t];
+            if (lt < 0) continue;
+            const int64_t k0 = full->seg_offset[t], k1 = full->seg_offset[static_cast<size_t>(t) + 1];
+            tr->seg_offset[lt] = o;
+            for (int64_t k = k0; k < k1; ++k, ++o) { tr->seg_region[o] = full->seg_region[k]; tr->seg_length[o] = full->seg_length[k]; }
+            tr->track_weight[lt] = full->track_weight[t];
+            tr->track_azim[lt] = full->track_azim[t];
+            tr->global_id[lt] = t;
+            for (int c = 0; c < 4; ++c) tr->ends[4 * static_cast<size_t>(lt) + c] = full->ends[4 * static_cast<size_t>(t) + c];
+            for (int d = 0; d < 2; ++d) {
+                const int32_t lk = full->link[2 * static_cast<size_t>(t) + d];
+                if (lk < 0) { tr->link[2 * static_cast<size_t>(lt) + d] = -1; continue; }
+                const int32_t l2 = local[lk >> 1];
+                if (l2 < 0) { delete tr; return nd_fail(ND_ERR_STATE, "nd_tracks_shard: a link leaves its angle pair"); }
+                tr->link[2 * static_cast<size_t>(lt) + d] = 2 * l2 + (lk & 1);
+            }
+        }
+        tr->seg_offset[n] = o;
+    } catch (const std::bad_alloc&) {
+        delete tr;
+        return nd_fail(ND_ERR_NOMEM, "nd_tracks_shard: out of host memory");
+    }
+    *out = tr;
     return ND_OK;
 }
 

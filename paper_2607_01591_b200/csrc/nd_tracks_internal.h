@@ -51,6 +51,7 @@ struct nd_tracks {
     std::vector<double> ends;
     std::vector<double> volume;
     std::vector<double> azim_phi, azim_weight, azim_spacing;
+    std::vector<int32_t> global_id;   // [T] id of every track in the unsharded laydown (identity unless made by nd_tracks_shard)
 };
 
 // What a ray walker needs besides the mesh arrays: the half-edge twins and every track's first triangle.

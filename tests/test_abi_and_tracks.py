@@ -133,24 +133,20 @@ def test_workspace_bytes_and_host_validation_without_a_gpu():
     assert h.value is None
 
 
-def test_cmfd_coarse_solve_validates_before_touching_the_gpu():
-    """Argument checks of nd_cmfd_coarse_solve (include/nd.h) come before any CUDA call, so they run without a GPU."""
-    import numpy as np
-    n, G = 4, 2
-    co = dict(V=np.ones(n), Phi=np.ones((n, G)), sigt=np.ones((n, G)), sigs=np.zeros((n, G, G)), nusf=np.ones((n, G)),
-              chi=np.ones((n, G)))
-    lo, hi = np.array([0, 1], np.int32), np.array([1, 2], np.int32)
-    cpl, Js, Jv = np.ones(2), np.zeros((2, G)), np.zeros((n, G))
-    with pytest.raises(nd.NdError, match="k0 > 0"):
-        nd.nd_cmfd_coarse_solve(co, lo, hi, cpl, Js, Jv, 0.0)
-    with pytest.raises(nd.NdError, match="tol > 0"):
-        nd.nd_cmfd_coarse_solve(co, lo, hi, cpl, Js, Jv, 1.0, tol=0.0)
-    with pytest.raises(nd.NdError, match="lo < hi"):
-        nd.nd_cmfd_coarse_solve(co, hi, lo, cpl, Js, Jv, 1.0)
-    with pytest.raises(nd.NdError, match="lo < hi"):
-        nd.nd_cmfd_coarse_solve(co, lo, np.array([1, 4], np.int32), cpl, Js, Jv, 1.0)
-    big = 4100
-    co_big = dict(V=np.ones(big), Phi=np.ones((big, G)), sigt=np.ones((big, G)), sigs=np.zeros((big, G, G)),
-                  nusf=np.ones((big, G)), chi=np.ones((big, G)))
-    with pytest.raises(nd.NdError, match="8192"):
-        nd.nd_cmfd_coarse_solve(co_big, lo, hi, cpl, Js, np.zeros((big, G)), 1.0)
+def test_cmfd_plan_entry_points_reject_null_arguments_without_a_gpu():
+    """Argument checks of the nd_cmfd_* calls (include/nd.h) come before any CUDA call, so they run without a GPU."""
+    L = nd.lib()
+    n = C.c_size_t()
+    k = C.c_double()
+    assert L.nd_status_string(L.nd_cmfd_workspace_bytes(None, None, 1, None, 0, C.byref(n))) == b"ND_ERR_NULL"
+    assert L.nd_status_string(L.nd_cmfd_workspace_bytes(None, None, 1, None, 0, None)) == b"ND_ERR_NULL"
+    h = C.c_void_p()
+    ws = (C.c_char * 512)()
+    assert L.nd_status_string(L.nd_cmfd_create(None, None, 1, None, 0, None, None, None, None, ws, 512, None, C.byref(h))) == b"ND_ERR_NULL"
+    assert L.nd_status_string(L.nd_cmfd_iteration(None, 1, C.byref(k), None, None)) == b"ND_ERR_NULL"
+    assert L.nd_status_string(L.nd_cmfd_sweep(None, None, None, None)) == b"ND_ERR_NULL"
+    assert L.nd_status_string(L.nd_cmfd_solve(None, 1.0, C.byref(k), None, None, None)) == b"ND_ERR_NULL"
+    assert L.nd_status_string(L.nd_cmfd_collapse(None, None, None)) == b"ND_ERR_NULL"
+    assert L.nd_status_string(L.nd_cmfd_prolong(None, None)) == b"ND_ERR_NULL"
+    assert L.nd_cmfd_destroy(None) == 0
+    assert b"NULL" in L.nd_last_error(None)

@@ -38,11 +38,11 @@ def _decode_and_check(st, mat, seg_offset, seg_region, seg_length, NT, Kmax, Lma
             co = np.concatenate([rg[:, 1] & 0xffff, [rg[-1, 1] >> 16]])
             assert np.array_equal(rg[:, 1] >> 16, co[1:]), "row ranges of consecutive regions are contiguous"
             assert o_rg + 8 * L <= head
+            assert np.all(np.diff(np.diff(co)) <= 0), "regions in descending order of their row counts"
             rec = c[head:head + 16 * nseg].view(np.uint32).reshape(nseg, 4)
             assert ss[0] == 0 and ss[NT] == nseg and np.all(np.diff(ss) >= 0) and np.all(np.diff(ss) <= Kmax)
             assert len(np.unique(regions)) == L
             assert co[0] == 0 and co[L] == nseg and np.all(np.diff(co) >= 1)
-            assert np.all(np.diff(np.diff(co)) <= 0), "regions in descending order of their row counts"
             row_region = np.repeat(regions, np.diff(co))          # region-major delta rows: region l owns rows co[l]..co[l+1]-1
             rows_seen = np.zeros(nseg, bool)
             last_row_of_region = {}
