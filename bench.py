@@ -6,8 +6,10 @@
 A STEP is one pass of the whole hot path (DESIGN.md rows A2-A7): source update -> transport sweep -> link swap
 -> flux finalise -> fission-rate reduction and k update, i.e. one power iteration, through the C ABI.
 metric = segment-group-polar updates per second (U = 2*S*P*G per sweep, both directions counted).
-Prints ONE JSON line.  Multi-GPU (N > 1): N independent replicas, one per rank (the path
-is single-GPU by north_star, replicas only, no collective on the data path).
+Prints ONE JSON line.  Multi-GPU (N > 1): the angle pairs of the laydown are sharded over the ranks
+(nd_tracks_shard; reflective links never leave a pair, so no boundary flux is exchanged) and the ranks share ONE collective
+per sweep, an FP64 NCCL all-reduce of the tally (nd_tally_reducer_set): strong scaling of one problem.  --replicas runs N
+independent copies instead (weak scaling, no collective).
 """
 import argparse
 import json
@@ -42,6 +44,8 @@ def parse():
         ap.add_argument("--" + name, type=int, default=0, help="nd_options tuning field (0 = library default)")
     ap.add_argument("--cpu-seconds", type=float, default=None,
                     help="target CPU time of one oracle sample (default: 15 s for cpu_baseline; --impl reference: 150 s / steps, 2..30 s)")
+    ap.add_argument("--replicas", action="store_true",
+                    help="N > 1: run N independent replicas (weak scaling) instead of sharding the angle pairs over the ranks")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -208,7 +212,8 @@ def workload_config(args, prob, tr):
             "n_azim": int(prob.n_azim), "spacing_cm": float(prob.spacing), "n_tracks": int(tr.n_tracks),
             "n_segments": int(tr.n_segments), "updates_per_sweep": int(2 * tr.n_segments * prob.n_polar * prob.n_groups),
             "bc_left_right_bottom_top": list(prob.bc), "step": "one power iteration (source, sweep, link swap, finalise, k)",
-            "parallelism": f"replicas x{args.gpus}" if args.gpus > 1 else "single GPU"}
+            "parallelism": ("single GPU" if args.gpus <= 1 else f"replicas x{args.gpus}" if args.replicas else
+                            f"angle pairs sharded over {args.gpus} ranks, one FP64 all-reduce of the tally per sweep")}
 
 
 def aggregate(ms_local: float, units_local: float):
@@ -244,7 +249,9 @@ def main():
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=dev)
 
-    prob, tr, setup = build_inputs(args)
+    prob, tr_full, setup = build_inputs(args)
+    sharded = world > 1 and not args.replicas
+    tr = tr_full.shard(world, rank) if sharded else tr_full     # NEXT-2: this rank's angle pairs (areas of the whole laydown)
     t0 = time.time()
     gp = nd.nd_problem_create(prob.xs, prob.polar_sin, prob.polar_weight, prob.mesh.material, tr, device=str(dev),
                               sweep_kernel=args.kernel, exp_mode=args.exp_mode,
@@ -253,6 +260,8 @@ def main():
                               blocks_per_sm=args.blocks_per_sm, tile_lag=args.tile_lag, item_order=args.item_order,
                               q_copies=args.q_copies)
     setup["create_s"] = round(time.time() - t0, 2)
+    if sharded:
+        gp.nd_tally_reducer_set(lambda tally: dist.all_reduce(tally))   # the one collective of the path: sum of the shards' tallies
     info = gp.nd_problem_info_get()
     R, G = prob.mesh.n_regions, prob.n_groups
     U = info["updates_per_sweep"]
@@ -370,11 +379,12 @@ def main():
                         "dram_traffic_GBps": (traffic / (sweep_ms * 1e-3) / 1e9) if traffic else None}}
     cb = None
     if not args.no_cpu_baseline:
-        cb = oracle_sample(prob, tr, args.cpu_seconds or 15.0)
+        cb = oracle_sample(prob, tr_full, args.cpu_seconds or 15.0)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
-            "ms_per_step": ms_per_step, "ms_per_sweep": sweep_ms, "higher_is_better": True, "scaling": "weak",
+            "ms_per_step": ms_per_step, "ms_per_sweep": sweep_ms, "higher_is_better": True,
+            "scaling": "strong" if sharded else "weak",
             "vs_baseline": None, "dtype": "f32 (segment arithmetic) + f64 (tallies, flux, source, k)", "data": "synthetic",
-            "config": dict(workload_config(args, prob, tr), l2="L2 flushed between steps" if need_flush else "inputs larger than L2",
+            "config": dict(workload_config(args, prob, tr_full), l2="L2 flushed between steps" if need_flush else "inputs larger than L2",
                            sweep_kernel=info["sweep_kernel"], setup_s=setup,
                            launch={k: info[k] for k in ("block_threads", "smem_bytes", "grid_blocks", "tracks_per_block", "n_batches",
                                                         "mean_regions_per_tile", "mean_segments_per_tile", "lockstep_efficiency")}),

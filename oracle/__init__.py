@@ -14,14 +14,15 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "moc_oracle.c")
+_SRC_P1 = os.path.join(_HERE, "moc_oracle_p1.c")          # NEXT-4: the same sweep with a P_1 scattering source
 _LIB = os.path.join(_HERE, "libmoc_oracle.so")
 CFLAGS = ["-O2", "-std=c11", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC"]
 
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (no -ffast-math, no -march) and return the .so path."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", *CFLAGS, _SRC, "-o", _LIB, "-lm"])
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_P1)):
+        subprocess.check_call(["gcc", *CFLAGS, _SRC, _SRC_P1, "-o", _LIB, "-lm"])
     return _LIB
 
 
