@@ -377,6 +377,33 @@ nd_status nd_cmfd_solve(nd_cmfd* c, double k0, double* k_out, double* Phi_new_or
                         void* cuda_stream);
 nd_status nd_cmfd_prolong(nd_cmfd* c, void* cuda_stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-4: a second workload on the same segment data: the transport sweep with a linearly anisotropic (P_1)
+ * scattering source, the Legendre expansion Eq. (2) truncated at l = 1.  Readings P-1..P-6, DESIGN.md 8e:
+ *   Q(Omega) = Q0 + 3 (Omega_x Q1x + Omega_y Q1y),  Q0 as nd_source_update,  Q1 = (1/4pi) Sigma_s1 J,  J = integral of Omega psi;
+ *   Omega_xy = sin(theta_p) x the unit vector of the direction of travel;  Eq. (5) with Q(Omega) of the chain's own direction;
+ *   phi = 4 pi Q0/Sigma_t + tally0/(Sigma_t A~);  J = [4 pi 3 c2 (M Q1) + tally_xy] / (Sigma_t A~), c2 = sum_p w_p sin^2(theta_p),
+ *   Mab[r] = sum over the segments of r of 2 omega_a delta_a s u_a u_b.
+ * This round: first correct kernels -- the simple one-warp-per-chain sweep over the plain segment stream with three FP64
+ * tallies, so the problem must have been created with sweep_kernel = ND_SWEEP_ATOMIC (else ND_ERR_STATE).
+ *   desc       the descriptor the problem was created from, WITH track_ends (direction of every track) -- HOST, borrowed
+ *   sigma_s1   HOST [M][g][g'] first Legendre moment of the scattering matrix, from g' into g
+ * All d_* arrays DEVICE [R][G] FP64.  nd_p1_power_iteration runs O-8 with the P_1 source on the problem's own state (flux,
+ * boundary flux, k) and the plan's currents (zero after nd_p1_state_reset / nd_p1_create); k_history HOST [n_iters] or NULL.
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct nd_p1 nd_p1;
+nd_status nd_p1_workspace_bytes(const nd_problem* p, size_t* device_bytes);
+nd_status nd_p1_create(nd_problem* p, const nd_problem_desc* desc, const double* sigma_s1, void* device_workspace, size_t device_bytes,
+                       void* cuda_stream, nd_p1** out);
+nd_status nd_p1_destroy(nd_p1* c);
+nd_status nd_p1_transport_sweep(nd_p1* c, const double* d_Q0, const double* d_Q1x, const double* d_Q1y, double* d_phi_out,
+                                double* d_Jx_out, double* d_Jy_out, void* cuda_stream);
+nd_status nd_p1_source_update(nd_p1* c, const double* d_phi, const double* d_Jx, const double* d_Jy, double k_eff, double* d_Q0_out,
+                              double* d_Q1x_out, double* d_Q1y_out, void* cuda_stream);
+nd_status nd_p1_state_reset(nd_p1* c, void* cuda_stream);
+nd_status nd_p1_power_iteration(nd_p1* c, int32_t n_iters, double* k_eff_out, double* d_phi_out_or_null, double* d_Jx_out_or_null,
+                                double* d_Jy_out_or_null, double* k_history_or_null, void* cuda_stream);
+
 /* Device-time accounting.  When enabled, every sweep-kernel launch is bracketed by CUDA events on its own
  * stream; nd_profile_read synchronises and returns the accumulated kernel milliseconds and launch counts
  * since the last nd_profile_enable(p,1).  kernels_launched counts every kernel the library launched. */

@@ -27,7 +27,8 @@ EXPORTS = [
     "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_outgoing_flux_get", "nd_flux_get", "nd_flux_set",
     "nd_track_volume_get", "nd_tally_get", "nd_cmfd_surfaces", "nd_microbench", "nd_cmfd_workspace_bytes", "nd_cmfd_create",
     "nd_cmfd_destroy", "nd_cmfd_iteration", "nd_cmfd_sweep", "nd_cmfd_currents_get", "nd_cmfd_collapse", "nd_cmfd_coarse_get",
-    "nd_cmfd_coarse_set", "nd_cmfd_solve", "nd_cmfd_prolong", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
+    "nd_cmfd_coarse_set", "nd_cmfd_solve", "nd_cmfd_prolong", "nd_p1_workspace_bytes", "nd_p1_create", "nd_p1_destroy",
+    "nd_p1_transport_sweep", "nd_p1_source_update", "nd_p1_state_reset", "nd_p1_power_iteration", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
     "nd_swath_stream_build", "nd_swath_stream_view", "nd_swath_stream_destroy",
     "nd_status_string", "nd_last_error", "nd_version", "nd_build_id",
 ]
@@ -174,6 +175,15 @@ def lib():
         L.nd_cmfd_coarse_set.argtypes = [C.c_void_p] * 10
         L.nd_cmfd_solve.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double), C.c_void_p, C.POINTER(C.c_int32), C.c_void_p]
         L.nd_cmfd_prolong.argtypes = [C.c_void_p, C.c_void_p]
+        L.nd_p1_workspace_bytes.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
+        L.nd_p1_create.argtypes = [C.c_void_p, C.POINTER(nd_problem_desc), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p,
+                                   C.POINTER(C.c_void_p)]
+        L.nd_p1_destroy.argtypes = [C.c_void_p]
+        L.nd_p1_transport_sweep.argtypes = [C.c_void_p] * 8
+        L.nd_p1_source_update.argtypes = [C.c_void_p] * 4 + [C.c_double] + [C.c_void_p] * 4
+        L.nd_p1_state_reset.argtypes = [C.c_void_p, C.c_void_p]
+        L.nd_p1_power_iteration.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double), C.c_void_p, C.c_void_p, C.c_void_p,
+                                            C.c_void_p, C.c_void_p]
         L.nd_profile_enable.argtypes = [C.c_void_p, C.c_int32]
         L.nd_profile_read.argtypes = [C.c_void_p, C.POINTER(nd_profile)]
         L.nd_sweep_phases_get.argtypes = [C.c_void_p, C.c_void_p]
@@ -501,6 +511,72 @@ class Problem:
         inf = nd_problem_info()
         _check(lib().nd_problem_info_get(self._h, C.byref(inf)), "nd_problem_info_get")
         return {f[0]: getattr(inf, f[0]) for f in nd_problem_info._fields_ if f[0] != "reserved"}
+
+
+class P1:
+    """Owner of an nd_p1 plan and its torch workspace (include/nd.h "NEXT-4": P_1 scattering source).  tracks: the Tracks (or
+    any object with seg_offset, seg_region, seg_length, track_weight, ends) the problem was created from."""
+
+    def __init__(self, prob, tracks, polar_sin, polar_weight, sigma_s1):
+        t = prob.torch
+        self.prob = prob
+        keep = dict(so=np.ascontiguousarray(tracks.seg_offset, np.int64), sr=np.ascontiguousarray(tracks.seg_region, np.int32),
+                    sl=np.ascontiguousarray(tracks.seg_length, np.float64), tw=np.ascontiguousarray(tracks.track_weight, np.float64),
+                    te=np.ascontiguousarray(tracks.ends, np.float64), ps=np.ascontiguousarray(polar_sin, np.float64),
+                    pw=np.ascontiguousarray(polar_weight, np.float64), s1=np.ascontiguousarray(sigma_s1, np.float64))
+        assert keep["s1"].shape == (prob.M, prob.G, prob.G)
+        d = nd_problem_desc()
+        d.n_regions, d.n_tracks, d.n_polar = prob.R, prob.T, prob.P
+        d.track_seg_offset, d.seg_region, d.seg_length = keep["so"].ctypes.data, keep["sr"].ctypes.data, keep["sl"].ctypes.data
+        d.track_weight, d.track_ends = keep["tw"].ctypes.data, keep["te"].ctypes.data
+        d.polar_sin, d.polar_weight = keep["ps"].ctypes.data, keep["pw"].ctypes.data
+        nbytes = C.c_size_t()
+        _check(lib().nd_p1_workspace_bytes(prob._h, C.byref(nbytes)), "nd_p1_workspace_bytes")
+        with t.cuda.device(prob.device):
+            self.workspace = t.empty(int(nbytes.value) + 256, dtype=t.uint8, device=prob.device)
+            ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+            h = C.c_void_p()
+            _check(lib().nd_p1_create(prob._h, C.byref(d), keep["s1"].ctypes.data, C.c_void_p(ptr), int(nbytes.value), prob._stream(),
+                                      C.byref(h)), "nd_p1_create")
+        self._h = h
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().nd_p1_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def _new(self):
+        t = self.prob.torch
+        return t.empty((self.prob.R, self.prob.G), dtype=t.float64, device=self.prob.device)
+
+    def nd_p1_transport_sweep(self, d_Q0, d_Q1x, d_Q1y):
+        phi, Jx, Jy = self._new(), self._new(), self._new()
+        _check(lib().nd_p1_transport_sweep(self._h, d_Q0.data_ptr(), d_Q1x.data_ptr(), d_Q1y.data_ptr(), phi.data_ptr(), Jx.data_ptr(),
+                                           Jy.data_ptr(), self.prob._stream()), "nd_p1_transport_sweep")
+        return phi, Jx, Jy
+
+    def nd_p1_source_update(self, d_phi, d_Jx, d_Jy, k_eff):
+        Q0, Q1x, Q1y = self._new(), self._new(), self._new()
+        _check(lib().nd_p1_source_update(self._h, d_phi.data_ptr(), d_Jx.data_ptr(), d_Jy.data_ptr(), float(k_eff), Q0.data_ptr(),
+                                         Q1x.data_ptr(), Q1y.data_ptr(), self.prob._stream()), "nd_p1_source_update")
+        return Q0, Q1x, Q1y
+
+    def nd_p1_state_reset(self):
+        _check(lib().nd_p1_state_reset(self._h, self.prob._stream()), "nd_p1_state_reset")
+
+    def nd_p1_power_iteration(self, n_iters):
+        k = C.c_double()
+        phi, Jx, Jy = self._new(), self._new(), self._new()
+        hist = np.empty(max(1, n_iters))
+        _check(lib().nd_p1_power_iteration(self._h, int(n_iters), C.byref(k), phi.data_ptr(), Jx.data_ptr(), Jy.data_ptr(),
+                                           hist.ctypes.data, self.prob._stream()), "nd_p1_power_iteration")
+        return dict(k_eff=k.value, phi=phi, Jx=Jx, Jy=Jy, k_history=hist[:n_iters])
 
 
 class Cmfd:

@@ -16,6 +16,7 @@
 #include "nd_internal.h"
 #include "nd_kernels.cuh"
 #include "nd_cmfd.cuh"
+#include "nd_p1.cuh"
 #include "nd_sweep_swath.cuh"
 #include "nd_swath.h"
 
@@ -1092,6 +1093,7 @@ extern "C" nd_status nd_tally_get(nd_problem* p, double* d_tally_out, void* cuda
 }
 
 #include "nd_cmfd_api.cuh"   // NEXT-3: the CMFD plan (nd_cmfd_*), on the problem's internals above
+#include "nd_p1_api.cuh"     // NEXT-4: the P_1-scattering plan (nd_p1_*)
 
 extern "C" nd_status nd_profile_enable(nd_problem* p, int32_t on)
 {
