@@ -139,6 +139,8 @@ typedef struct {            /* all pointers HOST, owned by the nd_tracks object,
     const double* azim_weight;       /* [N_a/2] omega_a per direction (sum over N_a directions = 1) */
     const double* azim_spacing;      /* [N_a/2] effective spacing delta_a */
     const int32_t* track_global;     /* [T] id of the track in the unsharded laydown (identity unless made by nd_tracks_shard) */
+    const int32_t* seg_region_device;/* DEVICE [S], NULL unless made by nd_tracks_generate_resident (then seg_region and   */
+    const double* seg_length_device; /* DEVICE [S]  seg_length above are NULL until nd_tracks_materialise)                */
 } nd_tracks_view_t;
 
 /* The same preprocessing with the ray walk (rule R-W, one step per segment: almost all of the work) on the GPU:
@@ -163,6 +165,25 @@ typedef struct {                /* where the time of nd_tracks_generate_device w
 nd_status nd_tracks_generate_device(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, void* device_workspace,
                                     size_t device_bytes, void* cuda_stream, nd_trace_timing* timing_or_null,
                                     nd_tracks** out);
+
+/* The device tracer with the segments left WHERE THEY ARE: seg_region / seg_length of all S segments stay in
+ * `device_workspace` (nd_tracks_view: seg_region_device / seg_length_device; same values, bit for bit, as the host arrays of
+ * nd_tracks_generate), and nothing of size S is copied to the host.  Pass them to nd_problem_create with
+ * nd_problem_desc.seg_on_device = 1.  The track volumes A~_r are summed on the GPU (FP64 atomics: equal to
+ * nd_tracks_generate's to rounding, not bit for bit).  The host arrays of the segments are made on demand by
+ * nd_tracks_materialise (what nd_cmfd_surfaces, nd_p1_create and nd_tracks_shard read).
+ *   device_workspace  DEVICE, 256-byte aligned, caller-owned; must stay untouched until nd_tracks_destroy or until the
+ *                     last use of the device pointers and of nd_tracks_materialise.  It must hold
+ *                     *min_bytes (nd_tracks_device_workspace_bytes) - 2^20 * bytes_per_segment + S * bytes_per_segment
+ *                     bytes; S is known only after the count pass, so a workspace that is too small gives
+ *                     ND_ERR_WORKSPACE with the size that suffices in *required_bytes (call again).
+ * Synchronises the stream before returning. */
+nd_status nd_tracks_generate_resident(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, void* device_workspace,
+                                      size_t device_bytes, void* cuda_stream, nd_trace_timing* timing_or_null,
+                                      size_t* required_bytes_or_null, nd_tracks** out);
+/* Copies the device-resident segment arrays to host arrays owned by `tracks` (no-op when they exist); nd_tracks_view then
+ * returns them.  Synchronises the stream. */
+nd_status nd_tracks_materialise(nd_tracks* tracks, void* cuda_stream);
 
 /* NEXT-2 (the paper names multi-GPU as future work): shard `shard` of `n_shards` of an ANGLE-PAIR
  * partition of a cyclic laydown.  A reflective link joins a track of angle j only to one of its complement N_a/2-1-j (O-3),
@@ -205,8 +226,16 @@ typedef struct {                    /* all pointers: HOST memory, borrowed for t
     const double* track_ends;       /* [T][4] x0,y0,x1,y1 (forward direction runs from 0 to 1) */
     /* Optional (NULL = the library forms A~ from this descriptor's own segments): the track-estimated areas A~_r to divide
        by, HOST [R], finite and >= 0.  A shard of an angle-pair partition (nd_tracks_shard) holds a part of the tracks but
-       must use the areas of all of them. */
+       must use the areas of all of them; for unsharded tracks nd_tracks_view's track_volume saves the pass over the segments. */
     const double* region_volume;
+    /* 0: seg_region / seg_length are HOST arrays.  1: they are DEVICE arrays (nd_tracks_generate_resident leaves them in
+       its workspace; nd_tracks_view: seg_region_device / seg_length_device), borrowed for the call only; every other array
+       of the descriptor stays on the host.  The whole of nd_problem_create's work on segments then runs on the GPU: their
+       validation, A~_r (when region_volume is NULL; FP64 atomics, so the last bits depend on the order), the atomic
+       kernel's SoA stream, and the swath kernel's chunk stream (one thread per swath through the same cutter/encoder as
+       the host builder: the two streams are equal byte for byte).  Needs track_azim / track_ends. */
+    int32_t seg_on_device;
+    int32_t reserved;               /* must be 0 */
 } nd_problem_desc;
 
 typedef struct nd_problem nd_problem; /* opaque host object; owns no device memory except what lies in the workspace */
@@ -431,6 +460,21 @@ typedef struct {
     int32_t block_threads, smem_bytes, grid_blocks, tracks_per_block;
 } nd_problem_info;
 nd_status nd_problem_info_get(const nd_problem* p, nd_problem_info* out);
+
+/* Diagnostics: where the swath kernel's chunk stream lies in the problem's workspace (DEVICE pointers, valid as long as
+ * the problem), whichever builder made it -- the host one (host segments) or the device one (seg_on_device).  Tests copy
+ * the arrays back and compare the two builders byte for byte.  ND_ERR_STATE unless the problem runs ND_SWEEP_SWATH. */
+typedef struct {
+    const void* blob;           /* all chunks (format: csrc/nd_swath.h) */
+    size_t blob_bytes;
+    const uint32_t* tile_ref;   /* [n_tiles + 1][2] chunk offset, head size (16-byte units); last = end sentinel */
+    const int64_t* swath_tile0; /* [n_swaths + 1] */
+    const int32_t* swath_track; /* [n_swaths][tracks_per_swath] */
+    const int32_t* items;       /* [n_items][4] swath, direction, cost, 0 */
+    int64_t n_tiles, n_swaths, n_items;
+    int32_t tracks_per_swath, built_on_device;
+} nd_stream_device_view_t;
+nd_status nd_problem_stream_view(const nd_problem* p, nd_stream_device_view_t* out);
 
 /* ------------------------------------------------------------------------------------------------
  * Diagnostics: the swath/tile chunk stream of ND_SWEEP_SWATH (row A1: "segment stream layout"), built on the

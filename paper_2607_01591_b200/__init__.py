@@ -16,13 +16,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libnd_moc.so")
 
 ND_OK = 0
+ND_ERR_WORKSPACE = 4
 ND_ERR_NOT_CONVERGED = 7
 ND_BC_VACUUM, ND_BC_REFLECTIVE = 0, 1
 ND_EXP_FAST, ND_EXP_EXPM1 = 0, 1
 ND_SWEEP_AUTO, ND_SWEEP_ATOMIC, ND_SWEEP_SWATH = 0, 1, 3
 
 EXPORTS = [
-    "nd_tracks_generate", "nd_tracks_device_workspace_bytes", "nd_tracks_generate_device", "nd_tracks_view", "nd_tracks_shard", "nd_tracks_destroy", "nd_tally_reducer_set", "nd_workspace_bytes", "nd_problem_create",
+    "nd_tracks_generate", "nd_tracks_device_workspace_bytes", "nd_tracks_generate_device", "nd_tracks_generate_resident", "nd_tracks_materialise", "nd_tracks_view", "nd_tracks_shard", "nd_tracks_destroy", "nd_tally_reducer_set", "nd_workspace_bytes", "nd_problem_create", "nd_problem_stream_view",
     "nd_problem_destroy", "nd_transport_sweep", "nd_source_update", "nd_power_iteration", "nd_state_reset",
     "nd_boundary_flux_fill", "nd_boundary_flux_get", "nd_boundary_flux_set", "nd_outgoing_flux_get", "nd_flux_get", "nd_flux_set",
     "nd_track_volume_get", "nd_tally_get", "nd_cmfd_surfaces", "nd_microbench", "nd_cmfd_workspace_bytes", "nd_cmfd_create",
@@ -56,7 +57,14 @@ class nd_tracks_view_t(C.Structure):
                 ("track_seg_offset", C.c_void_p), ("seg_region", C.c_void_p), ("seg_length", C.c_void_p),
                 ("track_weight", C.c_void_p), ("link", C.c_void_p), ("track_azim", C.c_void_p),
                 ("track_ends", C.c_void_p), ("track_volume", C.c_void_p), ("azim_phi", C.c_void_p),
-                ("azim_weight", C.c_void_p), ("azim_spacing", C.c_void_p), ("track_global", C.c_void_p)]
+                ("azim_weight", C.c_void_p), ("azim_spacing", C.c_void_p), ("track_global", C.c_void_p),
+                ("seg_region_device", C.c_void_p), ("seg_length_device", C.c_void_p)]
+
+
+class nd_stream_device_view_t(C.Structure):
+    _fields_ = [("blob", C.c_void_p), ("blob_bytes", C.c_size_t), ("tile_ref", C.c_void_p), ("swath_tile0", C.c_void_p),
+                ("swath_track", C.c_void_p), ("items", C.c_void_p), ("n_tiles", C.c_int64), ("n_swaths", C.c_int64),
+                ("n_items", C.c_int64), ("tracks_per_swath", C.c_int32), ("built_on_device", C.c_int32)]
 
 
 class nd_problem_desc(C.Structure):
@@ -65,7 +73,8 @@ class nd_problem_desc(C.Structure):
                 ("sigma_s", C.c_void_p), ("nu_sigma_f", C.c_void_p), ("chi", C.c_void_p), ("polar_sin", C.c_void_p),
                 ("polar_weight", C.c_void_p), ("track_seg_offset", C.c_void_p), ("seg_region", C.c_void_p),
                 ("seg_length", C.c_void_p), ("track_weight", C.c_void_p), ("link", C.c_void_p),
-                ("track_azim", C.c_void_p), ("track_ends", C.c_void_p), ("region_volume", C.c_void_p)]
+                ("track_azim", C.c_void_p), ("track_ends", C.c_void_p), ("region_volume", C.c_void_p),
+                ("seg_on_device", C.c_int32), ("reserved", C.c_int32)]
 
 
 ND_TALLY_REDUCE_FN = C.CFUNCTYPE(C.c_int32, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
@@ -137,10 +146,14 @@ def lib():
                                                        C.POINTER(C.c_size_t)]
         L.nd_tracks_generate_device.argtypes = [C.POINTER(nd_mesh_desc), C.c_int32, C.c_double, C.c_void_p, C.c_size_t,
                                                 C.c_void_p, C.POINTER(nd_trace_timing), C.POINTER(C.c_void_p)]
+        L.nd_tracks_generate_resident.argtypes = [C.POINTER(nd_mesh_desc), C.c_int32, C.c_double, C.c_void_p, C.c_size_t,
+                                                  C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t), C.POINTER(C.c_void_p)]
+        L.nd_tracks_materialise.argtypes = [C.c_void_p, C.c_void_p]
         L.nd_tracks_view.argtypes = [C.c_void_p, C.POINTER(nd_tracks_view_t)]
         L.nd_tracks_destroy.argtypes = [C.c_void_p]
         L.nd_tracks_shard.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_void_p)]
         L.nd_tally_reducer_set.argtypes = [C.c_void_p, ND_TALLY_REDUCE_FN, C.c_void_p]
+        L.nd_problem_stream_view.argtypes = [C.c_void_p, C.POINTER(nd_stream_device_view_t)]
         L.nd_workspace_bytes.argtypes = [C.POINTER(nd_problem_desc), C.POINTER(nd_options), C.POINTER(C.c_size_t)]
         L.nd_problem_create.argtypes = [C.POINTER(nd_problem_desc), C.POINTER(nd_options), C.c_void_p, C.c_size_t,
                                         C.c_void_p, C.POINTER(C.c_void_p)]
@@ -224,15 +237,20 @@ def nd_build_id():
 
 
 class Tracks:
-    """Result of nd_tracks_generate: numpy views of the library-owned host arrays (valid until .destroy())."""
+    """Result of nd_tracks_generate: numpy views of the library-owned host arrays (valid until .destroy()).
+    Made by nd_tracks_generate_resident, the segment arrays live on the device (`seg_device`: the two device pointers, kept
+    alive by `device_workspace`); `seg_region` / `seg_length` then copy them to the host on first use (nd_tracks_materialise)."""
 
-    def __init__(self, handle, view):
+    def __init__(self, handle, view, device_workspace=None, stream=None):
         self._h = handle
         T, R, S, NH = view.n_tracks, view.n_regions, view.n_segments, view.n_half
         self.n_tracks, self.n_regions, self.n_segments, self.n_half = T, R, S, NH
         self.seg_offset = _np_view(view.track_seg_offset, (T + 1,), np.int64)
-        self.seg_region = _np_view(view.seg_region, (S,), np.int32)
-        self.seg_length = _np_view(view.seg_length, (S,), np.float64)
+        self.device_workspace, self._stream = device_workspace, stream
+        self.seg_device = (int(view.seg_region_device), int(view.seg_length_device)) if view.seg_region_device else None
+        self._seg_host = None
+        if view.seg_region or S == 0:
+            self._seg_host = (_np_view(view.seg_region, (S,), np.int32), _np_view(view.seg_length, (S,), np.float64))
         self.track_weight = _np_view(view.track_weight, (T,), np.float64)
         self.link = _np_view(view.link, (T, 2), np.int32)
         self.track_azim = _np_view(view.track_azim, (T,), np.int32)
@@ -244,9 +262,30 @@ class Tracks:
         self.track_global = _np_view(view.track_global, (T,), np.int32)
         self.is_shard = False
 
+    def _materialise(self):
+        if self._seg_host is None:
+            _check(lib().nd_tracks_materialise(self._h, self._stream() if self._stream else None), "nd_tracks_materialise")
+            v = nd_tracks_view_t()
+            _check(lib().nd_tracks_view(self._h, C.byref(v)), "nd_tracks_view")
+            self._seg_host = (_np_view(v.seg_region, (self.n_segments,), np.int32), _np_view(v.seg_length, (self.n_segments,), np.float64))
+        return self._seg_host
+
+    @property
+    def on_host(self):
+        return self._seg_host is not None
+
+    @property
+    def seg_region(self):
+        return self._materialise()[0]
+
+    @property
+    def seg_length(self):
+        return self._materialise()[1]
+
     def shard(self, n_shards, shard):
         """NEXT-2 (nd_tracks_shard): the tracks of one shard of the angle-pair partition, as a new Tracks object whose
         `volume` holds the areas of the WHOLE laydown and `track_global` the ids in this object."""
+        self._materialise()
         h = C.c_void_p()
         _check(lib().nd_tracks_shard(self._h, int(n_shards), int(shard), C.byref(h)), "nd_tracks_shard")
         v = nd_tracks_view_t()
@@ -259,6 +298,7 @@ class Tracks:
         if self._h:
             lib().nd_tracks_destroy(self._h)
             self._h = None
+        self.device_workspace = None
 
     def __del__(self):
         try:
@@ -307,6 +347,46 @@ def nd_tracks_generate_device(xy, tri, W, H, bc, n_azim, spacing, segment_capaci
     return out
 
 
+def nd_tracks_generate_resident(xy, tri, W, H, bc, n_azim, spacing, segment_estimate=None, device="cuda:0") -> Tracks:
+    """Row A0 on the GPU with the segments LEFT on the device (nd.h: nd_tracks_generate_resident).  The returned Tracks owns
+    the torch workspace that holds them; pass it to nd_problem_create, which then builds its segment streams on the GPU.
+    `segment_estimate` sizes the first attempt (default: Cauchy's mean-chord estimate, sum of the triangle perimeters /
+    (pi * spacing) per angle, + 10 %); if the count pass finds more, the call is repeated once with the exact size."""
+    import torch
+    xy = np.ascontiguousarray(xy, np.float64)
+    tri = np.ascontiguousarray(tri, np.int32)
+    md = nd_mesh_desc(len(xy), len(tri), xy.ctypes.data, tri.ctypes.data, float(W), float(H), (C.c_int32 * 4)(*[int(b) for b in bc]))
+    nmin, per = C.c_size_t(), C.c_size_t()
+    _check(lib().nd_tracks_device_workspace_bytes(C.byref(md), int(n_azim), float(spacing), C.byref(nmin), C.byref(per)),
+           "nd_tracks_device_workspace_bytes")
+    if segment_estimate is None:
+        p = xy[tri]
+        perim = sum(np.hypot(*(p[:, (e + 1) % 3] - p[:, e]).T).sum() for e in range(3))
+        segment_estimate = int(1.1 * (n_azim // 2) * perim / (np.pi * float(spacing))) + 4096
+    dev = torch.device(device)
+    nbytes = int(nmin.value) + int(per.value) * int(segment_estimate)
+    stream = lambda: C.c_void_p(torch.cuda.current_stream(dev).cuda_stream)
+    with torch.cuda.device(dev):
+        for attempt in range(2):
+            ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev)
+            ptr = (ws.data_ptr() + 255) // 256 * 256
+            h, tm, need = C.c_void_p(), nd_trace_timing(), C.c_size_t(0)
+            rc = lib().nd_tracks_generate_resident(C.byref(md), int(n_azim), float(spacing), C.c_void_p(ptr), nbytes, stream(),
+                                                   C.byref(tm), C.byref(need), C.byref(h))
+            if rc == ND_ERR_WORKSPACE and need.value > nbytes and attempt == 0:
+                del ws
+                nbytes = int(need.value)
+                continue
+            _check(rc, "nd_tracks_generate_resident")
+            break
+    v = nd_tracks_view_t()
+    _check(lib().nd_tracks_view(h, C.byref(v)), "nd_tracks_view")
+    out = Tracks(h, v, device_workspace=ws, stream=stream)
+    out.timing = {f[0]: getattr(tm, f[0]) for f in nd_trace_timing._fields_ if f[0] != "reserved"}
+    out.timing["attempts"] = attempt + 1
+    return out
+
+
 def nd_cmfd_surfaces(seg_offset, seg_region, link, cell, n_cells, n_regions=None):
     """C-2 (nd.h): the interior surfaces of the coarse mesh `cell` as sorted (pair_lo, pair_hi) int32 arrays.  HOST only."""
     so, sr = np.ascontiguousarray(seg_offset, np.int64), np.ascontiguousarray(seg_region, np.int32)
@@ -343,10 +423,15 @@ class Problem:
                  seg_region, seg_length, track_weight, link, track_azim=None, track_ends=None, region_volume=None,
                  exp_mode=ND_EXP_FAST,
                  sweep_kernel=ND_SWEEP_AUTO, window_regions=0, block_warps=0, tile_segments=0,
-                 delta_buffers=0, blocks_per_sm=0, tile_lag=0, q_copies=0, graph_mode=0, cmfd_stream=0, item_order=0, device="cuda:0"):
+                 delta_buffers=0, blocks_per_sm=0, tile_lag=0, q_copies=0, graph_mode=0, cmfd_stream=0, item_order=0, device="cuda:0",
+                 seg_device=None):
+        """seg_device = (device pointer of seg_region, of seg_length): the segments are device-resident
+        (nd_problem_desc.seg_on_device = 1); seg_region / seg_length are then ignored and may be None."""
         import torch
         self.torch = torch
         self.device = torch.device(device)
+        if seg_device is not None:
+            seg_region, seg_length = np.zeros(0, np.int32), np.zeros(0, np.float64)
         keep = dict(
             rm=np.ascontiguousarray(region_material, np.int32), st=np.ascontiguousarray(sigma_t, np.float64),
             ss=np.ascontiguousarray(sigma_s, np.float64), nf=np.ascontiguousarray(nu_sigma_f, np.float64),
@@ -362,9 +447,13 @@ class Problem:
         if region_volume is not None:
             keep["rv"] = np.ascontiguousarray(region_volume, np.float64)
             geo = geo + [keep["rv"].ctypes.data]
+        elif seg_device is not None:
+            geo = geo + [None]
         self.R, (self.M, self.G), self.P, self.T = len(keep["rm"]), keep["st"].shape, len(keep["ps"]), len(keep["tw"])
         d = nd_problem_desc(self.R, self.M, self.G, self.P, self.T, *[keep[k].ctypes.data for k in
                             ("rm", "st", "ss", "nf", "ch", "ps", "pw", "so", "sr", "sl", "tw", "lk")], *geo)
+        if seg_device is not None:
+            d.seg_region, d.seg_length, d.seg_on_device = int(seg_device[0]), int(seg_device[1]), 1
         opt = nd_options(int(exp_mode), int(sweep_kernel), int(window_regions), int(block_warps),
                          int(tile_segments), int(delta_buffers), int(blocks_per_sm), int(tile_lag), int(q_copies), int(graph_mode), int(cmfd_stream), int(item_order))
         nbytes = C.c_size_t()
@@ -381,6 +470,22 @@ class Problem:
 
     def _stream(self):
         return C.c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream)
+
+    def nd_problem_stream_view(self):
+        """Diagnostics (nd.h): the swath kernel's chunk stream copied back from the workspace, as numpy arrays."""
+        v = nd_stream_device_view_t()
+        _check(lib().nd_problem_stream_view(self._h, C.byref(v)), "nd_problem_stream_view")
+        base, t = self.workspace.data_ptr(), self.torch
+
+        def grab(ptr, nbytes, dtype):
+            off = int(ptr) - base
+            return self.workspace[off:off + int(nbytes)].cpu().numpy().view(dtype)
+        NT = v.tracks_per_swath
+        return dict(blob=grab(v.blob, v.blob_bytes, np.uint8), tile_ref=grab(v.tile_ref, 8 * (v.n_tiles + 1), np.uint32).reshape(-1, 2),
+                    swath_tile0=grab(v.swath_tile0, 8 * (v.n_swaths + 1), np.int64),
+                    swath_track=grab(v.swath_track, 4 * v.n_swaths * NT, np.int32).reshape(-1, NT),
+                    items=grab(v.items, 16 * v.n_items, np.int32).reshape(-1, 4), n_tiles=v.n_tiles, n_swaths=v.n_swaths,
+                    tracks_per_swath=NT, built_on_device=bool(v.built_on_device))
 
     def nd_tally_reducer_set(self, fn):
         """NEXT-2 (nd.h): fn(tally) is called after every sweep with a torch FP64 tensor that ALIASES the problem's padded
@@ -710,7 +815,10 @@ def nd_swath_stream_build(region_material, n_materials, seg_offset, seg_region, 
 
 def nd_problem_create(xs, polar_sin, polar_weight, region_material, tracks, **options) -> Problem:
     """Convenience: build a Problem from a cross-section set (arrays sigma_t, sigma_s, nu_sigma_f, chi) and Tracks."""
+    host_build = options.pop("host_build", False)       # device-resident tracks: materialise them and use the host builder
+    resident = getattr(tracks, "seg_device", None) is not None and not host_build
     return Problem(region_material, xs.sigma_t, xs.sigma_s, xs.nu_sigma_f, xs.chi, polar_sin, polar_weight,
-                   tracks.seg_offset, tracks.seg_region, tracks.seg_length, tracks.track_weight, tracks.link,
-                   track_azim=tracks.track_azim, track_ends=tracks.ends,
-                   region_volume=tracks.volume if getattr(tracks, "is_shard", False) else None, **options)
+                   tracks.seg_offset, None if resident else tracks.seg_region, None if resident else tracks.seg_length,
+                   tracks.track_weight, tracks.link, track_azim=tracks.track_azim, track_ends=tracks.ends,
+                   seg_device=tracks.seg_device if resident else None,
+                   region_volume=getattr(tracks, "volume", None), **options)     # the library's own A~_r (whole laydown for a shard)

@@ -16,11 +16,11 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libnd_moc.so")
 BUILD = os.path.join(HERE, "build")
 
-NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC", "-Xcompiler", "-fopenmp",
               "-Xptxas", "-v", "--expt-relaxed-constexpr"]
 GXX_FLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fopenmp", "-fPIC", "-Wall"]
 
-CU_SOURCES = ["nd_api.cu", "nd_trace_device.cu", "nd_microbench.cu"]
+CU_SOURCES = ["nd_api.cu", "nd_trace_device.cu", "nd_microbench.cu", "nd_swath_device.cu"]
 CXX_SOURCES = ["nd_tracks.cpp", "nd_swath.cpp", "nd_cmfd_host.cpp"]
 
 

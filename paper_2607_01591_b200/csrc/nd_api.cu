@@ -11,6 +11,7 @@
 #include <vector>
 
 #include <cuda_runtime.h>
+#include <omp.h>
 
 #include "nd.h"
 #include "nd_internal.h"
@@ -19,6 +20,8 @@
 #include "nd_p1.cuh"
 #include "nd_sweep_swath.cuh"
 #include "nd_swath.h"
+#include "nd_swath_device.h"
+#include "nd_setup.cuh"
 
 // ------------------------------------------------------------------------------------------------
 // errors
@@ -206,7 +209,8 @@ int select_kernel(const nd_problem_desc* desc, const nd_options& opt, const Swat
 
 struct Layout { // byte offsets into the workspace
     size_t seg_rm, seg_len, trk_off, trk_w, link_src, psi_a, psi_b, q, tally, phi_a, phi_b, Q, reg_mat, vol, sigt, sigsT,
-        nusf, chi, sigt_f, scalars, partial, partial_b, exit_vac, stats, src_region, src_chunks, phase, blob, tile_chunk, swath_tile0, swath_track, items, counter, total;
+        nusf, chi, sigt_f, scalars, partial, partial_b, exit_vac, stats, src_region, src_chunks, phase, setup, slot_start, blob, tile_chunk, swath_tile0, swath_track, items, counter, total;
+    size_t slot_start_bytes;
 };
 
 inline size_t bump(size_t& cur, size_t bytes)
@@ -216,7 +220,14 @@ inline size_t bump(size_t& cur, size_t bytes)
     return at;
 }
 
-Layout make_layout(const Dims& d, int max_stats, const SwathConfig& sc, int kernel, bool keep_soa)
+// scratch of nd_problem_create's device passes (nd_problem_desc.seg_on_device): raw offsets, 2 * weights, entry regions, flags
+inline size_t setup_scratch_bytes(const Dims& d, const SwathConfig& sc, int kernel)
+{
+    const size_t T = (size_t)d.T;
+    return 4 * kAlign + 8 * (T + 1) + 8 * T + 8 * T + 256 + (is_swath(kernel) ? nd_swath_device_scratch_bytes(d.T, sc.max_swaths) : 0);
+}
+
+Layout make_layout(const Dims& d, int max_stats, const SwathConfig& sc, int kernel, bool keep_soa, bool seg_dev)
 {
     Layout L{};
     size_t c = 0;
@@ -252,6 +263,12 @@ Layout make_layout(const Dims& d, int max_stats, const SwathConfig& sc, int kern
     L.phase = bump(c, 256);
     L.src_region = bump(c, sizeof(int32_t) * (size_t)d.R);
     L.src_chunks = bump(c, sizeof(int4) * ((size_t)d.R / 4 + (size_t)d.M + 1));   // chunks hold >= 4 regions except one per material
+    if (seg_dev) {
+        L.setup = bump(c, setup_scratch_bytes(d, sc, kernel));
+        // the CMFD crossing lists are built on the host from every tile's slot_start array: the device builder writes them here
+        L.slot_start_bytes = is_swath(kernel) && keep_soa ? 2 * (size_t)sc.max_tiles * (sc.sp.NT + 1) : 0;
+        L.slot_start = bump(c, L.slot_start_bytes);
+    }
     if (is_swath(kernel)) {
         L.blob = bump(c, sc.max_blob);
         L.tile_chunk = bump(c, sizeof(uint2) * (size_t)sc.max_tiles);
@@ -315,7 +332,9 @@ struct nd_problem {
     uint8_t* blob = nullptr; uint2* tile_ref = nullptr; int64_t* swath_tile0 = nullptr; int32_t* swath_track = nullptr;
     int4* items = nullptr; int* counter = nullptr;
     int n_items = 0;
-    int64_t n_tiles = 0;
+    int64_t n_tiles = 0, n_swaths = 0;
+    size_t blob_bytes = 0;
+    bool stream_on_device = false;          // the chunk stream was built by nd_build_swaths_device
     double mean_regions_per_tile = 0.0, mean_segments_per_tile = 0.0;
     // host copies
     std::vector<double> h_vol;
@@ -574,7 +593,7 @@ extern "C" nd_status nd_workspace_bytes(const nd_problem_desc* desc, const nd_op
     if (opts) opt = *opts;
     SwathConfig sc;
     if (is_swath(opt.sweep_kernel) || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt);
-    *device_bytes = make_layout(d, kMaxStats, sc, select_kernel(desc, opt, sc), opt.cmfd_stream != 0).total;
+    *device_bytes = make_layout(d, kMaxStats, sc, select_kernel(desc, opt, sc), opt.cmfd_stream != 0, desc->seg_on_device != 0).total;
     return ND_OK;
 }
 
@@ -606,7 +625,12 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     SwathConfig sc;
     if (is_swath(opt.sweep_kernel) || opt.sweep_kernel == ND_SWEEP_AUTO) sc = make_swath_config(d, opt);
     const int kernel = select_kernel(desc, opt, sc);
-    const Layout L = make_layout(d, kMaxStats, sc, kernel, opt.cmfd_stream != 0);
+    const bool seg_dev = desc->seg_on_device != 0;
+    if (desc->seg_on_device < 0 || desc->seg_on_device > 1 || desc->reserved != 0)
+        return nd_fail(ND_ERR_INVALID, "nd_problem_desc.seg_on_device must be 0 or 1, reserved 0");
+    if (seg_dev && !desc->track_azim)
+        return nd_fail(ND_ERR_INVALID, "device-resident segments need the track geometry (track_azim, track_ends)");
+    const Layout L = make_layout(d, kMaxStats, sc, kernel, opt.cmfd_stream != 0, seg_dev);
     if (reinterpret_cast<uintptr_t>(device_workspace) % kAlign != 0) return nd_fail(ND_ERR_WORKSPACE, "workspace must be 256-byte aligned");
     if (device_bytes < L.total) return nd_fail(ND_ERR_WORKSPACE, "workspace smaller than nd_workspace_bytes");
 
@@ -629,9 +653,15 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     if (std::fabs(wsum - 1.0) > 1e-9) return nd_fail(ND_ERR_INVALID, "polar_weight must sum to 1");
     for (int t = 0; t < d.T; ++t)
         if (!(desc->track_weight[t] > 0.0) || !std::isfinite(desc->track_weight[t])) return nd_fail(ND_ERR_INVALID, "track_weight must be finite and > 0");
-    for (int64_t k = 0; k < d.S; ++k) {
-        if (desc->seg_region[k] < 0 || desc->seg_region[k] >= d.R) return nd_fail(ND_ERR_RANGE, "seg_region out of range");
-        if (!(desc->seg_length[k] > 0.0) || !std::isfinite(desc->seg_length[k])) return nd_fail(ND_ERR_INVALID, "seg_length must be finite and > 0");
+    if (!seg_dev) {   // 5e8 segments at config 5: all host threads (device-resident segments: k_seg_validate below)
+        int bad_region = 0, bad_length = 0;
+#pragma omp parallel for schedule(static) reduction(| : bad_region, bad_length)
+        for (int64_t k = 0; k < d.S; ++k) {
+            bad_region |= desc->seg_region[k] < 0 || desc->seg_region[k] >= d.R;
+            bad_length |= !(desc->seg_length[k] > 0.0) || !std::isfinite(desc->seg_length[k]);
+        }
+        if (bad_region) return nd_fail(ND_ERR_RANGE, "seg_region out of range");
+        if (bad_length) return nd_fail(ND_ERR_INVALID, "seg_length must be finite and > 0");
     }
     std::vector<int32_t> link_src;
     std::vector<uint8_t> h_exit_vac;
@@ -660,28 +690,49 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         p->h_vol.assign((size_t)d.R, 0.0);
         p->h_entry_region.assign(2 * (size_t)d.T, -1);
         int64_t o = 0;
-        for (int t = 0; t < d.T; ++t) {
+        for (int t = 0; t < d.T; ++t) {                   // padded offsets and the entry regions of both directions
             h_off[t] = o;
             const int64_t k0 = desc->track_seg_offset[t], k1 = desc->track_seg_offset[t + 1];
-            if (k1 > k0) {
+            if (k1 > k0 && !seg_dev) {
                 p->h_entry_region[2 * (size_t)t] = desc->seg_region[k0];
                 p->h_entry_region[2 * (size_t)t + 1] = desc->seg_region[k1 - 1];
             }
-            const double w2 = 2.0 * desc->track_weight[t];
-            uint32_t last = 0;
-            for (int64_t k = k0; k < k1; ++k) {
-                const int32_t r = desc->seg_region[k];
-                p->h_vol[r] += w2 * desc->seg_length[k];
-                if (soa) {
-                    last = ndk::pack_rm((uint32_t)r, (uint32_t)desc->region_material[r]);
-                    h_rm[o] = last;
-                    h_len[o] = (float)desc->seg_length[k];
-                }
-                ++o;
-            }
-            while (o % 4 != 0) { if (soa) { h_rm[o] = last; h_len[o] = 0.f; } ++o; } // zero-length segments are exact no-ops
+            o += (k1 - k0 + 3) / 4 * 4;
         }
         h_off[d.T] = o;
+        if (soa && !seg_dev) {
+#pragma omp parallel for schedule(dynamic, 256)
+            for (int t = 0; t < d.T; ++t) {
+                int64_t at = h_off[t];
+                uint32_t last = 0;
+                for (int64_t k = desc->track_seg_offset[t]; k < desc->track_seg_offset[t + 1]; ++k, ++at) {
+                    const int32_t r = desc->seg_region[k];
+                    last = ndk::pack_rm((uint32_t)r, (uint32_t)desc->region_material[r]);
+                    h_rm[at] = last;
+                    h_len[at] = (float)desc->seg_length[k];
+                }
+                for (; at < h_off[t + 1]; ++at) { h_rm[at] = last; h_len[at] = 0.f; }   // zero-length segments are exact no-ops
+            }
+        }
+        if (!desc->region_volume && !seg_dev) {
+            // O-5: A~_r = sum 2 omega_a delta_a s.  Small problems: one thread, canonical (track, segment) order.  Large ones:
+            // every thread sums a contiguous range of tracks into its own array, the arrays are added in thread order.
+            const int nth = d.S > (1 << 22) ? std::max(1, std::min(omp_get_max_threads(), 16)) : 1;
+            std::vector<double> part((size_t)d.R * (nth > 1 ? nth : 0), 0.0);
+#pragma omp parallel num_threads(nth)
+            {
+                const int me = omp_get_thread_num();
+                double* vol = nth > 1 ? part.data() + (size_t)d.R * me : p->h_vol.data();
+                const int t0 = (int)((int64_t)d.T * me / nth), t1 = (int)((int64_t)d.T * (me + 1) / nth);
+                for (int t = t0; t < t1; ++t) {
+                    const double w2 = 2.0 * desc->track_weight[t];
+                    for (int64_t k = desc->track_seg_offset[t]; k < desc->track_seg_offset[t + 1]; ++k)
+                        vol[desc->seg_region[k]] += w2 * desc->seg_length[k];
+                }
+            }
+            for (int th = 0; th < (nth > 1 ? nth : 0); ++th)
+                for (int r = 0; r < d.R; ++r) p->h_vol[(size_t)r] += part[(size_t)d.R * th + r];
+        }
         if (desc->region_volume) {   // a shard of an angle-pair partition: the areas of the whole laydown (nd_tracks_shard)
             for (int r = 0; r < d.R; ++r) {
                 if (!(desc->region_volume[r] >= 0.0) || !std::isfinite(desc->region_volume[r])) {
@@ -699,7 +750,7 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     NdSwathSet swaths;
     const bool want_swath = is_swath(kernel);
     const bool tiled = want_swath;
-    if (want_swath) {
+    if (want_swath && !seg_dev) {
         rc = nd_build_swaths(desc, desc->track_azim, desc->track_ends, sc.sp, 0, &swaths);
         if (rc != ND_OK) { delete p; return rc; }
         if (swaths.blob.size() > sc.max_blob || swaths.n_tiles + 1 > sc.max_tiles || swaths.n_swaths > sc.max_swaths ||
@@ -782,10 +833,10 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         }                                                                                               \
     } while (0)
     ND_CUDA_P(cudaMemsetAsync(ws, 0, tiled ? L.blob : L.total, st));
-    if (want_swath) {
+    if (want_swath && !seg_dev) {
         static_assert(sizeof(NdSwathItem) == sizeof(int4), "work item layout");
         p->n_items = (int)swaths.items.size();
-        p->n_tiles = swaths.n_tiles;
+        p->n_tiles = swaths.n_tiles; p->n_swaths = swaths.n_swaths; p->blob_bytes = swaths.blob.size();
         p->mean_regions_per_tile = swaths.mean_regions_per_tile;
         p->mean_segments_per_tile = swaths.mean_segments_per_tile;
         p->lockstep_efficiency = swaths.lockstep_efficiency;
@@ -801,8 +852,10 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         ND_CUDA_P(cudaMemcpyAsync(p->swath_track, swaths.swath_track.data(), sizeof(int32_t) * swaths.swath_track.size(), cudaMemcpyHostToDevice, st));
         ND_CUDA_P(cudaMemcpyAsync(p->items, swaths.items.data(), sizeof(NdSwathItem) * swaths.items.size(), cudaMemcpyHostToDevice, st));
     }
-    ND_CUDA_P(cudaMemcpyAsync(p->seg_rm, h_rm.data(), sizeof(uint32_t) * h_rm.size(), cudaMemcpyHostToDevice, st));
-    ND_CUDA_P(cudaMemcpyAsync(p->seg_len, h_len.data(), sizeof(float) * h_len.size(), cudaMemcpyHostToDevice, st));
+    if (!seg_dev) {
+        ND_CUDA_P(cudaMemcpyAsync(p->seg_rm, h_rm.data(), sizeof(uint32_t) * h_rm.size(), cudaMemcpyHostToDevice, st));
+        ND_CUDA_P(cudaMemcpyAsync(p->seg_len, h_len.data(), sizeof(float) * h_len.size(), cudaMemcpyHostToDevice, st));
+    }
     ND_CUDA_P(cudaMemcpyAsync(p->trk_off, h_off.data(), sizeof(int64_t) * h_off.size(), cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->trk_w, h_w.data(), sizeof(float) * h_w.size(), cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->link_src, link_src.data(), sizeof(int32_t) * link_src.size(), cudaMemcpyHostToDevice, st));
@@ -816,6 +869,60 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     ND_CUDA_P(cudaMemcpyAsync(p->sigt_f, h_sigt_f.data(), sizeof(float) * h_sigt_f.size(), cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->src_region, h_src_region.data(), sizeof(int32_t) * h_src_region.size(), cudaMemcpyHostToDevice, st));
     ND_CUDA_P(cudaMemcpyAsync(p->src_chunks, h_src_chunks.data(), sizeof(int4) * h_src_chunks.size(), cudaMemcpyHostToDevice, st));
+    if (seg_dev) {
+        // ---- the segment passes on the GPU: validation first (everything after it indexes with the region ids) ----
+        char* sx = ws + L.setup;
+        int* d_flags = (int*)sx; sx += kAlign;
+        int64_t* d_off = (int64_t*)sx; sx += (8 * ((size_t)d.T + 1) + kAlign - 1) / kAlign * kAlign;
+        double* d_w2 = (double*)sx; sx += (8 * (size_t)d.T + kAlign - 1) / kAlign * kAlign;
+        int32_t* d_entry = (int32_t*)sx; sx += (8 * (size_t)d.T + kAlign - 1) / kAlign * kAlign;
+        std::vector<double> h_w2((size_t)d.T);
+        for (int t = 0; t < d.T; ++t) h_w2[(size_t)t] = 2.0 * desc->track_weight[t];
+        ND_CUDA_P(cudaMemcpyAsync(d_off, desc->track_seg_offset, 8 * ((size_t)d.T + 1), cudaMemcpyHostToDevice, st));
+        ND_CUDA_P(cudaMemcpyAsync(d_w2, h_w2.data(), 8 * (size_t)d.T, cudaMemcpyHostToDevice, st));
+        ndk::k_seg_validate<<<grid_for(d.S, 256, 16 * p->n_sm), 256, 0, st>>>(desc->seg_region, desc->seg_length, d.S, d.R, d_flags);
+        ND_CUDA_P(cudaGetLastError());
+        int h_flags = 0;
+        ND_CUDA_P(cudaMemcpyAsync(&h_flags, d_flags, sizeof(int), cudaMemcpyDeviceToHost, st));
+        ND_CUDA_P(cudaStreamSynchronize(st));
+        if (h_flags & 1) return fail(nd_fail(ND_ERR_RANGE, "seg_region out of range"));
+        if (h_flags & 2) return fail(nd_fail(ND_ERR_INVALID, "seg_length must be finite and > 0"));
+        const int tb = (d.T + 127) / 128;
+        ndk::k_entry_regions<<<(d.T + 255) / 256, 256, 0, st>>>(d_off, desc->seg_region, d.T, d_entry);
+        ND_CUDA_P(cudaGetLastError());
+        ND_CUDA_P(cudaMemcpyAsync(p->h_entry_region.data(), d_entry, 8 * (size_t)d.T, cudaMemcpyDeviceToHost, st));
+        if (p->has_soa) {
+            ndk::k_pack_soa<<<tb, 128, 0, st>>>(d_off, p->trk_off, desc->seg_region, desc->seg_length, p->reg_mat, d.T, p->seg_rm, p->seg_len);
+            ND_CUDA_P(cudaGetLastError());
+        }
+        if (!desc->region_volume) {   // p->vol holds the zeros uploaded above
+            ndk::k_track_volume<<<tb, 128, 0, st>>>(d_off, desc->seg_region, desc->seg_length, d_w2, d.T, p->vol);
+            ND_CUDA_P(cudaGetLastError());
+            ND_CUDA_P(cudaMemcpyAsync(p->h_vol.data(), p->vol, 8 * (size_t)d.R, cudaMemcpyDeviceToHost, st));
+        }
+        if (want_swath) {
+            NdSwathDeviceTargets tg;
+            tg.blob = p->blob; tg.blob_cap = sc.max_blob; tg.tile_ref = p->tile_ref; tg.tile_cap = sc.max_tiles;
+            tg.swath_tile0 = p->swath_tile0; tg.max_swaths = sc.max_swaths; tg.swath_track = p->swath_track; tg.items = p->items;
+            tg.slot_start = L.slot_start_bytes ? (uint16_t*)(ws + L.slot_start) : nullptr; tg.slot_start_cap = L.slot_start_bytes;
+            tg.scratch = sx;
+            rc = nd_build_swaths_device(desc, p->reg_mat, sc.sp, tg, st, &swaths);
+            if (rc != ND_OK) return fail(rc);
+            if (swaths.max_head_bytes > sc.head_cap || swaths.max_rec_bytes > sc.rec_cap)
+                return fail(nd_fail(ND_ERR_WORKSPACE, "internal: swath stream larger than its workspace bound"));
+            p->n_items = (int)swaths.items.size();
+            p->n_tiles = swaths.n_tiles; p->n_swaths = swaths.n_swaths; p->blob_bytes = swaths.blob_bytes_device;
+            p->stream_on_device = true;
+            p->mean_regions_per_tile = swaths.mean_regions_per_tile;
+            p->mean_segments_per_tile = swaths.mean_segments_per_tile;
+            p->lockstep_efficiency = swaths.lockstep_efficiency;
+            if (opt.cmfd_stream) {
+                p->h_swath_track = swaths.swath_track;
+                p->h_swath_tile0 = swaths.swath_tile0;
+                p->h_slot_start.swap(swaths.slot_start);
+            }
+        }
+    }
     ND_CUDA_P(cudaStreamSynchronize(st));
 #undef ND_CUDA_P
     rc = reset_state(p, st);
@@ -1132,6 +1239,18 @@ extern "C" nd_status nd_sweep_phases_get(nd_problem* p, double* host_out)
     double tot = 0.0;
     for (int i = 0; i < ndk::kSwathPhases; ++i) tot += (double)h[i];
     for (int i = 0; i < ndk::kSwathPhases; ++i) host_out[i] = tot > 0.0 ? (double)h[i] / tot : 0.0;
+    return ND_OK;
+}
+
+extern "C" nd_status nd_problem_stream_view(const nd_problem* p, nd_stream_device_view_t* out)
+{
+    if (!p || !out) return nd_fail(ND_ERR_NULL, "nd_problem_stream_view: NULL argument");
+    if (!is_swath(p->sweep_kernel)) return nd_fail(ND_ERR_STATE, "nd_problem_stream_view: the problem does not run the swath kernel");
+    memset(out, 0, sizeof *out);
+    out->blob = p->blob; out->blob_bytes = p->blob_bytes; out->tile_ref = reinterpret_cast<const uint32_t*>(p->tile_ref);
+    out->swath_tile0 = p->swath_tile0; out->swath_track = p->swath_track; out->items = reinterpret_cast<const int32_t*>(p->items);
+    out->n_tiles = p->n_tiles; out->n_swaths = p->n_swaths; out->n_items = p->n_items;
+    out->tracks_per_swath = p->sc.sp.NT; out->built_on_device = p->stream_on_device ? 1 : 0;
     return ND_OK;
 }
 

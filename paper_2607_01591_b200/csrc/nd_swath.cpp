@@ -12,42 +12,74 @@
 
 #include "nd_internal.h"
 #include "nd_swath.h"
+#include "nd_swath_core.h"
 
 namespace {
 
 struct SwathBuild {
     std::vector<uint8_t> bytes;        // this swath's chunks, concatenated
-    std::vector<uint32_t> chunk_rel;   // chunk offsets relative to the swath's first byte, 16-B units
-    std::vector<uint32_t> head16;      // head size of every chunk, 16-B units
+    std::vector<uint32_t> ref;         // per chunk: offset from the swath's first byte, head size (16-B units)
     std::vector<uint16_t> slot_start;  // [tiles][NT+1] when requested
     int64_t n_seg = 0, sum_regions = 0, sum_max_cnt = 0, n_active = 0;
     int max_head = 0, max_rec = 0;
-    int32_t group = 0;                 // angle id of the swath's tracks
-    double perp = 0.0;                 // perpendicular coordinate of its first track
 };
 
 } // namespace
 
-nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim, const double* track_ends,
-                          const NdSwathParams& prm, int n_threads, NdSwathSet* out)
+// The length under which the fronts of a swath's tracks count as level: `lag` mean segment lengths.  With track geometry the
+// mean is (sum of the tracks' end-to-end lengths) / S, formed in track order on the host -- the same number whether the
+// segments live on the host or on the device; without geometry it is the mean of the segment lengths themselves.
+double nd_swath_lag_length(const nd_problem_desc* desc, const double* track_ends, double lag, int n_threads)
 {
-    const int T = desc->n_tracks, R = desc->n_regions, NT = prm.NT, Kmax = prm.Kmax, Lmax = prm.Lmax, NC = prm.NC;
+    if (lag < 0.0) return -1.0;
+    const int T = desc->n_tracks;
+    const int64_t S = desc->track_seg_offset[T];
+    if (S <= 0) return 0.0;
+    double sum = 0.0;
+    if (track_ends) {
+        for (int t = 0; t < T; ++t) {
+            if (desc->track_seg_offset[t + 1] == desc->track_seg_offset[t]) continue;
+            const double dx = track_ends[4 * (size_t)t + 2] - track_ends[4 * (size_t)t], dy = track_ends[4 * (size_t)t + 3] - track_ends[4 * (size_t)t + 1];
+            const double h = std::sqrt(dx * dx + dy * dy);
+            if (std::isfinite(h)) sum += h;
+        }
+    } else {
+#pragma omp parallel for reduction(+ : sum) num_threads(n_threads > 0 ? n_threads : 1)
+        for (int64_t k = 0; k < S; ++k) sum += desc->seg_length[k];
+    }
+    return lag * sum / (double)S;
+}
+
+nd_status nd_swath_check_params(const nd_problem_desc* desc, const NdSwathParams& prm, NdSwathCoreParams* core)
+{
+    const int NT = prm.NT, Kmax = prm.Kmax, Lmax = prm.Lmax, NC = prm.NC;
     if (NT < 1 || NT > 1024 || Kmax < 1 || Lmax < 1 || NC < 1 || NT % NC != 0 || prm.row_bytes < 16 || prm.row_bytes % 16 != 0)
         return nd_fail(ND_ERR_INVALID, "swath parameters out of range");
     const int64_t line = (int64_t)NC * prm.row_bytes;   // bytes between consecutive sigma_t rows in shared memory
     const int NCq = prm.NCq > 0 ? prm.NCq : NC;
     const int64_t line_q = (int64_t)NCq * prm.row_bytes; // bytes between consecutive q rows
-    const int64_t row_bytes = prm.row_bytes;             // bytes between consecutive delta rows
     if (Lmax > 65535 || (int64_t)NT * Kmax > 65535 || nd_swath_head_capacity(prm) / 16 > 65535 ||
         (int64_t)Lmax * line_q > (1ll << 30) || (int64_t)desc->n_materials * line > (1ll << 30))
         return nd_fail(ND_ERR_INVALID, "swath parameters: tile sizes must fit 16 bits");
+    core->NT = NT; core->Kmax = Kmax; core->Lmax = Lmax; core->line = line; core->line_q = line_q;
+    core->row_bytes = prm.row_bytes;   // bytes between consecutive delta rows
+    core->lag_len = -1.0;
+    return ND_OK;
+}
+
+// Steps 1 and 2 of the build, which need the track geometry but no segment: which tracks share a swath.
+nd_status nd_swath_plan(const nd_problem_desc* desc, const int32_t* track_azim, const double* track_ends, const NdSwathParams& prm,
+                        NdSwathPlan* plan)
+{
+    const int T = desc->n_tracks, NT = prm.NT;
     try {
-        out->prm = prm;
         // ---- 1. order tracks: by angle id, then by perpendicular coordinate ----
         std::vector<int32_t> order(T);
         std::iota(order.begin(), order.end(), 0);
-        std::vector<double> lam0(T, 0.0), perp(T, 0.0);
+        std::vector<double> perp(T, 0.0);
         std::vector<int32_t> group(T, 0);
+        plan->lam0.assign((size_t)T, 0.0);
+        std::vector<double>& lam0 = plan->lam0;
         if (track_azim && track_ends) {
             int32_t gmax = 0;
             for (int t = 0; t < T; ++t) { group[t] = track_azim[t] < 0 ? 0 : track_azim[t]; gmax = std::max(gmax, group[t]); }
@@ -75,16 +107,68 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
             });
         }
         // ---- 2. swaths: NT consecutive tracks of one group ----
-        std::vector<int32_t>& st = out->swath_track;
+        std::vector<int32_t>& st = plan->swath_track;
         st.clear();
+        plan->group.clear();
         for (int i = 0; i < T;) {
             int n = 0;
             const int g = group[order[i]];
             while (n < NT && i + n < T && group[order[i + n]] == g) ++n;
             for (int b = 0; b < NT; ++b) st.push_back(b < n ? order[i + b] : -1);
+            plan->group.push_back(g);
             i += n;
         }
-        const int64_t n_sw = (int64_t)(st.size() / NT);
+        plan->n_swaths = (int64_t)(st.size() / NT);
+    } catch (const std::bad_alloc&) {
+        return nd_fail(ND_ERR_NOMEM, "nd_swath_plan: out of host memory");
+    }
+    return ND_OK;
+}
+
+// Step 5: the work items (swath, direction) from every swath's cost (sum over its tiles of the longest slot).
+void nd_swath_items(const NdSwathPlan& plan, const int64_t* cost, int item_order, std::vector<NdSwathItem>* items)
+{
+    const int64_t n_sw = plan.n_swaths;
+    items->clear();
+    if (item_order == 0) {   // most expensive first
+        for (int64_t sw = 0; sw < n_sw; ++sw) {
+            const int32_t c32 = (int32_t)std::min<int64_t>(cost[sw], INT32_MAX);
+            items->push_back({(int32_t)sw, 0, c32, 0});
+            items->push_back({(int32_t)sw, 1, c32, 0});
+        }
+        std::stable_sort(items->begin(), items->end(), [](const NdSwathItem& a, const NdSwathItem& b) { return a.cost > b.cost; });
+    } else {
+        // Angle by angle; inside an angle all forward items in the order of the perpendicular coordinate, then all
+        // backward items: thread blocks that run at the same time carry neighbouring swaths at the same stage of their
+        // tracks, so the q and tally rows of the triangles two swaths share are still in L2 for the second one.  Swaths
+        // are already stored in (angle, perpendicular) order; the last items of the last angle are short corner swaths.
+        for (int64_t a = 0; a < n_sw;) {
+            int64_t b = a;
+            while (b < n_sw && plan.group[(size_t)b] == plan.group[(size_t)a]) ++b;
+            for (int dir = 0; dir < 2; ++dir)
+                for (int64_t sw = a; sw < b; ++sw)
+                    items->push_back({(int32_t)sw, dir, (int32_t)std::min<int64_t>(cost[sw], INT32_MAX), 0});
+            a = b;
+        }
+    }
+}
+
+nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim, const double* track_ends,
+                          const NdSwathParams& prm, int n_threads, NdSwathSet* out)
+{
+    const int NT = prm.NT, Kmax = prm.Kmax, Lmax = prm.Lmax;
+    NdSwathCoreParams cp{};
+    nd_status rc0 = nd_swath_check_params(desc, prm, &cp);
+    if (rc0 != ND_OK) return rc0;
+    NdSwathPlan plan;
+    rc0 = nd_swath_plan(desc, track_azim, track_ends, prm, &plan);
+    if (rc0 != ND_OK) return rc0;
+    try {
+        out->prm = prm;
+        out->swath_track = plan.swath_track;
+        const std::vector<int32_t>& st = out->swath_track;
+        const std::vector<double>& lam0 = plan.lam0;
+        const int64_t n_sw = plan.n_swaths;
         out->n_swaths = n_sw;
         // ---- 3. cut every swath into tiles and encode the chunks ----
         std::vector<SwathBuild> built((size_t)n_sw);
@@ -95,145 +179,53 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
         (void)n_threads;
 #endif
         const int64_t* off = desc->track_seg_offset;
-        double lag_len = -1.0;
-        if (prm.lag >= 0.0) {
-            double sum = 0.0;
-            const int64_t S = off[T];
-#pragma omp parallel for reduction(+ : sum) num_threads(nth)
-            for (int64_t k = 0; k < S; ++k) sum += desc->seg_length[k];
-            lag_len = S > 0 ? prm.lag * sum / (double)S : 0.0;
-        }
+        const double lag_len = nd_swath_lag_length(desc, track_ends, prm.lag, nth);
+        cp.lag_len = lag_len;
+        const int head_cap = nd_swath_head_capacity(prm), min_tile = Kmax < Lmax ? Kmax : Lmax;
+        bool oom = false;
 #pragma omp parallel num_threads(nth)
         {
-            std::vector<int32_t> stamp((size_t)R, -1), lidx((size_t)R, 0);
-            int32_t tile_serial = 0;
-            std::vector<int64_t> cur(NT), first(NT), endk(NT);
-            std::vector<double> lam(NT);
-            std::vector<int> cnt(NT);
-            std::vector<uint32_t> regions;
-            std::vector<int> rcount, rfill, perm, sorted_count;
-            std::vector<uint32_t> sorted_regions;
-            regions.reserve(Lmax);
+            // the cutter / encoder of one swath is nd_swath_core (shared with the device builder); it fills a thread-local
+            // buffer sized for the swath's upper bound, the used part is kept
+            std::vector<uint8_t> scratch((size_t)nd_swath_scratch_bytes(NT, Kmax, Lmax)), tmp;
+            std::vector<uint32_t> ref;
+            std::vector<uint16_t> sst;
+            const NdSwathScratch sc = nd_swath_scratch_at(scratch.data(), NT, Kmax, Lmax);
 #pragma omp for schedule(dynamic, 4)
             for (int64_t sw = 0; sw < n_sw; ++sw) {
+                if (oom) continue;
                 SwathBuild& sb = built[(size_t)sw];
                 const int32_t* trk = &st[(size_t)sw * NT];
-                if (trk[0] >= 0) { sb.group = group[trk[0]]; sb.perp = perp[trk[0]]; }
-                int64_t remaining = 0;
-                for (int b = 0; b < NT; ++b) {
-                    if (trk[b] >= 0) { cur[b] = off[trk[b]]; endk[b] = off[trk[b] + 1]; lam[b] = lam0[trk[b]]; ++sb.n_active; }
-                    else { cur[b] = endk[b] = 0; lam[b] = 0.0; }
-                    remaining += endk[b] - cur[b];
-                }
-                sb.n_seg = remaining;
-                while (remaining > 0) {
-                    if (++tile_serial == INT32_MAX) { std::fill(stamp.begin(), stamp.end(), -1); tile_serial = 0; }
-                    regions.clear();
-                    rcount.clear();
-                    for (int b = 0; b < NT; ++b) { first[b] = cur[b]; cnt[b] = 0; }
-                    int nseg = 0;
-                    auto take = [&](int b) -> bool {   // next segment of track b into the tile; false: region window full
-                        const int64_t k = cur[b];
-                        const int32_t r = desc->seg_region[k];
-                        if (stamp[r] != tile_serial) {
-                            if ((int)regions.size() == Lmax) return false;
-                            stamp[r] = tile_serial;
-                            lidx[r] = (int32_t)regions.size();
-                            regions.push_back((uint32_t)r);
-                            rcount.push_back(0);
-                        }
-                        ++rcount[lidx[r]];
-                        lam[b] += desc->seg_length[k];
-                        ++cur[b]; ++cnt[b]; ++nseg; --remaining;
-                        return true;
-                    };
-                    bool level = false;
-                    if (lag_len >= 0.0) {
-                        double lo = 0.0, hi = 0.0;
-                        bool any = false;
-                        for (int b = 0; b < NT; ++b)
-                            if (cur[b] < endk[b]) {
-                                if (!any) { lo = hi = lam[b]; any = true; }
-                                else { lo = std::min(lo, lam[b]); hi = std::max(hi, lam[b]); }
-                            }
-                        level = hi - lo <= lag_len;
-                    }
-                    if (level) {   // equal counts: round j gives every unfinished track its j-th segment
-                        bool full = false;
-                        for (int j = 0; j < Kmax && !full && remaining > 0; ++j)
-                            for (int b = 0; b < NT; ++b)
-                                if (cur[b] < endk[b] && cnt[b] == j && !take(b)) { full = true; break; }
-                    } else {       // geometric: the track furthest behind advances
-                        for (;;) {
-                            int bs = -1;
-                            for (int b = 0; b < NT; ++b)
-                                if (cur[b] < endk[b] && (bs < 0 || lam[b] < lam[bs])) bs = b;
-                            if (bs < 0 || cnt[bs] == Kmax || !take(bs)) break;
-                        }
-                    }
-                    // ---- encode ----
-                    const int L = (int)regions.size();
-                    {   // regions in descending order of their segment count: the flush units of one pass have lists of similar length
-                        perm.resize(L);
-                        std::iota(perm.begin(), perm.end(), 0);
-                        std::stable_sort(perm.begin(), perm.end(), [&](int a, int b) { return rcount[a] > rcount[b]; });
-                        sorted_regions.resize(L); sorted_count.resize(L);
-                        for (int l = 0; l < L; ++l) { sorted_regions[l] = regions[perm[l]]; sorted_count[l] = rcount[perm[l]]; lidx[regions[perm[l]]] = l; }
-                        regions.swap(sorted_regions); rcount.swap(sorted_count);
-                    }
-                    const int o_ss = 16;
-                    const int o_rg = o_ss + nd_swath_pad16(2 * (NT + 1));
-                    const int o_rc = o_rg + nd_swath_pad16(8 * L);   // = head bytes
-                    const int bytes = o_rc + 16 * nseg;
-                    const size_t base = sb.bytes.size();
-                    sb.chunk_rel.push_back((uint32_t)(base / 16));
-                    sb.head16.push_back((uint32_t)(o_rc / 16));
-                    sb.bytes.resize(base + (size_t)bytes, 0);
-                    uint8_t* c = sb.bytes.data() + base;
-                    const uint32_t hdr[4] = {(uint32_t)L | ((uint32_t)nseg << 16), (uint32_t)(o_rg / 16),
-                                             (uint32_t)o_rc, (uint32_t)bytes};
-                    memcpy(c, hdr, 16);
-                    uint16_t* ss = reinterpret_cast<uint16_t*>(c + o_ss);
-                    uint32_t* rg = reinterpret_cast<uint32_t*>(c + o_rg);
-                    uint32_t* rc = reinterpret_cast<uint32_t*>(c + o_rc);
-                    rfill.resize(L);
-                    for (int l = 0, e = 0; l < L; ++l) {
-                        rfill[l] = e;
-                        rg[2 * l] = regions[l];
-                        rg[2 * l + 1] = (uint32_t)e | ((uint32_t)(e + rcount[l]) << 16);
-                        e += rcount[l];
-                    }
-                    int o = 0, max_cnt = 0;
-                    for (int b = 0; b < NT; ++b) {
-                        ss[b] = (uint16_t)o;
-                        max_cnt = std::max(max_cnt, cnt[b]);
-                        for (int j = 0; j < cnt[b]; ++j, ++o) {
-                            const int64_t k = first[b] + j;
-                            const int32_t r = desc->seg_region[k];
-                            const int l = lidx[r];
-                            const float len = (float)desc->seg_length[k];
-                            uint32_t lenbits;
-                            memcpy(&lenbits, &len, 4);
-                            rc[4 * o] = lenbits;
-                            rc[4 * o + 1] = (uint32_t)(l * line_q);
-                            rc[4 * o + 2] = (uint32_t)(desc->region_material[r] * line);
-                            rc[4 * o + 3] = (uint32_t)(rfill[l]++ * row_bytes);   // region-major delta row: by slot, then along the track
-                        }
-                    }
-                    ss[NT] = (uint16_t)o;
-                    if (prm.keep_slot_start) sb.slot_start.insert(sb.slot_start.end(), ss, ss + NT + 1);
-                    sb.sum_regions += L;
-                    sb.sum_max_cnt += max_cnt;
-                    sb.max_head = std::max(sb.max_head, o_rc);
-                    sb.max_rec = std::max(sb.max_rec, 16 * nseg);
+                int64_t n_seg = 0;
+                for (int b = 0; b < NT; ++b)
+                    if (trk[b] >= 0) n_seg += off[trk[b] + 1] - off[trk[b]];
+                const int64_t max_tiles = n_seg / min_tile + NT + 1;
+                const size_t bound = 16 * (size_t)n_seg + (size_t)max_tiles * head_cap;
+                try {
+                    if (tmp.size() < bound) tmp.resize(bound);
+                    if ((int64_t)ref.size() < 2 * max_tiles) ref.resize(2 * (size_t)max_tiles);
+                    if (prm.keep_slot_start && sst.size() < (size_t)max_tiles * (NT + 1)) sst.resize((size_t)max_tiles * (NT + 1));
+                    memset(tmp.data(), 0, bound);
+                    NdSwathCoreOut co{};
+                    nd_swath_core<true>(cp, off, desc->seg_region, desc->seg_length, desc->region_material, trk, lam0.data(), sc, tmp.data(),
+                                        ref.data(), 0u, prm.keep_slot_start ? sst.data() : nullptr, &co);
+                    sb.bytes.assign(tmp.begin(), tmp.begin() + (size_t)co.n_bytes);
+                    sb.ref.assign(ref.begin(), ref.begin() + 2 * (size_t)co.n_tiles);
+                    if (prm.keep_slot_start) sb.slot_start.assign(sst.begin(), sst.begin() + (size_t)co.n_tiles * (NT + 1));
+                    sb.n_seg = co.n_seg; sb.sum_regions = co.sum_regions; sb.sum_max_cnt = co.sum_max_cnt; sb.n_active = co.n_active;
+                    sb.max_head = co.max_head; sb.max_rec = co.max_rec;
+                } catch (const std::bad_alloc&) {
+#pragma omp atomic write
+                    oom = true;
                 }
             }
         }
+        if (oom) return nd_fail(ND_ERR_NOMEM, "nd_build_swaths: out of host memory");
         // ---- 4. concatenate ----
         out->swath_tile0.assign((size_t)n_sw + 1, 0);
         std::vector<size_t> byte0((size_t)n_sw + 1, 0);
         for (int64_t sw = 0; sw < n_sw; ++sw) {
-            out->swath_tile0[sw + 1] = out->swath_tile0[sw] + (int64_t)built[sw].chunk_rel.size();
+            out->swath_tile0[sw + 1] = out->swath_tile0[sw] + (int64_t)(built[sw].ref.size() / 2);
             byte0[sw + 1] = byte0[sw] + built[sw].bytes.size();
         }
         out->n_tiles = out->swath_tile0[n_sw];
@@ -253,8 +245,8 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
             SwathBuild& sb = built[(size_t)sw];
             if (!sb.bytes.empty()) memcpy(out->blob.data() + byte0[sw], sb.bytes.data(), sb.bytes.size());
             const uint32_t b16 = (uint32_t)(byte0[sw] / 16);
-            for (size_t i = 0; i < sb.chunk_rel.size(); ++i)
-                out->tile_ref[(size_t)out->swath_tile0[sw] + i] = {b16 + sb.chunk_rel[i], sb.head16[i]};
+            for (size_t i = 0; i < sb.ref.size() / 2; ++i)
+                out->tile_ref[(size_t)out->swath_tile0[sw] + i] = {b16 + sb.ref[2 * i], sb.ref[2 * i + 1]};
             std::vector<uint8_t>().swap(sb.bytes);
         }
         if (prm.keep_slot_start) {
@@ -273,28 +265,9 @@ nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim
         out->mean_segments_per_tile = out->n_tiles ? (double)sum_seg / (double)out->n_tiles : 0.0;
         out->lockstep_efficiency = sum_slots ? (double)sum_seg / (double)sum_slots : 1.0;
         // ---- 5. work items (swath, direction) ----
-        out->items.clear();
-        if (prm.item_order == 0) {   // most expensive first
-            for (int64_t sw = 0; sw < n_sw; ++sw) {
-                const int32_t c32 = (int32_t)std::min<int64_t>(built[sw].sum_max_cnt, INT32_MAX);
-                out->items.push_back({(int32_t)sw, 0, c32, 0});
-                out->items.push_back({(int32_t)sw, 1, c32, 0});
-            }
-            std::stable_sort(out->items.begin(), out->items.end(), [](const NdSwathItem& a, const NdSwathItem& b) { return a.cost > b.cost; });
-        } else {
-            // Angle by angle; inside an angle all forward items in the order of the perpendicular coordinate, then all
-            // backward items: thread blocks that run at the same time carry neighbouring swaths at the same stage of their
-            // tracks, so the q and tally rows of the triangles two swaths share are still in L2 for the second one.  Swaths
-            // are already stored in (angle, perpendicular) order; the last items of the last angle are short corner swaths.
-            for (int64_t a = 0; a < n_sw;) {
-                int64_t b = a;
-                while (b < n_sw && built[b].group == built[a].group) ++b;
-                for (int dir = 0; dir < 2; ++dir)
-                    for (int64_t sw = a; sw < b; ++sw)
-                        out->items.push_back({(int32_t)sw, dir, (int32_t)std::min<int64_t>(built[sw].sum_max_cnt, INT32_MAX), 0});
-                a = b;
-            }
-        }
+        std::vector<int64_t> cost((size_t)n_sw);
+        for (int64_t sw = 0; sw < n_sw; ++sw) cost[(size_t)sw] = built[(size_t)sw].sum_max_cnt;
+        nd_swath_items(plan, cost.data(), prm.item_order, &out->items);
     } catch (const std::bad_alloc&) {
         return nd_fail(ND_ERR_NOMEM, "nd_build_swaths: out of host memory");
     }

@@ -67,6 +67,7 @@ struct NdSwathSet {
     std::vector<NdSwathItem> items;       // work items (swath, direction)
     std::vector<uint16_t> slot_start;     // [n_tiles][NT+1] (only with prm.keep_slot_start)
     NdRawBytes blob;                      // all chunks (every byte written by nd_build_swaths)
+    size_t blob_bytes_device = 0;         // device builder: bytes of the stream it wrote into the workspace (blob stays empty)
     int max_head_bytes = 0, max_rec_bytes = 0;
     double mean_regions_per_tile = 0.0, mean_segments_per_tile = 0.0, lockstep_efficiency = 0.0;
 };
@@ -92,6 +93,22 @@ inline size_t nd_swath_max_blob(const NdSwathParams& p, int64_t n_segments, int6
     const size_t per_tile = 16 + (size_t)nd_swath_pad16(2 * (p.NT + 1)) + 2 * 16;
     return (size_t)nd_swath_max_tiles(p, n_segments, n_tracks) * per_tile + 24 * (size_t)n_segments + 256;
 }
+
+struct NdSwathCoreParams;
+
+// which tracks share a swath (needs the track geometry, no segment)
+struct NdSwathPlan {
+    int64_t n_swaths = 0;
+    std::vector<int32_t> swath_track;   // [n_swaths][NT] canonical track id or -1
+    std::vector<int32_t> group;         // [n_swaths] angle id of the swath's tracks
+    std::vector<double> lam0;           // [T] coordinate of every track's start point along its angle's direction
+};
+
+nd_status nd_swath_check_params(const nd_problem_desc* desc, const NdSwathParams& prm, NdSwathCoreParams* core);
+nd_status nd_swath_plan(const nd_problem_desc* desc, const int32_t* track_azim, const double* track_ends, const NdSwathParams& prm,
+                        NdSwathPlan* plan);
+void nd_swath_items(const NdSwathPlan& plan, const int64_t* cost, int item_order, std::vector<NdSwathItem>* items);
+double nd_swath_lag_length(const nd_problem_desc* desc, const double* track_ends, double lag, int n_threads);
 
 // track_azim / track_ends may be NULL (no geometry): tracks are then grouped in descriptor order.
 nd_status nd_build_swaths(const nd_problem_desc* desc, const int32_t* track_azim, const double* track_ends,

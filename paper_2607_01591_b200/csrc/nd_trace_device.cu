@@ -30,6 +30,8 @@ struct WalkParams {
     int64_t* __restrict__ counts;          // [T]   (count pass; -1 = the walk left the mesh)
     int32_t* __restrict__ seg_region;      // fill pass: batch-local outputs
     double* __restrict__ seg_length;
+    const double* __restrict__ w2;         // [T] 2 * track weight   } resident fill pass: A~_r += 2 omega_a delta_a s (O-5)
+    double* vol;                           // [R] or NULL            }
     int64_t guard, base;                   // max steps; seg_off of the batch's first track
     int t0, t1;
 };
@@ -45,7 +47,11 @@ __global__ void __launch_bounds__(128) k_walk(const WalkParams p)
     int64_t count = 0;
     int32_t* reg = nullptr;
     double* len = nullptr;
-    if (kStore) { reg = p.seg_region + (p.seg_off[t] - p.base); len = p.seg_length + (p.seg_off[t] - p.base); }
+    double w2 = 0.0;
+    if (kStore) {
+        reg = p.seg_region + (p.seg_off[t] - p.base); len = p.seg_length + (p.seg_off[t] - p.base);
+        if (p.vol) w2 = p.w2[t];
+    }
     bool ok = false;
     for (int64_t step = 0; step <= p.guard; ++step) {
         const int v[3] = {p.tri[3 * (size_t)tr], p.tri[3 * (size_t)tr + 1], p.tri[3 * (size_t)tr + 2]};
@@ -72,7 +78,10 @@ __global__ void __launch_bounds__(128) k_walk(const WalkParams p)
         if (exit_e < 0) break;
         const double chord = __dsub_rn(lam_exit, lam_prev);
         if (chord > 0.0) {
-            if (kStore) { reg[count] = tr; len[count] = chord; }
+            if (kStore) {
+                reg[count] = tr; len[count] = chord;
+                if (p.vol) atomicAdd(p.vol + tr, w2 * chord);
+            }
             ++count;
         }
         lam_prev = lam_exit;
@@ -85,7 +94,7 @@ __global__ void __launch_bounds__(128) k_walk(const WalkParams p)
 
 inline size_t up256(size_t x) { return (x + 255) / 256 * 256; }
 
-struct TraceLayout { size_t xy, tri, twin, trk, start_tri, counts, seg_off, out, total_fixed; };
+struct TraceLayout { size_t xy, tri, twin, trk, start_tri, counts, seg_off, w2, vol, out, total_fixed; };
 
 TraceLayout trace_layout(size_t V, size_t R, size_t T)
 {
@@ -93,7 +102,7 @@ TraceLayout trace_layout(size_t V, size_t R, size_t T)
     size_t c = 0;
     auto bump = [&](size_t bytes) { const size_t at = c; c = up256(c + bytes); return at; };
     L.xy = bump(16 * V); L.tri = bump(12 * R); L.twin = bump(12 * R); L.trk = bump(32 * T); L.start_tri = bump(4 * T);
-    L.counts = bump(8 * T); L.seg_off = bump(8 * (T + 1));
+    L.counts = bump(8 * T); L.seg_off = bump(8 * (T + 1)); L.w2 = bump(8 * T); L.vol = bump(8 * R);
     L.out = c; L.total_fixed = c;
     return L;
 }
@@ -130,8 +139,10 @@ extern "C" nd_status nd_tracks_device_workspace_bytes(const nd_mesh_desc* mesh, 
     return ND_OK;
 }
 
-extern "C" nd_status nd_tracks_generate_device(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, void* device_workspace,
-                                               size_t device_bytes, void* cuda_stream, nd_trace_timing* timing, nd_tracks** out)
+namespace {
+
+nd_status trace_impl(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, void* device_workspace, size_t device_bytes,
+                     void* cuda_stream, nd_trace_timing* timing, bool resident, size_t* required_bytes, nd_tracks** out)
 {
     using clk = std::chrono::steady_clock;
     auto secs = [](clk::time_point a, clk::time_point b) { return std::chrono::duration<double>(b - a).count(); };
@@ -153,7 +164,7 @@ extern "C" nd_status nd_tracks_generate_device(const nd_mesh_desc* mesh, int32_t
         const TraceLayout L = trace_layout(V, R, T);
         if (device_bytes < L.total_fixed + kBytesPerSegment * 1024) { delete tr; return nd_fail(ND_ERR_WORKSPACE, "workspace smaller than nd_tracks_device_workspace_bytes"); }
         // the output area holds `cap` segments: int32 regions first, then doubles (8-byte aligned)
-        const size_t cap = ((device_bytes - L.total_fixed) / kBytesPerSegment) & ~(size_t)63;
+        size_t cap = ((device_bytes - L.total_fixed) / kBytesPerSegment) & ~(size_t)63;
         char* ws = static_cast<char*>(device_workspace);
         std::vector<double> h_trk(4 * T);
         for (size_t t = 0; t < T; ++t) {
@@ -191,13 +202,46 @@ extern "C" nd_status nd_tracks_generate_device(const nd_mesh_desc* mesh, int32_t
             tr->seg_offset[t + 1] = tr->seg_offset[t] + h_counts[t];
         }
         tr->n_segments = tr->seg_offset[T];
-        tr->seg_region.resize((size_t)tr->n_segments);
-        tr->seg_length.resize((size_t)tr->n_segments);
-        nd_touch_pages(tr->seg_region.data(), 4 * (size_t)tr->n_segments);
-        nd_touch_pages(tr->seg_length.data(), 8 * (size_t)tr->n_segments);
         ND_TRACE_CUDA(cudaMemcpyAsync(ws + L.seg_off, tr->seg_offset.data(), 8 * (T + 1), cudaMemcpyHostToDevice, st));
+        if (resident) {
+            // all S segments stay in the workspace: regions, then lengths; A~_r is summed by the fill pass
+            const size_t S = (size_t)tr->n_segments, need = L.total_fixed + up256(4 * S) + 8 * S + 512;
+            if (required_bytes) *required_bytes = need;
+            if (device_bytes < need) {
+                char buf[160];
+                snprintf(buf, sizeof buf, "nd_tracks_generate_resident: %lld segments need a workspace of %zu bytes", (long long)S, need);
+                delete tr;
+                cudaEventDestroy(ev[0]); cudaEventDestroy(ev[1]);
+                return nd_fail(ND_ERR_WORKSPACE, buf);
+            }
+            std::vector<double> h_w2(T);
+            for (size_t t = 0; t < T; ++t) h_w2[t] = 2.0 * tr->track_weight[t];
+            ND_TRACE_CUDA(cudaMemcpyAsync(ws + L.w2, h_w2.data(), 8 * T, cudaMemcpyHostToDevice, st));
+            ND_TRACE_CUDA(cudaMemsetAsync(ws + L.vol, 0, 8 * R, st));
+            wp.w2 = (const double*)(ws + L.w2); wp.vol = (double*)(ws + L.vol);
+            wp.seg_region = (int32_t*)(ws + L.out); wp.seg_length = (double*)(ws + L.out + up256(4 * S));
+            wp.t0 = 0; wp.t1 = (int)T; wp.base = 0;
+            ND_TRACE_CUDA(cudaEventRecord(ev[0], st));
+            k_walk<true><<<(unsigned)((T + 127) / 128), 128, 0, st>>>(wp);
+            ND_TRACE_CUDA(cudaGetLastError());
+            ND_TRACE_CUDA(cudaEventRecord(ev[1], st));
+            tr->volume.assign(R, 0.0);
+            ND_TRACE_CUDA(cudaMemcpyAsync(tr->volume.data(), wp.vol, 8 * R, cudaMemcpyDeviceToHost, st));
+            ND_TRACE_CUDA(cudaStreamSynchronize(st));
+            float ms = 0.f;
+            ND_TRACE_CUDA(cudaEventElapsedTime(&ms, ev[0], ev[1]));
+            tm.fill_kernel_ms = ms;
+            tm.batches = 1;
+            tr->d_seg_region = wp.seg_region; tr->d_seg_length = wp.seg_length; tr->host_segments = false;
+            cap = 0;
+        } else {
+            tr->seg_region.resize((size_t)tr->n_segments);
+            tr->seg_length.resize((size_t)tr->n_segments);
+            nd_touch_pages(tr->seg_region.data(), 4 * (size_t)tr->n_segments);
+            nd_touch_pages(tr->seg_length.data(), 8 * (size_t)tr->n_segments);
+        }
         // ---- pass 2: fill, in batches of tracks whose segments fit the output area ----
-        for (size_t t0 = 0; t0 < T;) {
+        for (size_t t0 = 0; t0 < T && !resident;) {
             size_t t1 = t0;
             while (t1 < T && (size_t)(tr->seg_offset[t1 + 1] - tr->seg_offset[t0]) <= cap) ++t1;
             if (t1 == t0) { delete tr; return nd_fail(ND_ERR_WORKSPACE, "nd_tracks_generate_device: one track has more segments than the workspace holds"); }
@@ -229,12 +273,56 @@ extern "C" nd_status nd_tracks_generate_device(const nd_mesh_desc* mesh, int32_t
         return nd_fail(ND_ERR_NOMEM, "nd_tracks_generate_device: out of host memory");
     }
     const clk::time_point t_fin = clk::now();
-    rc = nd_tracks_finish(tr);
+    rc = nd_tracks_finish(tr, !resident);
     if (rc != ND_OK) { delete tr; return rc; }
     tm.finish_s = secs(t_fin, clk::now());
     tm.total_s = secs(t_begin, clk::now());
     tm.n_segments = tr->n_segments;
     if (timing) *timing = tm;
     *out = tr;
+    return ND_OK;
+}
+
+} // namespace
+
+extern "C" nd_status nd_tracks_generate_device(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, void* device_workspace,
+                                               size_t device_bytes, void* cuda_stream, nd_trace_timing* timing, nd_tracks** out)
+{
+    return trace_impl(mesh, n_azim, spacing, device_workspace, device_bytes, cuda_stream, timing, false, nullptr, out);
+}
+
+extern "C" nd_status nd_tracks_generate_resident(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, void* device_workspace,
+                                                 size_t device_bytes, void* cuda_stream, nd_trace_timing* timing,
+                                                 size_t* required_bytes, nd_tracks** out)
+{
+    return trace_impl(mesh, n_azim, spacing, device_workspace, device_bytes, cuda_stream, timing, true, required_bytes, out);
+}
+
+extern "C" nd_status nd_tracks_materialise(nd_tracks* tr, void* cuda_stream)
+{
+    if (!tr) return nd_fail(ND_ERR_NULL, "nd_tracks_materialise: NULL argument");
+    if (tr->host_segments) return ND_OK;
+    if (!tr->d_seg_region || !tr->d_seg_length) return nd_fail(ND_ERR_STATE, "nd_tracks_materialise: no device-resident segments");
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const size_t S = (size_t)tr->n_segments;
+    try {
+        tr->seg_region.resize(S);
+        tr->seg_length.resize(S);
+    } catch (const std::bad_alloc&) {
+        return nd_fail(ND_ERR_NOMEM, "nd_tracks_materialise: out of host memory");
+    }
+    nd_touch_pages(tr->seg_region.data(), 4 * S);
+    nd_touch_pages(tr->seg_length.data(), 8 * S);
+    cudaError_t e = cudaSuccess;
+    if (S > 0) {
+        e = cudaMemcpyAsync(tr->seg_region.data(), tr->d_seg_region, 4 * S, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(tr->seg_length.data(), tr->d_seg_length, 8 * S, cudaMemcpyDeviceToHost, st);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+        tr->seg_region.resize(0); tr->seg_length.resize(0);
+        return nd_fail(ND_ERR_CUDA, cudaGetErrorString(e));
+    }
+    tr->host_segments = true;
     return ND_OK;
 }

@@ -343,14 +343,14 @@ nd_status nd_tracks_prepare(const nd_mesh_desc* mesh, int32_t n_azim, double spa
     return ND_OK;
 }
 
-nd_status nd_tracks_finish(nd_tracks* tr)
+nd_status nd_tracks_finish(nd_tracks* tr, bool volumes_from_segments)
 {
     if (!tr) return nd_fail(ND_ERR_NULL, "nd_tracks_finish: NULL argument");
     try {
         const int T = tr->n_tracks, nh = tr->n_half;
         // ---- O-5: track-estimated areas, summed in canonical (track, segment) order ----
-        tr->volume.assign(static_cast<size_t>(tr->n_regions), 0.0);
-        for (int t = 0; t < T; ++t) {
+        if (volumes_from_segments) tr->volume.assign(static_cast<size_t>(tr->n_regions), 0.0);
+        for (int t = 0; t < T && volumes_from_segments; ++t) {
             const double w2 = 2.0 * tr->track_weight[t];
             for (int64_t k = tr->seg_offset[t]; k < tr->seg_offset[static_cast<size_t>(t) + 1]; ++k)
                 tr->volume[tr->seg_region[k]] += w2 * tr->seg_length[k];
@@ -423,8 +423,10 @@ extern "C" nd_status nd_tracks_view(const nd_tracks* tr, nd_tracks_view_t* v)
     if (!tr || !v) return nd_fail(ND_ERR_NULL, "nd_tracks_view: NULL argument");
     v->n_tracks = tr->n_tracks; v->n_regions = tr->n_regions; v->n_segments = tr->n_segments; v->n_half = tr->n_half;
     v->track_seg_offset = tr->seg_offset.data();
-    v->seg_region = tr->seg_region.data();
-    v->seg_length = tr->seg_length.data();
+    v->seg_region = tr->host_segments ? tr->seg_region.data() : nullptr;
+    v->seg_length = tr->host_segments ? tr->seg_length.data() : nullptr;
+    v->seg_region_device = tr->d_seg_region;
+    v->seg_length_device = tr->d_seg_length;
     v->track_weight = tr->track_weight.data();
     v->link = tr->link.data();
     v->track_azim = tr->track_azim.data();
@@ -447,6 +449,7 @@ extern "C" nd_status nd_tracks_shard(const nd_tracks* full, int32_t n_shards, in
     if (nh < 2 || nh % 2 != 0 || (int)full->angles.size() != nh) return nd_fail(ND_ERR_STATE, "nd_tracks_shard: not a cyclic laydown");
     if (n_shards > np) return nd_fail(ND_ERR_INVALID, "nd_tracks_shard: more shards than angle pairs (N_a / 4)");
     if ((int)full->global_id.size() != T) return nd_fail(ND_ERR_STATE, "nd_tracks_shard: incomplete tracks object");
+    if (!full->host_segments) return nd_fail(ND_ERR_STATE, "nd_tracks_shard: device-resident tracks, call nd_tracks_materialise first");
     for (int t = 0; t < T; ++t)
         if (full->global_id[t] != t) return nd_fail(ND_ERR_STATE, "nd_tracks_shard: the input is already a shard");
     nd_tracks* tr = nullptr;

@@ -52,6 +52,11 @@ struct nd_tracks {
     std::vector<double> volume;
     std::vector<double> azim_phi, azim_weight, azim_spacing;
     std::vector<int32_t> global_id;   // [T] id of every track in the unsharded laydown (identity unless made by nd_tracks_shard)
+    // nd_tracks_generate_resident: the segment arrays in the caller's device workspace; the host arrays above stay empty
+    // until nd_tracks_materialise
+    const int32_t* d_seg_region = nullptr;
+    const double* d_seg_length = nullptr;
+    bool host_segments = true;
 };
 
 // What a ray walker needs besides the mesh arrays: the half-edge twins and every track's first triangle.
@@ -62,7 +67,8 @@ struct NdWalkInput {
 
 // Laydown (R-T), links (O-3), half-edge mesh and start triangles.  *out owns the result (segments still empty).
 nd_status nd_tracks_prepare(const nd_mesh_desc* mesh, int32_t n_azim, double spacing, nd_tracks** out, NdWalkInput* walk);
-// After seg_offset / seg_region / seg_length are filled: track volumes (O-5, canonical order) and the per-angle views.
-nd_status nd_tracks_finish(nd_tracks* tr);
+// After seg_offset / seg_region / seg_length are filled: track volumes (O-5, canonical order; skipped with
+// volumes_from_segments = false: the caller fills tr->volume) and the per-angle views.
+nd_status nd_tracks_finish(nd_tracks* tr, bool volumes_from_segments = true);
 
 #endif
