@@ -108,7 +108,7 @@ class ClockSampler:
 
 def build_inputs(args, tracer="device"):
     """Seeded synthetic problem + ray tracing (not timed).  tracer = "device": the library's GPU ray walk (row NEXT-1,
-    bit-identical to its host tracer and to the oracle's); "oracle": the oracle's own tracer (reference arm: nothing of
+    segments bit-identical to its host tracer's and to the oracle's) with the segments left in device memory; "oracle": the oracle's own tracer (reference arm: nothing of
     the library runs there)."""
     from moc_inputs import make_config
     t0 = time.time()
@@ -122,8 +122,10 @@ def build_inputs(args, tracer="device"):
     else:
         import paper_2607_01591_b200 as nd
         local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-        tr = nd.nd_tracks_generate_device(m.xy, m.tri, m.W, m.H, prob.bc, prob.n_azim, prob.spacing,
-                                          segment_capacity=1 << 28, device=f"cuda:{local_rank}")
+        # the segments stay on the GPU: nd_problem_create builds its streams there (no segment crosses PCIe); the oracle legs
+        # and the sharded run copy them back on first use (nd_tracks_materialise)
+        tr = nd.nd_tracks_generate_resident(m.xy, m.tri, m.W, m.H, prob.bc, prob.n_azim, prob.spacing, device=f"cuda:{local_rank}")
+        tracer = "device-resident"
     t2 = time.time()
     return prob, tr, {"mesh_s": round(t1 - t0, 2), "trace_s": round(t2 - t1, 2), "tracer": tracer}
 

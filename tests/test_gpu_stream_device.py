@@ -61,10 +61,11 @@ def test_resident_segments_are_bit_exact(idx, scale):
 
 
 def test_resident_workspace_is_sized_by_a_second_call():
-    prob = make_config(3, scale=0.03)
+    prob = make_config(3, scale=0.2)             # 6e6 segments: more than the 2^20 the minimum workspace holds
     a = _resident(prob)
     b = _resident(prob, segment_estimate=1)      # far too small: ND_ERR_WORKSPACE reports the size, the binding retries
     try:
+        assert a.n_segments > 1 << 21
         assert a.timing["attempts"] == 1, "the mean-chord estimate should suffice"
         assert b.timing["attempts"] == 2
         assert a.seg_region.tobytes() == b.seg_region.tobytes() and a.seg_length.tobytes() == b.seg_length.tobytes()
