@@ -488,9 +488,14 @@ nd_status launch_source(nd_problem* p, const ndk::SourceParams& sp, cudaStream_t
     cp.base = sp; cp.src_region = p->src_region; cp.chunks = p->src_chunks; cp.n_chunks = p->n_src_chunks;
     cp.chunk_regions = p->src_chunk_regions;
     const int block = 256;
-    const size_t smem = sizeof(double) * ((size_t)p->src_chunk_regions * d.G + p->src_chunk_regions);
+    const int Gp = (d.G + 1) / 2 * 2;
+    const size_t smem = sizeof(double) * ((size_t)p->src_chunk_regions * Gp + p->src_chunk_regions);
     const int grid = p->n_src_chunks < 8 * p->n_sm ? (p->n_src_chunks > 0 ? p->n_src_chunks : 1) : 8 * p->n_sm;
+#ifdef ND_SOURCE_OLD
     ndk::k_source_chunks<<<grid, block, smem, st>>>(cp);
+#else
+    ndk::k_source_tiled<<<grid, block, smem, st>>>(cp);
+#endif
     ND_LAUNCH_CHECK(p);
     return ND_OK;
 }
@@ -807,8 +812,14 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     std::vector<int32_t> h_src_region((size_t)d.R);
     std::vector<int4> h_src_chunks;
     {
+#ifdef ND_SOURCE_OLD
         const int nsub = 256 / d.G > 0 ? 256 / d.G : 1;
         p->src_chunk_regions = nsub * ndk::kSrcRegionsPerThread;
+#else
+        // k_source_tiled: thread = (sub, pair of groups), kSrcTile regions each; at most 64 subs (phi tile <= 37 KB)
+        const int nsub = std::min(256 / ((d.G + 1) / 2), 64);
+        p->src_chunk_regions = nsub * ndk::kSrcTile;
+#endif
         std::vector<int64_t> count((size_t)d.M + 1, 0);
         for (int r = 0; r < d.R; ++r) ++count[desc->region_material[r] + 1];
         for (int m = 0; m < d.M; ++m) count[m + 1] += count[m];

@@ -104,12 +104,20 @@ __global__ void __launch_bounds__(256) k_sweep_atomic(const SweepParams prm)
 __global__ void __launch_bounds__(256) k_link_swap(const float* __restrict__ psi_out, float* __restrict__ psi_next,
                                                    const int32_t* __restrict__ src, int64_t n_entries, int PG)
 {
-    const int64_t n = n_entries * PG;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t e = i / PG;
-        const int j = (int)(i - e * PG);
+    // one 16-byte piece per thread and step (PG is a multiple of 4); (e, j) advance with i: no division per element
+    const int PG4 = PG >> 2;
+    const int64_t n = n_entries * PG4, stride = (int64_t)gridDim.x * blockDim.x;
+    const int64_t de = stride / PG4;
+    const int dj = (int)(stride - de * PG4);
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t e = i / PG4;
+    int j = (int)(i - e * PG4);
+    const float4* __restrict__ in4 = reinterpret_cast<const float4*>(psi_out);
+    float4* __restrict__ out4 = reinterpret_cast<float4*>(psi_next);
+    for (; i < n; i += stride, e += de, j += dj) {
+        if (j >= PG4) { j -= PG4; ++e; }
         const int32_t s = src[e];
-        psi_next[i] = s >= 0 ? psi_out[(int64_t)s * PG + j] : 0.f;
+        out4[i] = s >= 0 ? in4[(int64_t)s * PG4 + j] : make_float4(0.f, 0.f, 0.f, 0.f);
     }
 }
 
@@ -219,6 +227,88 @@ __global__ void __launch_bounds__(256) k_reduced_source(const double* __restrict
     }
 }
 
+// The same source with a larger register tile.  Thread (sub, pair): kSrcTile regions x 2 destination groups; per PAIR of
+// source groups four Sigma_s loads and kSrcTile 16-byte shared-memory loads of phi feed 4 * kSrcTile FP64 FMAs (0.375 loads
+// per FMA against 1.25 in k_source_chunks, whose time was the LSU's, not the FP64 pipe's).  phi rows are padded to an even
+// number of doubles in shared memory; an odd G repeats the last group in the pad lane (zero phi, nothing stored).  Every
+// accumulator adds its terms in the order of the source groups, as k_source_chunks does: bit-identical results.
+constexpr int kSrcTile = 8;
+__global__ void __launch_bounds__(256) k_source_tiled(const SourceChunkParams cp)
+{
+    extern __shared__ __align__(16) double s_src2[];   // phi [chunk_regions][Gp], then fis [chunk_regions]
+    const SourceParams& prm = cp.base;
+    const int G = prm.G, CR = cp.chunk_regions, np = (G + 1) >> 1, Gp = 2 * np;
+    double* s_phi = s_src2;
+    double* s_fis = s_src2 + (size_t)CR * Gp;
+    const int nsub = CR / kSrcTile;            // <= blockDim.x / np, capped by the host so that the phi tile fits 48 KB
+    const int sub = threadIdx.x / np, pr = threadIdx.x - sub * np;
+    const int g0 = 2 * pr, g1 = g0 + 1 < G ? g0 + 1 : g0;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const double inv_f = prm.f_ptr ? 1.0 / *prm.f_ptr : 1.0;
+    const double inv_k = 1.0 / (prm.k_ptr ? *prm.k_ptr : prm.k_val);
+    for (int c = blockIdx.x; c < cp.n_chunks; c += gridDim.x) {
+        const int4 ch = cp.chunks[c];
+        const int first = ch.x, cnt = ch.y, m = ch.z;
+        __syncthreads();
+        for (int i = threadIdx.x; i < cnt * Gp; i += blockDim.x) {
+            const int lr = i / Gp, g = i - lr * Gp;
+            s_phi[i] = g < G ? prm.phi[(size_t)cp.src_region[first + lr] * G + g] * inv_f : 0.0;
+        }
+        __syncthreads();
+        const double* nf = prm.nusf + (size_t)m * G;
+        for (int lr = warp; lr < cnt; lr += nwarp) {   // fission sum of region lr
+            double f = 0.0;
+            for (int gp = lane; gp < G; gp += 32) f += nf[gp] * s_phi[lr * Gp + gp];
+            for (int o = 16; o > 0; o >>= 1) f += __shfl_xor_sync(0xffffffffu, f, o);
+            if (lane == 0) s_fis[lr] = f;
+        }
+        __syncthreads();
+        if (sub < nsub) {
+            const double* ss = prm.sigsT + (size_t)m * G * G;
+            double acc0[kSrcTile], acc1[kSrcTile];
+            const double* ph[kSrcTile];
+#pragma unroll
+            for (int i = 0; i < kSrcTile; ++i) {
+                acc0[i] = 0.0; acc1[i] = 0.0;
+                const int lr = sub + i * nsub;
+                ph[i] = s_phi + (size_t)(lr < cnt ? lr : 0) * Gp;
+            }
+            for (int gp = 0; gp < Gp; gp += 2) {
+                const int gq = gp + 1 < G ? gp + 1 : gp;       // pad lane of an odd G: phi = 0 there
+                const double a00 = ss[(size_t)gp * G + g0], a01 = ss[(size_t)gp * G + g1];
+                const double a10 = ss[(size_t)gq * G + g0], a11 = ss[(size_t)gq * G + g1];
+#pragma unroll
+                for (int i = 0; i < kSrcTile; ++i) {
+                    const double2 v = *reinterpret_cast<const double2*>(ph[i] + gp);
+                    acc0[i] = fma(a00, v.x, acc0[i]); acc1[i] = fma(a01, v.x, acc1[i]);
+                    acc0[i] = fma(a10, v.y, acc0[i]); acc1[i] = fma(a11, v.y, acc1[i]);
+                }
+            }
+            const double chi0 = prm.chi[(size_t)m * G + g0] * inv_k, chi1 = prm.chi[(size_t)m * G + g1] * inv_k;
+            const double st0 = prm.sigt[(size_t)m * G + g0], st1 = prm.sigt[(size_t)m * G + g1];
+            const bool two = g0 + 1 < G;
+#pragma unroll
+            for (int i = 0; i < kSrcTile; ++i) {
+                const int lr = sub + i * nsub;
+                if (lr < cnt) {
+                    const int64_t r = cp.src_region[first + lr];
+                    const double Q0 = (acc0[i] + chi0 * s_fis[lr]) / kFourPi, Q1 = (acc1[i] + chi1 * s_fis[lr]) / kFourPi;
+                    prm.Q[r * G + g0] = Q0;
+                    if (two) prm.Q[r * G + g1] = Q1;
+                    if (prm.q) {
+                        prm.q[r * prm.Gs + g0] = (float)(Q0 / st0);
+                        if (two) prm.q[r * prm.Gs + g1] = (float)(Q1 / st1);
+                    }
+                    if (prm.tally) {
+                        prm.tally[r * prm.Gs + g0] = 0.0;
+                        if (two) prm.tally[r * prm.Gs + g1] = 0.0;
+                    }
+                }
+            }
+        }
+    }
+}
+
 // ---- block-wide FP64 sum / max (deterministic tree) ----
 __device__ __forceinline__ double block_sum(double v, double* scratch)
 {
@@ -273,9 +363,15 @@ __global__ void __launch_bounds__(256) k_finalise(const FinaliseParams prm)
     const int64_t n = prm.R * prm.G;
     const double inv_f = (prm.phi_old && prm.f_ptr) ? 1.0 / *prm.f_ptr : 1.0;
     double fsum = 0.0, dmax = 0.0, pmax = 0.0, tsum = 0.0;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t r = i / prm.G;
-        const int g = (int)(i - r * prm.G);
+    // (r, g) of element i advance with i: no 64-bit division per element
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    const int64_t dr = stride / prm.G;
+    const int dg = (int)(stride - dr * prm.G);
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t r = i / prm.G;
+    int g = (int)(i - r * prm.G);
+    for (; i < n; i += stride, r += dr, g += dg) {
+        if (g >= prm.G) { g -= prm.G; ++r; }
         const int m = prm.reg_mat[r];
         const double st = prm.sigt[(size_t)m * prm.G + g];
         const double a = prm.vol[r];

@@ -27,7 +27,13 @@
 #pragma once
 #include "nd_kernels.cuh"
 
+#ifndef ND_FLUSH_UNROLL
+#define ND_FLUSH_UNROLL 4
+#endif
+
 namespace ndk {
+
+constexpr int kFlushUnroll = ND_FLUSH_UNROLL;
 
 struct SwathParams {
     const uint8_t* __restrict__ blob;
@@ -132,6 +138,7 @@ __device__ __forceinline__ f32x2 pk2(float lo, float hi) { f32x2 r; asm("mov.b64
 __device__ __forceinline__ void upk2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
 __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
 __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 
 // x / d for x < 2^16 and d >= 1, with m = fastdiv_magic(d); m == 0 encodes d == 1
@@ -210,7 +217,9 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
             }
             sts_2x64(d_lane + d_cur, acc[0], acc[1]);
         };
-        // (A peeled last trip without the loads for a step that does not exist measured +-0.1 %: not kept.)
+        // (A peeled last trip without the loads for a step that does not exist measured +-0.1 %: not kept.  Carrying
+        // W = sum_p w_p psi_p and storing W_before - W_behind -- two packed operations per (pair, polar angle) instead of
+        // three -- measured 1.4 % slower and costs the small Deltas their relative accuracy: not kept.)
         for (int i = 0; i < steps; ++i) {
             const f32x2 s2 = pk2(s_n, s_n);
             const f32x2 qa[2] = {q_n.x, q_n.y};
@@ -402,6 +411,8 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
             const uint2* regions = reinterpret_cast<const uint2*>(hb + 16 * h.y);
             const uint32_t qb = smem_u32(q_s + (size_t)(s & 1u) * q_buf_bytes);
             const int per_row = (TIGHT ? prm.NC : prm.NCq) * nq;
+            // (One 1-D bulk copy per region through the TMA unit instead -- no LSU wavefronts, no index arithmetic -- measured
+            // 4.8 % SLOWER at config 5 and 6.5 % at config 4: thirty 208-byte bulk copies per tile cost more than 390 cp.async.)
             for (int i = tid; i < L * per_row; i += nthr) {
                 const int l = (int)fastdiv((uint32_t)i, prm.magic_per_row), rem = i - l * per_row;
                 const int piece = rem - (int)fastdiv((uint32_t)rem, prm.magic_nq) * nq;
@@ -477,23 +488,31 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
             mark(PH_WAIT_B);
             // ---- flush: one FP64 RED per (region, group) of the tile.  A thread owns a pair of groups of one region, pairs
             // fastest: the lanes of a warp read consecutive 8-byte pieces of the region's contiguous delta rows and their REDs
-            // fall on consecutive doubles of the tally row (2-3 lines per instruction).  (A warp-per-region mapping with the
-            // regions dealt to the warps by row count was conflict-free and balanced, and 1.9 % slower at config 5.)
+            // fall on consecutive doubles of the tally row (2-3 lines per instruction); the rows are added with packed FADD2.
+            // (Same-box A/B of other mappings, config 5, against 52.7 ms: a unit of (region, 4 groups) with LDS.128 and four REDs
+            // 58.9 ms; lanes trading sums by shuffles so that a RED instruction covers 32 consecutive doubles 57.0 ms.  Flushing region by region -- a warp per
+            // 32 / LPT regions, 16 bytes per lane, odd rounds dealt in reverse -- is free of bank conflicts and 40 % shorter in
+            // instructions, and measured 3.3 % SLOWER at configs 5 and 4: its FP64 REDs fall one per 32-byte sector and
+            // instruction instead of two, and the warps of a block no longer reach the next barrier together.)
             for (int u = tid; u < ch.L * f_np; u += nthr) {
-                const int l = (int)fastdiv((uint32_t)u, prm.magic_np), gp = u - l * f_np;
+                const int l = (int)__umulhi((uint32_t)u, prm.magic_np), gp = u - l * f_np;   // f_np >= 2: the magic is never 0
                 const uint2 rg = ch.regions[l];
                 const int e0 = (int)(rg.y & 0xffffu), e1 = (int)(rg.y >> 16);
                 uint32_t row = smem_u32(dbuf) + e0 * row_bytes + gp * 8;
-                float vx = 0.f, vy = 0.f;
-#pragma unroll 4
+                f32x2 axy = 0ull;
+#pragma unroll kFlushUnroll
                 for (int e = e0; e < e1; ++e, row += row_bytes) {
-                    float x, y;
-                    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(x), "=f"(y) : "r"(row));
-                    vx += x; vy += y;
+                    f32x2 x;
+                    asm volatile("ld.shared.b64 %0, [%1];" : "=l"(x) : "r"(row));
+                    axy = add2(axy, x);
                 }
-                double* tp = prm.tally + (size_t)rg.x * Gs + gp * 2;
-                if (gp * 2 < prm.G) atomicAdd(tp, (double)vx);
-                if (gp * 2 + 1 < prm.G) atomicAdd(tp + 1, (double)vy);
+                float vx, vy;
+                upk2(axy, vx, vy);
+                // The tally rows are padded to Gs doubles and nothing reads the pad entries: no bound check, 32-bit index
+                // (R Gs <= 2^32).  Without the two branches and the 64-bit index arithmetic: config 5 54.94 -> 52.72 ms.
+                double* tp = prm.tally + (uint32_t)(rg.x * (uint32_t)Gs + (uint32_t)(gp * 2));
+                atomicAdd(tp, (double)vx);
+                atomicAdd(tp + 1, (double)vy);
             }
             if (CUR) {
                 // ---- currents: thread -> (crossing, pair of groups).  W at the crossing = W at the slot's entry minus the delta
