@@ -519,6 +519,26 @@ typedef struct {
 } nd_microbench_result;
 nd_status nd_microbench(void* device_workspace, size_t device_bytes, void* cuda_stream, nd_microbench_result* out);
 
+/* ------------------------------------------------------------------------------------------------
+ * Allocation-free fission rate (row A6: F = sum_r A~_r sum_g nuSigma_f[m(r)][g] phi[r][g], the k_eff update of Eq. (1),
+ * PAPER.md:48) for callers that can neither call cudaMalloc nor hand over a workspace (CUDA graph capture, serving loops).
+ * Its per-block partial sums live in a file-scope __device__ array of the library: 256 KiB that every GPU that loads
+ * libnd_moc.so holds until the process exits.  Same quantity as nd_source_update's d_fission_rate_out (which keeps its
+ * partial sums in the problem's workspace); the decomposition is fixed (4096 consecutive elements per partial sum), so the
+ * result does not depend on the GPU's SM count.
+ *   d_phi [R][G], d_region_material [R] (values in 0..M-1: NOT checked), d_nu_sigma_f [M][G], d_volume [R]: DEVICE, inputs;
+ *   d_fission_rate_out: DEVICE, one double.  Stream-ordered, asynchronous; calls no allocating routine.
+ * LIMIT: n_regions * n_groups <= ND_STATIC_FISSION_MAX_ELEMENTS, else ND_ERR_RANGE (nothing is launched).
+ * SHARED STATE: every call on a device uses the same array, which keeps the last call's partial sums.  Nothing has to be
+ * cleared (a call reads only what it wrote), but two calls that OVERLAP on the GPU -- different streams, concurrent graph
+ * replays -- race on it: order them on one stream or with events.
+ * Errors: ND_ERR_NULL, ND_ERR_INVALID (sizes < 1), ND_ERR_RANGE (limit; device ordinal > 63), ND_ERR_CUDA.
+ * ---------------------------------------------------------------------------------------------- */
+#define ND_STATIC_FISSION_MAX_ELEMENTS (1ll << 27)
+nd_status nd_fission_rate_static(int32_t n_regions, int32_t n_groups, const double* d_phi, const int32_t* d_region_material,
+                                 const double* d_nu_sigma_f, const double* d_volume, double* d_fission_rate_out,
+                                 void* cuda_stream);
+
 const char* nd_status_string(nd_status s);
 /* Message of the last call that failed ON THE CALLING THREAD (thread-local storage, valid until that thread's next failing
  * call).  The argument is accepted for symmetry and ignored: errors of calls that have no problem (nd_tracks_generate,

@@ -29,7 +29,7 @@ EXPORTS = [
     "nd_track_volume_get", "nd_tally_get", "nd_cmfd_surfaces", "nd_microbench", "nd_cmfd_workspace_bytes", "nd_cmfd_create",
     "nd_cmfd_destroy", "nd_cmfd_iteration", "nd_cmfd_sweep", "nd_cmfd_currents_get", "nd_cmfd_collapse", "nd_cmfd_coarse_get",
     "nd_cmfd_coarse_set", "nd_cmfd_solve", "nd_cmfd_prolong", "nd_p1_workspace_bytes", "nd_p1_create", "nd_p1_destroy",
-    "nd_p1_transport_sweep", "nd_p1_source_update", "nd_p1_state_reset", "nd_p1_power_iteration", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get",
+    "nd_p1_transport_sweep", "nd_p1_source_update", "nd_p1_state_reset", "nd_p1_power_iteration", "nd_profile_enable", "nd_profile_read", "nd_sweep_phases_get", "nd_problem_info_get", "nd_fission_rate_static",
     "nd_swath_stream_build", "nd_swath_stream_view", "nd_swath_stream_destroy",
     "nd_status_string", "nd_last_error", "nd_version", "nd_build_id",
 ]
@@ -153,6 +153,7 @@ def lib():
         L.nd_tracks_destroy.argtypes = [C.c_void_p]
         L.nd_tracks_shard.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_void_p)]
         L.nd_tally_reducer_set.argtypes = [C.c_void_p, ND_TALLY_REDUCE_FN, C.c_void_p]
+        L.nd_fission_rate_static.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.nd_problem_stream_view.argtypes = [C.c_void_p, C.POINTER(nd_stream_device_view_t)]
         L.nd_workspace_bytes.argtypes = [C.POINTER(nd_problem_desc), C.POINTER(nd_options), C.POINTER(C.c_size_t)]
         L.nd_problem_create.argtypes = [C.POINTER(nd_problem_desc), C.POINTER(nd_options), C.c_void_p, C.c_size_t,
@@ -401,6 +402,26 @@ def nd_cmfd_surfaces(seg_offset, seg_region, link, cell, n_cells, n_regions=None
         _check(lib().nd_cmfd_surfaces(C.byref(d), int(n_cells), cell.ctypes.data, n.value, C.byref(n), lo.ctypes.data,
                                       hi.ctypes.data), "nd_cmfd_surfaces")
     return lo[:n.value], hi[:n.value]
+
+
+ND_STATIC_FISSION_MAX_ELEMENTS = 1 << 27
+
+
+def nd_fission_rate_static(d_phi, d_region_material, d_nu_sigma_f, d_volume, d_out=None):
+    """Allocation-free fission rate (nd.h): torch device tensors phi [R][G] f64, region_material [R] i32, nu_sigma_f [M][G] f64,
+    volume [R] f64 in, a one-element f64 device tensor out (made here if not given: pass one to stay allocation-free)."""
+    import torch
+    R, G = d_phi.shape
+    for t, dt in ((d_phi, torch.float64), (d_region_material, torch.int32), (d_nu_sigma_f, torch.float64), (d_volume, torch.float64)):
+        assert t.is_cuda and t.is_contiguous() and t.dtype == dt
+    assert d_region_material.numel() == R and d_volume.numel() == R and d_nu_sigma_f.shape[1] == G
+    if d_out is None:
+        d_out = torch.empty(1, dtype=torch.float64, device=d_phi.device)
+    with torch.cuda.device(d_phi.device):
+        _check(lib().nd_fission_rate_static(int(R), int(G), d_phi.data_ptr(), d_region_material.data_ptr(), d_nu_sigma_f.data_ptr(),
+                                            d_volume.data_ptr(), d_out.data_ptr(),
+                                            C.c_void_p(torch.cuda.current_stream(d_phi.device).cuda_stream)), "nd_fission_rate_static")
+    return d_out
 
 
 def nd_microbench(device="cuda:0", workspace_bytes=(1 << 30) + (2 << 20)):

@@ -20,7 +20,7 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xptxas", "-v", "--expt-relaxed-constexpr"]
 GXX_FLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fopenmp", "-fPIC", "-Wall"]
 
-CU_SOURCES = ["nd_api.cu", "nd_trace_device.cu", "nd_microbench.cu", "nd_swath_device.cu"]
+CU_SOURCES = ["nd_api.cu", "nd_trace_device.cu", "nd_microbench.cu", "nd_swath_device.cu", "nd_noalloc.cu"]
 CXX_SOURCES = ["nd_tracks.cpp", "nd_swath.cpp", "nd_cmfd_host.cpp"]
 
 
