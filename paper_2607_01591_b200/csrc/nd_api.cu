@@ -326,6 +326,7 @@ struct nd_problem {
     double* scalars; double* partial; double* partial_b; uint8_t* exit_vac; double* stats;
     int32_t* src_region = nullptr; int4* src_chunks = nullptr;
     int n_src_chunks = 0, src_chunk_regions = 0;
+    bool source_attr_set = false;
     // swath sweep
     SwathConfig sc{};
     double lockstep_efficiency = 0.0;
@@ -489,12 +490,23 @@ nd_status launch_source(nd_problem* p, const ndk::SourceParams& sp, cudaStream_t
     cp.chunk_regions = p->src_chunk_regions;
     const int block = 256;
     const int Gp = (d.G + 1) / 2 * 2;
-    const size_t smem = sizeof(double) * ((size_t)p->src_chunk_regions * Gp + p->src_chunk_regions);
+    const size_t smem = sizeof(double) * ((size_t)p->src_chunk_regions * Gp + ((p->src_chunk_regions + 1) & ~1));
     const int grid = p->n_src_chunks < 8 * p->n_sm ? (p->n_src_chunks > 0 ? p->n_src_chunks : 1) : 8 * p->n_sm;
 #ifdef ND_SOURCE_OLD
     ndk::k_source_chunks<<<grid, block, smem, st>>>(cp);
 #else
-    ndk::k_source_tiled<<<grid, block, smem, st>>>(cp);
+    // the scattering matrix of the chunk's material beside the phi tile when both fit 100 KB (two blocks per SM: the kernel
+    // takes 128 registers)
+    const size_t smem_ss = smem + sizeof(double) * (size_t)d.G * Gp;
+    if (smem_ss <= 100 * 1024) {
+        if (!p->source_attr_set) {
+            ND_CUDA(cudaFuncSetAttribute(ndk::k_source_tiled<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ss));
+            p->source_attr_set = true;
+        }
+        ndk::k_source_tiled<true><<<grid, block, smem_ss, st>>>(cp);
+    } else {
+        ndk::k_source_tiled<false><<<grid, block, smem, st>>>(cp);
+    }
 #endif
     ND_LAUNCH_CHECK(p);
     return ND_OK;
@@ -565,7 +577,9 @@ nd_status launch_finalise(nd_problem* p, const double* Q, const double* phi_old,
     fp.phi_old = phi_old; fp.f_ptr = f_ptr; fp.phi_new = phi_out; fp.partial = p->partial;
     fp.R = d.R; fp.G = d.G; fp.Gs = d.Gs;
     const int grid = grid_for((int64_t)d.R * d.G, 256, kReduceBlocks);
-    ndk::k_finalise<<<grid, 256, 0, st>>>(fp);
+    const int MG = d.M * d.G;
+    if (MG <= ndk::kFinTab) ndk::k_finalise<true><<<grid, 256, 0, st>>>(fp, MG);
+    else ndk::k_finalise<false><<<grid, 256, 0, st>>>(fp, MG);
     ND_LAUNCH_CHECK(p);
     *grid_out = grid;
     return ND_OK;

@@ -232,14 +232,19 @@ __global__ void __launch_bounds__(256) k_reduced_source(const double* __restrict
 // per FMA against 1.25 in k_source_chunks, whose time was the LSU's, not the FP64 pipe's).  phi rows are padded to an even
 // number of doubles in shared memory; an odd G repeats the last group in the pad lane (zero phi, nothing stored).  Every
 // accumulator adds its terms in the order of the source groups, as k_source_chunks does: bit-identical results.
+// SS_SMEM: the chunk's scattering matrix is staged in shared memory ([G][Gp] doubles, reloaded only when the material
+// changes between two chunks of a block), so the inner loop waits on no global load; used when it fits beside the phi tile.
 constexpr int kSrcTile = 8;
+template <bool SS_SMEM>
 __global__ void __launch_bounds__(256) k_source_tiled(const SourceChunkParams cp)
 {
-    extern __shared__ __align__(16) double s_src2[];   // phi [chunk_regions][Gp], then fis [chunk_regions]
+    extern __shared__ __align__(16) double s_src2[];   // phi [chunk_regions][Gp], fis [chunk_regions], (Sigma_s^T [G][Gp])
     const SourceParams& prm = cp.base;
     const int G = prm.G, CR = cp.chunk_regions, np = (G + 1) >> 1, Gp = 2 * np;
     double* s_phi = s_src2;
     double* s_fis = s_src2 + (size_t)CR * Gp;
+    double* s_ss = s_fis + ((CR + 1) & ~1);            // 16-byte aligned
+    int m_loaded = -1;
     const int nsub = CR / kSrcTile;            // <= blockDim.x / np, capped by the host so that the phi tile fits 48 KB
     const int sub = threadIdx.x / np, pr = threadIdx.x - sub * np;
     const int g0 = 2 * pr, g1 = g0 + 1 < G ? g0 + 1 : g0;
@@ -253,6 +258,14 @@ __global__ void __launch_bounds__(256) k_source_tiled(const SourceChunkParams cp
         for (int i = threadIdx.x; i < cnt * Gp; i += blockDim.x) {
             const int lr = i / Gp, g = i - lr * Gp;
             s_phi[i] = g < G ? prm.phi[(size_t)cp.src_region[first + lr] * G + g] * inv_f : 0.0;
+        }
+        if (SS_SMEM && m != m_loaded) {   // rows gp of Sigma_s^T, padded to Gp (the pad column repeats the last group)
+            const double* src = prm.sigsT + (size_t)m * G * G;
+            for (int i = threadIdx.x; i < G * Gp; i += blockDim.x) {
+                const int gp = i / Gp, g = i - gp * Gp;
+                s_ss[i] = src[(size_t)gp * G + (g < G ? g : G - 1)];
+            }
+            m_loaded = m;
         }
         __syncthreads();
         const double* nf = prm.nusf + (size_t)m * G;
@@ -275,8 +288,15 @@ __global__ void __launch_bounds__(256) k_source_tiled(const SourceChunkParams cp
             }
             for (int gp = 0; gp < Gp; gp += 2) {
                 const int gq = gp + 1 < G ? gp + 1 : gp;       // pad lane of an odd G: phi = 0 there
-                const double a00 = ss[(size_t)gp * G + g0], a01 = ss[(size_t)gp * G + g1];
-                const double a10 = ss[(size_t)gq * G + g0], a11 = ss[(size_t)gq * G + g1];
+                double a00, a01, a10, a11;
+                if (SS_SMEM) {
+                    const double2 u = *reinterpret_cast<const double2*>(s_ss + (size_t)gp * Gp + g0);
+                    const double2 w = *reinterpret_cast<const double2*>(s_ss + (size_t)gq * Gp + g0);
+                    a00 = u.x; a01 = u.y; a10 = w.x; a11 = w.y;
+                } else {
+                    a00 = ss[(size_t)gp * G + g0]; a01 = ss[(size_t)gp * G + g1];
+                    a10 = ss[(size_t)gq * G + g0]; a11 = ss[(size_t)gq * G + g1];
+                }
 #pragma unroll
                 for (int i = 0; i < kSrcTile; ++i) {
                     const double2 v = *reinterpret_cast<const double2*>(ph[i] + gp);
@@ -357,9 +377,18 @@ struct FinaliseParams {
     int G, Gs;
 };
 
-__global__ void __launch_bounds__(256) k_finalise(const FinaliseParams prm)
+// TAB: Sigma_t and nu Sigma_f of all materials are staged in shared memory (M G <= kFinTab entries each), which takes two
+// global loads out of the chain that hangs on the region's material id.
+constexpr int kFinTab = 2048;
+template <bool TAB>
+__global__ void __launch_bounds__(256) k_finalise(const FinaliseParams prm, int MG)
 {
     __shared__ double scratch[32];
+    __shared__ double s_st[TAB ? kFinTab : 1], s_nf[TAB ? kFinTab : 1];
+    if (TAB) {
+        for (int i = threadIdx.x; i < MG; i += blockDim.x) { s_st[i] = prm.sigt[i]; s_nf[i] = prm.nusf[i]; }
+        __syncthreads();
+    }
     const int64_t n = prm.R * prm.G;
     const double inv_f = (prm.phi_old && prm.f_ptr) ? 1.0 / *prm.f_ptr : 1.0;
     double fsum = 0.0, dmax = 0.0, pmax = 0.0, tsum = 0.0;
@@ -373,14 +402,14 @@ __global__ void __launch_bounds__(256) k_finalise(const FinaliseParams prm)
     for (; i < n; i += stride, r += dr, g += dg) {
         if (g >= prm.G) { g -= prm.G; ++r; }
         const int m = prm.reg_mat[r];
-        const double st = prm.sigt[(size_t)m * prm.G + g];
+        const double st = TAB ? s_st[m * prm.G + g] : prm.sigt[(size_t)m * prm.G + g];
         const double a = prm.vol[r];
         const double tl = prm.tally[r * prm.Gs + g];
         tsum += tl;
         double phi = kFourPi * prm.Q[i] / st;
         if (a > 0.0) phi += tl / (st * a);
         prm.phi_new[i] = phi;
-        fsum += a * prm.nusf[(size_t)m * prm.G + g] * phi;
+        fsum += a * (TAB ? s_nf[m * prm.G + g] : prm.nusf[(size_t)m * prm.G + g]) * phi;
         if (prm.phi_old) {
             dmax = fmax(dmax, fabs(phi - prm.phi_old[i] * inv_f));
             pmax = fmax(pmax, fabs(phi));

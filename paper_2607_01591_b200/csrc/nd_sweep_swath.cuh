@@ -114,6 +114,10 @@ __device__ __forceinline__ void cp_async_16(uint32_t smem_dst, const void* gmem_
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_dst), "l"(gmem_src) : "memory");
 #endif
 }
+__device__ __forceinline__ void cp_async_8(uint32_t smem_dst, const void* gmem_src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_dst), "l"(gmem_src) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit_group() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
@@ -150,6 +154,12 @@ __device__ __forceinline__ uint4 lds_u4(uint32_t a)
 {
     uint4 v;
     asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint2 lds_u2(uint32_t a)
+{
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a) : "memory");
     return v;
 }
 __device__ __forceinline__ ulonglong2 lds_2x64(uint32_t a)
@@ -292,6 +302,7 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
     uint64_t* rfull = hfull + kSwathHeadBufs;                        // [kSwathRecBufs] record-arrival barriers
     uint64_t* xfull = reinterpret_cast<uint64_t*>(smem + 96);        // [kSwathXBufs] crossing-list barriers (CUR)
     volatile int* s_item = reinterpret_cast<volatile int*>(smem + 64);
+    const uint32_t s_pref = smem_u32(smem + 40);                     // [3] x 8 bytes: prefetched tile references (one thread's)
     uint32_t* s_null = reinterpret_cast<uint32_t*>(smem + 80);       // the null record: { 0.0f, 0, 0, offset of the spare delta row }
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int Gs = prm.Gs, row_bytes = 4 * Gs, line = prm.NC * row_bytes;
@@ -388,6 +399,31 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
             mbar_expect_tx(rfull + b, bytes);
             tma_load_1d(rec_s + (size_t)b * prm.rec_cap, prm.blob + ((size_t)ref.x + ref.y) * 16, bytes, rfull + b);
         };
+        // The tile references the issuing thread needs at tile k -- of the head of tile k+2 and of the records of tile k+1 --
+        // are fetched one tile ahead by three 8-byte cp.async into s_pref (no register lives across the segment loop), so the
+        // issuing thread's warp does not enter its loop two dependent global loads behind the others.  Used by the roomy
+        // variant (TIGHT = 0; config 3 -1.2 %); the register-capped one measured +-0.2 % and keeps the direct loads.
+        auto prefetch_refs = [&](int k) {   // one thread: what tile k will consume
+            if (k + 2 < nt) cp_async_8(s_pref, prm.tile_ref + tile_index(k + 2));
+            if (k + 1 < nt) {
+                const int64_t ti = tile_index(k + 1);
+                cp_async_8(s_pref + 8, prm.tile_ref + ti);
+                cp_async_8(s_pref + 16, prm.tile_ref + ti + 1);
+            }
+        };
+        auto issue_head_pref = [&](int k) {   // one thread, k = current tile + 2
+            const uint2 ref = lds_u2(s_pref);
+            const uint32_t b = (seq + k) % kSwathHeadBufs;
+            mbar_expect_tx(hfull + b, ref.y * 16u);
+            tma_load_1d(head_s + (size_t)b * prm.head_cap, prm.blob + (size_t)ref.x * 16, ref.y * 16u, hfull + b);
+        };
+        auto issue_rec_pref = [&](int k) {    // one thread, k = current tile + 1
+            const uint2 ref = lds_u2(s_pref + 8);
+            const uint32_t bytes = (lds_u2(s_pref + 16).x - ref.x - ref.y) * 16u;
+            const uint32_t b = (seq + k) % kSwathRecBufs;
+            mbar_expect_tx(rfull + b, bytes);
+            tma_load_1d(rec_s + (size_t)b * prm.rec_cap, prm.blob + ((size_t)ref.x + ref.y) * 16, bytes, rfull + b);
+        };
         auto wait_head = [&](int k) {
             const uint32_t s = seq + k;
             mbar_wait(hfull + (s % kSwathHeadBufs), (s / kSwathHeadBufs) & 1u);
@@ -425,6 +461,7 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
                 issue_rec(0);
                 if (nt > 1) issue_head(1);
                 if (CUR) issue_x(0);
+                if (!TIGHT) prefetch_refs(0);   // lands before the cp_async_wait_all below
             }
             wait_head(0);
             issue_q_rows(0);
@@ -448,9 +485,17 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
             // record buffer (free since the loop of tile k-1) the records of tile k+1, and its delta rows may be overwritten.
             __syncthreads();
             if (tid == 0) {
-                if (k + 2 < nt) issue_head(k + 2);
-                if (k + 1 < nt) issue_rec(k + 1);
-                if (CUR && k + 1 < nt) issue_x(k + 1);
+                if (!TIGHT) {
+                    if (k + 2 < nt) issue_head_pref(k + 2);
+                    if (k + 1 < nt) issue_rec_pref(k + 1);
+                    if (CUR && k + 1 < nt) issue_x(k + 1);
+                    prefetch_refs(k + 1);   // into the slots just read; complete at this thread's cp_async_wait_all behind the loop
+                    cp_async_commit_group();
+                } else {
+                    if (k + 2 < nt) issue_head(k + 2);
+                    if (k + 1 < nt) issue_rec(k + 1);
+                    if (CUR && k + 1 < nt) issue_x(k + 1);
+                }
             }
             wait_rec(k);
             if (PROF) prof_sink += *s_item;        // BAR.SYNC defers its blocking to the next consumer: make one here
@@ -493,8 +538,10 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
             // 58.9 ms; lanes trading sums by shuffles so that a RED instruction covers 32 consecutive doubles 57.0 ms.  Flushing region by region -- a warp per
             // 32 / LPT regions, 16 bytes per lane, odd rounds dealt in reverse -- is free of bank conflicts and 40 % shorter in
             // instructions, and measured 3.3 % SLOWER at configs 5 and 4: its FP64 REDs fall one per 32-byte sector and
-            // instruction instead of two, and the warps of a block no longer reach the next barrier together.)
-            for (int u = tid; u < ch.L * f_np; u += nthr) {
+            // instruction instead of two, and the warps of a block no longer reach the next barrier together.  A thread that keeps
+            // one pair of groups for the whole kernel and walks the regions nthr / f_np apart -- no division in this loop --
+            // measured 0.7 % slower.)
+            auto flush_unit = [&](int u) {
                 const int l = (int)__umulhi((uint32_t)u, prm.magic_np), gp = u - l * f_np;   // f_np >= 2: the magic is never 0
                 const uint2 rg = ch.regions[l];
                 const int e0 = (int)(rg.y & 0xffffu), e1 = (int)(rg.y >> 16);
@@ -513,6 +560,19 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
                 double* tp = prm.tally + (uint32_t)(rg.x * (uint32_t)Gs + (uint32_t)(gp * 2));
                 atomicAdd(tp, (double)vx);
                 atomicAdd(tp + 1, (double)vy);
+            };
+            if (TIGHT) {
+                for (int u = tid; u < ch.L * f_np; u += nthr) flush_unit(u);
+            } else {
+                // The regions are listed by descending row count, so in every pass the low threads hold the long lists: odd
+                // passes deal the units in reverse and the warps' sums over the passes come out level.  Worth 2.8 % where the
+                // flush is a large share (narrow rows, config 3); with 13 lanes per slot the extra index arithmetic costs
+                // more than the balance gains (config 5 +2.8 %), so the register-capped variant keeps the plain order.
+                const int f_nu = ch.L * f_np;
+                for (int base = 0, odd = 0; base < f_nu; base += nthr, odd ^= 1) {
+                    const int u = base + (odd ? nthr - 1 - tid : tid);
+                    if (u < f_nu) flush_unit(u);
+                }
             }
             if (CUR) {
                 // ---- currents: thread -> (crossing, pair of groups).  W at the crossing = W at the slot's entry minus the delta
