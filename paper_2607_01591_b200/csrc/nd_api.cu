@@ -482,6 +482,8 @@ nd_status launch_sweep_p(nd_problem* p, const ndk::SweepParams& prm, cudaStream_
 }
 
 // A5: source update over material-grouped chunks
+constexpr size_t kSourceSmemMax = 100 * 1024;
+
 nd_status launch_source(nd_problem* p, const ndk::SourceParams& sp, cudaStream_t st)
 {
     const Dims& d = p->d;
@@ -492,22 +494,18 @@ nd_status launch_source(nd_problem* p, const ndk::SourceParams& sp, cudaStream_t
     const int Gp = (d.G + 1) / 2 * 2;
     const size_t smem = sizeof(double) * ((size_t)p->src_chunk_regions * Gp + ((p->src_chunk_regions + 1) & ~1));
     const int grid = p->n_src_chunks < 8 * p->n_sm ? (p->n_src_chunks > 0 ? p->n_src_chunks : 1) : 8 * p->n_sm;
-#ifdef ND_SOURCE_OLD
-    ndk::k_source_chunks<<<grid, block, smem, st>>>(cp);
-#else
     // the scattering matrix of the chunk's material beside the phi tile when both fit 100 KB (two blocks per SM: the kernel
     // takes 128 registers)
     const size_t smem_ss = smem + sizeof(double) * (size_t)d.G * Gp;
-    if (smem_ss <= 100 * 1024) {
-        if (!p->source_attr_set) {
-            ND_CUDA(cudaFuncSetAttribute(ndk::k_source_tiled<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ss));
+    if (smem_ss <= kSourceSmemMax) {
+        if (!p->source_attr_set) {   // the attribute belongs to the kernel, not to the problem: every problem sets the same value
+            ND_CUDA(cudaFuncSetAttribute(ndk::k_source_tiled<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSourceSmemMax));
             p->source_attr_set = true;
         }
         ndk::k_source_tiled<true><<<grid, block, smem_ss, st>>>(cp);
     } else {
         ndk::k_source_tiled<false><<<grid, block, smem, st>>>(cp);
     }
-#endif
     ND_LAUNCH_CHECK(p);
     return ND_OK;
 }
@@ -822,18 +820,13 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
         p->inv_sin[i] = (float)(1.0 / desc->polar_sin[i]);
         p->wp[i] = (float)(desc->polar_weight[i] * desc->polar_sin[i]);
     }
-    // A5: regions grouped by material into chunks of nsub*4 regions (k_source_chunks)
+    // A5: regions grouped by material into chunks of nsub * kSrcTile regions (k_source_tiled)
     std::vector<int32_t> h_src_region((size_t)d.R);
     std::vector<int4> h_src_chunks;
     {
-#ifdef ND_SOURCE_OLD
-        const int nsub = 256 / d.G > 0 ? 256 / d.G : 1;
-        p->src_chunk_regions = nsub * ndk::kSrcRegionsPerThread;
-#else
         // k_source_tiled: thread = (sub, pair of groups), kSrcTile regions each; at most 64 subs (phi tile <= 37 KB)
         const int nsub = std::min(256 / ((d.G + 1) / 2), 64);
         p->src_chunk_regions = nsub * ndk::kSrcTile;
-#endif
         std::vector<int64_t> count((size_t)d.M + 1, 0);
         for (int r = 0; r < d.R; ++r) ++count[desc->region_material[r] + 1];
         for (int m = 0; m < d.M; ++m) count[m + 1] += count[m];

@@ -1,5 +1,5 @@
 // nd_kernels.cuh -- device kernels of the planar-MOC hot path (sm_100a).  Rows A2..A6 of DESIGN.md.
-//   k_source_chunks A5  scatter + fission source (Eq. (1)/(3) RHS), reduced source q, tally reset
+//   k_source_tiled  A5  scatter + fission source (Eq. (1)/(3) RHS), reduced source q, tally reset
 //   k_sweep_atomic  A2  Eq. (5) per (track, direction, polar, group); FP64 global atomics per segment
 //   k_link_swap     A3  boundary angular flux through the link table (compressed psi: track ends only)
 //   k_finalise      A4  phi = 4 pi Q/Sigma_t + tally/(Sigma_t A~) + partial fission-rate sums
@@ -121,7 +121,7 @@ __global__ void __launch_bounds__(256) k_link_swap(const float* __restrict__ psi
     }
 }
 
-// ---- A5: source (k_source_chunks below).
+// ---- A5: source (k_source_tiled below).
 // Q[r][g] = (1/4pi) ( sum_g' Ss[m][g][g'] phi[r][g']/F + chi[m][g]/k * sum_g' nSf[m][g'] phi[r][g']/F )
 // Also writes q = (float)(Q/Sigma_t) and zeroes the tally row.  sigsT is [m][g_from][g_to].
 struct SourceParams {
@@ -142,76 +142,13 @@ struct SourceParams {
 
 // ---- A5, tiled: regions are visited in material-grouped CHUNKS (host-built: src_region is a permutation of the
 // regions, chunk = (first, count, material)), so one thread block works with ONE scattering matrix at a time.
-// Thread (sub, g): 4 regions x 1 destination group in registers; per source group one Sigma_s load feeds 4 FP64 FMAs.
 // The fission sum nuSigma_f . phi is formed once per region (warp shuffle), not once per destination group.
-constexpr int kSrcRegionsPerThread = 4;
 struct SourceChunkParams {
     SourceParams base;
     const int32_t* __restrict__ src_region;   // [R] regions grouped by material
     const int4* __restrict__ chunks;          // (first index into src_region, count, material, -)
-    int n_chunks, chunk_regions;              // chunk_regions = nsub * kSrcRegionsPerThread (max count)
+    int n_chunks, chunk_regions;              // chunk_regions = nsub * kSrcTile (max count)
 };
-
-__global__ void __launch_bounds__(256) k_source_chunks(const SourceChunkParams cp)
-{
-    extern __shared__ double s_src[];          // phi [chunk_regions][G], then fis [chunk_regions]
-    const SourceParams& prm = cp.base;
-    const int G = prm.G, CR = cp.chunk_regions;
-    double* s_phi = s_src;
-    double* s_fis = s_src + (size_t)CR * G;
-    const int nsub = blockDim.x / G;           // >= 1 (G <= 256)
-    const int sub = threadIdx.x / G, g = threadIdx.x - sub * G;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-    const double inv_f = prm.f_ptr ? 1.0 / *prm.f_ptr : 1.0;
-    const double inv_k = 1.0 / (prm.k_ptr ? *prm.k_ptr : prm.k_val);
-    for (int c = blockIdx.x; c < cp.n_chunks; c += gridDim.x) {
-        const int4 ch = cp.chunks[c];
-        const int first = ch.x, cnt = ch.y, m = ch.z;
-        __syncthreads();
-        for (int i = threadIdx.x; i < cnt * G; i += blockDim.x) {
-            const int lr = i / G;
-            s_phi[i] = prm.phi[(size_t)cp.src_region[first + lr] * G + (i - lr * G)] * inv_f;
-        }
-        __syncthreads();
-        const double* nf = prm.nusf + (size_t)m * G;
-        for (int lr = warp; lr < cnt; lr += nwarp) {   // fission sum of region lr
-            double f = 0.0;
-            for (int gp = lane; gp < G; gp += 32) f += nf[gp] * s_phi[lr * G + gp];
-            for (int o = 16; o > 0; o >>= 1) f += __shfl_xor_sync(0xffffffffu, f, o);
-            if (lane == 0) s_fis[lr] = f;
-        }
-        __syncthreads();
-        if (sub < nsub) {
-            const double* ss = prm.sigsT + (size_t)m * G * G + g;
-            double acc[kSrcRegionsPerThread];
-            const double* ph[kSrcRegionsPerThread];
-#pragma unroll
-            for (int i = 0; i < kSrcRegionsPerThread; ++i) {
-                acc[i] = 0.0;
-                const int lr = sub + i * nsub;
-                ph[i] = s_phi + (size_t)(lr < cnt ? lr : 0) * G;
-            }
-            for (int gp = 0; gp < G; ++gp) {
-                const double a = ss[(size_t)gp * G];
-#pragma unroll
-                for (int i = 0; i < kSrcRegionsPerThread; ++i) acc[i] = fma(a, ph[i][gp], acc[i]);
-            }
-            const double chi_k = prm.chi[(size_t)m * G + g] * inv_k;
-            const double st = prm.sigt[(size_t)m * G + g];
-#pragma unroll
-            for (int i = 0; i < kSrcRegionsPerThread; ++i) {
-                const int lr = sub + i * nsub;
-                if (lr < cnt) {
-                    const int64_t r = cp.src_region[first + lr];
-                    const double Q = (acc[i] + chi_k * s_fis[lr]) / kFourPi;
-                    prm.Q[r * G + g] = Q;
-                    if (prm.q) prm.q[r * prm.Gs + g] = (float)(Q / st);
-                    if (prm.tally) prm.tally[r * prm.Gs + g] = 0.0;
-                }
-            }
-        }
-    }
-}
 
 // q = Q/Sigma_t and tally = 0 for a caller-supplied Q (fixed-source nd_transport_sweep)
 __global__ void __launch_bounds__(256) k_reduced_source(const double* __restrict__ Q, const int32_t* __restrict__ reg_mat,
@@ -227,11 +164,11 @@ __global__ void __launch_bounds__(256) k_reduced_source(const double* __restrict
     }
 }
 
-// The same source with a larger register tile.  Thread (sub, pair): kSrcTile regions x 2 destination groups; per PAIR of
-// source groups four Sigma_s loads and kSrcTile 16-byte shared-memory loads of phi feed 4 * kSrcTile FP64 FMAs (0.375 loads
-// per FMA against 1.25 in k_source_chunks, whose time was the LSU's, not the FP64 pipe's).  phi rows are padded to an even
+// Thread (sub, pair): kSrcTile regions x 2 destination groups in registers; per PAIR of source groups four Sigma_s loads and
+// kSrcTile 16-byte shared-memory loads of phi feed 4 * kSrcTile FP64 FMAs (0.375 loads per FMA; with 4 regions x 1 group per
+// thread it was 1.25, and the kernel's time was the LSU's, not the FP64 pipe's).  phi rows are padded to an even
 // number of doubles in shared memory; an odd G repeats the last group in the pad lane (zero phi, nothing stored).  Every
-// accumulator adds its terms in the order of the source groups, as k_source_chunks does: bit-identical results.
+// accumulator adds its terms in the order of the source groups.
 // SS_SMEM: the chunk's scattering matrix is staged in shared memory ([G][Gp] doubles, reloaded only when the material
 // changes between two chunks of a block), so the inner loop waits on no global load; used when it fits beside the phi tile.
 constexpr int kSrcTile = 8;

@@ -207,6 +207,9 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
         }
         ulonglong2 q_n = lds_2x64(q_lane + r_n.y);
         ulonglong2 st_n = lds_2x64(sigt_lane + r_n.z);
+#ifdef ND_MSKIP
+        uint32_t z_prev = r_n.z;
+#endif
         float s_n = __uint_as_float(r_n.x);
         // the 4 P updates of one step and the store of sum_p w_p Delta_p into the segment's delta row
         auto update = [&](const f32x2 (&qa)[2], const f32x2 (&ts)[2], uint32_t d_cur) {
@@ -229,7 +232,10 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
         };
         // (A peeled last trip without the loads for a step that does not exist measured +-0.1 %: not kept.  Carrying
         // W = sum_p w_p psi_p and storing W_before - W_behind -- two packed operations per (pair, polar angle) instead of
-        // three -- measured 1.4 % slower and costs the small Deltas their relative accuracy: not kept.)
+        // three -- measured 1.4 % slower and costs the small Deltas their relative accuracy: not kept.  Carrying the chains as
+        // D_p = psi_p - q, D'_p = fma(D_p, a_p, q - q'), sum_p w_p Delta_p = WD - WD' + (q - q') sum_p w_p -- 49.5 instead of 54
+        // instructions per step, every parity test green -- measured 5.4 % SLOWER at config 5: the loop is bound by the
+        // dependent chains behind each MUFU.EX2, not by its instruction count.)
         for (int i = 0; i < steps; ++i) {
             const f32x2 s2 = pk2(s_n, s_n);
             const f32x2 qa[2] = {q_n.x, q_n.y};
@@ -239,7 +245,11 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
             r_nn = lds_u4(i + 2 < cnt ? rec_pf : null_rec);
             rec_pf += rstep;
             q_n = lds_2x64(q_lane + r_use.y);
+#ifdef ND_MSKIP
+            if (r_use.z != z_prev) { st_n = lds_2x64(sigt_lane + r_use.z); z_prev = r_use.z; }
+#else
             st_n = lds_2x64(sigt_lane + r_use.z);
+#endif
             s_n = __uint_as_float(r_use.x);
             d_n = r_use.w;
             update(qa, ts, d_cur);

@@ -167,6 +167,23 @@ def test_source_update_matches_oracle():
             pair.close()
 
 
+def test_source_update_alternating_between_live_problems_of_different_size():
+    # the source kernel's dynamic shared-memory limit is an attribute of the KERNEL: a small problem created after a large one
+    # must not lower it under the large one's feet (G = 33 stages a 57 KB tile, G = 2 a few hundred bytes)
+    big, small = make_pair(4, 0.06), make_pair(1, 1.0)
+    try:
+        for pair in (big, small, big, small, big):
+            rng = np.random.default_rng(pair.G)
+            phi = rng.uniform(0.1, 3.0, size=(pair.R, pair.G))
+            Qg = pair.gpu.nd_source_update(torch.from_numpy(phi).cuda(), 1.1)
+            p = pair.prob
+            Qo = oracle.source(p.mesh.material, p.xs.sigma_s, p.xs.nu_sigma_f, p.xs.chi, phi, 1.1)
+            assert np.abs(Qg.cpu().numpy() - Qo).max() <= 1e-13 * np.abs(Qo).max()
+    finally:
+        big.close()
+        small.close()
+
+
 POWER_CASES = [(1, 1.0, 50), (2, 0.15, 20), (2, 1.0, 20), (3, 0.03, 20), (4, 0.06, 20), (5, 0.0008, 20)]
 
 
