@@ -207,9 +207,6 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
         }
         ulonglong2 q_n = lds_2x64(q_lane + r_n.y);
         ulonglong2 st_n = lds_2x64(sigt_lane + r_n.z);
-#ifdef ND_MSKIP
-        uint32_t z_prev = r_n.z;
-#endif
         float s_n = __uint_as_float(r_n.x);
         // the 4 P updates of one step and the store of sum_p w_p Delta_p into the segment's delta row
         auto update = [&](const f32x2 (&qa)[2], const f32x2 (&ts)[2], uint32_t d_cur) {
@@ -235,7 +232,9 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
         // three -- measured 1.4 % slower and costs the small Deltas their relative accuracy: not kept.  Carrying the chains as
         // D_p = psi_p - q, D'_p = fma(D_p, a_p, q - q'), sum_p w_p Delta_p = WD - WD' + (q - q') sum_p w_p -- 49.5 instead of 54
         // instructions per step, every parity test green -- measured 5.4 % SLOWER at config 5: the loop is bound by the
-        // dependent chains behind each MUFU.EX2, not by its instruction count.)
+        // dependent chains behind each MUFU.EX2, not by its instruction count.  Skipping the Sigma_t load when the material
+        // is the one of the previous segment -- 94 % of the segments at config 4, 12 % at config 5 -- measured -0.4 % at
+        // config 4, -1.5 % at config 3 and +3.1 % at config 5: not kept.)
         for (int i = 0; i < steps; ++i) {
             const f32x2 s2 = pk2(s_n, s_n);
             const f32x2 qa[2] = {q_n.x, q_n.y};
@@ -245,11 +244,7 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
             r_nn = lds_u4(i + 2 < cnt ? rec_pf : null_rec);
             rec_pf += rstep;
             q_n = lds_2x64(q_lane + r_use.y);
-#ifdef ND_MSKIP
-            if (r_use.z != z_prev) { st_n = lds_2x64(sigt_lane + r_use.z); z_prev = r_use.z; }
-#else
             st_n = lds_2x64(sigt_lane + r_use.z);
-#endif
             s_n = __uint_as_float(r_use.x);
             d_n = r_use.w;
             update(qa, ts, d_cur);
