@@ -492,16 +492,17 @@ nd_status launch_source(nd_problem* p, const ndk::SourceParams& sp, cudaStream_t
     cp.chunk_regions = p->src_chunk_regions;
     const int block = 256;
     const int Gp = (d.G + 1) / 2 * 2;
-    const size_t smem = sizeof(double) * ((size_t)p->src_chunk_regions * Gp + ((p->src_chunk_regions + 1) & ~1));
+    const size_t smem = sizeof(double) * (2 * (size_t)p->src_chunk_regions * Gp + ((p->src_chunk_regions + 1) & ~1));
     const int grid = p->n_src_chunks < 8 * p->n_sm ? (p->n_src_chunks > 0 ? p->n_src_chunks : 1) : 8 * p->n_sm;
-    // the scattering matrix of the chunk's material beside the phi tile when both fit 100 KB (two blocks per SM: the kernel
-    // takes 128 registers)
+    // two phi tiles (<= 64 KB + the fission sums, by the cap on the chunk size) and, when it still fits 100 KB, the scattering
+    // matrix of the chunk's material beside them (two blocks per SM: the kernel takes 128 registers)
     const size_t smem_ss = smem + sizeof(double) * (size_t)d.G * Gp;
+    if (!p->source_attr_set) {   // the attribute belongs to the kernel, not to the problem: every problem sets the same value
+        ND_CUDA(cudaFuncSetAttribute(ndk::k_source_tiled<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSourceSmemMax));
+        ND_CUDA(cudaFuncSetAttribute(ndk::k_source_tiled<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSourceSmemMax));
+        p->source_attr_set = true;
+    }
     if (smem_ss <= kSourceSmemMax) {
-        if (!p->source_attr_set) {   // the attribute belongs to the kernel, not to the problem: every problem sets the same value
-            ND_CUDA(cudaFuncSetAttribute(ndk::k_source_tiled<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSourceSmemMax));
-            p->source_attr_set = true;
-        }
         ndk::k_source_tiled<true><<<grid, block, smem_ss, st>>>(cp);
     } else {
         ndk::k_source_tiled<false><<<grid, block, smem, st>>>(cp);
@@ -824,7 +825,7 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     std::vector<int32_t> h_src_region((size_t)d.R);
     std::vector<int4> h_src_chunks;
     {
-        // k_source_tiled: thread = (sub, pair of groups), kSrcTile regions each; at most 64 subs (phi tile <= 37 KB)
+        // k_source_tiled: thread = (sub, pair of groups), kSrcTile regions each; at most 64 subs (two phi tiles <= 64 KB)
         const int nsub = std::min(256 / ((d.G + 1) / 2), 64);
         p->src_chunk_regions = nsub * ndk::kSrcTile;
         std::vector<int64_t> count((size_t)d.M + 1, 0);

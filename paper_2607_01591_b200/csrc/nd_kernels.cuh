@@ -172,29 +172,59 @@ __global__ void __launch_bounds__(256) k_reduced_source(const double* __restrict
 // SS_SMEM: the chunk's scattering matrix is staged in shared memory ([G][Gp] doubles, reloaded only when the material
 // changes between two chunks of a block), so the inner loop waits on no global load; used when it fits beside the phi tile.
 constexpr int kSrcTile = 8;
-template <bool SS_SMEM>
-__global__ void __launch_bounds__(256) k_source_tiled(const SourceChunkParams cp)
+__device__ __forceinline__ void src_cp_async_8(double* smem_dst, const double* gmem_src)
 {
-    extern __shared__ __align__(16) double s_src2[];   // phi [chunk_regions][Gp], fis [chunk_regions], (Sigma_s^T [G][Gp])
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+// The phi tile is DOUBLE-BUFFERED: the rows of the block's next chunk are gathered by 8-byte cp.async (a phi row starts on an
+// 8-byte boundary only) while the current chunk is computed, so the gather's latency is off the path.  phi / F is applied to
+// the results (the source is linear in phi), not to the staged values.
+template <bool SS_SMEM>
+__global__ void __launch_bounds__(256, 2) k_source_tiled(const SourceChunkParams cp)
+{
+    extern __shared__ __align__(16) double s_src2[];   // phi [2][chunk_regions][Gp], fis [chunk_regions], (Sigma_s^T [G][Gp])
     const SourceParams& prm = cp.base;
     const int G = prm.G, CR = cp.chunk_regions, np = (G + 1) >> 1, Gp = 2 * np;
-    double* s_phi = s_src2;
-    double* s_fis = s_src2 + (size_t)CR * Gp;
+    double* s_fis = s_src2 + 2 * (size_t)CR * Gp;
     double* s_ss = s_fis + ((CR + 1) & ~1);            // 16-byte aligned
     int m_loaded = -1;
-    const int nsub = CR / kSrcTile;            // <= blockDim.x / np, capped by the host so that the phi tile fits 48 KB
+    const int nsub = CR / kSrcTile;            // <= blockDim.x / np, capped by the host so that the phi tiles fit
     const int sub = threadIdx.x / np, pr = threadIdx.x - sub * np;
     const int g0 = 2 * pr, g1 = g0 + 1 < G ? g0 + 1 : g0;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
     const double inv_f = prm.f_ptr ? 1.0 / *prm.f_ptr : 1.0;
     const double inv_k = 1.0 / (prm.k_ptr ? *prm.k_ptr : prm.k_val);
-    for (int c = blockIdx.x; c < cp.n_chunks; c += gridDim.x) {
+    const double scale = inv_f / kFourPi;
+    if (Gp > G)   // the pad column of both buffers: never written by the copies
+        for (int i = threadIdx.x; i < 2 * CR; i += blockDim.x) s_src2[(size_t)i * Gp + G] = 0.0;
+    auto gather = [&](int c, int buf) {   // rows of chunk c -> buffer buf: a warp per row and a lane per group (wide rows)
+        const int4 ch = cp.chunks[c];
+        double* dst = s_src2 + (size_t)buf * CR * Gp;
+        if (G >= 24) {
+            for (int lr = warp; lr < ch.y; lr += nwarp) {
+                const double* src = prm.phi + (size_t)cp.src_region[ch.x + lr] * G;
+                for (int g = lane; g < G; g += 32) src_cp_async_8(dst + (size_t)lr * Gp + g, src + g);
+            }
+        } else {   // narrow rows: a thread per element
+            for (int i = threadIdx.x; i < ch.y * G; i += blockDim.x) {
+                const int lr = i / G, g = i - lr * G;
+                src_cp_async_8(dst + (size_t)lr * Gp + g, prm.phi + (size_t)cp.src_region[ch.x + lr] * G + g);
+            }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    int buf = 0;
+    if ((int)blockIdx.x < cp.n_chunks) gather(blockIdx.x, 0);
+    for (int c = blockIdx.x; c < cp.n_chunks; c += gridDim.x, buf ^= 1) {
         const int4 ch = cp.chunks[c];
         const int first = ch.x, cnt = ch.y, m = ch.z;
-        __syncthreads();
-        for (int i = threadIdx.x; i < cnt * Gp; i += blockDim.x) {
-            const int lr = i / Gp, g = i - lr * Gp;
-            s_phi[i] = g < G ? prm.phi[(size_t)cp.src_region[first + lr] * G + g] * inv_f : 0.0;
+        const double* s_phi = s_src2 + (size_t)buf * CR * Gp;
+        const int c_next = c + gridDim.x;
+        if (c_next < cp.n_chunks) {   // the other buffer is free: every thread is past the previous chunk (barrier below)
+            gather(c_next, buf ^ 1);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
         }
         if (SS_SMEM && m != m_loaded) {   // rows gp of Sigma_s^T, padded to Gp (the pad column repeats the last group)
             const double* src = prm.sigsT + (size_t)m * G * G;
@@ -249,20 +279,16 @@ __global__ void __launch_bounds__(256) k_source_tiled(const SourceChunkParams cp
                 const int lr = sub + i * nsub;
                 if (lr < cnt) {
                     const int64_t r = cp.src_region[first + lr];
-                    const double Q0 = (acc0[i] + chi0 * s_fis[lr]) / kFourPi, Q1 = (acc1[i] + chi1 * s_fis[lr]) / kFourPi;
+                    const double Q0 = (acc0[i] + chi0 * s_fis[lr]) * scale, Q1 = (acc1[i] + chi1 * s_fis[lr]) * scale;
                     prm.Q[r * G + g0] = Q0;
                     if (two) prm.Q[r * G + g1] = Q1;
-                    if (prm.q) {
-                        prm.q[r * prm.Gs + g0] = (float)(Q0 / st0);
-                        if (two) prm.q[r * prm.Gs + g1] = (float)(Q1 / st1);
-                    }
-                    if (prm.tally) {
-                        prm.tally[r * prm.Gs + g0] = 0.0;
-                        if (two) prm.tally[r * prm.Gs + g1] = 0.0;
-                    }
+                    // q and tally rows are padded to Gs (a multiple of 4): the pair (g0, g0 + 1) is always inside the row
+                    if (prm.q) *reinterpret_cast<float2*>(prm.q + r * prm.Gs + g0) = make_float2((float)(Q0 / st0), two ? (float)(Q1 / st1) : 0.f);
+                    if (prm.tally) *reinterpret_cast<double2*>(prm.tally + r * prm.Gs + g0) = make_double2(0.0, 0.0);
                 }
             }
         }
+        __syncthreads();   // the buffer just computed from is the target of the next iteration's gather
     }
 }
 
