@@ -150,3 +150,39 @@ def test_cmfd_plan_entry_points_reject_null_arguments_without_a_gpu():
     assert L.nd_status_string(L.nd_cmfd_prolong(None, None)) == b"ND_ERR_NULL"
     assert L.nd_cmfd_destroy(None) == 0
     assert b"NULL" in L.nd_last_error(None)
+
+
+def test_round2_entry_points_check_their_arguments_without_a_gpu():
+    """nd_tracks_generate_resident / nd_tracks_materialise / nd_problem_stream_view / nd_fission_rate_static and the
+    seg_on_device field of the descriptor: the argument checks come before any CUDA call."""
+    L = nd.lib()
+    name = lambda rc: L.nd_status_string(rc)
+    assert name(L.nd_tracks_generate_resident(None, 8, 0.1, None, 0, None, None, None, None)) == b"ND_ERR_NULL"
+    assert name(L.nd_tracks_materialise(None, None)) == b"ND_ERR_NULL"
+    assert name(L.nd_problem_stream_view(None, None)) == b"ND_ERR_NULL"
+    one = C.c_void_p(4096)
+    assert name(L.nd_fission_rate_static(4, 2, None, one, one, one, one, None)) == b"ND_ERR_NULL"
+    assert name(L.nd_fission_rate_static(0, 2, one, one, one, one, one, None)) == b"ND_ERR_INVALID"
+    assert name(L.nd_fission_rate_static((1 << 27) + 1, 1, one, one, one, one, one, None)) == b"ND_ERR_RANGE"
+    assert b"ND_STATIC_FISSION_MAX_ELEMENTS" in L.nd_last_error(None)
+    # host tracks have no device arrays, and materialising them is a no-op
+    m = rect_tri_mesh(2.0, 1.5, 3, 3, seed=1)
+    m.material[:] = 0
+    tr = nd.nd_tracks_generate(m.xy, m.tri, m.W, m.H, (1, 1, 1, 1), 8, 0.2)
+    assert tr.seg_device is None and tr.on_host
+    assert L.nd_tracks_materialise(tr._h, None) == nd.ND_OK
+    # the descriptor's seg_on_device: 0 or 1, and 1 needs the track geometry
+    xs = homogeneous_xs(3, 5)
+    d, keep = _desc_for(m, xs, tr)
+    h, n = C.c_void_p(), C.c_size_t()
+    assert L.nd_workspace_bytes(C.byref(d), None, C.byref(n)) == nd.ND_OK
+    fake_ws = C.c_void_p(256 * 4096)
+    d.seg_on_device = 2
+    assert name(L.nd_problem_create(C.byref(d), None, fake_ws, n.value, None, C.byref(h))) == b"ND_ERR_INVALID"
+    d.seg_on_device = 1                                  # _desc_for passes no track_azim / track_ends
+    assert name(L.nd_problem_create(C.byref(d), None, fake_ws, n.value, None, C.byref(h))) == b"ND_ERR_INVALID"
+    assert b"geometry" in L.nd_last_error(None)
+    d.seg_on_device, d.reserved = 0, 7
+    assert name(L.nd_problem_create(C.byref(d), None, fake_ws, n.value, None, C.byref(h))) == b"ND_ERR_INVALID"
+    assert h.value is None
+    tr.destroy()
