@@ -100,7 +100,10 @@ typedef struct {
     int32_t item_order;     /* ND_SWEEP_SWATH: order in which thread blocks take the (swath, direction) work items.  0 = default:
                                most expensive first (best load balance; measured fastest at every config); 1 = angle by angle,
                                adjacent swaths consecutively (blocks that run together touch neighbouring regions) */
-    int32_t reserved[4];    /* must be 0 */
+    int32_t p1_stream;      /* 1: lay the swath kernel's shared memory out for the P_1 sweep of an nd_p1 plan as well (a second q
+                               row per region and a second delta row per segment: about twice the tile storage, so tiles come
+                               out shorter and the isotropic sweep of this problem somewhat slower); 0 = default */
+    int32_t reserved[3];    /* must be 0 */
 } nd_options;
 
 /* ------------------------------------------------------------------------------------------------
@@ -413,8 +416,10 @@ nd_status nd_cmfd_prolong(nd_cmfd* c, void* cuda_stream);
  *   Omega_xy = sin(theta_p) x the unit vector of the direction of travel;  Eq. (5) with Q(Omega) of the chain's own direction;
  *   phi = 4 pi Q0/Sigma_t + tally0/(Sigma_t A~);  J = [4 pi 3 c2 (M Q1) + tally_xy] / (Sigma_t A~), c2 = sum_p w_p sin^2(theta_p),
  *   Mab[r] = sum over the segments of r of 2 omega_a delta_a s u_a u_b.
- * This round: first correct kernels -- the simple one-warp-per-chain sweep over the plain segment stream with three FP64
- * tallies, so the problem must have been created with sweep_kernel = ND_SWEEP_ATOMIC (else ND_ERR_STATE).
+ * Two sweep kernels: on a problem created with sweep_kernel = ND_SWEEP_ATOMIC the one-warp-per-chain sweep over the plain
+ * segment stream with three FP64 tallies per segment; on a swath-kernel problem created with nd_options.p1_stream = 1 the
+ * swath kernel itself (a second staged source row 3 (u . q1) per region, a second delta row per segment, three tallies per
+ * (region, group) of a tile: 2.6 - 5.4 times faster).  Any other problem: ND_ERR_STATE.
  *   desc       the descriptor the problem was created from, WITH track_ends (direction of every track) -- HOST, borrowed
  *   sigma_s1   HOST [M][g][g'] first Legendre moment of the scattering matrix, from g' into g
  * All d_* arrays DEVICE [R][G] FP64.  nd_p1_power_iteration runs O-8 with the P_1 source on the problem's own state (flux,

@@ -44,7 +44,7 @@ class NdError(RuntimeError):
 class nd_options(C.Structure):
     _fields_ = [("exp_mode", C.c_int32), ("sweep_kernel", C.c_int32),
                 ("window_regions", C.c_int32), ("block_warps", C.c_int32), ("tile_segments", C.c_int32),
-                ("delta_buffers", C.c_int32), ("blocks_per_sm", C.c_int32), ("tile_lag", C.c_int32), ("q_copies", C.c_int32), ("graph_mode", C.c_int32), ("cmfd_stream", C.c_int32), ("item_order", C.c_int32), ("reserved", C.c_int32 * 4)]
+                ("delta_buffers", C.c_int32), ("blocks_per_sm", C.c_int32), ("tile_lag", C.c_int32), ("q_copies", C.c_int32), ("graph_mode", C.c_int32), ("cmfd_stream", C.c_int32), ("item_order", C.c_int32), ("p1_stream", C.c_int32), ("reserved", C.c_int32 * 3)]
 
 
 class nd_mesh_desc(C.Structure):
@@ -444,7 +444,7 @@ class Problem:
                  seg_region, seg_length, track_weight, link, track_azim=None, track_ends=None, region_volume=None,
                  exp_mode=ND_EXP_FAST,
                  sweep_kernel=ND_SWEEP_AUTO, window_regions=0, block_warps=0, tile_segments=0,
-                 delta_buffers=0, blocks_per_sm=0, tile_lag=0, q_copies=0, graph_mode=0, cmfd_stream=0, item_order=0, device="cuda:0",
+                 delta_buffers=0, blocks_per_sm=0, tile_lag=0, q_copies=0, graph_mode=0, cmfd_stream=0, item_order=0, p1_stream=0, device="cuda:0",
                  seg_device=None):
         """seg_device = (device pointer of seg_region, of seg_length): the segments are device-resident
         (nd_problem_desc.seg_on_device = 1); seg_region / seg_length are then ignored and may be None."""
@@ -476,7 +476,7 @@ class Problem:
         if seg_device is not None:
             d.seg_region, d.seg_length, d.seg_on_device = int(seg_device[0]), int(seg_device[1]), 1
         opt = nd_options(int(exp_mode), int(sweep_kernel), int(window_regions), int(block_warps),
-                         int(tile_segments), int(delta_buffers), int(blocks_per_sm), int(tile_lag), int(q_copies), int(graph_mode), int(cmfd_stream), int(item_order))
+                         int(tile_segments), int(delta_buffers), int(blocks_per_sm), int(tile_lag), int(q_copies), int(graph_mode), int(cmfd_stream), int(item_order), int(p1_stream))
         nbytes = C.c_size_t()
         _check(lib().nd_workspace_bytes(C.byref(d), C.byref(opt), C.byref(nbytes)), "nd_workspace_bytes")
         self.workspace_bytes = int(nbytes.value)

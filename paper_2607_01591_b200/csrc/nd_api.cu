@@ -90,6 +90,7 @@ struct SwathConfig {
     bool tight = false;                                   // register-capped kernel variant (more than 512 resident threads per SM)
     int head_cap = 0, rec_cap = 0, off_sigt = 0, off_q = 0, off_dbuf = 0, off_head = 0, off_rec = 0, smem_bytes = 0;
     int x_cap = 0, off_x = 0, off_w = 0;                  // nd_options.cmfd_stream: crossing-list ring and the slots' W rows
+    int off_q2 = 0, off_dbuf2 = 0;                        // nd_options.p1_stream: second q rows and second delta buffer
     int64_t max_tiles = 0, max_swaths = 0;
     size_t max_blob = 0;
 };
@@ -140,6 +141,11 @@ SwathConfig make_swath_config_q(const Dims& d, const nd_options& opt, int q_copi
             c.off_x = c.off_w + pad128(NT * row_bytes);
             c.smem_bytes = c.off_x + ndk::kSwathXBufs * c.x_cap;
         }
+        if (opt.p1_stream) {     // P_1 sweep in the sweep kernel: qB rows beside the q rows, a second delta buffer
+            c.off_q2 = pad128(c.smem_bytes);
+            c.off_dbuf2 = c.off_q2 + pad128(2 * Lmax * line_q);
+            c.smem_bytes = c.off_dbuf2 + pad128(c.ndbuf * (NT * Kmax + 1) * row_bytes);
+        }
         return true;
     };
     // Defaults (measured, profiles/): occupancy beats tile length once a tile holds >= 8 segments per track.  Aim at
@@ -180,6 +186,7 @@ SwathConfig make_swath_config_q(const Dims& d, const nd_options& opt, int q_copi
     if (bps < 1) bps = 1;
     if (opt.blocks_per_sm > 0 && opt.blocks_per_sm < bps) bps = opt.blocks_per_sm;
     c.blocks_per_sm = bps;
+    if (opt.p1_stream && bps * warps * 32 > 512) bps = std::max(1, 512 / (warps * 32));   // the P_1 loop needs the roomy register budget
     c.tight = bps * warps * 32 > 512 && warps <= 12;
     if (bps * warps * 32 > 512 && !c.tight) c.blocks_per_sm = bps = 512 / (warps * 32) > 0 ? 512 / (warps * 32) : 1;
     c.max_swaths = d.T;
@@ -345,6 +352,7 @@ struct nd_problem {
     std::vector<int64_t> h_swath_tile0;    // [n_swaths+1]
     std::vector<uint16_t> h_slot_start;    // [n_tiles][NT+1]
     nd_cmfd* cmfd_sweep = nullptr;         // set while a sweep has to tally the currents of this plan (C-3)
+    nd_p1* p1_sweep = nullptr;             // set while the swath kernel sweeps with this plan's P_1 source (nd_options.p1_stream)
     float c[ndk::kMaxPolar]{}, inv_sin[ndk::kMaxPolar]{}, wp[ndk::kMaxPolar]{};
     // profiling
     bool profile = false, phase_profile = false;
@@ -365,6 +373,7 @@ struct nd_problem {
 namespace {
 
 void cmfd_fill_sweep_params(const nd_cmfd* c, ndk::SwathParams* prm);   // nd_cmfd_api.cuh
+void p1_fill_sweep_params(const nd_p1* c, ndk::SwathParams* prm);       // nd_p1_api.cuh
 nd_status cmfd_end_currents(nd_cmfd* c, const double* scale_div, cudaStream_t st);
 
 inline cudaStream_t as_stream(void* s) { return reinterpret_cast<cudaStream_t>(s); }
@@ -422,6 +431,13 @@ nd_status launch_swath_p(nd_problem* p, const ndk::SwathParams& prm, cudaStream_
     const bool tight = c.tight && !expm1;   // the expm1f cross-check path keeps the roomy register budget
     const bool prof = p->phase_profile && !expm1;   // instrumented build: clock64 marks around the phases of a tile
     const bool cur = prm.xblob != nullptr;          // CMFD: the sweep also tallies the coarse-surface currents (fast-exp path only)
+    if (prm.q1x != nullptr) {                       // P_1 source (an nd_p1 plan on a problem with nd_options.p1_stream)
+        auto k1 = ndk::k_sweep_swath<P, 0, 0, 0, 0, 1>;
+        ND_CUDA(cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes));
+        k1<<<swath_grid(p), 32 * c.warps, c.smem_bytes, st>>>(prm);
+        ND_LAUNCH_CHECK(p);
+        return ND_OK;
+    }
     auto kern = expm1 ? ndk::k_sweep_swath<P, 1, 0, 0>
                 : cur ? (tight ? ndk::k_sweep_swath<P, 0, 1, 0, 1> : ndk::k_sweep_swath<P, 0, 0, 0, 1>)
                       : (tight ? (prof ? ndk::k_sweep_swath<P, 0, 1, 1> : ndk::k_sweep_swath<P, 0, 1, 0>)
@@ -456,6 +472,8 @@ nd_status launch_swath(nd_problem* p, const double* scale_div, cudaStream_t st)
     prm.phase = p->phase;
     prm.x_cap = c.x_cap; prm.off_x = c.off_x; prm.off_w = c.off_w;
     if (p->cmfd_sweep) cmfd_fill_sweep_params(p->cmfd_sweep, &prm);
+    prm.off_q2 = c.off_q2; prm.off_dbuf2 = c.off_dbuf2;
+    if (p->p1_sweep) p1_fill_sweep_params(p->p1_sweep, &prm);
     ND_CUDA(cudaMemsetAsync(p->counter, 0, sizeof(int), st));
     switch (d.P) {
     case 1: return launch_swath_p<1>(p, prm, st);
@@ -629,9 +647,11 @@ extern "C" nd_status nd_problem_create(const nd_problem_desc* desc, const nd_opt
     nd_options opt{};
     if (opts) opt = *opts;
     if (opt.item_order < 0 || opt.item_order > 1) return nd_fail(ND_ERR_INVALID, "nd_options.item_order must be 0 or 1");
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < 3; ++i)
         if (opt.reserved[i] != 0) return nd_fail(ND_ERR_INVALID, "nd_options.reserved must be zero");
     if (opt.cmfd_stream < 0 || opt.cmfd_stream > 1) return nd_fail(ND_ERR_INVALID, "nd_options.cmfd_stream must be 0 or 1");
+    if (opt.p1_stream < 0 || opt.p1_stream > 1) return nd_fail(ND_ERR_INVALID, "nd_options.p1_stream must be 0 or 1");
+    if (opt.p1_stream && opt.cmfd_stream) return nd_fail(ND_ERR_INVALID, "nd_options: p1_stream and cmfd_stream exclude each other");
     if (opt.exp_mode != ND_EXP_FAST && opt.exp_mode != ND_EXP_EXPM1) return nd_fail(ND_ERR_INVALID, "unknown exp_mode");
     if (opt.sweep_kernel != ND_SWEEP_AUTO && opt.sweep_kernel != ND_SWEEP_ATOMIC && opt.sweep_kernel != ND_SWEEP_SWATH)
         return nd_fail(ND_ERR_INVALID, "unknown sweep_kernel");

@@ -44,6 +44,12 @@ P1Layout p1_layout(const Dims& d)
     return L;
 }
 
+void p1_fill_sweep_params(const nd_p1* c, ndk::SwathParams* prm)
+{
+    prm->q1x = c->q1x; prm->q1y = c->q1y; prm->trk_dir = c->trk_dir; prm->tally_x = c->tally_x; prm->tally_y = c->tally_y;
+    for (int i = 0; i < ndk::kMaxPolar; ++i) prm->sin_t[i] = c->sin_t[i];
+}
+
 // sweep with the reduced sources already in p->q, c->q1x, c->q1y and zeroed tallies; then link swap, phi and J
 nd_status p1_sweep_and_finalise(nd_p1* c, const double* Q0, const double* scale_div, const double* phi_old, const double* f_ptr,
                                 double* phi_out, double* Jx_out, double* Jy_out, int* grid_out, cudaStream_t st)
@@ -57,14 +63,21 @@ nd_status p1_sweep_and_finalise(nd_p1* c, const double* Q0, const double* scale_
     prm.T = d.T; prm.G = d.G; prm.Gs = d.Gs;
     for (int i = 0; i < ndk::kMaxPolar; ++i) { prm.c[i] = p->c[i]; prm.inv_sin[i] = p->inv_sin[i]; prm.wp[i] = p->wp[i]; pp.sin_t[i] = c->sin_t[i]; }
     pp.q1x = c->q1x; pp.q1y = c->q1y; pp.trk_dir = c->trk_dir; pp.tally_x = c->tally_x; pp.tally_y = c->tally_y;
-    const int grid = grid_for(2 * (int64_t)d.T * 32, 256, 16 * p->n_sm);
-    switch (d.P) {
-    case 1: ndk::k_sweep_p1<1><<<grid, 256, 0, st>>>(pp); break;
-    case 2: ndk::k_sweep_p1<2><<<grid, 256, 0, st>>>(pp); break;
-    case 3: ndk::k_sweep_p1<3><<<grid, 256, 0, st>>>(pp); break;
-    default: ndk::k_sweep_p1<4><<<grid, 256, 0, st>>>(pp); break;
+    if (is_swath(p->sweep_kernel)) {   // the swath kernel with the P_1 source (problem created with nd_options.p1_stream)
+        p->p1_sweep = c;
+        const nd_status rs = launch_swath(p, scale_div, st);
+        p->p1_sweep = nullptr;
+        if (rs != ND_OK) return rs;
+    } else {
+        const int grid = grid_for(2 * (int64_t)d.T * 32, 256, 16 * p->n_sm);
+        switch (d.P) {
+        case 1: ndk::k_sweep_p1<1><<<grid, 256, 0, st>>>(pp); break;
+        case 2: ndk::k_sweep_p1<2><<<grid, 256, 0, st>>>(pp); break;
+        case 3: ndk::k_sweep_p1<3><<<grid, 256, 0, st>>>(pp); break;
+        default: ndk::k_sweep_p1<4><<<grid, 256, 0, st>>>(pp); break;
+        }
+        ND_LAUNCH_CHECK(p);
     }
-    ND_LAUNCH_CHECK(p);
     const int PG = d.P * d.Gs;
     const int64_t n = 2 * (int64_t)d.T * PG;
     ndk::k_link_swap<<<grid_for(n, 256, 8 * p->n_sm), 256, 0, st>>>(p->psi_out, p->psi_in, p->link_src, 2 * (int64_t)d.T, PG);
@@ -91,8 +104,9 @@ extern "C" nd_status nd_p1_create(nd_problem* p, const nd_problem_desc* desc, co
                                   size_t device_bytes, void* cuda_stream, nd_p1** out)
 {
     if (!p || !desc || !sigma_s1 || !device_workspace || !out) return nd_fail(ND_ERR_NULL, "nd_p1_create: NULL argument");
-    if (!p->has_soa) return nd_fail(ND_ERR_STATE, "nd_p1_create: needs a problem created with sweep_kernel = ND_SWEEP_ATOMIC (the P_1 "
-                                                  "sweep reads the plain segment stream)");
+    if (!p->has_soa && !(is_swath(p->sweep_kernel) && p->opt.p1_stream))
+        return nd_fail(ND_ERR_STATE, "nd_p1_create: needs a problem created with sweep_kernel = ND_SWEEP_ATOMIC (the plain segment "
+                                     "stream) or a swath-kernel problem created with nd_options.p1_stream = 1");
     if (p->opt.exp_mode != ND_EXP_FAST) return nd_fail(ND_ERR_STATE, "nd_p1_create: built for exp_mode = ND_EXP_FAST");
     const Dims& d = p->d;
     if (!desc->track_ends || !desc->track_seg_offset || !desc->seg_region || !desc->seg_length || !desc->track_weight || !desc->polar_sin ||

@@ -68,6 +68,16 @@ struct SwathParams {
     long long J_stride;
     int J_replicas;
     int x_cap, off_x, off_w;                   // bytes of one crossing buffer; shared-memory offsets of the ring and of W
+    // ---- P_1 scattering source (NEXT-4, template flag P1S): q(Omega) = q0 + sin(theta_p) qB with
+    // qB = 3 (u . q1) of the item's direction of travel u, staged as a second row per region; a second delta row per segment
+    // carries sum_p w_p sin(theta_p) Delta_p, flushed into the two moment tallies times u_x, u_y ----
+    const float* __restrict__ q1x;             // [R][Gs] Q1x / Sigma_t (NULL: isotropic source)
+    const float* __restrict__ q1y;             // [R][Gs]
+    const float* __restrict__ trk_dir;         // [T][2] unit vector from the start to the end point of a track
+    double* __restrict__ tally_x;              // [R][Gs]
+    double* __restrict__ tally_y;              // [R][Gs]
+    float sin_t[kMaxPolar];                    // sin(theta_p)
+    int off_q2, off_dbuf2;                     // shared-memory offsets of the qB rows [2][Lmax][line_q] and of the second delta buffer
 };
 
 // phases of the instrumented build (nd_profile_enable(p, 2)): where the warps' cycles go
@@ -288,13 +298,78 @@ __device__ __forceinline__ void segment_loop(float (&psi)[P][4], const float (&w
     }
 }
 
+// The same loop with the P_1 source (P1S): the chain of polar angle p sees q0 + sin(theta_p) qB, qB = 3 (u . q1) staged as a
+// second row per region at the same offsets, and a second delta row per segment takes sum_p w_p sin(theta_p) Delta_p (P-1..P-4
+// of DESIGN.md 8e).  The null record reads row 0 of both buffers with zero length: an exact no-op, as above.
+template <int P>
+__device__ __forceinline__ void segment_loop_p1(float (&psi)[P][4], const float (&wpt)[P], const SwathParams& prm, uint32_t rec0,
+                                                int rstep, int cnt, int steps, uint32_t null_rec, uint32_t q_lane, uint32_t q2_lane,
+                                                uint32_t sigt_lane, uint32_t d_lane, uint32_t d2_lane)
+{
+    const uint4 r_n = lds_u4(cnt > 0 ? rec0 : null_rec);
+    uint4 r_nn = lds_u4(cnt > 1 ? rec0 + rstep : null_rec);
+    uint32_t rec_pf = rec0 + 2 * rstep;
+    uint32_t d_n = r_n.w;
+    f32x2 ps[P][2], w2[P], w2s[P], sin2[P];
+#pragma unroll
+    for (int p = 0; p < P; ++p) {
+        ps[p][0] = pk2(psi[p][0], psi[p][1]);
+        ps[p][1] = pk2(psi[p][2], psi[p][3]);
+        w2[p] = pk2(wpt[p], wpt[p]);
+        w2s[p] = pk2(wpt[p] * prm.sin_t[p], wpt[p] * prm.sin_t[p]);
+        sin2[p] = pk2(prm.sin_t[p], prm.sin_t[p]);
+    }
+    ulonglong2 q_n = lds_2x64(q_lane + r_n.y);
+    ulonglong2 qb_n = lds_2x64(q2_lane + r_n.y);
+    ulonglong2 st_n = lds_2x64(sigt_lane + r_n.z);
+    float s_n = __uint_as_float(r_n.x);
+    for (int i = 0; i < steps; ++i) {
+        const f32x2 s2 = pk2(s_n, s_n);
+        const f32x2 qa[2] = {q_n.x, q_n.y}, qb[2] = {qb_n.x, qb_n.y};
+        const f32x2 ts[2] = {mul2(st_n.x, s2), mul2(st_n.y, s2)};
+        const uint32_t d_cur = d_n;
+        const uint4 r_use = r_nn;
+        r_nn = lds_u4(i + 2 < cnt ? rec_pf : null_rec);
+        rec_pf += rstep;
+        q_n = lds_2x64(q_lane + r_use.y);
+        qb_n = lds_2x64(q2_lane + r_use.y);
+        st_n = lds_2x64(sigt_lane + r_use.z);
+        s_n = __uint_as_float(r_use.x);
+        d_n = r_use.w;
+        f32x2 acc[2], acc1[2];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+#pragma unroll
+            for (int p = 0; p < P; ++p) {
+                const f32x2 tau = p == 0 ? ts[j] : mul2(ts[j], prm.c2[p]);
+                float t0, t1;
+                upk2(tau, t0, t1);
+                const f32x2 a = pk2(ex2_approx(t0), ex2_approx(t1));
+                const f32x2 d = sub2(ps[p][j], fma2(sin2[p], qb[j], qa[j]));
+                const f32x2 delta = sub2(d, mul2(d, a));
+                ps[p][j] = sub2(ps[p][j], delta);
+                acc[j] = p == 0 ? mul2(w2[0], delta) : fma2(w2[p], delta, acc[j]);
+                acc1[j] = p == 0 ? mul2(w2s[0], delta) : fma2(w2s[p], delta, acc1[j]);
+            }
+        }
+        sts_2x64(d_lane + d_cur, acc[0], acc[1]);
+        sts_2x64(d2_lane + d_cur, acc1[0], acc1[1]);
+    }
+#pragma unroll
+    for (int p = 0; p < P; ++p) {
+        upk2(ps[p][0], psi[p][0], psi[p][1]);
+        upk2(ps[p][1], psi[p][2], psi[p][3]);
+    }
+}
+
 // TIGHT = 1 caps the registers at 85 (768 resident threads per SM: three 256-thread or two 384-thread blocks).
 // CUR = 1 also tallies the net currents through the surfaces of a coarse mesh (CMFD, C-3 of DESIGN.md 8d) WITHOUT touching the
 // segment loop: with W = sum_p w_p psi_p, a delta row is W before its segment minus W behind it, so W at a crossing is W at
 // the tile's entry (stored per slot before the loop) minus the delta rows of the slot's segments passed so far.
-template <int P, int EXPM, int TIGHT, int PROF, int CUR = 0>
+template <int P, int EXPM, int TIGHT, int PROF, int CUR = 0, int P1S = 0>
 __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swath(const SwathParams prm)
 {
+    static_assert(!P1S || (EXPM == 0 && TIGHT == 0 && PROF == 0 && CUR == 0), "the P_1 variant exists for the plain fast-exp roomy kernel");
     long long ph[kSwathPhases] = {0, 0, 0, 0, 0, 0};
     long long t_mark = PROF ? clock64() : 0;
     int prof_sink = 0;
@@ -366,6 +441,12 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
         if (item >= prm.n_items) break;
         const int4 it = prm.items[item];
         const int sw = it.x, dir = it.y;
+        float ux = 0.f, uy = 0.f;   // P1S: direction of travel of the item (all tracks of a swath share their angle)
+        if (P1S) {
+            const int t0 = prm.swath_track[(size_t)sw * prm.NT];
+            const float sgn = dir == 0 ? 1.f : -1.f;
+            ux = sgn * prm.trk_dir[2 * (size_t)t0]; uy = sgn * prm.trk_dir[2 * (size_t)t0 + 1];
+        }
         const int64_t tile0 = prm.swath_tile0[sw];
         const int nt = (int)(prm.swath_tile0[sw + 1] - tile0);
         // ---- this slot's track: psi enters the registers ----
@@ -458,6 +539,12 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
                 const int l = (int)fastdiv((uint32_t)i, prm.magic_per_row), rem = i - l * per_row;
                 const int piece = rem - (int)fastdiv((uint32_t)rem, prm.magic_nq) * nq;
                 cp_async_16(qb + l * line_q + rem * 16, prm.q + (size_t)regions[l].x * Gs + piece * 4);
+                if (P1S) {   // qB = 3 (u . q1): plain loads a tile ahead, stored beside the q0 row (same offsets in the second buffer)
+                    const size_t at = (size_t)regions[l].x * Gs + piece * 4;
+                    const float4 a = *reinterpret_cast<const float4*>(prm.q1x + at), b = *reinterpret_cast<const float4*>(prm.q1y + at);
+                    sts_f4(smem_u32(smem + prm.off_q2) + (s & 1u) * q_buf_bytes + l * line_q + rem * 16, 3.f * fmaf(ux, a.x, uy * b.x),
+                           3.f * fmaf(ux, a.y, uy * b.y), 3.f * fmaf(ux, a.z, uy * b.z), 3.f * fmaf(ux, a.w, uy * b.w));
+                }
             }
         };
         if (nt > 0) {
@@ -528,8 +615,13 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
                 // segment j (forward index inside the tile) is visited at step i: j = dir ? cnt-1-i : i.  Shadow lanes carry
                 // their slot's chains too and store the same values to the same rows.
                 const int j_c = dir ? cnt - 1 : 0;          // segment of the first step
-                segment_loop<P, EXPM>(psi, wpt, prm, rec + 16 * (s0 + j_c), dir ? -16 : 16, cnt, steps, null_rec, q_lane, sigt_lane,
-                                      smem_u32(dbuf) + ll * 16);
+                if (P1S)
+                    segment_loop_p1<P>(psi, wpt, prm, rec + 16 * (s0 + j_c), dir ? -16 : 16, cnt, steps, null_rec, q_lane,
+                                       q_lane + (uint32_t)(prm.off_q2 - prm.off_q), sigt_lane, smem_u32(dbuf) + ll * 16,
+                                       smem_u32(dbuf) + (uint32_t)(prm.off_dbuf2 - prm.off_dbuf) + ll * 16);
+                else
+                    segment_loop<P, EXPM>(psi, wpt, prm, rec + 16 * (s0 + j_c), dir ? -16 : 16, cnt, steps, null_rec, q_lane, sigt_lane,
+                                          smem_u32(dbuf) + ll * 16);
             }
             mark(PH_COMPUTE);
             cp_async_wait_all();   // this thread's q-row copies for tile k+1
@@ -565,6 +657,22 @@ __global__ void __launch_bounds__(TIGHT ? 384 : 512, TIGHT ? 2 : 1) k_sweep_swat
                 double* tp = prm.tally + (uint32_t)(rg.x * (uint32_t)Gs + (uint32_t)(gp * 2));
                 atomicAdd(tp, (double)vx);
                 atomicAdd(tp + 1, (double)vy);
+                if (P1S) {   // the second delta rows: sum_p w_p sin(theta_p) Delta_p, times the direction of travel (P-4)
+                    uint32_t row2 = smem_u32(dbuf) + (uint32_t)(prm.off_dbuf2 - prm.off_dbuf) + e0 * row_bytes + gp * 8;
+                    f32x2 bxy = 0ull;
+                    for (int e = e0; e < e1; ++e, row2 += row_bytes) {
+                        f32x2 x;
+                        asm volatile("ld.shared.b64 %0, [%1];" : "=l"(x) : "r"(row2));
+                        bxy = add2(bxy, x);
+                    }
+                    float bx, by;
+                    upk2(bxy, bx, by);
+                    const uint32_t idx = rg.x * (uint32_t)Gs + (uint32_t)(gp * 2);
+                    atomicAdd(prm.tally_x + idx, (double)(ux * bx));
+                    atomicAdd(prm.tally_x + idx + 1, (double)(ux * by));
+                    atomicAdd(prm.tally_y + idx, (double)(uy * bx));
+                    atomicAdd(prm.tally_y + idx + 1, (double)(uy * by));
+                }
             };
             if (TIGHT) {
                 for (int u = tid; u < ch.L * f_np; u += nthr) flush_unit(u);
