@@ -90,10 +90,11 @@ ND_HD void nd_swath_core(const NdSwathCoreParams& P, const int64_t* off, const i
         auto take = [&](int b) -> bool {
             const int64_t k = s.cur[b];
             const int32_t r = seg_region[k];
-            int l = 0;
-            while (l < L && s.regions[l] != r) ++l;
-            if (l == L) {
+            int l = L - 1;   // newest first: a track stays in a region for a few segments and its neighbours follow it
+            while (l >= 0 && s.regions[l] != r) --l;
+            if (l < 0) {
                 if (L == Lmax) return false;
+                l = L;
                 s.regions[L] = r; s.rcount[L] = 0; ++L;
             }
             ++s.rcount[l];
