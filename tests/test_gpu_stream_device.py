@@ -86,6 +86,8 @@ STREAM_CASES = [
     ((4, 0.06), dict(item_order=1)),
     ((5, 0.002), {}),
     ((5, 0.002), dict(q_copies=1, tile_lag=3)),
+    ((3, 0.05), dict(p1_stream=1)),                        # the larger shared-memory layout of the P_1 sweep: shorter tiles
+    ((5, 0.002), dict(p1_stream=1)),
 ]
 
 
