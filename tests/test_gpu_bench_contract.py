@@ -32,3 +32,20 @@ def test_bench_prints_one_contract_line():
     cb = j["cpu_baseline"]
     assert cb["kind"] == "oracle" and cb["cores"] >= 1 and cb["value"] > 0 and cb["unit"] == j["unit"]
     assert set(j["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+    mb = rf["microbench"]
+    assert 15.0 <= mb["mufu_ex2_per_clk_per_sm"] <= 16.5 and rf["build_id"]
+
+
+def test_microbench_measures_the_roofline_denominators():
+    """nd_microbench (include/nd.h "Diagnostics"; "measure both ... before quoting any roofline fraction"): the
+    exp pipe issues 16 MUFU.EX2 per clock per SM, so n_SM x 16 x clock bounds the sweep; the FP64 RED rates frame the flush."""
+    import paper_2607_01591_b200 as nd
+    r = nd.nd_microbench()
+    assert 15.0 <= r["mufu_ex2_per_clk_per_sm"] <= 16.5, r
+    assert r["n_sm"] >= 100 and 1000.0 <= r["sm_clock_mhz"] <= 2300.0
+    per_s = r["n_sm"] * r["mufu_ex2_per_clk_per_sm"] * r["sm_clock_mhz"] * 1e6
+    assert abs(r["mufu_ex2_per_s"] - per_s) <= 0.03 * per_s                       # CUDA events agree with clock64 x clock
+    assert r["red_f64_l2_per_s"] > 1e11 and r["red_f64_hbm_per_s"] > 5e10
+    assert r["red_f64_l2_per_s"] > r["red_f64_hbm_per_s"]                        # an L2-resident table takes the REDs faster
+    small = nd.nd_microbench(workspace_bytes=80 << 20)                           # no room for the HBM-resident table
+    assert small["red_f64_hbm_per_s"] == 0.0 and 15.0 <= small["mufu_ex2_per_clk_per_sm"] <= 16.5
